@@ -1,0 +1,130 @@
+/* tdlike.h - C ABI of the B200-native time-domain Gaussian log-likelihood library.
+ *
+ * The operation (arxiv 2603.06010; line numbers are /root/reference/PAPER.md):
+ *   C_s[i][j] = rho_s(|i-j|)                       symmetric Toeplitz noise covariance   (Eq. 5,  :107)
+ *   <x, y>_s  = x^T C_s^{-1} y                      time-domain inner product             (Eq. 6,  :113)
+ *   lnL       = const - 1/2 <d - h, d - h>          exact Gaussian likelihood             (Eq. 7,  :125; Eq. 10, :142)
+ *   segments / detectors are independent blocks whose log-likelihoods are summed        (items 1-3, :148-162)
+ *   <.,.> is evaluated exactly through the Gohberg-Semencul formula                      (Eq. 14, :241-246)
+ *       C^{-1} = (1/x_1)(L_x L_x^T - R_x^T R_x),  C x = e_1,
+ *   each triangular-Toeplitz product by circulant embedding + FFT, m >= 2n-1           (Eqs. 15-16, :246-252)
+ *   or, for short segments, as a dense Toeplitz-by-matrix contraction (the GEMV of :219-227, batched).
+ *
+ * All entry points return a td_status and never abort or throw.  Nothing here allocates or
+ * frees caller memory.  There is no CPU fallback: every call needs a CUDA device.
+ * A handle must not be used from two host threads at once (it owns workspace); calls issued
+ * on one stream are ordered.
+ */
+#ifndef TDLIKE_H_
+#define TDLIKE_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct td_handle td_handle; /* opaque; owns device-side generators, spectra, workspace */
+
+typedef enum {
+  TD_OK = 0,
+  TD_EINVAL = 1,       /* bad argument (null pointer, non-positive length, ldh < N_tot, ...) */
+  TD_ENOTSPD = 2,      /* an ACF is not symmetric-positive-definite (or not finite)           */
+  TD_ENOMEM = 3,       /* host or device allocation failed                                    */
+  TD_ECUDA = 4,        /* a CUDA runtime call / kernel launch failed                          */
+  TD_EUNSUPPORTED = 5  /* valid request this build cannot serve (e.g. forced path too large)  */
+} td_status;
+
+/* td_path: evaluation path selector for td_set_path / reported by td_get_info. */
+enum { TD_PATH_AUTO = 0, TD_PATH_FFT = 1, TD_PATH_DENSE = 2 };
+
+/* td_create - one-time setup (PAPER.md:215 "done once ... cached"; :241-246 Eq. 14 generator).
+ *   acf          HOST pointer, sum_s seg_lengths[s] doubles: per-segment autocorrelation
+ *                functions concatenated; segment s holds rho_s(0..N_s-1) (Eq. 11, :148-154:
+ *                a segment of N_s samples uses lags 0..N_s-1), rho_s(0) > 0.
+ *   seg_lengths  HOST pointer, n_seg entries, each >= 1.
+ *   n_seg        number of disjoint segments / detectors (>= 1).
+ *   device       CUDA device ordinal that will own the handle.
+ *   out          receives the handle on success; untouched on failure.
+ * Per segment it runs a Levinson-Durbin recursion on the device, giving the prediction-error
+ * filter a (a_0 = 1) and variance v with C a = v e_1 (so x = a/v, x_1 = 1/v in Eq. 14),
+ * b = (0, a_{N-1}, ..., a_1), the pre-transformed generator spectra for the FFT path and
+ * log det C_s as a by-product.  Synchronous (returns after the device work completed).
+ * Errors: TD_EINVAL, TD_ENOTSPD (recursion met E_k <= 0 or a non-finite value), TD_ENOMEM, TD_ECUDA.
+ */
+td_status td_create(const double* acf, const int64_t* seg_lengths, int n_seg, int device,
+                    td_handle** out);
+
+/* td_destroy - frees everything the handle owns.  NULL is accepted. */
+td_status td_destroy(td_handle* h);
+
+/* td_loglike_batch - the hot path (Eq. 10 summed over segments, :142, :162).
+ *   d    DEVICE pointer, N_tot doubles: kept samples only, segments concatenated in order
+ *        (gap samples are not passed; Eq. 12 read as independent blocks, reading A5).
+ *   H    DEVICE pointer, row-major [B][ldh] doubles, ldh >= N_tot; row b = template h_b with
+ *        the same segment packing as d.
+ *   ldh  leading dimension of H in elements.
+ *   B    number of templates; B == 0 is a no-op returning TD_OK.
+ *   out  DEVICE pointer, B doubles: out[b] = -1/2 sum_s (d_s - h_bs)^T C_s^{-1} (d_s - h_bs)
+ *        (the additive constant of Eq. 7 is NOT included; see td_get_info for log det).
+ *   stream  a cudaStream_t (as void*; NULL = legacy default stream).
+ * Asynchronous: kernels are enqueued on `stream`, no host synchronisation.  The residual
+ * d - h_b and the filtered vectors are never written to HBM on the fused path.
+ * NaN/Inf in row b of H (or in d) propagate to out[b].
+ */
+td_status td_loglike_batch(td_handle* h, const double* d, const double* H, int64_t ldh,
+                           int64_t B, double* out, void* stream);
+
+/* td_inner_batch - cross terms of Eq. 13 (:177-181): out_dh[b] = <d, h_b>, out_hh[b] = <h_b, h_b>,
+ * both summed over segments.  Either output may be NULL (not computed / not written).
+ * Same layouts, ownership and stream semantics as td_loglike_batch.
+ * Identity: -2 * loglike[b] = <d,d> - 2 <d,h_b> + <h_b,h_b>;  <d,d> is td_inner_batch with H = d, B = 1.
+ */
+td_status td_inner_batch(td_handle* h, const double* d, const double* H, int64_t ldh,
+                         int64_t B, double* out_dh, double* out_hh, void* stream);
+
+/* td_loglike_batch_host - td_loglike_batch for HOST buffers (the end-to-end call).
+ *   d, H, out are HOST pointers with the layouts above (H ideally page-locked, otherwise the
+ *   copies are not asynchronous).  The library copies d once, streams H to the device in row
+ *   chunks through two staging buffers on an internal copy stream so that the host-to-device
+ *   copy of chunk k+1 overlaps the kernels of chunk k, and copies out back.
+ * SYNCHRONOUS: returns after out[] is complete.  `stream` is the compute stream (NULL = default).
+ */
+td_status td_loglike_batch_host(td_handle* h, const double* d, const double* H, int64_t ldh,
+                                int64_t B, double* out, void* stream);
+
+/* td_set_path - force the evaluation path for subsequent calls (TD_PATH_AUTO restores the
+ * chooser).  TD_PATH_DENSE on a handle with a segment longer than the dense path supports
+ * returns TD_EUNSUPPORTED and leaves the setting unchanged. */
+td_status td_set_path(td_handle* h, int path);
+
+/* td_set_fft_variant - which implementation serves the FFT path: 0 = automatic (fused
+ * shared-memory kernel where a segment's transform fits one SM, staged global-memory kernels
+ * otherwise), 1 = same as 0, 2 = force the staged kernels for every segment (tests, profiling). */
+td_status td_set_fft_variant(td_handle* h, int variant);
+
+/* td_get_info - queries.  Any output pointer may be NULL.
+ *   n_tot      sum of segment lengths
+ *   n_seg      number of segments
+ *   v          HOST array [n_seg]: prediction-error variance v_s = 1/(C_s^{-1})_{00}
+ *   logdet     HOST array [n_seg]: log det C_s = sum_k log E_k
+ *   last_path  TD_PATH_FFT or TD_PATH_DENSE actually used by the last batch call (0 if none yet)
+ */
+td_status td_get_info(const td_handle* h, int64_t* n_tot, int* n_seg, double* v, double* logdet,
+                      int* last_path);
+
+/* td_get_generator - copies segment s's prediction-error filter a (N_s doubles, a[0] = 1) to the
+ * HOST buffer `a`.  For tests of the setup kernel (C a = v e_1). */
+td_status td_get_generator(const td_handle* h, int seg, double* a);
+
+/* td_last_launches - number of kernels of this library launched by the last batch call on
+ * this handle (evidence for bench.py's gpu_launches). */
+int td_last_launches(const td_handle* h);
+
+/* td_strerror - static string for a status code. */
+const char* td_strerror(td_status s);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TDLIKE_H_ */

@@ -1,0 +1,196 @@
+// td_common.cuh - complex helpers, in-register radix-R FFT butterflies, twiddle chains and
+// mixed-radix index maps shared by the fused (shared-memory) and staged (global-memory) FFT
+// kernels of the Gohberg-Semencul / circulant-embedding path (Eqs. 14-16).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace td {
+
+typedef double2 cplx;
+
+__host__ __device__ __forceinline__ cplx mk(double x, double y) { return make_double2(x, y); }
+__device__ __forceinline__ cplx cadd(cplx a, cplx b) { return mk(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ cplx csub(cplx a, cplx b) { return mk(a.x - b.x, a.y - b.y); }
+__device__ __forceinline__ cplx cconj(cplx a) { return mk(a.x, -a.y); }
+// a * b
+__device__ __forceinline__ cplx cmul(cplx a, cplx b) {
+  return mk(fma(a.x, b.x, -(a.y * b.y)), fma(a.x, b.y, a.y * b.x));
+}
+// a * conj(b)
+__device__ __forceinline__ cplx cmulc(cplx a, cplx b) {
+  return mk(fma(a.x, b.x, a.y * b.y), fma(a.y, b.x, -(a.x * b.y)));
+}
+__device__ __forceinline__ cplx csq(cplx a) { return mk(fma(a.x, a.x, -(a.y * a.y)), 2.0 * a.x * a.y); }
+
+// ---- compile-time loops ---------------------------------------------------------------
+template <int I> struct IC { static constexpr int value = I; };
+template <int B, int E, class F> __device__ __forceinline__ void static_for(F&& f) {
+  if constexpr (B < E) {
+    f(IC<B>{});
+    static_for<B + 1, E>(f);
+  }
+}
+__host__ __device__ constexpr int ilog2(int n) { return n <= 1 ? 0 : 1 + ilog2(n >> 1); }
+__host__ __device__ constexpr int brev_bits(int k, int bits) {
+  int r = 0;
+  for (int i = 0; i < bits; ++i) r |= ((k >> i) & 1) << (bits - 1 - i);
+  return r;
+}
+
+// ---- constants cos/sin(2 pi k / 32) ------------------------------------------------------
+__host__ __device__ constexpr double cos32q(int k) {  // k in [0, 8]
+  return k == 0 ? 1.0
+       : k == 1 ? 0.98078528040323044912618223613424
+       : k == 2 ? 0.92387953251128675612818318939679
+       : k == 3 ? 0.83146961230254523707878837761791
+       : k == 4 ? 0.70710678118654752440084436210485
+       : k == 5 ? 0.55557023301960222474283081394853
+       : k == 6 ? 0.38268343236508977172845998403040
+       : k == 7 ? 0.19509032201612826784828486847702
+                : 0.0;
+}
+__host__ __device__ constexpr double cos32(int k) {
+  k &= 31;
+  return k <= 8 ? cos32q(k) : k <= 16 ? -cos32q(16 - k) : k <= 24 ? -cos32q(k - 16) : cos32q(32 - k);
+}
+__host__ __device__ constexpr double sin32(int k) { return cos32(k - 8); }
+
+// a * w32^K (forward: w32 = exp(-2 pi i / 32)) or a * conj(w32)^K (INV)
+template <int K, bool INV> __device__ __forceinline__ cplx mul_w32(cplx a) {
+  constexpr int k = K & 31;
+  if constexpr (k == 0) return a;
+  else if constexpr (k == 16) return mk(-a.x, -a.y);
+  else if constexpr (k == 8) return INV ? mk(-a.y, a.x) : mk(a.y, -a.x);
+  else if constexpr (k == 24) return INV ? mk(a.y, -a.x) : mk(-a.y, a.x);
+  else {
+    constexpr double c = cos32(k), s = sin32(k);
+    if constexpr (!INV) return mk(fma(a.x, c, a.y * s), fma(a.y, c, -(a.x * s)));
+    else return mk(fma(a.x, c, -(a.y * s)), fma(a.y, c, a.x * s));
+  }
+}
+
+// In-register radix-R DFT (R = 2,4,8,16) by radix-2 DIF stages.  On return X_k (k natural)
+// is held in x[brev(k)].  Forward kernel exp(-2 pi i s k / R); INV uses the conjugate.
+template <int R, bool INV> __device__ __forceinline__ void fft_reg(cplx (&x)[R]) {
+  constexpr int LG = ilog2(R);
+  static_for<0, LG>([&](auto st) {
+    constexpr int half = R >> (decltype(st)::value + 1);
+    static_for<0, R / 2>([&](auto q) {
+      constexpr int blk = (decltype(q)::value / half) * 2 * half;
+      constexpr int j = decltype(q)::value % half;
+      cplx a = x[blk + j], b = x[blk + j + half];
+      x[blk + j] = cadd(a, b);
+      x[blk + j + half] = mul_w32<j * (16 / half), INV>(csub(a, b));
+    });
+  });
+}
+template <int R> __host__ __device__ constexpr int brevR(int k) { return brev_bits(k, ilog2(R)); }
+
+// w[t] = w1^t, t = 1..R-1 (w[0] unused), by a squaring/multiply tree of depth <= log2(R)+2.
+template <int R> __device__ __forceinline__ void tw_powers(cplx w1, cplx (&w)[R]) {
+  w[0] = mk(1.0, 0.0);
+  if constexpr (R > 1) w[1] = w1;
+  static_for<2, R>([&](auto t) {
+    constexpr int tt = decltype(t)::value;
+    if constexpr ((tt & 1) == 0) w[tt] = csq(w[tt / 2]);
+    else w[tt] = cmul(w[tt - 1], w1);
+  });
+}
+
+// ---- mixed-radix plan [R1, 16, 16, ...] ----------------------------------------------------
+// n = R1 * 16^(np-1), R1 in {2,4,8,16}.  A DIF forward transform with this plan leaves X_k at
+// position pos(k); the DIT inverse with the mirrored pass order consumes that same order.
+__host__ __device__ constexpr int plan_np(int n) { return (ilog2(n) + 3) / 4; }
+__host__ __device__ constexpr int plan_r1(int n) { return n >> (4 * (plan_np(n) - 1)); }
+
+__host__ __device__ __forceinline__ int plan_pos(int k, int n) {
+  const int r1 = plan_r1(n);
+  int stride = n / r1;
+  int p = (k % r1) * stride;
+  k /= r1;
+  while (stride > 1) {
+    stride >>= 4;
+    p += (k & 15) * stride;
+    k >>= 4;
+  }
+  return p;
+}
+// inverse map: frequency index held at position p
+__host__ __device__ __forceinline__ int plan_freq(int p, int n) {
+  const int r1 = plan_r1(n);
+  int stride = n / r1;
+  int k = p / stride;
+  p -= k * stride;
+  int mul = r1;
+  while (stride > 1) {
+    stride >>= 4;
+    const int dgt = p / stride;
+    p -= dgt * stride;
+    k += dgt * mul;
+    mul <<= 4;
+  }
+  return k;
+}
+
+// ---- array accessors --------------------------------------------------------------------
+// shared memory, padded one element per 16 so that stride-16 (last-pass) and contiguous
+// (other passes) accesses are both bank-conflict free for 16-byte elements.
+struct SmemArr {
+  cplx* p;
+  __device__ __forceinline__ cplx ld(int i) const { return p[i + (i >> 4)]; }
+  __device__ __forceinline__ void st(int i, cplx v) const { p[i + (i >> 4)] = v; }
+  __host__ __device__ static constexpr int padded(int n) { return n + (n >> 4); }
+};
+struct GmemArr {
+  cplx* p;
+  __device__ __forceinline__ cplx ld(int i) const { return p[i]; }
+  __device__ __forceinline__ void st(int i, cplx v) const { p[i] = v; }
+};
+
+// ---- one butterfly task of a pass ---------------------------------------------------------
+// DIF (forward): sub-transform length L, radix R, stride S = L/R, butterfly g:
+//   x_s = A[base + s S];  X = DFT_R(x);  A[base + t S] = X_t * w[t]   (w[t] = w_L^{j t}; skipped if !tw)
+template <int R, class Arr>
+__device__ __forceinline__ void dif_task(const Arr& A, int L, int g, const cplx (&w)[R], bool tw) {
+  const int S = L / R;
+  const int blk = g / S, j = g - blk * S;
+  const int base = blk * L + j;
+  cplx x[R];
+#pragma unroll
+  for (int s = 0; s < R; ++s) x[s] = A.ld(base + s * S);
+  fft_reg<R, false>(x);
+  static_for<0, R>([&](auto t) {
+    constexpr int tt = decltype(t)::value;
+    cplx v = x[brevR<R>(tt)];
+    if (tt > 0 && tw) v = cmul(v, w[tt]);
+    A.st(base + tt * S, v);
+  });
+}
+// DIT (inverse): x_s = A[base + s S] * conj(w[s]);  X = conj-DFT_R(x);  A[base + t S] = X_t
+template <int R, class Arr>
+__device__ __forceinline__ void dit_task(const Arr& A, int L, int g, const cplx (&w)[R], bool tw) {
+  const int S = L / R;
+  const int blk = g / S, j = g - blk * S;
+  const int base = blk * L + j;
+  cplx x[R];
+  static_for<0, R>([&](auto s) {
+    constexpr int ss = decltype(s)::value;
+    cplx v = A.ld(base + ss * S);
+    if (ss > 0 && tw) v = cmulc(v, w[ss]);
+    x[ss] = v;
+  });
+  fft_reg<R, true>(x);
+  static_for<0, R>([&](auto t) {
+    constexpr int tt = decltype(t)::value;
+    A.st(base + tt * S, x[brevR<R>(tt)]);
+  });
+}
+
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+
+}  // namespace td

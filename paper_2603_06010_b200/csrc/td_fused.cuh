@@ -1,0 +1,294 @@
+// td_fused.cuh - the fused FFT-path kernel: one CTA evaluates whole templates with every
+// intermediate (residual, spectra, filtered vectors) resident in shared memory / registers.
+//
+// Per template b and segment s (Eqs. 14-16):
+//   S1  r = d_s - h_bs                                  fused into the first pass's global loads
+//   S2  R^ = FFT_2M(r zero-padded), 2M >= 2 N_s          real input: packed as u_j = r_2j + i r_2j+1 and
+//                                                        transformed as two half-zero-pruned length-M/2
+//                                                        complex DIF FFTs (even / odd output bins), then untangled
+//   S3  Z = G .* R^,  G = conj(A^) + i conj(B^)          both generator spectra in one complex array; G is stored
+//                                                        pre-permuted to the DIT input order and pre-scaled by
+//                                                        1/(2M sqrt(v))
+//   S4  z_i = IFFT_2M(Z)_i, i < N_s only                 two length-M complex DIT FFTs (even / odd input bins)
+//                                                        + pruned last radix-2 stage; Re z = L(a)^T r/sqrt(v),
+//                                                        Im z = L(b)^T r/sqrt(v)
+//   S5  Q_s = sum_i Re(z_i)^2 - Im(z_i)^2               fused into the last inverse pass; warp-shuffle + block
+//       out[b] = -1/2 sum_s Q_s                          reduction; one 8-byte store per template
+#pragma once
+#include "td_common.cuh"
+
+namespace td {
+
+struct SegDev {
+  long long off;    // offset of this segment inside d / a row of H (elements)
+  int n;            // N_s
+  int _pad;
+  const cplx* G;    // [2][M]: even-bin then odd-bin generator spectrum, DIT input order, scaled
+  cplx* zd;         // [M]: z of the data vector d (td_inner_batch only)
+};
+
+enum { MODE_LOGLIKE = 0, MODE_INNER = 1, MODE_STOREZ = 2 };
+
+struct FusedParams {
+  const double* d;
+  const double* H;
+  long long ldh;
+  long long B;
+  double* out0;        // loglike: out; inner: out_dh (may be null)
+  double* out1;        // inner: out_hh (may be null)
+  const SegDev* segs;  // device array
+  int n_seg;
+  int accumulate;      // add to out instead of overwriting (segments of another size class ran before)
+  const cplx* T;       // T[k] = exp(-2 pi i k / (2M)), k < 2M
+};
+
+// x = (sample 2*idx, sample 2*idx+1) of the vector this MODE transforms, zero beyond n.
+template <int MODE>
+__device__ __forceinline__ cplx load_pair(const double* __restrict__ drow, const double* __restrict__ hrow,
+                                          int idx, int n, bool vec) {
+  const int i0 = 2 * idx;
+  double h0 = 0.0, h1 = 0.0, d0 = 0.0, d1 = 0.0;
+  if (i0 + 1 < n && vec) {
+    if (MODE != MODE_STOREZ) {
+      const double2 hv = __ldg(reinterpret_cast<const double2*>(hrow + i0));
+      h0 = hv.x; h1 = hv.y;
+    }
+    if (MODE != MODE_INNER) {
+      const double2 dv = *reinterpret_cast<const double2*>(drow + i0);
+      d0 = dv.x; d1 = dv.y;
+    }
+  } else {
+    if (i0 < n) {
+      if (MODE != MODE_STOREZ) h0 = __ldg(hrow + i0);
+      if (MODE != MODE_INNER) d0 = drow[i0];
+    }
+    if (i0 + 1 < n) {
+      if (MODE != MODE_STOREZ) h1 = __ldg(hrow + i0 + 1);
+      if (MODE != MODE_INNER) d1 = drow[i0 + 1];
+    }
+  }
+  if (MODE == MODE_LOGLIKE) return mk(d0 - h0, d1 - h1);
+  if (MODE == MODE_INNER) return mk(h0, h1);
+  return mk(d0, d1);
+}
+
+// First forward pass: reads the packed real input straight from global memory and produces
+// pass 1 of BOTH pruned half-length transforms (even bins: plain; odd bins: input pre-twisted
+// by w_M^j, split into a compile-time part w_{2R}^s on the inputs and w_M^j0 folded into the
+// output twiddles).
+template <int R, int MODE, class Arr>
+__device__ __forceinline__ void first_pass_task(const Arr& UE, const Arr& UO, int nf, int g,
+                                                const double* __restrict__ drow,
+                                                const double* __restrict__ hrow, int n, bool vec,
+                                                const cplx* __restrict__ T) {
+  const int S = nf / R;
+  const int j = g;  // single block of length nf
+  cplx x[R], y[R];
+#pragma unroll
+  for (int s = 0; s < R; ++s) x[s] = load_pair<MODE>(drow, hrow, j + s * S, n, vec);
+  static_for<0, R>([&](auto s) {
+    constexpr int ss = decltype(s)::value;
+    y[ss] = mul_w32<ss * (16 / R), false>(x[ss]);
+  });
+  cplx w[R];
+  tw_powers<R>(T[4 * j], w);   // w_nf^j = w_2M^{4j}
+  const cplx beta = T[2 * j];  // w_M^j
+  fft_reg<R, false>(x);
+  fft_reg<R, false>(y);
+  static_for<0, R>([&](auto t) {
+    constexpr int tt = decltype(t)::value;
+    cplx ve = x[brevR<R>(tt)], vo = y[brevR<R>(tt)];
+    if (tt > 0) {
+      ve = cmul(ve, w[tt]);
+      vo = cmul(vo, cmul(w[tt], beta));
+    } else {
+      vo = cmul(vo, beta);
+    }
+    UE.st(j + tt * S, ve);
+    UO.st(j + tt * S, vo);
+  });
+}
+
+// Untangle + generator product for the bin held at position p of branch br's forward result.
+// Only the canonical member of each conjugate pair does work.  Writes four spectrum bins.
+template <class ArrU, class ArrZ>
+__device__ __forceinline__ void untangle_task(const ArrU& U, const ArrZ& Z, const cplx* __restrict__ G,
+                                              int br, int p, int nf, int M, const cplx* __restrict__ T) {
+  const int kq = plan_freq(p, nf);
+  int kq2, i1, i2, i3;
+  if (br == 0) {
+    if (kq > nf / 2) return;
+    kq2 = (nf - kq) & (nf - 1);
+    i1 = nf - kq; i2 = nf + kq; i3 = (M - kq) & (M - 1);
+  } else {
+    if (kq >= nf / 2) return;
+    kq2 = nf - 1 - kq;
+    i1 = nf - 1 - kq; i2 = nf + kq; i3 = M - 1 - kq;
+  }
+  const cplx U1 = U.ld(p), U2 = U.ld(plan_pos(kq2, nf));
+  const cplx w = T[2 * kq + br];
+  const cplx A = mk(0.5 * (U1.x + U2.x), 0.5 * (U1.y - U2.y));
+  const cplx Bv = mk(0.5 * (U1.y + U2.y), -0.5 * (U1.x - U2.x));
+  const cplx wB = cmul(w, Bv);
+  const cplx Xk = cadd(A, wB), Xm = csub(A, wB);
+  const int p0 = plan_pos(kq, M), p1 = plan_pos(i1, M), p2 = plan_pos(i2, M), p3 = plan_pos(i3, M);
+  Z.st(p0, cmul(G[p0], Xk));
+  Z.st(p1, cmul(G[p1], cconj(Xm)));
+  Z.st(p2, cmul(G[p2], Xm));
+  Z.st(p3, cmul(G[p3], cconj(Xk)));
+}
+
+// Last inverse pass (radix R, L = M) for both branches, pruned final radix-2 stage
+// z_i = e_i + w_2M^{-i} o_i, restriction to i < n and the fused quadratic sums.
+template <int R, int MODE, class Arr>
+__device__ __forceinline__ void last_pass_task(const Arr& ZE, const Arr& ZO, int M, int g, int n,
+                                               const cplx* __restrict__ T, cplx* __restrict__ zd,
+                                               double& acc0, double& acc1) {
+  const int S = M / R;
+  const int j = g;
+  cplx w[R], e[R], o[R];
+  tw_powers<R>(T[2 * j], w);  // w_M^j
+  const cplx beta = T[j];     // w_2M^j
+  static_for<0, R>([&](auto s) {
+    constexpr int ss = decltype(s)::value;
+    cplx ve = ZE.ld(j + ss * S), vo = ZO.ld(j + ss * S);
+    if (ss > 0) {
+      ve = cmulc(ve, w[ss]);
+      vo = cmulc(vo, cmul(w[ss], beta));
+    } else {
+      vo = cmulc(vo, beta);
+    }
+    e[ss] = ve;
+    o[ss] = vo;
+  });
+  fft_reg<R, true>(e);
+  fft_reg<R, true>(o);
+  static_for<0, R>([&](auto t) {
+    constexpr int tt = decltype(t)::value;
+    const cplx ot = mul_w32<tt * (16 / R), true>(o[brevR<R>(tt)]);
+    const cplx z = cadd(e[brevR<R>(tt)], ot);
+    const int i = j + tt * S;
+    if (MODE == MODE_STOREZ) {
+      zd[i] = z;
+    } else if (i < n) {
+      if (MODE == MODE_INNER) {
+        const cplx q = zd[i];
+        acc0 = fma(z.x, q.x, fma(-z.y, q.y, acc0));
+      }
+      acc1 = fma(z.x, z.x, fma(-z.y, z.y, acc1));
+    }
+  });
+}
+
+// one radix-16 shared-memory pass over both branches
+template <int NT, bool FWD>
+__device__ __forceinline__ void smem_pass16(const SmemArr& AE, const SmemArr& AO, int n, int L,
+                                            const cplx* __restrict__ T, int TW, int tid) {
+  constexpr int R = 16;
+  const int TB = n / R, S = L / R;
+  const bool tw = S > 1;
+  if (TB >= NT) {
+    for (int g = tid; g < TB; g += NT) {
+      cplx w[R];
+      if (tw) tw_powers<R>(T[(g % S) * (TW / L)], w);
+      if (FWD) { dif_task<R>(AE, L, g, w, tw); dif_task<R>(AO, L, g, w, tw); }
+      else     { dit_task<R>(AE, L, g, w, tw); dit_task<R>(AO, L, g, w, tw); }
+    }
+  } else {
+    for (int id = tid; id < 2 * TB; id += NT) {
+      const int br = id / TB, g = id - br * TB;
+      cplx w[R];
+      if (tw) tw_powers<R>(T[(g % S) * (TW / L)], w);
+      if (FWD) dif_task<R>(br ? AO : AE, L, g, w, tw);
+      else     dit_task<R>(br ? AO : AE, L, g, w, tw);
+    }
+  }
+}
+
+template <int LOG2M> struct FusedShape {
+  static constexpr int M = 1 << LOG2M, NF = M / 2;
+  static constexpr int RF1 = plan_r1(NF), NPF = plan_np(NF);
+  static constexpr int RI1 = plan_r1(M), NPI = plan_np(M);
+  static constexpr size_t smem_bytes(int nt) {
+    return sizeof(cplx) * (2 * (size_t)SmemArr::padded(NF) + 2 * (size_t)SmemArr::padded(M)) + sizeof(double) * 2 * (nt / 32);
+  }
+};
+
+template <int LOG2M, int NT, int MODE>
+__global__ void __launch_bounds__(NT, 1) td_fused_kernel(const FusedParams P) {
+  using Sh = FusedShape<LOG2M>;
+  constexpr int M = Sh::M, NF = Sh::NF, TW = 2 * M;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  cplx* sm = reinterpret_cast<cplx*>(smem_raw);
+  const SmemArr UE{sm}, UO{sm + SmemArr::padded(NF)};
+  const SmemArr ZE{sm + 2 * SmemArr::padded(NF)}, ZO{sm + 2 * SmemArr::padded(NF) + SmemArr::padded(M)};
+  double* red = reinterpret_cast<double*>(sm + 2 * SmemArr::padded(NF) + 2 * SmemArr::padded(M));
+  const int tid = threadIdx.x;
+  const cplx* __restrict__ T = P.T;
+
+  for (long long b = blockIdx.x; b < P.B; b += gridDim.x) {
+    double tot0 = 0.0, tot1 = 0.0;
+    for (int s = 0; s < P.n_seg; ++s) {
+      const SegDev sg = P.segs[s];
+      const double* drow = P.d + sg.off;
+      const double* hrow = (MODE == MODE_STOREZ) ? drow : P.H + b * P.ldh + sg.off;
+      const bool vec = ((reinterpret_cast<uintptr_t>(drow) | reinterpret_cast<uintptr_t>(hrow)) & 15) == 0;
+      // ---- S1+S2: forward, pass 1 from global
+      for (int g = tid; g < NF / Sh::RF1; g += NT)
+        first_pass_task<Sh::RF1, MODE>(UE, UO, NF, g, drow, hrow, sg.n, vec, T);
+      __syncthreads();
+      // ---- forward passes 2..NPF (radix 16)
+      {
+        int L = NF / Sh::RF1;
+#pragma unroll
+        for (int q = 1; q < Sh::NPF; ++q) {
+          smem_pass16<NT, true>(UE, UO, NF, L, T, TW, tid);
+          __syncthreads();
+          L >>= 4;
+        }
+      }
+      // ---- untangle + S3 generator product
+      for (int id = tid; id < 2 * NF; id += NT) {
+        const int br = id / NF, p = id - br * NF;
+        untangle_task(br ? UO : UE, br ? ZO : ZE, sg.G + br * M, br, p, NF, M, T);
+      }
+      __syncthreads();
+      // ---- S4: inverse passes (radix 16), smallest sub-transform first
+      {
+        int L = 16;
+#pragma unroll
+        for (int q = 1; q < Sh::NPI; ++q) {
+          smem_pass16<NT, false>(ZE, ZO, M, L, T, TW, tid);
+          __syncthreads();
+          L <<= 4;
+        }
+      }
+      // ---- last inverse pass + pruned radix-2 stage + S5
+      double acc0 = 0.0, acc1 = 0.0;
+      for (int g = tid; g < M / Sh::RI1; g += NT)
+        last_pass_task<Sh::RI1, MODE>(ZE, ZO, M, g, sg.n, T, sg.zd, acc0, acc1);
+      if (MODE != MODE_STOREZ) {
+        acc0 = warp_sum(acc0);
+        acc1 = warp_sum(acc1);
+        if ((tid & 31) == 0) { red[2 * (tid >> 5)] = acc0; red[2 * (tid >> 5) + 1] = acc1; }
+      }
+      __syncthreads();
+      if (MODE != MODE_STOREZ && tid == 0) {
+#pragma unroll
+        for (int wq = 0; wq < NT / 32; ++wq) { tot0 += red[2 * wq]; tot1 += red[2 * wq + 1]; }
+      }
+    }
+    if (tid == 0) {
+      if (MODE == MODE_LOGLIKE) {
+        const double v = -0.5 * tot1;
+        P.out0[b] = P.accumulate ? P.out0[b] + v : v;
+      } else if (MODE == MODE_INNER) {
+        if (P.out0) P.out0[b] = P.accumulate ? P.out0[b] + tot0 : tot0;
+        if (P.out1) P.out1[b] = P.accumulate ? P.out1[b] + tot1 : tot1;
+      }
+    }
+    if (MODE == MODE_STOREZ) break;  // one vector only
+  }
+}
+
+}  // namespace td

@@ -1,0 +1,106 @@
+// td_setup.cuh - one-time setup kernels of td_create:
+//   Levinson-Durbin recursion per segment  ->  prediction-error filter a, variance v, log det C
+//   (the paper cites the O(N^2) Toeplitz factorisation without printing it: PAPER.md:176 refs
+//   [104,105], :215; C a = v e_1 gives x = C^{-1} e_1 = a / v of Eq. 14),
+//   twiddle table, and the packed generator g = a - i b (b = (0, a_{N-1}, ..., a_1)) whose
+//   length-2M transform, conjugated, is G = conj(A^) + i conj(B^).
+#pragma once
+#include "td_common.cuh"
+
+namespace td {
+
+__global__ void tw_table_kernel(cplx* T, int TW) {
+  const int k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= TW) return;
+  double s, c;
+  sincospi(2.0 * (double)k / (double)TW, &s, &c);  // exact argument for power-of-two TW
+  T[k] = mk(c, -s);
+}
+
+struct LevSeg {
+  const double* rho;  // device, n doubles
+  double* a;          // device, n doubles (output)
+  int n;
+  int _pad;
+};
+
+constexpr int LEV_NT = 1024;
+
+// status: 0 ok, 2 not SPD / non-finite
+__global__ void __launch_bounds__(LEV_NT) levinson_kernel(const LevSeg* __restrict__ segs, double* v_out,
+                                                          double* logdet_out, int* status) {
+  __shared__ double red[LEV_NT / 32];
+  __shared__ double bc;
+  const LevSeg sg = segs[blockIdx.x];
+  const double* __restrict__ rho = sg.rho;
+  double* a = sg.a;
+  const int n = sg.n, tid = threadIdx.x;
+  const double rho0 = rho[0];
+  if (!(rho0 > 0.0) || !isfinite(rho0)) {
+    if (tid == 0) status[blockIdx.x] = 2;
+    return;
+  }
+  for (int j = tid; j < n; j += LEV_NT) a[j] = (j == 0) ? 1.0 : 0.0;
+  double E = rho0, logdet = log(rho0);
+  __syncthreads();
+  for (int k = 1; k < n; ++k) {
+    double acc = 0.0;
+    for (int j = tid; j < k; j += LEV_NT) acc = fma(a[j], rho[k - j], acc);
+    acc = warp_sum(acc);
+    if ((tid & 31) == 0) red[tid >> 5] = acc;
+    __syncthreads();
+    if (tid < 32) {
+      double v = red[tid];
+      v = warp_sum(v);
+      if (tid == 0) bc = v;
+    }
+    __syncthreads();
+    const double kk = -bc / E;
+    if (!(fabs(kk) < 1.0)) {  // also catches NaN
+      if (tid == 0) status[blockIdx.x] = 2;
+      return;
+    }
+    for (int j = 1 + tid; 2 * j < k; j += LEV_NT) {
+      const double aj = a[j], ak = a[k - j];
+      a[j] = fma(kk, ak, aj);
+      a[k - j] = fma(kk, aj, ak);
+    }
+    if (tid == 0) {
+      if ((k & 1) == 0) { const double am = a[k / 2]; a[k / 2] = fma(kk, am, am); }
+      a[k] = kk;
+    }
+    E *= (1.0 - kk * kk);
+    logdet += log(E);
+    if (!(E > 0.0)) {
+      if (tid == 0) status[blockIdx.x] = 2;
+      return;
+    }
+    __syncthreads();
+  }
+  if (tid == 0) {
+    v_out[blockIdx.x] = E;
+    logdet_out[blockIdx.x] = logdet;
+    status[blockIdx.x] = 0;
+  }
+}
+
+// g[j] = a_j - i b_j for j < n (b_0 = 0, b_j = a_{n-j}), zero up to n2 = 2M
+__global__ void gen_pack_kernel(const double* __restrict__ a, int n, cplx* g, int n2) {
+  const int j = blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= n2) return;
+  cplx v = mk(0.0, 0.0);
+  if (j < n) v = mk(a[j], j == 0 ? 0.0 : -a[n - j]);
+  g[j] = v;
+}
+
+// F = DIF transform of g (length 2M, bins at plan_pos(q, 2M)).  G[br][plan_pos(k', M)] =
+// conj(F[2k'+br]) * scale : generator spectrum split into even/odd bins in DIT input order.
+__global__ void gen_permute_kernel(const cplx* __restrict__ F, cplx* G, int M, double scale) {
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= 2 * M) return;
+  const int br = idx / M, kq = idx - br * M;
+  const cplx f = F[plan_pos(2 * kq + br, 2 * M)];
+  G[(size_t)br * M + plan_pos(kq, M)] = mk(f.x * scale, -f.y * scale);
+}
+
+}  // namespace td

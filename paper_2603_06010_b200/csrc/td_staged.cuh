@@ -1,0 +1,104 @@
+// td_staged.cuh - the same FFT path as td_fused.cuh with the per-template spectra staged in a
+// global-memory workspace (kept L2-resident by chunking the batch) instead of shared memory.
+// It serves segments whose transforms do not fit one SM's shared memory (2M > 8192 here) and
+// the one-time generator transform of td_create.  Pass structure, twiddles, untangle and the
+// fused last pass are the functions of td_fused.cuh / td_common.cuh called on global arrays.
+#pragma once
+#include "td_fused.cuh"
+
+namespace td {
+
+constexpr int LG_NT = 128;
+
+// workspace of template slot c: U = [2][nf], Z = [2][M]
+struct StagedParams {
+  const double* d;
+  const double* H;   // already offset to the first template of this chunk
+  long long ldh;
+  int CB;            // templates in this chunk
+  SegDev seg;
+  int M;             // power of two, nf = M/2
+  cplx* U;           // [CB][2][nf]
+  cplx* Z;           // [CB][2][M]
+  const cplx* T;     // exp(-2 pi i k / (2M)), k < 2M
+  double* partial;   // [CB][nblk][2]
+  int nblk;
+};
+
+template <int R, int MODE>
+__global__ void __launch_bounds__(LG_NT) lg_first_kernel(const StagedParams P) {
+  const int nf = P.M / 2;
+  const int g = blockIdx.x * LG_NT + threadIdx.x;
+  const int c = blockIdx.y;
+  if (g >= nf / R) return;
+  const double* drow = P.d + P.seg.off;
+  const double* hrow = (MODE == MODE_STOREZ) ? drow : P.H + (long long)c * P.ldh + P.seg.off;
+  const bool vec = ((reinterpret_cast<uintptr_t>(drow) | reinterpret_cast<uintptr_t>(hrow)) & 15) == 0;
+  const GmemArr UE{P.U + ((size_t)c * 2 + 0) * nf}, UO{P.U + ((size_t)c * 2 + 1) * nf};
+  first_pass_task<R, MODE>(UE, UO, nf, g, drow, hrow, P.seg.n, vec, P.T);
+}
+
+// generic pass over `narr` independent arrays of length n laid out back to back
+template <int R, bool FWD>
+__global__ void __launch_bounds__(LG_NT) lg_pass_kernel(cplx* base, int n, int L, const cplx* __restrict__ T,
+                                                       int TW) {
+  const int g = blockIdx.x * LG_NT + threadIdx.x;
+  if (g >= n / R) return;
+  const GmemArr A{base + (size_t)blockIdx.y * n};
+  const int S = L / R;
+  const bool tw = S > 1;
+  cplx w[R];
+  if (tw) tw_powers<R>(T[(size_t)(g % S) * (TW / L)], w);
+  if (FWD) dif_task<R>(A, L, g, w, tw);
+  else dit_task<R>(A, L, g, w, tw);
+}
+
+__global__ void __launch_bounds__(LG_NT) lg_untangle_kernel(const StagedParams P) {
+  const int nf = P.M / 2;
+  const int p = blockIdx.x * LG_NT + threadIdx.x;
+  const int br = blockIdx.y, c = blockIdx.z;
+  if (p >= nf) return;
+  const GmemArr U{P.U + ((size_t)c * 2 + br) * nf};
+  const GmemArr Z{P.Z + ((size_t)c * 2 + br) * P.M};
+  untangle_task(U, Z, P.seg.G + (size_t)br * P.M, br, p, nf, P.M, P.T);
+}
+
+template <int R, int MODE>
+__global__ void __launch_bounds__(LG_NT) lg_last_kernel(const StagedParams P) {
+  __shared__ double red[2 * (LG_NT / 32)];
+  const int g = blockIdx.x * LG_NT + threadIdx.x;
+  const int c = blockIdx.y;
+  const GmemArr ZE{P.Z + ((size_t)c * 2 + 0) * P.M}, ZO{P.Z + ((size_t)c * 2 + 1) * P.M};
+  double acc0 = 0.0, acc1 = 0.0;
+  if (g < P.M / R) last_pass_task<R, MODE>(ZE, ZO, P.M, g, P.seg.n, P.T, P.seg.zd, acc0, acc1);
+  if (MODE == MODE_STOREZ) return;
+  acc0 = warp_sum(acc0);
+  acc1 = warp_sum(acc1);
+  const int tid = threadIdx.x;
+  if ((tid & 31) == 0) { red[2 * (tid >> 5)] = acc0; red[2 * (tid >> 5) + 1] = acc1; }
+  __syncthreads();
+  if (tid == 0) {
+    double t0 = 0.0, t1 = 0.0;
+#pragma unroll
+    for (int w = 0; w < LG_NT / 32; ++w) { t0 += red[2 * w]; t1 += red[2 * w + 1]; }
+    double* dst = P.partial + ((size_t)c * P.nblk + blockIdx.x) * 2;
+    dst[0] = (MODE == MODE_LOGLIKE) ? t1 : t0;  // loglike: slot 0 carries the quadratic sum
+    dst[1] = t1;
+  }
+}
+
+// out[b] (+)= scale * sum_blk partial[c][blk][which]   (fixed summation order: deterministic)
+__global__ void lg_finish_kernel(const double* __restrict__ partial, int nblk, int CB, double* out0, double* out1,
+                                 double scale0, double scale1, int accumulate) {
+  const int c = blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= CB) return;
+  double t0 = 0.0, t1 = 0.0;
+  for (int k = 0; k < nblk; ++k) {
+    t0 += partial[((size_t)c * nblk + k) * 2];
+    t1 += partial[((size_t)c * nblk + k) * 2 + 1];
+  }
+  if (out0) out0[c] = (accumulate ? out0[c] : 0.0) + scale0 * t0;
+  if (out1) out1[c] = (accumulate ? out1[c] : 0.0) + scale1 * t1;
+}
+
+}  // namespace td

@@ -1,0 +1,547 @@
+// tdlike.cu - host side of the C ABI declared in include/tdlike.h.
+// Owns the handle, runs the one-time setup (td_setup.cuh) and dispatches the batch calls to
+// the fused shared-memory kernel (td_fused.cuh), the staged kernels (td_staged.cuh) or the
+// dense tensor-pipe kernel (td_dense.cuh).  No CPU fallback exists on any path.
+#include "../../include/tdlike.h"
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <new>
+#include <vector>
+
+#include "td_dense.cuh"
+#include "td_fused.cuh"
+#include "td_setup.cuh"
+#include "td_staged.cuh"
+
+using namespace td;
+
+namespace {
+
+constexpr int FUSED_MIN_LOG2M = 8;   // M = 256
+constexpr int FUSED_MAX_LOG2M = 12;  // M = 4096 (2M = 8192-point transform, 204 KiB of shared memory)
+constexpr int FUSED_NT = 256;
+constexpr size_t STAGED_WS_BYTES = 64ull << 20;  // keep the staged workspace L2-resident (126 MB L2)
+
+struct SegHost {
+  int64_t off = 0;
+  int n = 0;
+  int log2M = 0;
+  double v = 0.0, logdet = 0.0;
+  double* a = nullptr;  // device [n]
+  cplx* G = nullptr;    // device [2][M]
+  cplx* zd = nullptr;   // device [M] (lazy)
+};
+
+struct ClassInfo {
+  int log2M = 0;
+  cplx* T = nullptr;            // device [2M]
+  std::vector<int> seg_ids;
+  SegDev* d_segs = nullptr;     // device [seg_ids.size()]
+};
+
+struct DevGuard {
+  int prev = -1;
+  bool ok = true;
+  explicit DevGuard(int dev) {
+    if (cudaGetDevice(&prev) != cudaSuccess) { ok = false; return; }
+    if (prev != dev && cudaSetDevice(dev) != cudaSuccess) ok = false;
+  }
+  ~DevGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
+}  // namespace
+
+struct td_handle {
+  int device = 0, n_seg = 0, num_sms = 0;
+  int64_t n_tot = 0;
+  std::vector<SegHost> segs;
+  std::vector<ClassInfo> classes;
+  int path = TD_PATH_AUTO, fft_variant = 0, last_path = 0, last_launches = 0;
+  int max_n = 0;
+  // staged workspace (grow-only)
+  cplx* wsU = nullptr; cplx* wsZ = nullptr; double* wsPartial = nullptr;
+  size_t wsU_elems = 0, wsZ_elems = 0, wsP_elems = 0;
+  // dense path state
+  DenseState dense;
+  // host-buffer entry point: staging (grow-only), copy stream, events
+  double* hsD = nullptr; double* hsH[2] = {nullptr, nullptr}; double* hsOut = nullptr;
+  size_t hsH_elems = 0, hsOut_elems = 0;
+  cudaStream_t copy_stream = nullptr;
+  cudaEvent_t ev_copied[2] = {nullptr, nullptr}, ev_done[2] = {nullptr, nullptr};
+};
+
+#define CK(call)                                                                               \
+  do {                                                                                         \
+    cudaError_t e_ = (call);                                                                   \
+    if (e_ != cudaSuccess) {                                                                   \
+      if (getenv("TDLIKE_DEBUG")) fprintf(stderr, "tdlike: %s -> %s (%s:%d)\n", #call,         \
+                                          cudaGetErrorString(e_), __FILE__, __LINE__);         \
+      return e_ == cudaErrorMemoryAllocation ? TD_ENOMEM : TD_ECUDA;                           \
+    }                                                                                          \
+  } while (0)
+
+namespace {
+
+int next_log2(int n) { int l = 0; while ((1 << l) < n) ++l; return l; }
+
+void free_handle(td_handle* h) {
+  if (!h) return;
+  for (auto& s : h->segs) { cudaFree(s.a); cudaFree(s.G); cudaFree(s.zd); }
+  for (auto& c : h->classes) { cudaFree(c.T); cudaFree(c.d_segs); }
+  cudaFree(h->wsU); cudaFree(h->wsZ); cudaFree(h->wsPartial);
+  dense_free(h->dense);
+  cudaFree(h->hsD); cudaFree(h->hsH[0]); cudaFree(h->hsH[1]); cudaFree(h->hsOut);
+  if (h->copy_stream) cudaStreamDestroy(h->copy_stream);
+  for (int i = 0; i < 2; ++i) { if (h->ev_copied[i]) cudaEventDestroy(h->ev_copied[i]); if (h->ev_done[i]) cudaEventDestroy(h->ev_done[i]); }
+  delete h;
+}
+
+template <bool FWD>
+td_status launch_pass(int R, cplx* base, int narr, int n, int L, const cplx* T, int TW, cudaStream_t st) {
+  dim3 grid((n / R + LG_NT - 1) / LG_NT, narr);
+  switch (R) {
+    case 2: lg_pass_kernel<2, FWD><<<grid, LG_NT, 0, st>>>(base, n, L, T, TW); break;
+    case 4: lg_pass_kernel<4, FWD><<<grid, LG_NT, 0, st>>>(base, n, L, T, TW); break;
+    case 8: lg_pass_kernel<8, FWD><<<grid, LG_NT, 0, st>>>(base, n, L, T, TW); break;
+    case 16: lg_pass_kernel<16, FWD><<<grid, LG_NT, 0, st>>>(base, n, L, T, TW); break;
+    default: return TD_EINVAL;
+  }
+  CK(cudaGetLastError());
+  return TD_OK;
+}
+
+// forward DIF of `narr` arrays of length n with plan [r1,16,16,...]; returns launches made
+td_status staged_forward(cplx* base, int narr, int n, int first_pass_done, const cplx* T, int TW,
+                         cudaStream_t st, int* launches) {
+  int L = n;
+  const int r1 = plan_r1(n), np = plan_np(n);
+  for (int q = 0; q < np; ++q) {
+    const int R = q == 0 ? r1 : 16;
+    if (!(q == 0 && first_pass_done)) {
+      td_status s = launch_pass<true>(R, base, narr, n, L, T, TW, st);
+      if (s != TD_OK) return s;
+      ++*launches;
+    }
+    L /= R;
+  }
+  return TD_OK;
+}
+
+// inverse DIT passes except the last (radix r1, L = n) one
+td_status staged_inverse_but_last(cplx* base, int narr, int n, const cplx* T, int TW, cudaStream_t st,
+                                  int* launches) {
+  const int np = plan_np(n);
+  int L = 16;
+  for (int q = 1; q < np; ++q) {
+    td_status s = launch_pass<false>(16, base, narr, n, L, T, TW, st);
+    if (s != TD_OK) return s;
+    ++*launches;
+    L <<= 4;
+  }
+  return TD_OK;
+}
+
+template <int MODE>
+td_status launch_first(int R, dim3 grid, const StagedParams& P, cudaStream_t st) {
+  switch (R) {
+    case 2: lg_first_kernel<2, MODE><<<grid, LG_NT, 0, st>>>(P); break;
+    case 4: lg_first_kernel<4, MODE><<<grid, LG_NT, 0, st>>>(P); break;
+    case 8: lg_first_kernel<8, MODE><<<grid, LG_NT, 0, st>>>(P); break;
+    case 16: lg_first_kernel<16, MODE><<<grid, LG_NT, 0, st>>>(P); break;
+    default: return TD_EINVAL;
+  }
+  CK(cudaGetLastError());
+  return TD_OK;
+}
+template <int MODE>
+td_status launch_last(int R, dim3 grid, const StagedParams& P, cudaStream_t st) {
+  switch (R) {
+    case 2: lg_last_kernel<2, MODE><<<grid, LG_NT, 0, st>>>(P); break;
+    case 4: lg_last_kernel<4, MODE><<<grid, LG_NT, 0, st>>>(P); break;
+    case 8: lg_last_kernel<8, MODE><<<grid, LG_NT, 0, st>>>(P); break;
+    case 16: lg_last_kernel<16, MODE><<<grid, LG_NT, 0, st>>>(P); break;
+    default: return TD_EINVAL;
+  }
+  CK(cudaGetLastError());
+  return TD_OK;
+}
+
+td_status ensure_ws(td_handle* h, size_t u, size_t z, size_t p) {
+  if (u > h->wsU_elems) { cudaFree(h->wsU); h->wsU = nullptr; h->wsU_elems = 0; CK(cudaMalloc(&h->wsU, u * sizeof(cplx))); h->wsU_elems = u; }
+  if (z > h->wsZ_elems) { cudaFree(h->wsZ); h->wsZ = nullptr; h->wsZ_elems = 0; CK(cudaMalloc(&h->wsZ, z * sizeof(cplx))); h->wsZ_elems = z; }
+  if (p > h->wsP_elems) { cudaFree(h->wsPartial); h->wsPartial = nullptr; h->wsP_elems = 0; CK(cudaMalloc(&h->wsPartial, p * sizeof(double))); h->wsP_elems = p; }
+  return TD_OK;
+}
+
+// One segment of a size class through the staged pipeline for templates [0, B).
+template <int MODE>
+td_status run_staged(td_handle* h, const ClassInfo& cls, const SegHost& sg, const double* d, const double* H,
+                     int64_t ldh, int64_t B, double* out0, double* out1, double scale0, double scale1,
+                     int accumulate, cudaStream_t st) {
+  const int M = 1 << cls.log2M, nf = M / 2, TW = 2 * M;
+  const size_t per_tmpl = (size_t)(2 * nf + 2 * M) * sizeof(cplx);
+  int64_t CB = std::max<int64_t>(1, (int64_t)(STAGED_WS_BYTES / per_tmpl));
+  CB = std::min<int64_t>(CB, std::max<int64_t>(B, 1));
+  CB = std::min<int64_t>(CB, 32767);  // grid.y = 2*CB arrays per pass
+  const int rI = plan_r1(M), rF = plan_r1(nf);
+  const int nblk = (M / rI + LG_NT - 1) / LG_NT;
+  td_status s = ensure_ws(h, (size_t)CB * 2 * nf, (size_t)CB * 2 * M, (size_t)CB * nblk * 2);
+  if (s != TD_OK) return s;
+  for (int64_t b0 = 0; b0 < B; b0 += CB) {
+    const int cb = (int)std::min<int64_t>(CB, B - b0);
+    StagedParams P;
+    P.d = d; P.H = H ? H + b0 * ldh : nullptr; P.ldh = ldh; P.CB = cb;
+    P.seg.off = sg.off; P.seg.n = sg.n; P.seg._pad = 0; P.seg.G = sg.G; P.seg.zd = sg.zd;
+    P.M = M; P.U = h->wsU; P.Z = h->wsZ; P.T = cls.T; P.partial = h->wsPartial; P.nblk = nblk;
+    s = launch_first<MODE>(rF, dim3((nf / rF + LG_NT - 1) / LG_NT, cb), P, st);
+    if (s != TD_OK) return s;
+    ++h->last_launches;
+    s = staged_forward(h->wsU, 2 * cb, nf, 1, cls.T, TW, st, &h->last_launches);
+    if (s != TD_OK) return s;
+    lg_untangle_kernel<<<dim3((nf + LG_NT - 1) / LG_NT, 2, cb), LG_NT, 0, st>>>(P);
+    CK(cudaGetLastError());
+    ++h->last_launches;
+    s = staged_inverse_but_last(h->wsZ, 2 * cb, M, cls.T, TW, st, &h->last_launches);
+    if (s != TD_OK) return s;
+    s = launch_last<MODE>(rI, dim3(nblk, cb), P, st);
+    if (s != TD_OK) return s;
+    ++h->last_launches;
+    if (MODE != MODE_STOREZ) {
+      lg_finish_kernel<<<(cb + 127) / 128, 128, 0, st>>>(h->wsPartial, nblk, cb, out0 ? out0 + b0 : nullptr,
+                                                        out1 ? out1 + b0 : nullptr, scale0, scale1, accumulate);
+      CK(cudaGetLastError());
+      ++h->last_launches;
+    }
+  }
+  return TD_OK;
+}
+
+template <int LOG2M, int MODE>
+td_status launch_fused_t(td_handle* h, const FusedParams& P, cudaStream_t st) {
+  auto kern = td_fused_kernel<LOG2M, FUSED_NT, MODE>;
+  const size_t smem = FusedShape<LOG2M>::smem_bytes(FUSED_NT);
+  CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  int nb = 0;
+  CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kern, FUSED_NT, smem));
+  if (nb < 1) return TD_EUNSUPPORTED;
+  const long long maxg = (long long)nb * h->num_sms;
+  const int grid = (int)std::max<long long>(1, std::min<long long>(MODE == MODE_STOREZ ? 1 : P.B, maxg));
+  kern<<<grid, FUSED_NT, smem, st>>>(P);
+  CK(cudaGetLastError());
+  ++h->last_launches;
+  return TD_OK;
+}
+
+template <int MODE>
+td_status launch_fused(td_handle* h, int log2M, const FusedParams& P, cudaStream_t st) {
+  switch (log2M) {
+    case 8: return launch_fused_t<8, MODE>(h, P, st);
+    case 9: return launch_fused_t<9, MODE>(h, P, st);
+    case 10: return launch_fused_t<10, MODE>(h, P, st);
+    case 11: return launch_fused_t<11, MODE>(h, P, st);
+    case 12: return launch_fused_t<12, MODE>(h, P, st);
+    default: return TD_EUNSUPPORTED;
+  }
+}
+
+bool class_is_fused(const td_handle* h, const ClassInfo& c) {
+  if (h->fft_variant == 2) return false;
+  return c.log2M >= FUSED_MIN_LOG2M && c.log2M <= FUSED_MAX_LOG2M;
+}
+
+// FFT path over all size classes.  MODE_LOGLIKE: out0 = loglike.  MODE_INNER: out0 = <d,h>, out1 = <h,h>.
+template <int MODE>
+td_status run_fft_path(td_handle* h, const double* d, const double* H, int64_t ldh, int64_t B, double* out0,
+                       double* out1, cudaStream_t st) {
+  int accumulate = 0;
+  const double sc0 = (MODE == MODE_LOGLIKE) ? -0.5 : 1.0, sc1 = 1.0;
+  for (const ClassInfo& cls : h->classes) {
+    if (class_is_fused(h, cls)) {
+      FusedParams P;
+      P.d = d; P.H = H; P.ldh = ldh; P.B = B; P.out0 = out0; P.out1 = out1;
+      P.segs = cls.d_segs; P.n_seg = (int)cls.seg_ids.size(); P.accumulate = accumulate; P.T = cls.T;
+      td_status s = launch_fused<MODE>(h, cls.log2M, P, st);
+      if (s != TD_OK) return s;
+      accumulate = 1;
+    } else {
+      for (int id : cls.seg_ids) {
+        td_status s = run_staged<MODE>(h, cls, h->segs[id], d, H, ldh, B, out0, out1, sc0, sc1, accumulate, st);
+        if (s != TD_OK) return s;
+        accumulate = 1;
+      }
+    }
+  }
+  return TD_OK;
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------
+// C ABI
+// ------------------------------------------------------------------------------------------
+extern "C" {
+
+const char* td_strerror(td_status s) {
+  switch (s) {
+    case TD_OK: return "ok";
+    case TD_EINVAL: return "invalid argument";
+    case TD_ENOTSPD: return "autocorrelation is not symmetric positive definite (or not finite)";
+    case TD_ENOMEM: return "out of memory";
+    case TD_ECUDA: return "CUDA error";
+    case TD_EUNSUPPORTED: return "unsupported request";
+  }
+  return "unknown status";
+}
+
+static td_status create_impl(td_handle* h, const double* acf, const int64_t* seg_lengths, int n_seg) {
+  cudaDeviceProp prop;
+  CK(cudaGetDeviceProperties(&prop, h->device));
+  h->num_sms = prop.multiProcessorCount;
+  h->n_seg = n_seg;
+  h->segs.resize(n_seg);
+  int64_t off = 0;
+  for (int s = 0; s < n_seg; ++s) {
+    SegHost& sg = h->segs[s];
+    sg.off = off; sg.n = (int)seg_lengths[s];
+    sg.log2M = std::max(FUSED_MIN_LOG2M, next_log2(sg.n));
+    off += sg.n;
+    h->max_n = std::max(h->max_n, sg.n);
+  }
+  h->n_tot = off;
+  // ---- device copies of the ACFs, Levinson-Durbin per segment (one CTA each)
+  double* d_rho = nullptr; double* d_v = nullptr; double* d_ld = nullptr; int* d_status = nullptr; LevSeg* d_lev = nullptr;
+  struct Tmp { double*& a; double*& b; double*& c; int*& d; LevSeg*& e; ~Tmp() { cudaFree(a); cudaFree(b); cudaFree(c); cudaFree(d); cudaFree(e); } }
+      tmp{d_rho, d_v, d_ld, d_status, d_lev};
+  CK(cudaMalloc(&d_rho, sizeof(double) * h->n_tot));
+  CK(cudaMemcpy(d_rho, acf, sizeof(double) * h->n_tot, cudaMemcpyHostToDevice));
+  CK(cudaMalloc(&d_v, sizeof(double) * n_seg));
+  CK(cudaMalloc(&d_ld, sizeof(double) * n_seg));
+  CK(cudaMalloc(&d_status, sizeof(int) * n_seg));
+  CK(cudaMemset(d_status, 0xff, sizeof(int) * n_seg));
+  CK(cudaMalloc(&d_lev, sizeof(LevSeg) * n_seg));
+  std::vector<LevSeg> lev(n_seg);
+  for (int s = 0; s < n_seg; ++s) {
+    SegHost& sg = h->segs[s];
+    CK(cudaMalloc(&sg.a, sizeof(double) * sg.n));
+    lev[s].rho = d_rho + sg.off; lev[s].a = sg.a; lev[s].n = sg.n; lev[s]._pad = 0;
+  }
+  CK(cudaMemcpy(d_lev, lev.data(), sizeof(LevSeg) * n_seg, cudaMemcpyHostToDevice));
+  levinson_kernel<<<n_seg, LEV_NT>>>(d_lev, d_v, d_ld, d_status);
+  CK(cudaGetLastError());
+  CK(cudaDeviceSynchronize());
+  std::vector<int> status(n_seg);
+  std::vector<double> v(n_seg), ld(n_seg);
+  CK(cudaMemcpy(status.data(), d_status, sizeof(int) * n_seg, cudaMemcpyDeviceToHost));
+  CK(cudaMemcpy(v.data(), d_v, sizeof(double) * n_seg, cudaMemcpyDeviceToHost));
+  CK(cudaMemcpy(ld.data(), d_ld, sizeof(double) * n_seg, cudaMemcpyDeviceToHost));
+  for (int s = 0; s < n_seg; ++s) {
+    if (status[s] != 0 || !(v[s] > 0.0) || !std::isfinite(v[s])) return TD_ENOTSPD;
+    h->segs[s].v = v[s]; h->segs[s].logdet = ld[s];
+  }
+  // ---- size classes, twiddle tables
+  for (int s = 0; s < n_seg; ++s) {
+    const int l2 = h->segs[s].log2M;
+    auto it = std::find_if(h->classes.begin(), h->classes.end(), [&](const ClassInfo& c) { return c.log2M == l2; });
+    if (it == h->classes.end()) { h->classes.emplace_back(); h->classes.back().log2M = l2; it = h->classes.end() - 1; }
+    it->seg_ids.push_back(s);
+  }
+  for (ClassInfo& c : h->classes) {
+    const int TW = 2 << c.log2M;
+    CK(cudaMalloc(&c.T, sizeof(cplx) * TW));
+    tw_table_kernel<<<(TW + 255) / 256, 256>>>(c.T, TW);
+    CK(cudaGetLastError());
+  }
+  // ---- generator spectra: G = conj(FFT_2M(a - i b)) / (2M sqrt(v)), split even/odd, DIT order
+  for (ClassInfo& c : h->classes) {
+    const int M = 1 << c.log2M, n2 = 2 * M;
+    cplx* F = nullptr;
+    CK(cudaMalloc(&F, sizeof(cplx) * n2));
+    td_status st = TD_OK;
+    for (int id : c.seg_ids) {
+      SegHost& sg = h->segs[id];
+      if (cudaMalloc(&sg.G, sizeof(cplx) * n2) != cudaSuccess) { st = TD_ENOMEM; break; }
+      gen_pack_kernel<<<(n2 + 255) / 256, 256>>>(sg.a, sg.n, F, n2);
+      int launches = 0;
+      st = staged_forward(F, 1, n2, 0, c.T, n2, 0, &launches);
+      if (st != TD_OK) break;
+      gen_permute_kernel<<<(n2 + 255) / 256, 256>>>(F, sg.G, M, 1.0 / ((double)n2 * std::sqrt(sg.v)));
+      if (cudaGetLastError() != cudaSuccess) { st = TD_ECUDA; break; }
+    }
+    cudaError_t e = cudaDeviceSynchronize();
+    cudaFree(F);
+    if (st != TD_OK) return st;
+    if (e != cudaSuccess) return TD_ECUDA;
+    std::vector<SegDev> sd(c.seg_ids.size());
+    for (size_t i = 0; i < sd.size(); ++i) {
+      const SegHost& sg = h->segs[c.seg_ids[i]];
+      sd[i].off = sg.off; sd[i].n = sg.n; sd[i]._pad = 0; sd[i].G = sg.G; sd[i].zd = nullptr;
+    }
+    CK(cudaMalloc(&c.d_segs, sizeof(SegDev) * sd.size()));
+    CK(cudaMemcpy(c.d_segs, sd.data(), sizeof(SegDev) * sd.size(), cudaMemcpyHostToDevice));
+  }
+  return TD_OK;
+}
+
+td_status td_create(const double* acf, const int64_t* seg_lengths, int n_seg, int device, td_handle** out) {
+  if (!acf || !seg_lengths || !out || n_seg < 1) return TD_EINVAL;
+  int64_t tot = 0;
+  for (int s = 0; s < n_seg; ++s) {
+    if (seg_lengths[s] < 1 || seg_lengths[s] > (1 << 26)) return TD_EINVAL;
+    tot += seg_lengths[s];
+  }
+  for (int64_t i = 0; i < tot; ++i) if (!std::isfinite(acf[i])) return TD_ENOTSPD;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return TD_ECUDA;
+  if (device < 0 || device >= ndev) return TD_EINVAL;
+  DevGuard guard(device);
+  if (!guard.ok) return TD_ECUDA;
+  td_handle* h = new (std::nothrow) td_handle();
+  if (!h) return TD_ENOMEM;
+  h->device = device;
+  td_status s = create_impl(h, acf, seg_lengths, n_seg);
+  if (s != TD_OK) { free_handle(h); return s; }
+  *out = h;
+  return TD_OK;
+}
+
+td_status td_destroy(td_handle* h) {
+  if (!h) return TD_OK;
+  DevGuard guard(h->device);
+  free_handle(h);
+  return TD_OK;
+}
+
+td_status td_loglike_batch(td_handle* h, const double* d, const double* H, int64_t ldh, int64_t B, double* out,
+                           void* stream) {
+  if (!h || B < 0) return TD_EINVAL;
+  if (B == 0) return TD_OK;
+  if (!d || !H || !out || ldh < h->n_tot) return TD_EINVAL;
+  DevGuard guard(h->device);
+  if (!guard.ok) return TD_ECUDA;
+  h->last_launches = 0;
+  h->last_path = TD_PATH_FFT;
+  return run_fft_path<MODE_LOGLIKE>(h, d, H, ldh, B, out, nullptr, (cudaStream_t)stream);
+}
+
+td_status td_loglike_batch_host(td_handle* h, const double* d, const double* H, int64_t ldh, int64_t B, double* out,
+                                void* stream) {
+  if (!h || B < 0) return TD_EINVAL;
+  if (B == 0) return TD_OK;
+  if (!d || !H || !out || ldh < h->n_tot) return TD_EINVAL;
+  DevGuard guard(h->device);
+  if (!guard.ok) return TD_ECUDA;
+  cudaStream_t st = (cudaStream_t)stream;
+  const int64_t n = h->n_tot;
+  // rows per chunk: ~32 MiB of template data, at least one row
+  const int64_t CH = std::max<int64_t>(1, std::min<int64_t>(B, (32ll << 20) / (8 * n)));
+  if (!h->copy_stream) {
+    CK(cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking));
+    for (int i = 0; i < 2; ++i) {
+      CK(cudaEventCreateWithFlags(&h->ev_copied[i], cudaEventDisableTiming));
+      CK(cudaEventCreateWithFlags(&h->ev_done[i], cudaEventDisableTiming));
+    }
+    CK(cudaMalloc(&h->hsD, sizeof(double) * n));
+  }
+  if ((size_t)(CH * n) > h->hsH_elems) {
+    for (int i = 0; i < 2; ++i) { cudaFree(h->hsH[i]); h->hsH[i] = nullptr; }
+    h->hsH_elems = 0;
+    for (int i = 0; i < 2; ++i) CK(cudaMalloc(&h->hsH[i], sizeof(double) * CH * n));
+    h->hsH_elems = (size_t)(CH * n);
+  }
+  if ((size_t)B > h->hsOut_elems) {
+    cudaFree(h->hsOut); h->hsOut = nullptr; h->hsOut_elems = 0;
+    CK(cudaMalloc(&h->hsOut, sizeof(double) * B));
+    h->hsOut_elems = (size_t)B;
+  }
+  CK(cudaMemcpyAsync(h->hsD, d, sizeof(double) * n, cudaMemcpyHostToDevice, st));
+  int launches = 0, k = 0;
+  for (int64_t b0 = 0; b0 < B; b0 += CH, ++k) {
+    const int buf = k & 1;
+    const int64_t cb = std::min<int64_t>(CH, B - b0);
+    if (k >= 2) CK(cudaStreamWaitEvent(h->copy_stream, h->ev_done[buf], 0));  // staging buffer free again
+    CK(cudaMemcpy2DAsync(h->hsH[buf], sizeof(double) * n, H + b0 * ldh, sizeof(double) * ldh, sizeof(double) * n,
+                         (size_t)cb, cudaMemcpyHostToDevice, h->copy_stream));
+    CK(cudaEventRecord(h->ev_copied[buf], h->copy_stream));
+    CK(cudaStreamWaitEvent(st, h->ev_copied[buf], 0));
+    td_status s = td_loglike_batch(h, h->hsD, h->hsH[buf], n, cb, h->hsOut + b0, st);
+    if (s != TD_OK) return s;
+    launches += h->last_launches;
+    CK(cudaEventRecord(h->ev_done[buf], st));
+  }
+  h->last_launches = launches;
+  CK(cudaMemcpyAsync(out, h->hsOut, sizeof(double) * B, cudaMemcpyDeviceToHost, st));
+  CK(cudaStreamSynchronize(st));
+  return TD_OK;
+}
+
+td_status td_inner_batch(td_handle* h, const double* d, const double* H, int64_t ldh, int64_t B, double* out_dh,
+                         double* out_hh, void* stream) {
+  if (!h || B < 0) return TD_EINVAL;
+  if (B == 0 || (!out_dh && !out_hh)) return TD_OK;
+  if (!d || !H || ldh < h->n_tot) return TD_EINVAL;
+  DevGuard guard(h->device);
+  if (!guard.ok) return TD_ECUDA;
+  cudaStream_t st = (cudaStream_t)stream;
+  h->last_launches = 0;
+  h->last_path = TD_PATH_FFT;
+  // z of the data vector, once per call (per segment), then the bilinear sums against it
+  for (ClassInfo& c : h->classes) {
+    bool fresh = false;
+    for (int id : c.seg_ids) {
+      SegHost& sg = h->segs[id];
+      if (!sg.zd) { CK(cudaMalloc(&sg.zd, sizeof(cplx) << c.log2M)); fresh = true; }
+    }
+    if (fresh) {
+      std::vector<SegDev> sd(c.seg_ids.size());
+      for (size_t i = 0; i < sd.size(); ++i) {
+        const SegHost& sg = h->segs[c.seg_ids[i]];
+        sd[i].off = sg.off; sd[i].n = sg.n; sd[i]._pad = 0; sd[i].G = sg.G; sd[i].zd = sg.zd;
+      }
+      CK(cudaMemcpyAsync(c.d_segs, sd.data(), sizeof(SegDev) * sd.size(), cudaMemcpyHostToDevice, st));
+      CK(cudaStreamSynchronize(st));  // sd is a host temporary (first td_inner_batch call only)
+    }
+  }
+  td_status s = run_fft_path<MODE_STOREZ>(h, d, nullptr, h->n_tot, 1, nullptr, nullptr, st);
+  if (s != TD_OK) return s;
+  return run_fft_path<MODE_INNER>(h, d, H, ldh, B, out_dh, out_hh, st);
+}
+
+td_status td_set_path(td_handle* h, int path) {
+  if (!h || path < TD_PATH_AUTO || path > TD_PATH_DENSE) return TD_EINVAL;
+  if (path == TD_PATH_DENSE && h->max_n > h->dense.max_n) return TD_EUNSUPPORTED;
+  h->path = path;
+  return TD_OK;
+}
+
+td_status td_set_fft_variant(td_handle* h, int variant) {
+  if (!h || variant < 0 || variant > 2) return TD_EINVAL;
+  h->fft_variant = variant;
+  return TD_OK;
+}
+
+td_status td_get_info(const td_handle* h, int64_t* n_tot, int* n_seg, double* v, double* logdet, int* last_path) {
+  if (!h) return TD_EINVAL;
+  if (n_tot) *n_tot = h->n_tot;
+  if (n_seg) *n_seg = h->n_seg;
+  for (int s = 0; s < h->n_seg; ++s) {
+    if (v) v[s] = h->segs[s].v;
+    if (logdet) logdet[s] = h->segs[s].logdet;
+  }
+  if (last_path) *last_path = h->last_path;
+  return TD_OK;
+}
+
+td_status td_get_generator(const td_handle* h, int seg, double* a) {
+  if (!h || !a || seg < 0 || seg >= h->n_seg) return TD_EINVAL;
+  DevGuard guard(h->device);
+  if (!guard.ok) return TD_ECUDA;
+  CK(cudaMemcpy(a, h->segs[seg].a, sizeof(double) * h->segs[seg].n, cudaMemcpyDeviceToHost));
+  return TD_OK;
+}
+
+int td_last_launches(const td_handle* h) { return h ? h->last_launches : 0; }
+
+}  // extern "C"

@@ -1,0 +1,226 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element,
+on the same seeded inputs.  Tolerance (BASELINE.json north_star): 1e-9 relative on each logL_b,
+with the A12 floor |gpu - oracle| <= 1e-9 * max(|oracle|, 1)."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+from oracle import td_oracle as O
+from paper_2603_06010_b200 import binding as tdb
+from paper_2603_06010_b200 import workloads as W
+
+TOL = 1e-9
+
+
+def _dev(x):
+    return torch.as_tensor(np.ascontiguousarray(x), dtype=torch.float64).cuda()
+
+
+def _assert_close(gpu, ref, tol=TOL, what=""):
+    gpu = np.asarray(gpu)
+    ref = np.asarray(ref)
+    err = np.abs(gpu - ref) / np.maximum(np.abs(ref), 1.0)
+    assert np.all(np.isfinite(gpu)), what
+    assert err.max() <= tol, f"{what}: max rel err {err.max():.3e} at {err.argmax()}"
+    return err.max()
+
+
+def _gpu_loglike(w, variant=0, path=None):
+    with tdb.TDLikelihood(w.acf, w.seg_lengths) as h:
+        if variant:
+            h.set_fft_variant(variant)
+        if path is not None:
+            h.set_path(path)
+        out = h.loglike_batch(_dev(w.d), _dev(w.H))
+        torch.cuda.synchronize()
+        return out.cpu().numpy(), h.info(), h.last_launches()
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _require_cuda():
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    tdb.load(build_if_missing=False)   # the in-tree library must be present: no fallback
+
+
+# ------------------------------------------------------------------ configs of BASELINE.json
+def test_c1_fused_full():
+    w = W.make("c1")
+    ref = O.loglike_batch(w.acf, w.seg_lengths, w.d, w.H)
+    out, info, nl = _gpu_loglike(w)
+    _assert_close(out, ref, what="c1")
+    assert info["last_path"] == tdb.TD_PATH_FFT and nl == 1
+
+
+def test_c1_staged_variant():
+    w = W.make("c1")
+    ref = O.loglike_batch(w.acf, w.seg_lengths, w.d, w.H)
+    out, _, nl = _gpu_loglike(w, variant=2)
+    _assert_close(out, ref, what="c1 staged")
+    assert nl > 1
+
+
+def test_c2_headline_size_subset():
+    w = W.make("c2", B=96)
+    ref = O.loglike_batch(w.acf, w.seg_lengths, w.d, w.H)
+    out, _, _ = _gpu_loglike(w)
+    _assert_close(out, ref, what="c2")
+    out2, _, _ = _gpu_loglike(w, variant=2)
+    _assert_close(out2, ref, what="c2 staged")
+
+
+def test_c3_gapped_segments():
+    w = W.make("c3", B=24)
+    ref = O.loglike_batch(w.acf, w.seg_lengths, w.d, w.H)
+    out, _, _ = _gpu_loglike(w)
+    _assert_close(out, ref, what="c3")
+
+
+def test_c5_three_detectors():
+    w = W.make("c5", B=12)
+    ref = O.loglike_batch(w.acf, w.seg_lengths, w.d, w.H)
+    out, _, _ = _gpu_loglike(w)
+    _assert_close(out, ref, what="c5")
+
+
+def test_c4_long_segment_vs_library_levinson():
+    """N = 65536: dense C would be 32 GiB, so the oracle route is solve_toeplitz (pin P13)."""
+    w = W.make("c4", B=3)
+    ref = O.loglike_batch_solve_toeplitz(w.acf, w.seg_lengths, w.d, w.H)
+    out, _, _ = _gpu_loglike(w)
+    _assert_close(out, ref, what="c4")
+
+
+# ------------------------------------------------------------------ shapes: ragged, tiny, mixed classes
+@pytest.mark.parametrize("n", [1, 2, 3, 5, 31, 255, 256, 257, 777, 1000, 2049, 4095])
+def test_ragged_lengths(n):
+    rng = np.random.default_rng(n)
+    rho = W.acf_from_psd(4096.0, 2 * max(n, 64), n)
+    d = rng.standard_normal(n) * 1e-21
+    H = rng.standard_normal((7, n)) * 1e-21
+    ref = O.loglike_batch(rho, [n], d, H)
+    for variant in (0, 2):
+        with tdb.TDLikelihood(rho, [n]) as h:
+            h.set_fft_variant(variant)
+            out = h.loglike_batch(_dev(d), _dev(H)).cpu().numpy()
+        _assert_close(out, ref, what=f"n={n} variant={variant}")
+
+
+def test_mixed_size_classes_and_odd_offsets():
+    rng = np.random.default_rng(5)
+    lens = [301, 1000, 4097, 77]
+    rho = W.acf_from_psd(4096.0, 2 * 8192, max(lens))
+    scales = [1.0, 0.7, 1.9, 3.0]
+    acf = np.concatenate([s * rho[:n] for s, n in zip(scales, lens)])
+    nt = sum(lens)
+    d = rng.standard_normal(nt) * 1e-21
+    H = rng.standard_normal((9, nt)) * 1e-21
+    ref = O.loglike_batch(acf, lens, d, H)
+    with tdb.TDLikelihood(acf, lens) as h:
+        out = h.loglike_batch(_dev(d), _dev(H)).cpu().numpy()
+    _assert_close(out, ref, what="mixed classes")
+
+
+def test_strided_rows_and_exact_zero_and_nan_row():
+    w = W.make("c1", B=8)
+    n = w.n_tot
+    Hpad = torch.zeros(8, n + 37, dtype=torch.float64, device="cuda")
+    Hpad[:, :n] = _dev(w.H)
+    Hpad[3, :n] = _dev(w.d)                       # h = d  ->  logL = 0 exactly (P8 iv)
+    Hpad[5, 100] = float("nan")
+    ref = O.loglike_batch(w.acf, w.seg_lengths, w.d, w.H)
+    with tdb.TDLikelihood(w.acf, w.seg_lengths) as h:
+        out = h.loglike_batch(_dev(w.d), Hpad[:, :n]).cpu().numpy()
+    assert out[3] == 0.0
+    assert np.isnan(out[5])
+    keep = [0, 1, 2, 4, 6, 7]
+    _assert_close(out[keep], ref[keep], what="strided")
+
+
+# ------------------------------------------------------------------ setup kernel (S0)
+@pytest.mark.parametrize("n", [64, 1024, 5000])
+def test_generator_matches_oracle_levinson(n):
+    rho = W.acf_from_psd(4096.0, 2 * 8192, n)
+    a_ref, v_ref, ld_ref = O.levinson_durbin_fast(rho)
+    with tdb.TDLikelihood(rho, [n]) as h:
+        a = h.generator(0)
+        info = h.info()
+    assert np.max(np.abs(a - a_ref)) <= 1e-10 * np.max(np.abs(a_ref))
+    assert abs(info["v"][0] - v_ref) <= 1e-11 * v_ref
+    assert abs(info["logdet"][0] - ld_ref) <= 1e-10 * abs(ld_ref)
+    L = O.cholesky_lower(rho)
+    assert abs(info["logdet"][0] - 2 * np.sum(np.log(np.diag(L)))) <= 1e-9 * abs(ld_ref)
+
+
+# ------------------------------------------------------------------ td_inner_batch (Eq. 13 terms)
+@pytest.mark.parametrize("name,B,variant", [("c1", 16, 0), ("c1", 16, 2), ("c3", 6, 0)])
+def test_inner_batch(name, B, variant):
+    w = W.make(name, B=B)
+    dh_ref, hh_ref = O.inner_batch(w.acf, w.seg_lengths, w.d, w.H)
+    with tdb.TDLikelihood(w.acf, w.seg_lengths) as h:
+        h.set_fft_variant(variant)
+        d, H = _dev(w.d), _dev(w.H)
+        dh, hh = h.inner_batch(d, H)
+        ll = h.loglike_batch(d, H)
+        dd, _ = h.inner_batch(d, d[None, :])
+        only_hh = h.inner_batch(d, H, want_dh=False)[1]
+    dh, hh, ll, dd = dh.cpu().numpy(), hh.cpu().numpy(), ll.cpu().numpy(), dd.cpu().numpy()[0]
+    scale = dd + hh
+    assert np.max(np.abs(dh - dh_ref) / scale) <= TOL
+    assert np.max(np.abs(hh - hh_ref) / np.abs(hh_ref)) <= TOL
+    assert np.max(np.abs(-2 * ll - (dd - 2 * dh + hh)) / scale) <= TOL      # bilinear identity (P11)
+    assert np.array_equal(only_hh.cpu().numpy(), hh)
+
+
+# ------------------------------------------------------------------ host-buffer entry point
+def test_host_entry_matches_device_entry():
+    w = W.make("c1", B=50)
+    Hp = torch.as_tensor(w.H).pin_memory()
+    with tdb.TDLikelihood(w.acf, w.seg_lengths) as h:
+        a = h.loglike_batch(_dev(w.d), _dev(w.H)).cpu().numpy()
+        b = h.loglike_batch_host(w.d, Hp)
+        c = h.loglike_batch_host(w.d, w.H)        # pageable numpy
+    assert np.array_equal(a, b) and np.array_equal(a, c)
+
+
+# ------------------------------------------------------------------ errors and edges
+def test_error_paths():
+    rho = W.acf_from_psd(4096.0, 2048, 512)
+    bad = np.array([1.0, 0.99, 0.2, -0.9])
+    with pytest.raises(tdb.TDError) as e:
+        tdb.TDLikelihood(bad, [4])
+    assert e.value.status == tdb.TD_ENOTSPD
+    with pytest.raises(tdb.TDError) as e:
+        tdb.TDLikelihood(np.array([0.0, 0.0]), [2])
+    assert e.value.status == tdb.TD_ENOTSPD
+    nanrho = rho.copy()
+    nanrho[7] = np.nan
+    with pytest.raises(tdb.TDError) as e:
+        tdb.TDLikelihood(nanrho, [512])
+    assert e.value.status == tdb.TD_ENOTSPD
+    with pytest.raises(tdb.TDError) as e:
+        tdb.TDLikelihood(rho, [0, 512][:1] + [512])   # zero-length segment
+    with tdb.TDLikelihood(rho, [512]) as h:
+        d = torch.zeros(512, dtype=torch.float64, device="cuda")
+        H0 = torch.zeros(0, 512, dtype=torch.float64, device="cuda")
+        assert h.loglike_batch(d, H0).numel() == 0          # B = 0 is a no-op
+        lib = tdb.load()
+        st = lib.td_loglike_batch(h._h, d.data_ptr(), d.data_ptr(), 100, 1, d.data_ptr(), None)
+        assert st == tdb.TD_EINVAL                           # ldh < N_tot
+        st = lib.td_loglike_batch(h._h, None, d.data_ptr(), 512, 1, d.data_ptr(), None)
+        assert st == tdb.TD_EINVAL
+
+
+def test_async_on_caller_stream_and_repeatable():
+    w = W.make("c1", B=32)
+    s = torch.cuda.Stream()
+    with tdb.TDLikelihood(w.acf, w.seg_lengths) as h:
+        d, H = _dev(w.d), _dev(w.H)
+        torch.cuda.synchronize()
+        with torch.cuda.stream(s):
+            o1 = h.loglike_batch(d, H)
+            o2 = h.loglike_batch(d, H)
+        s.synchronize()
+    assert torch.equal(o1, o2)                               # deterministic reduction order
