@@ -1,0 +1,314 @@
+#!/usr/bin/env python
+"""bench.py - the headline metric of BASELINE.json: fp64 likelihood evaluations / second.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config c2] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path (residual, forward FFT, generator product, inverse
+FFT, fused quadratic reduction, summed over segments) over one batch of B synthetic templates
+of the named config; the default workload is config c2 (N = 4096, B = 4096), the one the
+metric is quoted on.  With --gpus N > 1 (launched by torchrun) every rank processes its own
+batch of B templates (weak scaling, no data-path collective: templates are independent).
+
+Prints ONE JSON line (rank 0).  Keys follow the driver's contract; see DESIGN.md "Measurement".
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import math
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "fp64 likelihood evals/sec"
+UNIT = "evals/s"
+# fp64 ALU roofline: 64 DFMA/clk/SM x 148 SMs x 1.965 GHz x 2 flop (guide unit counts and
+# clocks.max.sm; a register-resident DMMA m8n8k4 loop measured 37.15 TFLOP/s and a DFMA loop
+# 34.0 TFLOP/s on this pool - profiles/r01_peaks.md).  DESIGN.md "Rooflines".
+FP64_PEAK_TFLOPS = 37.2
+
+
+def alg_flops_per_eval(seg_lengths) -> float:
+    """three real length-m FFT equivalents + 2 half-spectrum products + O(N) tail."""
+    tot = 0.0
+    for n in seg_lengths:
+        m = 2 * (1 << max(8, int(math.ceil(math.log2(max(int(n), 1))))))
+        tot += 3 * 2.5 * m * math.log2(m) + 6 * m + 5 * int(n)
+    return tot
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return json.load(open(p)), "measured"
+        except Exception:
+            pass
+    return {"hbm_gbs": 6650.0}, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows = []
+        self.proc = None
+        self.index = index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "50"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), line.strip()))
+
+    def stop(self, t0: float, t1: float) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.06)
+        self.proc.terminate()
+        sm, mx, reasons = [], None, set()
+        rows = [r for (ts, r) in self.rows if t0 - 0.05 <= ts <= t1 + 0.1] or [r for _, r in self.rows]
+        for r in rows:
+            f = [x.strip() for x in r.split(",")]
+            try:
+                sm.append(float(f[0])); mx = float(f[1])
+            except Exception:
+                continue
+            for name, val in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": mx, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def oracle_rate(w, budget_templates: int):
+    """The oracle as it stands on the host cores: (evals/s of the batched solve, factor seconds, cores, sample)."""
+    from oracle import td_oracle as O
+    try:
+        from threadpoolctl import threadpool_info
+        th = max([p.get("num_threads", 1) for p in threadpool_info()] or [os.cpu_count() or 1])
+    except Exception:
+        th = os.cpu_count() or 1
+    nb = min(w.B, budget_templates)
+    t0 = time.perf_counter()
+    if w.n_tot > 40000 and len(w.seg_lengths) == 1:
+        out = O.loglike_batch_solve_toeplitz(w.acf, w.seg_lengths, w.d, w.H[:nb])
+        tf, ts = 0.0, time.perf_counter() - t0
+        kind = "scipy solve_toeplitz per template (dense C does not fit)"
+    else:
+        fac = O.factorize(w.acf, w.seg_lengths)
+        tf = time.perf_counter() - t0
+        t1 = time.perf_counter()
+        out = O.loglike_batch(w.acf, w.seg_lengths, w.d, w.H[:nb], factors=fac)
+        ts = time.perf_counter() - t1
+        kind = "Cholesky once (%.2f s, not counted) + batched forward substitution" % tf
+    return nb / ts, tf, th, f"{nb} of {w.B} templates of {w.name}; {kind}", out
+
+
+def run_reference(args):
+    from paper_2603_06010_b200 import workloads as W
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    nb = {"c1": 64, "c2": 1024, "c3": 256, "c4": 2, "c5": 256}.get(args.config, 256)
+    w = W.make(args.config, B=nb)
+    rates = []
+    for i in range(args.warmup + args.steps):
+        r, tf, th, sample, _ = oracle_rate(w, nb)
+        if i >= args.warmup:
+            rates.append(r)
+    val = float(np.mean(rates))
+    line = {"metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * nb / val, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic", "impl": "reference",
+            "config": {"workload": f"{args.config}: bounded sample, each step = {sample}"},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": th, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--config", default="c2")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--B", type=int, default=None, help="override templates per GPU (default: the config's B)")
+    ap.add_argument("--path", type=int, default=0, help="0 auto, 1 FFT, 2 dense")
+    ap.add_argument("--fft-variant", type=int, default=0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import torch.distributed as dist
+    from paper_2603_06010_b200 import binding as tdb
+    from paper_2603_06010_b200 import workloads as W
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback exists)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    tdb.load(build_if_missing=False)
+
+    w = W.make(args.config, B=args.B)
+    B, n_tot = w.B, w.n_tot
+    h = tdb.TDLikelihood(w.acf, w.seg_lengths, device=local)
+    if args.path:
+        h.set_path(args.path)
+    if args.fft_variant:
+        h.set_fft_variant(args.fft_variant)
+    d = torch.as_tensor(w.d).to(dev)
+    H_host = torch.as_tensor(w.H).pin_memory()
+    # >= 3 distinct device copies of H, rotated, so no step is served from the 126 MB L2
+    nbuf = max(3, int(math.ceil(3 * 126e6 / (8.0 * B * n_tot))))
+    nbuf = min(nbuf, 64)
+    Hs = [H_host.to(dev, non_blocking=True) for _ in range(nbuf)]
+    out = torch.empty(B, dtype=torch.float64, device=dev)
+    stream = torch.cuda.current_stream(dev)
+    torch.cuda.synchronize()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+
+    # ---------------- device-resident throughput
+    for i in range(args.warmup):
+        h.loglike_batch(d, Hs[i % nbuf], out=out)
+    torch.cuda.synchronize()
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.12)
+    evs = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+    launches = 0
+    torch.cuda.synchronize()
+    barrier()
+    t_wall0 = time.time()
+    evs[0].record(stream)
+    for i in range(args.steps):
+        h.loglike_batch(d, Hs[i % nbuf], out=out)
+        launches += h.last_launches()
+        evs[i + 1].record(stream)
+    torch.cuda.synchronize()
+    t_wall1 = time.time()
+    barrier()
+    total_ms = evs[0].elapsed_time(evs[-1])
+    step_ms = [evs[i].elapsed_time(evs[i + 1]) for i in range(args.steps)]
+    clocks = sampler.stop(t_wall0, t_wall1) if rank == 0 else None
+    path_used = h.info()["last_path"]
+    if world > 1:
+        t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    value = world * B * args.steps / (total_ms * 1e-3)
+
+    # ---------------- end to end: host buffers through the C ABI (H2D of H and d, D2H of out, per step)
+    e2e = None
+    if not args.no_e2e:
+        out_host = np.empty(B)
+        for _ in range(2):
+            h.loglike_batch_host(w.d, H_host, out_host)
+        torch.cuda.synchronize()
+        barrier()
+        k_e2e = max(3, min(args.steps, 10))
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(k_e2e):
+            h.loglike_batch_host(w.d, H_host, out_host)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        barrier()
+        ms = e0.elapsed_time(e1)
+        if world > 1:
+            t = torch.tensor([ms], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms = float(t.item())
+        e2e = {"value": world * B * k_e2e / (ms * 1e-3), "unit": UNIT,
+               "h2d_bytes_per_step": int(8 * B * n_tot + 8 * n_tot), "d2h_bytes_per_step": int(8 * B),
+               "steps": k_e2e, "api": "td_loglike_batch_host (pinned H, chunked copies overlapped with kernels)"}
+        max_dev = float(np.max(np.abs(out_host - out.cpu().numpy())))
+        e2e["max_abs_diff_vs_device_call"] = max_dev
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---------------- rooflines (dominant kernel = the one kernel of the step on the fused path)
+    peaks, peaks_kind = measured_peaks()
+    kern_ms = float(np.mean(step_ms))
+    falg = alg_flops_per_eval(w.seg_lengths)
+    ach_tf = falg * B / (kern_ms * 1e-3) / 1e12
+    ach_gbs = (8.0 * n_tot * B + 8.0 * B) / (kern_ms * 1e-3) / 1e9
+    traffic = None
+    tp = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tp):
+        try:
+            traffic = json.load(open(tp)).get(args.config)
+        except Exception:
+            traffic = None
+    roofline = {"bound": "alu", "achieved": ach_tf, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
+                "frac": ach_tf / FP64_PEAK_TFLOPS, "traffic": traffic,
+                "kernel": "td_fused_kernel" if path_used == 1 else "td_dense_kernel",
+                "kernel_ms": kern_ms, "alg_flops_per_eval": falg,
+                "peak_source": "derived: 64 DFMA/clk/SM x 148 SM x 1.965 GHz x 2 (DESIGN.md); measured DMMA loop 37.15, DFMA loop 34.0"}
+    roofline_hbm = {"bound": "hbm", "achieved": ach_gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                    "frac": ach_gbs / peaks["hbm_gbs"], "peak_source": peaks_kind + " (MEASURED_PEAKS.json copy bandwidth)",
+                    "alg_bytes_per_eval": 8.0 * n_tot + 8.0}
+
+    # ---------------- the oracle on the host cores, bounded sample
+    cpu = None
+    if not args.no_cpu_baseline:
+        budget = {"c1": 64, "c2": 2048, "c3": 256, "c4": 2, "c5": 256}.get(args.config, 256)
+        r, tf, th, sample, ref = oracle_rate(w, budget)
+        got = out.cpu().numpy()[: len(ref)]
+        cpu = {"value": r, "unit": UNIT, "cores": th, "kind": "oracle", "sample": sample,
+               "max_rel_err_gpu_vs_oracle": float(np.max(np.abs(got - ref) / np.maximum(np.abs(ref), 1.0)))}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"{args.config}: {w.description}; N_tot={n_tot}, segments={list(map(int, w.seg_lengths))}, B={B} per GPU",
+                       "path": {1: "fft", 2: "dense"}.get(path_used, "?"),
+                       "l2": f"{nbuf} distinct device copies of H rotated between steps (H = {8 * B * n_tot / 2**20:.0f} MiB each)",
+                       "parallelism": f"dp{world} over templates"},
+            "roofline": roofline, "roofline_hbm": roofline_hbm, "cpu_baseline": cpu, "e2e": e2e,
+            "gpu_launches": launches, "clocks": clocks}
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()
