@@ -133,6 +133,27 @@ __host__ __device__ __forceinline__ int plan_freq(int p, int n) {
   return k;
 }
 
+// compile-time version of the same maps (all shifts and masks)
+template <int N> struct PlanT {
+  static constexpr int LOGN = ilog2(N), NP = plan_np(N), R1 = plan_r1(N), LR1 = ilog2(R1);
+  __device__ static __forceinline__ int pos(int k) {
+    int p = (k & (R1 - 1)) << (LOGN - LR1);
+    k >>= LR1;
+#pragma unroll
+    for (int q = 1; q < NP; ++q) {
+      p += (k & 15) << (LOGN - LR1 - 4 * q);
+      k >>= 4;
+    }
+    return p;
+  }
+  __device__ static __forceinline__ int freq(int p) {
+    int k = p >> (LOGN - LR1);
+#pragma unroll
+    for (int q = 1; q < NP; ++q) k += ((p >> (LOGN - LR1 - 4 * q)) & 15) << (LR1 + 4 * (q - 1));
+    return k;
+  }
+};
+
 // ---- array accessors --------------------------------------------------------------------
 // shared memory, padded one element per 16 so that stride-16 (last-pass) and contiguous
 // (other passes) accesses are both bank-conflict free for 16-byte elements.
@@ -178,6 +199,42 @@ __device__ __forceinline__ void dit_task(const Arr& A, int L, int g, const cplx 
     constexpr int ss = decltype(s)::value;
     cplx v = A.ld(base + ss * S);
     if (ss > 0 && tw) v = cmulc(v, w[ss]);
+    x[ss] = v;
+  });
+  fft_reg<R, true>(x);
+  static_for<0, R>([&](auto t) {
+    constexpr int tt = decltype(t)::value;
+    A.st(base + tt * S, x[brevR<R>(tt)]);
+  });
+}
+
+// compile-time-shape variants (S, masks and shifts fold to constants)
+template <int R, int L, class Arr>
+__device__ __forceinline__ void dif_task_c(const Arr& A, int g, const cplx (&w)[R]) {
+  constexpr int S = L / R, LS = ilog2(S);
+  const int blk = g >> LS, j = g & (S - 1);
+  const int base = blk * L + j;
+  cplx x[R];
+#pragma unroll
+  for (int s = 0; s < R; ++s) x[s] = A.ld(base + s * S);
+  fft_reg<R, false>(x);
+  static_for<0, R>([&](auto t) {
+    constexpr int tt = decltype(t)::value;
+    cplx v = x[brevR<R>(tt)];
+    if constexpr (tt > 0 && (S > 1)) v = cmul(v, w[tt]);
+    A.st(base + tt * S, v);
+  });
+}
+template <int R, int L, class Arr>
+__device__ __forceinline__ void dit_task_c(const Arr& A, int g, const cplx (&w)[R]) {
+  constexpr int S = L / R, LS = ilog2(S);
+  const int blk = g >> LS, j = g & (S - 1);
+  const int base = blk * L + j;
+  cplx x[R];
+  static_for<0, R>([&](auto s) {
+    constexpr int ss = decltype(s)::value;
+    cplx v = A.ld(base + ss * S);
+    if constexpr (ss > 0 && (S > 1)) v = cmulc(v, w[ss]);
     x[ss] = v;
   });
   fft_reg<R, true>(x);

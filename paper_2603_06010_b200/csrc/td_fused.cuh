@@ -180,39 +180,152 @@ __device__ __forceinline__ void last_pass_task(const Arr& ZE, const Arr& ZO, int
   });
 }
 
-// one radix-16 shared-memory pass over both branches
-template <int NT, bool FWD>
-__device__ __forceinline__ void smem_pass16(const SmemArr& AE, const SmemArr& AO, int n, int L,
-                                            const cplx* __restrict__ T, int TW, int tid) {
-  constexpr int R = 16;
-  const int TB = n / R, S = L / R;
-  const bool tw = S > 1;
-  if (TB >= NT) {
-    for (int g = tid; g < TB; g += NT) {
-      cplx w[R];
-      if (tw) tw_powers<R>(T[(g % S) * (TW / L)], w);
-      if (FWD) { dif_task<R>(AE, L, g, w, tw); dif_task<R>(AO, L, g, w, tw); }
-      else     { dit_task<R>(AE, L, g, w, tw); dit_task<R>(AO, L, g, w, tw); }
-    }
-  } else {
-    for (int id = tid; id < 2 * TB; id += NT) {
-      const int br = id / TB, g = id - br * TB;
-      cplx w[R];
-      if (tw) tw_powers<R>(T[(g % S) * (TW / L)], w);
-      if (FWD) dif_task<R>(br ? AO : AE, L, g, w, tw);
-      else     dit_task<R>(br ? AO : AE, L, g, w, tw);
-    }
-  }
-}
-
+// ---------------------------------------------------------------------------------------------
+// Fused kernel proper: every shape is a compile-time constant, twiddle bases come from a small
+// shared-memory table (tw[k] = w_2M^k, k < TWS) and conjugate pairs are enumerated directly.
+// ---------------------------------------------------------------------------------------------
 template <int LOG2M> struct FusedShape {
   static constexpr int M = 1 << LOG2M, NF = M / 2;
   static constexpr int RF1 = plan_r1(NF), NPF = plan_np(NF);
   static constexpr int RI1 = plan_r1(M), NPI = plan_np(M);
+  static constexpr int RMIN = RF1 < RI1 ? RF1 : RI1;
+  static constexpr int TWS = 2 * M / RMIN;  // largest base-twiddle index used + 1 (<= this)
   static constexpr size_t smem_bytes(int nt) {
-    return sizeof(cplx) * (2 * (size_t)SmemArr::padded(NF) + 2 * (size_t)SmemArr::padded(M)) + sizeof(double) * 2 * (nt / 32);
+    return sizeof(cplx) * (2 * (size_t)SmemArr::padded(NF) + 2 * (size_t)SmemArr::padded(M) + TWS + 16) +
+           sizeof(double) * 2 * (nt / 32);
   }
 };
+
+template <int NT, bool FWD, int N, int L>
+__device__ __forceinline__ void smem_pass16c(const SmemArr& AE, const SmemArr& AO, const cplx* __restrict__ tw,
+                                             int TW, int tid) {
+  constexpr int R = 16, TB = N / R, S = L / R;
+  if constexpr (TB >= NT) {
+#pragma unroll 1
+    for (int g = tid; g < TB; g += NT) {
+      cplx w[R];
+      if constexpr (S > 1) tw_powers<R>(tw[(g & (S - 1)) * (TW / L)], w);
+      if constexpr (FWD) { dif_task_c<R, L>(AE, g, w); dif_task_c<R, L>(AO, g, w); }
+      else               { dit_task_c<R, L>(AE, g, w); dit_task_c<R, L>(AO, g, w); }
+    }
+  } else {
+#pragma unroll 1
+    for (int id = tid; id < 2 * TB; id += NT) {
+      const int br = id / TB, g = id - br * TB;
+      cplx w[R];
+      if constexpr (S > 1) tw_powers<R>(tw[(g & (S - 1)) * (TW / L)], w);
+      if constexpr (FWD) dif_task_c<R, L>(br ? AO : AE, g, w);
+      else               dit_task_c<R, L>(br ? AO : AE, g, w);
+    }
+  }
+}
+
+// first forward pass with compile-time shapes and shared-memory twiddles
+template <int R, int NF, int MODE>
+__device__ __forceinline__ void first_pass_c(const SmemArr& UE, const SmemArr& UO, int j,
+                                             const double* __restrict__ drow, const double* __restrict__ hrow,
+                                             int n, bool vec, const cplx* __restrict__ tw) {
+  constexpr int S = NF / R;
+  cplx x[R], y[R];
+#pragma unroll
+  for (int s = 0; s < R; ++s) x[s] = load_pair<MODE>(drow, hrow, j + s * S, n, vec);
+  static_for<0, R>([&](auto s) {
+    constexpr int ss = decltype(s)::value;
+    y[ss] = mul_w32<ss * (16 / R), false>(x[ss]);
+  });
+  cplx w[R];
+  const cplx beta = tw[2 * j];  // w_M^j
+  tw_powers<R>(tw[4 * j], w);   // w_NF^j
+  fft_reg<R, false>(x);
+  fft_reg<R, false>(y);
+  static_for<0, R>([&](auto t) {
+    constexpr int tt = decltype(t)::value;
+    cplx ve = x[brevR<R>(tt)], vo = y[brevR<R>(tt)];
+    if constexpr (tt > 0) {
+      ve = cmul(ve, w[tt]);
+      vo = cmul(vo, cmul(w[tt], beta));
+    } else {
+      vo = cmul(vo, beta);
+    }
+    UE.st(j + tt * S, ve);
+    UO.st(j + tt * S, vo);
+  });
+}
+
+// untangle + generator product for the conjugate pair (k', partner) of branch BR.
+// k' = kap + (NF/16) t: the bins of one last-pass block, so lanes t = 0..15 read 16 consecutive
+// positions.  w_2M^(2k'+BR) = tw[2 kap + BR] * w_32^t.
+template <int BR, int NF>
+__device__ __forceinline__ void untangle_pair(const SmemArr& U, const SmemArr& Z, const cplx* __restrict__ G,
+                                              int kap, int t, const cplx* __restrict__ tw,
+                                              const cplx* __restrict__ c32) {
+  constexpr int M = 2 * NF;
+  const int kq = kap + (NF / 16) * t;
+  int kq2, i1, i3;
+  const int i2 = NF + kq;
+  if constexpr (BR == 0) {
+    kq2 = (NF - kq) & (NF - 1);
+    i1 = NF - kq;
+    i3 = (M - kq) & (M - 1);
+  } else {
+    kq2 = NF - 1 - kq;
+    i1 = NF - 1 - kq;
+    i3 = M - 1 - kq;
+  }
+  const int p0 = PlanT<M>::pos(kq), p1 = PlanT<M>::pos(i1), p2 = PlanT<M>::pos(i2), p3 = PlanT<M>::pos(i3);
+  const cplx g0 = __ldg(G + p0), g1 = __ldg(G + p1), g2 = __ldg(G + p2), g3 = __ldg(G + p3);
+  const cplx U1 = U.ld(PlanT<NF>::pos(kq)), U2 = U.ld(PlanT<NF>::pos(kq2));
+  const cplx w = cmul(tw[2 * kap + BR], c32[t]);
+  const cplx A = mk(0.5 * (U1.x + U2.x), 0.5 * (U1.y - U2.y));
+  const cplx Bv = mk(0.5 * (U1.y + U2.y), -0.5 * (U1.x - U2.x));
+  const cplx wB = cmul(w, Bv);
+  const cplx Xk = cadd(A, wB), Xm = csub(A, wB);
+  Z.st(p0, cmul(g0, Xk));
+  Z.st(p1, cmul(g1, cconj(Xm)));
+  Z.st(p2, cmul(g2, Xm));
+  Z.st(p3, cmul(g3, cconj(Xk)));
+}
+
+template <int R, int M, int MODE>
+__device__ __forceinline__ void last_pass_c(const SmemArr& ZE, const SmemArr& ZO, int j, int n,
+                                            const cplx* __restrict__ tw, cplx* __restrict__ zd, double& acc0,
+                                            double& acc1) {
+  constexpr int S = M / R;
+  cplx w[R], e[R], o[R];
+  const cplx beta = tw[j];     // w_2M^j
+  tw_powers<R>(tw[2 * j], w);  // w_M^j
+  static_for<0, R>([&](auto s) {
+    constexpr int ss = decltype(s)::value;
+    cplx ve = ZE.ld(j + ss * S), vo = ZO.ld(j + ss * S);
+    if constexpr (ss > 0) {
+      ve = cmulc(ve, w[ss]);
+      vo = cmulc(vo, cmul(w[ss], beta));
+    } else {
+      vo = cmulc(vo, beta);
+    }
+    e[ss] = ve;
+    o[ss] = vo;
+  });
+  fft_reg<R, true>(e);
+  fft_reg<R, true>(o);
+  static_for<0, R>([&](auto t) {
+    constexpr int tt = decltype(t)::value;
+    const cplx ot = mul_w32<tt * (16 / R), true>(o[brevR<R>(tt)]);
+    const cplx z = cadd(e[brevR<R>(tt)], ot);
+    const int i = j + tt * S;
+    if constexpr (MODE == MODE_STOREZ) {
+      zd[i] = z;
+    } else {
+      if (i < n) {
+        if constexpr (MODE == MODE_INNER) {
+          const cplx q = zd[i];
+          acc0 = fma(z.x, q.x, fma(-z.y, q.y, acc0));
+        }
+        acc1 = fma(z.x, z.x, fma(-z.y, z.y, acc1));
+      }
+    }
+  });
+}
 
 template <int LOG2M, int NT, int MODE>
 __global__ void __launch_bounds__(NT, 1) td_fused_kernel(const FusedParams P) {
@@ -222,9 +335,14 @@ __global__ void __launch_bounds__(NT, 1) td_fused_kernel(const FusedParams P) {
   cplx* sm = reinterpret_cast<cplx*>(smem_raw);
   const SmemArr UE{sm}, UO{sm + SmemArr::padded(NF)};
   const SmemArr ZE{sm + 2 * SmemArr::padded(NF)}, ZO{sm + 2 * SmemArr::padded(NF) + SmemArr::padded(M)};
-  double* red = reinterpret_cast<double*>(sm + 2 * SmemArr::padded(NF) + 2 * SmemArr::padded(M));
+  cplx* tw = sm + 2 * SmemArr::padded(NF) + 2 * SmemArr::padded(M);
+  cplx* c32 = tw + Sh::TWS;
+  double* red = reinterpret_cast<double*>(c32 + 16);
   const int tid = threadIdx.x;
-  const cplx* __restrict__ T = P.T;
+
+  for (int k = tid; k < Sh::TWS; k += NT) tw[k] = P.T[k];
+  if (tid < 16) c32[tid] = P.T[tid * (TW / 32)];
+  __syncthreads();
 
   for (long long b = blockIdx.x; b < P.B; b += gridDim.x) {
     double tot0 = 0.0, tot1 = 0.0;
@@ -234,39 +352,43 @@ __global__ void __launch_bounds__(NT, 1) td_fused_kernel(const FusedParams P) {
       const double* hrow = (MODE == MODE_STOREZ) ? drow : P.H + b * P.ldh + sg.off;
       const bool vec = ((reinterpret_cast<uintptr_t>(drow) | reinterpret_cast<uintptr_t>(hrow)) & 15) == 0;
       // ---- S1+S2: forward, pass 1 from global
+#pragma unroll 1
       for (int g = tid; g < NF / Sh::RF1; g += NT)
-        first_pass_task<Sh::RF1, MODE>(UE, UO, NF, g, drow, hrow, sg.n, vec, T);
+        first_pass_c<Sh::RF1, NF, MODE>(UE, UO, g, drow, hrow, sg.n, vec, tw);
       __syncthreads();
       // ---- forward passes 2..NPF (radix 16)
-      {
-        int L = NF / Sh::RF1;
-#pragma unroll
-        for (int q = 1; q < Sh::NPF; ++q) {
-          smem_pass16<NT, true>(UE, UO, NF, L, T, TW, tid);
-          __syncthreads();
-          L >>= 4;
-        }
-      }
+      static_for<1, Sh::NPF>([&](auto q) {
+        constexpr int L = (NF / Sh::RF1) >> (4 * (decltype(q)::value - 1));
+        smem_pass16c<NT, true, NF, L>(UE, UO, tw, TW, tid);
+        __syncthreads();
+      });
       // ---- untangle + S3 generator product
-      for (int id = tid; id < 2 * NF; id += NT) {
-        const int br = id / NF, p = id - br * NF;
-        untangle_task(br ? UO : UE, br ? ZO : ZE, sg.G + br * M, br, p, NF, M, T);
+      {
+        constexpr int NKE = (NF / 32 + 1) * 16, NKO = NF / 2;
+#pragma unroll 1
+        for (int id = tid; id < NKE + NKO; id += NT) {
+          if (id < NKE) {
+            const int kap = id >> 4, t = id & 15;
+            const bool skip = (kap == 0 && t > 8) || (kap == NF / 32 && t > 7);
+            if (!skip) untangle_pair<0, NF>(UE, ZE, sg.G, kap, t, tw, c32);
+          } else {
+            const int id2 = id - NKE;
+            untangle_pair<1, NF>(UO, ZO, sg.G + M, id2 >> 4, id2 & 15, tw, c32);
+          }
+        }
       }
       __syncthreads();
       // ---- S4: inverse passes (radix 16), smallest sub-transform first
-      {
-        int L = 16;
-#pragma unroll
-        for (int q = 1; q < Sh::NPI; ++q) {
-          smem_pass16<NT, false>(ZE, ZO, M, L, T, TW, tid);
-          __syncthreads();
-          L <<= 4;
-        }
-      }
+      static_for<1, Sh::NPI>([&](auto q) {
+        constexpr int L = 16 << (4 * (decltype(q)::value - 1));
+        smem_pass16c<NT, false, M, L>(ZE, ZO, tw, TW, tid);
+        __syncthreads();
+      });
       // ---- last inverse pass + pruned radix-2 stage + S5
       double acc0 = 0.0, acc1 = 0.0;
+#pragma unroll 1
       for (int g = tid; g < M / Sh::RI1; g += NT)
-        last_pass_task<Sh::RI1, MODE>(ZE, ZO, M, g, sg.n, T, sg.zd, acc0, acc1);
+        last_pass_c<Sh::RI1, M, MODE>(ZE, ZO, g, sg.n, tw, sg.zd, acc0, acc1);
       if (MODE != MODE_STOREZ) {
         acc0 = warp_sum(acc0);
         acc1 = warp_sum(acc1);
