@@ -192,7 +192,7 @@ template <int LOG2M> struct FusedShape {
   static constexpr int TWS = 2 * M / RMIN;  // largest base-twiddle index used + 1 (<= this)
   static constexpr size_t smem_bytes(int nt) {
     return sizeof(cplx) * (2 * (size_t)SmemArr::padded(NF) + 2 * (size_t)SmemArr::padded(M) + TWS + 16) +
-           sizeof(double) * 2 * (nt / 32);
+           sizeof(double) * 2 * (nt / 32) + 16;  // + mbarrier
   }
 };
 
@@ -327,7 +327,156 @@ __device__ __forceinline__ void last_pass_c(const SmemArr& ZE, const SmemArr& ZO
   });
 }
 
-template <int LOG2M, int NT, int MODE>
+// ---- async bulk copy (TMA, 1-D) + mbarrier helpers -------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t mbar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(mbar), "r"(count) : "memory");
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t mbar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(mbar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t mbar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+               "l"(src), "r"(bytes), "r"(mbar)
+               : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t mbar, uint32_t parity) {
+  uint32_t ok;
+  do {
+    asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
+                 : "=r"(ok)
+                 : "r"(mbar), "r"(parity)
+                 : "memory");
+  } while (!ok);
+}
+
+// both branches of one radix-16 butterfly task interleaved (twice the independent work per thread)
+template <bool FWD, int L>
+__device__ __forceinline__ void pass16_pair(const SmemArr& AE, const SmemArr& AO, int g, const cplx (&w)[16]) {
+  constexpr int R = 16, S = L / R, LS = ilog2(S);
+  const int blk = g >> LS, j = g & (S - 1);
+  const int base = blk * L + j;
+  cplx x[R], y[R];
+  static_for<0, R>([&](auto s) {
+    constexpr int ss = decltype(s)::value;
+    cplx a = AE.ld(base + ss * S), b = AO.ld(base + ss * S);
+    if constexpr (!FWD && ss > 0 && (S > 1)) { a = cmulc(a, w[ss]); b = cmulc(b, w[ss]); }
+    x[ss] = a; y[ss] = b;
+  });
+  fft_reg<R, !FWD>(x);
+  fft_reg<R, !FWD>(y);
+  static_for<0, R>([&](auto t) {
+    constexpr int tt = decltype(t)::value;
+    cplx a = x[brevR<R>(tt)], b = y[brevR<R>(tt)];
+    if constexpr (FWD && tt > 0 && (S > 1)) { a = cmul(a, w[tt]); b = cmul(b, w[tt]); }
+    AE.st(base + tt * S, a);
+    AO.st(base + tt * S, b);
+  });
+}
+
+template <int NT, bool FWD, int N, int L, bool ILV>
+__device__ __forceinline__ void smem_pass16v(const SmemArr& AE, const SmemArr& AO, const cplx* __restrict__ tw,
+                                             int TW, int tid) {
+  constexpr int TB = N / 16, S = L / 16;
+  if constexpr (ILV && TB >= NT) {
+#pragma unroll 1
+    for (int g = tid; g < TB; g += NT) {
+      cplx w[16];
+      if constexpr (S > 1) tw_powers<16>(tw[(g & (S - 1)) * (TW / L)], w);
+      pass16_pair<FWD, L>(AE, AO, g, w);
+    }
+  } else {
+    smem_pass16c<NT, FWD, N, L>(AE, AO, tw, TW, tid);
+  }
+}
+
+// first pass fed from the staged (TMA-prefetched) rows in shared memory: values only
+template <int R, int NF, int MODE>
+__device__ __forceinline__ void first_pass_load_staged(cplx (&x)[R], int j, const double* stH, const double* stD,
+                                                       int n) {
+  constexpr int S = NF / R;
+#pragma unroll
+  for (int s = 0; s < R; ++s) {
+    const int i0 = 2 * (j + s * S);
+    double2 h = mk(0.0, 0.0), d = mk(0.0, 0.0);
+    if (i0 < n) {  // n even on this path: i0 + 1 < n too
+      if (MODE != MODE_STOREZ) h = *reinterpret_cast<const double2*>(stH + i0);
+      if (MODE != MODE_INNER) d = *reinterpret_cast<const double2*>(stD + i0);
+    }
+    x[s] = (MODE == MODE_LOGLIKE) ? mk(d.x - h.x, d.y - h.y) : (MODE == MODE_INNER ? h : d);
+  }
+}
+template <int R, int NF>
+__device__ __forceinline__ void first_pass_compute(const SmemArr& UE, const SmemArr& UO, int j, cplx (&x)[R],
+                                                   const cplx* __restrict__ tw) {
+  constexpr int S = NF / R;
+  cplx y[R];
+  static_for<0, R>([&](auto s) {
+    constexpr int ss = decltype(s)::value;
+    y[ss] = mul_w32<ss * (16 / R), false>(x[ss]);
+  });
+  cplx w[R];
+  const cplx beta = tw[2 * j];
+  tw_powers<R>(tw[4 * j], w);
+  fft_reg<R, false>(x);
+  fft_reg<R, false>(y);
+  static_for<0, R>([&](auto t) {
+    constexpr int tt = decltype(t)::value;
+    cplx ve = x[brevR<R>(tt)], vo = y[brevR<R>(tt)];
+    if constexpr (tt > 0) {
+      ve = cmul(ve, w[tt]);
+      vo = cmul(vo, cmul(w[tt], beta));
+    } else {
+      vo = cmul(vo, beta);
+    }
+    UE.st(j + tt * S, ve);
+    UO.st(j + tt * S, vo);
+  });
+}
+
+// untangle task id -> (branch, kap, t); E-branch ids [0, NF/2), O-branch ids [NF/2, NF).
+// E: row kap = 0 is remapped: t = 0 -> the self-paired bin k' = 0 (its twin k' = NF/2 is done
+// by one extra task), t = 1..7 -> kap 0, t = 8..15 -> the self-paired block kap = NF/32, t - 8.
+template <int NF> struct UntangleIdx {
+  int br, kap, t;
+  __device__ __forceinline__ explicit UntangleIdx(int id) {
+    br = id >= NF / 2;
+    const int q = br ? id - NF / 2 : id;
+    kap = q >> 4; t = q & 15;
+    if (!br && kap == 0 && t >= 8) { kap = NF / 32; t -= 8; }
+  }
+};
+template <int NF> struct UntanglePos {
+  int pu1, pu2, p0, p1, p2, p3, twi, t;
+  __device__ __forceinline__ UntanglePos(int br, int kap, int tt) {
+    constexpr int M = 2 * NF;
+    const int kq = kap + (NF / 16) * tt;
+    int kq2, i1, i3;
+    if (br == 0) { kq2 = (NF - kq) & (NF - 1); i1 = NF - kq; i3 = (M - kq) & (M - 1); }
+    else         { kq2 = NF - 1 - kq; i1 = NF - 1 - kq; i3 = M - 1 - kq; }
+    pu1 = PlanT<NF>::pos(kq); pu2 = PlanT<NF>::pos(kq2);
+    p0 = PlanT<M>::pos(kq); p1 = PlanT<M>::pos(i1); p2 = PlanT<M>::pos(NF + kq); p3 = PlanT<M>::pos(i3);
+    twi = 2 * kap + br; t = tt;
+  }
+};
+template <int NF>
+__device__ __forceinline__ void untangle_apply(const SmemArr& U, const SmemArr& Z, const UntanglePos<NF>& q,
+                                               const cplx (&g)[4], const cplx* __restrict__ tw,
+                                               const cplx* __restrict__ c32) {
+  const cplx U1 = U.ld(q.pu1), U2 = U.ld(q.pu2);
+  const cplx w = cmul(tw[q.twi], c32[q.t]);
+  const cplx A = mk(0.5 * (U1.x + U2.x), 0.5 * (U1.y - U2.y));
+  const cplx Bv = mk(0.5 * (U1.y + U2.y), -0.5 * (U1.x - U2.x));
+  const cplx wB = cmul(w, Bv);
+  const cplx Xk = cadd(A, wB), Xm = csub(A, wB);
+  Z.st(q.p0, cmul(g[0], Xk));
+  Z.st(q.p1, cmul(g[1], cconj(Xm)));
+  Z.st(q.p2, cmul(g[2], Xm));
+  Z.st(q.p3, cmul(g[3], cconj(Xk)));
+}
+
+template <int LOG2M, int NT, int MODE, bool ILV = true>
 __global__ void __launch_bounds__(NT, 1) td_fused_kernel(const FusedParams P) {
   using Sh = FusedShape<LOG2M>;
   constexpr int M = Sh::M, NF = Sh::NF, TW = 2 * M;
@@ -338,78 +487,144 @@ __global__ void __launch_bounds__(NT, 1) td_fused_kernel(const FusedParams P) {
   cplx* tw = sm + 2 * SmemArr::padded(NF) + 2 * SmemArr::padded(M);
   cplx* c32 = tw + Sh::TWS;
   double* red = reinterpret_cast<double*>(c32 + 16);
+  const uint32_t mbar = smem_u32(red + 2 * (NT / 32));
+  // staging for the prefetched rows lives in the U region (dead between untangle and the next first pass)
+  double* stH = reinterpret_cast<double*>(sm);
+  double* stD = stH + M;
   const int tid = threadIdx.x;
 
   for (int k = tid; k < Sh::TWS; k += NT) tw[k] = P.T[k];
   if (tid < 16) c32[tid] = P.T[tid * (TW / 32)];
+  if (tid == 0) mbar_init(mbar, 1);
   __syncthreads();
 
-  for (long long b = blockIdx.x; b < P.B; b += gridDim.x) {
-    double tot0 = 0.0, tot1 = 0.0;
-    for (int s = 0; s < P.n_seg; ++s) {
-      const SegDev sg = P.segs[s];
-      const double* drow = P.d + sg.off;
-      const double* hrow = (MODE == MODE_STOREZ) ? drow : P.H + b * P.ldh + sg.off;
+  // rows of item (b, s); staged (TMA) only when 16-byte aligned and N_s even
+  auto rows = [&](long long b, int s, const double*& drow, const double*& hrow, int& n) -> bool {
+    const SegDev sg = P.segs[s];
+    drow = P.d + sg.off;
+    hrow = (MODE == MODE_STOREZ) ? drow : P.H + b * P.ldh + sg.off;
+    n = sg.n;
+    return (((reinterpret_cast<uintptr_t>(drow) | reinterpret_cast<uintptr_t>(hrow)) & 15) == 0) && ((n & 1) == 0);
+  };
+  auto prefetch = [&](long long b, int s) -> bool {
+    const double *drow, *hrow; int n;
+    const bool ok = rows(b, s, drow, hrow, n);
+    if (ok && tid == 0) {
+      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+      const uint32_t bytes = (uint32_t)n * 8u;
+      const int ncopies = (MODE == MODE_LOGLIKE) ? 2 : 1;
+      mbar_expect_tx(mbar, bytes * ncopies);
+      if (MODE != MODE_STOREZ) bulk_g2s(smem_u32(stH), hrow, bytes, mbar);
+      if (MODE != MODE_INNER) bulk_g2s(smem_u32(stD), drow, bytes, mbar);
+    }
+    return ok;
+  };
+
+  long long b = blockIdx.x;
+  int s = 0;
+  bool have = b < P.B;
+  uint32_t parity = 0;
+  bool staged = have ? prefetch(b, s) : false;
+  double tot0 = 0.0, tot1 = 0.0;
+  while (have) {
+    long long nb = b; int ns = s + 1;
+    if (ns == P.n_seg) { ns = 0; nb = b + gridDim.x; }
+    const bool have_next = (MODE != MODE_STOREZ || nb == b) && nb < P.B;
+    const SegDev sg = P.segs[s];
+    // ---- S1+S2: forward, pass 1
+    if (staged) {
+      mbar_wait(mbar, parity);
+      parity ^= 1;
+      constexpr int NTASK = NF / Sh::RF1;
+      static_assert(NTASK <= NT || NTASK % NT == 0, "first pass tiling");
+      constexpr int IT = (NTASK + NT - 1) / NT;
+      cplx xs[IT][Sh::RF1];
+#pragma unroll
+      for (int it = 0; it < IT; ++it)
+        if (tid + it * NT < NTASK) first_pass_load_staged<Sh::RF1, NF, MODE>(xs[it], tid + it * NT, stH, stD, sg.n);
+      __syncthreads();  // staging consumed: the U region may now be overwritten
+#pragma unroll
+      for (int it = 0; it < IT; ++it)
+        if (tid + it * NT < NTASK) first_pass_compute<Sh::RF1, NF>(UE, UO, tid + it * NT, xs[it], tw);
+    } else {
+      const double *drow, *hrow; int n;
+      rows(b, s, drow, hrow, n);
       const bool vec = ((reinterpret_cast<uintptr_t>(drow) | reinterpret_cast<uintptr_t>(hrow)) & 15) == 0;
-      // ---- S1+S2: forward, pass 1 from global
 #pragma unroll 1
       for (int g = tid; g < NF / Sh::RF1; g += NT)
-        first_pass_c<Sh::RF1, NF, MODE>(UE, UO, g, drow, hrow, sg.n, vec, tw);
+        first_pass_c<Sh::RF1, NF, MODE>(UE, UO, g, drow, hrow, n, vec, tw);
+    }
+    __syncthreads();
+    // ---- forward passes 2..NPF (radix 16)
+    static_for<1, Sh::NPF>([&](auto q) {
+      constexpr int L = (NF / Sh::RF1) >> (4 * (decltype(q)::value - 1));
+      smem_pass16v<NT, true, NF, L, ILV>(UE, UO, tw, TW, tid);
       __syncthreads();
-      // ---- forward passes 2..NPF (radix 16)
-      static_for<1, Sh::NPF>([&](auto q) {
-        constexpr int L = (NF / Sh::RF1) >> (4 * (decltype(q)::value - 1));
-        smem_pass16c<NT, true, NF, L>(UE, UO, tw, TW, tid);
-        __syncthreads();
-      });
-      // ---- untangle + S3 generator product
-      {
-        constexpr int NKE = (NF / 32 + 1) * 16, NKO = NF / 2;
-#pragma unroll 1
-        for (int id = tid; id < NKE + NKO; id += NT) {
-          if (id < NKE) {
-            const int kap = id >> 4, t = id & 15;
-            const bool skip = (kap == 0 && t > 8) || (kap == NF / 32 && t > 7);
-            if (!skip) untangle_pair<0, NF>(UE, ZE, sg.G, kap, t, tw, c32);
-          } else {
-            const int id2 = id - NKE;
-            untangle_pair<1, NF>(UO, ZO, sg.G + M, id2 >> 4, id2 & 15, tw, c32);
-          }
+    });
+    // ---- untangle + S3 generator product (G loads hoisted ahead of the shared-memory work)
+    {
+      constexpr int IT = (NF + NT - 1) / NT;
+      cplx g[IT][4];
+#pragma unroll
+      for (int it = 0; it < IT; ++it) {
+        const int id = tid + it * NT;
+        if (id < NF) {
+          const UntangleIdx<NF> ix(id);
+          const UntanglePos<NF> q(ix.br, ix.kap, ix.t);
+          const cplx* G = sg.G + ix.br * M;
+          g[it][0] = __ldg(G + q.p0); g[it][1] = __ldg(G + q.p1); g[it][2] = __ldg(G + q.p2); g[it][3] = __ldg(G + q.p3);
         }
       }
-      __syncthreads();
-      // ---- S4: inverse passes (radix 16), smallest sub-transform first
-      static_for<1, Sh::NPI>([&](auto q) {
-        constexpr int L = 16 << (4 * (decltype(q)::value - 1));
-        smem_pass16c<NT, false, M, L>(ZE, ZO, tw, TW, tid);
-        __syncthreads();
-      });
-      // ---- last inverse pass + pruned radix-2 stage + S5
-      double acc0 = 0.0, acc1 = 0.0;
-#pragma unroll 1
-      for (int g = tid; g < M / Sh::RI1; g += NT)
-        last_pass_c<Sh::RI1, M, MODE>(ZE, ZO, g, sg.n, tw, sg.zd, acc0, acc1);
-      if (MODE != MODE_STOREZ) {
-        acc0 = warp_sum(acc0);
-        acc1 = warp_sum(acc1);
-        if ((tid & 31) == 0) { red[2 * (tid >> 5)] = acc0; red[2 * (tid >> 5) + 1] = acc1; }
-      }
-      __syncthreads();
-      if (MODE != MODE_STOREZ && tid == 0) {
 #pragma unroll
-        for (int wq = 0; wq < NT / 32; ++wq) { tot0 += red[2 * wq]; tot1 += red[2 * wq + 1]; }
+      for (int it = 0; it < IT; ++it) {
+        const int id = tid + it * NT;
+        if (id < NF) {
+          const UntangleIdx<NF> ix(id);
+          const UntanglePos<NF> q(ix.br, ix.kap, ix.t);
+          untangle_apply<NF>(ix.br ? UO : UE, ix.br ? ZO : ZE, q, g[it], tw, c32);
+        }
+      }
+      if (tid == NT - 1) {  // twin self-paired bin k' = NF/2 of the even branch (kap = 0, t = 8)
+        const UntanglePos<NF> q(0, 0, 8);
+        cplx gg[4] = {__ldg(sg.G + q.p0), __ldg(sg.G + q.p1), __ldg(sg.G + q.p2), __ldg(sg.G + q.p3)};
+        untangle_apply<NF>(UE, ZE, q, gg, tw, c32);
       }
     }
-    if (tid == 0) {
-      if (MODE == MODE_LOGLIKE) {
-        const double v = -0.5 * tot1;
-        P.out0[b] = P.accumulate ? P.out0[b] + v : v;
-      } else if (MODE == MODE_INNER) {
-        if (P.out0) P.out0[b] = P.accumulate ? P.out0[b] + tot0 : tot0;
-        if (P.out1) P.out1[b] = P.accumulate ? P.out1[b] + tot1 : tot1;
+    __syncthreads();
+    // ---- the U region is dead: prefetch the next item's rows into it while the inverse runs
+    const bool staged_next = have_next ? prefetch(nb, ns) : false;
+    // ---- S4: inverse passes (radix 16), smallest sub-transform first
+    static_for<1, Sh::NPI>([&](auto q) {
+      constexpr int L = 16 << (4 * (decltype(q)::value - 1));
+      smem_pass16v<NT, false, M, L, ILV>(ZE, ZO, tw, TW, tid);
+      __syncthreads();
+    });
+    // ---- last inverse pass + pruned radix-2 stage + S5
+    double acc0 = 0.0, acc1 = 0.0;
+#pragma unroll 1
+    for (int g = tid; g < M / Sh::RI1; g += NT)
+      last_pass_c<Sh::RI1, M, MODE>(ZE, ZO, g, sg.n, tw, sg.zd, acc0, acc1);
+    if (MODE != MODE_STOREZ) {
+      acc0 = warp_sum(acc0);
+      acc1 = warp_sum(acc1);
+      if ((tid & 31) == 0) { red[2 * (tid >> 5)] = acc0; red[2 * (tid >> 5) + 1] = acc1; }
+    }
+    __syncthreads();
+    if (MODE != MODE_STOREZ && tid == 0) {
+#pragma unroll
+      for (int wq = 0; wq < NT / 32; ++wq) { tot0 += red[2 * wq]; tot1 += red[2 * wq + 1]; }
+      if (s == P.n_seg - 1) {
+        if (MODE == MODE_LOGLIKE) {
+          const double v = -0.5 * tot1;
+          P.out0[b] = P.accumulate ? P.out0[b] + v : v;
+        } else {
+          if (P.out0) P.out0[b] = P.accumulate ? P.out0[b] + tot0 : tot0;
+          if (P.out1) P.out1[b] = P.accumulate ? P.out1[b] + tot1 : tot1;
+        }
+        tot0 = 0.0; tot1 = 0.0;
       }
     }
-    if (MODE == MODE_STOREZ) break;  // one vector only
+    b = nb; s = ns; have = have_next; staged = staged_next;
   }
 }
 

@@ -219,9 +219,9 @@ td_status run_staged(td_handle* h, const ClassInfo& cls, const SegHost& sg, cons
   return TD_OK;
 }
 
-template <int LOG2M, int MODE>
-td_status launch_fused_t(td_handle* h, const FusedParams& P, cudaStream_t st) {
-  auto kern = td_fused_kernel<LOG2M, FUSED_NT, MODE>;
+template <int LOG2M, int MODE, int FUSED_NT, bool ILV = true>
+td_status launch_fused_nt(td_handle* h, const FusedParams& P, cudaStream_t st) {
+  auto kern = td_fused_kernel<LOG2M, FUSED_NT, MODE, ILV>;
   const size_t smem = FusedShape<LOG2M>::smem_bytes(FUSED_NT);
   CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   int nb = 0;
@@ -233,6 +233,17 @@ td_status launch_fused_t(td_handle* h, const FusedParams& P, cudaStream_t st) {
   CK(cudaGetLastError());
   ++h->last_launches;
   return TD_OK;
+}
+
+template <int LOG2M, int MODE>
+td_status launch_fused_t(td_handle* h, const FusedParams& P, cudaStream_t st) {
+  if constexpr (LOG2M == 12 && MODE == MODE_LOGLIKE) {  // experiment knobs (headline shape only)
+    static const int nt = getenv("TDLIKE_NT") ? atoi(getenv("TDLIKE_NT")) : 256;
+    static const int ilv = getenv("TDLIKE_ILV") ? atoi(getenv("TDLIKE_ILV")) : 1;
+    if (nt == 512) return launch_fused_nt<LOG2M, MODE, 512>(h, P, st);
+    if (!ilv) return launch_fused_nt<LOG2M, MODE, FUSED_NT, false>(h, P, st);
+  }
+  return launch_fused_nt<LOG2M, MODE, FUSED_NT>(h, P, st);
 }
 
 template <int MODE>
