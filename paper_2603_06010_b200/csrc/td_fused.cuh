@@ -8,7 +8,7 @@
 //                                                        complex DIF FFTs (even / odd output bins), then untangled
 //   S3  Z = G .* R^,  G = conj(A^) + i conj(B^)          both generator spectra in one complex array; G is stored
 //                                                        pre-permuted to the DIT input order and pre-scaled by
-//                                                        1/(2M sqrt(v))
+//                                                        1/(4M sqrt(v)) (1/2M inverse FFT, 1/2 untangle)
 //   S4  z_i = IFFT_2M(Z)_i, i < N_s only                 two length-M complex DIT FFTs (even / odd input bins)
 //                                                        + pruned last radix-2 stage; Re z = L(a)^T r/sqrt(v),
 //                                                        Im z = L(b)^T r/sqrt(v)
@@ -127,8 +127,8 @@ __device__ __forceinline__ void untangle_task(const ArrU& U, const ArrZ& Z, cons
   }
   const cplx U1 = U.ld(p), U2 = U.ld(plan_pos(kq2, nf));
   const cplx w = T[2 * kq + br];
-  const cplx A = mk(0.5 * (U1.x + U2.x), 0.5 * (U1.y - U2.y));
-  const cplx Bv = mk(0.5 * (U1.y + U2.y), -0.5 * (U1.x - U2.x));
+  const cplx A = mk(U1.x + U2.x, U1.y - U2.y);        // 2 A_k  (the 1/2 lives in G's scale)
+  const cplx Bv = mk(U1.y + U2.y, -(U1.x - U2.x));    // 2 B_k
   const cplx wB = cmul(w, Bv);
   const cplx Xk = cadd(A, wB), Xm = csub(A, wB);
   const int p0 = plan_pos(kq, M), p1 = plan_pos(i1, M), p2 = plan_pos(i2, M), p3 = plan_pos(i3, M);
@@ -276,8 +276,8 @@ __device__ __forceinline__ void untangle_pair(const SmemArr& U, const SmemArr& Z
   const cplx g0 = __ldg(G + p0), g1 = __ldg(G + p1), g2 = __ldg(G + p2), g3 = __ldg(G + p3);
   const cplx U1 = U.ld(PlanT<NF>::pos(kq)), U2 = U.ld(PlanT<NF>::pos(kq2));
   const cplx w = cmul(tw[2 * kap + BR], c32[t]);
-  const cplx A = mk(0.5 * (U1.x + U2.x), 0.5 * (U1.y - U2.y));
-  const cplx Bv = mk(0.5 * (U1.y + U2.y), -0.5 * (U1.x - U2.x));
+  const cplx A = mk(U1.x + U2.x, U1.y - U2.y);        // 2 A_k  (the 1/2 lives in G's scale)
+  const cplx Bv = mk(U1.y + U2.y, -(U1.x - U2.x));    // 2 B_k
   const cplx wB = cmul(w, Bv);
   const cplx Xk = cadd(A, wB), Xm = csub(A, wB);
   Z.st(p0, cmul(g0, Xk));
@@ -364,13 +364,19 @@ __device__ __forceinline__ void pass16_pair(const SmemArr& AE, const SmemArr& AO
     if constexpr (!FWD && ss > 0 && (S > 1)) { a = cmulc(a, w[ss]); b = cmulc(b, w[ss]); }
     x[ss] = a; y[ss] = b;
   });
+  // software pipeline: E computes while O's loads land; E's stores drain while O computes
   fft_reg<R, !FWD>(x);
+  static_for<0, R>([&](auto t) {
+    constexpr int tt = decltype(t)::value;
+    cplx a = x[brevR<R>(tt)];
+    if constexpr (FWD && tt > 0 && (S > 1)) a = cmul(a, w[tt]);
+    AE.st(base + tt * S, a);
+  });
   fft_reg<R, !FWD>(y);
   static_for<0, R>([&](auto t) {
     constexpr int tt = decltype(t)::value;
-    cplx a = x[brevR<R>(tt)], b = y[brevR<R>(tt)];
-    if constexpr (FWD && tt > 0 && (S > 1)) { a = cmul(a, w[tt]); b = cmul(b, w[tt]); }
-    AE.st(base + tt * S, a);
+    cplx b = y[brevR<R>(tt)];
+    if constexpr (FWD && tt > 0 && (S > 1)) b = cmul(b, w[tt]);
     AO.st(base + tt * S, b);
   });
 }
@@ -466,8 +472,8 @@ __device__ __forceinline__ void untangle_apply(const SmemArr& U, const SmemArr& 
                                                const cplx* __restrict__ c32) {
   const cplx U1 = U.ld(q.pu1), U2 = U.ld(q.pu2);
   const cplx w = cmul(tw[q.twi], c32[q.t]);
-  const cplx A = mk(0.5 * (U1.x + U2.x), 0.5 * (U1.y - U2.y));
-  const cplx Bv = mk(0.5 * (U1.y + U2.y), -0.5 * (U1.x - U2.x));
+  const cplx A = mk(U1.x + U2.x, U1.y - U2.y);        // 2 A_k  (the 1/2 lives in G's scale)
+  const cplx Bv = mk(U1.y + U2.y, -(U1.x - U2.x));    // 2 B_k
   const cplx wB = cmul(w, Bv);
   const cplx Xk = cadd(A, wB), Xm = csub(A, wB);
   Z.st(q.p0, cmul(g[0], Xk));

@@ -1,0 +1,258 @@
+// td_fused4.cuh - the fused FFT-path kernel for M = 1024 / 2048 / 4096 (transform lengths
+// 2M = 2048 / 4096 / 8192), restructured around the two things the first fused kernel lost
+// time on (profiles/r01_fused_v3_regions.md): CTA-wide barriers that put every warp in the
+// same load -> compute -> store phase, and the stand-alone untangle pass.
+//
+//  * plans  NF = M/2 = [RF1,16,16],  M = [RI1,16,16],  RI1 = 2 RF1;  NT = 32 RF1 = M/16 threads;
+//    warps [0, NW/2) own the even-bin branch, warps [NW/2, NW) the odd-bin branch.
+//  * forward passes 2 and 3 touch only the 2 x 256 elements a warp owns: one __syncwarp between them.
+//  * "mid": forward bins are untangled IN REGISTERS from the two mirror blocks, multiplied by the
+//    generator spectrum and pushed through the first inverse radix-16 pass before they are stored.
+//    The generator spectrum of the segment is TMA-prefetched into the Z region (dead during the
+//    forward half) in the padded Z layout, so mid reads G[p] and writes Z[p] in place.
+//  * inverse pass 2 is again warp-local; only the last pass (which joins the two branches and
+//    carries the fused quadratic reduction) needs the whole CTA.
+//  * the next item's rows are TMA-prefetched into the U region by whichever warp finishes mid last.
+// CTA barriers per (template, segment): 5 (was 9).
+#pragma once
+#include "td_fused.cuh"
+
+namespace td {
+
+template <int LOG2M> struct Fused4Shape {
+  static constexpr int M = 1 << LOG2M, NF = M / 2;
+  static constexpr int RF1 = plan_r1(NF), RI1 = plan_r1(M);
+  static_assert(plan_np(NF) == 3 && plan_np(M) == 3 && RI1 == 2 * RF1, "fused4 needs [R,16,16] plans");
+  static constexpr int NT = 32 * RF1, NW = RF1, NWB = RF1 / 2;
+  static constexpr int TWS = 2 * M / RF1;
+  static constexpr int PADM = SmemArr::padded(M), PADNF = SmemArr::padded(NF);
+  static constexpr size_t smem_bytes() {
+    return sizeof(cplx) * (2 * (size_t)PADNF + 2 * (size_t)PADM + TWS) + sizeof(double) * 2 * NW + 32;
+  }
+};
+
+struct Fused4Params {
+  FusedParams base;
+  const cplx* const* Gp;  // device array [n_seg]: generator spectrum in the PADDED Z layout [2][padded(M)]
+};
+
+template <int LOG2M, int MODE>
+__global__ void __launch_bounds__(Fused4Shape<LOG2M>::NT, 1) td_fused4_kernel(const Fused4Params P4) {
+  using Sh = Fused4Shape<LOG2M>;
+  constexpr int M = Sh::M, NF = Sh::NF, TW = 2 * M, NT = Sh::NT, NW = Sh::NW, NWB = Sh::NWB;
+  constexpr int RF1 = Sh::RF1, RI1 = Sh::RI1;
+  const FusedParams& P = P4.base;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  cplx* sm = reinterpret_cast<cplx*>(smem_raw);
+  const SmemArr UE{sm}, UO{sm + Sh::PADNF};
+  const SmemArr ZE{sm + 2 * Sh::PADNF}, ZO{sm + 2 * Sh::PADNF + Sh::PADM};
+  cplx* tw = sm + 2 * Sh::PADNF + 2 * Sh::PADM;
+  double* red = reinterpret_cast<double*>(tw + Sh::TWS);
+  const uint32_t mbar_rows = smem_u32(red + 2 * NW);
+  const uint32_t mbar_g = mbar_rows + 8;
+  int* mid_count = reinterpret_cast<int*>(red + 2 * NW + 2);
+  double* stH = reinterpret_cast<double*>(sm);
+  double* stD = stH + M;
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int br = warp / NWB, wb = warp - br * NWB;  // branch (0 even bins, 1 odd bins), warp within branch
+  const SmemArr U = br ? UO : UE, Z = br ? ZO : ZE;
+
+  for (int k = tid; k < Sh::TWS; k += NT) tw[k] = P.T[k];
+  if (tid == 0) { mbar_init(mbar_rows, 1); mbar_init(mbar_g, 1); *mid_count = 0; }
+  __syncthreads();
+
+  auto rows = [&](long long b, int s, const double*& drow, const double*& hrow, int& n) -> bool {
+    const SegDev sg = P.segs[s];
+    drow = P.d + sg.off;
+    hrow = (MODE == MODE_STOREZ) ? drow : P.H + b * P.ldh + sg.off;
+    n = sg.n;
+    return (((reinterpret_cast<uintptr_t>(drow) | reinterpret_cast<uintptr_t>(hrow)) & 15) == 0) && ((n & 1) == 0);
+  };
+  // issued by ONE thread
+  auto prefetch_rows = [&](long long b, int s) {
+    const double *drow, *hrow; int n;
+    if (rows(b, s, drow, hrow, n)) {
+      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+      const uint32_t bytes = (uint32_t)n * 8u;
+      mbar_expect_tx(mbar_rows, bytes * ((MODE == MODE_LOGLIKE) ? 2 : 1));
+      if (MODE != MODE_STOREZ) bulk_g2s(smem_u32(stH), hrow, bytes, mbar_rows);
+      if (MODE != MODE_INNER) bulk_g2s(smem_u32(stD), drow, bytes, mbar_rows);
+    }
+  };
+  auto prefetch_g = [&](int s) {
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    constexpr uint32_t bytes = (uint32_t)(Sh::PADM * sizeof(cplx));
+    mbar_expect_tx(mbar_g, 2 * bytes);
+    const cplx* g = P4.Gp[s];
+    bulk_g2s(smem_u32(ZE.p), g, bytes, mbar_g);
+    bulk_g2s(smem_u32(ZO.p), g + Sh::PADM, bytes, mbar_g);
+  };
+
+  long long b = blockIdx.x;
+  int s = 0;
+  bool have = b < P.B;
+  uint32_t par_rows = 0, par_g = 0;
+  bool staged = false;
+  if (have) {
+    const double *dr, *hr; int nn;
+    staged = rows(b, s, dr, hr, nn);
+    if (tid == 0) { prefetch_rows(b, s); prefetch_g(s); }
+  }
+  double tot0 = 0.0, tot1 = 0.0;
+  while (have) {
+    long long nb = b; int ns = s + 1;
+    if (ns == P.n_seg) { ns = 0; nb = b + gridDim.x; }
+    const bool have_next = (MODE != MODE_STOREZ || nb == b) && nb < P.B;
+    const SegDev sg = P.segs[s];
+    // ---------------- forward pass 1 (radix RF1, stride 256): both branches from one set of inputs
+    {
+      constexpr int NTASK = NF / RF1;  // 256
+      constexpr int IT = NTASK / NT;
+      static_assert(NTASK % NT == 0, "first pass tiling");
+      if (staged) {
+        mbar_wait(mbar_rows, par_rows);
+        par_rows ^= 1;
+        cplx xs[IT][RF1];
+#pragma unroll
+        for (int it = 0; it < IT; ++it) first_pass_load_staged<RF1, NF, MODE>(xs[it], tid + it * NT, stH, stD, sg.n);
+        __syncthreads();  // staging consumed: the U region may now be overwritten
+#pragma unroll
+        for (int it = 0; it < IT; ++it) first_pass_compute<RF1, NF>(UE, UO, tid + it * NT, xs[it], tw);
+      } else {
+        const double *drow, *hrow; int n;
+        rows(b, s, drow, hrow, n);
+        const bool vec = ((reinterpret_cast<uintptr_t>(drow) | reinterpret_cast<uintptr_t>(hrow)) & 15) == 0;
+#pragma unroll 1
+        for (int g = tid; g < NTASK; g += NT) first_pass_c<RF1, NF, MODE>(UE, UO, g, drow, hrow, n, vec, tw);
+      }
+    }
+    __syncthreads();
+    // ---------------- forward passes 2 and 3, warp-local (this warp owns blocks s1 = 2wb, 2wb+1 of its branch)
+    {
+      cplx x[16], w[16];
+      {
+        const int s1 = 2 * wb + (lane >> 4), j = lane & 15;
+        const int base = s1 * 256 + j;
+        tw_powers<16>(tw[j * (TW / 256)], w);
+#pragma unroll
+        for (int q = 0; q < 16; ++q) x[q] = U.ld(base + 16 * q);
+        fft_reg<16, false>(x);
+        static_for<0, 16>([&](auto t) {
+          constexpr int tt = decltype(t)::value;
+          cplx v = x[brevR<16>(tt)];
+          if constexpr (tt > 0) v = cmul(v, w[tt]);
+          U.st(base + 16 * tt, v);
+        });
+      }
+      __syncwarp();
+      {
+        const int base = (32 * wb + lane) * 16;
+#pragma unroll
+        for (int q = 0; q < 16; ++q) x[q] = U.ld(base + q);
+        fft_reg<16, false>(x);
+        static_for<0, 16>([&](auto t) { U.st(base + decltype(t)::value, x[brevR<16>(decltype(t)::value)]); });
+      }
+    }
+    __syncthreads();
+    // ---------------- mid: untangle (registers) x generator (in place in Z) -> first inverse pass
+    mbar_wait(mbar_g, par_g);
+    par_g ^= 1;
+    {
+      const int s1 = 4 * wb + (lane >> 3), s2 = lane & 7;
+      const int kap = s1 + RI1 * s2;  // forward low-part kappa = inverse block index tau
+      int kap2;
+      bool selfzero = false;
+      if (br == 0) { kap2 = (NF / 16 - kap) & (NF / 16 - 1); selfzero = (kap == 0); }
+      else         { kap2 = NF / 16 - 1 - kap; }
+      const int fb = ((kap & (RF1 - 1)) * 16 + kap / RF1) * 16;
+      const int fb2 = ((kap2 & (RF1 - 1)) * 16 + kap2 / RF1) * 16;
+      cplx u1[16], v2[16];
+#pragma unroll
+      for (int t = 0; t < 16; ++t) { u1[t] = U.ld(fb + t); v2[t] = U.ld(fb2 + t); }
+      const cplx basew = tw[2 * kap + br];  // w_2M^(2 kap + br)
+      // Xk[t] -> u1[t], Xm[t] -> v2[15 - t] slot reuse is awkward with the kappa = 0 mirror, so
+      // the pairs are formed into fresh arrays half at a time (even t, then odd t).
+      const int zb0 = (s1 * 16 + s2) * 16, zb1 = (s1 * 16 + s2 + 8) * 16;
+      static_for<0, 2>([&](auto par) {
+        constexpr int pp = decltype(par)::value;  // 0: even t -> inverse block tau; 1: odd t -> block tau + M/32
+        cplx e[16];
+        static_for<0, 8>([&](auto hh) {
+          constexpr int t = 2 * decltype(hh)::value + pp;
+          const cplx U1 = u1[t];
+          const cplx U2 = selfzero ? v2[(16 - t) & 15] : v2[15 - t];
+          const cplx A = mk(U1.x + U2.x, U1.y - U2.y);
+          const cplx Bv = mk(U1.y + U2.y, -(U1.x - U2.x));
+          const cplx wB = cmul(basew, mul_w32<t, false>(Bv));
+          e[decltype(hh)::value] = cadd(A, wB);      // 2 X_{kq},      entry s = t/2
+          e[8 + decltype(hh)::value] = csub(A, wB);  // 2 X_{NF + kq}, entry s = 8 + t/2
+        });
+        const int zb = pp ? zb1 : zb0;
+#pragma unroll
+        for (int q = 0; q < 16; ++q) e[q] = cmul(Z.ld(zb + q), e[q]);  // generator spectrum sits in Z
+        fft_reg<16, true>(e);
+        static_for<0, 16>([&](auto t) { Z.st(zb + decltype(t)::value, e[brevR<16>(decltype(t)::value)]); });
+      });
+    }
+    // the warp finishing mid last knows the U region is dead: it prefetches the next item's rows
+    __syncwarp();
+    if (lane == 0) {
+      const int old = atomicAdd(mid_count, 1);
+      if (old == NW - 1) {
+        *mid_count = 0;
+        if (have_next) prefetch_rows(nb, ns);
+      }
+    }
+    bool staged_next = false;
+    if (have_next) { const double *dr, *hr; int nn; staged_next = rows(nb, ns, dr, hr, nn); }
+    // ---------------- inverse pass 2 (L = 256), warp-local: blocks s1 = 4wb .. 4wb+3
+    {
+      cplx x[16], w[16];
+      const int j = lane & 15;
+      tw_powers<16>(tw[j * (TW / 256)], w);
+#pragma unroll
+      for (int it = 0; it < 2; ++it) {
+        const int s1 = 4 * wb + 2 * it + (lane >> 4);
+        const int base = s1 * 256 + j;
+        static_for<0, 16>([&](auto q) {
+          constexpr int qq = decltype(q)::value;
+          cplx v = Z.ld(base + 16 * qq);
+          if constexpr (qq > 0) v = cmulc(v, w[qq]);
+          x[qq] = v;
+        });
+        fft_reg<16, true>(x);
+        static_for<0, 16>([&](auto t) { Z.st(base + 16 * decltype(t)::value, x[brevR<16>(decltype(t)::value)]); });
+      }
+    }
+    __syncthreads();
+    // ---------------- last inverse pass (radix RI1, joins the branches) + pruned radix-2 stage + S5
+    double acc0 = 0.0, acc1 = 0.0;
+#pragma unroll 1
+    for (int g = tid; g < M / RI1; g += NT) last_pass_c<RI1, M, MODE>(ZE, ZO, g, sg.n, tw, sg.zd, acc0, acc1);
+    if (MODE != MODE_STOREZ) {
+      acc0 = warp_sum(acc0);
+      acc1 = warp_sum(acc1);
+      if (lane == 0) { red[2 * warp] = acc0; red[2 * warp + 1] = acc1; }
+    }
+    __syncthreads();  // Z fully consumed
+    if (tid == 0) {
+      if (have_next) prefetch_g(ns);
+      if (MODE != MODE_STOREZ) {
+#pragma unroll
+        for (int wq = 0; wq < NW; ++wq) { tot0 += red[2 * wq]; tot1 += red[2 * wq + 1]; }
+        if (s == P.n_seg - 1) {
+          if (MODE == MODE_LOGLIKE) {
+            const double v = -0.5 * tot1;
+            P.out0[b] = P.accumulate ? P.out0[b] + v : v;
+          } else {
+            if (P.out0) P.out0[b] = P.accumulate ? P.out0[b] + tot0 : tot0;
+            if (P.out1) P.out1[b] = P.accumulate ? P.out1[b] + tot1 : tot1;
+          }
+          tot0 = 0.0; tot1 = 0.0;
+        }
+      }
+    }
+    b = nb; s = ns; have = have_next; staged = staged_next;
+  }
+}
+
+}  // namespace td

@@ -95,12 +95,16 @@ __global__ void gen_pack_kernel(const double* __restrict__ a, int n, cplx* g, in
 
 // F = DIF transform of g (length 2M, bins at plan_pos(q, 2M)).  G[br][plan_pos(k', M)] =
 // conj(F[2k'+br]) * scale : generator spectrum split into even/odd bins in DIT input order.
-__global__ void gen_permute_kernel(const cplx* __restrict__ F, cplx* G, int M, double scale) {
+// padded != 0: each branch is written in the padded shared-memory layout (element i at i + i/16,
+// branch stride padded(M)) so that one bulk copy drops it into the fused kernel's Z region.
+__global__ void gen_permute_kernel(const cplx* __restrict__ F, cplx* G, int M, double scale, int padded) {
   const int idx = blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= 2 * M) return;
   const int br = idx / M, kq = idx - br * M;
   const cplx f = F[plan_pos(2 * kq + br, 2 * M)];
-  G[(size_t)br * M + plan_pos(kq, M)] = mk(f.x * scale, -f.y * scale);
+  const int p = plan_pos(kq, M);
+  const size_t dst = padded ? (size_t)br * SmemArr::padded(M) + p + (p >> 4) : (size_t)br * M + p;
+  G[dst] = mk(f.x * scale, -f.y * scale);
 }
 
 }  // namespace td

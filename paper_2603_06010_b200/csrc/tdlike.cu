@@ -13,6 +13,7 @@
 
 #include "td_dense.cuh"
 #include "td_fused.cuh"
+#include "td_fused4.cuh"
 #include "td_setup.cuh"
 #include "td_staged.cuh"
 
@@ -32,6 +33,7 @@ struct SegHost {
   double v = 0.0, logdet = 0.0;
   double* a = nullptr;  // device [n]
   cplx* G = nullptr;    // device [2][M]
+  cplx* Gp = nullptr;   // device [2][padded(M)], padded Z layout (fused4 classes only)
   cplx* zd = nullptr;   // device [M] (lazy)
 };
 
@@ -40,6 +42,7 @@ struct ClassInfo {
   cplx* T = nullptr;            // device [2M]
   std::vector<int> seg_ids;
   SegDev* d_segs = nullptr;     // device [seg_ids.size()]
+  const cplx** d_Gp = nullptr;  // device [seg_ids.size()] (fused4 classes only)
 };
 
 struct DevGuard {
@@ -89,8 +92,8 @@ int next_log2(int n) { int l = 0; while ((1 << l) < n) ++l; return l; }
 
 void free_handle(td_handle* h) {
   if (!h) return;
-  for (auto& s : h->segs) { cudaFree(s.a); cudaFree(s.G); cudaFree(s.zd); }
-  for (auto& c : h->classes) { cudaFree(c.T); cudaFree(c.d_segs); }
+  for (auto& s : h->segs) { cudaFree(s.a); cudaFree(s.G); cudaFree(s.Gp); cudaFree(s.zd); }
+  for (auto& c : h->classes) { cudaFree(c.T); cudaFree(c.d_segs); cudaFree(c.d_Gp); }
   cudaFree(h->wsU); cudaFree(h->wsZ); cudaFree(h->wsPartial);
   dense_free(h->dense);
   cudaFree(h->hsD); cudaFree(h->hsH[0]); cudaFree(h->hsH[1]); cudaFree(h->hsOut);
@@ -236,6 +239,25 @@ td_status launch_fused_nt(td_handle* h, const FusedParams& P, cudaStream_t st) {
 }
 
 template <int LOG2M, int MODE>
+td_status launch_fused4(td_handle* h, const FusedParams& P, const cplx* const* Gp, cudaStream_t st) {
+  auto kern = td_fused4_kernel<LOG2M, MODE>;
+  constexpr int NT = Fused4Shape<LOG2M>::NT;
+  const size_t smem = Fused4Shape<LOG2M>::smem_bytes();
+  CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  int nb = 0;
+  CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kern, NT, smem));
+  if (nb < 1) return TD_EUNSUPPORTED;
+  const long long maxg = (long long)nb * h->num_sms;
+  const int grid = (int)std::max<long long>(1, std::min<long long>(MODE == MODE_STOREZ ? 1 : P.B, maxg));
+  Fused4Params P4;
+  P4.base = P; P4.Gp = Gp;
+  kern<<<grid, NT, smem, st>>>(P4);
+  CK(cudaGetLastError());
+  ++h->last_launches;
+  return TD_OK;
+}
+
+template <int LOG2M, int MODE>
 td_status launch_fused_t(td_handle* h, const FusedParams& P, cudaStream_t st) {
   if constexpr (LOG2M == 12 && MODE == MODE_LOGLIKE) {  // experiment knobs (headline shape only)
     static const int nt = getenv("TDLIKE_NT") ? atoi(getenv("TDLIKE_NT")) : 256;
@@ -247,7 +269,16 @@ td_status launch_fused_t(td_handle* h, const FusedParams& P, cudaStream_t st) {
 }
 
 template <int MODE>
-td_status launch_fused(td_handle* h, int log2M, const FusedParams& P, cudaStream_t st) {
+td_status launch_fused(td_handle* h, int log2M, const FusedParams& P, const cplx* const* Gp, cudaStream_t st) {
+  static const int v3 = getenv("TDLIKE_FUSED") ? atoi(getenv("TDLIKE_FUSED")) == 3 : 0;
+  if (!v3 && Gp) {
+    switch (log2M) {
+      case 10: return launch_fused4<10, MODE>(h, P, Gp, st);
+      case 11: return launch_fused4<11, MODE>(h, P, Gp, st);
+      case 12: return launch_fused4<12, MODE>(h, P, Gp, st);
+      default: break;
+    }
+  }
   switch (log2M) {
     case 8: return launch_fused_t<8, MODE>(h, P, st);
     case 9: return launch_fused_t<9, MODE>(h, P, st);
@@ -274,7 +305,7 @@ td_status run_fft_path(td_handle* h, const double* d, const double* H, int64_t l
       FusedParams P;
       P.d = d; P.H = H; P.ldh = ldh; P.B = B; P.out0 = out0; P.out1 = out1;
       P.segs = cls.d_segs; P.n_seg = (int)cls.seg_ids.size(); P.accumulate = accumulate; P.T = cls.T;
-      td_status s = launch_fused<MODE>(h, cls.log2M, P, st);
+      td_status s = launch_fused<MODE>(h, cls.log2M, P, cls.d_Gp, st);
       if (s != TD_OK) return s;
       accumulate = 1;
     } else {
@@ -365,7 +396,7 @@ static td_status create_impl(td_handle* h, const double* acf, const int64_t* seg
     tw_table_kernel<<<(TW + 255) / 256, 256>>>(c.T, TW);
     CK(cudaGetLastError());
   }
-  // ---- generator spectra: G = conj(FFT_2M(a - i b)) / (2M sqrt(v)), split even/odd, DIT order
+  // ---- generator spectra: G = conj(FFT_2M(a - i b)) / (4M sqrt(v)), split even/odd, DIT order
   for (ClassInfo& c : h->classes) {
     const int M = 1 << c.log2M, n2 = 2 * M;
     cplx* F = nullptr;
@@ -378,7 +409,14 @@ static td_status create_impl(td_handle* h, const double* acf, const int64_t* seg
       int launches = 0;
       st = staged_forward(F, 1, n2, 0, c.T, n2, 0, &launches);
       if (st != TD_OK) break;
-      gen_permute_kernel<<<(n2 + 255) / 256, 256>>>(F, sg.G, M, 1.0 / ((double)n2 * std::sqrt(sg.v)));
+      const double gscale = 0.5 / ((double)n2 * std::sqrt(sg.v));
+      gen_permute_kernel<<<(n2 + 255) / 256, 256>>>(F, sg.G, M, gscale, 0);
+      if (c.log2M >= 10 && c.log2M <= FUSED_MAX_LOG2M) {
+        const size_t pb = sizeof(cplx) * 2 * SmemArr::padded(M);
+        if (cudaMalloc(&sg.Gp, pb) != cudaSuccess) { st = TD_ENOMEM; break; }
+        cudaMemsetAsync(sg.Gp, 0, pb, 0);
+        gen_permute_kernel<<<(n2 + 255) / 256, 256>>>(F, sg.Gp, M, gscale, 1);
+      }
       if (cudaGetLastError() != cudaSuccess) { st = TD_ECUDA; break; }
     }
     cudaError_t e = cudaDeviceSynchronize();
@@ -392,6 +430,12 @@ static td_status create_impl(td_handle* h, const double* acf, const int64_t* seg
     }
     CK(cudaMalloc(&c.d_segs, sizeof(SegDev) * sd.size()));
     CK(cudaMemcpy(c.d_segs, sd.data(), sizeof(SegDev) * sd.size(), cudaMemcpyHostToDevice));
+    if (c.log2M >= 10 && c.log2M <= FUSED_MAX_LOG2M) {
+      std::vector<const cplx*> gp(c.seg_ids.size());
+      for (size_t i = 0; i < gp.size(); ++i) gp[i] = h->segs[c.seg_ids[i]].Gp;
+      CK(cudaMalloc(&c.d_Gp, sizeof(cplx*) * gp.size()));
+      CK(cudaMemcpy(c.d_Gp, gp.data(), sizeof(cplx*) * gp.size(), cudaMemcpyHostToDevice));
+    }
   }
   return TD_OK;
 }
