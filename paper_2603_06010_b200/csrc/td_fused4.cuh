@@ -146,11 +146,19 @@ __global__ void __launch_bounds__(Fused4Shape<LOG2M>::NT, 1) td_fused4_kernel(co
       }
       __syncwarp();
       {
-        const int base = (32 * wb + lane) * 16;
+        // pass 3 (L = 16).  Lane -> block (s1', s2') with s2' = (l & 15) ^ ((l & 1) << 3): both the
+        // loads (block s1'*16 + s2') and the stores are bank-conflict free.  The result block is
+        // stored at the warp-owned slot s1'*16 + (s2' >> 1) + 8 (s2' & 1) ("mid layout": the 8 blocks
+        // one quarter-warp of mid reads are consecutive), hence all loads precede all stores.
+        const int s1p = 2 * wb + (lane >> 4);
+        const int s2p = (lane & 15) ^ ((lane & 1) << 3);
+        const int src = (s1p * 16 + s2p) * 16;
+        const int dst = (s1p * 16 + (s2p >> 1) + 8 * (s2p & 1)) * 16;
 #pragma unroll
-        for (int q = 0; q < 16; ++q) x[q] = U.ld(base + q);
+        for (int q = 0; q < 16; ++q) x[q] = U.ld(src + q);
+        __syncwarp();
         fft_reg<16, false>(x);
-        static_for<0, 16>([&](auto t) { U.st(base + decltype(t)::value, x[brevR<16>(decltype(t)::value)]); });
+        static_for<0, 16>([&](auto t) { U.st(dst + decltype(t)::value, x[brevR<16>(decltype(t)::value)]); });
       }
     }
     __syncthreads();
@@ -164,31 +172,31 @@ __global__ void __launch_bounds__(Fused4Shape<LOG2M>::NT, 1) td_fused4_kernel(co
       bool selfzero = false;
       if (br == 0) { kap2 = (NF / 16 - kap) & (NF / 16 - 1); selfzero = (kap == 0); }
       else         { kap2 = NF / 16 - 1 - kap; }
-      const int fb = ((kap & (RF1 - 1)) * 16 + kap / RF1) * 16;
-      const int fb2 = ((kap2 & (RF1 - 1)) * 16 + kap2 / RF1) * 16;
-      cplx u1[16], v2[16];
-#pragma unroll
-      for (int t = 0; t < 16; ++t) { u1[t] = U.ld(fb + t); v2[t] = U.ld(fb2 + t); }
+      // U blocks in the "mid layout" written by forward pass 3
+      auto slot = [](int k) { const int a = k & (RF1 - 1), c = k / RF1; return (a * 16 + (c >> 1) + 8 * (c & 1)) * 16; };
+      const int fb = slot(kap), fb2 = slot(kap2);
       const cplx basew = tw[2 * kap + br];  // w_2M^(2 kap + br)
-      // Xk[t] -> u1[t], Xm[t] -> v2[15 - t] slot reuse is awkward with the kappa = 0 mirror, so
-      // the pairs are formed into fresh arrays half at a time (even t, then odd t).
-      const int zb0 = (s1 * 16 + s2) * 16, zb1 = (s1 * 16 + s2 + 8) * 16;
+      const int zb0 = (s1 * 16 + s2) * 16;
       static_for<0, 2>([&](auto par) {
         constexpr int pp = decltype(par)::value;  // 0: even t -> inverse block tau; 1: odd t -> block tau + M/32
-        cplx e[16];
+        const int zb = zb0 + pp * 8 * 16;
+        cplx ua[8], ub[8], e[16];
         static_for<0, 8>([&](auto hh) {
           constexpr int t = 2 * decltype(hh)::value + pp;
-          const cplx U1 = u1[t];
-          const cplx U2 = selfzero ? v2[(16 - t) & 15] : v2[15 - t];
+          ua[decltype(hh)::value] = U.ld(fb + t);
+          ub[decltype(hh)::value] = U.ld(fb2 + (selfzero ? ((16 - t) & 15) : (15 - t)));
+        });
+#pragma unroll
+        for (int q = 0; q < 16; ++q) e[q] = Z.ld(zb + q);  // generator spectrum sits in Z
+        static_for<0, 8>([&](auto hh) {
+          constexpr int h8 = decltype(hh)::value, t = 2 * h8 + pp;
+          const cplx U1 = ua[h8], U2 = ub[h8];
           const cplx A = mk(U1.x + U2.x, U1.y - U2.y);
           const cplx Bv = mk(U1.y + U2.y, -(U1.x - U2.x));
           const cplx wB = cmul(basew, mul_w32<t, false>(Bv));
-          e[decltype(hh)::value] = cadd(A, wB);      // 2 X_{kq},      entry s = t/2
-          e[8 + decltype(hh)::value] = csub(A, wB);  // 2 X_{NF + kq}, entry s = 8 + t/2
+          e[h8] = cmul(e[h8], cadd(A, wB));          // G * 2 X_{kq},      entry s = t/2
+          e[8 + h8] = cmul(e[8 + h8], csub(A, wB));  // G * 2 X_{NF + kq}, entry s = 8 + t/2
         });
-        const int zb = pp ? zb1 : zb0;
-#pragma unroll
-        for (int q = 0; q < 16; ++q) e[q] = cmul(Z.ld(zb + q), e[q]);  // generator spectrum sits in Z
         fft_reg<16, true>(e);
         static_for<0, 16>([&](auto t) { Z.st(zb + decltype(t)::value, e[brevR<16>(decltype(t)::value)]); });
       });
@@ -209,19 +217,18 @@ __global__ void __launch_bounds__(Fused4Shape<LOG2M>::NT, 1) td_fused4_kernel(co
       cplx x[16], w[16];
       const int j = lane & 15;
       tw_powers<16>(tw[j * (TW / 256)], w);
-#pragma unroll
-      for (int it = 0; it < 2; ++it) {
-        const int s1 = 4 * wb + 2 * it + (lane >> 4);
-        const int base = s1 * 256 + j;
-        static_for<0, 16>([&](auto q) {
-          constexpr int qq = decltype(q)::value;
-          cplx v = Z.ld(base + 16 * qq);
-          if constexpr (qq > 0) v = cmulc(v, w[qq]);
-          x[qq] = v;
-        });
-        fft_reg<16, true>(x);
-        static_for<0, 16>([&](auto t) { Z.st(base + 16 * decltype(t)::value, x[brevR<16>(decltype(t)::value)]); });
-      }
+      cplx y[16];
+      const int base0 = (4 * wb + (lane >> 4)) * 256 + j, base1 = base0 + 2 * 256;
+      static_for<0, 16>([&](auto q) {
+        constexpr int qq = decltype(q)::value;
+        cplx a = Z.ld(base0 + 16 * qq), c = Z.ld(base1 + 16 * qq);
+        if constexpr (qq > 0) { a = cmulc(a, w[qq]); c = cmulc(c, w[qq]); }
+        x[qq] = a; y[qq] = c;
+      });
+      fft_reg<16, true>(x);
+      static_for<0, 16>([&](auto t) { Z.st(base0 + 16 * decltype(t)::value, x[brevR<16>(decltype(t)::value)]); });
+      fft_reg<16, true>(y);
+      static_for<0, 16>([&](auto t) { Z.st(base1 + 16 * decltype(t)::value, y[brevR<16>(decltype(t)::value)]); });
     }
     __syncthreads();
     // ---------------- last inverse pass (radix RI1, joins the branches) + pruned radix-2 stage + S5
