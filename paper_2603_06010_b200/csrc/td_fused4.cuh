@@ -36,6 +36,107 @@ struct Fused4Params {
   const cplx* const* Gp;  // device array [n_seg]: generator spectrum in the PADDED Z layout [2][padded(M)]
 };
 
+// ---- pieces shared by the one-CTA kernel below and the 2-CTA cluster kernel (td_cluster.cuh) -------
+// All three work on ONE branch (U, Z of that branch); wb = index of the warp within the branch,
+// TW = 2M, RF1 = first forward radix (forward blocks of 256: RF1 per branch), RI1 = 2 RF1.
+
+// forward passes 2 and 3, warp-local (this warp owns blocks s1 = 2wb, 2wb+1 of its branch)
+template <int TW>
+__device__ __forceinline__ void f4_forward23(const SmemArr& U, int wb, int lane, const cplx* __restrict__ tw) {
+  cplx x[16], w[16];
+  {
+    const int s1 = 2 * wb + (lane >> 4), j = lane & 15;
+    const int base = s1 * 256 + j;
+    tw_powers<16>(tw[j * (TW / 256)], w);
+#pragma unroll
+    for (int q = 0; q < 16; ++q) x[q] = U.ld(base + 16 * q);
+    fft_reg<16, false>(x);
+    static_for<0, 16>([&](auto t) {
+      constexpr int tt = decltype(t)::value;
+      cplx v = x[brevR<16>(tt)];
+      if constexpr (tt > 0) v = cmul(v, w[tt]);
+      U.st(base + 16 * tt, v);
+    });
+  }
+  __syncwarp();
+  {
+    // pass 3 (L = 16).  Lane -> block (s1', s2') with s2' = (l & 15) ^ ((l & 1) << 3): both the
+    // loads (block s1'*16 + s2') and the stores are bank-conflict free.  The result block is
+    // stored at the warp-owned slot s1'*16 + (s2' >> 1) + 8 (s2' & 1) ("mid layout": the 8 blocks
+    // one quarter-warp of mid reads are consecutive), hence all loads precede all stores.
+    const int s1p = 2 * wb + (lane >> 4);
+    const int s2p = (lane & 15) ^ ((lane & 1) << 3);
+    const int src = (s1p * 16 + s2p) * 16;
+    const int dst = (s1p * 16 + (s2p >> 1) + 8 * (s2p & 1)) * 16;
+#pragma unroll
+    for (int q = 0; q < 16; ++q) x[q] = U.ld(src + q);
+    __syncwarp();
+    fft_reg<16, false>(x);
+    static_for<0, 16>([&](auto t) { U.st(dst + decltype(t)::value, x[brevR<16>(decltype(t)::value)]); });
+  }
+}
+
+// mid: untangle (registers) x generator (in place in Z) -> first inverse pass
+template <int NF, int RF1>
+__device__ __forceinline__ void f4_mid(const SmemArr& U, const SmemArr& Z, int br, int wb, int lane,
+                                       const cplx* __restrict__ tw) {
+  constexpr int RI1 = 2 * RF1;
+  const int s1 = 4 * wb + (lane >> 3), s2 = lane & 7;
+  const int kap = s1 + RI1 * s2;  // forward low-part kappa = inverse block index tau
+  int kap2;
+  bool selfzero = false;
+  if (br == 0) { kap2 = (NF / 16 - kap) & (NF / 16 - 1); selfzero = (kap == 0); }
+  else         { kap2 = NF / 16 - 1 - kap; }
+  // U blocks in the "mid layout" written by forward pass 3
+  auto slot = [](int k) { const int a = k & (RF1 - 1), c = k / RF1; return (a * 16 + (c >> 1) + 8 * (c & 1)) * 16; };
+  const int fb = slot(kap), fb2 = slot(kap2);
+  const cplx basew = tw[2 * kap + br];  // w_2M^(2 kap + br)
+  const int zb0 = (s1 * 16 + s2) * 16;
+  static_for<0, 2>([&](auto par) {
+    constexpr int pp = decltype(par)::value;  // 0: even t -> inverse block tau; 1: odd t -> block tau + M/32
+    const int zb = zb0 + pp * 8 * 16;
+    cplx ua[8], ub[8], e[16];
+    static_for<0, 8>([&](auto hh) {
+      constexpr int t = 2 * decltype(hh)::value + pp;
+      ua[decltype(hh)::value] = U.ld(fb + t);
+      ub[decltype(hh)::value] = U.ld(fb2 + (selfzero ? ((16 - t) & 15) : (15 - t)));
+    });
+#pragma unroll
+    for (int q = 0; q < 16; ++q) e[q] = Z.ld(zb + q);  // generator spectrum sits in Z
+    static_for<0, 8>([&](auto hh) {
+      constexpr int h8 = decltype(hh)::value, t = 2 * h8 + pp;
+      const cplx U1 = ua[h8], U2 = ub[h8];
+      const cplx A = mk(U1.x + U2.x, U1.y - U2.y);
+      const cplx Bv = mk(U1.y + U2.y, -(U1.x - U2.x));
+      const cplx wB = cmul(basew, mul_w32<t, false>(Bv));
+      e[h8] = cmul(e[h8], cadd(A, wB));          // G * 2 X_{kq},      entry s = t/2
+      e[8 + h8] = cmul(e[8 + h8], csub(A, wB));  // G * 2 X_{NF + kq}, entry s = 8 + t/2
+    });
+    fft_reg<16, true>(e);
+    static_for<0, 16>([&](auto t) { Z.st(zb + decltype(t)::value, e[brevR<16>(decltype(t)::value)]); });
+  });
+}
+
+// inverse pass 2 (L = 256), warp-local: blocks s1 = 4wb .. 4wb+3
+template <int TW>
+__device__ __forceinline__ void f4_inverse2(const SmemArr& Z, int wb, int lane, const cplx* __restrict__ tw) {
+  cplx x[16], w[16];
+  const int j = lane & 15;
+  tw_powers<16>(tw[j * (TW / 256)], w);
+  cplx y[16];
+  const int base0 = (4 * wb + (lane >> 4)) * 256 + j, base1 = base0 + 2 * 256;
+  static_for<0, 16>([&](auto q) {
+    constexpr int qq = decltype(q)::value;
+    cplx a = Z.ld(base0 + 16 * qq), c = Z.ld(base1 + 16 * qq);
+    if constexpr (qq > 0) { a = cmulc(a, w[qq]); c = cmulc(c, w[qq]); }
+    x[qq] = a; y[qq] = c;
+  });
+  fft_reg<16, true>(x);
+  static_for<0, 16>([&](auto t) { Z.st(base0 + 16 * decltype(t)::value, x[brevR<16>(decltype(t)::value)]); });
+  fft_reg<16, true>(y);
+  static_for<0, 16>([&](auto t) { Z.st(base1 + 16 * decltype(t)::value, y[brevR<16>(decltype(t)::value)]); });
+}
+
 template <int LOG2M, int MODE>
 __global__ void __launch_bounds__(Fused4Shape<LOG2M>::NT, 1) td_fused4_kernel(const Fused4Params P4) {
   using Sh = Fused4Shape<LOG2M>;
@@ -127,80 +228,13 @@ __global__ void __launch_bounds__(Fused4Shape<LOG2M>::NT, 1) td_fused4_kernel(co
       }
     }
     __syncthreads();
-    // ---------------- forward passes 2 and 3, warp-local (this warp owns blocks s1 = 2wb, 2wb+1 of its branch)
-    {
-      cplx x[16], w[16];
-      {
-        const int s1 = 2 * wb + (lane >> 4), j = lane & 15;
-        const int base = s1 * 256 + j;
-        tw_powers<16>(tw[j * (TW / 256)], w);
-#pragma unroll
-        for (int q = 0; q < 16; ++q) x[q] = U.ld(base + 16 * q);
-        fft_reg<16, false>(x);
-        static_for<0, 16>([&](auto t) {
-          constexpr int tt = decltype(t)::value;
-          cplx v = x[brevR<16>(tt)];
-          if constexpr (tt > 0) v = cmul(v, w[tt]);
-          U.st(base + 16 * tt, v);
-        });
-      }
-      __syncwarp();
-      {
-        // pass 3 (L = 16).  Lane -> block (s1', s2') with s2' = (l & 15) ^ ((l & 1) << 3): both the
-        // loads (block s1'*16 + s2') and the stores are bank-conflict free.  The result block is
-        // stored at the warp-owned slot s1'*16 + (s2' >> 1) + 8 (s2' & 1) ("mid layout": the 8 blocks
-        // one quarter-warp of mid reads are consecutive), hence all loads precede all stores.
-        const int s1p = 2 * wb + (lane >> 4);
-        const int s2p = (lane & 15) ^ ((lane & 1) << 3);
-        const int src = (s1p * 16 + s2p) * 16;
-        const int dst = (s1p * 16 + (s2p >> 1) + 8 * (s2p & 1)) * 16;
-#pragma unroll
-        for (int q = 0; q < 16; ++q) x[q] = U.ld(src + q);
-        __syncwarp();
-        fft_reg<16, false>(x);
-        static_for<0, 16>([&](auto t) { U.st(dst + decltype(t)::value, x[brevR<16>(decltype(t)::value)]); });
-      }
-    }
+    // ---------------- forward passes 2 and 3, warp-local
+    f4_forward23<TW>(U, wb, lane, tw);
     __syncthreads();
     // ---------------- mid: untangle (registers) x generator (in place in Z) -> first inverse pass
     mbar_wait(mbar_g, par_g);
     par_g ^= 1;
-    {
-      const int s1 = 4 * wb + (lane >> 3), s2 = lane & 7;
-      const int kap = s1 + RI1 * s2;  // forward low-part kappa = inverse block index tau
-      int kap2;
-      bool selfzero = false;
-      if (br == 0) { kap2 = (NF / 16 - kap) & (NF / 16 - 1); selfzero = (kap == 0); }
-      else         { kap2 = NF / 16 - 1 - kap; }
-      // U blocks in the "mid layout" written by forward pass 3
-      auto slot = [](int k) { const int a = k & (RF1 - 1), c = k / RF1; return (a * 16 + (c >> 1) + 8 * (c & 1)) * 16; };
-      const int fb = slot(kap), fb2 = slot(kap2);
-      const cplx basew = tw[2 * kap + br];  // w_2M^(2 kap + br)
-      const int zb0 = (s1 * 16 + s2) * 16;
-      static_for<0, 2>([&](auto par) {
-        constexpr int pp = decltype(par)::value;  // 0: even t -> inverse block tau; 1: odd t -> block tau + M/32
-        const int zb = zb0 + pp * 8 * 16;
-        cplx ua[8], ub[8], e[16];
-        static_for<0, 8>([&](auto hh) {
-          constexpr int t = 2 * decltype(hh)::value + pp;
-          ua[decltype(hh)::value] = U.ld(fb + t);
-          ub[decltype(hh)::value] = U.ld(fb2 + (selfzero ? ((16 - t) & 15) : (15 - t)));
-        });
-#pragma unroll
-        for (int q = 0; q < 16; ++q) e[q] = Z.ld(zb + q);  // generator spectrum sits in Z
-        static_for<0, 8>([&](auto hh) {
-          constexpr int h8 = decltype(hh)::value, t = 2 * h8 + pp;
-          const cplx U1 = ua[h8], U2 = ub[h8];
-          const cplx A = mk(U1.x + U2.x, U1.y - U2.y);
-          const cplx Bv = mk(U1.y + U2.y, -(U1.x - U2.x));
-          const cplx wB = cmul(basew, mul_w32<t, false>(Bv));
-          e[h8] = cmul(e[h8], cadd(A, wB));          // G * 2 X_{kq},      entry s = t/2
-          e[8 + h8] = cmul(e[8 + h8], csub(A, wB));  // G * 2 X_{NF + kq}, entry s = 8 + t/2
-        });
-        fft_reg<16, true>(e);
-        static_for<0, 16>([&](auto t) { Z.st(zb + decltype(t)::value, e[brevR<16>(decltype(t)::value)]); });
-      });
-    }
+    f4_mid<NF, RF1>(U, Z, br, wb, lane, tw);
     // the warp finishing mid last knows the U region is dead: it prefetches the next item's rows
     __syncwarp();
     if (lane == 0) {
@@ -212,24 +246,8 @@ __global__ void __launch_bounds__(Fused4Shape<LOG2M>::NT, 1) td_fused4_kernel(co
     }
     bool staged_next = false;
     if (have_next) { const double *dr, *hr; int nn; staged_next = rows(nb, ns, dr, hr, nn); }
-    // ---------------- inverse pass 2 (L = 256), warp-local: blocks s1 = 4wb .. 4wb+3
-    {
-      cplx x[16], w[16];
-      const int j = lane & 15;
-      tw_powers<16>(tw[j * (TW / 256)], w);
-      cplx y[16];
-      const int base0 = (4 * wb + (lane >> 4)) * 256 + j, base1 = base0 + 2 * 256;
-      static_for<0, 16>([&](auto q) {
-        constexpr int qq = decltype(q)::value;
-        cplx a = Z.ld(base0 + 16 * qq), c = Z.ld(base1 + 16 * qq);
-        if constexpr (qq > 0) { a = cmulc(a, w[qq]); c = cmulc(c, w[qq]); }
-        x[qq] = a; y[qq] = c;
-      });
-      fft_reg<16, true>(x);
-      static_for<0, 16>([&](auto t) { Z.st(base0 + 16 * decltype(t)::value, x[brevR<16>(decltype(t)::value)]); });
-      fft_reg<16, true>(y);
-      static_for<0, 16>([&](auto t) { Z.st(base1 + 16 * decltype(t)::value, y[brevR<16>(decltype(t)::value)]); });
-    }
+    // ---------------- inverse pass 2 (L = 256), warp-local
+    f4_inverse2<TW>(Z, wb, lane, tw);
     __syncthreads();
     // ---------------- last inverse pass (radix RI1, joins the branches) + pruned radix-2 stage + S5
     double acc0 = 0.0, acc1 = 0.0;

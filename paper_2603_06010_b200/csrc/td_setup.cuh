@@ -93,17 +93,19 @@ __global__ void gen_pack_kernel(const double* __restrict__ a, int n, cplx* g, in
   g[j] = v;
 }
 
-// F = DIF transform of g (length 2M, bins at plan_pos(q, 2M)).  G[br][plan_pos(k', M)] =
-// conj(F[2k'+br]) * scale : generator spectrum split into even/odd bins in DIT input order.
-// padded != 0: each branch is written in the padded shared-memory layout (element i at i + i/16,
-// branch stride padded(M)) so that one bulk copy drops it into the fused kernel's Z region.
-__global__ void gen_permute_kernel(const cplx* __restrict__ F, cplx* G, int M, double scale, int padded) {
+// F = DIF transform of g (length 2M, bins at plan_pos(q, 2M)).  G[br][pos(k')] = conj(F[2k'+br]) * scale :
+// generator spectrum split into even/odd bins in the inverse transform's input order.
+// layout 0: pos = plan_pos(k', M), branch stride M (td_fused.cuh, td_staged.cuh).
+// layout 1: same order in the padded shared-memory layout (element i at i + i/16, branch stride
+//           padded(M)) so that one bulk copy drops it into the fused4 kernel's Z region.
+// layout 2: padded, order of the cluster kernel's [32,16,16] inverse plan (td_cluster.cuh).
+__global__ void gen_permute_kernel(const cplx* __restrict__ F, cplx* G, int M, double scale, int layout) {
   const int idx = blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= 2 * M) return;
   const int br = idx / M, kq = idx - br * M;
   const cplx f = F[plan_pos(2 * kq + br, 2 * M)];
-  const int p = plan_pos(kq, M);
-  const size_t dst = padded ? (size_t)br * SmemArr::padded(M) + p + (p >> 4) : (size_t)br * M + p;
+  const int p = layout == 2 ? (((kq & 31) << 8) | (((kq >> 5) & 15) << 4) | (kq >> 9)) : plan_pos(kq, M);
+  const size_t dst = layout ? (size_t)br * SmemArr::padded(M) + p + (p >> 4) : (size_t)br * M + p;
   G[dst] = mk(f.x * scale, -f.y * scale);
 }
 

@@ -13,6 +13,7 @@
 
 #include "td_dense.cuh"
 #include "td_fused.cuh"
+#include "td_cluster.cuh"
 #include "td_fused4.cuh"
 #include "td_setup.cuh"
 #include "td_staged.cuh"
@@ -22,7 +23,8 @@ using namespace td;
 namespace {
 
 constexpr int FUSED_MIN_LOG2M = 8;   // M = 256
-constexpr int FUSED_MAX_LOG2M = 12;  // M = 4096 (2M = 8192-point transform, 204 KiB of shared memory)
+// one-CTA fused kernels: M = 256..4096 (2M = 8192-point transform, 204 KiB of shared memory at M = 4096)
+constexpr int CLUSTER_LOG2M = 13;    // M = 8192: 2-CTA cluster, one branch per CTA (td_cluster.cuh)
 constexpr int FUSED_NT = 256;
 constexpr size_t STAGED_WS_BYTES = 64ull << 20;  // keep the staged workspace L2-resident (126 MB L2)
 
@@ -257,6 +259,30 @@ td_status launch_fused4(td_handle* h, const FusedParams& P, const cplx* const* G
   return TD_OK;
 }
 
+template <int MODE>
+td_status launch_cluster(td_handle* h, const FusedParams& P, const cplx* const* Gp, cudaStream_t st) {
+  auto kern = td_cluster_kernel<MODE>;
+  const size_t smem = ClusterShape::smem_bytes();
+  CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  cudaLaunchConfig_t cfg = {};
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeClusterDimension;
+  attr[0].val.clusterDim.x = 2; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+  cfg.blockDim = dim3(ClusterShape::NT); cfg.dynamicSmemBytes = smem; cfg.stream = st;
+  cfg.attrs = attr; cfg.numAttrs = 1;
+  cfg.gridDim = dim3(2 * (h->num_sms / 2));
+  int ncl = 0;
+  CK(cudaOccupancyMaxActiveClusters(&ncl, kern, &cfg));
+  if (ncl < 1) return TD_EUNSUPPORTED;
+  const long long want = MODE == MODE_STOREZ ? 1 : P.B;
+  cfg.gridDim = dim3(2 * (unsigned)std::max<long long>(1, std::min<long long>(want, ncl)));
+  Fused4Params P4;
+  P4.base = P; P4.Gp = Gp;
+  CK(cudaLaunchKernelEx(&cfg, kern, P4));
+  ++h->last_launches;
+  return TD_OK;
+}
+
 template <int LOG2M, int MODE>
 td_status launch_fused_t(td_handle* h, const FusedParams& P, cudaStream_t st) {
   if constexpr (LOG2M == 12 && MODE == MODE_LOGLIKE) {  // experiment knobs (headline shape only)
@@ -271,6 +297,7 @@ td_status launch_fused_t(td_handle* h, const FusedParams& P, cudaStream_t st) {
 template <int MODE>
 td_status launch_fused(td_handle* h, int log2M, const FusedParams& P, const cplx* const* Gp, cudaStream_t st) {
   static const int v3 = getenv("TDLIKE_FUSED") ? atoi(getenv("TDLIKE_FUSED")) == 3 : 0;
+  if (log2M == CLUSTER_LOG2M) return Gp ? launch_cluster<MODE>(h, P, Gp, st) : TD_EUNSUPPORTED;
   if (!v3 && Gp) {
     switch (log2M) {
       case 10: return launch_fused4<10, MODE>(h, P, Gp, st);
@@ -291,7 +318,7 @@ td_status launch_fused(td_handle* h, int log2M, const FusedParams& P, const cplx
 
 bool class_is_fused(const td_handle* h, const ClassInfo& c) {
   if (h->fft_variant == 2) return false;
-  return c.log2M >= FUSED_MIN_LOG2M && c.log2M <= FUSED_MAX_LOG2M;
+  return c.log2M >= FUSED_MIN_LOG2M && c.log2M <= CLUSTER_LOG2M;
 }
 
 // FFT path over all size classes.  MODE_LOGLIKE: out0 = loglike.  MODE_INNER: out0 = <d,h>, out1 = <h,h>.
@@ -411,11 +438,11 @@ static td_status create_impl(td_handle* h, const double* acf, const int64_t* seg
       if (st != TD_OK) break;
       const double gscale = 0.5 / ((double)n2 * std::sqrt(sg.v));
       gen_permute_kernel<<<(n2 + 255) / 256, 256>>>(F, sg.G, M, gscale, 0);
-      if (c.log2M >= 10 && c.log2M <= FUSED_MAX_LOG2M) {
+      if (c.log2M >= 10 && c.log2M <= CLUSTER_LOG2M) {
         const size_t pb = sizeof(cplx) * 2 * SmemArr::padded(M);
         if (cudaMalloc(&sg.Gp, pb) != cudaSuccess) { st = TD_ENOMEM; break; }
         cudaMemsetAsync(sg.Gp, 0, pb, 0);
-        gen_permute_kernel<<<(n2 + 255) / 256, 256>>>(F, sg.Gp, M, gscale, 1);
+        gen_permute_kernel<<<(n2 + 255) / 256, 256>>>(F, sg.Gp, M, gscale, c.log2M == CLUSTER_LOG2M ? 2 : 1);
       }
       if (cudaGetLastError() != cudaSuccess) { st = TD_ECUDA; break; }
     }
@@ -430,7 +457,7 @@ static td_status create_impl(td_handle* h, const double* acf, const int64_t* seg
     }
     CK(cudaMalloc(&c.d_segs, sizeof(SegDev) * sd.size()));
     CK(cudaMemcpy(c.d_segs, sd.data(), sizeof(SegDev) * sd.size(), cudaMemcpyHostToDevice));
-    if (c.log2M >= 10 && c.log2M <= FUSED_MAX_LOG2M) {
+    if (c.log2M >= 10 && c.log2M <= CLUSTER_LOG2M) {
       std::vector<const cplx*> gp(c.seg_ids.size());
       for (size_t i = 0; i < gp.size(); ++i) gp[i] = h->segs[c.seg_ids[i]].Gp;
       CK(cudaMalloc(&c.d_Gp, sizeof(cplx*) * gp.size()));

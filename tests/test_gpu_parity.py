@@ -94,6 +94,49 @@ def test_c4_long_segment_vs_library_levinson():
 
 
 # ------------------------------------------------------------------ shapes: ragged, tiny, mixed classes
+@pytest.mark.parametrize("n", [4097, 6001, 8192])
+def test_cluster_kernel_lengths(n):
+    """M = 8192: the 2-CTA cluster kernel (even, odd and unaligned rows; B not a multiple of the grid)."""
+    rng = np.random.default_rng(n)
+    rho = W.acf_from_psd(4096.0, 2 * 8192, n)
+    d = rng.standard_normal(n) * 1e-21
+    H = rng.standard_normal((5, n)) * 1e-21
+    ref = O.loglike_batch(rho, [n], d, H)
+    dh_ref, hh_ref = O.inner_batch(rho, [n], d, H)
+    with tdb.TDLikelihood(rho, [n]) as h:
+        dd, HH = _dev(d), _dev(H)
+        out = h.loglike_batch(dd, HH).cpu().numpy()
+        assert h.last_launches() == 1
+        dh, hh = h.inner_batch(dd, HH)
+        h.set_fft_variant(2)
+        out2 = h.loglike_batch(dd, HH).cpu().numpy()
+    _assert_close(out, ref, what=f"cluster n={n}")
+    _assert_close(out2, ref, what=f"staged n={n}")
+    scale = hh_ref + float(O.inner_batch(rho, [n], d, d[None, :])[1][0])
+    assert np.max(np.abs(dh.cpu().numpy() - dh_ref) / scale) <= TOL
+    assert np.max(np.abs(hh.cpu().numpy() - hh_ref) / np.abs(hh_ref)) <= TOL
+
+
+def test_cluster_many_templates_repeatable():
+    """More templates than clusters (74): every cluster loops; bitwise repeatable."""
+    w = W.make("c5", B=200, n_scale=1)
+    sub = slice(0, 8)
+    ref = O.loglike_batch(w.acf, w.seg_lengths, w.d, w.H[sub])
+    with tdb.TDLikelihood(w.acf, w.seg_lengths) as h:
+        d, H = _dev(w.d), _dev(w.H)
+        o1 = h.loglike_batch(d, H)
+        o2 = h.loglike_batch(d, H)
+        torch.cuda.synchronize()
+        assert h.last_launches() == 1
+    assert torch.equal(o1, o2)
+    _assert_close(o1.cpu().numpy()[sub], ref, what="c5 B=200")
+    # every other template: against the staged (global-memory) variant of the same library
+    with tdb.TDLikelihood(w.acf, w.seg_lengths) as h:
+        h.set_fft_variant(2)
+        o3 = h.loglike_batch(_dev(w.d), _dev(w.H)).cpu().numpy()
+    _assert_close(o1.cpu().numpy(), o3, tol=1e-11, what="cluster vs staged")
+
+
 @pytest.mark.parametrize("n", [1, 2, 3, 5, 31, 255, 256, 257, 777, 1000, 2049, 4095])
 def test_ragged_lengths(n):
     rng = np.random.default_rng(n)
