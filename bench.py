@@ -31,9 +31,12 @@ if ROOT not in sys.path:
 METRIC = "fp64 likelihood evals/sec"
 UNIT = "evals/s"
 # fp64 ALU roofline: 64 DFMA/clk/SM x 148 SMs x 1.965 GHz x 2 flop (guide unit counts and
-# clocks.max.sm; a register-resident DMMA m8n8k4 loop measured 37.15 TFLOP/s and a DFMA loop
-# 34.0 TFLOP/s on this pool - profiles/r01_peaks.md).  DESIGN.md "Rooflines".
+# clocks.max.sm); the register-loop DFMA / DMMA throughputs are measured in every run
+# (td_probe_fp64) and reported beside it.  DESIGN.md 6.
 FP64_PEAK_TFLOPS = 37.2
+# dominant kernel of a step, per config
+DOMINANT = {"c1": "td_fused4_kernel<10>", "c2": "td_fused4_kernel<12>", "c3": "td_cluster_kernel",
+            "c4": "staged lg_* kernels", "c5": "td_cluster_kernel"}
 
 
 def alg_flops_per_eval(seg_lengths) -> float:
@@ -159,6 +162,8 @@ def main():
     ap.add_argument("--fft-variant", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--probe-peaks", action="store_true",
+                    help="print the measured fp64 DFMA / DMMA / DADD register-loop throughputs and exit")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
@@ -179,6 +184,12 @@ def main():
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
     tdb.load(build_if_missing=False)
+    if args.probe_peaks:
+        if rank == 0:
+            names = {0: "dfma", 1: "dmma_m8n8k4", 2: "dfma_and_dmma_interleaved", 3: "dadd"}
+            print(json.dumps({"fp64_tflops": {names[k]: tdb.probe_fp64(k, local) for k in range(4)},
+                              "derived_peak": FP64_PEAK_TFLOPS}))
+        return
 
     w = W.make(args.config, B=args.B)
     B, n_tot = w.B, w.n_tot
@@ -268,7 +279,9 @@ def main():
     # ---------------- rooflines (dominant kernel = the one kernel of the step on the fused path)
     peaks, peaks_kind = measured_peaks()
     kern_ms = float(np.mean(step_ms))
-    falg = alg_flops_per_eval(w.seg_lengths)
+    dense = path_used == 2
+    falg = float(sum(2.0 * int(n) * int(n) for n in w.seg_lengths)) if dense else alg_flops_per_eval(w.seg_lengths)
+    probe = {"dfma": tdb.probe_fp64(0, local), "dmma": tdb.probe_fp64(1, local)}
     ach_tf = falg * B / (kern_ms * 1e-3) / 1e12
     ach_gbs = (8.0 * n_tot * B + 8.0 * B) / (kern_ms * 1e-3) / 1e9
     traffic = None
@@ -278,11 +291,13 @@ def main():
             traffic = json.load(open(tp)).get(args.config)
         except Exception:
             traffic = None
-    roofline = {"bound": "alu", "achieved": ach_tf, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
+    roofline = {"bound": "tensor" if dense else "alu", "achieved": ach_tf, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
                 "frac": ach_tf / FP64_PEAK_TFLOPS, "traffic": traffic,
-                "kernel": "td_fused_kernel" if path_used == 1 else "td_dense_kernel",
+                "kernel": "td_dense_kernel" if dense else DOMINANT.get(args.config, "td_fused_kernel"),
+                "measured_register_loop_tflops": probe,
                 "kernel_ms": kern_ms, "alg_flops_per_eval": falg,
-                "peak_source": "derived: 64 DFMA/clk/SM x 148 SM x 1.965 GHz x 2 (DESIGN.md); measured DMMA loop 37.15, DFMA loop 34.0"}
+                "peak_source": "derived: 64 DFMA/clk/SM x 148 SM x 1.965 GHz x 2 (DESIGN.md 6); the fp64 tensor pipe "
+                               "(DMMA.8x8x4) has the same peak; register-loop measurements of this run beside it"}
     roofline_hbm = {"bound": "hbm", "achieved": ach_gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s",
                     "frac": ach_gbs / peaks["hbm_gbs"], "peak_source": peaks_kind + " (MEASURED_PEAKS.json copy bandwidth)",
                     "alg_bytes_per_eval": 8.0 * n_tot + 8.0}

@@ -35,7 +35,9 @@ typedef enum {
   TD_EUNSUPPORTED = 5  /* valid request this build cannot serve (e.g. forced path too large)  */
 } td_status;
 
-/* td_path: evaluation path selector for td_set_path / reported by td_get_info. */
+/* td_path: evaluation path selector for td_set_path / reported by td_get_info.
+ * TD_PATH_AUTO: per size class, the dense path for short segments (measured crossover, DESIGN.md
+ * 6.4), the FFT path otherwise; both accumulate into the same outputs within one call. */
 enum { TD_PATH_AUTO = 0, TD_PATH_FFT = 1, TD_PATH_DENSE = 2 };
 
 /* td_create - one-time setup (PAPER.md:215 "done once ... cached"; :241-246 Eq. 14 generator).
@@ -108,7 +110,8 @@ td_status td_set_fft_variant(td_handle* h, int variant);
  *   n_seg      number of segments
  *   v          HOST array [n_seg]: prediction-error variance v_s = 1/(C_s^{-1})_{00}
  *   logdet     HOST array [n_seg]: log det C_s = sum_k log E_k
- *   last_path  TD_PATH_FFT or TD_PATH_DENSE actually used by the last batch call (0 if none yet)
+ *   last_path  path actually used by the last batch call (0 if none yet): TD_PATH_DENSE if every
+ *              segment went through the dense kernel, TD_PATH_FFT otherwise
  */
 td_status td_get_info(const td_handle* h, int64_t* n_tot, int* n_seg, double* v, double* logdet,
                       int* last_path);
@@ -120,6 +123,14 @@ td_status td_get_generator(const td_handle* h, int seg, double* a);
 /* td_last_launches - number of kernels of this library launched by the last batch call on
  * this handle (evidence for bench.py's gpu_launches). */
 int td_last_launches(const td_handle* h);
+
+/* td_probe_fp64 - measures the fp64 throughput of `device` with register-resident loops (no memory
+ * traffic), for the roofline denominators of bench.py:
+ *   kind 0  DFMA chains (vector fp64 pipe),   kind 1  mma.sync.m8n8k4.f64 chains (fp64 tensor pipe),
+ *   kind 2  both interleaved in the same warps,  kind 3  DADD chains (1 flop per instruction).
+ * tflops (HOST pointer) receives the best of 5 timed launches in TFLOP/s.  Synchronous; uses the
+ * legacy default stream.  Errors: TD_EINVAL, TD_ECUDA. */
+td_status td_probe_fp64(int kind, int device, double* tflops);
 
 /* td_strerror - static string for a status code. */
 const char* td_strerror(td_status s);

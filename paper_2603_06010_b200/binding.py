@@ -31,6 +31,7 @@ SYMBOLS = {
     "td_get_info": (_INT, [_VP, C.POINTER(C.c_int64), C.POINTER(_INT), _DP, _DP, C.POINTER(_INT)]),
     "td_get_generator": (_INT, [_VP, _INT, _DP]),
     "td_last_launches": (_INT, [_VP]),
+    "td_probe_fp64": (_INT, [_INT, _INT, _DP]),
     "td_strerror": (C.c_char_p, [_INT]),
 }
 
@@ -193,6 +194,13 @@ class TDLikelihood:
 
     def last_launches(self) -> int:
         return int(self._lib.td_last_launches(self._h))
+
+
+def probe_fp64(kind: int, device: int = 0) -> float:
+    """TFLOP/s of a register-resident fp64 loop (0 DFMA, 1 DMMA m8n8k4, 2 both, 3 DADD)."""
+    v = C.c_double()
+    _check(load().td_probe_fp64(int(kind), int(device), C.byref(v)), "td_probe_fp64")
+    return float(v.value)
 
 
 # C-named convenience wrappers -------------------------------------------------------------

@@ -9,6 +9,9 @@ namespace td {
 
 typedef double2 cplx;
 
+// what a batch kernel accumulates: -1/2 <d-h, d-h> | (<d,h>, <h,h>) | nothing (stores z of the data vector)
+enum { MODE_LOGLIKE = 0, MODE_INNER = 1, MODE_STOREZ = 2 };
+
 __host__ __device__ __forceinline__ cplx mk(double x, double y) { return make_double2(x, y); }
 __device__ __forceinline__ cplx cadd(cplx a, cplx b) { return mk(a.x + b.x, a.y + b.y); }
 __device__ __forceinline__ cplx csub(cplx a, cplx b) { return mk(a.x - b.x, a.y - b.y); }

@@ -27,8 +27,6 @@ struct SegDev {
   cplx* zd;         // [M]: z of the data vector d (td_inner_batch only)
 };
 
-enum { MODE_LOGLIKE = 0, MODE_INNER = 1, MODE_STOREZ = 2 };
-
 struct FusedParams {
   const double* d;
   const double* H;

@@ -15,6 +15,7 @@
 #include "td_fused.cuh"
 #include "td_cluster.cuh"
 #include "td_fused4.cuh"
+#include "td_probe.cuh"
 #include "td_setup.cuh"
 #include "td_staged.cuh"
 
@@ -26,6 +27,7 @@ constexpr int FUSED_MIN_LOG2M = 8;   // M = 256
 // one-CTA fused kernels: M = 256..4096 (2M = 8192-point transform, 204 KiB of shared memory at M = 4096)
 constexpr int CLUSTER_LOG2M = 13;    // M = 8192: 2-CTA cluster, one branch per CTA (td_cluster.cuh)
 constexpr int FUSED_NT = 256;
+constexpr int DENSE_AUTO_N = 128;     // AUTO: dense path for segments up to this length (measured crossover)
 constexpr size_t STAGED_WS_BYTES = 64ull << 20;  // keep the staged workspace L2-resident (126 MB L2)
 
 struct SegHost {
@@ -43,6 +45,7 @@ struct ClassInfo {
   int log2M = 0;
   cplx* T = nullptr;            // device [2M]
   std::vector<int> seg_ids;
+  int max_n = 0;                // longest segment of the class
   SegDev* d_segs = nullptr;     // device [seg_ids.size()]
   const cplx** d_Gp = nullptr;  // device [seg_ids.size()] (fused4 classes only)
 };
@@ -321,13 +324,62 @@ bool class_is_fused(const td_handle* h, const ClassInfo& c) {
   return c.log2M >= FUSED_MIN_LOG2M && c.log2M <= CLUSTER_LOG2M;
 }
 
+
+// AUTO sends a size class to the dense path when every segment in it is at most dense.auto_n long.
+bool class_is_dense(const td_handle* h, const ClassInfo& c) {
+  if (h->path == TD_PATH_DENSE) return true;
+  if (h->path == TD_PATH_FFT) return false;
+  return c.max_n <= h->dense.auto_n;
+}
+
+// (re)builds the device segment tables of the dense path from the host-side segment records
+td_status dense_upload(td_handle* h) {
+  DenseState& D = h->dense;
+  std::vector<DenseSeg> all, aut;
+  int npad_all = 0, npad_auto = 0;
+  for (const ClassInfo& c : h->classes)
+    for (int id : c.seg_ids) {
+      const SegHost& sg = h->segs[id];
+      if (sg.n > DENSE_MAX_N) continue;
+      DenseSeg ds;
+      ds.off = sg.off; ds.n = sg.n; ds.npad = (sg.n + 31) / 32 * 32; ds.a = sg.a; ds.rsv = 1.0 / std::sqrt(sg.v); ds.zd = sg.zd;
+      all.push_back(ds); npad_all = std::max(npad_all, ds.npad);
+      if (c.max_n <= D.auto_n) { aut.push_back(ds); npad_auto = std::max(npad_auto, ds.npad); }
+    }
+  D.max_n = DENSE_MAX_N;
+  const bool all_fit = h->max_n <= DENSE_MAX_N;
+  if (all_fit && !D.d_all) CK(cudaMalloc(&D.d_all, sizeof(DenseSeg) * all.size()));
+  if (!aut.empty() && !D.d_auto) CK(cudaMalloc(&D.d_auto, sizeof(DenseSeg) * aut.size()));
+  if (all_fit) { CK(cudaMemcpy(D.d_all, all.data(), sizeof(DenseSeg) * all.size(), cudaMemcpyHostToDevice)); D.n_all = (int)all.size(); D.npad_all = npad_all; }
+  if (!aut.empty()) { CK(cudaMemcpy(D.d_auto, aut.data(), sizeof(DenseSeg) * aut.size(), cudaMemcpyHostToDevice)); D.n_auto = (int)aut.size(); D.npad_auto = npad_auto; }
+  return TD_OK;
+}
+
+template <int MODE>
+td_status launch_dense(td_handle* h, const DenseSeg* segs, int n_seg, int max_npad, const double* d, const double* H,
+                       int64_t ldh, int64_t B, double* out0, double* out1, int accumulate, cudaStream_t st) {
+  auto kern = td_dense_kernel<MODE>;
+  DenseParams P;
+  P.d = d; P.H = H; P.ldh = ldh; P.B = B; P.out0 = out0; P.out1 = out1; P.segs = segs; P.n_seg = n_seg;
+  P.accumulate = accumulate; P.max_npad = max_npad; P.nwr = dense_nwr(max_npad);
+  const int bt = 16 * (DENSE_NW / P.nwr);
+  const size_t smem = dense_smem_bytes(max_npad);
+  CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  const int64_t grid = (B + bt - 1) / bt;
+  if (grid > 0x7fffffffll) return TD_EUNSUPPORTED;
+  kern<<<(unsigned)grid, DENSE_NT, smem, st>>>(P);
+  CK(cudaGetLastError());
+  ++h->last_launches;
+  return TD_OK;
+}
+
 // FFT path over all size classes.  MODE_LOGLIKE: out0 = loglike.  MODE_INNER: out0 = <d,h>, out1 = <h,h>.
 template <int MODE>
 td_status run_fft_path(td_handle* h, const double* d, const double* H, int64_t ldh, int64_t B, double* out0,
-                       double* out1, cudaStream_t st) {
-  int accumulate = 0;
+                       double* out1, cudaStream_t st, bool skip_dense_classes = false, int accumulate = 0) {
   const double sc0 = (MODE == MODE_LOGLIKE) ? -0.5 : 1.0, sc1 = 1.0;
   for (const ClassInfo& cls : h->classes) {
+    if (skip_dense_classes && class_is_dense(h, cls)) continue;
     if (class_is_fused(h, cls)) {
       FusedParams P;
       P.d = d; P.H = H; P.ldh = ldh; P.B = B; P.out0 = out0; P.out1 = out1;
@@ -344,6 +396,27 @@ td_status run_fft_path(td_handle* h, const double* d, const double* H, int64_t l
     }
   }
   return TD_OK;
+}
+
+// One batch call: the dense kernel for the classes the chooser (or td_set_path) gives it, the FFT
+// kernels for the rest, all accumulating into the same outputs.
+template <int MODE>
+td_status run_batch(td_handle* h, const double* d, const double* H, int64_t ldh, int64_t B, double* out0,
+                    double* out1, cudaStream_t st) {
+  const DenseState& D = h->dense;
+  const DenseSeg* dsegs = nullptr;
+  int nd = 0, npad = 0;
+  if (h->path == TD_PATH_DENSE) { dsegs = D.d_all; nd = D.n_all; npad = D.npad_all; }
+  else if (h->path == TD_PATH_AUTO) { dsegs = D.d_auto; nd = D.n_auto; npad = D.npad_auto; }
+  int accumulate = 0;
+  if (nd > 0) {
+    td_status s = launch_dense<MODE>(h, dsegs, nd, npad, d, H, ldh, B, out0, out1, 0, st);
+    if (s != TD_OK) return s;
+    accumulate = 1;
+  }
+  h->last_path = (nd == h->n_seg) ? TD_PATH_DENSE : TD_PATH_FFT;
+  if (nd == h->n_seg) return TD_OK;
+  return run_fft_path<MODE>(h, d, H, ldh, B, out0, out1, st, true, accumulate);
 }
 
 }  // namespace
@@ -416,6 +489,7 @@ static td_status create_impl(td_handle* h, const double* acf, const int64_t* seg
     auto it = std::find_if(h->classes.begin(), h->classes.end(), [&](const ClassInfo& c) { return c.log2M == l2; });
     if (it == h->classes.end()) { h->classes.emplace_back(); h->classes.back().log2M = l2; it = h->classes.end() - 1; }
     it->seg_ids.push_back(s);
+    it->max_n = std::max(it->max_n, h->segs[s].n);
   }
   for (ClassInfo& c : h->classes) {
     const int TW = 2 << c.log2M;
@@ -464,7 +538,9 @@ static td_status create_impl(td_handle* h, const double* acf, const int64_t* seg
       CK(cudaMemcpy(c.d_Gp, gp.data(), sizeof(cplx*) * gp.size(), cudaMemcpyHostToDevice));
     }
   }
-  return TD_OK;
+  // ---- dense path tables (the chooser's crossover is measured: DESIGN.md 6.4)
+  h->dense.auto_n = getenv("TDLIKE_DENSE_AUTO_N") ? atoi(getenv("TDLIKE_DENSE_AUTO_N")) : DENSE_AUTO_N;
+  return dense_upload(h);
 }
 
 td_status td_create(const double* acf, const int64_t* seg_lengths, int n_seg, int device, td_handle** out) {
@@ -504,8 +580,7 @@ td_status td_loglike_batch(td_handle* h, const double* d, const double* H, int64
   DevGuard guard(h->device);
   if (!guard.ok) return TD_ECUDA;
   h->last_launches = 0;
-  h->last_path = TD_PATH_FFT;
-  return run_fft_path<MODE_LOGLIKE>(h, d, H, ldh, B, out, nullptr, (cudaStream_t)stream);
+  return run_batch<MODE_LOGLIKE>(h, d, H, ldh, B, out, nullptr, (cudaStream_t)stream);
 }
 
 td_status td_loglike_batch_host(td_handle* h, const double* d, const double* H, int64_t ldh, int64_t B, double* out,
@@ -568,7 +643,6 @@ td_status td_inner_batch(td_handle* h, const double* d, const double* H, int64_t
   if (!guard.ok) return TD_ECUDA;
   cudaStream_t st = (cudaStream_t)stream;
   h->last_launches = 0;
-  h->last_path = TD_PATH_FFT;
   // z of the data vector, once per call (per segment), then the bilinear sums against it
   for (ClassInfo& c : h->classes) {
     bool fresh = false;
@@ -584,11 +658,13 @@ td_status td_inner_batch(td_handle* h, const double* d, const double* H, int64_t
       }
       CK(cudaMemcpyAsync(c.d_segs, sd.data(), sizeof(SegDev) * sd.size(), cudaMemcpyHostToDevice, st));
       CK(cudaStreamSynchronize(st));  // sd is a host temporary (first td_inner_batch call only)
+      td_status su = dense_upload(h);
+      if (su != TD_OK) return su;
     }
   }
   td_status s = run_fft_path<MODE_STOREZ>(h, d, nullptr, h->n_tot, 1, nullptr, nullptr, st);
   if (s != TD_OK) return s;
-  return run_fft_path<MODE_INNER>(h, d, H, ldh, B, out_dh, out_hh, st);
+  return run_batch<MODE_INNER>(h, d, H, ldh, B, out_dh, out_hh, st);
 }
 
 td_status td_set_path(td_handle* h, int path) {
@@ -621,6 +697,42 @@ td_status td_get_generator(const td_handle* h, int seg, double* a) {
   DevGuard guard(h->device);
   if (!guard.ok) return TD_ECUDA;
   CK(cudaMemcpy(a, h->segs[seg].a, sizeof(double) * h->segs[seg].n, cudaMemcpyDeviceToHost));
+  return TD_OK;
+}
+
+td_status td_probe_fp64(int kind, int device, double* tflops) {
+  if (kind < 0 || kind > 3 || !tflops) return TD_EINVAL;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return TD_ECUDA;
+  if (device < 0 || device >= ndev) return TD_EINVAL;
+  DevGuard guard(device);
+  if (!guard.ok) return TD_ECUDA;
+  cudaDeviceProp prop;
+  CK(cudaGetDeviceProperties(&prop, device));
+  const int grid = prop.multiProcessorCount * 8, iters = 200;
+  double* sink = nullptr;
+  CK(cudaMalloc(&sink, sizeof(double)));
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  cudaEventCreate(&e0); cudaEventCreate(&e1);
+  float best = 1e30f;
+  td_status rc = TD_OK;
+  for (int rep = 0; rep < 6 && rc == TD_OK; ++rep) {
+    cudaEventRecord(e0, 0);
+    switch (kind) {
+      case 0: probe_kernel<0><<<grid, PROBE_NT>>>(sink, iters, 1.0 + rep); break;
+      case 1: probe_kernel<1><<<grid, PROBE_NT>>>(sink, iters, 1.0 + rep); break;
+      case 2: probe_kernel<2><<<grid, PROBE_NT>>>(sink, iters, 1.0 + rep); break;
+      default: probe_kernel<3><<<grid, PROBE_NT>>>(sink, iters, 1.0 + rep); break;
+    }
+    cudaEventRecord(e1, 0);
+    if (cudaEventSynchronize(e1) != cudaSuccess || cudaGetLastError() != cudaSuccess) { rc = TD_ECUDA; break; }
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, e0, e1);
+    if (rep > 0 && ms < best) best = ms;  // first launch is the warm-up
+  }
+  cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(sink);
+  if (rc != TD_OK) return rc;
+  *tflops = probe_flops(kind, grid, iters) / (best * 1e-3) / 1e12;
   return TD_OK;
 }
 

@@ -16,7 +16,7 @@ HEADER = os.path.join(ROOT, "include", "tdlike.h")
 def _declared():
     src = open(HEADER).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
-    return sorted(set(re.findall(r"\b(td_[a-z_]+)\s*\(", src)))
+    return sorted(set(re.findall(r"\b(td_[a-z0-9_]+)\s*\(", src)))
 
 
 def test_library_builds_and_loads_without_gpu():
@@ -32,7 +32,7 @@ def test_every_declared_symbol_is_exported_and_bound():
     assert {"td_create", "td_destroy", "td_loglike_batch", "td_inner_batch", "td_set_path", "td_get_info",
             "td_strerror"} <= set(names)
     nm = subprocess.run(["nm", "-D", "--defined-only", tdb.LIB_PATH], capture_output=True, text=True, check=True).stdout
-    exported = set(re.findall(r"\bT (td_[a-z_]+)\b", nm))
+    exported = set(re.findall(r"\bT (td_[a-z0-9_]+)\b", nm))
     assert set(names) <= exported, set(names) - exported
     assert set(names) == set(tdb.SYMBOLS), set(names) ^ set(tdb.SYMBOLS)
 

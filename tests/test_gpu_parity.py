@@ -267,3 +267,83 @@ def test_async_on_caller_stream_and_repeatable():
             o2 = h.loglike_batch(d, H)
         s.synchronize()
     assert torch.equal(o1, o2)                               # deterministic reduction order
+
+
+# ------------------------------------------------------------------ dense path (S2'-S4')
+@pytest.mark.parametrize("n", [1, 5, 31, 32, 33, 64, 100, 128, 200, 256, 300, 512, 777, 1024])
+def test_dense_path_lengths(n):
+    """Forced dense path: every row-group / warp arrangement (NWR = 1, 2, 4, 8), ragged N and B."""
+    rng = np.random.default_rng(1000 + n)
+    rho = W.acf_from_psd(4096.0, 2 * 8192, n)
+    d = rng.standard_normal(n) * 1e-21
+    H = rng.standard_normal((37, n)) * 1e-21
+    ref = O.loglike_batch(rho, [n], d, H)
+    out, info, nl = _gpu_loglike(W.Workload("t", 0, 4096.0, np.array([n]), rho, d, H, np.ones(1)), path=tdb.TD_PATH_DENSE)
+    _assert_close(out, ref, what=f"dense n={n}")
+    assert info["last_path"] == tdb.TD_PATH_DENSE and nl == 1
+
+
+@pytest.mark.parametrize("name", ["d1", "d2", "d3"])
+def test_dense_configs_both_paths(name):
+    """d1-d3 (ringdown-only segments): dense and FFT paths against the oracle and each other."""
+    w = W.make(name, B=300)
+    ref = O.loglike_batch(w.acf, w.seg_lengths, w.d, w.H)
+    od, info_d, _ = _gpu_loglike(w, path=tdb.TD_PATH_DENSE)
+    of, info_f, _ = _gpu_loglike(w, path=tdb.TD_PATH_FFT)
+    _assert_close(od, ref, what=name + " dense")
+    _assert_close(of, ref, what=name + " fft")
+    assert info_d["last_path"] == tdb.TD_PATH_DENSE and info_f["last_path"] == tdb.TD_PATH_FFT
+
+
+def test_dense_multi_segment_and_inner():
+    rng = np.random.default_rng(77)
+    lens = [64, 200, 33, 512]
+    rho = W.acf_from_psd(4096.0, 2 * 8192, max(lens))
+    scales = [1.0, 0.6, 2.5, 1.7]
+    acf = np.concatenate([s * rho[:n] for s, n in zip(scales, lens)])
+    nt = sum(lens)
+    d = rng.standard_normal(nt) * 1e-21
+    H = rng.standard_normal((45, nt)) * 1e-21
+    ref = O.loglike_batch(acf, lens, d, H)
+    dh_ref, hh_ref = O.inner_batch(acf, lens, d, H)
+    with tdb.TDLikelihood(acf, lens) as h:
+        h.set_path(tdb.TD_PATH_DENSE)
+        dd_, HH = _dev(d), _dev(H)
+        out = h.loglike_batch(dd_, HH).cpu().numpy()
+        assert h.info()["last_path"] == tdb.TD_PATH_DENSE
+        dh, hh = h.inner_batch(dd_, HH)
+        dd, _ = h.inner_batch(dd_, dd_[None, :])
+    _assert_close(out, ref, what="dense multi-segment")
+    dh, hh, dd = dh.cpu().numpy(), hh.cpu().numpy(), dd.cpu().numpy()[0]
+    scale = dd + hh
+    assert np.max(np.abs(dh - dh_ref) / scale) <= TOL
+    assert np.max(np.abs(hh - hh_ref) / np.abs(hh_ref)) <= TOL
+    assert np.max(np.abs(-2 * out - (dd - 2 * dh + hh)) / scale) <= TOL
+
+
+def test_auto_chooser_mixes_paths():
+    """AUTO: the short segment goes to the dense kernel, the long one to the FFT kernel, one sum."""
+    rng = np.random.default_rng(78)
+    lens = [64, 3000]
+    rho = W.acf_from_psd(4096.0, 2 * 8192, max(lens))
+    acf = np.concatenate([rho[:64], 1.4 * rho[:3000]])
+    nt = sum(lens)
+    d = rng.standard_normal(nt) * 1e-21
+    H = rng.standard_normal((19, nt)) * 1e-21
+    ref = O.loglike_batch(acf, lens, d, H)
+    with tdb.TDLikelihood(acf, lens) as h:
+        out = h.loglike_batch(_dev(d), _dev(H)).cpu().numpy()
+        assert h.last_launches() == 2 and h.info()["last_path"] == tdb.TD_PATH_FFT
+        dh, hh = h.inner_batch(_dev(d), _dev(H))
+        with pytest.raises(tdb.TDError) as e:
+            h.set_path(tdb.TD_PATH_DENSE)          # 3000 > dense limit
+        assert e.value.status == tdb.TD_EUNSUPPORTED
+    _assert_close(out, ref, what="auto mixed")
+    dh_ref, hh_ref = O.inner_batch(acf, lens, d, H)
+    assert np.max(np.abs(hh.cpu().numpy() - hh_ref) / np.abs(hh_ref)) <= TOL
+
+
+def test_probe_fp64_reports_plausible_peaks():
+    dfma = tdb.probe_fp64(0)
+    dmma = tdb.probe_fp64(1)
+    assert 10.0 < dfma < 60.0 and 10.0 < dmma < 90.0
