@@ -100,7 +100,6 @@ void free_handle(td_handle* h) {
   for (auto& s : h->segs) { cudaFree(s.a); cudaFree(s.G); cudaFree(s.Gp); cudaFree(s.zd); }
   for (auto& c : h->classes) { cudaFree(c.T); cudaFree(c.d_segs); cudaFree(c.d_Gp); }
   cudaFree(h->wsU); cudaFree(h->wsZ); cudaFree(h->wsPartial);
-  dense_free(h->dense);
   cudaFree(h->hsD); cudaFree(h->hsH[0]); cudaFree(h->hsH[1]); cudaFree(h->hsOut);
   if (h->copy_stream) cudaStreamDestroy(h->copy_stream);
   for (int i = 0; i < 2; ++i) { if (h->ev_copied[i]) cudaEventDestroy(h->ev_copied[i]); if (h->ev_done[i]) cudaEventDestroy(h->ev_done[i]); }
@@ -332,44 +331,56 @@ bool class_is_dense(const td_handle* h, const ClassInfo& c) {
   return c.max_n <= h->dense.auto_n;
 }
 
-// (re)builds the device segment tables of the dense path from the host-side segment records
+// (re)builds the segment tables of the dense path from the host-side segment records
 td_status dense_upload(td_handle* h) {
   DenseState& D = h->dense;
-  std::vector<DenseSeg> all, aut;
-  int npad_all = 0, npad_auto = 0;
+  D.all.clear(); D.aut.clear();
   for (const ClassInfo& c : h->classes)
     for (int id : c.seg_ids) {
       const SegHost& sg = h->segs[id];
       if (sg.n > DENSE_MAX_N) continue;
       DenseSeg ds;
       ds.off = sg.off; ds.n = sg.n; ds.npad = (sg.n + 31) / 32 * 32; ds.a = sg.a; ds.rsv = 1.0 / std::sqrt(sg.v); ds.zd = sg.zd;
-      all.push_back(ds); npad_all = std::max(npad_all, ds.npad);
-      if (c.max_n <= D.auto_n) { aut.push_back(ds); npad_auto = std::max(npad_auto, ds.npad); }
+      D.all.push_back(ds);
+      if (c.max_n <= D.auto_n) D.aut.push_back(ds);
     }
   D.max_n = DENSE_MAX_N;
-  const bool all_fit = h->max_n <= DENSE_MAX_N;
-  if (all_fit && !D.d_all) CK(cudaMalloc(&D.d_all, sizeof(DenseSeg) * all.size()));
-  if (!aut.empty() && !D.d_auto) CK(cudaMalloc(&D.d_auto, sizeof(DenseSeg) * aut.size()));
-  if (all_fit) { CK(cudaMemcpy(D.d_all, all.data(), sizeof(DenseSeg) * all.size(), cudaMemcpyHostToDevice)); D.n_all = (int)all.size(); D.npad_all = npad_all; }
-  if (!aut.empty()) { CK(cudaMemcpy(D.d_auto, aut.data(), sizeof(DenseSeg) * aut.size(), cudaMemcpyHostToDevice)); D.n_auto = (int)aut.size(); D.npad_auto = npad_auto; }
+  if (h->max_n > DENSE_MAX_N) D.all.clear();
   return TD_OK;
 }
 
+// one launch per segment; segments accumulate into the outputs in launch order
 template <int MODE>
-td_status launch_dense(td_handle* h, const DenseSeg* segs, int n_seg, int max_npad, const double* d, const double* H,
-                       int64_t ldh, int64_t B, double* out0, double* out1, int accumulate, cudaStream_t st) {
-  auto kern = td_dense_kernel<MODE>;
-  DenseParams P;
-  P.d = d; P.H = H; P.ldh = ldh; P.B = B; P.out0 = out0; P.out1 = out1; P.segs = segs; P.n_seg = n_seg;
-  P.accumulate = accumulate; P.max_npad = max_npad; P.nwr = dense_nwr(max_npad);
-  const int bt = 16 * (DENSE_NW / P.nwr);
-  const size_t smem = dense_smem_bytes(max_npad);
-  CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  const int64_t grid = (B + bt - 1) / bt;
-  if (grid > 0x7fffffffll) return TD_EUNSUPPORTED;
-  kern<<<(unsigned)grid, DENSE_NT, smem, st>>>(P);
-  CK(cudaGetLastError());
-  ++h->last_launches;
+td_status launch_dense(td_handle* h, const std::vector<DenseSeg>& segs, const double* d, const double* H, int64_t ldh,
+                       int64_t B, double* out0, double* out1, int accumulate, cudaStream_t st) {
+  for (const DenseSeg& sg : segs) {
+    DenseParams P;
+    P.d = d; P.H = H; P.ldh = ldh; P.B = B; P.out0 = out0; P.out1 = out1; P.seg = sg;
+    P.accumulate = accumulate; P.nwr = dense_nwr(sg.npad); P.nbuf = dense_nbuf(sg.npad);
+    void (*kern)(const DenseParams) = P.nwr == 1 ? td_dense_kernel<MODE, 1> : P.nwr == 2 ? td_dense_kernel<MODE, 2>
+                                    : P.nwr == 4 ? td_dense_kernel<MODE, 4> : td_dense_kernel<MODE, 8>;
+    // 16-byte copies when every row start is 16-byte aligned and the length is even
+    P.vec_ok = (sg.off % 2 == 0) && (sg.n % 2 == 0) && (ldh % 2 == 0) && ((reinterpret_cast<uintptr_t>(H) & 15) == 0);
+    P.ntiles = (B + 15) / 16;
+    // DMMAs of one warp per tile x 16 cycles each: the lag that lets one group's bookkeeping hide under the other's DMMAs
+    {
+      const int NG = sg.npad / 32;
+      long long nd = 0;
+      for (int p = 0; 2 * p < NG; p += P.nwr) {  // warp wr = 0
+        nd += 80 + 128ll * (NG - p - 1);
+        if (NG - 1 - p != p) nd += 80 + 128ll * p;
+      }
+      P.stagger_cycles = (int)std::min<long long>(nd * 16, 1 << 22);
+    }
+    const size_t smem = dense_smem_bytes(sg.npad, P.nbuf);
+    CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    const int nwc = DENSE_NW / P.nwr;
+    const int64_t grid = std::min<int64_t>((P.ntiles + nwc - 1) / nwc, h->num_sms);
+    kern<<<(unsigned)grid, DENSE_NT, smem, st>>>(P);
+    CK(cudaGetLastError());
+    ++h->last_launches;
+    accumulate = 1;
+  }
   return TD_OK;
 }
 
@@ -404,13 +415,13 @@ template <int MODE>
 td_status run_batch(td_handle* h, const double* d, const double* H, int64_t ldh, int64_t B, double* out0,
                     double* out1, cudaStream_t st) {
   const DenseState& D = h->dense;
-  const DenseSeg* dsegs = nullptr;
-  int nd = 0, npad = 0;
-  if (h->path == TD_PATH_DENSE) { dsegs = D.d_all; nd = D.n_all; npad = D.npad_all; }
-  else if (h->path == TD_PATH_AUTO) { dsegs = D.d_auto; nd = D.n_auto; npad = D.npad_auto; }
+  const std::vector<DenseSeg>* dsegs = nullptr;
+  if (h->path == TD_PATH_DENSE) dsegs = &D.all;
+  else if (h->path == TD_PATH_AUTO) dsegs = &D.aut;
+  const int nd = dsegs ? (int)dsegs->size() : 0;
   int accumulate = 0;
   if (nd > 0) {
-    td_status s = launch_dense<MODE>(h, dsegs, nd, npad, d, H, ldh, B, out0, out1, 0, st);
+    td_status s = launch_dense<MODE>(h, *dsegs, d, H, ldh, B, out0, out1, 0, st);
     if (s != TD_OK) return s;
     accumulate = 1;
   }
