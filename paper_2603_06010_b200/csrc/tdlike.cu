@@ -27,7 +27,7 @@ constexpr int FUSED_MIN_LOG2M = 8;   // M = 256
 // one-CTA fused kernels: M = 256..4096 (2M = 8192-point transform, 204 KiB of shared memory at M = 4096)
 constexpr int CLUSTER_LOG2M = 13;    // M = 8192: 2-CTA cluster, one branch per CTA (td_cluster.cuh)
 constexpr int FUSED_NT = 256;
-constexpr int DENSE_AUTO_N = 128;     // AUTO: dense path for segments up to this length (measured crossover)
+constexpr int DENSE_AUTO_N = 512;     // AUTO: dense path for segments up to this length (measured crossover: profiles/r01_chooser.md)
 constexpr size_t STAGED_WS_BYTES = 64ull << 20;  // keep the staged workspace L2-resident (126 MB L2)
 
 struct SegHost {
@@ -550,7 +550,7 @@ static td_status create_impl(td_handle* h, const double* acf, const int64_t* seg
     }
   }
   // ---- dense path tables (the chooser's crossover is measured: DESIGN.md 6.4)
-  h->dense.auto_n = getenv("TDLIKE_DENSE_AUTO_N") ? atoi(getenv("TDLIKE_DENSE_AUTO_N")) : DENSE_AUTO_N;
+  h->dense.auto_n = DENSE_AUTO_N;
   return dense_upload(h);
 }
 

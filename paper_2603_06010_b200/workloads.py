@@ -127,6 +127,8 @@ _SPECS = {
     "d1": (260306021, (1 << 24) // 64),
     "d2": (260306022, (1 << 24) // 128),
     "d3": (260306023, (1 << 24) // 256),
+    "d4": (260306024, (1 << 24) // 512),
+    "d5": (260306025, (1 << 24) // 1024),
 }
 CONFIG_NAMES = tuple(_SPECS)
 
@@ -158,7 +160,7 @@ def _chunks(B: int, n: int, budget_elems: int = 1 << 25):
 
 
 def make(name: str, B: Optional[int] = None, n_scale: int = 1) -> Workload:
-    """Build config `name` (c1..c5 of BASELINE.json, d1..d3 the dense-regime extensions).
+    """Build config `name` (c1..c5 of BASELINE.json, d1..d5 the dense-regime / crossover extensions).
 
     B overrides the number of templates (draw vectors then have that length).  n_scale > 1
     divides every length (fs kept, durations shortened) to give reduced-size versions with the
@@ -256,9 +258,9 @@ def make(name: str, B: Optional[int] = None, n_scale: int = 1) -> Workload:
         return Workload(name, seed, fs, np.array([N] * 3, np.int64), acf, noise + H[0], H, scales,
                         "3 detectors x N, projected damped sinusoids, network SNR")
 
-    if name in ("d1", "d2", "d3"):
+    if name in ("d1", "d2", "d3", "d4", "d5"):
         fs = 4096.0
-        N = {"d1": 64, "d2": 128, "d3": 256}[name]
+        N = {"d1": 64, "d2": 128, "d3": 256, "d4": 512, "d5": 1024}[name]
         M = 2 * 4096                      # ACF taken from the 1 s grid, truncated (Eq. 11)
         rho = acf_from_psd(fs, M, N)
         n = _noise(rng, fs, M, N)

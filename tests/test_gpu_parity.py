@@ -147,6 +147,7 @@ def test_ragged_lengths(n):
     for variant in (0, 2):
         with tdb.TDLikelihood(rho, [n]) as h:
             h.set_fft_variant(variant)
+            h.set_path(tdb.TD_PATH_FFT)        # AUTO would send n <= 512 to the dense kernel
             out = h.loglike_batch(_dev(d), _dev(H)).cpu().numpy()
         _assert_close(out, ref, what=f"n={n} variant={variant}")
 
