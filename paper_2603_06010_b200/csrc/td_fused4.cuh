@@ -16,6 +16,7 @@
 // CTA barriers per (template, segment): 5 (was 9).
 #pragma once
 #include "td_fused.cuh"
+#include "td_dit16.cuh"
 
 namespace td {
 
@@ -112,7 +113,7 @@ __device__ __forceinline__ void f4_mid(const SmemArr& U, const SmemArr& Z, int b
       e[h8] = cmul(e[h8], cadd(A, wB));          // G * 2 X_{kq},      entry s = t/2
       e[8 + h8] = cmul(e[8 + h8], csub(A, wB));  // G * 2 X_{NF + kq}, entry s = 8 + t/2
     });
-    fft_reg<16, true>(e);
+    dit16<true, false>(e, mk(1.0, 0.0));
     static_for<0, 16>([&](auto t) { Z.st(zb + decltype(t)::value, e[brevR<16>(decltype(t)::value)]); });
   });
 }
@@ -120,20 +121,15 @@ __device__ __forceinline__ void f4_mid(const SmemArr& U, const SmemArr& Z, int b
 // inverse pass 2 (L = 256), warp-local: blocks s1 = 4wb .. 4wb+3
 template <int TW>
 __device__ __forceinline__ void f4_inverse2(const SmemArr& Z, int wb, int lane, const cplx* __restrict__ tw) {
-  cplx x[16], w[16];
+  cplx x[16], y[16];
   const int j = lane & 15;
-  tw_powers<16>(tw[j * (TW / 256)], w);
-  cplx y[16];
+  const cplx w1 = cconj(tw[j * (TW / 256)]);  // the inverse transform's w_256^(-j); its powers are built inside dit16
   const int base0 = (4 * wb + (lane >> 4)) * 256 + j, base1 = base0 + 2 * 256;
-  static_for<0, 16>([&](auto q) {
-    constexpr int qq = decltype(q)::value;
-    cplx a = Z.ld(base0 + 16 * qq), c = Z.ld(base1 + 16 * qq);
-    if constexpr (qq > 0) { a = cmulc(a, w[qq]); c = cmulc(c, w[qq]); }
-    x[qq] = a; y[qq] = c;
-  });
-  fft_reg<16, true>(x);
+#pragma unroll
+  for (int q = 0; q < 16; ++q) { x[q] = Z.ld(base0 + 16 * q); y[q] = Z.ld(base1 + 16 * q); }
+  dit16<true, true>(x, w1);
   static_for<0, 16>([&](auto t) { Z.st(base0 + 16 * decltype(t)::value, x[brevR<16>(decltype(t)::value)]); });
-  fft_reg<16, true>(y);
+  dit16<true, true>(y, w1);
   static_for<0, 16>([&](auto t) { Z.st(base1 + 16 * decltype(t)::value, y[brevR<16>(decltype(t)::value)]); });
 }
 
@@ -230,7 +226,7 @@ __global__ void __launch_bounds__(Fused4Shape<LOG2M>::NT, 1) td_fused4_kernel(co
     __syncthreads();
     // ---------------- forward passes 2 and 3, warp-local
     f4_forward23<TW>(U, wb, lane, tw);
-    __syncthreads();
+    asm volatile("bar.sync %0, %1;" ::"r"(1 + br), "r"(NT / 2) : "memory");  // mid reads mirror blocks of the SAME branch only
     // ---------------- mid: untangle (registers) x generator (in place in Z) -> first inverse pass
     mbar_wait(mbar_g, par_g);
     par_g ^= 1;
