@@ -53,6 +53,47 @@ __global__ void __launch_bounds__(LG_NT) lg_pass_kernel(cplx* base, int n, int L
   else dit_task<R>(A, L, g, w, tw);
 }
 
+// Three radix-16 passes of one contiguous 4096-element block in shared memory: the forward (DIF)
+// passes L = 4096, 256, 16 that end every plan, or the inverse (DIT) passes L = 16, 256, 4096 that
+// start it.  One read and one write of the workspace instead of three of each: the staged path is
+// bound by L2 traffic (profiles/r01_c4_staged.md), so this is where its time goes.
+constexpr int LGB_NT = 256, LGB_N = 4096;
+constexpr size_t LGB_SMEM = sizeof(cplx) * SmemArr::padded(LGB_N);
+
+template <bool FWD>
+__global__ void __launch_bounds__(LGB_NT, 2) lg_block_kernel(cplx* base, int n, const cplx* __restrict__ T, int TW) {
+  extern __shared__ __align__(16) unsigned char lgb_raw[];
+  const SmemArr A{reinterpret_cast<cplx*>(lgb_raw)};
+  cplx* g = base + (size_t)blockIdx.y * n + (size_t)blockIdx.x * LGB_N;
+  const int tid = threadIdx.x;
+#pragma unroll
+  for (int q = 0; q < LGB_N / LGB_NT; ++q) A.st(tid + q * LGB_NT, g[tid + q * LGB_NT]);
+  __syncthreads();
+  if (FWD) {
+    static_for<0, 3>([&](auto pp) {
+      constexpr int L = LGB_N >> (4 * decltype(pp)::value), S = L / 16;
+      cplx w[16];
+      if constexpr (S > 1) tw_powers<16>(T[(size_t)(tid & (S - 1)) * (TW / L)], w);
+      dif_task_c<16, L>(A, tid, w);
+      __syncthreads();
+    });
+  } else {
+    static_for<0, 3>([&](auto pp) {
+      constexpr int L = 16 << (4 * decltype(pp)::value), S = L / 16;
+      const int blk = tid / S, j = tid & (S - 1), b0 = blk * L + j;
+      cplx x[16];
+#pragma unroll
+      for (int q = 0; q < 16; ++q) x[q] = A.ld(b0 + q * S);
+      if constexpr (S > 1) dit16<true, true>(x, cconj(T[(size_t)j * (TW / L)]));
+      else dit16<true, false>(x, mk(1.0, 0.0));
+      static_for<0, 16>([&](auto t) { A.st(b0 + decltype(t)::value * S, x[brevR<16>(decltype(t)::value)]); });
+      __syncthreads();
+    });
+  }
+#pragma unroll
+  for (int q = 0; q < LGB_N / LGB_NT; ++q) g[tid + q * LGB_NT] = A.ld(tid + q * LGB_NT);
+}
+
 __global__ void __launch_bounds__(LG_NT) lg_untangle_kernel(const StagedParams P) {
   const int nf = P.M / 2;
   const int p = blockIdx.x * LG_NT + threadIdx.x;

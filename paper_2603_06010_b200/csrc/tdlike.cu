@@ -120,13 +120,29 @@ td_status launch_pass(int R, cplx* base, int narr, int n, int L, const cplx* T, 
   return TD_OK;
 }
 
-// forward DIF of `narr` arrays of length n with plan [r1,16,16,...]; returns launches made
+template <bool FWD>
+td_status launch_block(cplx* base, int narr, int n, const cplx* T, int TW, cudaStream_t st) {
+  auto kern = lg_block_kernel<FWD>;
+  CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)LGB_SMEM));
+  kern<<<dim3(n / LGB_N, narr), LGB_NT, LGB_SMEM, st>>>(base, n, T, TW);
+  CK(cudaGetLastError());
+  return TD_OK;
+}
+
+// forward DIF of `narr` arrays of length n with plan [r1,16,16,...]; the last three passes
+// (L = 4096, 256, 16) run as one shared-memory block kernel when the plan has them
 td_status staged_forward(cplx* base, int narr, int n, int first_pass_done, const cplx* T, int TW,
                          cudaStream_t st, int* launches) {
   int L = n;
   const int r1 = plan_r1(n), np = plan_np(n);
   for (int q = 0; q < np; ++q) {
     const int R = q == 0 ? r1 : 16;
+    if (q >= 1 && q == np - 3 && L == LGB_N) {
+      td_status s = launch_block<true>(base, narr, n, T, TW, st);
+      if (s != TD_OK) return s;
+      ++*launches;
+      break;
+    }
     if (!(q == 0 && first_pass_done)) {
       td_status s = launch_pass<true>(R, base, narr, n, L, T, TW, st);
       if (s != TD_OK) return s;
@@ -137,12 +153,19 @@ td_status staged_forward(cplx* base, int narr, int n, int first_pass_done, const
   return TD_OK;
 }
 
-// inverse DIT passes except the last (radix r1, L = n) one
+// inverse DIT passes except the last (radix r1, L = n) one; the first three (L = 16, 256, 4096)
+// as one shared-memory block kernel when the plan has them
 td_status staged_inverse_but_last(cplx* base, int narr, int n, const cplx* T, int TW, cudaStream_t st,
                                   int* launches) {
   const int np = plan_np(n);
-  int L = 16;
-  for (int q = 1; q < np; ++q) {
+  int L = 16, q = 1;
+  if (np - 1 >= 3) {
+    td_status s = launch_block<false>(base, narr, n, T, TW, st);
+    if (s != TD_OK) return s;
+    ++*launches;
+    L <<= 12; q = 4;
+  }
+  for (; q < np; ++q) {
     td_status s = launch_pass<false>(16, base, narr, n, L, T, TW, st);
     if (s != TD_OK) return s;
     ++*launches;
@@ -287,20 +310,13 @@ td_status launch_cluster(td_handle* h, const FusedParams& P, const cplx* const* 
 
 template <int LOG2M, int MODE>
 td_status launch_fused_t(td_handle* h, const FusedParams& P, cudaStream_t st) {
-  if constexpr (LOG2M == 12 && MODE == MODE_LOGLIKE) {  // experiment knobs (headline shape only)
-    static const int nt = getenv("TDLIKE_NT") ? atoi(getenv("TDLIKE_NT")) : 256;
-    static const int ilv = getenv("TDLIKE_ILV") ? atoi(getenv("TDLIKE_ILV")) : 1;
-    if (nt == 512) return launch_fused_nt<LOG2M, MODE, 512>(h, P, st);
-    if (!ilv) return launch_fused_nt<LOG2M, MODE, FUSED_NT, false>(h, P, st);
-  }
   return launch_fused_nt<LOG2M, MODE, FUSED_NT>(h, P, st);
 }
 
 template <int MODE>
 td_status launch_fused(td_handle* h, int log2M, const FusedParams& P, const cplx* const* Gp, cudaStream_t st) {
-  static const int v3 = getenv("TDLIKE_FUSED") ? atoi(getenv("TDLIKE_FUSED")) == 3 : 0;
   if (log2M == CLUSTER_LOG2M) return Gp ? launch_cluster<MODE>(h, P, Gp, st) : TD_EUNSUPPORTED;
-  if (!v3 && Gp) {
+  if (Gp) {
     switch (log2M) {
       case 10: return launch_fused4<10, MODE>(h, P, Gp, st);
       case 11: return launch_fused4<11, MODE>(h, P, Gp, st);
@@ -311,10 +327,7 @@ td_status launch_fused(td_handle* h, int log2M, const FusedParams& P, const cplx
   switch (log2M) {
     case 8: return launch_fused_t<8, MODE>(h, P, st);
     case 9: return launch_fused_t<9, MODE>(h, P, st);
-    case 10: return launch_fused_t<10, MODE>(h, P, st);
-    case 11: return launch_fused_t<11, MODE>(h, P, st);
-    case 12: return launch_fused_t<12, MODE>(h, P, st);
-    default: return TD_EUNSUPPORTED;
+    default: return TD_EUNSUPPORTED;  // M >= 1024 always has the padded generator copy (Gp) of td_create
   }
 }
 
