@@ -348,3 +348,52 @@ def test_probe_fp64_reports_plausible_peaks():
     dfma = tdb.probe_fp64(0)
     dmma = tdb.probe_fp64(1)
     assert 10.0 < dfma < 60.0 and 10.0 < dmma < 90.0
+
+
+# ------------------------------------------------------------------ full sizes, in the launch configuration bench.py times
+def _full_size_check(name, sample, oracle=None, path=None):
+    """The whole batch of config `name` goes through the library exactly as bench.py launches it; the oracle
+    recomputes the sampled rows one by one; every row is checked through properties that hold at any size:
+    finite, logL <= 0, and the bilinear identity -2 logL = <d,d> - 2 <d,h> + <h,h> (pin P11) with the cross
+    terms coming from td_inner_batch (a different kernel mode)."""
+    w = W.make(name)
+    idx = np.unique(np.concatenate([np.arange(0, w.B, max(1, w.B // sample)), [w.B - 1]]))
+    fn = oracle or O.loglike_batch
+    ref = fn(w.acf, w.seg_lengths, w.d, w.H[idx])
+    with tdb.TDLikelihood(w.acf, w.seg_lengths) as h:
+        if path is not None:
+            h.set_path(path)
+        d, H = _dev(w.d), _dev(w.H)
+        out = h.loglike_batch(d, H)
+        dh, hh = h.inner_batch(d, H)
+        dd = h.inner_batch(d, d[None, :])[1]
+        torch.cuda.synchronize()
+        out, dh, hh, dd = out.cpu().numpy(), dh.cpu().numpy(), hh.cpu().numpy(), float(dd.cpu().numpy()[0])
+    _assert_close(out[idx], ref, what=f"{name} full size, sampled rows")
+    assert np.all(np.isfinite(out)) and np.all(out <= 0.0)
+    scale = dd + hh
+    assert np.max(np.abs(-2.0 * out - (dd - 2.0 * dh + hh)) / scale) <= TOL, f"{name}: bilinear identity"
+    # template 0 is the injection: logL_0 = -1/2 n^T C^-1 n is chi-square distributed around -N/2 (pin P14)
+    n_tot = int(np.sum(w.seg_lengths))
+    assert abs(out[0] + 0.5 * n_tot) <= 5.0 * np.sqrt(0.5 * n_tot)
+
+
+def test_full_size_c2_headline():
+    _full_size_check("c2", sample=48)
+
+
+def test_full_size_c3_gapped():
+    _full_size_check("c3", sample=12)
+
+
+def test_full_size_c5_network():
+    _full_size_check("c5", sample=6)
+
+
+def test_full_size_c4_long():
+    _full_size_check("c4", sample=1, oracle=O.loglike_batch_solve_toeplitz)
+
+
+@pytest.mark.parametrize("name", ["d1", "d4"])
+def test_full_size_dense_regime(name):
+    _full_size_check(name, sample=64, path=tdb.TD_PATH_DENSE)
