@@ -107,31 +107,36 @@ template <int R> __device__ __forceinline__ void tw_powers(cplx w1, cplx (&w)[R]
 __host__ __device__ constexpr int plan_np(int n) { return (ilog2(n) + 3) / 4; }
 __host__ __device__ constexpr int plan_r1(int n) { return n >> (4 * (plan_np(n) - 1)); }
 
+__host__ __device__ __forceinline__ int ilog2_rt(int n) {
+#ifdef __CUDA_ARCH__
+  return 31 - __clz(n);
+#else
+  return ilog2(n);
+#endif
+}
 __host__ __device__ __forceinline__ int plan_pos(int k, int n) {
-  const int r1 = plan_r1(n);
-  int stride = n / r1;
-  int p = (k % r1) * stride;
-  k /= r1;
-  while (stride > 1) {
-    stride >>= 4;
-    p += (k & 15) * stride;
+  // n is a power of two: shifts and masks only (this runs per element in the staged untangle kernel)
+  const int logn = ilog2_rt(n), np = (logn + 3) >> 2, lr1 = logn - 4 * (np - 1);
+  int sh = logn - lr1;
+  int p = (k & ((1 << lr1) - 1)) << sh;
+  k >>= lr1;
+  while (sh > 0) {
+    sh -= 4;
+    p += (k & 15) << sh;
     k >>= 4;
   }
   return p;
 }
 // inverse map: frequency index held at position p
 __host__ __device__ __forceinline__ int plan_freq(int p, int n) {
-  const int r1 = plan_r1(n);
-  int stride = n / r1;
-  int k = p / stride;
-  p -= k * stride;
-  int mul = r1;
-  while (stride > 1) {
-    stride >>= 4;
-    const int dgt = p / stride;
-    p -= dgt * stride;
-    k += dgt * mul;
-    mul <<= 4;
+  const int logn = ilog2_rt(n), np = (logn + 3) >> 2, lr1 = logn - 4 * (np - 1);
+  int sh = logn - lr1;
+  int k = p >> sh;
+  int mul = lr1;
+  while (sh > 0) {
+    sh -= 4;
+    k += ((p >> sh) & 15) << mul;
+    mul += 4;
   }
   return k;
 }

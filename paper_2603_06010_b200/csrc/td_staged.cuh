@@ -60,6 +60,21 @@ __global__ void __launch_bounds__(LG_NT) lg_pass_kernel(cplx* base, int n, int L
 constexpr int LGB_NT = 256, LGB_N = 4096;
 constexpr size_t LGB_SMEM = sizeof(cplx) * SmemArr::padded(LGB_N);
 
+// the inverse (DIT) passes L = 16, 256, 4096 of one 4096-element block in shared memory (LGB_NT threads)
+__device__ __forceinline__ void block_inverse3(const SmemArr& A, int tid, const cplx* __restrict__ T, int TW) {
+  static_for<0, 3>([&](auto pp) {
+    constexpr int L = 16 << (4 * decltype(pp)::value), S = L / 16;
+    const int blk = tid / S, j = tid & (S - 1), b0 = blk * L + j;
+    cplx x[16];
+#pragma unroll
+    for (int q = 0; q < 16; ++q) x[q] = A.ld(b0 + q * S);
+    if constexpr (S > 1) dit16<true, true>(x, cconj(T[(size_t)j * (TW / L)]));
+    else dit16<true, false>(x, mk(1.0, 0.0));
+    static_for<0, 16>([&](auto t) { A.st(b0 + decltype(t)::value * S, x[brevR<16>(decltype(t)::value)]); });
+    __syncthreads();
+  });
+}
+
 template <bool FWD>
 __global__ void __launch_bounds__(LGB_NT, 2) lg_block_kernel(cplx* base, int n, const cplx* __restrict__ T, int TW) {
   extern __shared__ __align__(16) unsigned char lgb_raw[];
@@ -78,17 +93,7 @@ __global__ void __launch_bounds__(LGB_NT, 2) lg_block_kernel(cplx* base, int n, 
       __syncthreads();
     });
   } else {
-    static_for<0, 3>([&](auto pp) {
-      constexpr int L = 16 << (4 * decltype(pp)::value), S = L / 16;
-      const int blk = tid / S, j = tid & (S - 1), b0 = blk * L + j;
-      cplx x[16];
-#pragma unroll
-      for (int q = 0; q < 16; ++q) x[q] = A.ld(b0 + q * S);
-      if constexpr (S > 1) dit16<true, true>(x, cconj(T[(size_t)j * (TW / L)]));
-      else dit16<true, false>(x, mk(1.0, 0.0));
-      static_for<0, 16>([&](auto t) { A.st(b0 + decltype(t)::value * S, x[brevR<16>(decltype(t)::value)]); });
-      __syncthreads();
-    });
+    block_inverse3(A, tid, T, TW);
   }
 #pragma unroll
   for (int q = 0; q < LGB_N / LGB_NT; ++q) g[tid + q * LGB_NT] = A.ld(tid + q * LGB_NT);

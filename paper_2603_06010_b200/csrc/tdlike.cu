@@ -218,19 +218,22 @@ td_status run_staged(td_handle* h, const ClassInfo& cls, const SegHost& sg, cons
   CB = std::min<int64_t>(CB, 32767);  // grid.y = 2*CB arrays per pass
   const int rI = plan_r1(M), rF = plan_r1(nf);
   const int nblk = (M / rI + LG_NT - 1) / LG_NT;
-  td_status s = ensure_ws(h, (size_t)CB * 2 * nf, (size_t)CB * 2 * M, (size_t)CB * nblk * 2);
+  td_status s = ensure_ws(h, (size_t)CB * 2 * nf, (size_t)CB * 2 * M, (size_t)std::max<int64_t>(B, 1) * nblk * 2);
   if (s != TD_OK) return s;
   for (int64_t b0 = 0; b0 < B; b0 += CB) {
     const int cb = (int)std::min<int64_t>(CB, B - b0);
     StagedParams P;
     P.d = d; P.H = H ? H + b0 * ldh : nullptr; P.ldh = ldh; P.CB = cb;
     P.seg.off = sg.off; P.seg.n = sg.n; P.seg._pad = 0; P.seg.G = sg.G; P.seg.zd = sg.zd;
-    P.M = M; P.U = h->wsU; P.Z = h->wsZ; P.T = cls.T; P.partial = h->wsPartial; P.nblk = nblk;
+    P.M = M; P.U = h->wsU; P.Z = h->wsZ; P.T = cls.T; P.partial = h->wsPartial + (size_t)b0 * nblk * 2; P.nblk = nblk;
     s = launch_first<MODE>(rF, dim3((nf / rF + LG_NT - 1) / LG_NT, cb), P, st);
     if (s != TD_OK) return s;
     ++h->last_launches;
     s = staged_forward(h->wsU, 2 * cb, nf, 1, cls.T, TW, st, &h->last_launches);
     if (s != TD_OK) return s;
+    // (fusing the untangle into the inverse block kernel - one CTA building a block, or a mirror pair of blocks, of Z in
+    // shared memory straight from U and G - was measured: 50-68 us per chunk against 18 + 24 us for the two kernels; the
+    // gather serialises 16 index-heavy tasks per thread, which the stand-alone kernel hides behind 1.4 M threads)
     lg_untangle_kernel<<<dim3((nf + LG_NT - 1) / LG_NT, 2, cb), LG_NT, 0, st>>>(P);
     CK(cudaGetLastError());
     ++h->last_launches;
@@ -239,12 +242,11 @@ td_status run_staged(td_handle* h, const ClassInfo& cls, const SegHost& sg, cons
     s = launch_last<MODE>(rI, dim3(nblk, cb), P, st);
     if (s != TD_OK) return s;
     ++h->last_launches;
-    if (MODE != MODE_STOREZ) {
-      lg_finish_kernel<<<(cb + 127) / 128, 128, 0, st>>>(h->wsPartial, nblk, cb, out0 ? out0 + b0 : nullptr,
-                                                        out1 ? out1 + b0 : nullptr, scale0, scale1, accumulate);
-      CK(cudaGetLastError());
-      ++h->last_launches;
-    }
+  }
+  if (MODE != MODE_STOREZ && B > 0) {  // one reduction of the per-block partial sums for the whole batch (fixed order)
+    lg_finish_kernel<<<(unsigned)((B + 127) / 128), 128, 0, st>>>(h->wsPartial, nblk, (int)B, out0, out1, scale0, scale1, accumulate);
+    CK(cudaGetLastError());
+    ++h->last_launches;
   }
   return TD_OK;
 }
