@@ -187,8 +187,10 @@ def main():
     if args.probe_peaks:
         if rank == 0:
             names = {0: "dfma", 1: "dmma_m8n8k4", 2: "dfma_and_dmma_interleaved", 3: "dadd"}
+            phase = {f"{nt}thr_{g}grp": tdb.probe_phase(nt, g, local)
+                     for nt, g in ((256, 1), (256, 2), (256, 8), (512, 1), (512, 2), (512, 16))}
             print(json.dumps({"fp64_tflops": {names[k]: tdb.probe_fp64(k, local) for k in range(4)},
-                              "derived_peak": FP64_PEAK_TFLOPS}))
+                              "derived_peak": FP64_PEAK_TFLOPS, "phase_cycles": phase}))
         return
 
     w = W.make(args.config, B=args.B)

@@ -132,6 +132,13 @@ int td_last_launches(const td_handle* h);
  * legacy default stream.  Errors: TD_EINVAL, TD_ECUDA. */
 td_status td_probe_fp64(int kind, int device, double* tflops);
 
+/* td_probe_phase - one "phase" of the fused FFT kernels in isolation (evidence for DESIGN.md 6.1): a CTA of `threads`
+ * threads pushes 2 x 4096 complex through 512 radix-16 shared-memory tasks per phase, with a barrier over the whole CTA
+ * (groups = 1) or only inside each of `groups` independent thread groups.  cycles (HOST pointer) receives the SM cycles
+ * per phase of one CTA running alone.  Supported (threads, groups): (256,1) (256,2) (256,8) (512,1) (512,2) (512,16);
+ * anything else returns TD_EINVAL.  Synchronous; legacy default stream. */
+td_status td_probe_phase(int threads, int groups, int device, double* cycles);
+
 /* td_strerror - static string for a status code. */
 const char* td_strerror(td_status s);
 

@@ -32,6 +32,7 @@ SYMBOLS = {
     "td_get_generator": (_INT, [_VP, _INT, _DP]),
     "td_last_launches": (_INT, [_VP]),
     "td_probe_fp64": (_INT, [_INT, _INT, _DP]),
+    "td_probe_phase": (_INT, [_INT, _INT, _INT, _DP]),
     "td_strerror": (C.c_char_p, [_INT]),
 }
 
@@ -200,6 +201,13 @@ def probe_fp64(kind: int, device: int = 0) -> float:
     """TFLOP/s of a register-resident fp64 loop (0 DFMA, 1 DMMA m8n8k4, 2 both, 3 DADD)."""
     v = C.c_double()
     _check(load().td_probe_fp64(int(kind), int(device), C.byref(v)), "td_probe_fp64")
+    return float(v.value)
+
+
+def probe_phase(threads: int, groups: int, device: int = 0) -> float:
+    """SM cycles per isolated radix-16 shared-memory phase (see td_probe_phase in include/tdlike.h)."""
+    v = C.c_double()
+    _check(load().td_probe_phase(int(threads), int(groups), int(device), C.byref(v)), "td_probe_phase")
     return float(v.value)
 
 

@@ -108,6 +108,7 @@ __global__ void __launch_bounds__(ClusterShape::NT, 1) td_cluster_kernel(const F
   cplx* xbuf = Z.p;                                        // exchange buffer [16][256] in the Z region
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int br = (int)cluster_ctarank();                   // branch: 0 even bins, 1 odd bins
+  const F4Own own = f4_own<Sh::RF1, true>(br, (int)(threadIdx.x >> 5));
   const uint32_t xbuf_remote = map_to_cta(smem_u32(xbuf), (uint32_t)(br ^ 1));
   const uint32_t xsum_remote = map_to_cta(smem_u32(xsum), 0u);
   const long long ncl = gridDim.x >> 1;
@@ -229,12 +230,12 @@ __global__ void __launch_bounds__(ClusterShape::NT, 1) td_cluster_kernel(const F
     }
     __syncthreads();
     // ---------------- forward passes 2 and 3, warp-local
-    f4_forward23<TW>(U, warp, lane, tw);
-    __syncthreads();
+    f4_forward23<TW>(U, own, lane, tw);
+    __syncwarp();  // mirror-closed ownership (f4_own): mid reads only this warp's U blocks
     // ---------------- mid: untangle x generator (in place in Z) -> first inverse pass
     mbar_wait(mbar_g, par_g);
     par_g ^= 1;
-    f4_mid<NF, Sh::RF1>(U, Z, br, warp, lane, tw);
+    f4_mid<NF, Sh::RF1>(U, Z, br, own, lane, tw);
     __syncwarp();
     if (lane == 0) {
       const int old = atomicAdd(mid_count, 1);
@@ -246,7 +247,7 @@ __global__ void __launch_bounds__(ClusterShape::NT, 1) td_cluster_kernel(const F
     bool staged_next = false;
     if (have_next) { const double *dr, *hr; int nn; staged_next = rows(nb, ns, dr, hr, nn); }
     // ---------------- inverse pass 2 (L = 256), warp-local
-    f4_inverse2<TW>(Z, warp, lane, tw);
+    f4_inverse2<TW>(Z, own, lane, tw);
     __syncthreads();
     // ---------------- last inverse pass: radix 32 on this branch, exchange halves, fused S5
     double acc0 = 0.0, acc1 = 0.0;

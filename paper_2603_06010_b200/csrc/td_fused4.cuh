@@ -28,7 +28,7 @@ template <int LOG2M> struct Fused4Shape {
   static constexpr int TWS = 2 * M / RF1;
   static constexpr int PADM = SmemArr::padded(M), PADNF = SmemArr::padded(NF);
   static constexpr size_t smem_bytes() {
-    return sizeof(cplx) * (2 * (size_t)PADNF + 2 * (size_t)PADM + TWS) + sizeof(double) * 2 * NW + 32;
+    return sizeof(cplx) * (2 * (size_t)PADNF + 2 * (size_t)PADM + TWS) + sizeof(double) * 2 * NW + 48;
   }
 };
 
@@ -41,12 +41,28 @@ struct Fused4Params {
 // All three work on ONE branch (U, Z of that branch); wb = index of the warp within the branch,
 // TW = 2M, RF1 = first forward radix (forward blocks of 256: RF1 per branch), RI1 = 2 RF1.
 
-// forward passes 2 and 3, warp-local (this warp owns blocks s1 = 2wb, 2wb+1 of its branch)
+// Which 256-element blocks a warp owns.  Plain: U blocks {2wb, 2wb+1}, Z blocks {4wb .. 4wb+3}.  Mirror-closed (MC): the
+// forward bins of U block r are k = r (mod RF1) and the untangle pairs k with -k (even branch) or -1-k (odd branch), so a
+// warp that owns {r, mirror(r)} reads only its own blocks in mid, and the Z blocks it fills there, {r, r+RF1, m, m+RF1},
+// are the ones it transforms in inverse pass 2: forward passes 2-3, mid and inverse pass 2 form ONE warp-local stretch
+// with no CTA or branch barrier inside (profiles/r01_peaks.md, phase probe: barrier-free groups overlap loads, butterflies
+// and stores of different warps; a barrier per pass costs ~25 %).
+struct F4Own { int u0, u1, z0, z1, z2, z3; };
+template <int RF1, bool MC> __device__ __forceinline__ F4Own f4_own(int br, int wb) {
+  if constexpr (!MC) return F4Own{2 * wb, 2 * wb + 1, 4 * wb, 4 * wb + 1, 4 * wb + 2, 4 * wb + 3};
+  else {
+    const int r = wb;
+    const int m = br ? RF1 - 1 - wb : (wb == 0 ? RF1 / 2 : RF1 - wb);
+    return F4Own{r, m, r, m, r + RF1, m + RF1};
+  }
+}
+
+// forward passes 2 and 3, warp-local (this warp owns U blocks o.u0, o.u1 of its branch)
 template <int TW>
-__device__ __forceinline__ void f4_forward23(const SmemArr& U, int wb, int lane, const cplx* __restrict__ tw) {
+__device__ __forceinline__ void f4_forward23(const SmemArr& U, const F4Own& o, int lane, const cplx* __restrict__ tw) {
   cplx x[16], w[16];
   {
-    const int s1 = 2 * wb + (lane >> 4), j = lane & 15;
+    const int s1 = (lane >> 4) ? o.u1 : o.u0, j = lane & 15;
     const int base = s1 * 256 + j;
     tw_powers<16>(tw[j * (TW / 256)], w);
 #pragma unroll
@@ -65,7 +81,7 @@ __device__ __forceinline__ void f4_forward23(const SmemArr& U, int wb, int lane,
     // loads (block s1'*16 + s2') and the stores are bank-conflict free.  The result block is
     // stored at the warp-owned slot s1'*16 + (s2' >> 1) + 8 (s2' & 1) ("mid layout": the 8 blocks
     // one quarter-warp of mid reads are consecutive), hence all loads precede all stores.
-    const int s1p = 2 * wb + (lane >> 4);
+    const int s1p = (lane >> 4) ? o.u1 : o.u0;
     const int s2p = (lane & 15) ^ ((lane & 1) << 3);
     const int src = (s1p * 16 + s2p) * 16;
     const int dst = (s1p * 16 + (s2p >> 1) + 8 * (s2p & 1)) * 16;
@@ -79,10 +95,11 @@ __device__ __forceinline__ void f4_forward23(const SmemArr& U, int wb, int lane,
 
 // mid: untangle (registers) x generator (in place in Z) -> first inverse pass
 template <int NF, int RF1>
-__device__ __forceinline__ void f4_mid(const SmemArr& U, const SmemArr& Z, int br, int wb, int lane,
+__device__ __forceinline__ void f4_mid(const SmemArr& U, const SmemArr& Z, int br, const F4Own& o, int lane,
                                        const cplx* __restrict__ tw) {
   constexpr int RI1 = 2 * RF1;
-  const int s1 = 4 * wb + (lane >> 3), s2 = lane & 7;
+  const int q4 = lane >> 3;
+  const int s1 = q4 == 0 ? o.z0 : q4 == 1 ? o.z1 : q4 == 2 ? o.z2 : o.z3, s2 = lane & 7;
   const int kap = s1 + RI1 * s2;  // forward low-part kappa = inverse block index tau
   int kap2;
   bool selfzero = false;
@@ -120,11 +137,11 @@ __device__ __forceinline__ void f4_mid(const SmemArr& U, const SmemArr& Z, int b
 
 // inverse pass 2 (L = 256), warp-local: blocks s1 = 4wb .. 4wb+3
 template <int TW>
-__device__ __forceinline__ void f4_inverse2(const SmemArr& Z, int wb, int lane, const cplx* __restrict__ tw) {
+__device__ __forceinline__ void f4_inverse2(const SmemArr& Z, const F4Own& o, int lane, const cplx* __restrict__ tw) {
   cplx x[16], y[16];
   const int j = lane & 15;
   const cplx w1 = cconj(tw[j * (TW / 256)]);  // the inverse transform's w_256^(-j); its powers are built inside dit16
-  const int base0 = (4 * wb + (lane >> 4)) * 256 + j, base1 = base0 + 2 * 256;
+  const int base0 = ((lane >> 4) ? o.z1 : o.z0) * 256 + j, base1 = ((lane >> 4) ? o.z3 : o.z2) * 256 + j;
 #pragma unroll
   for (int q = 0; q < 16; ++q) { x[q] = Z.ld(base0 + 16 * q); y[q] = Z.ld(base1 + 16 * q); }
   dit16<true, true>(x, w1);
@@ -148,14 +165,17 @@ __global__ void __launch_bounds__(Fused4Shape<LOG2M>::NT, 1) td_fused4_kernel(co
   const uint32_t mbar_rows = smem_u32(red + 2 * NW);
   const uint32_t mbar_g = mbar_rows + 8;
   int* mid_count = reinterpret_cast<int*>(red + 2 * NW + 2);
+  int* last_count = mid_count + 1;
+  double* totS = red + 2 * NW + 3;  // running sums of the current template over its segments
   double* stH = reinterpret_cast<double*>(sm);
   double* stD = stH + M;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int br = warp / NWB, wb = warp - br * NWB;  // branch (0 even bins, 1 odd bins), warp within branch
   const SmemArr U = br ? UO : UE, Z = br ? ZO : ZE;
+  const F4Own own = f4_own<RF1, true>(br, wb);
 
   for (int k = tid; k < Sh::TWS; k += NT) tw[k] = P.T[k];
-  if (tid == 0) { mbar_init(mbar_rows, 1); mbar_init(mbar_g, 1); *mid_count = 0; }
+  if (tid == 0) { mbar_init(mbar_rows, 1); mbar_init(mbar_g, 1); *mid_count = 0; *last_count = 0; totS[0] = 0.0; totS[1] = 0.0; }
   __syncthreads();
 
   auto rows = [&](long long b, int s, const double*& drow, const double*& hrow, int& n) -> bool {
@@ -195,7 +215,6 @@ __global__ void __launch_bounds__(Fused4Shape<LOG2M>::NT, 1) td_fused4_kernel(co
     staged = rows(b, s, dr, hr, nn);
     if (tid == 0) { prefetch_rows(b, s); prefetch_g(s); }
   }
-  double tot0 = 0.0, tot1 = 0.0;
   while (have) {
     long long nb = b; int ns = s + 1;
     if (ns == P.n_seg) { ns = 0; nb = b + gridDim.x; }
@@ -225,12 +244,12 @@ __global__ void __launch_bounds__(Fused4Shape<LOG2M>::NT, 1) td_fused4_kernel(co
     }
     __syncthreads();
     // ---------------- forward passes 2 and 3, warp-local
-    f4_forward23<TW>(U, wb, lane, tw);
-    asm volatile("bar.sync %0, %1;" ::"r"(1 + br), "r"(NT / 2) : "memory");  // mid reads mirror blocks of the SAME branch only
+    f4_forward23<TW>(U, own, lane, tw);
+    __syncwarp();  // mirror-closed ownership: mid reads only this warp's U blocks
     // ---------------- mid: untangle (registers) x generator (in place in Z) -> first inverse pass
     mbar_wait(mbar_g, par_g);
     par_g ^= 1;
-    f4_mid<NF, RF1>(U, Z, br, wb, lane, tw);
+    f4_mid<NF, RF1>(U, Z, br, own, lane, tw);
     // the warp finishing mid last knows the U region is dead: it prefetches the next item's rows
     __syncwarp();
     if (lane == 0) {
@@ -243,7 +262,7 @@ __global__ void __launch_bounds__(Fused4Shape<LOG2M>::NT, 1) td_fused4_kernel(co
     bool staged_next = false;
     if (have_next) { const double *dr, *hr; int nn; staged_next = rows(nb, ns, dr, hr, nn); }
     // ---------------- inverse pass 2 (L = 256), warp-local
-    f4_inverse2<TW>(Z, wb, lane, tw);
+    f4_inverse2<TW>(Z, own, lane, tw);
     __syncthreads();
     // ---------------- last inverse pass (radix RI1, joins the branches) + pruned radix-2 stage + S5
     double acc0 = 0.0, acc1 = 0.0;
@@ -252,23 +271,35 @@ __global__ void __launch_bounds__(Fused4Shape<LOG2M>::NT, 1) td_fused4_kernel(co
     if (MODE != MODE_STOREZ) {
       acc0 = warp_sum(acc0);
       acc1 = warp_sum(acc1);
-      if (lane == 0) { red[2 * warp] = acc0; red[2 * warp + 1] = acc1; }
     }
-    __syncthreads();  // Z fully consumed
-    if (tid == 0) {
-      if (have_next) prefetch_g(ns);
-      if (MODE != MODE_STOREZ) {
+    // No CTA barrier at the end of an item: the warp that finishes the last pass last (a counter, as for mid) knows
+    // that Z is consumed and every partial sum is in place; it prefetches the next generator spectrum into Z and
+    // finishes the reduction (fixed order over the warps), while the other warps are already loading the next item's
+    // staged rows.  `red` is rewritten only after the next item's barriers, which this warp has to pass as well.
+    __syncwarp();
+    if (lane == 0) {
+      if (MODE != MODE_STOREZ) { red[2 * warp] = acc0; red[2 * warp + 1] = acc1; }
+      __threadfence_block();
+      const int old = atomicAdd(last_count, 1);
+      if (old == NW - 1) {
+        *last_count = 0;
+        __threadfence_block();
+        if (have_next) prefetch_g(ns);
+        if (MODE != MODE_STOREZ) {
+          double tot0 = totS[0], tot1 = totS[1];
 #pragma unroll
-        for (int wq = 0; wq < NW; ++wq) { tot0 += red[2 * wq]; tot1 += red[2 * wq + 1]; }
-        if (s == P.n_seg - 1) {
-          if (MODE == MODE_LOGLIKE) {
-            const double v = -0.5 * tot1;
-            P.out0[b] = P.accumulate ? P.out0[b] + v : v;
-          } else {
-            if (P.out0) P.out0[b] = P.accumulate ? P.out0[b] + tot0 : tot0;
-            if (P.out1) P.out1[b] = P.accumulate ? P.out1[b] + tot1 : tot1;
+          for (int wq = 0; wq < NW; ++wq) { tot0 += red[2 * wq]; tot1 += red[2 * wq + 1]; }
+          if (s == P.n_seg - 1) {
+            if (MODE == MODE_LOGLIKE) {
+              const double v = -0.5 * tot1;
+              P.out0[b] = P.accumulate ? P.out0[b] + v : v;
+            } else {
+              if (P.out0) P.out0[b] = P.accumulate ? P.out0[b] + tot0 : tot0;
+              if (P.out1) P.out1[b] = P.accumulate ? P.out1[b] + tot1 : tot1;
+            }
+            tot0 = 0.0; tot1 = 0.0;
           }
-          tot0 = 0.0; tot1 = 0.0;
+          totS[0] = tot0; totS[1] = tot1;
         }
       }
     }

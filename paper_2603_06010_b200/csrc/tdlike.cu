@@ -762,6 +762,40 @@ td_status td_probe_fp64(int kind, int device, double* tflops) {
   return TD_OK;
 }
 
+td_status td_probe_phase(int threads, int groups, int device, double* cycles) {
+  if (!cycles) return TD_EINVAL;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return TD_ECUDA;
+  if (device < 0 || device >= ndev) return TD_EINVAL;
+  void (*kern)(double*, long long*, int, const cplx*) = nullptr;
+  if (threads == 256 && groups == 1) kern = probe_phase_kernel<256, 1>;
+  else if (threads == 256 && groups == 2) kern = probe_phase_kernel<256, 2>;
+  else if (threads == 256 && groups == 8) kern = probe_phase_kernel<256, 8>;
+  else if (threads == 512 && groups == 1) kern = probe_phase_kernel<512, 1>;
+  else if (threads == 512 && groups == 2) kern = probe_phase_kernel<512, 2>;
+  else if (threads == 512 && groups == 16) kern = probe_phase_kernel<512, 16>;
+  else return TD_EINVAL;
+  DevGuard guard(device);
+  if (!guard.ok) return TD_ECUDA;
+  const size_t smem = sizeof(cplx) * SmemArr::padded(8192);
+  CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  double* sink = nullptr; long long* cyc = nullptr; cplx* T = nullptr;
+  std::vector<cplx> hT(512);
+  for (int i = 0; i < 512; ++i) hT[i] = mk(std::cos(2.0 * M_PI * i / 8192.0), -std::sin(2.0 * M_PI * i / 8192.0));
+  td_status rc = TD_OK;
+  if (cudaMalloc(&sink, 8) != cudaSuccess || cudaMalloc(&cyc, 8) != cudaSuccess || cudaMalloc(&T, sizeof(cplx) * 512) != cudaSuccess) rc = TD_ENOMEM;
+  long long c = 0;
+  if (rc == TD_OK) {
+    const int iters = 200;
+    cudaMemcpy(T, hT.data(), sizeof(cplx) * 512, cudaMemcpyHostToDevice);
+    for (int rep = 0; rep < 2; ++rep) kern<<<1, threads, smem>>>(sink, cyc, iters, T);
+    if (cudaDeviceSynchronize() != cudaSuccess || cudaGetLastError() != cudaSuccess) rc = TD_ECUDA;
+    else { cudaMemcpy(&c, cyc, 8, cudaMemcpyDeviceToHost); *cycles = (double)c / iters; }
+  }
+  cudaFree(sink); cudaFree(cyc); cudaFree(T);
+  return rc;
+}
+
 int td_last_launches(const td_handle* h) { return h ? h->last_launches : 0; }
 
 }  // extern "C"
