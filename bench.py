@@ -160,6 +160,8 @@ def main():
     ap.add_argument("--B", type=int, default=None, help="override templates per GPU (default: the config's B)")
     ap.add_argument("--path", type=int, default=0, help="0 auto, 1 FFT, 2 dense")
     ap.add_argument("--fft-variant", type=int, default=0)
+    ap.add_argument("--op", default="loglike", choices=["loglike", "dh"],
+                    help="loglike: the headline hot path; dh: only the cross term <d|h_b> (td_inner_batch, out_hh = NULL)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--probe-peaks", action="store_true",
@@ -214,9 +216,17 @@ def main():
         if world > 1:
             dist.barrier()
 
+    if args.op == "dh":
+        def step(Hd):
+            h.inner_batch(d, Hd, want_hh=False, out_dh=out)
+        args.no_e2e = True
+    else:
+        def step(Hd):
+            h.loglike_batch(d, Hd, out=out)
+
     # ---------------- device-resident throughput
     for i in range(args.warmup):
-        h.loglike_batch(d, Hs[i % nbuf], out=out)
+        step(Hs[i % nbuf])
     torch.cuda.synchronize()
     barrier()
     sampler = ClockSampler(local)
@@ -230,7 +240,7 @@ def main():
     t_wall0 = time.time()
     evs[0].record(stream)
     for i in range(args.steps):
-        h.loglike_batch(d, Hs[i % nbuf], out=out)
+        step(Hs[i % nbuf])
         launches += h.last_launches()
         evs[i + 1].record(stream)
     torch.cuda.synchronize()
@@ -300,6 +310,13 @@ def main():
                 "kernel_ms": kern_ms, "alg_flops_per_eval": falg,
                 "peak_source": "derived: 64 DFMA/clk/SM x 148 SM x 1.965 GHz x 2 (DESIGN.md 6); the fp64 tensor pipe "
                                "(DMMA.8x8x4) has the same peak; register-loop measurements of this run beside it"}
+    if args.op == "dh":
+        # the cross term is one streaming pass over H: HBM is the bounding roofline; 2 flop per 8 bytes
+        roofline = {"bound": "hbm", "achieved": ach_gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                    "frac": ach_gbs / peaks["hbm_gbs"], "traffic": None, "kernel": "dot_rows_kernel",
+                    "kernel_ms": kern_ms, "peak_source": peaks_kind + " (MEASURED_PEAKS.json copy bandwidth); the step also "
+                    "holds the once-per-call setup kernels (z of d, weights u = C^-1 d)"}
+        args.no_cpu_baseline = True
     roofline_hbm = {"bound": "hbm", "achieved": ach_gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s",
                     "frac": ach_gbs / peaks["hbm_gbs"], "peak_source": peaks_kind + " (MEASURED_PEAKS.json copy bandwidth)",
                     "alg_bytes_per_eval": 8.0 * n_tot + 8.0}
@@ -313,11 +330,11 @@ def main():
         cpu = {"value": r, "unit": UNIT, "cores": th, "kind": "oracle", "sample": sample,
                "max_rel_err_gpu_vs_oracle": float(np.max(np.abs(got - ref) / np.maximum(np.abs(ref), 1.0)))}
 
-    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+    line = {"metric": METRIC if args.op == "loglike" else "fp64 cross-term <d|h_b> evals/sec (not the headline)", "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": f"{args.config}: {w.description}; N_tot={n_tot}, segments={list(map(int, w.seg_lengths))}, B={B} per GPU",
-                       "path": {1: "fft", 2: "dense"}.get(path_used, "?"),
+                       "path": {1: "fft", 2: "dense", 3: "dot"}.get(path_used, "?"),
                        "l2": f"{nbuf} distinct device copies of H rotated between steps (H = {8 * B * n_tot / 2**20:.0f} MiB each)",
                        "parallelism": f"dp{world} over templates"},
             "roofline": roofline, "roofline_hbm": roofline_hbm, "cpu_baseline": cpu, "e2e": e2e,

@@ -38,7 +38,8 @@ typedef enum {
 /* td_path: evaluation path selector for td_set_path / reported by td_get_info.
  * TD_PATH_AUTO: per size class, the dense path for short segments (measured crossover, DESIGN.md
  * 6.4), the FFT path otherwise; both accumulate into the same outputs within one call. */
-enum { TD_PATH_AUTO = 0, TD_PATH_FFT = 1, TD_PATH_DENSE = 2 };
+enum { TD_PATH_AUTO = 0, TD_PATH_FFT = 1, TD_PATH_DENSE = 2,
+       TD_PATH_DOT = 3 /* reported by td_get_info only: <d,h_b> evaluated as u . h_b, u = C^{-1} d */ };
 
 /* td_create - one-time setup (PAPER.md:215 "done once ... cached"; :241-246 Eq. 14 generator).
  *   acf          HOST pointer, sum_s seg_lengths[s] doubles: per-segment autocorrelation
@@ -81,6 +82,9 @@ td_status td_loglike_batch(td_handle* h, const double* d, const double* H, int64
  * both summed over segments.  Either output may be NULL (not computed / not written).
  * Same layouts, ownership and stream semantics as td_loglike_batch.
  * Identity: -2 * loglike[b] = <d,d> - 2 <d,h_b> + <h_b,h_b>;  <d,d> is td_inner_batch with H = d, B = 1.
+ * With out_hh == NULL under TD_PATH_AUTO (segments up to 16384 samples) the cross term is evaluated as the batched dot
+ * product u . h_b against u = C^{-1} d, computed once per call from the Gohberg-Semencul form (the paper's cached
+ * whitened data, :225, :306, taken one step further): one pass over H, HBM-bound; td_get_info then reports TD_PATH_DOT.
  */
 td_status td_inner_batch(td_handle* h, const double* d, const double* H, int64_t ldh,
                          int64_t B, double* out_dh, double* out_hh, void* stream);
@@ -111,7 +115,7 @@ td_status td_set_fft_variant(td_handle* h, int variant);
  *   v          HOST array [n_seg]: prediction-error variance v_s = 1/(C_s^{-1})_{00}
  *   logdet     HOST array [n_seg]: log det C_s = sum_k log E_k
  *   last_path  path actually used by the last batch call (0 if none yet): TD_PATH_DENSE if every
- *              segment went through the dense kernel, TD_PATH_FFT otherwise
+ *              segment went through the dense kernel, TD_PATH_DOT for the dot-product cross term, TD_PATH_FFT otherwise
  */
 td_status td_get_info(const td_handle* h, int64_t* n_tot, int* n_seg, double* v, double* logdet,
                       int* last_path);

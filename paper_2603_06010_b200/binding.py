@@ -16,7 +16,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "lib", "libtdlike.so")
 
 TD_OK, TD_EINVAL, TD_ENOTSPD, TD_ENOMEM, TD_ECUDA, TD_EUNSUPPORTED = range(6)
-TD_PATH_AUTO, TD_PATH_FFT, TD_PATH_DENSE = 0, 1, 2
+TD_PATH_AUTO, TD_PATH_FFT, TD_PATH_DENSE, TD_PATH_DOT = 0, 1, 2, 3
 
 # every symbol include/tdlike.h declares: name -> (restype, argtypes)
 _VP, _I64, _INT, _DP = C.c_void_p, C.c_int64, C.c_int, C.POINTER(C.c_double)
@@ -143,11 +143,12 @@ class TDLikelihood:
         _check(st, "td_loglike_batch")
         return out
 
-    def inner_batch(self, d, H, want_dh: bool = True, want_hh: bool = True, stream=None):
-        """(<d,h_b>, <h_b,h_b>) summed over segments (Eq. 13 terms)."""
+    def inner_batch(self, d, H, want_dh: bool = True, want_hh: bool = True, stream=None, out_dh=None):
+        """(<d,h_b>, <h_b,h_b>) summed over segments (Eq. 13 terms).  want_hh=False: only the cross term, which
+        under TD_PATH_AUTO is one streaming pass over H (u . h_b, u = C^-1 d)."""
         import torch
         B, ldh = int(H.shape[0]), int(H.stride(0)) if H.shape[0] > 1 else max(int(H.stride(0)), int(H.shape[1]))
-        dh = torch.empty(B, dtype=torch.float64, device=H.device) if want_dh else None
+        dh = (out_dh if out_dh is not None else torch.empty(B, dtype=torch.float64, device=H.device)) if want_dh else None
         hh = torch.empty(B, dtype=torch.float64, device=H.device) if want_hh else None
         st = self._lib.td_inner_batch(self._h, _ptr(d, "d", self.device), _ptr(H, "H", self.device), ldh, B,
                                       _ptr(dh, "dh") if want_dh else None, _ptr(hh, "hh") if want_hh else None,

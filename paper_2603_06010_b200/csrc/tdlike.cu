@@ -12,6 +12,7 @@
 #include <vector>
 
 #include "td_dense.cuh"
+#include "td_dot.cuh"
 #include "td_fused.cuh"
 #include "td_cluster.cuh"
 #include "td_fused4.cuh"
@@ -71,6 +72,7 @@ struct td_handle {
   int max_n = 0;
   // staged workspace (grow-only)
   cplx* wsU = nullptr; cplx* wsZ = nullptr; double* wsPartial = nullptr;
+  double* ud = nullptr;  // [n_tot] weights u = C^{-1} d of the dot path (td_dot.cuh), lazily allocated
   size_t wsU_elems = 0, wsZ_elems = 0, wsP_elems = 0;
   // dense path state
   DenseState dense;
@@ -99,7 +101,7 @@ void free_handle(td_handle* h) {
   if (!h) return;
   for (auto& s : h->segs) { cudaFree(s.a); cudaFree(s.G); cudaFree(s.Gp); cudaFree(s.zd); }
   for (auto& c : h->classes) { cudaFree(c.T); cudaFree(c.d_segs); cudaFree(c.d_Gp); }
-  cudaFree(h->wsU); cudaFree(h->wsZ); cudaFree(h->wsPartial);
+  cudaFree(h->wsU); cudaFree(h->wsZ); cudaFree(h->wsPartial); cudaFree(h->ud);
   cudaFree(h->hsD); cudaFree(h->hsH[0]); cudaFree(h->hsH[1]); cudaFree(h->hsOut);
   if (h->copy_stream) cudaStreamDestroy(h->copy_stream);
   for (int i = 0; i < 2; ++i) { if (h->ev_copied[i]) cudaEventDestroy(h->ev_copied[i]); if (h->ev_done[i]) cudaEventDestroy(h->ev_done[i]); }
@@ -445,6 +447,36 @@ td_status run_batch(td_handle* h, const double* d, const double* H, int64_t ldh,
   return run_fft_path<MODE>(h, d, H, ldh, B, out0, out1, st, true, accumulate);
 }
 
+// <d, h_b> = u . h_b with u = C^{-1} d (td_dot.cuh); z of the data vector is already in every segment's zd
+td_status run_dot(td_handle* h, const double* H, int64_t ldh, int64_t B, double* out_dh, cudaStream_t st) {
+  if (!h->ud) CK(cudaMalloc(&h->ud, sizeof(double) * (size_t)h->n_tot));
+  {
+    size_t need = 0;  // per-tile partial weights of the longest segment: ntile rows of ntile * 128 doubles
+    for (const SegHost& sg : h->segs) { const size_t nt = (sg.n + DOTW_NT - 1) / DOTW_NT; need = std::max(need, nt * nt * DOTW_NT); }
+    td_status s = ensure_ws(h, 0, 0, need);
+    if (s != TD_OK) return s;
+  }
+  for (const SegHost& sg : h->segs) {
+    const int nt = (int)((sg.n + DOTW_NT - 1) / DOTW_NT);
+    dot_weight_tile_kernel<<<(unsigned)(nt * (nt + 1) / 2), DOTW_NT, 0, st>>>(sg.a, sg.zd, (int)sg.n, h->wsPartial, nt);
+    CK(cudaGetLastError());
+    dot_weight_sum_kernel<<<(unsigned)((sg.n + 255) / 256), 256, 0, st>>>(h->wsPartial, (int)sg.n, nt, 1.0 / std::sqrt(sg.v), h->ud + sg.off);
+    CK(cudaGetLastError());
+    h->last_launches += 2;
+  }
+  const bool vec = (ldh % 2 == 0) && ((reinterpret_cast<uintptr_t>(H) & 15) == 0);
+  void (*kern)(const double*, const double*, long long, long long, int, double*, int) =
+      vec ? dot_rows_kernel<true> : dot_rows_kernel<false>;
+  int nb = 0;
+  CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kern, DOT_NT, 0));
+  const unsigned grid = (unsigned)std::max<int64_t>(1, std::min<int64_t>((B + 1) / 2, (int64_t)std::max(nb, 1) * h->num_sms));
+  kern<<<grid, DOT_NT, 0, st>>>(h->ud, H, ldh, B, (int)h->n_tot, out_dh, 0);
+  CK(cudaGetLastError());
+  ++h->last_launches;
+  h->last_path = TD_PATH_DOT;
+  return TD_OK;
+}
+
 }  // namespace
 
 // ------------------------------------------------------------------------------------------
@@ -690,6 +722,9 @@ td_status td_inner_batch(td_handle* h, const double* d, const double* H, int64_t
   }
   td_status s = run_fft_path<MODE_STOREZ>(h, d, nullptr, h->n_tot, 1, nullptr, nullptr, st);
   if (s != TD_OK) return s;
+  // only the cross term is wanted: one streaming pass over H against the cached weights u = C^{-1} d
+  if (out_dh && !out_hh && h->path == TD_PATH_AUTO && h->max_n <= DOT_MAX_N && h->n_tot <= 0x7fffffff)
+    return run_dot(h, H, ldh, B, out_dh, st);
   return run_batch<MODE_INNER>(h, d, H, ldh, B, out_dh, out_hh, st);
 }
 

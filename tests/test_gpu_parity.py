@@ -397,3 +397,41 @@ def test_full_size_c4_long():
 @pytest.mark.parametrize("name", ["d1", "d4"])
 def test_full_size_dense_regime(name):
     _full_size_check(name, sample=64, path=tdb.TD_PATH_DENSE)
+
+
+# ------------------------------------------------------------------ cross term as a batched dot product (td_dot.cuh)
+@pytest.mark.parametrize("name,B,n_scale", [("c1", 64, 1), ("c2", 40, 1), ("c3", 9, 1), ("c5", 5, 1), ("d2", 100, 1)])
+def test_cross_term_dot_path(name, B, n_scale):
+    """out_hh = NULL under AUTO: <d,h_b> = u . h_b with u = C^-1 d.  Against the oracle, and against the FFT kernels."""
+    w = W.make(name, B=B, n_scale=n_scale)
+    dh_ref, hh_ref = O.inner_batch(w.acf, w.seg_lengths, w.d, w.H)
+    dd = float(O.inner_batch(w.acf, w.seg_lengths, w.d, w.d[None, :])[1][0])
+    scale = dd + hh_ref
+    with tdb.TDLikelihood(w.acf, w.seg_lengths) as h:
+        d, H = _dev(w.d), _dev(w.H)
+        dh, none = h.inner_batch(d, H, want_hh=False)
+        assert none is None and h.info()["last_path"] == tdb.TD_PATH_DOT
+        dh2, _ = h.inner_batch(d, H, want_hh=False)
+        assert torch.equal(dh, dh2)                       # fixed summation order
+        h.set_path(tdb.TD_PATH_FFT)
+        dh_fft, _ = h.inner_batch(d, H, want_hh=False)
+        assert h.info()["last_path"] == tdb.TD_PATH_FFT
+    assert np.max(np.abs(dh.cpu().numpy() - dh_ref) / scale) <= TOL
+    assert np.max(np.abs(dh.cpu().numpy() - dh_fft.cpu().numpy()) / scale) <= TOL
+
+
+def test_cross_term_dot_path_unaligned_rows_and_odd_length():
+    rng = np.random.default_rng(11)
+    lens = [301, 1000, 77]
+    rho = W.acf_from_psd(4096.0, 2 * 8192, max(lens))
+    acf = np.concatenate([s * rho[:n] for s, n in zip([1.0, 0.7, 3.0], lens)])
+    nt = sum(lens)
+    d = rng.standard_normal(nt) * 1e-21
+    Hbig = rng.standard_normal((13, nt + 3)) * 1e-21     # odd leading dimension: scalar loads
+    H = Hbig[:, :nt]
+    dh_ref, hh_ref = O.inner_batch(acf, lens, d, H)
+    dd = float(O.inner_batch(acf, lens, d, d[None, :])[1][0])
+    with tdb.TDLikelihood(acf, lens) as h:
+        dh, _ = h.inner_batch(_dev(d), _dev(Hbig)[:, :nt], want_hh=False)
+        assert h.info()["last_path"] == tdb.TD_PATH_DOT
+    assert np.max(np.abs(dh.cpu().numpy() - dh_ref) / (dd + hh_ref)) <= TOL
