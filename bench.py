@@ -283,6 +283,33 @@ def main():
         max_dev = float(np.max(np.abs(out_host - out.cpu().numpy())))
         e2e["max_abs_diff_vs_device_call"] = max_dev
 
+    # ---------------- the same evaluations from template PARAMETERS on the host (td_loglike_ringdown_batch_host):
+    # 5 doubles per template cross the bus, the rows are synthesised on the device.  Extra key, not `e2e`.
+    e2e_params = None
+    if not args.no_e2e and args.op == "loglike" and w.params is not None and len(w.seg_lengths) == 1:
+        out_p = np.empty(B)
+        for _ in range(2):
+            h.loglike_ringdown_batch_host(w.d, w.params, w.fs, out_p)
+        torch.cuda.synchronize()
+        barrier()
+        k_p = max(3, min(args.steps, 10))
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(k_p):
+            h.loglike_ringdown_batch_host(w.d, w.params, w.fs, out_p)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        barrier()
+        ms = e0.elapsed_time(e1)
+        if world > 1:
+            t = torch.tensor([ms], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms = float(t.item())
+        e2e_params = {"value": world * B * k_p / (ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(40 * B + 8 * n_tot),
+                      "d2h_bytes_per_step": int(8 * B), "steps": k_p,
+                      "api": "td_loglike_ringdown_batch_host (host parameters (A, f, tau, phi, t0); templates synthesised on the device)",
+                      "max_rel_diff_vs_device_call": float(np.max(np.abs(out_p - out.cpu().numpy()) / np.maximum(np.abs(out_p), 1.0)))}
+
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -337,7 +364,7 @@ def main():
                        "path": {1: "fft", 2: "dense", 3: "dot"}.get(path_used, "?"),
                        "l2": f"{nbuf} distinct device copies of H rotated between steps (H = {8 * B * n_tot / 2**20:.0f} MiB each)",
                        "parallelism": f"dp{world} over templates"},
-            "roofline": roofline, "roofline_hbm": roofline_hbm, "cpu_baseline": cpu, "e2e": e2e,
+            "roofline": roofline, "roofline_hbm": roofline_hbm, "cpu_baseline": cpu, "e2e": e2e, "e2e_params": e2e_params,
             "gpu_launches": launches, "clocks": clocks}
     print(json.dumps(line))
     if world > 1:

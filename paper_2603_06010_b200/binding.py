@@ -26,6 +26,8 @@ SYMBOLS = {
     "td_loglike_batch": (_INT, [_VP, _VP, _VP, _I64, _I64, _VP, _VP]),
     "td_inner_batch": (_INT, [_VP, _VP, _VP, _I64, _I64, _VP, _VP, _VP]),
     "td_loglike_batch_host": (_INT, [_VP, _VP, _VP, _I64, _I64, _VP, _VP]),
+    "td_loglike_ringdown_batch": (_INT, [_VP, _VP, _VP, _I64, C.c_double, _VP, _VP]),
+    "td_loglike_ringdown_batch_host": (_INT, [_VP, _VP, _VP, _I64, C.c_double, _VP, _VP]),
     "td_set_path": (_INT, [_VP, _INT]),
     "td_set_fft_variant": (_INT, [_VP, _INT]),
     "td_get_info": (_INT, [_VP, C.POINTER(C.c_int64), C.POINTER(_INT), _DP, _DP, C.POINTER(_INT)]),
@@ -171,6 +173,33 @@ class TDLikelihood:
         st = self._lib.td_loglike_batch_host(self._h, d_host.ctypes.data, Hp, ldh, B, out_host.ctypes.data,
                                              _stream_ptr(stream, torch.device("cuda", self.device)))
         _check(st, "td_loglike_batch_host")
+        return out_host
+
+    def loglike_ringdown_batch(self, d, params, fs: float, out=None, stream=None):
+        """logL of damped-sinusoid templates given as rows (A, f, tau, phi, t0) of a CUDA float64 [B, 5] tensor."""
+        import torch
+        if params.dim() != 2 or params.shape[1] != 5 or not params.is_contiguous():
+            raise ValueError("params must be a contiguous [B, 5] tensor")
+        B = int(params.shape[0])
+        if out is None:
+            out = torch.empty(B, dtype=torch.float64, device=params.device)
+        st = self._lib.td_loglike_ringdown_batch(self._h, _ptr(d, "d", self.device), _ptr(params, "params", self.device), B,
+                                                 float(fs), _ptr(out, "out", self.device), _stream_ptr(stream, params.device))
+        _check(st, "td_loglike_ringdown_batch")
+        return out
+
+    def loglike_ringdown_batch_host(self, d_host: np.ndarray, params_host: np.ndarray, fs: float,
+                                    out_host: Optional[np.ndarray] = None, stream=None):
+        """Same from HOST arrays: 5 doubles per template cross the bus instead of N."""
+        import torch
+        params_host = np.ascontiguousarray(params_host, dtype=np.float64)
+        d_host = np.ascontiguousarray(d_host, dtype=np.float64)
+        B = int(params_host.shape[0])
+        if out_host is None:
+            out_host = np.empty(B, dtype=np.float64)
+        st = self._lib.td_loglike_ringdown_batch_host(self._h, d_host.ctypes.data, params_host.ctypes.data, B, float(fs),
+                                                      out_host.ctypes.data, _stream_ptr(stream, torch.device("cuda", self.device)))
+        _check(st, "td_loglike_ringdown_batch_host")
         return out_host
 
     # -- options / queries ---------------------------------------------------------------

@@ -104,6 +104,7 @@ class Workload:
     H: np.ndarray                # float64 [B, N_tot], row b = template b, same packing
     scales: np.ndarray           # float64 [n_seg] PSD scale of each segment
     description: str = ""
+    params: Optional[np.ndarray] = None   # float64 [B, 5] = (A, f, tau, phi, t0) where the rows of H are damped sinusoids
 
     @property
     def n_tot(self) -> int:
@@ -183,11 +184,13 @@ def make(name: str, B: Optional[int] = None, n_scale: int = 1) -> Workload:
         t0, snr = U(0.3, 0.7, B) * T, U(8, 30, B)
         t = np.arange(N) / fs
         H = np.empty((B, N))
+        amp = np.empty(B)
         for lo, hi in _chunks(B, N):
             h = _damped(t, f[lo:hi], tau[lo:hi], phi[lo:hi], t0[lo:hi])
-            H[lo:hi] = h * (snr[lo:hi] / _snr_fd(h, fs))[:, None]
+            amp[lo:hi] = snr[lo:hi] / _snr_fd(h, fs)
+            H[lo:hi] = h * amp[lo:hi, None]
         return Workload(name, seed, fs, np.array([N], np.int64), rho, n + H[0], H, np.ones(1),
-                        "single segment, damped sinusoids")
+                        "single segment, damped sinusoids", np.stack([amp, f, tau, phi, t0], axis=1))
 
     if name == "c3":
         fs = 4096.0
@@ -267,13 +270,15 @@ def make(name: str, B: Optional[int] = None, n_scale: int = 1) -> Workload:
         f, tau, phi, snr = U(150, 400, B), U(2e-3, 10e-3, B), U(0, 2 * np.pi, B), U(8, 30, B)
         t = np.arange(N) / fs
         H = np.empty((B, N))
+        amp = np.empty(B)
         # SNR estimate on a zero-padded 4096 grid so the FD estimate resolves the PSD
         for lo, hi in _chunks(B, 4096):
             h = _damped(t, f[lo:hi], tau[lo:hi], phi[lo:hi], np.zeros(hi - lo))
             hp = np.zeros((hi - lo, 4096))
             hp[:, :N] = h
-            H[lo:hi] = h * (snr[lo:hi] / _snr_fd(hp, fs))[:, None]
+            amp[lo:hi] = snr[lo:hi] / _snr_fd(hp, fs)
+            H[lo:hi] = h * amp[lo:hi, None]
         return Workload(name, seed, fs, np.array([N], np.int64), rho, n + H[0], H, np.ones(1),
-                        "ringdown-only short segment (dense-path regime)")
+                        "ringdown-only short segment (dense-path regime)", np.stack([amp, f, tau, phi, np.zeros(B)], axis=1))
 
     raise KeyError(name)

@@ -435,3 +435,39 @@ def test_cross_term_dot_path_unaligned_rows_and_odd_length():
         dh, _ = h.inner_batch(_dev(d), _dev(Hbig)[:, :nt], want_hh=False)
         assert h.info()["last_path"] == tdb.TD_PATH_DOT
     assert np.max(np.abs(dh.cpu().numpy() - dh_ref) / (dd + hh_ref)) <= TOL
+
+
+# ------------------------------------------------------------------ templates synthesised on the device (td_synth.cuh)
+@pytest.mark.parametrize("name,B", [("c1", 64), ("c2", 200), ("d2", 333)])
+def test_ringdown_params_entry_matches_oracle(name, B):
+    """td_loglike_ringdown_batch: rows (A, f, tau, phi, t0) instead of H.  The oracle sees the H numpy built from the
+    same parameters; the device and host entries must agree with it and with each other."""
+    w = W.make(name, B=B)
+    ref = O.loglike_batch(w.acf, w.seg_lengths, w.d, w.H)
+    with tdb.TDLikelihood(w.acf, w.seg_lengths) as h:
+        out = h.loglike_ringdown_batch(_dev(w.d), _dev(w.params), w.fs)
+        torch.cuda.synchronize()
+        assert h.last_launches() >= 2
+        out_host = h.loglike_ringdown_batch_host(w.d, w.params, w.fs)
+    _assert_close(out.cpu().numpy(), ref, what=f"{name} ringdown params")
+    assert np.array_equal(out.cpu().numpy(), out_host)
+
+
+def test_ringdown_params_entry_errors_and_edges():
+    w = W.make("c3", B=4)
+    with tdb.TDLikelihood(w.acf, w.seg_lengths) as h:
+        with pytest.raises(tdb.TDError) as e:
+            h.loglike_ringdown_batch(_dev(w.d), _dev(np.ones((4, 5))), w.fs)
+        assert e.value.status == tdb.TD_EUNSUPPORTED       # three segments: no single time axis
+    w = W.make("c1", B=5)
+    p = w.params.copy()
+    p[1, 4] = 2.0        # t0 beyond the segment: the template is identically zero -> logL = -1/2 <d,d>
+    p[2, 4] = -0.25      # t0 before the segment: live from the first sample
+    t = np.arange(w.n_tot) / w.fs
+    H = p[:, 0:1] * W._damped(t, p[:, 1], p[:, 2], p[:, 3], p[:, 4])
+    ref = O.loglike_batch(w.acf, w.seg_lengths, w.d, H)
+    with tdb.TDLikelihood(w.acf, w.seg_lengths) as h:
+        out = h.loglike_ringdown_batch(_dev(w.d), _dev(p), w.fs).cpu().numpy()
+        with pytest.raises(tdb.TDError):
+            h.loglike_ringdown_batch(_dev(w.d), _dev(p), 0.0)
+    _assert_close(out, ref, what="ringdown edges")
