@@ -471,3 +471,26 @@ def test_ringdown_params_entry_errors_and_edges():
         with pytest.raises(tdb.TDError):
             h.loglike_ringdown_batch(_dev(w.d), _dev(p), 0.0)
     _assert_close(out, ref, what="ringdown edges")
+
+
+@pytest.mark.parametrize("name,B", [("c1", 700), ("c2", 650)])
+def test_fused_many_items_per_cta_repeatable(name, B):
+    """More templates than SMs: every CTA loops over several items, with the counter-based hand-over between items
+    (no CTA barrier at the end of an item).  Bitwise repeatable, equal to the staged global-memory variant, and a
+    sample against the oracle.  (compute-sanitizer is not available on the GPU pool: races would show up here.)"""
+    w = W.make(name, B=B)
+    sub = np.arange(0, B, 37)
+    ref = O.loglike_batch(w.acf, w.seg_lengths, w.d, w.H[sub])
+    with tdb.TDLikelihood(w.acf, w.seg_lengths) as h:
+        d, H = _dev(w.d), _dev(w.H)
+        outs = [h.loglike_batch(d, H) for _ in range(4)]
+        inn = [h.inner_batch(d, H) for _ in range(2)]
+        torch.cuda.synchronize()
+        h.set_fft_variant(2)
+        o_staged = h.loglike_batch(d, H).cpu().numpy()
+    for o in outs[1:]:
+        assert torch.equal(outs[0], o)
+    assert torch.equal(inn[0][0], inn[1][0]) and torch.equal(inn[0][1], inn[1][1])
+    o0 = outs[0].cpu().numpy()
+    _assert_close(o0[sub], ref, what=f"{name} B={B}")
+    _assert_close(o0, o_staged, tol=1e-11, what="fused vs staged")
