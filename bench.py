@@ -286,7 +286,7 @@ def main():
     # ---------------- the same evaluations from template PARAMETERS on the host (td_loglike_ringdown_batch_host):
     # 5 doubles per template cross the bus, the rows are synthesised on the device.  Extra key, not `e2e`.
     e2e_params = None
-    if not args.no_e2e and args.op == "loglike" and w.params is not None and len(w.seg_lengths) == 1:
+    if not args.no_e2e and args.op == "loglike" and w.params is not None:
         out_p = np.empty(B)
         for _ in range(2):
             h.loglike_ringdown_batch_host(w.d, w.params, w.fs, out_p)
@@ -305,7 +305,7 @@ def main():
             t = torch.tensor([ms], dtype=torch.float64, device=dev)
             dist.all_reduce(t, op=dist.ReduceOp.MAX)
             ms = float(t.item())
-        e2e_params = {"value": world * B * k_p / (ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(40 * B + 8 * n_tot),
+        e2e_params = {"value": world * B * k_p / (ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(8 * w.params.size + 8 * n_tot),
                       "d2h_bytes_per_step": int(8 * B), "steps": k_p,
                       "api": "td_loglike_ringdown_batch_host (host parameters (A, f, tau, phi, t0); templates synthesised on the device)",
                       "max_rel_diff_vs_device_call": float(np.max(np.abs(out_p - out.cpu().numpy()) / np.maximum(np.abs(out_p), 1.0)))}

@@ -101,17 +101,19 @@ td_status td_loglike_batch_host(td_handle* h, const double* d, const double* H, 
 
 /* td_loglike_ringdown_batch - td_loglike_batch for templates given by PARAMETERS (waveform
  * generation and placement, moved onto the device for the analytic family of the configs):
- *   params  DEVICE pointer, row-major [B][5] doubles (A, f, tau, phi, t0):
- *           h_b(t_i) = A exp(-(t_i - t0)/tau) cos(2 pi f (t_i - t0) + phi) for t_i >= t0, 0 before, t_i = i / fs
+ *   params  DEVICE pointer, row-major [B][n_seg][5] doubles (A, f, tau, phi, t0), one row per (template, segment):
+ *           h_bs(t_i) = A exp(-(t_i - t0)/tau) cos(2 pi f (t_i - t0) + phi) for t_i >= t0, 0 before, t_i = i / fs
+ *           counted from the segment's first sample.  A detector projection F+ h_c + Fx h_s with a time shift dt
+ *           (:164, :209) is such a row: amplitude A hypot(F+, Fx), phase phi - atan2(Fx, F+), onset t0 + dt.
  *   fs      sampling rate in Hz (> 0);  d, out, stream as in td_loglike_batch.
- * Single-segment handles only (TD_EUNSUPPORTED otherwise).  The rows are synthesised into a scratch panel owned by the
+ * The rows are synthesised into a scratch panel owned by the
  * handle, chunk by chunk (about 64 MB, so that it stays in L2), and each chunk goes through the same kernels as td_loglike_batch.
  * Asynchronous on `stream`. */
 td_status td_loglike_ringdown_batch(td_handle* h, const double* d, const double* params, int64_t B, double fs,
                                     double* out, void* stream);
 
 /* td_loglike_ringdown_batch_host - the same from HOST buffers (d, params, out): 40 bytes per template cross the bus
- * instead of 8 N.  SYNCHRONOUS: returns after out[] is complete. */
+ * and segment instead of 8 N_s.  SYNCHRONOUS: returns after out[] is complete. */
 td_status td_loglike_ringdown_batch_host(td_handle* h, const double* d, const double* params, int64_t B, double fs,
                                          double* out, void* stream);
 

@@ -176,10 +176,13 @@ class TDLikelihood:
         return out_host
 
     def loglike_ringdown_batch(self, d, params, fs: float, out=None, stream=None):
-        """logL of damped-sinusoid templates given as rows (A, f, tau, phi, t0) of a CUDA float64 [B, 5] tensor."""
+        """logL of damped-sinusoid templates given as rows (A, f, tau, phi, t0): CUDA float64 [B, 5] (one segment)
+        or [B, n_seg, 5] (one row per template and segment / detector)."""
         import torch
-        if params.dim() != 2 or params.shape[1] != 5 or not params.is_contiguous():
-            raise ValueError("params must be a contiguous [B, 5] tensor")
+        n_seg = len(self.seg_lengths)
+        ok = (params.dim() == 3 and params.shape[1] == n_seg) or (params.dim() == 2 and n_seg == 1)
+        if not ok or params.shape[-1] != 5 or not params.is_contiguous():
+            raise ValueError(f"params must be a contiguous [B, {n_seg}, 5] tensor")
         B = int(params.shape[0])
         if out is None:
             out = torch.empty(B, dtype=torch.float64, device=params.device)
@@ -194,6 +197,8 @@ class TDLikelihood:
         import torch
         params_host = np.ascontiguousarray(params_host, dtype=np.float64)
         d_host = np.ascontiguousarray(d_host, dtype=np.float64)
+        if params_host.shape[-1] != 5 or params_host.size != params_host.shape[0] * len(self.seg_lengths) * 5:
+            raise ValueError("params must have shape [B, n_seg, 5]")
         B = int(params_host.shape[0])
         if out_host is None:
             out_host = np.empty(B, dtype=np.float64)

@@ -1,6 +1,6 @@
 // td_synth.cuh - template synthesis on the device: the step immediately before the hot
 // path, waveform generation and placement in the data vector, for the analytic
-// damped-sinusoid family of BASELINE.json's configs c1 / c2 / d*:
+// damped-sinusoid family of BASELINE.json's configs c1 / c2 / c5 / d*:
 //     h_b(t_i) = A exp(-(t_i - t0)/tau) cos(2 pi f (t_i - t0) + phi)   for t_i >= t0,  0 before,   t_i = i / fs.
 // A caller (a sampler) then ships 5 doubles per template instead of N: the rows are written to a scratch panel that
 // is consumed by the likelihood kernels chunk by chunk while it is still L2-resident, so H never crosses PCIe and
@@ -14,14 +14,22 @@ namespace td {
 
 constexpr int SYN_NT = 256;
 
-// params: [B][5] = (A, f, tau, phi, t0).  Writes rows b0 .. b0 + cb - 1 of the batch to Hs[(b - b0) * ldh + i], i < n.
+struct SynSeg { long long off; int n; int _pad; };  // a segment inside a row of H
+
+// params: [B][n_seg][5] = (A, f, tau, phi, t0) per (template, segment / detector), time counted from the segment's first
+// sample (a projected and time-shifted damped sinusoid F+ h_c + Fx h_s is again one: amplitude A hypot(F+, Fx), phase
+// phi - atan2(Fx, F+), onset t0 + dt - PAPER.md:164, :209).  Block (r, s) writes segment s of row b0 + r of the batch to
+// Hs[r * ldh + off_s + i], i < n_s.
 __global__ void __launch_bounds__(SYN_NT) synth_ringdown_kernel(const double* __restrict__ params, long long b0, int cb,
-                                                                int n, double fs, double* __restrict__ Hs, long long ldh) {
-  const int r = blockIdx.x;
+                                                                const SynSeg* __restrict__ segs, int n_seg, double fs,
+                                                                double* __restrict__ Hs, long long ldh) {
+  const int r = blockIdx.x, sgi = blockIdx.y;
   if (r >= cb) return;
-  const double* p = params + (b0 + r) * 5;
+  const SynSeg sg = segs[sgi];
+  const int n = sg.n;
+  const double* p = params + ((b0 + r) * n_seg + sgi) * 5;
   const double A = p[0], f = p[1], tau = p[2], phi = p[3], t0 = p[4];
-  double* row = Hs + (long long)r * ldh;
+  double* row = Hs + (long long)r * ldh + sg.off;
   // thread tid owns the samples i = tid + k SYN_NT (coalesced stores); its recurrence steps SYN_NT samples at a time
   const int tid = threadIdx.x;
   if (tid >= n) return;

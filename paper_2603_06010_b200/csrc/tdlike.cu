@@ -75,6 +75,7 @@ struct td_handle {
   cplx* wsU = nullptr; cplx* wsZ = nullptr; double* wsPartial = nullptr;
   double* synH = nullptr; size_t synH_elems = 0;  // scratch panel of synthesised templates (td_synth.cuh)
   double* synP = nullptr; size_t synP_elems = 0;  // device copy of host parameters
+  SynSeg* synSeg = nullptr;                       // device [n_seg]: offsets and lengths for the synthesis kernel
   double* ud = nullptr;  // [n_tot] weights u = C^{-1} d of the dot path (td_dot.cuh), lazily allocated
   size_t wsU_elems = 0, wsZ_elems = 0, wsP_elems = 0;
   // dense path state
@@ -104,7 +105,7 @@ void free_handle(td_handle* h) {
   if (!h) return;
   for (auto& s : h->segs) { cudaFree(s.a); cudaFree(s.G); cudaFree(s.Gp); cudaFree(s.zd); }
   for (auto& c : h->classes) { cudaFree(c.T); cudaFree(c.d_segs); cudaFree(c.d_Gp); }
-  cudaFree(h->wsU); cudaFree(h->wsZ); cudaFree(h->wsPartial); cudaFree(h->ud); cudaFree(h->synH); cudaFree(h->synP);
+  cudaFree(h->wsU); cudaFree(h->wsZ); cudaFree(h->wsPartial); cudaFree(h->ud); cudaFree(h->synH); cudaFree(h->synP); cudaFree(h->synSeg);
   cudaFree(h->hsD); cudaFree(h->hsH[0]); cudaFree(h->hsH[1]); cudaFree(h->hsOut);
   if (h->copy_stream) cudaStreamDestroy(h->copy_stream);
   for (int i = 0; i < 2; ++i) { if (h->ev_copied[i]) cudaEventDestroy(h->ev_copied[i]); if (h->ev_done[i]) cudaEventDestroy(h->ev_done[i]); }
@@ -700,11 +701,16 @@ td_status td_loglike_ringdown_batch(td_handle* h, const double* d, const double*
   if (!h || B < 0) return TD_EINVAL;
   if (B == 0) return TD_OK;
   if (!d || !params || !out || !(fs > 0.0)) return TD_EINVAL;
-  if (h->n_seg != 1) return TD_EUNSUPPORTED;  // t_i = i / fs counts from the start of the one segment
   DevGuard guard(h->device);
   if (!guard.ok) return TD_ECUDA;
   cudaStream_t st = (cudaStream_t)stream;
   const int64_t n = h->n_tot, ldh = (n + 1) & ~1ll;  // even leading dimension: 16-byte aligned rows
+  if (!h->synSeg) {
+    std::vector<SynSeg> hs(h->n_seg);
+    for (int s = 0; s < h->n_seg; ++s) { hs[s].off = h->segs[s].off; hs[s].n = (int)h->segs[s].n; hs[s]._pad = 0; }
+    CK(cudaMalloc(&h->synSeg, sizeof(SynSeg) * h->n_seg));
+    CK(cudaMemcpy(h->synSeg, hs.data(), sizeof(SynSeg) * h->n_seg, cudaMemcpyHostToDevice));
+  }
   // chunk: a whole number of waves of the persistent kernels, about 64 MB so the panel (mostly) stays in the 126 MB L2
   int64_t CH = std::max<int64_t>(1, (66ll << 20) / (8 * ldh));
   if (CH > h->num_sms) CH -= CH % h->num_sms;
@@ -717,7 +723,7 @@ td_status td_loglike_ringdown_batch(td_handle* h, const double* d, const double*
   int launches = 0;
   for (int64_t b0 = 0; b0 < B; b0 += CH) {
     const int64_t cb = std::min<int64_t>(CH, B - b0);
-    synth_ringdown_kernel<<<(unsigned)cb, SYN_NT, 0, st>>>(params, b0, (int)cb, (int)n, fs, h->synH, ldh);
+    synth_ringdown_kernel<<<dim3((unsigned)cb, (unsigned)h->n_seg), SYN_NT, 0, st>>>(params, b0, (int)cb, h->synSeg, h->n_seg, fs, h->synH, ldh);
     CK(cudaGetLastError());
     h->last_launches = 0;
     td_status s = run_batch<MODE_LOGLIKE>(h, d, h->synH, ldh, cb, out + b0, nullptr, st);
@@ -733,19 +739,18 @@ td_status td_loglike_ringdown_batch_host(td_handle* h, const double* d, const do
   if (!h || B < 0) return TD_EINVAL;
   if (B == 0) return TD_OK;
   if (!d || !params || !out) return TD_EINVAL;
-  if (h->n_seg != 1) return TD_EUNSUPPORTED;
   DevGuard guard(h->device);
   if (!guard.ok) return TD_ECUDA;
   cudaStream_t st = (cudaStream_t)stream;
-  const int64_t n = h->n_tot;
-  const size_t need = (size_t)(5 * B + n + B);  // parameters, data vector, results
+  const int64_t n = h->n_tot, np5 = 5ll * h->n_seg * B;
+  const size_t need = (size_t)(np5 + n + B);  // parameters, data vector, results
   if (need > h->synP_elems) {
     cudaFree(h->synP); h->synP = nullptr; h->synP_elems = 0;
     CK(cudaMalloc(&h->synP, sizeof(double) * need));
     h->synP_elems = need;
   }
-  double* dP = h->synP; double* dD = dP + 5 * B; double* dO = dD + n;
-  CK(cudaMemcpyAsync(dP, params, sizeof(double) * 5 * B, cudaMemcpyHostToDevice, st));
+  double* dP = h->synP; double* dD = dP + np5; double* dO = dD + n;
+  CK(cudaMemcpyAsync(dP, params, sizeof(double) * np5, cudaMemcpyHostToDevice, st));
   CK(cudaMemcpyAsync(dD, d, sizeof(double) * n, cudaMemcpyHostToDevice, st));
   td_status s = td_loglike_ringdown_batch(h, dD, dP, B, fs, dO, stream);
   if (s != TD_OK) return s;

@@ -104,7 +104,8 @@ class Workload:
     H: np.ndarray                # float64 [B, N_tot], row b = template b, same packing
     scales: np.ndarray           # float64 [n_seg] PSD scale of each segment
     description: str = ""
-    params: Optional[np.ndarray] = None   # float64 [B, 5] = (A, f, tau, phi, t0) where the rows of H are damped sinusoids
+    params: Optional[np.ndarray] = None   # float64 [B, 5] or [B, n_seg, 5] = (A, f, tau, phi, t0) per (template, segment)
+                                          # where the rows of H are damped sinusoids (time counted from each segment's start)
 
     @property
     def n_tot(self) -> int:
@@ -249,6 +250,7 @@ def make(name: str, B: Optional[int] = None, n_scale: int = 1) -> Workload:
         Fp, Fx, dts = U(-1, 1, (B, 3)), U(-1, 1, (B, 3)), U(-10e-3, 10e-3, (B, 3))
         t = np.arange(N) / fs
         H = np.empty((B, 3 * N))
+        amp = np.empty(B)
         for lo, hi in _chunks(B, 3 * N):
             net2 = np.zeros(hi - lo)
             for det in range(3):
@@ -257,9 +259,14 @@ def make(name: str, B: Optional[int] = None, n_scale: int = 1) -> Workload:
                      + Fx[lo:hi, det, None] * _damped(t, f[lo:hi], tau[lo:hi], phi[lo:hi], ts, quadrature=True))
                 H[lo:hi, det * N:(det + 1) * N] = h
                 net2 += _snr_fd(h, fs) ** 2 / scales[det]
-            H[lo:hi] *= (snr[lo:hi] / np.sqrt(net2))[:, None]
+            amp[lo:hi] = snr[lo:hi] / np.sqrt(net2)
+            H[lo:hi] *= amp[lo:hi, None]
+        # per detector the projected template F+ h_c + Fx h_s is again a damped sinusoid:
+        # amplitude A hypot(F+, Fx), phase phi - atan2(Fx, F+), onset t0 + dt   ->  params [B, 3, 5]
+        params = np.stack([amp[:, None] * np.hypot(Fp, Fx), np.repeat(f[:, None], 3, 1), np.repeat(tau[:, None], 3, 1),
+                           phi[:, None] - np.arctan2(Fx, Fp), t0[:, None] + dts], axis=2)
         return Workload(name, seed, fs, np.array([N] * 3, np.int64), acf, noise + H[0], H, scales,
-                        "3 detectors x N, projected damped sinusoids, network SNR")
+                        "3 detectors x N, projected damped sinusoids, network SNR", params)
 
     if name in ("d1", "d2", "d3", "d4", "d5"):
         fs = 4096.0
