@@ -283,20 +283,20 @@ def main():
         max_dev = float(np.max(np.abs(out_host - out.cpu().numpy())))
         e2e["max_abs_diff_vs_device_call"] = max_dev
 
-    # ---------------- the same evaluations from template PARAMETERS on the host (td_loglike_ringdown_batch_host):
+    # ---------------- the same evaluations from template PARAMETERS on the host (td_loglike_family_batch_host):
     # 5 doubles per template cross the bus, the rows are synthesised on the device.  Extra key, not `e2e`.
     e2e_params = None
     if not args.no_e2e and args.op == "loglike" and w.params is not None:
         out_p = np.empty(B)
         for _ in range(2):
-            h.loglike_ringdown_batch_host(w.d, w.params, w.fs, out_p)
+            h.loglike_family_batch_host(w.d, w.family, w.params, w.fs, out_p)
         torch.cuda.synchronize()
         barrier()
         k_p = max(3, min(args.steps, 10))
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record(stream)
         for _ in range(k_p):
-            h.loglike_ringdown_batch_host(w.d, w.params, w.fs, out_p)
+            h.loglike_family_batch_host(w.d, w.family, w.params, w.fs, out_p)
         e1.record(stream)
         torch.cuda.synchronize()
         barrier()
@@ -307,7 +307,7 @@ def main():
             ms = float(t.item())
         e2e_params = {"value": world * B * k_p / (ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(8 * w.params.size + 8 * n_tot),
                       "d2h_bytes_per_step": int(8 * B), "steps": k_p,
-                      "api": "td_loglike_ringdown_batch_host (host parameters (A, f, tau, phi, t0); templates synthesised on the device)",
+                      "api": f"td_loglike_family_batch_host (host parameters, family {W.FAMILIES[w.family]}; templates synthesised on the device)",
                       "max_rel_diff_vs_device_call": float(np.max(np.abs(out_p - out.cpu().numpy()) / np.maximum(np.abs(out_p), 1.0)))}
 
     if rank != 0:

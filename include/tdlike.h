@@ -99,21 +99,36 @@ td_status td_inner_batch(td_handle* h, const double* d, const double* H, int64_t
 td_status td_loglike_batch_host(td_handle* h, const double* d, const double* H, int64_t ldh,
                                 int64_t B, double* out, void* stream);
 
-/* td_loglike_ringdown_batch - td_loglike_batch for templates given by PARAMETERS (waveform
- * generation and placement, moved onto the device for the analytic family of the configs):
- *   params  DEVICE pointer, row-major [B][n_seg][5] doubles (A, f, tau, phi, t0), one row per (template, segment):
- *           h_bs(t_i) = A exp(-(t_i - t0)/tau) cos(2 pi f (t_i - t0) + phi) for t_i >= t0, 0 before, t_i = i / fs
- *           counted from the segment's first sample.  A detector projection F+ h_c + Fx h_s with a time shift dt
- *           (:164, :209) is such a row: amplitude A hypot(F+, Fx), phase phi - atan2(Fx, F+), onset t0 + dt.
+/* td_family: analytic template families of td_loglike_family_batch (rows of 5 parameters; t_i = i / fs counted from the
+ * segment's first sample, n = the segment's length):
+ *   TD_FAMILY_RINGDOWN      (A, f, tau, phi, t0):      A exp(-(t_i - t0)/tau) cos(2 pi f (t_i - t0) + phi) for t_i >= t0, else 0
+ *   TD_FAMILY_SINE_GAUSSIAN (A, f, w, phi, t0):        A exp(-((t_i - t0)/w)^2) cos(2 pi f t_i + phi)
+ *   TD_FAMILY_CHIRP         (A, f0, fdot, phi, alpha): A tukey_alpha(i / (n - 1)) cos(2 pi (f0 t_i + fdot t_i^2 / 2) + phi)
+ * (the template families of BASELINE.json's configs c1/c2/c5, c3 and c4). */
+enum { TD_FAMILY_RINGDOWN = 0, TD_FAMILY_SINE_GAUSSIAN = 1, TD_FAMILY_CHIRP = 2 };
+
+/* td_loglike_family_batch - td_loglike_batch for templates given by PARAMETERS (waveform
+ * generation and placement, moved onto the device for the analytic families of the configs):
+ *   family  one of td_family.
+ *   params  DEVICE pointer, row-major [B][n_seg][5] doubles, one row per (template, segment / detector), in the
+ *           segment's own time.  A detector projection F+ h_c + Fx h_s of a ringdown with a time shift dt (:164, :209)
+ *           is such a row: amplitude A hypot(F+, Fx), phase phi - atan2(Fx, F+), onset t0 + dt; a segment that starts at
+ *           time ts of a longer record takes t0 - ts (and phi + 2 pi f ts for the sine-Gaussian).
  *   fs      sampling rate in Hz (> 0);  d, out, stream as in td_loglike_batch.
- * The rows are synthesised into a scratch panel owned by the
- * handle, chunk by chunk (about 64 MB, so that it stays in L2), and each chunk goes through the same kernels as td_loglike_batch.
- * Asynchronous on `stream`. */
+ * The rows are synthesised into a scratch panel owned by the handle, chunk by chunk (about 64 MB, so that it stays in
+ * L2), and each chunk goes through the same kernels as td_loglike_batch.  Asynchronous on `stream`.
+ * Errors: TD_EINVAL (unknown family, fs <= 0, null pointers), TD_ENOMEM, TD_ECUDA. */
+td_status td_loglike_family_batch(td_handle* h, const double* d, int family, const double* params, int64_t B, double fs,
+                                  double* out, void* stream);
+
+/* td_loglike_family_batch_host - the same from HOST buffers (d, params, out): 40 bytes per template and segment cross
+ * the bus instead of 8 N_s.  SYNCHRONOUS: returns after out[] is complete. */
+td_status td_loglike_family_batch_host(td_handle* h, const double* d, int family, const double* params, int64_t B,
+                                       double fs, double* out, void* stream);
+
+/* td_loglike_ringdown_batch, td_loglike_ringdown_batch_host - the two calls above with family = TD_FAMILY_RINGDOWN. */
 td_status td_loglike_ringdown_batch(td_handle* h, const double* d, const double* params, int64_t B, double fs,
                                     double* out, void* stream);
-
-/* td_loglike_ringdown_batch_host - the same from HOST buffers (d, params, out): 40 bytes per template cross the bus
- * and segment instead of 8 N_s.  SYNCHRONOUS: returns after out[] is complete. */
 td_status td_loglike_ringdown_batch_host(td_handle* h, const double* d, const double* params, int64_t B, double fs,
                                          double* out, void* stream);
 

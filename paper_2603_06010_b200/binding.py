@@ -17,6 +17,7 @@ LIB_PATH = os.path.join(_HERE, "lib", "libtdlike.so")
 
 TD_OK, TD_EINVAL, TD_ENOTSPD, TD_ENOMEM, TD_ECUDA, TD_EUNSUPPORTED = range(6)
 TD_PATH_AUTO, TD_PATH_FFT, TD_PATH_DENSE, TD_PATH_DOT = 0, 1, 2, 3
+TD_FAMILY_RINGDOWN, TD_FAMILY_SINE_GAUSSIAN, TD_FAMILY_CHIRP = 0, 1, 2
 
 # every symbol include/tdlike.h declares: name -> (restype, argtypes)
 _VP, _I64, _INT, _DP = C.c_void_p, C.c_int64, C.c_int, C.POINTER(C.c_double)
@@ -26,6 +27,8 @@ SYMBOLS = {
     "td_loglike_batch": (_INT, [_VP, _VP, _VP, _I64, _I64, _VP, _VP]),
     "td_inner_batch": (_INT, [_VP, _VP, _VP, _I64, _I64, _VP, _VP, _VP]),
     "td_loglike_batch_host": (_INT, [_VP, _VP, _VP, _I64, _I64, _VP, _VP]),
+    "td_loglike_family_batch": (_INT, [_VP, _VP, _INT, _VP, _I64, C.c_double, _VP, _VP]),
+    "td_loglike_family_batch_host": (_INT, [_VP, _VP, _INT, _VP, _I64, C.c_double, _VP, _VP]),
     "td_loglike_ringdown_batch": (_INT, [_VP, _VP, _VP, _I64, C.c_double, _VP, _VP]),
     "td_loglike_ringdown_batch_host": (_INT, [_VP, _VP, _VP, _I64, C.c_double, _VP, _VP]),
     "td_set_path": (_INT, [_VP, _INT]),
@@ -176,8 +179,14 @@ class TDLikelihood:
         return out_host
 
     def loglike_ringdown_batch(self, d, params, fs: float, out=None, stream=None):
-        """logL of damped-sinusoid templates given as rows (A, f, tau, phi, t0): CUDA float64 [B, 5] (one segment)
-        or [B, n_seg, 5] (one row per template and segment / detector)."""
+        return self.loglike_family_batch(d, TD_FAMILY_RINGDOWN, params, fs, out=out, stream=stream)
+
+    def loglike_ringdown_batch_host(self, d_host, params_host, fs: float, out_host=None, stream=None):
+        return self.loglike_family_batch_host(d_host, TD_FAMILY_RINGDOWN, params_host, fs, out_host=out_host, stream=stream)
+
+    def loglike_family_batch(self, d, family: int, params, fs: float, out=None, stream=None):
+        """logL of templates of an analytic family (TD_FAMILY_*) given as rows of 5 parameters: CUDA float64 [B, 5]
+        (one segment) or [B, n_seg, 5] (one row per template and segment / detector)."""
         import torch
         n_seg = len(self.seg_lengths)
         ok = (params.dim() == 3 and params.shape[1] == n_seg) or (params.dim() == 2 and n_seg == 1)
@@ -186,13 +195,14 @@ class TDLikelihood:
         B = int(params.shape[0])
         if out is None:
             out = torch.empty(B, dtype=torch.float64, device=params.device)
-        st = self._lib.td_loglike_ringdown_batch(self._h, _ptr(d, "d", self.device), _ptr(params, "params", self.device), B,
-                                                 float(fs), _ptr(out, "out", self.device), _stream_ptr(stream, params.device))
-        _check(st, "td_loglike_ringdown_batch")
+        st = self._lib.td_loglike_family_batch(self._h, _ptr(d, "d", self.device), int(family),
+                                               _ptr(params, "params", self.device), B, float(fs),
+                                               _ptr(out, "out", self.device), _stream_ptr(stream, params.device))
+        _check(st, "td_loglike_family_batch")
         return out
 
-    def loglike_ringdown_batch_host(self, d_host: np.ndarray, params_host: np.ndarray, fs: float,
-                                    out_host: Optional[np.ndarray] = None, stream=None):
+    def loglike_family_batch_host(self, d_host: np.ndarray, family: int, params_host: np.ndarray, fs: float,
+                                  out_host: Optional[np.ndarray] = None, stream=None):
         """Same from HOST arrays: 5 doubles per template cross the bus instead of N."""
         import torch
         params_host = np.ascontiguousarray(params_host, dtype=np.float64)
@@ -202,9 +212,10 @@ class TDLikelihood:
         B = int(params_host.shape[0])
         if out_host is None:
             out_host = np.empty(B, dtype=np.float64)
-        st = self._lib.td_loglike_ringdown_batch_host(self._h, d_host.ctypes.data, params_host.ctypes.data, B, float(fs),
-                                                      out_host.ctypes.data, _stream_ptr(stream, torch.device("cuda", self.device)))
-        _check(st, "td_loglike_ringdown_batch_host")
+        st = self._lib.td_loglike_family_batch_host(self._h, d_host.ctypes.data, int(family), params_host.ctypes.data, B,
+                                                    float(fs), out_host.ctypes.data,
+                                                    _stream_ptr(stream, torch.device("cuda", self.device)))
+        _check(st, "td_loglike_family_batch_host")
         return out_host
 
     # -- options / queries ---------------------------------------------------------------

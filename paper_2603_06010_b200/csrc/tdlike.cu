@@ -696,9 +696,9 @@ td_status td_loglike_batch_host(td_handle* h, const double* d, const double* H, 
   return TD_OK;
 }
 
-td_status td_loglike_ringdown_batch(td_handle* h, const double* d, const double* params, int64_t B, double fs,
-                                    double* out, void* stream) {
-  if (!h || B < 0) return TD_EINVAL;
+td_status td_loglike_family_batch(td_handle* h, const double* d, int family, const double* params, int64_t B, double fs,
+                                  double* out, void* stream) {
+  if (!h || B < 0 || family < 0 || family >= SYN_NFAM) return TD_EINVAL;
   if (B == 0) return TD_OK;
   if (!d || !params || !out || !(fs > 0.0)) return TD_EINVAL;
   DevGuard guard(h->device);
@@ -723,7 +723,10 @@ td_status td_loglike_ringdown_batch(td_handle* h, const double* d, const double*
   int launches = 0;
   for (int64_t b0 = 0; b0 < B; b0 += CH) {
     const int64_t cb = std::min<int64_t>(CH, B - b0);
-    synth_ringdown_kernel<<<dim3((unsigned)cb, (unsigned)h->n_seg), SYN_NT, 0, st>>>(params, b0, (int)cb, h->synSeg, h->n_seg, fs, h->synH, ldh);
+    const dim3 sgrid((unsigned)cb, (unsigned)h->n_seg);
+    if (family == SYN_RINGDOWN) synth_kernel<SYN_RINGDOWN><<<sgrid, SYN_NT, 0, st>>>(params, b0, (int)cb, h->synSeg, h->n_seg, fs, h->synH, ldh);
+    else if (family == SYN_SINEGAUSS) synth_kernel<SYN_SINEGAUSS><<<sgrid, SYN_NT, 0, st>>>(params, b0, (int)cb, h->synSeg, h->n_seg, fs, h->synH, ldh);
+    else synth_kernel<SYN_CHIRP><<<sgrid, SYN_NT, 0, st>>>(params, b0, (int)cb, h->synSeg, h->n_seg, fs, h->synH, ldh);
     CK(cudaGetLastError());
     h->last_launches = 0;
     td_status s = run_batch<MODE_LOGLIKE>(h, d, h->synH, ldh, cb, out + b0, nullptr, st);
@@ -734,9 +737,19 @@ td_status td_loglike_ringdown_batch(td_handle* h, const double* d, const double*
   return TD_OK;
 }
 
+td_status td_loglike_ringdown_batch(td_handle* h, const double* d, const double* params, int64_t B, double fs,
+                                    double* out, void* stream) {
+  return td_loglike_family_batch(h, d, SYN_RINGDOWN, params, B, fs, out, stream);
+}
+
 td_status td_loglike_ringdown_batch_host(td_handle* h, const double* d, const double* params, int64_t B, double fs,
                                          double* out, void* stream) {
-  if (!h || B < 0) return TD_EINVAL;
+  return td_loglike_family_batch_host(h, d, SYN_RINGDOWN, params, B, fs, out, stream);
+}
+
+td_status td_loglike_family_batch_host(td_handle* h, const double* d, int family, const double* params, int64_t B,
+                                       double fs, double* out, void* stream) {
+  if (!h || B < 0 || family < 0 || family >= SYN_NFAM) return TD_EINVAL;
   if (B == 0) return TD_OK;
   if (!d || !params || !out) return TD_EINVAL;
   DevGuard guard(h->device);
@@ -752,7 +765,7 @@ td_status td_loglike_ringdown_batch_host(td_handle* h, const double* d, const do
   double* dP = h->synP; double* dD = dP + np5; double* dO = dD + n;
   CK(cudaMemcpyAsync(dP, params, sizeof(double) * np5, cudaMemcpyHostToDevice, st));
   CK(cudaMemcpyAsync(dD, d, sizeof(double) * n, cudaMemcpyHostToDevice, st));
-  td_status s = td_loglike_ringdown_batch(h, dD, dP, B, fs, dO, stream);
+  td_status s = td_loglike_family_batch(h, dD, family, dP, B, fs, dO, stream);
   if (s != TD_OK) return s;
   CK(cudaMemcpyAsync(out, dO, sizeof(double) * B, cudaMemcpyDeviceToHost, st));
   CK(cudaStreamSynchronize(st));

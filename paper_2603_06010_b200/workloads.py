@@ -105,7 +105,9 @@ class Workload:
     scales: np.ndarray           # float64 [n_seg] PSD scale of each segment
     description: str = ""
     params: Optional[np.ndarray] = None   # float64 [B, 5] or [B, n_seg, 5] = (A, f, tau, phi, t0) per (template, segment)
-                                          # where the rows of H are damped sinusoids (time counted from each segment's start)
+                                          # where the rows of H come from an analytic family (time counted from each
+                                          # segment's start), see FAMILIES
+    family: int = 0                       # index into FAMILIES
 
     @property
     def n_tot(self) -> int:
@@ -118,6 +120,12 @@ class Workload:
     def offsets(self) -> np.ndarray:
         return np.concatenate(([0], np.cumsum(self.seg_lengths)))[:-1]
 
+
+# analytic template families (rows of 5 parameters), the codes of include/tdlike.h:
+#   0 ringdown        (A, f, tau, phi, t0):   A exp(-(t-t0)/tau) cos(2 pi f (t-t0) + phi), t >= t0
+#   1 sine-Gaussian   (A, f, w, phi, t0):     A exp(-((t-t0)/w)^2) cos(2 pi f t + phi)
+#   2 chirp           (A, f0, fdot, phi, alpha): A tukey_alpha(i/(n-1)) cos(2 pi (f0 t + fdot t^2 / 2) + phi)
+FAMILIES = ("ringdown", "sine_gaussian", "chirp")
 
 # name -> (seed, default B)
 _SPECS = {
@@ -211,13 +219,19 @@ def make(name: str, B: Optional[int] = None, n_scale: int = 1) -> Workload:
         t = np.arange(Ng) / fs
         keep = np.concatenate([np.arange(a, b) for a, b in ranges])
         H = np.empty((B, len(keep)))
+        amp = np.empty(B)
         for lo, hi in _chunks(B, Ng):
             h = np.exp(-(((t[None, :] - t0[lo:hi, None]) / w[lo:hi, None]) ** 2)) * np.cos(
                 2 * np.pi * f[lo:hi, None] * t[None, :] + phi[lo:hi, None])
-            h *= (snr[lo:hi] / _snr_fd(h, fs))[:, None]
+            amp[lo:hi] = snr[lo:hi] / _snr_fd(h, fs)
+            h *= amp[lo:hi, None]
             H[lo:hi] = h[:, keep]
+        # per segment, in the segment's own time (start ts = a / fs): onset t0 - ts, phase phi + 2 pi f ts
+        ts = np.array([a for a, _ in ranges]) / fs
+        params = np.stack([np.repeat(amp[:, None], 3, 1), np.repeat(f[:, None], 3, 1), np.repeat(w[:, None], 3, 1),
+                           phi[:, None] + 2 * np.pi * f[:, None] * ts[None, :], t0[:, None] - ts[None, :]], axis=2)
         return Workload(name, seed, fs, lens, acf, noise + H[0], H, scales,
-                        "3 disjoint segments with 128-sample gaps, sine-Gaussians")
+                        "3 disjoint segments with 128-sample gaps, sine-Gaussians", params, 1)
 
     if name == "c4":
         fs = 4096.0
@@ -229,12 +243,15 @@ def make(name: str, B: Optional[int] = None, n_scale: int = 1) -> Workload:
         t = np.arange(N) / fs
         win = _tukey(N, 0.1)
         H = np.empty((B, N))
+        amp = np.empty(B)
         for lo, hi in _chunks(B, N):
             h = win[None, :] * np.cos(2 * np.pi * (f0[lo:hi, None] * t[None, :]
                                                    + 0.5 * fdot[lo:hi, None] * t[None, :] ** 2) + phi[lo:hi, None])
-            H[lo:hi] = h * (snr[lo:hi] / _snr_fd(h, fs))[:, None]
+            amp[lo:hi] = snr[lo:hi] / _snr_fd(h, fs)
+            H[lo:hi] = h * amp[lo:hi, None]
         return Workload(name, seed, fs, np.array([N], np.int64), rho, n + H[0], H, np.ones(1),
-                        "long single segment, linear chirps with Tukey(0.1) envelope")
+                        "long single segment, linear chirps with Tukey(0.1) envelope",
+                        np.stack([amp, f0, fdot, phi, np.full(B, 0.1)], axis=1), 2)
 
     if name == "c5":
         fs = 4096.0

@@ -438,17 +438,19 @@ def test_cross_term_dot_path_unaligned_rows_and_odd_length():
 
 
 # ------------------------------------------------------------------ templates synthesised on the device (td_synth.cuh)
-@pytest.mark.parametrize("name,B", [("c1", 64), ("c2", 200), ("d2", 333), ("c5", 10)])
-def test_ringdown_params_entry_matches_oracle(name, B):
-    """td_loglike_ringdown_batch: rows (A, f, tau, phi, t0) instead of H.  The oracle sees the H numpy built from the
-    same parameters; the device and host entries must agree with it and with each other."""
-    w = W.make(name, B=B)
+@pytest.mark.parametrize("name,B,n_scale", [("c1", 64, 1), ("c2", 200, 1), ("d2", 333, 1), ("c5", 10, 1), ("c3", 12, 1),
+                                            ("c4", 3, 8)])
+def test_family_params_entry_matches_oracle(name, B, n_scale):
+    """td_loglike_family_batch: rows of 5 parameters instead of H (ringdown c1/c2/c5/d*, sine-Gaussian c3, chirp c4).
+    The oracle sees the H numpy built from the same parameters; the device and host entries must agree with it and
+    with each other."""
+    w = W.make(name, B=B, n_scale=n_scale)
     ref = O.loglike_batch(w.acf, w.seg_lengths, w.d, w.H)
     with tdb.TDLikelihood(w.acf, w.seg_lengths) as h:
-        out = h.loglike_ringdown_batch(_dev(w.d), _dev(w.params), w.fs)
+        out = h.loglike_family_batch(_dev(w.d), w.family, _dev(w.params), w.fs)
         torch.cuda.synchronize()
         assert h.last_launches() >= 2
-        out_host = h.loglike_ringdown_batch_host(w.d, w.params, w.fs)
+        out_host = h.loglike_family_batch_host(w.d, w.family, w.params, w.fs)
     _assert_close(out.cpu().numpy(), ref, what=f"{name} ringdown params")
     assert np.array_equal(out.cpu().numpy(), out_host)
 
@@ -469,6 +471,9 @@ def test_ringdown_params_entry_errors_and_edges():
         out = h.loglike_ringdown_batch(_dev(w.d), _dev(p), w.fs).cpu().numpy()
         with pytest.raises(tdb.TDError):
             h.loglike_ringdown_batch(_dev(w.d), _dev(p), 0.0)
+        with pytest.raises(tdb.TDError) as e:
+            h.loglike_family_batch(_dev(w.d), 7, _dev(p), w.fs)
+        assert e.value.status == tdb.TD_EINVAL
     _assert_close(out, ref, what="ringdown edges")
 
 
