@@ -498,3 +498,44 @@ def test_fused_many_items_per_cta_repeatable(name, B):
     o0 = outs[0].cpu().numpy()
     _assert_close(o0[sub], ref, what=f"{name} B={B}")
     _assert_close(o0, o_staged, tol=1e-11, what="fused vs staged")
+
+
+# ------------------------------------------------------------------ degenerate rows on the dense, dot and cluster paths
+@pytest.mark.parametrize("name,n_scale,path", [("d2", 1, tdb.TD_PATH_DENSE), ("d4", 1, tdb.TD_PATH_DENSE),
+                                               ("c5", 1, tdb.TD_PATH_AUTO), ("c4", 4, tdb.TD_PATH_AUTO)])
+def test_exact_zero_nan_row_and_single_template(name, n_scale, path):
+    """h = d gives exactly 0 (pin P8 iv), a NaN poisons only its own row, B = 1 and a strided H work, on the dense
+    (cp.async panels), cluster and staged kernels; the dot path keeps a NaN row to itself as well."""
+    w = W.make(name, B=9, n_scale=n_scale)
+    n = w.n_tot
+    fn = O.loglike_batch_solve_toeplitz if name == "c4" else O.loglike_batch
+    ref = fn(w.acf, w.seg_lengths, w.d, w.H)
+    Hpad = torch.zeros(9, n + 6, dtype=torch.float64, device="cuda")
+    Hpad[:, :n] = _dev(w.H)
+    Hpad[3, :n] = _dev(w.d)
+    Hpad[5, n // 2] = float("nan")
+    with tdb.TDLikelihood(w.acf, w.seg_lengths) as h:
+        h.set_path(path)
+        out = h.loglike_batch(_dev(w.d), Hpad[:, :n]).cpu().numpy()
+        one = h.loglike_batch(_dev(w.d), Hpad[7:8, :n]).cpu().numpy()
+        h.set_path(tdb.TD_PATH_AUTO)
+        dh, _ = h.inner_batch(_dev(w.d), Hpad[:, :n], want_hh=False)
+        dh = dh.cpu().numpy()
+    assert out[3] == 0.0
+    assert np.isnan(out[5]) and np.isnan(dh[5])
+    keep = [0, 1, 2, 4, 6, 7, 8]
+    _assert_close(out[keep], ref[keep], what=f"{name} degenerate rows")
+    assert one[0] == out[7]
+    assert np.all(np.isfinite(dh[keep]))
+
+
+def test_empty_batch_is_a_no_op_everywhere():
+    w = W.make("c1", B=2)
+    with tdb.TDLikelihood(w.acf, w.seg_lengths) as h:
+        d = _dev(w.d)
+        H0 = torch.zeros(0, w.n_tot, dtype=torch.float64, device="cuda")
+        assert h.loglike_batch(d, H0).numel() == 0
+        dh, hh = h.inner_batch(d, H0)
+        assert dh.numel() == 0 and hh.numel() == 0
+        p0 = torch.zeros(0, 5, dtype=torch.float64, device="cuda")
+        assert h.loglike_family_batch(d, tdb.TD_FAMILY_RINGDOWN, p0, w.fs).numel() == 0
