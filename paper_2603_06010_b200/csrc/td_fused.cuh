@@ -145,27 +145,43 @@ __device__ __forceinline__ void last_pass_task(const Arr& ZE, const Arr& ZO, int
                                                double& acc0, double& acc1) {
   const int S = M / R;
   const int j = g;
-  cplx w[R], e[R], o[R];
-  tw_powers<R>(T[2 * j], w);  // w_M^j
+  cplx e[R], o[R], gm[R];     // z_t = e_t + gm_t o_t: the pruned last radix-2 stage
   const cplx beta = T[j];     // w_2M^j
-  static_for<0, R>([&](auto s) {
-    constexpr int ss = decltype(s)::value;
-    cplx ve = ZE.ld(j + ss * S), vo = ZO.ld(j + ss * S);
-    if (ss > 0) {
-      ve = cmulc(ve, w[ss]);
-      vo = cmulc(vo, cmul(w[ss], beta));
-    } else {
-      vo = cmulc(vo, beta);
-    }
-    e[ss] = ve;
-    o[ss] = vo;
-  });
-  fft_reg<R, true>(e);
-  fft_reg<R, true>(o);
+  if constexpr (R == 16) {
+    // merged-twiddle 6-FMA butterflies (td_dit16.cuh), as in last_pass_c
+    const cplx w1 = cconj(T[2 * j]);  // w_M^(-j)
+#pragma unroll
+    for (int ss = 0; ss < R; ++ss) { e[ss] = ZE.ld(j + ss * S); o[ss] = ZO.ld(j + ss * S); }
+    dit16<true, true>(e, w1);
+    dit16<true, true>(o, w1);
+    const cplx cb = cconj(beta);
+    static_for<0, R>([&](auto t) { gm[decltype(t)::value] = mul_w32<decltype(t)::value, true>(cb); });
+  } else {
+    cplx w[R];
+    tw_powers<R>(T[2 * j], w);  // w_M^j
+    static_for<0, R>([&](auto s) {
+      constexpr int ss = decltype(s)::value;
+      cplx ve = ZE.ld(j + ss * S), vo = ZO.ld(j + ss * S);
+      if (ss > 0) {
+        ve = cmulc(ve, w[ss]);
+        vo = cmulc(vo, cmul(w[ss], beta));
+      } else {
+        vo = cmulc(vo, beta);
+      }
+      e[ss] = ve;
+      o[ss] = vo;
+    });
+    fft_reg<R, true>(e);
+    fft_reg<R, true>(o);
+    static_for<0, R>([&](auto t) {
+      constexpr int tt = decltype(t)::value;
+      gm[tt] = mk(cos32(tt * (16 / R)), sin32(tt * (16 / R)));
+    });
+  }
   static_for<0, R>([&](auto t) {
     constexpr int tt = decltype(t)::value;
-    const cplx ot = mul_w32<tt * (16 / R), true>(o[brevR<R>(tt)]);
-    const cplx z = cadd(e[brevR<R>(tt)], ot);
+    const cplx ev = e[brevR<R>(tt)], ov = o[brevR<R>(tt)];
+    const cplx z = mk(fma(gm[tt].x, ov.x, fma(-gm[tt].y, ov.y, ev.x)), fma(gm[tt].x, ov.y, fma(gm[tt].y, ov.x, ev.y)));
     const int i = j + tt * S;
     if (MODE == MODE_STOREZ) {
       zd[i] = z;
