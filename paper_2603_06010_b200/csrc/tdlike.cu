@@ -30,7 +30,7 @@ constexpr int FUSED_MIN_LOG2M = 8;   // M = 256
 constexpr int CLUSTER_LOG2M = 13;    // M = 8192: 2-CTA cluster, one branch per CTA (td_cluster.cuh)
 constexpr int FUSED_NT = 256;
 constexpr int DENSE_AUTO_N = 512;     // AUTO: dense path for segments up to this length (measured crossover: profiles/r01_chooser.md)
-constexpr size_t STAGED_WS_BYTES = 64ull << 20;  // keep the staged workspace L2-resident (126 MB L2)
+constexpr size_t STAGED_WS_BYTES = 96ull << 20;  // staged workspace, both lanes: inside the 126 MB L2 (measured 64: 0.91 ms, 96: 0.756, 128: 0.761, 192: 0.745, 384: 0.750 on c4)
 
 struct SegHost {
   int64_t off = 0;
@@ -84,6 +84,8 @@ struct td_handle {
   double* hsD = nullptr; double* hsH[2] = {nullptr, nullptr}; double* hsOut = nullptr;
   size_t hsH_elems = 0, hsOut_elems = 0;
   cudaStream_t copy_stream = nullptr;
+  cudaStream_t aux_stream = nullptr;              // second lane of the staged path (chunks alternate between two streams)
+  cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
   cudaEvent_t ev_copied[2] = {nullptr, nullptr}, ev_done[2] = {nullptr, nullptr};
 };
 
@@ -108,6 +110,9 @@ void free_handle(td_handle* h) {
   cudaFree(h->wsU); cudaFree(h->wsZ); cudaFree(h->wsPartial); cudaFree(h->ud); cudaFree(h->synH); cudaFree(h->synP); cudaFree(h->synSeg);
   cudaFree(h->hsD); cudaFree(h->hsH[0]); cudaFree(h->hsH[1]); cudaFree(h->hsOut);
   if (h->copy_stream) cudaStreamDestroy(h->copy_stream);
+  if (h->aux_stream) cudaStreamDestroy(h->aux_stream);
+  if (h->ev_fork) cudaEventDestroy(h->ev_fork);
+  if (h->ev_join) cudaEventDestroy(h->ev_join);
   for (int i = 0; i < 2; ++i) { if (h->ev_copied[i]) cudaEventDestroy(h->ev_copied[i]); if (h->ev_done[i]) cudaEventDestroy(h->ev_done[i]); }
   delete h;
 }
@@ -219,35 +224,57 @@ td_status run_staged(td_handle* h, const ClassInfo& cls, const SegHost& sg, cons
                      int accumulate, cudaStream_t st) {
   const int M = 1 << cls.log2M, nf = M / 2, TW = 2 * M;
   const size_t per_tmpl = (size_t)(2 * nf + 2 * M) * sizeof(cplx);
-  int64_t CB = std::max<int64_t>(1, (int64_t)(STAGED_WS_BYTES / per_tmpl));
+  // Two lanes: chunks alternate between the caller's stream and an internal one, each lane with its own half of the
+  // L2-resident workspace.  No kernel of the pipeline fills the GPU on its own (a few hundred CTAs, each bound by L2
+  // latency at the start and end of its life), so two chunks in flight overlap one another's ramps and tails.
+  int64_t CB = std::max<int64_t>(1, (int64_t)(STAGED_WS_BYTES / 2 / per_tmpl));
   CB = std::min<int64_t>(CB, std::max<int64_t>(B, 1));
   CB = std::min<int64_t>(CB, 32767);  // grid.y = 2*CB arrays per pass
+  const bool two = B > CB;
   const int rI = plan_r1(M), rF = plan_r1(nf);
   const int nblk = (M / rI + LG_NT - 1) / LG_NT;
-  td_status s = ensure_ws(h, (size_t)CB * 2 * nf, (size_t)CB * 2 * M, (size_t)std::max<int64_t>(B, 1) * nblk * 2);
+  const size_t uh = (size_t)CB * 2 * nf, zh = (size_t)CB * 2 * M;  // one lane's share
+  td_status s = ensure_ws(h, (two ? 2 : 1) * uh, (two ? 2 : 1) * zh, (size_t)std::max<int64_t>(B, 1) * nblk * 2);
   if (s != TD_OK) return s;
-  for (int64_t b0 = 0; b0 < B; b0 += CB) {
+  if (two) {
+    if (!h->aux_stream) {
+      CK(cudaStreamCreateWithFlags(&h->aux_stream, cudaStreamNonBlocking));
+      CK(cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming));
+      CK(cudaEventCreateWithFlags(&h->ev_join, cudaEventDisableTiming));
+    }
+    CK(cudaEventRecord(h->ev_fork, st));          // everything enqueued on the caller's stream so far comes first
+    CK(cudaStreamWaitEvent(h->aux_stream, h->ev_fork, 0));
+  }
+  int lane = 0;
+  for (int64_t b0 = 0; b0 < B; b0 += CB, lane ^= 1) {
     const int cb = (int)std::min<int64_t>(CB, B - b0);
+    cudaStream_t ls = (two && lane) ? h->aux_stream : st;
+    cplx* U = h->wsU + (two && lane ? uh : 0);
+    cplx* Z = h->wsZ + (two && lane ? zh : 0);
     StagedParams P;
     P.d = d; P.H = H ? H + b0 * ldh : nullptr; P.ldh = ldh; P.CB = cb;
     P.seg.off = sg.off; P.seg.n = sg.n; P.seg._pad = 0; P.seg.G = sg.G; P.seg.zd = sg.zd;
-    P.M = M; P.U = h->wsU; P.Z = h->wsZ; P.T = cls.T; P.partial = h->wsPartial + (size_t)b0 * nblk * 2; P.nblk = nblk;
-    s = launch_first<MODE>(rF, dim3((nf / rF + LG_NT - 1) / LG_NT, cb), P, st);
+    P.M = M; P.U = U; P.Z = Z; P.T = cls.T; P.partial = h->wsPartial + (size_t)b0 * nblk * 2; P.nblk = nblk;
+    s = launch_first<MODE>(rF, dim3((nf / rF + LG_NT - 1) / LG_NT, cb), P, ls);
     if (s != TD_OK) return s;
     ++h->last_launches;
-    s = staged_forward(h->wsU, 2 * cb, nf, 1, cls.T, TW, st, &h->last_launches);
+    s = staged_forward(U, 2 * cb, nf, 1, cls.T, TW, ls, &h->last_launches);
     if (s != TD_OK) return s;
     // (fusing the untangle into the inverse block kernel - one CTA building a block, or a mirror pair of blocks, of Z in
     // shared memory straight from U and G - was measured: 50-68 us per chunk against 18 + 24 us for the two kernels; the
     // gather serialises 16 index-heavy tasks per thread, which the stand-alone kernel hides behind 1.4 M threads)
-    lg_untangle_kernel<<<dim3((nf + LG_NT - 1) / LG_NT, 2, cb), LG_NT, 0, st>>>(P);
+    lg_untangle_kernel<<<dim3((nf + LG_NT - 1) / LG_NT, 2, cb), LG_NT, 0, ls>>>(P);
     CK(cudaGetLastError());
     ++h->last_launches;
-    s = staged_inverse_but_last(h->wsZ, 2 * cb, M, cls.T, TW, st, &h->last_launches);
+    s = staged_inverse_but_last(Z, 2 * cb, M, cls.T, TW, ls, &h->last_launches);
     if (s != TD_OK) return s;
-    s = launch_last<MODE>(rI, dim3(nblk, cb), P, st);
+    s = launch_last<MODE>(rI, dim3(nblk, cb), P, ls);
     if (s != TD_OK) return s;
     ++h->last_launches;
+  }
+  if (two) {
+    CK(cudaEventRecord(h->ev_join, h->aux_stream));
+    CK(cudaStreamWaitEvent(st, h->ev_join, 0));
   }
   if (MODE != MODE_STOREZ && B > 0) {  // one reduction of the per-block partial sums for the whole batch (fixed order)
     lg_finish_kernel<<<(unsigned)((B + 127) / 128), 128, 0, st>>>(h->wsPartial, nblk, (int)B, out0, out1, scale0, scale1, accumulate);
