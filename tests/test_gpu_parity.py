@@ -539,3 +539,20 @@ def test_empty_batch_is_a_no_op_everywhere():
         assert dh.numel() == 0 and hh.numel() == 0
         p0 = torch.zeros(0, 5, dtype=torch.float64, device="cuda")
         assert h.loglike_family_batch(d, tdb.TD_FAMILY_RINGDOWN, p0, w.fs).numel() == 0
+
+
+def test_long_segment_five_pass_plan():
+    """N = 131072 (M = 2^17 = [2,16,16,16,16]): the staged path with a generic global pass around the shared-memory
+    block kernels, the longest plan exercised; oracle route = library Levinson solve (pin P13; dense C would be 128 GiB)."""
+    N = 131072
+    rng = np.random.default_rng(N)
+    rho = W.acf_from_psd(4096.0, 2 * N, N)
+    d = rng.standard_normal(N) * 1e-21
+    H = rng.standard_normal((3, N)) * 1e-21
+    ref = O.loglike_batch_solve_toeplitz(rho, [N], d, H[:1])
+    with tdb.TDLikelihood(rho, [N]) as h:
+        out = h.loglike_batch(_dev(d), _dev(H)).cpu().numpy()
+        out2 = h.loglike_batch(_dev(d), _dev(H[::-1].copy())).cpu().numpy()
+    _assert_close(out[:1], ref, what="N = 131072")
+    assert np.array_equal(out, out2[::-1])          # a row's result does not depend on its slot in the batch
+    assert np.all(out < 0.0)
