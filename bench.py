@@ -197,7 +197,9 @@ def main():
 
     w = W.make(args.config, B=args.B)
     B, n_tot = w.B, w.n_tot
-    h = tdb.TDLikelihood(w.acf, w.seg_lengths, device=local)
+    t_setup = time.perf_counter()
+    h = tdb.TDLikelihood(w.acf, w.seg_lengths, device=local)   # S0: Levinson-Durbin + generator spectra, once per handle
+    t_setup = time.perf_counter() - t_setup
     if args.path:
         h.set_path(args.path)
     if args.fft_variant:
@@ -363,7 +365,8 @@ def main():
             "config": {"workload": f"{args.config}: {w.description}; N_tot={n_tot}, segments={list(map(int, w.seg_lengths))}, B={B} per GPU",
                        "path": {1: "fft", 2: "dense", 3: "dot"}.get(path_used, "?"),
                        "l2": f"{nbuf} distinct device copies of H rotated between steps (H = {8 * B * n_tot / 2**20:.0f} MiB each)",
-                       "parallelism": f"dp{world} over templates"},
+                       "parallelism": f"dp{world} over templates",
+                       "setup_ms_not_in_metric": round(1e3 * t_setup, 3)},
             "roofline": roofline, "roofline_hbm": roofline_hbm, "cpu_baseline": cpu, "e2e": e2e, "e2e_params": e2e_params,
             "gpu_launches": launches, "clocks": clocks}
     print(json.dumps(line))
