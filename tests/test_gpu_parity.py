@@ -556,3 +556,12 @@ def test_long_segment_five_pass_plan():
     _assert_close(out[:1], ref, what="N = 131072")
     assert np.array_equal(out, out2[::-1])          # a row's result does not depend on its slot in the batch
     assert np.all(out < 0.0)
+
+
+def test_phase_probe_reports_plausible_cycles_and_rejects_unknown_shapes():
+    lockstep = tdb.probe_phase(256, 1)
+    free = tdb.probe_phase(256, 8)
+    assert 1500.0 < free < lockstep < 8000.0       # floors ~2000 cycles; barrier-free groups overlap better
+    with pytest.raises(tdb.TDError) as e:
+        tdb.probe_phase(384, 3)
+    assert e.value.status == tdb.TD_EINVAL
