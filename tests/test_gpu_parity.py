@@ -565,3 +565,25 @@ def test_phase_probe_reports_plausible_cycles_and_rejects_unknown_shapes():
     with pytest.raises(tdb.TDError) as e:
         tdb.probe_phase(384, 3)
     assert e.value.status == tdb.TD_EINVAL
+
+
+def test_staged_two_lane_pipeline_on_a_side_stream():
+    """The staged path alternates chunks between the caller's stream and an internal one (fork / join events).
+    On a non-default stream, back to back, with the inputs produced on that same stream just before: results must be
+    bitwise repeatable, complete when the caller's stream is, and equal to the oracle on a sample."""
+    w = W.make("c4", B=150, n_scale=4)              # N = 16384: 61 templates per chunk and lane -> 3 chunks, both lanes
+    ref = O.loglike_batch_solve_toeplitz(w.acf, w.seg_lengths, w.d, w.H[:2])
+    s = torch.cuda.Stream()
+    with tdb.TDLikelihood(w.acf, w.seg_lengths) as h:
+        Hc = torch.as_tensor(w.H).pin_memory()
+        torch.cuda.synchronize()
+        with torch.cuda.stream(s):
+            d = torch.as_tensor(w.d).pin_memory().to("cuda", non_blocking=True)
+            H = Hc.to("cuda", non_blocking=True)   # the kernels of both lanes must wait for this copy
+            o1 = h.loglike_batch(d, H)
+            o2 = h.loglike_batch(d, H)
+            o1c = o1.clone()                        # ordered after the join on the caller's stream
+        s.synchronize()
+        assert h.last_launches() > 12               # more than two chunks' worth of kernels
+    assert torch.equal(o1c, o2)
+    _assert_close(o1c.cpu().numpy()[:2], ref, what="staged two-lane")
