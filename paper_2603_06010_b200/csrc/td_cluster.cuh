@@ -77,6 +77,13 @@ __device__ __forceinline__ uint32_t map_to_cta(uint32_t smem_addr, uint32_t rank
 __device__ __forceinline__ void st_cluster(uint32_t addr, cplx v) {
   asm volatile("st.shared::cluster.v2.f64 [%0], {%1, %2};" ::"r"(addr), "d"(v.x), "d"(v.y) : "memory");
 }
+// asynchronous remote store that also counts its 16 bytes on the destination CTA's mbarrier: the receiver waits on a
+// LOCAL mbarrier for the bytes instead of a cluster-wide barrier round trip
+__device__ __forceinline__ void st_async_cluster(uint32_t addr, cplx v, uint32_t mbar) {
+  asm volatile("st.async.shared::cluster.mbarrier::complete_tx::bytes.v2.f64 [%0], {%1, %2}, [%3];" ::"r"(addr), "d"(v.x),
+               "d"(v.y), "r"(mbar)
+               : "memory");
+}
 
 struct ClusterShape {
   static constexpr int LOG2M = 13, M = 1 << LOG2M, NF = M / 2, TW = 2 * M;
@@ -84,7 +91,7 @@ struct ClusterShape {
   static constexpr int TWS = 2 * M / RF1;  // 1024 base twiddles w_2M^k
   static constexpr int PADM = SmemArr::padded(M), PADNF = SmemArr::padded(NF);
   static constexpr size_t smem_bytes() {
-    return sizeof(cplx) * ((size_t)PADNF + (size_t)PADM + TWS) + sizeof(double) * (2 * NW + 2) + 32;
+    return sizeof(cplx) * ((size_t)PADNF + (size_t)PADM + TWS) + sizeof(double) * (2 * NW + 2) + 48;
   }
   // position of bin k in the inverse transform's input order (plan [32,16,16])
   __host__ __device__ static constexpr int pos(int k) { return ((k & 31) << 8) | (((k >> 5) & 15) << 4) | (k >> 9); }
@@ -104,6 +111,7 @@ __global__ void __launch_bounds__(ClusterShape::NT, 1) td_cluster_kernel(const F
   const uint32_t mbar_rows = smem_u32(xsum + 2);
   const uint32_t mbar_g = mbar_rows + 8;
   int* mid_count = reinterpret_cast<int*>(xsum + 4);
+  const uint32_t mbar_x = smem_u32(xsum + 5);              // half-results of the partner have landed in xbuf (tx bytes)
   double* stH = reinterpret_cast<double*>(sm);             // staged row (<= M doubles) in the U region
   cplx* xbuf = Z.p;                                        // exchange buffer [16][256] in the Z region
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -111,10 +119,11 @@ __global__ void __launch_bounds__(ClusterShape::NT, 1) td_cluster_kernel(const F
   const F4Own own = f4_own<Sh::RF1, true>(br, (int)(threadIdx.x >> 5));
   const uint32_t xbuf_remote = map_to_cta(smem_u32(xbuf), (uint32_t)(br ^ 1));
   const uint32_t xsum_remote = map_to_cta(smem_u32(xsum), 0u);
+  const uint32_t mbar_x_remote = map_to_cta(mbar_x, (uint32_t)(br ^ 1));
   const long long ncl = gridDim.x >> 1;
 
   for (int k = tid; k < Sh::TWS; k += NT) tw[k] = P.T[k];
-  if (tid == 0) { mbar_init(mbar_rows, 1); mbar_init(mbar_g, 1); *mid_count = 0; }
+  if (tid == 0) { mbar_init(mbar_rows, 1); mbar_init(mbar_g, 1); mbar_init(mbar_x, 1); *mid_count = 0; }
   __syncthreads();
 
   // rows of item (b, s): hrow is the row that gets staged (the template; d itself for STOREZ)
@@ -144,7 +153,7 @@ __global__ void __launch_bounds__(ClusterShape::NT, 1) td_cluster_kernel(const F
   long long b = blockIdx.x >> 1;
   int s = 0;
   bool have = b < P.B;
-  uint32_t par_rows = 0, par_g = 0;
+  uint32_t par_rows = 0, par_g = 0, par_x = 0;
   bool staged = false;
   if (have) {
     const double *dr, *hr; int nn;
@@ -256,6 +265,8 @@ __global__ void __launch_bounds__(ClusterShape::NT, 1) td_cluster_kernel(const F
       cplx x[32];
 #pragma unroll
       for (int q = 0; q < 32; ++q) x[q] = Z.ld(j + 256 * q);
+      // arm the exchange mbarrier for this item's 16 x 256 complex from the partner, then
+      if (tid == 0) mbar_expect_tx(mbar_x, (uint32_t)(16 * NT * sizeof(cplx)));
       cluster_arrive();  // (A) my Z region is free: the partner may write its half-results into it
       {
         // x_q *= conj(w_M^{j q}) (and conj(w_2M^j) on the odd branch); powers as w^{4 hi} * w^{lo}
@@ -292,16 +303,16 @@ __global__ void __launch_bounds__(ClusterShape::NT, 1) td_cluster_kernel(const F
       if (br == 0) {
         static_for<16, 32>([&](auto t) {
           constexpr int tt = decltype(t)::value;
-          st_cluster(xbuf_remote + (uint32_t)(((tt - 16) * 256 + j) * sizeof(cplx)), x[brevR<32>(tt)]);
+          st_async_cluster(xbuf_remote + (uint32_t)(((tt - 16) * 256 + j) * sizeof(cplx)), x[brevR<32>(tt)], mbar_x_remote);
         });
       } else {
         static_for<0, 16>([&](auto t) {
           constexpr int tt = decltype(t)::value;
-          st_cluster(xbuf_remote + (uint32_t)((tt * 256 + j) * sizeof(cplx)), x[brevR<32>(tt)]);
+          st_async_cluster(xbuf_remote + (uint32_t)((tt * 256 + j) * sizeof(cplx)), x[brevR<32>(tt)], mbar_x_remote);
         });
       }
-      cluster_arrive();  // (B) half-results delivered
-      cluster_wait();
+      mbar_wait(mbar_x, par_x);  // (B) the partner's half-results have landed (local mbarrier: no cluster barrier)
+      par_x ^= 1;
       static_for<0, 16>([&](auto t) {
         constexpr int tt = decltype(t)::value;
         const cplx mine = br ? x[brevR<32>(tt + 16)] : x[brevR<32>(tt)];
