@@ -91,7 +91,7 @@ struct ClusterShape {
   static constexpr int TWS = 2 * M / RF1;  // 1024 base twiddles w_2M^k
   static constexpr int PADM = SmemArr::padded(M), PADNF = SmemArr::padded(NF);
   static constexpr size_t smem_bytes() {
-    return sizeof(cplx) * ((size_t)PADNF + (size_t)PADM + TWS) + sizeof(double) * (2 * NW + 2) + 48;
+    return sizeof(cplx) * ((size_t)PADNF + (size_t)PADM + TWS) + sizeof(double) * (2 * NW + 2) + 48 + F4_SEGCACHE * sizeof(SegDev);
   }
   // position of bin k in the inverse transform's input order (plan [32,16,16])
   __host__ __device__ static constexpr int pos(int k) { return ((k & 31) << 8) | (((k >> 5) & 15) << 4) | (k >> 9); }
@@ -111,6 +111,8 @@ __global__ void __launch_bounds__(ClusterShape::NT, 1) td_cluster_kernel(const F
   const uint32_t mbar_rows = smem_u32(xsum + 2);
   const uint32_t mbar_g = mbar_rows + 8;
   int* mid_count = reinterpret_cast<int*>(xsum + 4);
+  SegDev* segS = reinterpret_cast<SegDev*>(xsum + 6);
+  const SegDev* segs = P.n_seg <= F4_SEGCACHE ? segS : P.segs;
   const uint32_t mbar_x = smem_u32(xsum + 5);              // half-results of the partner have landed in xbuf (tx bytes)
   double* stH = reinterpret_cast<double*>(sm);             // staged row (<= M doubles) in the U region
   cplx* xbuf = Z.p;                                        // exchange buffer [16][256] in the Z region
@@ -123,12 +125,13 @@ __global__ void __launch_bounds__(ClusterShape::NT, 1) td_cluster_kernel(const F
   const long long ncl = gridDim.x >> 1;
 
   for (int k = tid; k < Sh::TWS; k += NT) tw[k] = P.T[k];
+  if (tid < P.n_seg && tid < F4_SEGCACHE) segS[tid] = P.segs[tid];
   if (tid == 0) { mbar_init(mbar_rows, 1); mbar_init(mbar_g, 1); mbar_init(mbar_x, 1); *mid_count = 0; }
   __syncthreads();
 
   // rows of item (b, s): hrow is the row that gets staged (the template; d itself for STOREZ)
   auto rows = [&](long long b, int s, const double*& drow, const double*& hrow, int& n) -> bool {
-    const SegDev sg = P.segs[s];
+    const SegDev sg = segs[s];
     drow = P.d + sg.off;
     hrow = (MODE == MODE_STOREZ) ? drow : P.H + b * P.ldh + sg.off;
     n = sg.n;
@@ -186,7 +189,7 @@ __global__ void __launch_bounds__(ClusterShape::NT, 1) td_cluster_kernel(const F
     long long nb = b; int ns = s + 1;
     if (ns == P.n_seg) { ns = 0; nb = b + ncl; }
     const bool have_next = (MODE != MODE_STOREZ || nb == b) && nb < P.B;
-    const SegDev sg = P.segs[s];
+    const SegDev sg = segs[s];
     // ---------------- forward pass 1 (radix 16, stride 256) of THIS CTA's branch; task j = tid
     {
       const int j = tid;

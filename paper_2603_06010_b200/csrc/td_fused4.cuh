@@ -20,6 +20,8 @@
 
 namespace td {
 
+constexpr int F4_SEGCACHE = 8;  // segment records cached in shared memory (more segments: read from global per item)
+
 template <int LOG2M> struct Fused4Shape {
   static constexpr int M = 1 << LOG2M, NF = M / 2;
   static constexpr int RF1 = plan_r1(NF), RI1 = plan_r1(M);
@@ -28,7 +30,7 @@ template <int LOG2M> struct Fused4Shape {
   static constexpr int TWS = 2 * M / RF1;
   static constexpr int PADM = SmemArr::padded(M), PADNF = SmemArr::padded(NF);
   static constexpr size_t smem_bytes() {
-    return sizeof(cplx) * (2 * (size_t)PADNF + 2 * (size_t)PADM + TWS) + sizeof(double) * 2 * NW + 48;
+    return sizeof(cplx) * (2 * (size_t)PADNF + 2 * (size_t)PADM + TWS) + sizeof(double) * 2 * NW + 48 + F4_SEGCACHE * sizeof(SegDev);
   }
 };
 
@@ -167,6 +169,8 @@ __global__ void __launch_bounds__(Fused4Shape<LOG2M>::NT, 1) td_fused4_kernel(co
   int* mid_count = reinterpret_cast<int*>(red + 2 * NW + 2);
   int* last_count = mid_count + 1;
   double* totS = red + 2 * NW + 3;  // running sums of the current template over its segments
+  SegDev* segS = reinterpret_cast<SegDev*>(red + 2 * NW + 6);
+  const SegDev* segs = P.n_seg <= F4_SEGCACHE ? segS : P.segs;
   double* stH = reinterpret_cast<double*>(sm);
   double* stD = stH + M;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -175,11 +179,12 @@ __global__ void __launch_bounds__(Fused4Shape<LOG2M>::NT, 1) td_fused4_kernel(co
   const F4Own own = f4_own<RF1, true>(br, wb);
 
   for (int k = tid; k < Sh::TWS; k += NT) tw[k] = P.T[k];
+  if (tid < P.n_seg && tid < F4_SEGCACHE) segS[tid] = P.segs[tid];
   if (tid == 0) { mbar_init(mbar_rows, 1); mbar_init(mbar_g, 1); *mid_count = 0; *last_count = 0; totS[0] = 0.0; totS[1] = 0.0; }
   __syncthreads();
 
   auto rows = [&](long long b, int s, const double*& drow, const double*& hrow, int& n) -> bool {
-    const SegDev sg = P.segs[s];
+    const SegDev sg = segs[s];
     drow = P.d + sg.off;
     hrow = (MODE == MODE_STOREZ) ? drow : P.H + b * P.ldh + sg.off;
     n = sg.n;
@@ -219,7 +224,7 @@ __global__ void __launch_bounds__(Fused4Shape<LOG2M>::NT, 1) td_fused4_kernel(co
     long long nb = b; int ns = s + 1;
     if (ns == P.n_seg) { ns = 0; nb = b + gridDim.x; }
     const bool have_next = (MODE != MODE_STOREZ || nb == b) && nb < P.B;
-    const SegDev sg = P.segs[s];
+    const SegDev sg = segs[s];
     // ---------------- forward pass 1 (radix RF1, stride 256): both branches from one set of inputs
     {
       constexpr int NTASK = NF / RF1;  // 256
