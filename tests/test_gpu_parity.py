@@ -587,3 +587,20 @@ def test_staged_two_lane_pipeline_on_a_side_stream():
         assert h.last_launches() > 12               # more than two chunks' worth of kernels
     assert torch.equal(o1c, o2)
     _assert_close(o1c.cpu().numpy()[:2], ref, what="staged two-lane")
+
+
+def test_many_segments_in_one_size_class():
+    """Ten segments of one size class: more than the fused kernel caches in shared memory (F4_SEGCACHE = 8), so the
+    segment records come from global memory; plus nine segments of the cluster class."""
+    rng = np.random.default_rng(21)
+    for lens in ([1024] * 10, [5000] * 9):
+        rho = W.acf_from_psd(4096.0, 2 * 8192, max(lens))
+        acf = np.concatenate([(1.0 + 0.1 * k) * rho[:n] for k, n in enumerate(lens)])
+        nt = sum(lens)
+        d = rng.standard_normal(nt) * 1e-21
+        H = rng.standard_normal((5, nt)) * 1e-21
+        ref = O.loglike_batch(acf, lens, d, H)
+        with tdb.TDLikelihood(acf, lens) as h:
+            out = h.loglike_batch(_dev(d), _dev(H)).cpu().numpy()
+            assert h.last_launches() == 1
+        _assert_close(out, ref, what=f"{len(lens)} segments of {lens[0]}")
