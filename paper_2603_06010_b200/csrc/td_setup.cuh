@@ -5,6 +5,7 @@
 //   twiddle table, and the packed generator g = a - i b (b = (0, a_{N-1}, ..., a_1)) whose
 //   length-2M transform, conjugated, is G = conj(A^) + i conj(B^).
 #pragma once
+#include <cooperative_groups.h>
 #include "td_common.cuh"
 
 namespace td {
@@ -21,7 +22,7 @@ struct LevSeg {
   const double* rho;  // device, n doubles
   double* a;          // device, n doubles (output)
   int n;
-  int _pad;
+  int coop;           // handled by levinson_coop_kernel (long segment): levinson_kernel skips it
 };
 
 constexpr int LEV_NT = 1024;
@@ -32,6 +33,7 @@ __global__ void __launch_bounds__(LEV_NT) levinson_kernel(const LevSeg* __restri
   __shared__ double red[LEV_NT / 32];
   __shared__ double bc;
   const LevSeg sg = segs[blockIdx.x];
+  if (sg.coop) return;
   const double* __restrict__ rho = sg.rho;
   double* a = sg.a;
   const int n = sg.n, tid = threadIdx.x;
@@ -81,6 +83,79 @@ __global__ void __launch_bounds__(LEV_NT) levinson_kernel(const LevSeg* __restri
     v_out[blockIdx.x] = E;
     logdet_out[blockIdx.x] = logdet;
     status[blockIdx.x] = 0;
+  }
+}
+
+// The same recursion for one LONG segment on many CTAs (cooperative launch, two grid-wide barriers per order): a single
+// CTA streams a and rho (2 x 8 N bytes at the last orders) through one SM for every order, which is 0.96 s at N = 65536;
+// spread over the grid the step is bounded by the barrier, not by one SM's bandwidth.  Every thread carries its own copy
+// of E and log det (identical arithmetic on identical partial sums), so the SPD test exits the whole grid uniformly.
+constexpr int LEVC_NT = 512;
+constexpr int LEV_COOP_MIN_N = 16384;
+
+__global__ void __launch_bounds__(LEVC_NT) levinson_coop_kernel(const LevSeg sg, double* partial, double* v_out,
+                                                               double* logdet_out, int* status) {
+  namespace cg = cooperative_groups;
+  cg::grid_group grid = cg::this_grid();
+  __shared__ double red[LEVC_NT / 32];
+  __shared__ double bc;
+  const double* __restrict__ rho = sg.rho;
+  double* a = sg.a;
+  const int n = sg.n, tid = threadIdx.x, G = gridDim.x;
+  const int gtid = blockIdx.x * LEVC_NT + tid, gsz = G * LEVC_NT;
+  const double rho0 = rho[0];
+  if (!(rho0 > 0.0) || !isfinite(rho0)) {
+    if (gtid == 0) *status = 2;
+    return;
+  }
+  for (int j = gtid; j < n; j += gsz) a[j] = (j == 0) ? 1.0 : 0.0;
+  double E = rho0, logdet = log(rho0);
+  grid.sync();
+  for (int k = 1; k < n; ++k) {
+    double acc = 0.0;
+    for (int j = gtid; j < k; j += gsz) acc = fma(a[j], rho[k - j], acc);
+    acc = warp_sum(acc);
+    if ((tid & 31) == 0) red[tid >> 5] = acc;
+    __syncthreads();
+    if (tid < 32) {
+      double v = tid < LEVC_NT / 32 ? red[tid] : 0.0;
+      v = warp_sum(v);
+      if (tid == 0) partial[(size_t)(k & 1) * G + blockIdx.x] = v;
+    }
+    grid.sync();
+    if (tid < 32) {  // fixed order: lane l adds partials l, l + 32, ...; then the warp tree
+      double v = 0.0;
+      for (int c = tid; c < G; c += 32) v += partial[(size_t)(k & 1) * G + c];
+      v = warp_sum(v);
+      if (tid == 0) bc = v;
+    }
+    __syncthreads();
+    const double kk = -bc / E;
+    if (!(fabs(kk) < 1.0)) {  // also catches NaN; the same value in every thread of the grid
+      if (gtid == 0) *status = 2;
+      return;
+    }
+    for (int j = 1 + gtid; 2 * j < k; j += gsz) {
+      const double aj = a[j], ak = a[k - j];
+      a[j] = fma(kk, ak, aj);
+      a[k - j] = fma(kk, aj, ak);
+    }
+    if (gtid == 0) {
+      if ((k & 1) == 0) { const double am = a[k / 2]; a[k / 2] = fma(kk, am, am); }
+      a[k] = kk;
+    }
+    E *= (1.0 - kk * kk);
+    logdet += log(E);
+    if (!(E > 0.0)) {
+      if (gtid == 0) *status = 2;
+      return;
+    }
+    grid.sync();
+  }
+  if (gtid == 0) {
+    *v_out = E;
+    *logdet_out = logdet;
+    *status = 0;
   }
 }
 

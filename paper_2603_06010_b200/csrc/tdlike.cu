@@ -557,12 +557,30 @@ static td_status create_impl(td_handle* h, const double* acf, const int64_t* seg
   for (int s = 0; s < n_seg; ++s) {
     SegHost& sg = h->segs[s];
     CK(cudaMalloc(&sg.a, sizeof(double) * sg.n));
-    lev[s].rho = d_rho + sg.off; lev[s].a = sg.a; lev[s].n = sg.n; lev[s]._pad = 0;
+    lev[s].rho = d_rho + sg.off; lev[s].a = sg.a; lev[s].n = sg.n; lev[s].coop = sg.n >= LEV_COOP_MIN_N ? 1 : 0;
   }
   CK(cudaMemcpy(d_lev, lev.data(), sizeof(LevSeg) * n_seg, cudaMemcpyHostToDevice));
   levinson_kernel<<<n_seg, LEV_NT>>>(d_lev, d_v, d_ld, d_status);
   CK(cudaGetLastError());
-  CK(cudaDeviceSynchronize());
+  {
+    // long segments: the cooperative multi-CTA recursion, one launch each
+    int coop_ok = 0, nb = 0;
+    CK(cudaDeviceGetAttribute(&coop_ok, cudaDevAttrCooperativeLaunch, h->device));
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, levinson_coop_kernel, LEVC_NT, 0));
+    const int G = std::min(48, std::max(1, nb) * h->num_sms);
+    double* d_part = nullptr;
+    for (int s = 0; s < n_seg; ++s) {
+      if (!lev[s].coop) continue;
+      if (!coop_ok) return TD_EUNSUPPORTED;
+      if (!d_part) CK(cudaMalloc(&d_part, sizeof(double) * 2 * G));
+      LevSeg one = lev[s];
+      double* pv = d_v + s; double* pl = d_ld + s; int* ps = d_status + s;
+      void* args[] = {&one, &d_part, &pv, &pl, &ps};
+      CK(cudaLaunchCooperativeKernel((void*)levinson_coop_kernel, dim3(G), dim3(LEVC_NT), args, 0, 0));
+    }
+    CK(cudaDeviceSynchronize());
+    cudaFree(d_part);
+  }
   std::vector<int> status(n_seg);
   std::vector<double> v(n_seg), ld(n_seg);
   CK(cudaMemcpy(status.data(), d_status, sizeof(int) * n_seg, cudaMemcpyDeviceToHost));

@@ -604,3 +604,28 @@ def test_many_segments_in_one_size_class():
             out = h.loglike_batch(_dev(d), _dev(H)).cpu().numpy()
             assert h.last_launches() == 1
         _assert_close(out, ref, what=f"{len(lens)} segments of {lens[0]}")
+
+
+@pytest.mark.parametrize("n", [16384, 20001])
+def test_cooperative_setup_matches_oracle_levinson(n):
+    """Segments of >= 16384 samples run the recursion on a cooperative multi-CTA grid (levinson_coop_kernel)."""
+    rho = W.acf_from_psd(4096.0, 2 * 65536, n)
+    a_ref, v_ref, ld_ref = O.levinson_durbin_fast(rho)
+    with tdb.TDLikelihood(rho, [n]) as h:
+        a = h.generator(0)
+        info = h.info()
+    assert np.max(np.abs(a - a_ref)) <= 1e-10 * np.max(np.abs(a_ref))
+    assert abs(info["v"][0] - v_ref) <= 1e-11 * v_ref
+    assert abs(info["logdet"][0] - ld_ref) <= 1e-10 * abs(ld_ref)
+
+
+def test_long_non_spd_acf_is_rejected_by_the_cooperative_setup():
+    bad = W.acf_from_psd(4096.0, 2 * 65536, 20000).copy()
+    bad[1] = 1.5 * bad[0]                              # |rho_1| > rho_0: not positive definite
+    with pytest.raises(tdb.TDError) as e:
+        tdb.TDLikelihood(bad, [20000])
+    assert e.value.status == tdb.TD_ENOTSPD
+    bad[1] = float("nan")
+    with pytest.raises(tdb.TDError) as e:
+        tdb.TDLikelihood(bad, [20000])
+    assert e.value.status == tdb.TD_ENOTSPD
