@@ -5,8 +5,8 @@
 //   1 sine-Gaussian (c3)         (A, f, w, phi, t0):        A exp(-((t_i - t0)/w)^2) cos(2 pi f t_i + phi)
 //   2 chirp (c4)                 (A, f0, fdot, phi, alpha): A tukey_alpha(i/(n-1)) cos(2 pi (f0 t_i + fdot t_i^2 / 2) + phi)
 // A caller (a sampler) then ships 5 doubles per template instead of N: the rows are written to a scratch panel that
-// is consumed by the likelihood kernels chunk by chunk while it is still L2-resident, so H never crosses PCIe and
-// (for chunks that fit L2) never reaches HBM.
+// is consumed by the likelihood kernels chunk by chunk (about 128 MB each: through L2, spilling to HBM), so H never
+// crosses PCIe.
 #pragma once
 #include "td_common.cuh"
 

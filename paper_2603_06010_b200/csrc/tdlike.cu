@@ -756,8 +756,10 @@ td_status td_loglike_family_batch(td_handle* h, const double* d, int family, con
     CK(cudaMalloc(&h->synSeg, sizeof(SynSeg) * h->n_seg));
     CK(cudaMemcpy(h->synSeg, hs.data(), sizeof(SynSeg) * h->n_seg, cudaMemcpyHostToDevice));
   }
-  // chunk: a whole number of waves of the persistent kernels, about 64 MB so the panel (mostly) stays in the 126 MB L2
-  int64_t CH = std::max<int64_t>(1, (66ll << 20) / (8 * ldh));
+  // chunk: a whole number of waves of the persistent kernels, about 128 MB (measured on c2 / c3 / c5: 64 MB chunks, which stay
+  // in L2, give 11.1-11.9 / 1.47 / 1.61 M evals/s end to end, 136 MB chunks 12.2 / 1.51 / 1.64: fewer launches and tails
+  // outweigh the panel's trip through HBM, which the ALU-bound kernels hide)
+  int64_t CH = std::max<int64_t>(1, (136ll << 20) / (8 * ldh));
   if (CH > h->num_sms) CH -= CH % h->num_sms;
   CH = std::min<int64_t>(CH, B);
   if ((size_t)(CH * ldh) > h->synH_elems) {
