@@ -27,9 +27,14 @@ Pins (tests/test_oracle_pins.py, all `-m "not gpu"`): brute-force inverse by Gau
 loops at N <= 256 (P1), white noise closed form (P2), AR(1) tridiagonal closed form (P3),
 Levinson/Gohberg-Semencul route vs Cholesky route (P4), generator residual (P5), inverse
 Cholesky row (P6), chi-square invariant (P7), invariances (P8), block additivity (P9),
-circulant/Whittle limit = Eq. 1 (P10), bilinear identity / Eq. 13 (P11), Eq. 14 as printed
-(P12), independent library Levinson solve (P13), injection sanity (P14).
+circulant/Whittle limit = Eq. 1 (P10), bilinear identity / Eq. 13 (P11: also the sum over
+segments of inner_batch against single-segment calls and the brute-force bilinear form, and
+snrs against the white-noise closed form), Eq. 14 as printed (P12), independent library
+Levinson solve (P13), injection sanity (P14); the chunk loop (B > 1024) and the `factors=`
+branch against the AR(1) closed form row by row (test_p1_p9_large_batch_...).
 Every function below is covered by at least one of them; nothing here is "parity unpinned".
+The template families / projection of the step before the hot path live in oracle/templates.py
+(pins P15-P18).
 """
 from __future__ import annotations
 

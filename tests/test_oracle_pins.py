@@ -13,6 +13,7 @@ import pytest
 import scipy.linalg as sla
 
 from oracle import td_oracle as O
+from oracle import templates as OT
 from paper_2603_06010_b200 import workloads as W
 
 GOLD = os.path.join(os.path.dirname(__file__), "golden")
@@ -99,7 +100,7 @@ def test_p3_golden_file():
 
 
 # ---------------------------------------------------------------- P4 two exact routes
-@pytest.mark.parametrize("n", [17, 256, 1024])
+@pytest.mark.parametrize("n", [17, 256, 1024, 4096])
 def test_p4_levinson_gs_vs_cholesky(n):
     rng = np.random.default_rng(4)
     rho = _psd_rho(n)
@@ -222,8 +223,96 @@ def test_p11_bilinear_and_snr():
     # symmetry <x,y> = <y,x>: swap roles of d and h_1
     dh2, _ = O.inner_batch(w.acf, w.seg_lengths, w.H[1], w.d[None, :])
     assert _rel(dh2[0], dh[1]) < 1e-12
-    mf, eff2 = O.snrs(w.acf, w.seg_lengths, w.d, w.H)
-    assert np.allclose(mf, dh / np.sqrt(hh)) and np.allclose(eff2, 2 * dh - hh, rtol=1e-9)
+
+
+def test_p11_inner_batch_sums_over_segments():
+    """<x,y> over several segments = sum of the single-segment values, with different
+    scales per segment so that `=` instead of `+=` (or a dropped segment) cannot pass; <d,d> against quadform."""
+    rng = np.random.default_rng(11)
+    lens = [90, 41, 130]
+    rho = _psd_rho(max(lens))
+    scales = [1.0, 0.6, 2.2]
+    acf = np.concatenate([s * rho[:n] for s, n in zip(scales, lens)])
+    nt = sum(lens)
+    d = rng.standard_normal(nt) * 1e-21
+    H = rng.standard_normal((7, nt)) * 1e-21
+    dh, hh = O.inner_batch(acf, lens, d, H)
+    dh_parts, hh_parts, dd_parts = np.zeros(7), np.zeros(7), 0.0
+    off = 0
+    for s, n in zip(scales, lens):
+        a, b = O.inner_batch(s * rho[:n], [n], d[off:off + n], H[:, off:off + n])
+        dh_parts += a
+        hh_parts += b
+        dd_parts += O.quadform(s * rho[:n], d[off:off + n])
+        off += n
+    assert np.max(np.abs(dh - dh_parts)) <= 1e-12 * np.max(np.abs(hh_parts))
+    assert np.max(np.abs(hh - hh_parts) / hh_parts) < 1e-12
+    # every segment contributes: no single partial sum equals the total
+    a0, b0 = O.inner_batch(scales[0] * rho[:lens[0]], [lens[0]], d[:lens[0]], H[:, :lens[0]])
+    assert np.min(np.abs(hh - b0) / hh) > 0.1
+    dd = O.inner_batch(acf, lens, d, d[None, :])[1][0]
+    assert _rel(dd, dd_parts) < 1e-12
+    # and per row against the brute-force bilinear form x^T C^-1 y = (Q(x+y) - Q(x-y)) / 4 at a small size
+    lens2 = [12, 9]
+    acf2 = np.concatenate([W.ar_acf([0.5, -0.2], 1.3, 12), 2.0 * W.ar_acf([0.5, -0.2], 1.3, 9)])
+    x = rng.standard_normal(21)
+    Y = rng.standard_normal((3, 21))
+    dh2, hh2 = O.inner_batch(acf2, lens2, x, Y)
+    for b in range(3):
+        want_dh = want_hh = 0.0
+        for lo, hi in ((0, 12), (12, 21)):
+            r = acf2[lo:hi]
+            want_dh += 0.25 * (O.quadform_bruteforce(r, x[lo:hi] + Y[b, lo:hi]) - O.quadform_bruteforce(r, x[lo:hi] - Y[b, lo:hi]))
+            want_hh += O.quadform_bruteforce(r, Y[b, lo:hi])
+        assert abs(dh2[b] - want_dh) < 1e-11 * want_hh and _rel(hh2[b], want_hh) < 1e-11
+
+
+def test_p11_snrs_white_noise_hand_case():
+    """Eq. 13 quantities where they have a closed form: white noise of variance s2 gives <x,y> = x.y / s2, so
+    rho_mf = d.h / (sigma sqrt(h.h)) and rho_eff^2 = (d.d - (d-h).(d-h)) / s2."""
+    rng = np.random.default_rng(13)
+    lens, s2 = [50, 30], [2.5e-42, 0.4e-42]
+    acf = np.zeros(80)
+    acf[0], acf[50] = s2
+    d = rng.standard_normal(80) * 1e-21
+    H = rng.standard_normal((4, 80)) * 1e-21
+    wgt = np.concatenate([np.full(50, 1 / s2[0]), np.full(30, 1 / s2[1])])
+    mf, eff2 = O.snrs(acf, lens, d, H)
+    want_mf = (H * wgt) @ d / np.sqrt(np.sum(H * H * wgt, axis=1))
+    r = d[None, :] - H
+    want_eff2 = np.sum(d * d * wgt) - np.sum(r * r * wgt, axis=1)
+    assert np.max(np.abs(mf - want_mf) / np.abs(want_mf)) < 1e-12
+    assert np.max(np.abs(eff2 - want_eff2)) < 1e-12 * np.sum(d * d * wgt)
+    # a template equal to the data: rho_mf = sqrt(<d,d>), rho_eff^2 = <d,d>
+    mf1, eff1 = O.snrs(acf, lens, d, d[None, :])
+    assert _rel(mf1[0] ** 2, np.sum(d * d * wgt)) < 1e-12 and _rel(eff1[0], np.sum(d * d * wgt)) < 1e-12
+
+
+def test_p1_p9_large_batch_chunk_loop_and_cached_factors():
+    """B = 1500 > the 1024-row chunk of loglike_batch / inner_batch, through the `factors=` branch bench.py times:
+    every row against the AR(1) closed form (P3), two segments of different variance (P9)."""
+    rng = np.random.default_rng(15)
+    phi, lens, s2 = 0.8, [24, 17], [1.7, 0.3]
+    acf = np.concatenate([s * phi ** np.arange(n) / (1 - phi * phi) for s, n in zip(s2, lens)])
+    nt, B = sum(lens), 1500
+    d = rng.standard_normal(nt)
+    H = rng.standard_normal((B, nt))
+    R = d[None, :] - H
+    want = np.zeros(B)
+    off = 0
+    for s, n in zip(s2, lens):
+        x = R[:, off:off + n]
+        want += ((1 - phi * phi) * x[:, 0] ** 2 + np.sum((x[:, 1:] - phi * x[:, :-1]) ** 2, axis=1)) / s
+        off += n
+    fac = O.factorize(acf, lens)
+    for kw in ({}, {"factors": fac}, {"chunk": 7}):
+        got = O.loglike_batch(acf, lens, d, H, **kw)
+        assert np.max(np.abs(-2 * got - want) / want) < 1e-12
+    # rows beyond the first chunk are really computed (not left at zero) and differ from one another
+    assert np.all(want[1024:] > 0) and len(np.unique(np.round(want[1024:], 9))) == B - 1024
+    dh, hh = O.inner_batch(acf, lens, d, H)
+    dd = -2 * O.loglike_batch(acf, lens, d, np.zeros((1, nt)))[0]
+    assert np.max(np.abs(want - (dd - 2 * dh + hh)) / (dd + hh)) < 1e-12
 
 
 # ---------------------------------------------------------------- P12 Eq. 14 as printed
@@ -251,6 +340,97 @@ def test_p14_injection(name, scale):
     n = w.n_tot
     assert abs(ll[0] + n / 2) < 4.5 * np.sqrt(n / 2)      # logL_0 = -1/2 n^T C^-1 n ~ -N/2 +- sqrt(N/2)
     assert ll[0] > ll[1] and ll[0] > ll[2]                # the injected template fits best
+
+
+# ---------------------------------------------------------------- P15-P18 template families (oracle/templates.py)
+def _golden_template_rows():
+    fam = {"ringdown": OT.RINGDOWN, "sine_gaussian": OT.SINE_GAUSSIAN, "chirp": OT.CHIRP}
+    for line in open(os.path.join(GOLD, "templates.txt")):
+        if not line.strip() or line[0] == "#":
+            continue
+        head, tail = line.split("|")
+        f = head.split()
+        fs, n = float(f[1]), int(f[2])
+        A, p1, p2, phi, p4 = float(f[3]), float(f[4]), float(f[5]), float(f[6]) * np.pi, float(f[7])
+        want = {int(kv.split("=")[0]): float(kv.split("=")[1]) for kv in tail.split()}
+        yield fam[f[0]], fs, n, (A, p1, p2, phi, p4), want
+
+
+def test_p15_templates_golden_file():
+    """Hand-evaluated samples (tests/golden/templates.txt): onset on and between samples, Gaussian envelope centred
+    at t0 with the carrier counted from t = 0, chirp phase and Tukey taper."""
+    rows = list(_golden_template_rows())
+    assert len(rows) == 4
+    for fam, fs, n, p, want in rows:
+        H = OT.family_rows(fam, np.array([p]), [n], fs)[0]
+        t = np.arange(n) / fs
+        direct = {OT.RINGDOWN: OT.ringdown, OT.SINE_GAUSSIAN: OT.sine_gaussian, OT.CHIRP: OT.chirp}[fam](t, *p)
+        assert np.array_equal(H, direct)
+        for i, v in want.items():
+            assert abs(H[i] - v) <= 2e-15 * max(abs(p[0]), 1.0), (fam, i, H[i], v)
+
+
+@pytest.mark.parametrize("n,alpha", [(9, 0.5), (64, 0.1), (1000, 0.1), (8192, 0.1), (50, 1.0), (31, 0.25)])
+def test_p16_tukey_against_scipy(n, alpha):
+    import scipy.signal.windows as sw
+    assert np.max(np.abs(OT.tukey(n, alpha) - sw.tukey(n, alpha, sym=True))) < 1e-14
+
+
+def test_p17_projection_fold_identity():
+    """F+ h_c + Fx h_s with a time shift is ONE damped sinusoid: A hypot(F+,Fx) cos(theta + phi - atan2(Fx,F+))
+    = F+ cos(theta + phi) + Fx sin(theta + phi)  (the row packing of td_loglike_family_batch)."""
+    rng = np.random.default_rng(17)
+    fs, n = 4096.0, 700
+    t = np.arange(n) / fs
+    for _ in range(20):
+        A, f, tau, phi = rng.uniform(0.5, 2), rng.uniform(100, 400), rng.uniform(2e-3, 2e-2), rng.uniform(0, 2 * np.pi)
+        t0, Fp, Fx, dt = rng.uniform(0.02, 0.1), rng.uniform(-1, 1), rng.uniform(-1, 1), rng.uniform(-0.01, 0.01)
+        literal = OT.projected_ringdown(t, A, f, tau, phi, t0, Fp, Fx, dt)
+        A2, phi2, t02 = OT.fold_projection(A, phi, t0, Fp, Fx, dt)
+        folded = OT.ringdown(t, A2, f, tau, phi2, t02)
+        assert np.max(np.abs(literal - folded)) <= 1e-14 * A * np.hypot(Fp, Fx) + 1e-300
+        assert np.all(literal[t < t0 + dt] == 0.0) and literal[t >= t0 + dt][0] != 0.0
+    # the scalar identity itself, at hand-picked angles: F+ = 3, Fx = 4 -> amplitude 5, phase atan2(4, 3)
+    for x in (0.0, 0.3, 2.0):
+        assert abs(3 * np.cos(x) + 4 * np.sin(x) - 5 * np.cos(x - np.arctan2(4.0, 3.0))) < 1e-14
+
+
+def test_p17_segment_time_fold():
+    """A row written in the time of a segment that starts at ts equals the record-time waveform on that segment's
+    samples (gaps: only kept samples exist on the device)."""
+    fs, ts, n = 4096.0, 5128 / 4096.0, 300
+    t_seg = np.arange(n) / fs
+    t_rec = ts + t_seg
+    row = (1.3, 180.0, 0.02, 0.7, 1.27)
+    A, f, w, phi, t0 = OT.fold_segment_time(OT.SINE_GAUSSIAN, row, ts)
+    assert np.max(np.abs(OT.sine_gaussian(t_seg, A, f, w, phi, t0) - OT.sine_gaussian(t_rec, *row))) < 1e-11
+    A, f, tau, phi, t0 = OT.fold_segment_time(OT.RINGDOWN, row, ts)
+    assert np.max(np.abs(OT.ringdown(t_seg, A, f, tau, phi, t0) - OT.ringdown(t_rec, *row))) < 1e-11
+
+
+def test_p18_chirp_instantaneous_phase():
+    """cos(2 pi (f0 t + fdot t^2/2) + phi): where f0 t + fdot t^2/2 is an integer the sample is +A w, at a half-integer
+    -A w, at a quarter 0; f0 = 16, fdot = 32, fs = 64 -> t = 1/4: 4 + 1 = 5; t = 1/8: 2 + 1/4; t = 3/8: 6 + 9/4 = 8.25;
+    t = 1/2: 8 + 4 = 12; and with phi = pi the sign flips."""
+    fs, n = 64.0, 65
+    t = np.arange(n) / fs
+    h = OT.chirp(t, 2.0, 16.0, 32.0, 0.0, 1e-9)          # alpha -> 0: the taper touches only the end samples
+    assert abs(h[16] - 2.0) < 1e-13 and abs(h[32] - 2.0) < 1e-12
+    assert abs(h[8]) < 1e-13 and abs(h[24]) < 1e-12
+    hp = OT.chirp(t, 2.0, 16.0, 32.0, np.pi, 1e-9)
+    assert abs(hp[16] + 2.0) < 1e-13
+    # instantaneous frequency f0 + fdot t: between consecutive samples the phase advances by 2 pi (f0 + fdot (t + dt/2)) dt
+    ph = 2 * np.pi * (16.0 * t + 16.0 * t * t)
+    assert np.allclose(np.diff(ph), 2 * np.pi * (16.0 + 32.0 * (t[:-1] + 0.5 / fs)) / fs, rtol=1e-13)
+
+
+@pytest.mark.parametrize("name,B,scale", [("c1", 5, 1), ("c2", 4, 4), ("c3", 4, 4), ("c4", 3, 16), ("c5", 4, 8), ("d2", 6, 1)])
+def test_input_generator_rows_equal_oracle_templates(name, B, scale):
+    """The rows of H that the shared input generator draws are the oracle's family formulas at the parameters it
+    reports (w.params): ties the inputs of every family test to oracle/templates.py, in both directions."""
+    w = W.make(name, B=B, n_scale=scale)
+    H = OT.family_rows(w.family, w.params, w.seg_lengths, w.fs)
+    assert np.max(np.abs(H - w.H)) <= 1e-9 * np.max(np.abs(w.H))
 
 
 def test_not_spd_is_rejected():
