@@ -10,13 +10,16 @@
 //     odd branch: per CTA  U = NF complex (64 KiB), Z = M complex (128 KiB), twiddle table 16 KiB.
 //   * plans NF = [16,16,16], M = [32,16,16]; forward passes 2-3, "mid" (untangle x generator + first
 //     inverse pass in registers) and inverse pass 2 are the warp-local pieces of td_fused4.cuh.
-//   * the last pass (radix 32 in registers) ends with z_i = e_i + w_2M^{-i} o_i, which needs both
-//     branches: each CTA keeps the half of its outputs that falls in its own half of the index range
-//     (rank 0: i < M/2, rank 1: i >= M/2) and stores the other half into the partner's shared memory
-//     through distributed shared memory (st.shared::cluster), between two cluster barriers; then each
-//     CTA reduces its half of S5.  Rank 1's partial sum travels to rank 0 the same way.
-//   * the template row is TMA-bulk-prefetched into the (dead) U region, the branch's generator spectrum
-//     into the Z region; d is subtracted on load straight from global memory (L2-resident).
+//   * generator values, data samples and pass-2 twiddles of every thread live in tensor memory (td_fused4.cuh), so the
+//     Z region carries nothing between the last pass of one item and mid of the next.  That makes the exchange of the
+//     last pass ASYNCHRONOUS: z_i = e_i + w_2M^{-i} o_i needs both branches, each CTA keeps the outputs of its own half
+//     of the index range (rank 0: i < M/2, rank 1: i >= M/2).  A thread writes its own half into its warp's Z blocks,
+//     sends the other half into the partner warp's Z blocks with st.async (distributed shared memory, bytes counted
+//     on the receiver's mbarrier) and goes straight on to the next item's forward passes; the sum of squares of the
+//     previous item (S5) is taken just before mid overwrites those blocks - by then the partner's half has long arrived
+//     (r01: a quarter of the warp samples sat in this exchange).  The layout is warp-closed: a warp reads back only the
+//     blocks it overwrites itself, so the deferred S5 needs no CTA barrier.
+//   * the template row is TMA-bulk-prefetched into the (dead) U region.
 // Only H is read from HBM; nothing but out[b] is written.
 #pragma once
 #include "td_fused4.cuh"
@@ -91,7 +94,7 @@ struct ClusterShape {
   static constexpr int TWS = 2 * M / RF1;  // 1024 base twiddles w_2M^k
   static constexpr int PADM = SmemArr::padded(M), PADNF = SmemArr::padded(NF);
   static constexpr size_t smem_bytes() {
-    return sizeof(cplx) * ((size_t)PADNF + (size_t)PADM + TWS) + sizeof(double) * (2 * NW + 2) + 48 + F4_SEGCACHE * sizeof(SegDev);
+    return sizeof(cplx) * ((size_t)PADNF + (size_t)PADM + TWS) + sizeof(double) * (4 * NW + 2) + 48 + 64 + F4_SEGCACHE * sizeof(SegDev);
   }
   // position of bin k in the inverse transform's input order (plan [32,16,16])
   __host__ __device__ static constexpr int pos(int k) { return ((k & 31) << 8) | (((k >> 5) & 15) << 4) | (k >> 9); }
@@ -106,28 +109,37 @@ __global__ void __launch_bounds__(ClusterShape::NT, 1) td_cluster_kernel(const F
   cplx* sm = reinterpret_cast<cplx*>(smem_raw);
   const SmemArr U{sm}, Z{sm + Sh::PADNF};
   cplx* tw = sm + Sh::PADNF + Sh::PADM;
-  double* red = reinterpret_cast<double*>(tw + Sh::TWS);   // [2 NW] block reduction
-  double* xsum = red + 2 * NW;                             // [2] rank 1's partial sums, written remotely (rank 0 only)
+  double* red = reinterpret_cast<double*>(tw + Sh::TWS);   // [2][2 NW] per-warp partial sums, double-buffered by item parity
+  double* xsum = red + 4 * NW;                             // [2] rank 1's partial sums, written remotely (rank 0 only)
   const uint32_t mbar_rows = smem_u32(xsum + 2);
-  const uint32_t mbar_g = mbar_rows + 8;
-  int* mid_count = reinterpret_cast<int*>(xsum + 4);
-  SegDev* segS = reinterpret_cast<SegDev*>(xsum + 6);
+  const uint32_t mbar_x = mbar_rows + 8;                   // the partner's half-results have landed (tx bytes)
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(xsum + 4);
+  // thread 0's bookkeeping of the deferred reduction lives in shared memory (registers are what this kernel is short of)
+  struct Book { double pend0, pend1; long long pend_b, prev_b; int pend_add, prev_add; };
+  Book* bk = reinterpret_cast<Book*>(xsum + 6);
+  SegDev* segS = reinterpret_cast<SegDev*>(xsum + 14);
   const SegDev* segs = P.n_seg <= F4_SEGCACHE ? segS : P.segs;
-  const uint32_t mbar_x = smem_u32(xsum + 5);              // half-results of the partner have landed in xbuf (tx bytes)
   double* stH = reinterpret_cast<double*>(sm);             // staged row (<= M doubles) in the U region
-  cplx* xbuf = Z.p;                                        // exchange buffer [16][256] in the Z region
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int br = (int)cluster_ctarank();                   // branch: 0 even bins, 1 odd bins
-  const F4Own own = f4_own<Sh::RF1, true>(br, (int)(threadIdx.x >> 5));
-  const uint32_t xbuf_remote = map_to_cta(smem_u32(xbuf), (uint32_t)(br ^ 1));
+  const F4Own own = f4_own<Sh::RF1, true>(br, warp);
+  const F4Own pown = f4_own<Sh::RF1, true>(br ^ 1, warp);  // the partner warp's blocks (same warp index, other CTA)
+  const uint32_t z_remote = map_to_cta(smem_u32(Z.p), (uint32_t)(br ^ 1));
   const uint32_t xsum_remote = map_to_cta(smem_u32(xsum), 0u);
   const uint32_t mbar_x_remote = map_to_cta(mbar_x, (uint32_t)(br ^ 1));
-  const long long ncl = gridDim.x >> 1;
+  const long long ncl = gridDim.x >> 1, cl = blockIdx.x >> 1;
+  // half-result t (0..15) of this lane: element (t & 7) * 32 + lane of the warp's block [t >> 3]
+  auto hslot = [&](int blk, int t) { const int i = blk * 256 + (t & 7) * 32 + lane; return i + (i >> 4); };
 
   for (int k = tid; k < Sh::TWS; k += NT) tw[k] = P.T[k];
   if (tid < P.n_seg && tid < F4_SEGCACHE) segS[tid] = P.segs[tid];
-  if (tid == 0) { mbar_init(mbar_rows, 1); mbar_init(mbar_g, 1); mbar_init(mbar_x, 1); *mid_count = 0; }
+  if (tid == 0) { mbar_init(mbar_rows, 1); mbar_init(mbar_x, 1); bk->pend_b = -1; bk->prev_b = -1; }
+  if (warp == 0) tmem_alloc<512>(smem_u32(tmem_slot));
+  tmem_fence_before();
   __syncthreads();
+  tmem_fence_after();
+  const uint32_t tcol = *tmem_slot + ((uint32_t)(32 * (warp & 3)) << 16) + (uint32_t)((warp >> 2) * 256);
+  f4_store_twiddles<TW>(lane, tw, tcol + F4_TC_TW);
 
   // rows of item (b, s): hrow is the row that gets staged (the template; d itself for STOREZ)
   auto rows = [&](long long b, int s, const double*& drow, const double*& hrow, int& n) -> bool {
@@ -146,220 +158,233 @@ __global__ void __launch_bounds__(ClusterShape::NT, 1) td_cluster_kernel(const F
       bulk_g2s(smem_u32(stH), hrow, bytes, mbar_rows);
     }
   };
-  auto prefetch_g = [&](int s) {  // ONE thread
-    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-    constexpr uint32_t bytes = (uint32_t)(Sh::PADM * sizeof(cplx));
-    mbar_expect_tx(mbar_g, bytes);
-    bulk_g2s(smem_u32(Z.p), P4.Gp[s] + (size_t)br * Sh::PADM, bytes, mbar_g);
-  };
 
-  long long b = blockIdx.x >> 1;
-  int s = 0;
-  bool have = b < P.B;
-  uint32_t par_rows = 0, par_g = 0, par_x = 0;
+  const long long Bs = (MODE == MODE_STOREZ) ? 1 : P.B;
+  const bool active = cl < Bs;   // (always: the grid is min(B, clusters); an idle cluster still takes part in the barriers below)
+  uint32_t par_rows = 0, par_x = 0;
   bool staged = false;
-  if (have) {
+  if (active) {
     const double *dr, *hr; int nn;
-    staged = rows(b, s, dr, hr, nn);
-    if (tid == 0) { prefetch_rows(b, s); prefetch_g(s); }
+    staged = rows(cl, 0, dr, hr, nn);
+    if (tid == 0) prefetch_rows(cl, 0);
   }
-  // rank 0, thread 0: running totals of the current template and the item whose partner sum is in flight
-  double tot0 = 0.0, tot1 = 0.0, pend0 = 0.0, pend1 = 0.0;
-  long long pend_b = 0;
-  bool pend = false, pend_last = false;
-  auto settle = [&]() {  // rank 0 / thread 0, after a cluster barrier that follows rank 1's remote store
-    if (MODE != MODE_STOREZ && pend) {
-      tot0 += pend0 + xsum[0];
-      tot1 += pend1 + xsum[1];
-      if (pend_last) {
-        if (MODE == MODE_LOGLIKE) {
-          const double v = -0.5 * tot1;
-          P.out0[pend_b] = P.accumulate ? P.out0[pend_b] + v : v;
-        } else {
-          if (P.out0) P.out0[pend_b] = P.accumulate ? P.out0[pend_b] + tot0 : tot0;
-          if (P.out1) P.out1[pend_b] = P.accumulate ? P.out1[pend_b] + tot1 : tot1;
+  // bookkeeping of the deferred reduction: `prev_*` = the item whose half-results sit in Z; rank 0 / thread 0 also keeps
+  // the item whose CTA sums are complete but whose partner sums are still on their way (`pend_*`)
+  int item = 0, prev_n = 0;
+  cplx* prev_zd = nullptr;
+  // S5 of the previous item: this half of z = e + w o from the warp's own Z blocks, squares summed per warp
+  auto s5_deferred = [&]() {
+    mbar_wait(mbar_x, par_x);
+    par_x ^= 1;
+    double p0[2] = {0.0, 0.0}, p1[2] = {0.0, 0.0};
+    static_for<0, 16>([&](auto t) {
+      constexpr int tt = decltype(t)::value;
+      const cplx a = Z.p[hslot(tt < 8 ? own.z0 : own.z1, tt)], bq = Z.p[hslot(tt < 8 ? own.z2 : own.z3, tt)];
+      const cplx z = cadd(a, bq);
+      const int i = tid + 256 * tt + br * (M / 2);
+      if constexpr (MODE == MODE_STOREZ) {
+        prev_zd[i] = z;
+      } else {
+        if (i < prev_n) {
+          if constexpr (MODE == MODE_INNER) {
+            const cplx q = prev_zd[i];
+            p0[tt & 1] = fma(z.x, q.x, fma(-z.y, q.y, p0[tt & 1]));
+          }
+          p1[tt & 1] = fma(z.x, z.x, fma(-z.y, z.y, p1[tt & 1]));
         }
-        tot0 = 0.0; tot1 = 0.0;
       }
-      pend = false;
+    });
+    if (MODE != MODE_STOREZ) {
+      double acc0 = 0.0, acc1 = warp_sum(p1[0] + p1[1]);
+      if (MODE == MODE_INNER) acc0 = warp_sum(p0[0] + p0[1]);
+      if (lane == 0) { double* r = red + 2 * NW * ((item & 1) ^ 1); r[2 * warp] = acc0; r[2 * warp + 1] = acc1; }
+    }
+  };
+  // thread 0, after a CTA barrier that follows s5_deferred: this CTA's sums of the previous item, fixed order over the warps
+  auto cta_sums = [&]() {
+    if (MODE == MODE_STOREZ || bk->prev_b < 0) return;
+    const double* r = red + 2 * NW * ((item & 1) ^ 1);
+    double p0 = 0.0, p1 = 0.0;
+#pragma unroll
+    for (int wq = 0; wq < NW; ++wq) { p0 += r[2 * wq]; p1 += r[2 * wq + 1]; }
+    if (br) {
+      asm volatile("st.shared::cluster.v2.f64 [%0], {%1, %2};" ::"r"(xsum_remote), "d"(p0), "d"(p1) : "memory");
+    } else {
+      bk->pend0 = p0; bk->pend1 = p1; bk->pend_b = bk->prev_b; bk->pend_add = bk->prev_add;
+    }
+    bk->prev_b = -1;
+  };
+  auto settle = [&]() {  // rank 0 / thread 0, after a cluster barrier that follows rank 1's remote store
+    if (MODE != MODE_STOREZ && bk->pend_b >= 0) {
+      const double t0 = bk->pend0 + xsum[0], t1 = bk->pend1 + xsum[1];
+      const long long pend_b = bk->pend_b;
+      const int pend_add = bk->pend_add;
+      if (MODE == MODE_LOGLIKE) {
+        const double v = -0.5 * t1;
+        P.out0[pend_b] = pend_add ? P.out0[pend_b] + v : v;
+      } else {
+        if (P.out0) P.out0[pend_b] = pend_add ? P.out0[pend_b] + t0 : t0;
+        if (P.out1) P.out1[pend_b] = pend_add ? P.out1[pend_b] + t1 : t1;
+      }
+      bk->pend_b = -1;
     }
   };
 
-  while (have) {
-    long long nb = b; int ns = s + 1;
-    if (ns == P.n_seg) { ns = 0; nb = b + ncl; }
-    const bool have_next = (MODE != MODE_STOREZ || nb == b) && nb < P.B;
+  for (int s = 0; active && s < P.n_seg; ++s) {
     const SegDev sg = segs[s];
-    // ---------------- forward pass 1 (radix 16, stride 256) of THIS CTA's branch; task j = tid
-    {
-      const int j = tid;
-      const double *drow, *hrow; int n;
-      rows(b, s, drow, hrow, n);
-      cplx x[16];
-      if (staged) {
-        double2 dv[16];
-        if (MODE == MODE_LOGLIKE) {
-          const bool dvec = (reinterpret_cast<uintptr_t>(drow) & 15) == 0;
+    // ---------------- per-segment constants into this thread's TMEM columns
+    f4_store_generator(P4.Gp[s] + (size_t)br * Sh::PADM, own, lane, tcol + F4_TC_G);
+    if (MODE == MODE_LOGLIKE) {
+      const double* drow = P.d + sg.off;
+#pragma unroll
+      for (int q = 0; q < 16; ++q) {
+        const int i0 = 2 * (tid + 256 * q);
+        tmem_st_c(tcol + F4_TC_D + 4 * q, mk(i0 < sg.n ? __ldg(drow + i0) : 0.0, i0 + 1 < sg.n ? __ldg(drow + i0 + 1) : 0.0));
+      }
+    }
+    tmem_wait_st();
+    for (long long b = cl; b < Bs; b += ncl) {
+      long long nb = b + ncl; int ns = s;
+      if (nb >= Bs) { nb = cl; ns = s + 1; }
+      const bool have_next = ns < P.n_seg;
+      // ---------------- forward pass 1 (radix 16, stride 256) of THIS CTA's branch; task j = tid
+      {
+        const int j = tid;
+        cplx x[16];
+        if (staged) {
+          int dr[4][16];
+          if (MODE == MODE_LOGLIKE) {
+#pragma unroll
+            for (int g = 0; g < 4; ++g) tmem_ld16(tcol + F4_TC_D + 16 * g, dr[g]);
+          }
+          mbar_wait(mbar_rows, par_rows);
+          par_rows ^= 1;
 #pragma unroll
           for (int q = 0; q < 16; ++q) {
             const int i0 = 2 * (j + 256 * q);
-            dv[q] = mk(0.0, 0.0);
-            if (i0 < n) {  // n even on this path
-              if (dvec) dv[q] = __ldg(reinterpret_cast<const double2*>(drow + i0));
-              else dv[q] = mk(__ldg(drow + i0), __ldg(drow + i0 + 1));
-            }
+            double2 h = mk(0.0, 0.0);
+            if (i0 < sg.n) h = *reinterpret_cast<const double2*>(stH + i0);  // n even on this path
+            x[q] = h;
           }
+          if (MODE == MODE_LOGLIKE) {
+            tmem_wait_ld();
+#pragma unroll
+            for (int g = 0; g < 4; ++g) tmem_use16(dr[g]);
+#pragma unroll
+            for (int q = 0; q < 16; ++q) { const cplx dv = tmem_c(dr[q >> 2], q & 3); x[q] = mk(dv.x - x[q].x, dv.y - x[q].y); }
+          }
+          __syncthreads();  // staging consumed: the U region may now be overwritten
+        } else {
+          const double *drow, *hrow; int n;
+          rows(b, s, drow, hrow, n);
+          const bool vec = ((reinterpret_cast<uintptr_t>(drow) | reinterpret_cast<uintptr_t>(hrow)) & 15) == 0;
+#pragma unroll
+          for (int q = 0; q < 16; ++q) x[q] = load_pair<MODE>(drow, hrow, j + 256 * q, n, vec);
         }
-        mbar_wait(mbar_rows, par_rows);
-        par_rows ^= 1;
-#pragma unroll
-        for (int q = 0; q < 16; ++q) {
-          const int i0 = 2 * (j + 256 * q);
-          double2 h = mk(0.0, 0.0);
-          if (i0 < n) h = *reinterpret_cast<const double2*>(stH + i0);
-          x[q] = (MODE == MODE_LOGLIKE) ? mk(dv[q].x - h.x, dv[q].y - h.y) : h;
-        }
-        __syncthreads();  // staging consumed: the U region may now be overwritten
-      } else {
-        const bool vec = ((reinterpret_cast<uintptr_t>(drow) | reinterpret_cast<uintptr_t>(hrow)) & 15) == 0;
-#pragma unroll
-        for (int q = 0; q < 16; ++q) x[q] = load_pair<MODE>(drow, hrow, j + 256 * q, n, vec);
-      }
-      cplx w[16];
-      tw_powers<16>(tw[4 * j], w);  // w_NF^j
-      if (br) {
-        const cplx beta = tw[2 * j];  // w_M^j
-        static_for<0, 16>([&](auto q) { x[decltype(q)::value] = mul_w32<decltype(q)::value, false>(x[decltype(q)::value]); });
-        static_for<0, 16>([&](auto t) { w[decltype(t)::value] = cmul(w[decltype(t)::value], beta); });
-      }
-      fft_reg<16, false>(x);
-      static_for<0, 16>([&](auto t) {
-        constexpr int tt = decltype(t)::value;
-        cplx v = x[brevR<16>(tt)];
-        if (tt > 0 || br) v = cmul(v, w[tt]);
-        U.st(j + 256 * tt, v);
-      });
-    }
-    __syncthreads();
-    // ---------------- forward passes 2 and 3, warp-local
-    f4_forward23<TW>(U, own, lane, tw);
-    __syncwarp();  // mirror-closed ownership (f4_own): mid reads only this warp's U blocks
-    // ---------------- mid: untangle x generator (in place in Z) -> first inverse pass
-    mbar_wait(mbar_g, par_g);
-    par_g ^= 1;
-    f4_mid<NF, Sh::RF1>(U, Z, br, own, lane, tw);
-    __syncwarp();
-    if (lane == 0) {
-      const int old = atomicAdd(mid_count, 1);
-      if (old == NW - 1) {
-        *mid_count = 0;
-        if (have_next) prefetch_rows(nb, ns);
-      }
-    }
-    bool staged_next = false;
-    if (have_next) { const double *dr, *hr; int nn; staged_next = rows(nb, ns, dr, hr, nn); }
-    // ---------------- inverse pass 2 (L = 256), warp-local
-    f4_inverse2<TW>(Z, own, lane, tw);
-    __syncthreads();
-    // ---------------- last inverse pass: radix 32 on this branch, exchange halves, fused S5
-    double acc0 = 0.0, acc1 = 0.0;
-    {
-      const int j = tid;
-      cplx x[32];
-#pragma unroll
-      for (int q = 0; q < 32; ++q) x[q] = Z.ld(j + 256 * q);
-      // arm the exchange mbarrier for this item's 16 x 256 complex from the partner, then
-      if (tid == 0) mbar_expect_tx(mbar_x, (uint32_t)(16 * NT * sizeof(cplx)));
-      cluster_arrive();  // (A) my Z region is free: the partner may write its half-results into it
-      {
-        // x_q *= conj(w_M^{j q}) (and conj(w_2M^j) on the odd branch); powers as w^{4 hi} * w^{lo}
-        cplx lo[4], hi[8];
-        tw_powers<4>(tw[2 * j], lo);
-        hi[0] = mk(1.0, 0.0);
-        hi[1] = csq(lo[2]);
-        static_for<2, 8>([&](auto q) {
-          constexpr int qq = decltype(q)::value;
-          if constexpr ((qq & 1) == 0) hi[qq] = csq(hi[qq / 2]);
-          else hi[qq] = cmul(hi[qq - 1], hi[1]);
-        });
+        cplx w[16];
+        tw_powers<16>(tw[4 * j], w);  // w_NF^j
         if (br) {
-          const cplx beta = tw[j];
-          static_for<0, 4>([&](auto r) { lo[decltype(r)::value] = cmul(lo[decltype(r)::value], beta); });
+          const cplx beta = tw[2 * j];  // w_M^j
+          static_for<0, 16>([&](auto q) { x[decltype(q)::value] = mul_w32<decltype(q)::value, false>(x[decltype(q)::value]); });
+          static_for<0, 16>([&](auto t) { w[decltype(t)::value] = cmul(w[decltype(t)::value], beta); });
         }
-        static_for<0, 32>([&](auto q) {
-          constexpr int qq = decltype(q)::value;
-          if constexpr (qq < 4) {
-            if (qq > 0 || br) x[qq] = cmulc(x[qq], lo[qq]);
-          } else {
-            x[qq] = cmulc(x[qq], cmul(hi[qq >> 2], lo[qq & 3]));
-          }
-        });
-      }
-      fft_reg<32, true>(x);
-      if (br) static_for<1, 32>([&](auto t) {
-        constexpr int tt = decltype(t)::value;
-        x[brevR<32>(tt)] = mul_w64_inv<tt>(x[brevR<32>(tt)]);
-      });
-      cluster_wait();    // (A) done on both sides
-      if (br == 0 && tid == 0) settle();  // rank 1's sums of the previous item arrived before its (A)
-      // output t -> index i = j + 256 t; t < 16 belongs to rank 0's half, t >= 16 to rank 1's
-      if (br == 0) {
-        static_for<16, 32>([&](auto t) {
-          constexpr int tt = decltype(t)::value;
-          st_async_cluster(xbuf_remote + (uint32_t)(((tt - 16) * 256 + j) * sizeof(cplx)), x[brevR<32>(tt)], mbar_x_remote);
-        });
-      } else {
+        fft_reg<16, false>(x);
         static_for<0, 16>([&](auto t) {
           constexpr int tt = decltype(t)::value;
-          st_async_cluster(xbuf_remote + (uint32_t)((tt * 256 + j) * sizeof(cplx)), x[brevR<32>(tt)], mbar_x_remote);
+          cplx v = x[brevR<16>(tt)];
+          if (tt > 0 || br) v = cmul(v, w[tt]);
+          U.st(j + 256 * tt, v);
         });
       }
-      mbar_wait(mbar_x, par_x);  // (B) the partner's half-results have landed (local mbarrier: no cluster barrier)
-      par_x ^= 1;
-      static_for<0, 16>([&](auto t) {
-        constexpr int tt = decltype(t)::value;
-        const cplx mine = br ? x[brevR<32>(tt + 16)] : x[brevR<32>(tt)];
-        const cplx z = cadd(mine, xbuf[tt * 256 + j]);
-        const int i = j + 256 * tt + br * (M / 2);
-        if constexpr (MODE == MODE_STOREZ) {
-          sg.zd[i] = z;
-        } else {
-          if (i < sg.n) {
-            if constexpr (MODE == MODE_INNER) {
-              const cplx q = sg.zd[i];
-              acc0 = fma(z.x, q.x, fma(-z.y, q.y, acc0));
-            }
-            acc1 = fma(z.x, z.x, fma(-z.y, z.y, acc1));
-          }
-        }
-      });
-    }
-    if (MODE != MODE_STOREZ) {
-      acc0 = warp_sum(acc0);
-      acc1 = warp_sum(acc1);
-      if (lane == 0) { red[2 * warp] = acc0; red[2 * warp + 1] = acc1; }
-    }
-    __syncthreads();  // exchange buffer (Z region) fully consumed
-    if (tid == 0) {
-      if (have_next) prefetch_g(ns);
-      if (MODE != MODE_STOREZ) {
-        double p0 = 0.0, p1 = 0.0;
-#pragma unroll
-        for (int wq = 0; wq < NW; ++wq) { p0 += red[2 * wq]; p1 += red[2 * wq + 1]; }
-        if (br) {
-          asm volatile("st.shared::cluster.v2.f64 [%0], {%1, %2};" ::"r"(xsum_remote), "d"(p0), "d"(p1) : "memory");
-        } else {
-          pend = true; pend0 = p0; pend1 = p1; pend_b = b; pend_last = (s == P.n_seg - 1);
-        }
+      __syncthreads();
+      // ---------------- forward passes 2 and 3, warp-local
+      f4_forward23<TW, true>(U, own, lane, tw, tcol + F4_TC_TW);
+      __syncwarp();  // mirror-closed ownership (f4_own): mid reads only this warp's U blocks
+      // ---------------- S5 of the PREVIOUS item, from the Z blocks this warp is about to overwrite
+      if (item > 0) s5_deferred();
+      __syncwarp();
+      // ---------------- mid: untangle x generator (TMEM) -> first inverse pass -> Z
+      f4_mid<NF, Sh::RF1, true>(U, Z, br, own, lane, tw, tcol + F4_TC_G);
+      __syncwarp();
+      bool staged_next = false;
+      if (have_next) { const double *dr, *hr; int nn; staged_next = rows(nb, ns, dr, hr, nn); }
+      // ---------------- inverse pass 2 (L = 256), warp-local
+      f4_inverse2<TW>(Z, own, lane, tw);
+      __syncthreads();
+      if (tid == 0) {
+        if (have_next) prefetch_rows(nb, ns);  // every warp is past mid: the U region is dead
+        cta_sums();                            // every warp is past the previous item's S5
       }
+      // ---------------- last inverse pass: radix 32 on this branch; halves to their owners
+      {
+        const int j = tid;
+        cplx x[32];
+#pragma unroll
+        for (int q = 0; q < 32; ++q) x[q] = Z.ld(j + 256 * q);
+        // arm the exchange mbarrier for this item's 16 x 256 complex from the partner, then
+        if (tid == 0) mbar_expect_tx(mbar_x, (uint32_t)(16 * NT * sizeof(cplx)));
+        cluster_arrive();  // (A) every thread of this CTA has read its Z values: the region may be overwritten
+        {
+          // x_q *= conj(w_M^{j q}) (and conj(w_2M^j) on the odd branch); powers as w^{4 hi} * w^{lo}
+          cplx lo[4], hi[8];
+          tw_powers<4>(tw[2 * j], lo);
+          hi[0] = mk(1.0, 0.0);
+          hi[1] = csq(lo[2]);
+          static_for<2, 8>([&](auto q) {
+            constexpr int qq = decltype(q)::value;
+            if constexpr ((qq & 1) == 0) hi[qq] = csq(hi[qq / 2]);
+            else hi[qq] = cmul(hi[qq - 1], hi[1]);
+          });
+          if (br) {
+            const cplx beta = tw[j];
+            static_for<0, 4>([&](auto r) { lo[decltype(r)::value] = cmul(lo[decltype(r)::value], beta); });
+          }
+          static_for<0, 32>([&](auto q) {
+            constexpr int qq = decltype(q)::value;
+            if constexpr (qq < 4) {
+              if (qq > 0 || br) x[qq] = cmulc(x[qq], lo[qq]);
+            } else {
+              x[qq] = cmulc(x[qq], cmul(hi[qq >> 2], lo[qq & 3]));
+            }
+          });
+        }
+        fft_reg<32, true>(x);
+        if (br) static_for<1, 32>([&](auto t) {
+          constexpr int tt = decltype(t)::value;
+          x[brevR<32>(tt)] = mul_w64_inv<tt>(x[brevR<32>(tt)]);
+        });
+        cluster_wait();    // (A) on both sides
+        if (br == 0 && tid == 0) settle();  // rank 1 stored the sums of the item before the previous one ahead of its (A)
+        // output t -> index i = j + 256 t; t < 16 belongs to rank 0's half, t >= 16 to rank 1's.  Own half: this warp's
+        // blocks z0, z1; the other half: the partner warp's blocks z2, z3 (asynchronous, counted on its mbarrier).
+        static_for<0, 16>([&](auto t) {
+          constexpr int tt = decltype(t)::value;
+          const cplx mine = br ? x[brevR<32>(tt + 16)] : x[brevR<32>(tt)];
+          const cplx theirs = br ? x[brevR<32>(tt)] : x[brevR<32>(tt + 16)];
+          Z.p[hslot(tt < 8 ? own.z0 : own.z1, tt)] = mine;
+          st_async_cluster(z_remote + (uint32_t)(hslot(tt < 8 ? pown.z2 : pown.z3, tt) * sizeof(cplx)), theirs, mbar_x_remote);
+        });
+      }
+      prev_n = sg.n; prev_zd = sg.zd;
+      if (tid == 0) { bk->prev_b = b; bk->prev_add = (P.accumulate || s > 0) ? 1 : 0; }
+      ++item;
+      staged = staged_next;
     }
-    b = nb; s = ns; have = have_next; staged = staged_next;
+  }
+  // ---------------- the last item's S5, then the sums travel: CTA -> rank 0 -> out
+  if (item > 0) s5_deferred();
+  __syncthreads();
+  if (tid == 0) {
+    // rank 0 may still hold an item whose partner sums arrived with the last (A): there is none - settle() ran after it
+    cta_sums();
   }
   // rank 1's last partial sums become visible with this barrier; no CTA exits while its partner may
   // still store into its shared memory
   cluster_arrive();
   cluster_wait();
   if (br == 0 && tid == 0) settle();
+  __syncthreads();
+  if (warp == 0) tmem_dealloc<512>(*tmem_slot);
 }
 
 }  // namespace td

@@ -282,4 +282,51 @@ __device__ __forceinline__ void mbar_wait(uint32_t mbar, uint32_t parity) {
   } while (!ok);
 }
 
+// ---- tensor memory (TMEM) as a per-thread constant cache ---------------------------------------------------
+// sm_100a gives every SM 256 KB of tensor memory (512 columns x 128 lanes x 32 bit) next to the 227 KB of shared memory.
+// The fp64 FFT path has no use for tcgen05.mma (no f64 kind), but tcgen05.st / tcgen05.ld move registers to and from TMEM
+// on a datapath of their own (measured on B200: 228 B/cycle/SM with eight warps, _work probe; shared memory: 128 B/cycle).
+// With the .32x32b shape a thread reaches exactly one TMEM lane (32 (warp % 4) + lane) and any column, so TMEM is private
+// per-thread storage: 2 KB per lane, shared by the warps w and w + 4 of a CTA.  The fused kernels keep there what a
+// thread needs again for every template and never changes: its 32 values of the generator spectrum, its samples of the
+// data vector and its twiddle powers.  None of this touches shared memory or L2 after the first item.
+// NCOLS = 256 or 512 columns (a power of two >= 32); executed by ONE whole warp, which also frees them.  A CTA that asks for
+// more columns than are free on its SM waits inside the instruction until a co-resident CTA frees its own.
+template <int NCOLS> __device__ __forceinline__ void tmem_alloc(uint32_t smem_slot) {
+  asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_slot), "n"(NCOLS) : "memory");
+  asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+}
+template <int NCOLS> __device__ __forceinline__ void tmem_dealloc(uint32_t taddr) {
+  asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(taddr), "n"(NCOLS) : "memory");
+}
+__device__ __forceinline__ void tmem_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tmem_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+// one complex double = 4 columns
+__device__ __forceinline__ void tmem_st_c(uint32_t taddr, cplx v) {
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1, %2, %3, %4};" ::"r"(taddr), "r"(__double2loint(v.x)),
+               "r"(__double2hiint(v.x)), "r"(__double2loint(v.y)), "r"(__double2hiint(v.y))
+               : "memory");
+}
+// 4 complex doubles = 16 columns.  tcgen05.ld is asynchronous: issue all loads, tmem_wait_ld(), then tmem_use16() on each
+// register group (an empty asm that "rewrites" the registers, so that no use can be scheduled above the wait), then read.
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, int (&r)[16]) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+      : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
+        "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+      : "r"(taddr)
+      : "memory");
+}
+__device__ __forceinline__ void tmem_use16(int (&r)[16]) {
+  asm volatile("" : "+r"(r[0]), "+r"(r[1]), "+r"(r[2]), "+r"(r[3]), "+r"(r[4]), "+r"(r[5]), "+r"(r[6]), "+r"(r[7]), "+r"(r[8]),
+               "+r"(r[9]), "+r"(r[10]), "+r"(r[11]), "+r"(r[12]), "+r"(r[13]), "+r"(r[14]), "+r"(r[15])
+               :
+               : "memory");
+}
+__device__ __forceinline__ cplx tmem_c(const int (&r)[16], int q) {  // q-th complex of a group of 4
+  return mk(__hiloint2double(r[4 * q + 1], r[4 * q]), __hiloint2double(r[4 * q + 3], r[4 * q + 2]));
+}
+
 }  // namespace td

@@ -340,6 +340,8 @@ __device__ __forceinline__ void last_pass_c(const SmemArr& ZE, const SmemArr& ZO
       gm[tt] = mk(cos32(tt * (16 / R)), sin32(tt * (16 / R)));  // conj(w_32)^(tt 16/R), compile-time constants
     });
   }
+  // four independent partial sums per output (a single chain of 2 R dependent FMAs would be latency-bound)
+  double p0[4] = {0.0, 0.0, 0.0, 0.0}, p1[4] = {0.0, 0.0, 0.0, 0.0};
   static_for<0, R>([&](auto t) {
     constexpr int tt = decltype(t)::value;
     const cplx ev = e[brevR<R>(tt)], ov = o[brevR<R>(tt)];
@@ -351,12 +353,16 @@ __device__ __forceinline__ void last_pass_c(const SmemArr& ZE, const SmemArr& ZO
       if (i < n) {
         if constexpr (MODE == MODE_INNER) {
           const cplx q = zd[i];
-          acc0 = fma(z.x, q.x, fma(-z.y, q.y, acc0));
+          p0[tt & 1] = fma(z.x, q.x, p0[tt & 1]);
+          p0[2 + (tt & 1)] = fma(-z.y, q.y, p0[2 + (tt & 1)]);
         }
-        acc1 = fma(z.x, z.x, fma(-z.y, z.y, acc1));
+        p1[tt & 1] = fma(z.x, z.x, p1[tt & 1]);
+        p1[2 + (tt & 1)] = fma(-z.y, z.y, p1[2 + (tt & 1)]);
       }
     }
   });
+  if constexpr (MODE == MODE_INNER) acc0 += (p0[0] + p0[1]) + (p0[2] + p0[3]);
+  if constexpr (MODE != MODE_STOREZ) acc1 += (p1[0] + p1[1]) + (p1[2] + p1[3]);
 }
 
 // both branches of one radix-16 butterfly task interleaved (twice the independent work per thread)

@@ -1,19 +1,23 @@
 // td_fused4.cuh - the fused FFT-path kernel for M = 1024 / 2048 / 4096 (transform lengths
-// 2M = 2048 / 4096 / 8192), restructured around the two things the first fused kernel lost
-// time on (profiles/r01_fused_v3_regions.md): CTA-wide barriers that put every warp in the
-// same load -> compute -> store phase, and the stand-alone untangle pass.
+// 2M = 2048 / 4096 / 8192), built around two measurements (profiles/r02_c2_phase_clocks.md): CTA-wide barriers put every
+// warp in the same load -> compute -> store phase, and whatever a thread needs again for every template costs
+// shared-memory bandwidth each time unless it lives somewhere else.
 //
 //  * plans  NF = M/2 = [RF1,16,16],  M = [RI1,16,16],  RI1 = 2 RF1;  NT = 32 RF1 = M/16 threads;
 //    warps [0, NW/2) own the even-bin branch, warps [NW/2, NW) the odd-bin branch.
 //  * forward passes 2 and 3 touch only the 2 x 256 elements a warp owns: one __syncwarp between them.
 //  * "mid": forward bins are untangled IN REGISTERS from the two mirror blocks, multiplied by the
 //    generator spectrum and pushed through the first inverse radix-16 pass before they are stored.
-//    The generator spectrum of the segment is TMA-prefetched into the Z region (dead during the
-//    forward half) in the padded Z layout, so mid reads G[p] and writes Z[p] in place.
 //  * inverse pass 2 is again warp-local; only the last pass (which joins the two branches and
 //    carries the fused quadratic reduction) needs the whole CTA.
-//  * the next item's rows are TMA-prefetched into the U region by whichever warp finishes mid last.
-// CTA barriers per (template, segment): 5 (was 9).
+//  * TENSOR MEMORY AS A CONSTANT CACHE: a thread multiplies the same 32 generator values, subtracts the same 16 data
+//    samples and uses the same 15 twiddle powers for every template.  They are written once per (CTA, segment) into the
+//    thread's private columns of the SM's 256 KB tensor memory (tcgen05.st) and read back with tcgen05.ld, a datapath
+//    that shares nothing with shared memory or the fp64 pipe.  This replaces, per template, a 128 KB + 32 KB bulk copy
+//    from L2, 160 KB of shared-memory reads and 80 fp64 instructions per thread.  Segments are the OUTER loop
+//    (out[b] accumulates over them) so that the constants change n_seg times per kernel, not per item.
+//  * the next item's template row is TMA-prefetched into the U region by whichever warp finishes mid last.
+// CTA barriers per (template, segment): 4 (staging consumed, after pass 1, before the last pass; end of item is a counter).
 #pragma once
 #include "td_fused.cuh"
 #include "td_dit16.cuh"
@@ -22,6 +26,12 @@ namespace td {
 
 constexpr int F4_SEGCACHE = 8;  // segment records cached in shared memory (more segments: read from global per item)
 
+// TMEM columns of a thread, relative to its warp's column base (a complex double = 4 columns; warps w and w + 4 share
+// a lane quarter and take columns [0, 256) and [256, 512))
+constexpr int F4_TC_G = 0;     // 128 columns: the 2 x 16 generator values of mid
+constexpr int F4_TC_D = 128;   // up to 64 columns: the thread's samples of the data vector (first forward pass)
+constexpr int F4_TC_TW = 192;  // 64 columns: twiddle powers of forward pass 2
+
 template <int LOG2M> struct Fused4Shape {
   static constexpr int M = 1 << LOG2M, NF = M / 2;
   static constexpr int RF1 = plan_r1(NF), RI1 = plan_r1(M);
@@ -29,14 +39,22 @@ template <int LOG2M> struct Fused4Shape {
   static constexpr int NT = 32 * RF1, NW = RF1, NWB = RF1 / 2;
   static constexpr int TWS = 2 * M / RF1;
   static constexpr int PADM = SmemArr::padded(M), PADNF = SmemArr::padded(NF);
+  static constexpr int TMEM_COLS = NW > 4 ? 512 : 256;  // 256 columns per thread; warps w and w + 4 share a lane quarter
   static constexpr size_t smem_bytes() {
-    return sizeof(cplx) * (2 * (size_t)PADNF + 2 * (size_t)PADM + TWS) + sizeof(double) * 2 * NW + 48 + F4_SEGCACHE * sizeof(SegDev);
+    return sizeof(cplx) * (2 * (size_t)PADNF + 2 * (size_t)PADM + TWS) + sizeof(double) * 4 * NW + 48 + F4_SEGCACHE * sizeof(SegDev)
+#ifdef TD_PHASE_CLOCKS
+           + 16 * 16 * sizeof(long long)
+#endif
+        ;
   }
 };
 
 struct Fused4Params {
   FusedParams base;
   const cplx* const* Gp;  // device array [n_seg]: generator spectrum in the PADDED Z layout [2][padded(M)]
+#ifdef TD_DEBUG_KNOBS
+  int skew;               // debug builds: cycles the odd-bin warps wait after the barrier that follows pass 1
+#endif
 };
 
 // ---- pieces shared by the one-CTA kernel below and the 2-CTA cluster kernel (td_cluster.cuh) -------
@@ -59,16 +77,33 @@ template <int RF1, bool MC> __device__ __forceinline__ F4Own f4_own(int br, int 
   }
 }
 
-// forward passes 2 and 3, warp-local (this warp owns U blocks o.u0, o.u1 of its branch)
-template <int TW>
-__device__ __forceinline__ void f4_forward23(const SmemArr& U, const F4Own& o, int lane, const cplx* __restrict__ tw) {
-  cplx x[16], w[16];
+// forward passes 2 and 3, warp-local (this warp owns U blocks o.u0, o.u1 of its branch).
+// TWT: the sixteen twiddle powers of pass 2 come from the thread's TMEM columns at `ttw` (64 columns, written once per
+// kernel by f4_store_twiddles) instead of being rebuilt for every item.
+template <int TW, bool TWT = false>
+__device__ __forceinline__ void f4_forward23(const SmemArr& U, const F4Own& o, int lane, const cplx* __restrict__ tw,
+                                             uint32_t ttw = 0) {
+  cplx x[16];
   {
     const int s1 = (lane >> 4) ? o.u1 : o.u0, j = lane & 15;
     const int base = s1 * 256 + j;
-    tw_powers<16>(tw[j * (TW / 256)], w);
+    cplx w[16];
+    int wr[4][16];
+    if constexpr (TWT) {
+#pragma unroll
+      for (int g = 0; g < 4; ++g) tmem_ld16(ttw + 16 * g, wr[g]);
+    } else {
+      tw_powers<16>(tw[j * (TW / 256)], w);
+    }
 #pragma unroll
     for (int q = 0; q < 16; ++q) x[q] = U.ld(base + 16 * q);
+    if constexpr (TWT) {
+      tmem_wait_ld();
+#pragma unroll
+      for (int g = 0; g < 4; ++g) tmem_use16(wr[g]);
+#pragma unroll
+      for (int q = 0; q < 16; ++q) w[q] = tmem_c(wr[q >> 2], q & 3);
+    }
     fft_reg<16, false>(x);
     static_for<0, 16>([&](auto t) {
       constexpr int tt = decltype(t)::value;
@@ -94,11 +129,37 @@ __device__ __forceinline__ void f4_forward23(const SmemArr& U, const F4Own& o, i
     static_for<0, 16>([&](auto t) { U.st(dst + decltype(t)::value, x[brevR<16>(decltype(t)::value)]); });
   }
 }
+// the powers w_256^(j t), t = 0..15, j = lane & 15, of forward pass 2 into 64 TMEM columns at ttw (once per kernel)
+template <int TW>
+__device__ __forceinline__ void f4_store_twiddles(int lane, const cplx* __restrict__ tw, uint32_t ttw) {
+  cplx w[16];
+  tw_powers<16>(tw[(lane & 15) * (TW / 256)], w);
+#pragma unroll
+  for (int q = 0; q < 16; ++q) tmem_st_c(ttw + 4 * q, w[q]);
+}
 
-// mid: untangle (registers) x generator (in place in Z) -> first inverse pass
-template <int NF, int RF1>
+// this lane's 2 x 16 generator values (g = one branch of the segment's spectrum in the padded Z layout, global memory)
+// into 128 TMEM columns at tg: once per (CTA, segment) instead of a 128 KB bulk copy and 128 KB of shared-memory reads
+// per item.  The element order is the one f4_mid multiplies in.
+__device__ __forceinline__ void f4_store_generator(const cplx* __restrict__ g, const F4Own& o, int lane, uint32_t tg) {
+  const int q4 = lane >> 3;
+  const int s1 = q4 == 0 ? o.z0 : q4 == 1 ? o.z1 : q4 == 2 ? o.z2 : o.z3, s2 = lane & 7;
+#pragma unroll
+  for (int par = 0; par < 2; ++par) {
+    const int zb = (s1 * 16 + s2) * 16 + par * 8 * 16;
+#pragma unroll
+    for (int q = 0; q < 16; ++q) {
+      const int i = zb + q;
+      tmem_st_c(tg + 4 * (16 * par + q), __ldg(g + i + (i >> 4)));
+    }
+  }
+}
+
+// mid: untangle (registers) x generator -> first inverse pass.  GT: the generator values come from TMEM (tg, see
+// f4_store_generator); otherwise they sit in Z (bulk-copied there in the padded layout) and are multiplied in place.
+template <int NF, int RF1, bool GT = false>
 __device__ __forceinline__ void f4_mid(const SmemArr& U, const SmemArr& Z, int br, const F4Own& o, int lane,
-                                       const cplx* __restrict__ tw) {
+                                       const cplx* __restrict__ tw, uint32_t tg = 0) {
   constexpr int RI1 = 2 * RF1;
   const int q4 = lane >> 3;
   const int s1 = q4 == 0 ? o.z0 : q4 == 1 ? o.z1 : q4 == 2 ? o.z2 : o.z3, s2 = lane & 7;
@@ -112,17 +173,37 @@ __device__ __forceinline__ void f4_mid(const SmemArr& U, const SmemArr& Z, int b
   const int fb = slot(kap), fb2 = slot(kap2);
   const cplx basew = tw[2 * kap + br];  // w_2M^(2 kap + br)
   const int zb0 = (s1 * 16 + s2) * 16;
-  static_for<0, 2>([&](auto par) {
-    constexpr int pp = decltype(par)::value;  // 0: even t -> inverse block tau; 1: odd t -> block tau + M/32
-    const int zb = zb0 + pp * 8 * 16;
-    cplx ua[8], ub[8], e[16];
+  // Two halves (even t -> inverse block tau, odd t -> block tau + M/32), software-pipelined: the U loads of half 1 are in
+  // flight while half 0 runs its radix-16 butterfly, and half 0's stores drain while half 1 computes.
+  cplx ua[8], ub[8], e[16];
+  int gr[4][16];
+  auto load_u = [&](auto par) {
+    constexpr int pp = decltype(par)::value;
     static_for<0, 8>([&](auto hh) {
       constexpr int t = 2 * decltype(hh)::value + pp;
       ua[decltype(hh)::value] = U.ld(fb + t);
       ub[decltype(hh)::value] = U.ld(fb2 + (selfzero ? ((16 - t) & 15) : (15 - t)));
     });
+  };
+  auto load_g = [&](auto par) {
+    constexpr int pp = decltype(par)::value;
+    if constexpr (GT) {
 #pragma unroll
-    for (int q = 0; q < 16; ++q) e[q] = Z.ld(zb + q);  // generator spectrum sits in Z
+      for (int g = 0; g < 4; ++g) tmem_ld16(tg + 64 * pp + 16 * g, gr[g]);
+    } else {
+#pragma unroll
+      for (int q = 0; q < 16; ++q) e[q] = Z.ld(zb0 + pp * 8 * 16 + q);  // generator spectrum sits in Z
+    }
+  };
+  auto untangle = [&](auto par) {  // ua, ub, generator -> e
+    constexpr int pp = decltype(par)::value;
+    if constexpr (GT) {
+      tmem_wait_ld();
+#pragma unroll
+      for (int g = 0; g < 4; ++g) tmem_use16(gr[g]);
+#pragma unroll
+      for (int q = 0; q < 16; ++q) e[q] = tmem_c(gr[q >> 2], q & 3);
+    }
     static_for<0, 8>([&](auto hh) {
       constexpr int h8 = decltype(hh)::value, t = 2 * h8 + pp;
       const cplx U1 = ua[h8], U2 = ub[h8];
@@ -132,9 +213,27 @@ __device__ __forceinline__ void f4_mid(const SmemArr& U, const SmemArr& Z, int b
       e[h8] = cmul(e[h8], cadd(A, wB));          // G * 2 X_{kq},      entry s = t/2
       e[8 + h8] = cmul(e[8 + h8], csub(A, wB));  // G * 2 X_{NF + kq}, entry s = 8 + t/2
     });
-    dit16<true, false>(e, mk(1.0, 0.0));
-    static_for<0, 16>([&](auto t) { Z.st(zb + decltype(t)::value, e[brevR<16>(decltype(t)::value)]); });
-  });
+  };
+  auto store_e = [&](auto par) {
+    constexpr int pp = decltype(par)::value;
+    static_for<0, 16>([&](auto t) { Z.st(zb0 + pp * 8 * 16 + decltype(t)::value, e[brevR<16>(decltype(t)::value)]); });
+  };
+  load_g(IC<0>{});
+  load_u(IC<0>{});
+  untangle(IC<0>{});
+  if constexpr (GT) {
+    load_g(IC<1>{});
+    load_u(IC<1>{});   // in flight during the butterfly below
+  }
+  dit16<true, false>(e, mk(1.0, 0.0));
+  store_e(IC<0>{});
+  if constexpr (!GT) {
+    load_g(IC<1>{});   // e is the landing area of the generator values on this path: only now free
+    load_u(IC<1>{});
+  }
+  untangle(IC<1>{});
+  dit16<true, false>(e, mk(1.0, 0.0));
+  store_e(IC<1>{});
 }
 
 // inverse pass 2 (L = 256), warp-local: blocks s1 = 4wb .. 4wb+3
@@ -152,27 +251,33 @@ __device__ __forceinline__ void f4_inverse2(const SmemArr& Z, const F4Own& o, in
   static_for<0, 16>([&](auto t) { Z.st(base1 + 16 * decltype(t)::value, y[brevR<16>(decltype(t)::value)]); });
 }
 
+#ifdef TD_PHASE_CLOCKS
+// debug builds only (_work probes): per-warp cycle counts of every phase of the item loop
+__device__ long long g_phase_clk[148 * 16 * 16];
+#define TDCLK(k) do { if (lane == 0) { const long long t_ = clock64(); clk_s[warp * 16 + (k)] += t_ - tlast; tlast = t_; } } while (0)
+#else
+#define TDCLK(k) do { } while (0)
+#endif
+
 template <int LOG2M, int MODE>
 __global__ void __launch_bounds__(Fused4Shape<LOG2M>::NT, 1) td_fused4_kernel(const Fused4Params P4) {
   using Sh = Fused4Shape<LOG2M>;
   constexpr int M = Sh::M, NF = Sh::NF, TW = 2 * M, NT = Sh::NT, NW = Sh::NW, NWB = Sh::NWB;
   constexpr int RF1 = Sh::RF1, RI1 = Sh::RI1;
+  constexpr int NTASK = NF / RF1, IT = NTASK / NT, S1 = NF / RF1;  // first pass: IT tasks of radix RF1 per thread
+  static_assert(NTASK % NT == 0 && IT * RF1 == 8, "first pass tiling: 8 complex inputs per thread");
   const FusedParams& P = P4.base;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   cplx* sm = reinterpret_cast<cplx*>(smem_raw);
   const SmemArr UE{sm}, UO{sm + Sh::PADNF};
   const SmemArr ZE{sm + 2 * Sh::PADNF}, ZO{sm + 2 * Sh::PADNF + Sh::PADM};
   cplx* tw = sm + 2 * Sh::PADNF + 2 * Sh::PADM;
-  double* red = reinterpret_cast<double*>(tw + Sh::TWS);
-  const uint32_t mbar_rows = smem_u32(red + 2 * NW);
-  const uint32_t mbar_g = mbar_rows + 8;
-  int* mid_count = reinterpret_cast<int*>(red + 2 * NW + 2);
-  int* last_count = mid_count + 1;
-  double* totS = red + 2 * NW + 3;  // running sums of the current template over its segments
-  SegDev* segS = reinterpret_cast<SegDev*>(red + 2 * NW + 6);
+  double* red = reinterpret_cast<double*>(tw + Sh::TWS);  // [2][2 NW]: per-warp partial sums, double-buffered by item parity
+  const uint32_t mbar_rows = smem_u32(red + 4 * NW);
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(red + 4 * NW + 1);
+  SegDev* segS = reinterpret_cast<SegDev*>(red + 4 * NW + 3);
   const SegDev* segs = P.n_seg <= F4_SEGCACHE ? segS : P.segs;
-  double* stH = reinterpret_cast<double*>(sm);
-  double* stD = stH + M;
+  double* stH = reinterpret_cast<double*>(sm);  // the staged template row lives in the U region (dead after mid)
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int br = warp / NWB, wb = warp - br * NWB;  // branch (0 even bins, 1 odd bins), warp within branch
   const SmemArr U = br ? UO : UE, Z = br ? ZO : ZE;
@@ -180,65 +285,126 @@ __global__ void __launch_bounds__(Fused4Shape<LOG2M>::NT, 1) td_fused4_kernel(co
 
   for (int k = tid; k < Sh::TWS; k += NT) tw[k] = P.T[k];
   if (tid < P.n_seg && tid < F4_SEGCACHE) segS[tid] = P.segs[tid];
-  if (tid == 0) { mbar_init(mbar_rows, 1); mbar_init(mbar_g, 1); *mid_count = 0; *last_count = 0; totS[0] = 0.0; totS[1] = 0.0; }
+  if (tid == 0) mbar_init(mbar_rows, 1);
+  if (warp == 0) tmem_alloc<Sh::TMEM_COLS>(smem_u32(tmem_slot));
+#ifdef TD_PHASE_CLOCKS
+  long long* clk_s = reinterpret_cast<long long*>(segS + F4_SEGCACHE);
+  if (tid < 16 * NW) clk_s[tid] = 0;
+  long long tlast = clock64();
+#endif
+  tmem_fence_before();
   __syncthreads();
+  tmem_fence_after();
+  // this thread's TMEM window: lane 32 (warp % 4) + lane, 256 columns
+  const uint32_t tcol = *tmem_slot + ((uint32_t)(32 * (warp & 3)) << 16) + (uint32_t)((warp >> 2) * 256);
+  f4_store_twiddles<TW>(lane, tw, tcol + F4_TC_TW);
 
+  // rows of item (b, s); the template row is staged by TMA when it is 16-byte aligned and N_s is even
   auto rows = [&](long long b, int s, const double*& drow, const double*& hrow, int& n) -> bool {
     const SegDev sg = segs[s];
     drow = P.d + sg.off;
     hrow = (MODE == MODE_STOREZ) ? drow : P.H + b * P.ldh + sg.off;
     n = sg.n;
-    return (((reinterpret_cast<uintptr_t>(drow) | reinterpret_cast<uintptr_t>(hrow)) & 15) == 0) && ((n & 1) == 0);
+    return ((reinterpret_cast<uintptr_t>(hrow) & 15) == 0) && ((n & 1) == 0);
   };
-  // issued by ONE thread
-  auto prefetch_rows = [&](long long b, int s) {
+  auto prefetch_rows = [&](long long b, int s) {  // issued by ONE thread
     const double *drow, *hrow; int n;
     if (rows(b, s, drow, hrow, n)) {
       asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
       const uint32_t bytes = (uint32_t)n * 8u;
-      mbar_expect_tx(mbar_rows, bytes * ((MODE == MODE_LOGLIKE) ? 2 : 1));
-      if (MODE != MODE_STOREZ) bulk_g2s(smem_u32(stH), hrow, bytes, mbar_rows);
-      if (MODE != MODE_INNER) bulk_g2s(smem_u32(stD), drow, bytes, mbar_rows);
+      mbar_expect_tx(mbar_rows, bytes);
+      bulk_g2s(smem_u32(stH), hrow, bytes, mbar_rows);
     }
   };
-  auto prefetch_g = [&](int s) {
-    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-    constexpr uint32_t bytes = (uint32_t)(Sh::PADM * sizeof(cplx));
-    mbar_expect_tx(mbar_g, 2 * bytes);
-    const cplx* g = P4.Gp[s];
-    bulk_g2s(smem_u32(ZE.p), g, bytes, mbar_g);
-    bulk_g2s(smem_u32(ZO.p), g + Sh::PADM, bytes, mbar_g);
-  };
 
-  long long b = blockIdx.x;
-  int s = 0;
-  bool have = b < P.B;
-  uint32_t par_rows = 0, par_g = 0;
-  bool staged = false;
-  if (have) {
-    const double *dr, *hr; int nn;
-    staged = rows(b, s, dr, hr, nn);
-    if (tid == 0) { prefetch_rows(b, s); prefetch_g(s); }
+  const long long Bs = (MODE == MODE_STOREZ) ? 1 : P.B;  // STOREZ transforms the data vector itself, once per segment
+  if ((long long)blockIdx.x >= Bs) {                     // (never: the grid is min(B, SMs); keeps the TMEM protocol whole)
+    __syncthreads();
+    if (warp == 0) tmem_dealloc<Sh::TMEM_COLS>(*tmem_slot);
+    return;
   }
-  while (have) {
-    long long nb = b; int ns = s + 1;
-    if (ns == P.n_seg) { ns = 0; nb = b + gridDim.x; }
-    const bool have_next = (MODE != MODE_STOREZ || nb == b) && nb < P.B;
+  // The partial sums of an item are combined (fixed order over the warps) by thread 0 after the first CTA barrier of the
+  // NEXT item: no atomics, no fences, no barrier at the end of an item.  Segments accumulate into out[b].
+  long long pend_b = -1;
+  int pend_add = 0, item = 0;
+  auto finalize = [&]() {  // thread 0 only
+    if (MODE != MODE_STOREZ && pend_b >= 0) {
+      const double* r = red + 2 * NW * ((item & 1) ^ 1);   // the previous item's buffer
+      double tot0 = 0.0, tot1 = 0.0;
+#pragma unroll
+      for (int wq = 0; wq < NW; ++wq) { tot0 += r[2 * wq]; tot1 += r[2 * wq + 1]; }
+      if (MODE == MODE_LOGLIKE) {
+        const double v = -0.5 * tot1;
+        P.out0[pend_b] = pend_add ? P.out0[pend_b] + v : v;
+      } else {
+        if (P.out0) P.out0[pend_b] = pend_add ? P.out0[pend_b] + tot0 : tot0;
+        if (P.out1) P.out1[pend_b] = pend_add ? P.out1[pend_b] + tot1 : tot1;
+      }
+      pend_b = -1;
+    }
+  };
+  uint32_t par_rows = 0;
+  bool staged;
+  {
+    const double *dr, *hr; int nn;
+    staged = rows(blockIdx.x, 0, dr, hr, nn);
+    if (tid == 0) prefetch_rows(blockIdx.x, 0);
+  }
+  for (int s = 0; s < P.n_seg; ++s) {
     const SegDev sg = segs[s];
-    // ---------------- forward pass 1 (radix RF1, stride 256): both branches from one set of inputs
-    {
-      constexpr int NTASK = NF / RF1;  // 256
-      constexpr int IT = NTASK / NT;
-      static_assert(NTASK % NT == 0, "first pass tiling");
+    // ---------------- per-segment constants into this thread's TMEM columns: generator values, data samples
+    f4_store_generator(P4.Gp[s] + (size_t)br * Sh::PADM, own, lane, tcol + F4_TC_G);
+    if (MODE == MODE_LOGLIKE) {
+      const double* drow = P.d + sg.off;
+#pragma unroll
+      for (int it = 0; it < IT; ++it)
+#pragma unroll
+        for (int ss = 0; ss < RF1; ++ss) {
+          const int i0 = 2 * (tid + it * NT + ss * S1);
+          const cplx dv = mk(i0 < sg.n ? __ldg(drow + i0) : 0.0, i0 + 1 < sg.n ? __ldg(drow + i0 + 1) : 0.0);
+          tmem_st_c(tcol + F4_TC_D + 4 * (it * RF1 + ss), dv);
+        }
+    }
+    tmem_wait_st();
+    for (long long b = blockIdx.x; b < Bs; b += gridDim.x) {
+      long long nb = b + gridDim.x; int ns = s;
+      if (nb >= Bs) { nb = blockIdx.x; ns = s + 1; }
+      const bool have_next = ns < P.n_seg;
+      // ---------------- forward pass 1 (radix RF1, stride 256): both branches from one set of inputs
       if (staged) {
+        int dr[2][16];
+        if (MODE == MODE_LOGLIKE) { tmem_ld16(tcol + F4_TC_D, dr[0]); tmem_ld16(tcol + F4_TC_D + 16, dr[1]); }
+        TDCLK(0);
         mbar_wait(mbar_rows, par_rows);
         par_rows ^= 1;
+        TDCLK(1);
         cplx xs[IT][RF1];
 #pragma unroll
-        for (int it = 0; it < IT; ++it) first_pass_load_staged<RF1, NF, MODE>(xs[it], tid + it * NT, stH, stD, sg.n);
+        for (int it = 0; it < IT; ++it)
+#pragma unroll
+          for (int ss = 0; ss < RF1; ++ss) {
+            const int i0 = 2 * (tid + it * NT + ss * S1);
+            double2 hv = mk(0.0, 0.0);
+            if (i0 < sg.n) hv = *reinterpret_cast<const double2*>(stH + i0);  // n even on this path: i0 + 1 < n too
+            xs[it][ss] = hv;
+          }
+        if (MODE == MODE_LOGLIKE) {
+          tmem_wait_ld();
+          tmem_use16(dr[0]); tmem_use16(dr[1]);
+#pragma unroll
+          for (int it = 0; it < IT; ++it)
+#pragma unroll
+            for (int ss = 0; ss < RF1; ++ss) {
+              const cplx dv = tmem_c(dr[(it * RF1 + ss) >> 2], (it * RF1 + ss) & 3);
+              xs[it][ss] = mk(dv.x - xs[it][ss].x, dv.y - xs[it][ss].y);   // S1: r = d - h
+            }
+        }
+        TDCLK(2);
         __syncthreads();  // staging consumed: the U region may now be overwritten
+        TDCLK(3);
 #pragma unroll
         for (int it = 0; it < IT; ++it) first_pass_compute<RF1, NF>(UE, UO, tid + it * NT, xs[it], tw);
+        TDCLK(4);
       } else {
         const double *drow, *hrow; int n;
         rows(b, s, drow, hrow, n);
@@ -246,70 +412,51 @@ __global__ void __launch_bounds__(Fused4Shape<LOG2M>::NT, 1) td_fused4_kernel(co
 #pragma unroll 1
         for (int g = tid; g < NTASK; g += NT) first_pass_c<RF1, NF, MODE>(UE, UO, g, drow, hrow, n, vec, tw);
       }
-    }
-    __syncthreads();
-    // ---------------- forward passes 2 and 3, warp-local
-    f4_forward23<TW>(U, own, lane, tw);
-    __syncwarp();  // mirror-closed ownership: mid reads only this warp's U blocks
-    // ---------------- mid: untangle (registers) x generator (in place in Z) -> first inverse pass
-    mbar_wait(mbar_g, par_g);
-    par_g ^= 1;
-    f4_mid<NF, RF1>(U, Z, br, own, lane, tw);
-    // the warp finishing mid last knows the U region is dead: it prefetches the next item's rows
-    __syncwarp();
-    if (lane == 0) {
-      const int old = atomicAdd(mid_count, 1);
-      if (old == NW - 1) {
-        *mid_count = 0;
-        if (have_next) prefetch_rows(nb, ns);
-      }
-    }
-    bool staged_next = false;
-    if (have_next) { const double *dr, *hr; int nn; staged_next = rows(nb, ns, dr, hr, nn); }
-    // ---------------- inverse pass 2 (L = 256), warp-local
-    f4_inverse2<TW>(Z, own, lane, tw);
-    __syncthreads();
-    // ---------------- last inverse pass (radix RI1, joins the branches) + pruned radix-2 stage + S5
-    double acc0 = 0.0, acc1 = 0.0;
+      __syncthreads();
+      if (tid == 0) finalize();  // the previous item's sums: every warp has passed its last pass
+#ifdef TD_DEBUG_KNOBS
+      if (br && P4.skew > 0) { const long long t_ = clock64(); while (clock64() - t_ < P4.skew) { } }
+#endif
+      TDCLK(5);
+      // ---------------- forward passes 2 and 3, warp-local
+      f4_forward23<TW, true>(U, own, lane, tw, tcol + F4_TC_TW);
+      __syncwarp();  // mirror-closed ownership: mid reads only this warp's U blocks
+      TDCLK(6);
+      // ---------------- mid: untangle (registers) x generator (TMEM) -> first inverse pass -> Z
+      f4_mid<NF, RF1, true>(U, Z, br, own, lane, tw, tcol + F4_TC_G);
+      TDCLK(8);
+      bool staged_next = false;
+      if (have_next) { const double *dr, *hr; int nn; staged_next = rows(nb, ns, dr, hr, nn); }
+      TDCLK(9);
+      // ---------------- inverse pass 2 (L = 256), warp-local
+      f4_inverse2<TW>(Z, own, lane, tw);
+      TDCLK(10);
+      __syncthreads();
+      // every warp is past mid: the U region is dead and takes the next item's template row
+      if (tid == 0 && have_next) prefetch_rows(nb, ns);
+      TDCLK(11);
+      // ---------------- last inverse pass (radix RI1, joins the branches) + pruned radix-2 stage + S5
+      double acc0 = 0.0, acc1 = 0.0;
 #pragma unroll 1
-    for (int g = tid; g < M / RI1; g += NT) last_pass_c<RI1, M, MODE>(ZE, ZO, g, sg.n, tw, sg.zd, acc0, acc1);
-    if (MODE != MODE_STOREZ) {
-      acc0 = warp_sum(acc0);
-      acc1 = warp_sum(acc1);
-    }
-    // No CTA barrier at the end of an item: the warp that finishes the last pass last (a counter, as for mid) knows
-    // that Z is consumed and every partial sum is in place; it prefetches the next generator spectrum into Z and
-    // finishes the reduction (fixed order over the warps), while the other warps are already loading the next item's
-    // staged rows.  `red` is rewritten only after the next item's barriers, which this warp has to pass as well.
-    __syncwarp();
-    if (lane == 0) {
-      if (MODE != MODE_STOREZ) { red[2 * warp] = acc0; red[2 * warp + 1] = acc1; }
-      __threadfence_block();
-      const int old = atomicAdd(last_count, 1);
-      if (old == NW - 1) {
-        *last_count = 0;
-        __threadfence_block();
-        if (have_next) prefetch_g(ns);
-        if (MODE != MODE_STOREZ) {
-          double tot0 = totS[0], tot1 = totS[1];
-#pragma unroll
-          for (int wq = 0; wq < NW; ++wq) { tot0 += red[2 * wq]; tot1 += red[2 * wq + 1]; }
-          if (s == P.n_seg - 1) {
-            if (MODE == MODE_LOGLIKE) {
-              const double v = -0.5 * tot1;
-              P.out0[b] = P.accumulate ? P.out0[b] + v : v;
-            } else {
-              if (P.out0) P.out0[b] = P.accumulate ? P.out0[b] + tot0 : tot0;
-              if (P.out1) P.out1[b] = P.accumulate ? P.out1[b] + tot1 : tot1;
-            }
-            tot0 = 0.0; tot1 = 0.0;
-          }
-          totS[0] = tot0; totS[1] = tot1;
-        }
+      for (int g = tid; g < M / RI1; g += NT) last_pass_c<RI1, M, MODE>(ZE, ZO, g, sg.n, tw, sg.zd, acc0, acc1);
+      if (MODE == MODE_INNER) acc0 = warp_sum(acc0);
+      if (MODE != MODE_STOREZ) acc1 = warp_sum(acc1);
+      TDCLK(12);
+      if (MODE != MODE_STOREZ && lane == 0) {
+        double* r = red + 2 * NW * (item & 1);
+        r[2 * warp] = acc0; r[2 * warp + 1] = acc1;
       }
+      if (tid == 0) { pend_b = b; pend_add = (P.accumulate || s > 0) ? 1 : 0; }
+      ++item;
+      staged = staged_next;
     }
-    b = nb; s = ns; have = have_next; staged = staged_next;
   }
+  __syncthreads();
+  if (tid == 0) finalize();
+  if (warp == 0) tmem_dealloc<Sh::TMEM_COLS>(*tmem_slot);
+#ifdef TD_PHASE_CLOCKS
+  if (tid < 16 * NW && blockIdx.x < 148) g_phase_clk[blockIdx.x * 256 + tid] = clk_s[tid];
+#endif
 }
 
 }  // namespace td

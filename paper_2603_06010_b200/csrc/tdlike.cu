@@ -99,6 +99,15 @@ struct td_handle {
     }                                                                                          \
   } while (0)
 
+#ifdef TD_DEBUG_KNOBS
+// experiment knobs of debug builds (_work probes); the product build compiles the defaults in
+static int g_tune[16] = {-1, -1, -1, -1, -1, -1, -1, -1, -1, -1, -1, -1, -1, -1, -1, -1};
+static inline int tune(int i, int dflt) { return g_tune[i] < 0 ? dflt : g_tune[i]; }
+extern "C" void td_debug_set_tune(int i, int v) { if (i >= 0 && i < 16) g_tune[i] = v; }
+#else
+static inline constexpr int tune(int, int dflt) { return dflt; }
+#endif
+
 namespace {
 
 int next_log2(int n) { int l = 0; while ((1 << l) < n) ++l; return l; }
@@ -309,10 +318,14 @@ td_status launch_fused4(td_handle* h, const FusedParams& P, const cplx* const* G
   int nb = 0;
   CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kern, NT, smem));
   if (nb < 1) return TD_EUNSUPPORTED;
+  nb = std::min(nb, 512 / Fused4Shape<LOG2M>::TMEM_COLS);  // co-resident CTAs share the SM's 512 tensor-memory columns
   const long long maxg = (long long)nb * h->num_sms;
   const int grid = (int)std::max<long long>(1, std::min<long long>(MODE == MODE_STOREZ ? 1 : P.B, maxg));
   Fused4Params P4;
   P4.base = P; P4.Gp = Gp;
+#ifdef TD_DEBUG_KNOBS
+  P4.skew = tune(1, 0);
+#endif
   kern<<<grid, NT, smem, st>>>(P4);
   CK(cudaGetLastError());
   ++h->last_launches;
@@ -338,6 +351,9 @@ td_status launch_cluster(td_handle* h, const FusedParams& P, const cplx* const* 
   cfg.gridDim = dim3(2 * (unsigned)std::max<long long>(1, std::min<long long>(want, ncl)));
   Fused4Params P4;
   P4.base = P; P4.Gp = Gp;
+#ifdef TD_DEBUG_KNOBS
+  P4.skew = 0;
+#endif
   CK(cudaLaunchKernelEx(&cfg, kern, P4));
   ++h->last_launches;
   return TD_OK;
@@ -959,5 +975,11 @@ td_status td_probe_phase(int threads, int groups, int device, double* cycles) {
 }
 
 int td_last_launches(const td_handle* h) { return h ? h->last_launches : 0; }
+
+#ifdef TD_PHASE_CLOCKS
+int td_debug_phase_clocks(long long* host, int n) {
+  return (int)cudaMemcpyFromSymbol(host, td::g_phase_clk, sizeof(long long) * n);
+}
+#endif
 
 }  // extern "C"
