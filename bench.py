@@ -32,7 +32,7 @@ METRIC = "fp64 likelihood evals/sec"
 UNIT = "evals/s"
 # fp64 ALU roofline: 64 DFMA/clk/SM x 148 SMs x 1.965 GHz x 2 flop (guide unit counts and
 # clocks.max.sm); the register-loop DFMA / DMMA throughputs are measured in every run
-# (td_probe_fp64) and reported beside it.  DESIGN.md 6.
+# (libtdprobe.so, include/tdprobe.h) and reported beside it.  DESIGN.md 6.
 FP64_PEAK_TFLOPS = 37.2
 # dominant kernel of a step, per config
 DOMINANT = {"c1": "td_fused4_kernel<10>", "c2": "td_fused4_kernel<12>", "c3": "td_cluster_kernel",
@@ -188,11 +188,9 @@ def main():
     tdb.load(build_if_missing=False)
     if args.probe_peaks:
         if rank == 0:
-            names = {0: "dfma", 1: "dmma_m8n8k4", 2: "dfma_and_dmma_interleaved", 3: "dadd"}
-            phase = {f"{nt}thr_{g}grp": tdb.probe_phase(nt, g, local)
-                     for nt, g in ((256, 1), (256, 2), (256, 8), (512, 1), (512, 2), (512, 16))}
-            print(json.dumps({"fp64_tflops": {names[k]: tdb.probe_fp64(k, local) for k in range(4)},
-                              "derived_peak": FP64_PEAK_TFLOPS, "phase_cycles": phase}))
+            names = {0: "dfma", 1: "dmma_m8n8k4", 2: "dfma_and_dmma_interleaved", 3: "dadd", 4: "ffma_fp32"}
+            print(json.dumps({"tflops": {names[k]: tdb.probe_throughput(k, local) for k in range(5)},
+                              "derived_fp64_peak": FP64_PEAK_TFLOPS}))
         return
 
     w = W.make(args.config, B=args.B)
@@ -322,7 +320,7 @@ def main():
     kern_ms = float(np.mean(step_ms))
     dense = path_used == 2
     falg = float(sum(2.0 * int(n) * int(n) for n in w.seg_lengths)) if dense else alg_flops_per_eval(w.seg_lengths)
-    probe = {"dfma": tdb.probe_fp64(0, local), "dmma": tdb.probe_fp64(1, local)}
+    probe = {"dfma": tdb.probe_throughput(0, local), "dmma": tdb.probe_throughput(1, local)}
     ach_tf = falg * B / (kern_ms * 1e-3) / 1e12
     ach_gbs = (8.0 * n_tot * B + 8.0 * B) / (kern_ms * 1e-3) / 1e9
     traffic = None

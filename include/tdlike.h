@@ -12,8 +12,19 @@
  *
  * All entry points return a td_status and never abort or throw.  Nothing here allocates or
  * frees caller memory.  There is no CPU fallback: every call needs a CUDA device.
- * A handle must not be used from two host threads at once (it owns workspace); calls issued
- * on one stream are ordered.
+ *
+ * Threads and streams.  A handle must not be used from two host threads at once.  The handle owns device scratch
+ * (the workspace of the long-segment kernels, z and u = C^{-1} d of the data vector for td_inner_batch, the synthesis
+ * panel of td_loglike_family_batch): calls issued on ONE stream are ordered by the stream; a call issued on a
+ * DIFFERENT stream than the previous scratch-using call first waits (cudaStreamWaitEvent) for that call, so one thread
+ * alternating between streams gets correct, serialised results.  Inside a CUDA stream capture the library records and
+ * waits on nothing: the captured graph's own dependencies order the work, and the caller must not replay such a graph
+ * concurrently with other calls on the same handle.
+ *
+ * Allocation.  td_create allocates everything whose size does not depend on the batch, sets every kernel attribute and
+ * caches every occupancy figure.  The device-pointer calls (td_loglike_batch, td_inner_batch) never allocate or
+ * synchronise: they only enqueue kernels, and can be captured into a CUDA graph.  Buffers that grow with the batch
+ * (host staging, the synthesis panel) are sized by td_reserve, or on first use when the caller did not reserve.
  */
 #ifndef TDLIKE_H_
 #define TDLIKE_H_
@@ -71,8 +82,8 @@ td_status td_destroy(td_handle* h);
  *   out  DEVICE pointer, B doubles: out[b] = -1/2 sum_s (d_s - h_bs)^T C_s^{-1} (d_s - h_bs)
  *        (the additive constant of Eq. 7 is NOT included; see td_get_info for log det).
  *   stream  a cudaStream_t (as void*; NULL = legacy default stream).
- * Asynchronous: kernels are enqueued on `stream`, no host synchronisation.  The residual
- * d - h_b and the filtered vectors are never written to HBM on the fused path.
+ * Asynchronous: kernels are enqueued on `stream`; no host synchronisation, no allocation (CUDA-graph capturable).
+ * The residual d - h_b and the filtered vectors are never written to HBM on the fused path.
  * NaN/Inf in row b of H (or in d) propagate to out[b].
  */
 td_status td_loglike_batch(td_handle* h, const double* d, const double* H, int64_t ldh,
@@ -126,11 +137,12 @@ td_status td_loglike_family_batch(td_handle* h, const double* d, int family, con
 td_status td_loglike_family_batch_host(td_handle* h, const double* d, int family, const double* params, int64_t B,
                                        double fs, double* out, void* stream);
 
-/* td_loglike_ringdown_batch, td_loglike_ringdown_batch_host - the two calls above with family = TD_FAMILY_RINGDOWN. */
-td_status td_loglike_ringdown_batch(td_handle* h, const double* d, const double* params, int64_t B, double fs,
-                                    double* out, void* stream);
-td_status td_loglike_ringdown_batch_host(td_handle* h, const double* d, const double* params, int64_t B, double fs,
-                                         double* out, void* stream);
+/* td_reserve - sizes every batch-dependent buffer of the handle for calls of up to B_max templates: the partial sums of
+ * the long-segment kernels, the device staging of td_loglike_batch_host (H chunks, d, out), the synthesis panel and the
+ * parameter buffer of td_loglike_family_batch(_host).  After it, no entry point allocates for B <= B_max (so the
+ * parameter entry point, too, is allocation-free and capturable).  Grow-only; synchronous (cudaMalloc).
+ * Errors: TD_EINVAL (B_max < 0), TD_ENOMEM, TD_ECUDA. */
+td_status td_reserve(td_handle* h, int64_t B_max);
 
 /* td_set_path - force the evaluation path for subsequent calls (TD_PATH_AUTO restores the
  * chooser).  TD_PATH_DENSE on a handle with a segment longer than the dense path supports
@@ -160,21 +172,6 @@ td_status td_get_generator(const td_handle* h, int seg, double* a);
 /* td_last_launches - number of kernels of this library launched by the last batch call on
  * this handle (evidence for bench.py's gpu_launches). */
 int td_last_launches(const td_handle* h);
-
-/* td_probe_fp64 - measures the fp64 throughput of `device` with register-resident loops (no memory
- * traffic), for the roofline denominators of bench.py:
- *   kind 0  DFMA chains (vector fp64 pipe),   kind 1  mma.sync.m8n8k4.f64 chains (fp64 tensor pipe),
- *   kind 2  both interleaved in the same warps,  kind 3  DADD chains (1 flop per instruction).
- * tflops (HOST pointer) receives the best of 5 timed launches in TFLOP/s.  Synchronous; uses the
- * legacy default stream.  Errors: TD_EINVAL, TD_ECUDA. */
-td_status td_probe_fp64(int kind, int device, double* tflops);
-
-/* td_probe_phase - one "phase" of the fused FFT kernels in isolation (evidence for DESIGN.md 6.1): a CTA of `threads`
- * threads pushes 2 x 4096 complex through 512 radix-16 shared-memory tasks per phase, with a barrier over the whole CTA
- * (groups = 1) or only inside each of `groups` independent thread groups.  cycles (HOST pointer) receives the SM cycles
- * per phase of one CTA running alone.  Supported (threads, groups): (256,1) (256,2) (256,8) (512,1) (512,2) (512,16);
- * anything else returns TD_EINVAL.  Synchronous; legacy default stream. */
-td_status td_probe_phase(int threads, int groups, int device, double* cycles);
 
 /* td_strerror - static string for a status code. */
 const char* td_strerror(td_status s);

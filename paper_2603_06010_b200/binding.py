@@ -29,15 +29,12 @@ SYMBOLS = {
     "td_loglike_batch_host": (_INT, [_VP, _VP, _VP, _I64, _I64, _VP, _VP]),
     "td_loglike_family_batch": (_INT, [_VP, _VP, _INT, _VP, _I64, C.c_double, _VP, _VP]),
     "td_loglike_family_batch_host": (_INT, [_VP, _VP, _INT, _VP, _I64, C.c_double, _VP, _VP]),
-    "td_loglike_ringdown_batch": (_INT, [_VP, _VP, _VP, _I64, C.c_double, _VP, _VP]),
-    "td_loglike_ringdown_batch_host": (_INT, [_VP, _VP, _VP, _I64, C.c_double, _VP, _VP]),
+    "td_reserve": (_INT, [_VP, _I64]),
     "td_set_path": (_INT, [_VP, _INT]),
     "td_set_fft_variant": (_INT, [_VP, _INT]),
     "td_get_info": (_INT, [_VP, C.POINTER(C.c_int64), C.POINTER(_INT), _DP, _DP, C.POINTER(_INT)]),
     "td_get_generator": (_INT, [_VP, _INT, _DP]),
     "td_last_launches": (_INT, [_VP]),
-    "td_probe_fp64": (_INT, [_INT, _INT, _DP]),
-    "td_probe_phase": (_INT, [_INT, _INT, _INT, _DP]),
     "td_strerror": (C.c_char_p, [_INT]),
 }
 
@@ -178,12 +175,6 @@ class TDLikelihood:
         _check(st, "td_loglike_batch_host")
         return out_host
 
-    def loglike_ringdown_batch(self, d, params, fs: float, out=None, stream=None):
-        return self.loglike_family_batch(d, TD_FAMILY_RINGDOWN, params, fs, out=out, stream=stream)
-
-    def loglike_ringdown_batch_host(self, d_host, params_host, fs: float, out_host=None, stream=None):
-        return self.loglike_family_batch_host(d_host, TD_FAMILY_RINGDOWN, params_host, fs, out_host=out_host, stream=stream)
-
     def loglike_family_batch(self, d, family: int, params, fs: float, out=None, stream=None):
         """logL of templates of an analytic family (TD_FAMILY_*) given as rows of 5 parameters: CUDA float64 [B, 5]
         (one segment) or [B, n_seg, 5] (one row per template and segment / detector)."""
@@ -219,6 +210,10 @@ class TDLikelihood:
         return out_host
 
     # -- options / queries ---------------------------------------------------------------
+    def reserve(self, B_max: int):
+        """Size every batch-dependent buffer for calls of up to B_max templates (td_reserve)."""
+        _check(self._lib.td_reserve(self._h, int(B_max)), "td_reserve")
+
     def set_path(self, path: int):
         _check(self._lib.td_set_path(self._h, int(path)), "td_set_path")
 
@@ -243,17 +238,21 @@ class TDLikelihood:
         return int(self._lib.td_last_launches(self._h))
 
 
-def probe_fp64(kind: int, device: int = 0) -> float:
-    """TFLOP/s of a register-resident fp64 loop (0 DFMA, 1 DMMA m8n8k4, 2 both, 3 DADD)."""
-    v = C.c_double()
-    _check(load().td_probe_fp64(int(kind), int(device), C.byref(v)), "td_probe_fp64")
-    return float(v.value)
+PROBE_LIB_PATH = os.path.join(_HERE, "lib", "libtdprobe.so")
+_probe_lib = None
 
 
-def probe_phase(threads: int, groups: int, device: int = 0) -> float:
-    """SM cycles per isolated radix-16 shared-memory phase (see td_probe_phase in include/tdlike.h)."""
+def probe_throughput(kind: int, device: int = 0) -> float:
+    """TFLOP/s of a register-resident loop (0 DFMA, 1 DMMA m8n8k4, 2 both, 3 DADD, 4 FFMA), from the bench-only
+    library libtdprobe.so (include/tdprobe.h); not part of the product library."""
+    global _probe_lib
+    if _probe_lib is None:
+        lib = C.CDLL(PROBE_LIB_PATH)
+        lib.td_probe_throughput.restype = _INT
+        lib.td_probe_throughput.argtypes = [_INT, _INT, _DP]
+        _probe_lib = lib
     v = C.c_double()
-    _check(load().td_probe_phase(int(threads), int(groups), int(device), C.byref(v)), "td_probe_phase")
+    _check(_probe_lib.td_probe_throughput(int(kind), int(device), C.byref(v)), "td_probe_throughput")
     return float(v.value)
 
 

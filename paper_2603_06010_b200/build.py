@@ -15,6 +15,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIBDIR = os.path.join(HERE, "lib")
 LIB = os.path.join(LIBDIR, "libtdlike.so")
+PROBE_LIB = os.path.join(LIBDIR, "libtdprobe.so")   # bench-only (include/tdprobe.h), separate from the product library
+PROBE_SRC = os.path.join(CSRC, "probe", "tdprobe.cu")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 
 FLAGS = [
@@ -28,28 +30,31 @@ def sources():
 
 
 def deps():
-    out = [os.path.join(CSRC, f) for f in os.listdir(CSRC)]
+    out = [os.path.join(CSRC, f) for f in os.listdir(CSRC) if os.path.isfile(os.path.join(CSRC, f))]
     out.append(os.path.join(os.path.dirname(HERE), "include", "tdlike.h"))
     return out
 
 
 def up_to_date() -> bool:
-    if not os.path.exists(LIB):
+    if not os.path.exists(LIB) or not os.path.exists(PROBE_LIB):
         return False
     t = os.path.getmtime(LIB)
-    return all(os.path.getmtime(p) <= t for p in deps())
+    inc = os.path.join(os.path.dirname(HERE), "include", "tdprobe.h")
+    return (all(os.path.getmtime(p) <= t for p in deps())
+            and all(os.path.getmtime(p) <= os.path.getmtime(PROBE_LIB) for p in (PROBE_SRC, inc)))
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
     if not force and up_to_date():
         return LIB
     os.makedirs(LIBDIR, exist_ok=True)
-    cmd = [NVCC] + FLAGS + (["-Xptxas", "-v"] if verbose else []) + sources() + ["-o", LIB]
-    res = subprocess.run(cmd, capture_output=True, text=True)
-    if verbose or res.returncode != 0:
-        sys.stderr.write(res.stdout + res.stderr)
-    if res.returncode != 0:
-        raise RuntimeError("nvcc failed: " + " ".join(cmd))
+    for srcs, lib in ((sources(), LIB), ([PROBE_SRC], PROBE_LIB)):
+        cmd = [NVCC] + FLAGS + (["-Xptxas", "-v"] if verbose else []) + srcs + ["-o", lib]
+        res = subprocess.run(cmd, capture_output=True, text=True)
+        if verbose or res.returncode != 0:
+            sys.stderr.write(res.stdout + res.stderr)
+        if res.returncode != 0:
+            raise RuntimeError("nvcc failed: " + " ".join(cmd))
     return LIB
 
 

@@ -5,8 +5,7 @@
 //   kind 2: both in the same warps, interleaved     (do the two pipes overlap on sm_100a?)
 //   kind 3: DADD chains                             1 flop per lane-instruction (the FFT's dominant op)
 #pragma once
-#include "td_common.cuh"
-#include "td_dit16.cuh"
+#include <cuda_runtime.h>
 
 namespace td {
 
@@ -47,43 +46,6 @@ inline double probe_flops(int kind, int grid, int iters) {
   if (kind == 3) fl += 1.0 * per_thread_steps * threads;
   if (kind == 1 || kind == 2) fl += 512.0 * per_thread_steps * (threads / 32.0);
   return fl;
-}
-
-// ---- phase probe ---------------------------------------------------------------------------------
-// One "phase" of the fused FFT kernels in isolation: 2 x 4096 complex in padded shared memory, every element goes
-// through one radix-16 task (16 loads, merged-twiddle butterfly, 16 stores), then a barrier - over all NT threads
-// (NGRP = 1: what a CTA-wide pass does) or only within each of NGRP independent thread groups, which then drift into a
-// steady state where one group's loads and stores overlap another's butterflies.  Floors per phase: 2048 cycles of
-// shared-memory wavefronts, ~2000 cycles of fp64 issue.  Reported: cycles per phase (clock64 of thread 0, one CTA).
-template <int NT, int NGRP>
-__global__ void __launch_bounds__(NT, 1) probe_phase_kernel(double* sink, long long* cyc, int iters, const cplx* __restrict__ T) {
-  extern __shared__ __align__(16) unsigned char probe_raw[];
-  cplx* sm = reinterpret_cast<cplx*>(probe_raw);
-  const SmemArr Z{sm};
-  const int tid = threadIdx.x, grp = tid / (NT / NGRP);
-  for (int i = tid; i < SmemArr::padded(8192); i += NT) sm[i] = mk(1e-3 * i, 1.0);
-  __syncthreads();
-  constexpr int PER = 512 / NT;  // 512 radix-16 tasks per phase
-  const long long t0 = clock64();
-  for (int it = 0; it < iters; ++it) {
-    cplx x[PER][16];
-#pragma unroll
-    for (int u = 0; u < PER; ++u) {
-      const int g = tid + u * NT, base = (g >> 4) * 256 + (g & 15);
-#pragma unroll
-      for (int q = 0; q < 16; ++q) x[u][q] = Z.ld(base + 16 * q);
-    }
-#pragma unroll
-    for (int u = 0; u < PER; ++u) {
-      const int g = tid + u * NT, base = (g >> 4) * 256 + (g & 15);
-      dit16<true, true>(x[u], T[(g & 15) * 32]);
-      static_for<0, 16>([&](auto t) { Z.st(base + 16 * decltype(t)::value, x[u][brevR<16>(decltype(t)::value)]); });
-    }
-    if (NT / NGRP == 32) __syncwarp();
-    else asm volatile("bar.sync %0, %1;" ::"r"(1 + grp), "r"(NT / NGRP) : "memory");
-  }
-  __syncthreads();
-  if (tid == 0) { *cyc = clock64() - t0; sink[0] = sm[5].x; }
 }
 
 }  // namespace td

@@ -16,7 +16,6 @@
 #include "td_fused.cuh"
 #include "td_cluster.cuh"
 #include "td_fused4.cuh"
-#include "td_probe.cuh"
 #include "td_setup.cuh"
 #include "td_staged.cuh"
 #include "td_synth.cuh"
@@ -66,13 +65,16 @@ struct DevGuard {
 
 struct td_handle {
   int device = 0, n_seg = 0, num_sms = 0;
+  size_t smem_optin = 0;  // opt-in shared memory per CTA of the device
   int64_t n_tot = 0;
   std::vector<SegHost> segs;
   std::vector<ClassInfo> classes;
   int path = TD_PATH_AUTO, fft_variant = 0, last_path = 0, last_launches = 0;
   int max_n = 0;
-  // staged workspace (grow-only)
+  // staged workspace: U / Z sized by td_create (two lanes of an L2-resident chunk), the per-block partial sums by
+  // td_create / td_reserve (a batch larger than they hold is processed in sub-batches)
   cplx* wsU = nullptr; cplx* wsZ = nullptr; double* wsPartial = nullptr;
+  double* wsDot = nullptr;  // per-tile partial weights of the dot path (td_dot.cuh)
   double* synH = nullptr; size_t synH_elems = 0;  // scratch panel of synthesised templates (td_synth.cuh)
   double* synP = nullptr; size_t synP_elems = 0;  // device copy of host parameters
   SynSeg* synSeg = nullptr;                       // device [n_seg]: offsets and lengths for the synthesis kernel
@@ -87,16 +89,16 @@ struct td_handle {
   cudaStream_t aux_stream = nullptr;              // second lane of the staged path (chunks alternate between two streams)
   cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
   cudaEvent_t ev_copied[2] = {nullptr, nullptr}, ev_done[2] = {nullptr, nullptr};
+  // cross-stream ordering of calls that touch handle-owned scratch (include/tdlike.h "Streams")
+  cudaEvent_t ev_last = nullptr;
+  cudaStream_t last_stream = nullptr;
+  bool last_valid = false, touched = false;
 };
 
 #define CK(call)                                                                               \
   do {                                                                                         \
     cudaError_t e_ = (call);                                                                   \
-    if (e_ != cudaSuccess) {                                                                   \
-      if (getenv("TDLIKE_DEBUG")) fprintf(stderr, "tdlike: %s -> %s (%s:%d)\n", #call,         \
-                                          cudaGetErrorString(e_), __FILE__, __LINE__);         \
-      return e_ == cudaErrorMemoryAllocation ? TD_ENOMEM : TD_ECUDA;                           \
-    }                                                                                          \
+    if (e_ != cudaSuccess) return e_ == cudaErrorMemoryAllocation ? TD_ENOMEM : TD_ECUDA;      \
   } while (0)
 
 #ifdef TD_DEBUG_KNOBS
@@ -112,16 +114,34 @@ namespace {
 
 int next_log2(int n) { int l = 0; while ((1 << l) < n) ++l; return l; }
 
+// One-time launch configuration per (kernel instantiation, device): the dynamic shared-memory attribute and the
+// occupancy query run on the first use only; td_create makes that first use (a "dry" pass over every kernel its size
+// classes can reach), so a batch call contains nothing but launches.  `cache` is the caller's function-local static.
+constexpr int TD_MAX_DEV = 64;
+template <class K>
+td_status kernel_config(K kern, int nt, size_t smem_attr, size_t smem, int device, int* cache, int* blocks_per_sm) {
+  if (device < 0 || device >= TD_MAX_DEV) return TD_EUNSUPPORTED;
+  if (cache[device] == 0) {
+    if (smem_attr > 48 * 1024) CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_attr));
+    int nb = 0;
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kern, nt, smem));
+    cache[device] = nb + 1;
+  }
+  *blocks_per_sm = cache[device] - 1;
+  return TD_OK;
+}
+
 void free_handle(td_handle* h) {
   if (!h) return;
   for (auto& s : h->segs) { cudaFree(s.a); cudaFree(s.G); cudaFree(s.Gp); cudaFree(s.zd); }
   for (auto& c : h->classes) { cudaFree(c.T); cudaFree(c.d_segs); cudaFree(c.d_Gp); }
-  cudaFree(h->wsU); cudaFree(h->wsZ); cudaFree(h->wsPartial); cudaFree(h->ud); cudaFree(h->synH); cudaFree(h->synP); cudaFree(h->synSeg);
+  cudaFree(h->wsU); cudaFree(h->wsZ); cudaFree(h->wsPartial); cudaFree(h->wsDot); cudaFree(h->ud); cudaFree(h->synH); cudaFree(h->synP); cudaFree(h->synSeg);
   cudaFree(h->hsD); cudaFree(h->hsH[0]); cudaFree(h->hsH[1]); cudaFree(h->hsOut);
   if (h->copy_stream) cudaStreamDestroy(h->copy_stream);
   if (h->aux_stream) cudaStreamDestroy(h->aux_stream);
   if (h->ev_fork) cudaEventDestroy(h->ev_fork);
   if (h->ev_join) cudaEventDestroy(h->ev_join);
+  if (h->ev_last) cudaEventDestroy(h->ev_last);
   for (int i = 0; i < 2; ++i) { if (h->ev_copied[i]) cudaEventDestroy(h->ev_copied[i]); if (h->ev_done[i]) cudaEventDestroy(h->ev_done[i]); }
   delete h;
 }
@@ -141,9 +161,12 @@ td_status launch_pass(int R, cplx* base, int narr, int n, int L, const cplx* T, 
 }
 
 template <bool FWD>
-td_status launch_block(cplx* base, int narr, int n, const cplx* T, int TW, cudaStream_t st) {
+td_status launch_block(int device, cplx* base, int narr, int n, const cplx* T, int TW, cudaStream_t st, bool dry = false) {
   auto kern = lg_block_kernel<FWD>;
-  CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)LGB_SMEM));
+  static int cache[TD_MAX_DEV];
+  int nb = 0;
+  td_status cs = kernel_config(kern, LGB_NT, LGB_SMEM, LGB_SMEM, device, cache, &nb);
+  if (cs != TD_OK || dry) return cs;
   kern<<<dim3(n / LGB_N, narr), LGB_NT, LGB_SMEM, st>>>(base, n, T, TW);
   CK(cudaGetLastError());
   return TD_OK;
@@ -151,14 +174,14 @@ td_status launch_block(cplx* base, int narr, int n, const cplx* T, int TW, cudaS
 
 // forward DIF of `narr` arrays of length n with plan [r1,16,16,...]; the last three passes
 // (L = 4096, 256, 16) run as one shared-memory block kernel when the plan has them
-td_status staged_forward(cplx* base, int narr, int n, int first_pass_done, const cplx* T, int TW,
+td_status staged_forward(int device, cplx* base, int narr, int n, int first_pass_done, const cplx* T, int TW,
                          cudaStream_t st, int* launches) {
   int L = n;
   const int r1 = plan_r1(n), np = plan_np(n);
   for (int q = 0; q < np; ++q) {
     const int R = q == 0 ? r1 : 16;
     if (q >= 1 && q == np - 3 && L == LGB_N) {
-      td_status s = launch_block<true>(base, narr, n, T, TW, st);
+      td_status s = launch_block<true>(device, base, narr, n, T, TW, st);
       if (s != TD_OK) return s;
       ++*launches;
       break;
@@ -175,12 +198,12 @@ td_status staged_forward(cplx* base, int narr, int n, int first_pass_done, const
 
 // inverse DIT passes except the last (radix r1, L = n) one; the first three (L = 16, 256, 4096)
 // as one shared-memory block kernel when the plan has them
-td_status staged_inverse_but_last(cplx* base, int narr, int n, const cplx* T, int TW, cudaStream_t st,
+td_status staged_inverse_but_last(int device, cplx* base, int narr, int n, const cplx* T, int TW, cudaStream_t st,
                                   int* launches) {
   const int np = plan_np(n);
   int L = 16, q = 1;
   if (np - 1 >= 3) {
-    td_status s = launch_block<false>(base, narr, n, T, TW, st);
+    td_status s = launch_block<false>(device, base, narr, n, T, TW, st);
     if (s != TD_OK) return s;
     ++*launches;
     L <<= 12; q = 4;
@@ -219,43 +242,74 @@ td_status launch_last(int R, dim3 grid, const StagedParams& P, cudaStream_t st) 
   return TD_OK;
 }
 
-td_status ensure_ws(td_handle* h, size_t u, size_t z, size_t p) {
-  if (u > h->wsU_elems) { cudaFree(h->wsU); h->wsU = nullptr; h->wsU_elems = 0; CK(cudaMalloc(&h->wsU, u * sizeof(cplx))); h->wsU_elems = u; }
-  if (z > h->wsZ_elems) { cudaFree(h->wsZ); h->wsZ = nullptr; h->wsZ_elems = 0; CK(cudaMalloc(&h->wsZ, z * sizeof(cplx))); h->wsZ_elems = z; }
-  if (p > h->wsP_elems) { cudaFree(h->wsPartial); h->wsPartial = nullptr; h->wsP_elems = 0; CK(cudaMalloc(&h->wsPartial, p * sizeof(double))); h->wsP_elems = p; }
+// grow-only device buffer (td_create / td_reserve; a batch call reaches the cudaMalloc only when the caller did not reserve)
+template <class T> td_status grow(T*& p, size_t& have, size_t want) {
+  if (want <= have) return TD_OK;
+  cudaFree(p); p = nullptr; have = 0;
+  CK(cudaMalloc(&p, want * sizeof(T)));
+  have = want;
+  return TD_OK;
+}
+
+// staged path geometry of one size class: templates per lane chunk, workspace shares
+struct StagedGeom { int64_t CB; size_t uh, zh; int nblk, rI, rF; };
+StagedGeom staged_geom(int log2M) {
+  const int M = 1 << log2M, nf = M / 2;
+  const size_t per_tmpl = (size_t)(2 * nf + 2 * M) * sizeof(cplx);
+  StagedGeom g;
+  g.CB = std::max<int64_t>(1, (int64_t)(STAGED_WS_BYTES / 2 / per_tmpl));
+  g.CB = std::min<int64_t>(g.CB, 32767);  // grid.y = 2*CB arrays per pass
+  g.rI = plan_r1(M); g.rF = plan_r1(nf);
+  g.nblk = (M / g.rI + LG_NT - 1) / LG_NT;
+  g.uh = (size_t)g.CB * 2 * nf; g.zh = (size_t)g.CB * 2 * M;
+  return g;
+}
+constexpr size_t STAGED_PARTIAL_DEFAULT = 16ull << 20, STAGED_PARTIAL_MAX = 1ull << 30;  // bytes of per-block partial sums
+
+// cross-stream ordering of the calls that use handle-owned scratch (staged workspace, z / u of the data vector, the
+// synthesis panel): a call on another stream than the previous such call first waits for it.  Inside a stream capture
+// nothing is recorded or waited on (the graph's own edges order the work).
+td_status order_begin(td_handle* h, cudaStream_t st) {
+  h->touched = false;
+  if (!h->last_valid || h->last_stream == st) return TD_OK;
+  cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+  CK(cudaStreamIsCapturing(st, &cs));
+  if (cs == cudaStreamCaptureStatusNone) CK(cudaStreamWaitEvent(st, h->ev_last, 0));
+  return TD_OK;
+}
+td_status order_end(td_handle* h, cudaStream_t st) {
+  if (!h->touched) return TD_OK;
+  cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+  CK(cudaStreamIsCapturing(st, &cs));
+  if (cs != cudaStreamCaptureStatusNone) { h->last_valid = false; return TD_OK; }
+  CK(cudaEventRecord(h->ev_last, st));
+  h->last_stream = st; h->last_valid = true;
   return TD_OK;
 }
 
 // One segment of a size class through the staged pipeline for templates [0, B).
 template <int MODE>
-td_status run_staged(td_handle* h, const ClassInfo& cls, const SegHost& sg, const double* d, const double* H,
-                     int64_t ldh, int64_t B, double* out0, double* out1, double scale0, double scale1,
-                     int accumulate, cudaStream_t st) {
+td_status run_staged_sub(td_handle* h, const ClassInfo& cls, const SegHost& sg, const double* d, const double* H,
+                         int64_t ldh, int64_t B, double* out0, double* out1, double scale0, double scale1,
+                         int accumulate, cudaStream_t st) {
   const int M = 1 << cls.log2M, nf = M / 2, TW = 2 * M;
-  const size_t per_tmpl = (size_t)(2 * nf + 2 * M) * sizeof(cplx);
   // Two lanes: chunks alternate between the caller's stream and an internal one, each lane with its own half of the
   // L2-resident workspace.  No kernel of the pipeline fills the GPU on its own (a few hundred CTAs, each bound by L2
   // latency at the start and end of its life), so two chunks in flight overlap one another's ramps and tails.
-  int64_t CB = std::max<int64_t>(1, (int64_t)(STAGED_WS_BYTES / 2 / per_tmpl));
-  CB = std::min<int64_t>(CB, std::max<int64_t>(B, 1));
-  CB = std::min<int64_t>(CB, 32767);  // grid.y = 2*CB arrays per pass
+  const StagedGeom g = staged_geom(cls.log2M);
+  const int64_t CB = std::min<int64_t>(g.CB, std::max<int64_t>(B, 1));
   const bool two = B > CB;
-  const int rI = plan_r1(M), rF = plan_r1(nf);
-  const int nblk = (M / rI + LG_NT - 1) / LG_NT;
-  const size_t uh = (size_t)CB * 2 * nf, zh = (size_t)CB * 2 * M;  // one lane's share
-  td_status s = ensure_ws(h, (two ? 2 : 1) * uh, (two ? 2 : 1) * zh, (size_t)std::max<int64_t>(B, 1) * nblk * 2);
-  if (s != TD_OK) return s;
+  const int rI = g.rI, rF = g.rF, nblk = g.nblk;
+  const size_t uh = g.uh, zh = g.zh;  // one lane's share
+  if (h->wsU_elems < 2 * uh || h->wsZ_elems < 2 * zh) return TD_EUNSUPPORTED;  // (never: td_create sized them)
+  h->touched = true;
   if (two) {
-    if (!h->aux_stream) {
-      CK(cudaStreamCreateWithFlags(&h->aux_stream, cudaStreamNonBlocking));
-      CK(cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming));
-      CK(cudaEventCreateWithFlags(&h->ev_join, cudaEventDisableTiming));
-    }
     CK(cudaEventRecord(h->ev_fork, st));          // everything enqueued on the caller's stream so far comes first
     CK(cudaStreamWaitEvent(h->aux_stream, h->ev_fork, 0));
   }
   int lane = 0;
-  for (int64_t b0 = 0; b0 < B; b0 += CB, lane ^= 1) {
+  td_status s = TD_OK;
+  for (int64_t b0 = 0; b0 < B && s == TD_OK; b0 += CB, lane ^= 1) {
     const int cb = (int)std::min<int64_t>(CB, B - b0);
     cudaStream_t ls = (two && lane) ? h->aux_stream : st;
     cplx* U = h->wsU + (two && lane ? uh : 0);
@@ -265,27 +319,28 @@ td_status run_staged(td_handle* h, const ClassInfo& cls, const SegHost& sg, cons
     P.seg.off = sg.off; P.seg.n = sg.n; P.seg._pad = 0; P.seg.G = sg.G; P.seg.zd = sg.zd;
     P.M = M; P.U = U; P.Z = Z; P.T = cls.T; P.partial = h->wsPartial + (size_t)b0 * nblk * 2; P.nblk = nblk;
     s = launch_first<MODE>(rF, dim3((nf / rF + LG_NT - 1) / LG_NT, cb), P, ls);
-    if (s != TD_OK) return s;
+    if (s != TD_OK) break;
     ++h->last_launches;
-    s = staged_forward(U, 2 * cb, nf, 1, cls.T, TW, ls, &h->last_launches);
-    if (s != TD_OK) return s;
+    s = staged_forward(h->device, U, 2 * cb, nf, 1, cls.T, TW, ls, &h->last_launches);
+    if (s != TD_OK) break;
     // (fusing the untangle into the inverse block kernel - one CTA building a block, or a mirror pair of blocks, of Z in
     // shared memory straight from U and G - was measured: 50-68 us per chunk against 18 + 24 us for the two kernels; the
     // gather serialises 16 index-heavy tasks per thread, which the stand-alone kernel hides behind 1.4 M threads)
     lg_untangle_kernel<<<dim3((nf + LG_NT - 1) / LG_NT, 2, cb), LG_NT, 0, ls>>>(P);
-    CK(cudaGetLastError());
+    if (cudaGetLastError() != cudaSuccess) { s = TD_ECUDA; break; }
     ++h->last_launches;
-    s = staged_inverse_but_last(Z, 2 * cb, M, cls.T, TW, ls, &h->last_launches);
-    if (s != TD_OK) return s;
+    s = staged_inverse_but_last(h->device, Z, 2 * cb, M, cls.T, TW, ls, &h->last_launches);
+    if (s != TD_OK) break;
     s = launch_last<MODE>(rI, dim3(nblk, cb), P, ls);
-    if (s != TD_OK) return s;
+    if (s != TD_OK) break;
     ++h->last_launches;
   }
-  if (two) {
-    CK(cudaEventRecord(h->ev_join, h->aux_stream));
-    CK(cudaStreamWaitEvent(st, h->ev_join, 0));
+  if (two) {  // the aux lane is joined on every path, also after an error
+    const bool j = cudaEventRecord(h->ev_join, h->aux_stream) == cudaSuccess && cudaStreamWaitEvent(st, h->ev_join, 0) == cudaSuccess;
+    if (!j && s == TD_OK) s = TD_ECUDA;
   }
-  if (MODE != MODE_STOREZ && B > 0) {  // one reduction of the per-block partial sums for the whole batch (fixed order)
+  if (s != TD_OK) return s;
+  if (MODE != MODE_STOREZ && B > 0) {  // one reduction of the per-block partial sums for the whole sub-batch (fixed order)
     lg_finish_kernel<<<(unsigned)((B + 127) / 128), 128, 0, st>>>(h->wsPartial, nblk, (int)B, out0, out1, scale0, scale1, accumulate);
     CK(cudaGetLastError());
     ++h->last_launches;
@@ -293,14 +348,33 @@ td_status run_staged(td_handle* h, const ClassInfo& cls, const SegHost& sg, cons
   return TD_OK;
 }
 
+// sub-batches of as many templates as the partial-sum buffer holds (td_reserve sizes it for the caller's largest batch)
+template <int MODE>
+td_status run_staged(td_handle* h, const ClassInfo& cls, const SegHost& sg, const double* d, const double* H,
+                     int64_t ldh, int64_t B, double* out0, double* out1, double scale0, double scale1,
+                     int accumulate, cudaStream_t st) {
+  const StagedGeom g = staged_geom(cls.log2M);
+  const int64_t SB = std::min<int64_t>(std::max<int64_t>(1, (int64_t)(h->wsP_elems / ((size_t)g.nblk * 2))), 1 << 30);
+  if (h->wsP_elems < (size_t)g.nblk * 2) return TD_EUNSUPPORTED;  // (never: td_create holds at least one template)
+  for (int64_t b0 = 0; b0 < std::max<int64_t>(B, 1); b0 += SB) {
+    const int64_t nb = std::min<int64_t>(SB, B - b0);
+    td_status s = run_staged_sub<MODE>(h, cls, sg, d, H ? H + b0 * ldh : nullptr, ldh, nb, out0 ? out0 + b0 : nullptr,
+                                       out1 ? out1 + b0 : nullptr, scale0, scale1, accumulate, st);
+    if (s != TD_OK) return s;
+  }
+  return TD_OK;
+}
+
 template <int LOG2M, int MODE, int FUSED_NT, bool ILV = true>
-td_status launch_fused_nt(td_handle* h, const FusedParams& P, cudaStream_t st) {
+td_status launch_fused_nt(td_handle* h, const FusedParams& P, cudaStream_t st, bool dry) {
   auto kern = td_fused_kernel<LOG2M, FUSED_NT, MODE, ILV>;
   const size_t smem = FusedShape<LOG2M>::smem_bytes(FUSED_NT);
-  CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  static int cache[TD_MAX_DEV];
   int nb = 0;
-  CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kern, FUSED_NT, smem));
+  td_status cs = kernel_config(kern, FUSED_NT, smem, smem, h->device, cache, &nb);
+  if (cs != TD_OK) return cs;
   if (nb < 1) return TD_EUNSUPPORTED;
+  if (dry) return TD_OK;
   const long long maxg = (long long)nb * h->num_sms;
   const int grid = (int)std::max<long long>(1, std::min<long long>(MODE == MODE_STOREZ ? 1 : P.B, maxg));
   kern<<<grid, FUSED_NT, smem, st>>>(P);
@@ -310,14 +384,16 @@ td_status launch_fused_nt(td_handle* h, const FusedParams& P, cudaStream_t st) {
 }
 
 template <int LOG2M, int MODE>
-td_status launch_fused4(td_handle* h, const FusedParams& P, const cplx* const* Gp, cudaStream_t st) {
+td_status launch_fused4(td_handle* h, const FusedParams& P, const cplx* const* Gp, cudaStream_t st, bool dry) {
   auto kern = td_fused4_kernel<LOG2M, MODE>;
   constexpr int NT = Fused4Shape<LOG2M>::NT;
   const size_t smem = Fused4Shape<LOG2M>::smem_bytes();
-  CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  static int cache[TD_MAX_DEV];
   int nb = 0;
-  CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kern, NT, smem));
+  td_status cs = kernel_config(kern, NT, smem, smem, h->device, cache, &nb);
+  if (cs != TD_OK) return cs;
   if (nb < 1) return TD_EUNSUPPORTED;
+  if (dry) return TD_OK;
   nb = std::min(nb, 512 / Fused4Shape<LOG2M>::TMEM_COLS);  // co-resident CTAs share the SM's 512 tensor-memory columns
   const long long maxg = (long long)nb * h->num_sms;
   const int grid = (int)std::max<long long>(1, std::min<long long>(MODE == MODE_STOREZ ? 1 : P.B, maxg));
@@ -333,20 +409,27 @@ td_status launch_fused4(td_handle* h, const FusedParams& P, const cplx* const* G
 }
 
 template <int MODE>
-td_status launch_cluster(td_handle* h, const FusedParams& P, const cplx* const* Gp, cudaStream_t st) {
+td_status launch_cluster(td_handle* h, const FusedParams& P, const cplx* const* Gp, cudaStream_t st, bool dry) {
   auto kern = td_cluster_kernel<MODE>;
   const size_t smem = ClusterShape::smem_bytes();
-  CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  static int cache[TD_MAX_DEV];  // 0 = not configured on this device yet, else 1 + clusters that can be co-resident
+  if (h->device < 0 || h->device >= TD_MAX_DEV) return TD_EUNSUPPORTED;
   cudaLaunchConfig_t cfg = {};
   cudaLaunchAttribute attr[1];
   attr[0].id = cudaLaunchAttributeClusterDimension;
   attr[0].val.clusterDim.x = 2; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
   cfg.blockDim = dim3(ClusterShape::NT); cfg.dynamicSmemBytes = smem; cfg.stream = st;
   cfg.attrs = attr; cfg.numAttrs = 1;
-  cfg.gridDim = dim3(2 * (h->num_sms / 2));
-  int ncl = 0;
-  CK(cudaOccupancyMaxActiveClusters(&ncl, kern, &cfg));
+  if (cache[h->device] == 0) {
+    CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    cfg.gridDim = dim3(2 * (h->num_sms / 2));
+    int n = 0;
+    CK(cudaOccupancyMaxActiveClusters(&n, kern, &cfg));
+    cache[h->device] = n + 1;
+  }
+  const int ncl = cache[h->device] - 1;
   if (ncl < 1) return TD_EUNSUPPORTED;
+  if (dry) return TD_OK;
   const long long want = MODE == MODE_STOREZ ? 1 : P.B;
   cfg.gridDim = dim3(2 * (unsigned)std::max<long long>(1, std::min<long long>(want, ncl)));
   Fused4Params P4;
@@ -360,31 +443,33 @@ td_status launch_cluster(td_handle* h, const FusedParams& P, const cplx* const* 
 }
 
 template <int LOG2M, int MODE>
-td_status launch_fused_t(td_handle* h, const FusedParams& P, cudaStream_t st) {
-  return launch_fused_nt<LOG2M, MODE, FUSED_NT>(h, P, st);
+td_status launch_fused_t(td_handle* h, const FusedParams& P, cudaStream_t st, bool dry) {
+  return launch_fused_nt<LOG2M, MODE, FUSED_NT>(h, P, st, dry);
 }
 
 template <int MODE>
-td_status launch_fused(td_handle* h, int log2M, const FusedParams& P, const cplx* const* Gp, cudaStream_t st) {
-  if (log2M == CLUSTER_LOG2M) return Gp ? launch_cluster<MODE>(h, P, Gp, st) : TD_EUNSUPPORTED;
+td_status launch_fused(td_handle* h, int log2M, const FusedParams& P, const cplx* const* Gp, cudaStream_t st,
+                       bool dry = false) {
+  if (log2M == CLUSTER_LOG2M) return Gp ? launch_cluster<MODE>(h, P, Gp, st, dry) : TD_EUNSUPPORTED;
   if (Gp) {
     switch (log2M) {
-      case 10: return launch_fused4<10, MODE>(h, P, Gp, st);
-      case 11: return launch_fused4<11, MODE>(h, P, Gp, st);
-      case 12: return launch_fused4<12, MODE>(h, P, Gp, st);
+      case 10: return launch_fused4<10, MODE>(h, P, Gp, st, dry);
+      case 11: return launch_fused4<11, MODE>(h, P, Gp, st, dry);
+      case 12: return launch_fused4<12, MODE>(h, P, Gp, st, dry);
       default: break;
     }
   }
   switch (log2M) {
-    case 8: return launch_fused_t<8, MODE>(h, P, st);
-    case 9: return launch_fused_t<9, MODE>(h, P, st);
+    case 8: return launch_fused_t<8, MODE>(h, P, st, dry);
+    case 9: return launch_fused_t<9, MODE>(h, P, st, dry);
     default: return TD_EUNSUPPORTED;  // M >= 1024 always has the padded generator copy (Gp) of td_create
   }
 }
 
+bool class_is_fused_shape(int log2M) { return log2M >= FUSED_MIN_LOG2M && log2M <= CLUSTER_LOG2M; }
 bool class_is_fused(const td_handle* h, const ClassInfo& c) {
   if (h->fft_variant == 2) return false;
-  return c.log2M >= FUSED_MIN_LOG2M && c.log2M <= CLUSTER_LOG2M;
+  return class_is_fused_shape(c.log2M);
 }
 
 
@@ -416,7 +501,8 @@ td_status dense_upload(td_handle* h) {
 // one launch per segment; segments accumulate into the outputs in launch order
 template <int MODE>
 td_status launch_dense(td_handle* h, const std::vector<DenseSeg>& segs, const double* d, const double* H, int64_t ldh,
-                       int64_t B, double* out0, double* out1, int accumulate, cudaStream_t st) {
+                       int64_t B, double* out0, double* out1, int accumulate, cudaStream_t st, bool dry = false) {
+  static int cache[4][TD_MAX_DEV];  // per NWR instantiation of this MODE
   for (const DenseSeg& sg : segs) {
     DenseParams P;
     P.d = d; P.H = H; P.ldh = ldh; P.B = B; P.out0 = out0; P.out1 = out1; P.seg = sg;
@@ -437,7 +523,15 @@ td_status launch_dense(td_handle* h, const std::vector<DenseSeg>& segs, const do
       P.stagger_cycles = (int)std::min<long long>(nd * 16, 1 << 22);
     }
     const size_t smem = dense_smem_bytes(sg.npad, P.nbuf);
-    CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    {
+      // the attribute is set once to the device's opt-in maximum (the size itself varies with the segment length)
+      int nb = 0;
+      td_status cs = kernel_config(kern, DENSE_NT, h->smem_optin, smem, h->device,
+                                   cache[P.nwr == 1 ? 0 : P.nwr == 2 ? 1 : P.nwr == 4 ? 2 : 3], &nb);
+      if (cs != TD_OK) return cs;
+      if (smem > h->smem_optin) return TD_EUNSUPPORTED;
+    }
+    if (dry) continue;
     const int nwc = DENSE_NW / P.nwr;
     const int64_t grid = std::min<int64_t>((P.ntiles + nwc - 1) / nwc, h->num_sms);
     kern<<<(unsigned)grid, DENSE_NT, smem, st>>>(P);
@@ -496,32 +590,71 @@ td_status run_batch(td_handle* h, const double* d, const double* H, int64_t ldh,
 
 // <d, h_b> = u . h_b with u = C^{-1} d (td_dot.cuh); z of the data vector is already in every segment's zd
 td_status run_dot(td_handle* h, const double* H, int64_t ldh, int64_t B, double* out_dh, cudaStream_t st) {
-  if (!h->ud) CK(cudaMalloc(&h->ud, sizeof(double) * (size_t)h->n_tot));
-  {
-    size_t need = 0;  // per-tile partial weights of the longest segment: ntile rows of ntile * 128 doubles
-    for (const SegHost& sg : h->segs) { const size_t nt = (sg.n + DOTW_NT - 1) / DOTW_NT; need = std::max(need, nt * nt * DOTW_NT); }
-    td_status s = ensure_ws(h, 0, 0, need);
-    if (s != TD_OK) return s;
-  }
+  // h->ud and the per-tile partial weights (h->wsDot) were allocated by td_create
   for (const SegHost& sg : h->segs) {
     const int nt = (int)((sg.n + DOTW_NT - 1) / DOTW_NT);
-    dot_weight_tile_kernel<<<(unsigned)(nt * (nt + 1) / 2), DOTW_NT, 0, st>>>(sg.a, sg.zd, (int)sg.n, h->wsPartial, nt);
+    dot_weight_tile_kernel<<<(unsigned)(nt * (nt + 1) / 2), DOTW_NT, 0, st>>>(sg.a, sg.zd, (int)sg.n, h->wsDot, nt);
     CK(cudaGetLastError());
-    dot_weight_sum_kernel<<<(unsigned)((sg.n + 255) / 256), 256, 0, st>>>(h->wsPartial, (int)sg.n, nt, 1.0 / std::sqrt(sg.v), h->ud + sg.off);
+    dot_weight_sum_kernel<<<(unsigned)((sg.n + 255) / 256), 256, 0, st>>>(h->wsDot, (int)sg.n, nt, 1.0 / std::sqrt(sg.v), h->ud + sg.off);
     CK(cudaGetLastError());
     h->last_launches += 2;
   }
   const bool vec = (ldh % 2 == 0) && ((reinterpret_cast<uintptr_t>(H) & 15) == 0);
   void (*kern)(const double*, const double*, long long, long long, int, double*, int) =
       vec ? dot_rows_kernel<true> : dot_rows_kernel<false>;
+  static int cache[2][TD_MAX_DEV];
   int nb = 0;
-  CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kern, DOT_NT, 0));
+  {
+    td_status cs = kernel_config(kern, DOT_NT, 0, 0, h->device, cache[vec ? 1 : 0], &nb);
+    if (cs != TD_OK) return cs;
+  }
   const unsigned grid = (unsigned)std::max<int64_t>(1, std::min<int64_t>((B + 1) / 2, (int64_t)std::max(nb, 1) * h->num_sms));
   kern<<<grid, DOT_NT, 0, st>>>(h->ud, H, ldh, B, (int)h->n_tot, out_dh, 0);
   CK(cudaGetLastError());
   ++h->last_launches;
   h->last_path = TD_PATH_DOT;
   return TD_OK;
+}
+
+// workspace of the staged kernels for every class that may run through them (all classes when the staged variant is forced)
+td_status staged_alloc(td_handle* h, bool all_classes) {
+  for (const ClassInfo& c : h->classes) {
+    if (!all_classes && class_is_fused_shape(c.log2M)) continue;
+    const StagedGeom g = staged_geom(c.log2M);
+    td_status a = grow(h->wsU, h->wsU_elems, 2 * g.uh);
+    if (a == TD_OK) a = grow(h->wsZ, h->wsZ_elems, 2 * g.zh);
+    if (a == TD_OK) a = grow(h->wsPartial, h->wsP_elems, std::max<size_t>(STAGED_PARTIAL_DEFAULT / sizeof(double), (size_t)g.nblk * 2));
+    if (a != TD_OK) return a;
+  }
+  return TD_OK;
+}
+
+// Dry pass over every kernel the handle's size classes can reach, in all three modes: sets the shared-memory attributes
+// and caches the occupancy figures (kernel_config), launches nothing.
+template <int MODE> td_status warm_mode(td_handle* h) {
+  FusedParams P = {};
+  P.B = 1;
+  for (const ClassInfo& cls : h->classes) {
+    if (!class_is_fused_shape(cls.log2M)) continue;
+    td_status s = launch_fused<MODE>(h, cls.log2M, P, cls.d_Gp, nullptr, true);
+    if (s != TD_OK) return s;
+  }
+  if (!h->dense.all.empty()) {
+    td_status s = launch_dense<MODE>(h, h->dense.all, nullptr, nullptr, 0, 1, nullptr, nullptr, 0, nullptr, true);
+    if (s != TD_OK) return s;
+  } else if (!h->dense.aut.empty()) {
+    td_status s = launch_dense<MODE>(h, h->dense.aut, nullptr, nullptr, 0, 1, nullptr, nullptr, 0, nullptr, true);
+    if (s != TD_OK) return s;
+  }
+  return TD_OK;
+}
+td_status warm_kernels(td_handle* h) {
+  td_status s = warm_mode<MODE_LOGLIKE>(h);
+  if (s == TD_OK) s = warm_mode<MODE_INNER>(h);
+  if (s == TD_OK) s = warm_mode<MODE_STOREZ>(h);
+  if (s == TD_OK) s = launch_block<true>(h->device, nullptr, 0, 0, nullptr, 0, nullptr, true);
+  if (s == TD_OK) s = launch_block<false>(h->device, nullptr, 0, 0, nullptr, 0, nullptr, true);
+  return s;
 }
 
 }  // namespace
@@ -547,6 +680,7 @@ static td_status create_impl(td_handle* h, const double* acf, const int64_t* seg
   cudaDeviceProp prop;
   CK(cudaGetDeviceProperties(&prop, h->device));
   h->num_sms = prop.multiProcessorCount;
+  h->smem_optin = prop.sharedMemPerBlockOptin;
   h->n_seg = n_seg;
   h->segs.resize(n_seg);
   int64_t off = 0;
@@ -629,9 +763,10 @@ static td_status create_impl(td_handle* h, const double* acf, const int64_t* seg
     for (int id : c.seg_ids) {
       SegHost& sg = h->segs[id];
       if (cudaMalloc(&sg.G, sizeof(cplx) * n2) != cudaSuccess) { st = TD_ENOMEM; break; }
+      if (cudaMalloc(&sg.zd, sizeof(cplx) * M) != cudaSuccess) { st = TD_ENOMEM; break; }  // z of the data vector (td_inner_batch)
       gen_pack_kernel<<<(n2 + 255) / 256, 256>>>(sg.a, sg.n, F, n2);
       int launches = 0;
-      st = staged_forward(F, 1, n2, 0, c.T, n2, 0, &launches);
+      st = staged_forward(h->device, F, 1, n2, 0, c.T, n2, 0, &launches);
       if (st != TD_OK) break;
       const double gscale = 0.5 / ((double)n2 * std::sqrt(sg.v));
       gen_permute_kernel<<<(n2 + 255) / 256, 256>>>(F, sg.G, M, gscale, 0);
@@ -650,7 +785,7 @@ static td_status create_impl(td_handle* h, const double* acf, const int64_t* seg
     std::vector<SegDev> sd(c.seg_ids.size());
     for (size_t i = 0; i < sd.size(); ++i) {
       const SegHost& sg = h->segs[c.seg_ids[i]];
-      sd[i].off = sg.off; sd[i].n = sg.n; sd[i]._pad = 0; sd[i].G = sg.G; sd[i].zd = nullptr;
+      sd[i].off = sg.off; sd[i].n = sg.n; sd[i]._pad = 0; sd[i].G = sg.G; sd[i].zd = sg.zd;
     }
     CK(cudaMalloc(&c.d_segs, sizeof(SegDev) * sd.size()));
     CK(cudaMemcpy(c.d_segs, sd.data(), sizeof(SegDev) * sd.size(), cudaMemcpyHostToDevice));
@@ -663,7 +798,38 @@ static td_status create_impl(td_handle* h, const double* acf, const int64_t* seg
   }
   // ---- dense path tables (the chooser's crossover is measured: DESIGN.md 6.4)
   h->dense.auto_n = DENSE_AUTO_N;
-  return dense_upload(h);
+  td_status ds = dense_upload(h);
+  if (ds != TD_OK) return ds;
+  // ---- everything a batch call would otherwise create on first use: streams, events, scratch that does not grow with B
+  CK(cudaStreamCreateWithFlags(&h->aux_stream, cudaStreamNonBlocking));
+  CK(cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking));
+  CK(cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming));
+  CK(cudaEventCreateWithFlags(&h->ev_join, cudaEventDisableTiming));
+  CK(cudaEventCreateWithFlags(&h->ev_last, cudaEventDisableTiming));
+  for (int i = 0; i < 2; ++i) {
+    CK(cudaEventCreateWithFlags(&h->ev_copied[i], cudaEventDisableTiming));
+    CK(cudaEventCreateWithFlags(&h->ev_done[i], cudaEventDisableTiming));
+  }
+  CK(cudaMalloc(&h->ud, sizeof(double) * (size_t)h->n_tot));
+  if (h->max_n <= DOT_MAX_N) {  // per-tile partial weights of the longest segment: ntile rows of ntile * 128 doubles
+    size_t need = 0;
+    for (const SegHost& sg : h->segs) { const size_t nt = (sg.n + DOTW_NT - 1) / DOTW_NT; need = std::max(need, nt * nt * DOTW_NT); }
+    CK(cudaMalloc(&h->wsDot, sizeof(double) * need));
+  }
+  {
+    std::vector<SynSeg> hs(n_seg);
+    for (int s = 0; s < n_seg; ++s) { hs[s].off = h->segs[s].off; hs[s].n = (int)h->segs[s].n; hs[s]._pad = 0; }
+    CK(cudaMalloc(&h->synSeg, sizeof(SynSeg) * n_seg));
+    CK(cudaMemcpy(h->synSeg, hs.data(), sizeof(SynSeg) * n_seg, cudaMemcpyHostToDevice));
+  }
+  // staged classes: both lanes of the L2-resident workspace, partial sums for a default batch (td_reserve grows them)
+  {
+    td_status a = staged_alloc(h, false);
+    if (a != TD_OK) return a;
+  }
+  // ---- one dry pass over every kernel this handle can launch: shared-memory attributes and occupancy are cached now,
+  // so that a batch call is launches only (and can be captured into a CUDA graph)
+  return warm_kernels(h);
 }
 
 td_status td_create(const double* acf, const int64_t* seg_lengths, int n_seg, int device, td_handle** out) {
@@ -702,8 +868,58 @@ td_status td_loglike_batch(td_handle* h, const double* d, const double* H, int64
   if (!d || !H || !out || ldh < h->n_tot) return TD_EINVAL;
   DevGuard guard(h->device);
   if (!guard.ok) return TD_ECUDA;
+  cudaStream_t st = (cudaStream_t)stream;
   h->last_launches = 0;
-  return run_batch<MODE_LOGLIKE>(h, d, H, ldh, B, out, nullptr, (cudaStream_t)stream);
+  td_status s = order_begin(h, st);
+  if (s != TD_OK) return s;
+  s = run_batch<MODE_LOGLIKE>(h, d, H, ldh, B, out, nullptr, st);
+  const td_status e = order_end(h, st);
+  return s != TD_OK ? s : e;
+}
+
+// rows per chunk of the host entry point: ~32 MiB of template data, at least one row
+static int64_t host_chunk_rows(const td_handle* h, int64_t B) {
+  return std::max<int64_t>(1, std::min<int64_t>(B, (32ll << 20) / (8 * h->n_tot)));
+}
+// rows per chunk of the synthesis panel: a whole number of waves of the persistent kernels, about 128 MB (measured on
+// c2 / c3 / c5: 64 MB chunks, which stay in L2, give 11.1-11.9 / 1.47 / 1.61 M evals/s end to end, 136 MB chunks
+// 12.2 / 1.51 / 1.64: fewer launches and tails outweigh the panel's trip through HBM, which the ALU-bound kernels hide)
+static int64_t family_chunk_rows(const td_handle* h, int64_t B, int64_t ldh) {
+  int64_t CH = std::max<int64_t>(1, (136ll << 20) / (8 * ldh));
+  if (CH > h->num_sms) CH -= CH % h->num_sms;
+  return std::min<int64_t>(CH, B);
+}
+// section offsets of the packed device buffer of td_loglike_family_batch_host, each rounded up to an even element count so
+// that d (and out) start on a 16-byte boundary whatever the parity of 5 n_seg B (the TMA-staged first pass needs it)
+static size_t even_up(size_t x) { return (x + 1) & ~(size_t)1; }
+
+td_status td_reserve(td_handle* h, int64_t B_max) {
+  if (!h || B_max < 0) return TD_EINVAL;
+  if (B_max == 0) return TD_OK;
+  DevGuard guard(h->device);
+  if (!guard.ok) return TD_ECUDA;
+  const int64_t n = h->n_tot, ldh = (n + 1) & ~1ll;
+  // staged classes: per-block partial sums for B_max templates (bounded: larger batches run in sub-batches)
+  for (const ClassInfo& c : h->classes) {
+    if (class_is_fused(h, c)) continue;
+    const StagedGeom g = staged_geom(c.log2M);
+    const size_t want = std::min<size_t>((size_t)B_max * g.nblk * 2, std::max<size_t>(STAGED_PARTIAL_MAX / sizeof(double), (size_t)g.nblk * 2));
+    td_status a = grow(h->wsPartial, h->wsP_elems, want);
+    if (a != TD_OK) return a;
+  }
+  // host entry points: staging of H, d and out; parameter entry points: the synthesis panel and the packed parameter buffer
+  const int64_t CH = host_chunk_rows(h, B_max);
+  if ((size_t)(CH * n) > h->hsH_elems) {
+    for (int i = 0; i < 2; ++i) { cudaFree(h->hsH[i]); h->hsH[i] = nullptr; }
+    h->hsH_elems = 0;
+    for (int i = 0; i < 2; ++i) CK(cudaMalloc(&h->hsH[i], sizeof(double) * CH * n));
+    h->hsH_elems = (size_t)(CH * n);
+  }
+  if (!h->hsD) CK(cudaMalloc(&h->hsD, sizeof(double) * n));
+  td_status a = grow(h->hsOut, h->hsOut_elems, (size_t)B_max);
+  if (a == TD_OK) a = grow(h->synH, h->synH_elems, (size_t)(family_chunk_rows(h, B_max, ldh) * ldh));
+  if (a == TD_OK) a = grow(h->synP, h->synP_elems, even_up((size_t)(5ll * h->n_seg * B_max)) + even_up((size_t)n) + (size_t)B_max);
+  return a;
 }
 
 td_status td_loglike_batch_host(td_handle* h, const double* d, const double* H, int64_t ldh, int64_t B, double* out,
@@ -715,74 +931,50 @@ td_status td_loglike_batch_host(td_handle* h, const double* d, const double* H, 
   if (!guard.ok) return TD_ECUDA;
   cudaStream_t st = (cudaStream_t)stream;
   const int64_t n = h->n_tot;
-  // rows per chunk: ~32 MiB of template data, at least one row
-  const int64_t CH = std::max<int64_t>(1, std::min<int64_t>(B, (32ll << 20) / (8 * n)));
-  if (!h->copy_stream) {
-    CK(cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking));
-    for (int i = 0; i < 2; ++i) {
-      CK(cudaEventCreateWithFlags(&h->ev_copied[i], cudaEventDisableTiming));
-      CK(cudaEventCreateWithFlags(&h->ev_done[i], cudaEventDisableTiming));
-    }
-    CK(cudaMalloc(&h->hsD, sizeof(double) * n));
+  const int64_t CH = host_chunk_rows(h, B);
+  if ((size_t)(CH * n) > h->hsH_elems || (size_t)B > h->hsOut_elems || !h->hsD) {  // not reserved: grow now
+    td_status a = td_reserve(h, B);
+    if (a != TD_OK) return a;
   }
-  if ((size_t)(CH * n) > h->hsH_elems) {
-    for (int i = 0; i < 2; ++i) { cudaFree(h->hsH[i]); h->hsH[i] = nullptr; }
-    h->hsH_elems = 0;
-    for (int i = 0; i < 2; ++i) CK(cudaMalloc(&h->hsH[i], sizeof(double) * CH * n));
-    h->hsH_elems = (size_t)(CH * n);
-  }
-  if ((size_t)B > h->hsOut_elems) {
-    cudaFree(h->hsOut); h->hsOut = nullptr; h->hsOut_elems = 0;
-    CK(cudaMalloc(&h->hsOut, sizeof(double) * B));
-    h->hsOut_elems = (size_t)B;
-  }
-  CK(cudaMemcpyAsync(h->hsD, d, sizeof(double) * n, cudaMemcpyHostToDevice, st));
+  h->touched = false;
+  td_status s = order_begin(h, st);
+  if (s != TD_OK) return s;
+  cudaError_t ce = cudaMemcpyAsync(h->hsD, d, sizeof(double) * n, cudaMemcpyHostToDevice, st);
   int launches = 0, k = 0;
-  for (int64_t b0 = 0; b0 < B; b0 += CH, ++k) {
+  for (int64_t b0 = 0; b0 < B && ce == cudaSuccess && s == TD_OK; b0 += CH, ++k) {
     const int buf = k & 1;
     const int64_t cb = std::min<int64_t>(CH, B - b0);
-    if (k >= 2) CK(cudaStreamWaitEvent(h->copy_stream, h->ev_done[buf], 0));  // staging buffer free again
-    CK(cudaMemcpy2DAsync(h->hsH[buf], sizeof(double) * n, H + b0 * ldh, sizeof(double) * ldh, sizeof(double) * n,
-                         (size_t)cb, cudaMemcpyHostToDevice, h->copy_stream));
-    CK(cudaEventRecord(h->ev_copied[buf], h->copy_stream));
-    CK(cudaStreamWaitEvent(st, h->ev_copied[buf], 0));
-    td_status s = td_loglike_batch(h, h->hsD, h->hsH[buf], n, cb, h->hsOut + b0, st);
-    if (s != TD_OK) return s;
+    if (k >= 2) ce = cudaStreamWaitEvent(h->copy_stream, h->ev_done[buf], 0);  // staging buffer free again
+    if (ce == cudaSuccess)
+      ce = cudaMemcpy2DAsync(h->hsH[buf], sizeof(double) * n, H + b0 * ldh, sizeof(double) * ldh, sizeof(double) * n,
+                             (size_t)cb, cudaMemcpyHostToDevice, h->copy_stream);
+    if (ce == cudaSuccess) ce = cudaEventRecord(h->ev_copied[buf], h->copy_stream);
+    if (ce == cudaSuccess) ce = cudaStreamWaitEvent(st, h->ev_copied[buf], 0);
+    if (ce != cudaSuccess) break;
+    h->last_launches = 0;
+    s = run_batch<MODE_LOGLIKE>(h, h->hsD, h->hsH[buf], n, cb, h->hsOut + b0, nullptr, st);
     launches += h->last_launches;
-    CK(cudaEventRecord(h->ev_done[buf], st));
+    if (s == TD_OK) ce = cudaEventRecord(h->ev_done[buf], st);
   }
   h->last_launches = launches;
-  CK(cudaMemcpyAsync(out, h->hsOut, sizeof(double) * B, cudaMemcpyDeviceToHost, st));
-  CK(cudaStreamSynchronize(st));
+  if (ce == cudaSuccess && s == TD_OK) ce = cudaMemcpyAsync(out, h->hsOut, sizeof(double) * B, cudaMemcpyDeviceToHost, st);
+  // on every path, also after an error: no copy that touches the caller's H / out is left in flight
+  const cudaError_t c1 = cudaStreamSynchronize(h->copy_stream), c2 = cudaStreamSynchronize(st);
+  h->last_valid = false;  // both streams are idle: nothing to order against
+  if (s != TD_OK) return s;
+  if (ce != cudaSuccess || c1 != cudaSuccess || c2 != cudaSuccess) return TD_ECUDA;
   return TD_OK;
 }
 
-td_status td_loglike_family_batch(td_handle* h, const double* d, int family, const double* params, int64_t B, double fs,
-                                  double* out, void* stream) {
-  if (!h || B < 0 || family < 0 || family >= SYN_NFAM) return TD_EINVAL;
-  if (B == 0) return TD_OK;
-  if (!d || !params || !out || !(fs > 0.0)) return TD_EINVAL;
-  DevGuard guard(h->device);
-  if (!guard.ok) return TD_ECUDA;
-  cudaStream_t st = (cudaStream_t)stream;
+static td_status family_batch_impl(td_handle* h, const double* d, int family, const double* params, int64_t B, double fs,
+                                   double* out, cudaStream_t st) {
   const int64_t n = h->n_tot, ldh = (n + 1) & ~1ll;  // even leading dimension: 16-byte aligned rows
-  if (!h->synSeg) {
-    std::vector<SynSeg> hs(h->n_seg);
-    for (int s = 0; s < h->n_seg; ++s) { hs[s].off = h->segs[s].off; hs[s].n = (int)h->segs[s].n; hs[s]._pad = 0; }
-    CK(cudaMalloc(&h->synSeg, sizeof(SynSeg) * h->n_seg));
-    CK(cudaMemcpy(h->synSeg, hs.data(), sizeof(SynSeg) * h->n_seg, cudaMemcpyHostToDevice));
+  const int64_t CH = family_chunk_rows(h, B, ldh);
+  {
+    td_status a = grow(h->synH, h->synH_elems, (size_t)(CH * ldh));  // no-op after td_reserve / the first call
+    if (a != TD_OK) return a;
   }
-  // chunk: a whole number of waves of the persistent kernels, about 128 MB (measured on c2 / c3 / c5: 64 MB chunks, which stay
-  // in L2, give 11.1-11.9 / 1.47 / 1.61 M evals/s end to end, 136 MB chunks 12.2 / 1.51 / 1.64: fewer launches and tails
-  // outweigh the panel's trip through HBM, which the ALU-bound kernels hide)
-  int64_t CH = std::max<int64_t>(1, (136ll << 20) / (8 * ldh));
-  if (CH > h->num_sms) CH -= CH % h->num_sms;
-  CH = std::min<int64_t>(CH, B);
-  if ((size_t)(CH * ldh) > h->synH_elems) {
-    cudaFree(h->synH); h->synH = nullptr; h->synH_elems = 0;
-    CK(cudaMalloc(&h->synH, sizeof(double) * CH * ldh));
-    h->synH_elems = (size_t)(CH * ldh);
-  }
+  h->touched = true;
   int launches = 0;
   for (int64_t b0 = 0; b0 < B; b0 += CH) {
     const int64_t cb = std::min<int64_t>(CH, B - b0);
@@ -800,39 +992,46 @@ td_status td_loglike_family_batch(td_handle* h, const double* d, int family, con
   return TD_OK;
 }
 
-td_status td_loglike_ringdown_batch(td_handle* h, const double* d, const double* params, int64_t B, double fs,
-                                    double* out, void* stream) {
-  return td_loglike_family_batch(h, d, SYN_RINGDOWN, params, B, fs, out, stream);
-}
-
-td_status td_loglike_ringdown_batch_host(td_handle* h, const double* d, const double* params, int64_t B, double fs,
-                                         double* out, void* stream) {
-  return td_loglike_family_batch_host(h, d, SYN_RINGDOWN, params, B, fs, out, stream);
+td_status td_loglike_family_batch(td_handle* h, const double* d, int family, const double* params, int64_t B, double fs,
+                                  double* out, void* stream) {
+  if (!h || B < 0 || family < 0 || family >= SYN_NFAM) return TD_EINVAL;
+  if (B == 0) return TD_OK;
+  if (!d || !params || !out || !(fs > 0.0)) return TD_EINVAL;
+  DevGuard guard(h->device);
+  if (!guard.ok) return TD_ECUDA;
+  cudaStream_t st = (cudaStream_t)stream;
+  td_status s = order_begin(h, st);
+  if (s != TD_OK) return s;
+  s = family_batch_impl(h, d, family, params, B, fs, out, st);
+  const td_status e = order_end(h, st);
+  return s != TD_OK ? s : e;
 }
 
 td_status td_loglike_family_batch_host(td_handle* h, const double* d, int family, const double* params, int64_t B,
                                        double fs, double* out, void* stream) {
   if (!h || B < 0 || family < 0 || family >= SYN_NFAM) return TD_EINVAL;
   if (B == 0) return TD_OK;
-  if (!d || !params || !out) return TD_EINVAL;
+  if (!d || !params || !out || !(fs > 0.0)) return TD_EINVAL;
   DevGuard guard(h->device);
   if (!guard.ok) return TD_ECUDA;
   cudaStream_t st = (cudaStream_t)stream;
   const int64_t n = h->n_tot, np5 = 5ll * h->n_seg * B;
-  const size_t need = (size_t)(np5 + n + B);  // parameters, data vector, results
-  if (need > h->synP_elems) {
-    cudaFree(h->synP); h->synP = nullptr; h->synP_elems = 0;
-    CK(cudaMalloc(&h->synP, sizeof(double) * need));
-    h->synP_elems = need;
+  const size_t offD = even_up((size_t)np5), offO = offD + even_up((size_t)n);  // parameters | data vector | results
+  {
+    td_status a = grow(h->synP, h->synP_elems, offO + (size_t)B);  // no-op after td_reserve
+    if (a != TD_OK) return a;
   }
-  double* dP = h->synP; double* dD = dP + np5; double* dO = dD + n;
-  CK(cudaMemcpyAsync(dP, params, sizeof(double) * np5, cudaMemcpyHostToDevice, st));
-  CK(cudaMemcpyAsync(dD, d, sizeof(double) * n, cudaMemcpyHostToDevice, st));
-  td_status s = td_loglike_family_batch(h, dD, family, dP, B, fs, dO, stream);
+  td_status s = order_begin(h, st);
   if (s != TD_OK) return s;
-  CK(cudaMemcpyAsync(out, dO, sizeof(double) * B, cudaMemcpyDeviceToHost, st));
-  CK(cudaStreamSynchronize(st));
-  return TD_OK;
+  double* dP = h->synP; double* dD = dP + offD; double* dO = dP + offO;
+  cudaError_t ce = cudaMemcpyAsync(dP, params, sizeof(double) * np5, cudaMemcpyHostToDevice, st);
+  if (ce == cudaSuccess) ce = cudaMemcpyAsync(dD, d, sizeof(double) * n, cudaMemcpyHostToDevice, st);
+  if (ce == cudaSuccess) s = family_batch_impl(h, dD, family, dP, B, fs, dO, st);
+  if (ce == cudaSuccess && s == TD_OK) ce = cudaMemcpyAsync(out, dO, sizeof(double) * B, cudaMemcpyDeviceToHost, st);
+  const cudaError_t c2 = cudaStreamSynchronize(st);  // on every path: no copy touching the caller's buffers stays in flight
+  h->last_valid = false;
+  if (s != TD_OK) return s;
+  return (ce != cudaSuccess || c2 != cudaSuccess) ? TD_ECUDA : TD_OK;
 }
 
 td_status td_inner_batch(td_handle* h, const double* d, const double* H, int64_t ldh, int64_t B, double* out_dh,
@@ -844,31 +1043,20 @@ td_status td_inner_batch(td_handle* h, const double* d, const double* H, int64_t
   if (!guard.ok) return TD_ECUDA;
   cudaStream_t st = (cudaStream_t)stream;
   h->last_launches = 0;
-  // z of the data vector, once per call (per segment), then the bilinear sums against it
-  for (ClassInfo& c : h->classes) {
-    bool fresh = false;
-    for (int id : c.seg_ids) {
-      SegHost& sg = h->segs[id];
-      if (!sg.zd) { CK(cudaMalloc(&sg.zd, sizeof(cplx) << c.log2M)); fresh = true; }
-    }
-    if (fresh) {
-      std::vector<SegDev> sd(c.seg_ids.size());
-      for (size_t i = 0; i < sd.size(); ++i) {
-        const SegHost& sg = h->segs[c.seg_ids[i]];
-        sd[i].off = sg.off; sd[i].n = sg.n; sd[i]._pad = 0; sd[i].G = sg.G; sd[i].zd = sg.zd;
-      }
-      CK(cudaMemcpyAsync(c.d_segs, sd.data(), sizeof(SegDev) * sd.size(), cudaMemcpyHostToDevice, st));
-      CK(cudaStreamSynchronize(st));  // sd is a host temporary (first td_inner_batch call only)
-      td_status su = dense_upload(h);
-      if (su != TD_OK) return su;
-    }
-  }
-  td_status s = run_fft_path<MODE_STOREZ>(h, d, nullptr, h->n_tot, 1, nullptr, nullptr, st);
+  td_status s = order_begin(h, st);
   if (s != TD_OK) return s;
-  // only the cross term is wanted: one streaming pass over H against the cached weights u = C^{-1} d
-  if (out_dh && !out_hh && h->path == TD_PATH_AUTO && h->max_n <= DOT_MAX_N && h->n_tot <= 0x7fffffff)
-    return run_dot(h, H, ldh, B, out_dh, st);
-  return run_batch<MODE_INNER>(h, d, H, ldh, B, out_dh, out_hh, st);
+  h->touched = true;  // z of the data vector (and u on the dot path) live in the handle
+  // z of the data vector, once per call (per segment), then the bilinear sums against it
+  s = run_fft_path<MODE_STOREZ>(h, d, nullptr, h->n_tot, 1, nullptr, nullptr, st);
+  if (s == TD_OK) {
+    // only the cross term is wanted: one streaming pass over H against the cached weights u = C^{-1} d
+    if (out_dh && !out_hh && h->path == TD_PATH_AUTO && h->max_n <= DOT_MAX_N && h->n_tot <= 0x7fffffff)
+      s = run_dot(h, H, ldh, B, out_dh, st);
+    else
+      s = run_batch<MODE_INNER>(h, d, H, ldh, B, out_dh, out_hh, st);
+  }
+  const td_status e = order_end(h, st);
+  return s != TD_OK ? s : e;
 }
 
 td_status td_set_path(td_handle* h, int path) {
@@ -880,6 +1068,12 @@ td_status td_set_path(td_handle* h, int path) {
 
 td_status td_set_fft_variant(td_handle* h, int variant) {
   if (!h || variant < 0 || variant > 2) return TD_EINVAL;
+  if (variant == 2) {
+    DevGuard guard(h->device);
+    if (!guard.ok) return TD_ECUDA;
+    td_status a = staged_alloc(h, true);
+    if (a != TD_OK) return a;
+  }
   h->fft_variant = variant;
   return TD_OK;
 }
@@ -902,76 +1096,6 @@ td_status td_get_generator(const td_handle* h, int seg, double* a) {
   if (!guard.ok) return TD_ECUDA;
   CK(cudaMemcpy(a, h->segs[seg].a, sizeof(double) * h->segs[seg].n, cudaMemcpyDeviceToHost));
   return TD_OK;
-}
-
-td_status td_probe_fp64(int kind, int device, double* tflops) {
-  if (kind < 0 || kind > 3 || !tflops) return TD_EINVAL;
-  int ndev = 0;
-  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return TD_ECUDA;
-  if (device < 0 || device >= ndev) return TD_EINVAL;
-  DevGuard guard(device);
-  if (!guard.ok) return TD_ECUDA;
-  cudaDeviceProp prop;
-  CK(cudaGetDeviceProperties(&prop, device));
-  const int grid = prop.multiProcessorCount * 8, iters = 200;
-  double* sink = nullptr;
-  CK(cudaMalloc(&sink, sizeof(double)));
-  cudaEvent_t e0 = nullptr, e1 = nullptr;
-  cudaEventCreate(&e0); cudaEventCreate(&e1);
-  float best = 1e30f;
-  td_status rc = TD_OK;
-  for (int rep = 0; rep < 6 && rc == TD_OK; ++rep) {
-    cudaEventRecord(e0, 0);
-    switch (kind) {
-      case 0: probe_kernel<0><<<grid, PROBE_NT>>>(sink, iters, 1.0 + rep); break;
-      case 1: probe_kernel<1><<<grid, PROBE_NT>>>(sink, iters, 1.0 + rep); break;
-      case 2: probe_kernel<2><<<grid, PROBE_NT>>>(sink, iters, 1.0 + rep); break;
-      default: probe_kernel<3><<<grid, PROBE_NT>>>(sink, iters, 1.0 + rep); break;
-    }
-    cudaEventRecord(e1, 0);
-    if (cudaEventSynchronize(e1) != cudaSuccess || cudaGetLastError() != cudaSuccess) { rc = TD_ECUDA; break; }
-    float ms = 0.f;
-    cudaEventElapsedTime(&ms, e0, e1);
-    if (rep > 0 && ms < best) best = ms;  // first launch is the warm-up
-  }
-  cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(sink);
-  if (rc != TD_OK) return rc;
-  *tflops = probe_flops(kind, grid, iters) / (best * 1e-3) / 1e12;
-  return TD_OK;
-}
-
-td_status td_probe_phase(int threads, int groups, int device, double* cycles) {
-  if (!cycles) return TD_EINVAL;
-  int ndev = 0;
-  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return TD_ECUDA;
-  if (device < 0 || device >= ndev) return TD_EINVAL;
-  void (*kern)(double*, long long*, int, const cplx*) = nullptr;
-  if (threads == 256 && groups == 1) kern = probe_phase_kernel<256, 1>;
-  else if (threads == 256 && groups == 2) kern = probe_phase_kernel<256, 2>;
-  else if (threads == 256 && groups == 8) kern = probe_phase_kernel<256, 8>;
-  else if (threads == 512 && groups == 1) kern = probe_phase_kernel<512, 1>;
-  else if (threads == 512 && groups == 2) kern = probe_phase_kernel<512, 2>;
-  else if (threads == 512 && groups == 16) kern = probe_phase_kernel<512, 16>;
-  else return TD_EINVAL;
-  DevGuard guard(device);
-  if (!guard.ok) return TD_ECUDA;
-  const size_t smem = sizeof(cplx) * SmemArr::padded(8192);
-  CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  double* sink = nullptr; long long* cyc = nullptr; cplx* T = nullptr;
-  std::vector<cplx> hT(512);
-  for (int i = 0; i < 512; ++i) hT[i] = mk(std::cos(2.0 * M_PI * i / 8192.0), -std::sin(2.0 * M_PI * i / 8192.0));
-  td_status rc = TD_OK;
-  if (cudaMalloc(&sink, 8) != cudaSuccess || cudaMalloc(&cyc, 8) != cudaSuccess || cudaMalloc(&T, sizeof(cplx) * 512) != cudaSuccess) rc = TD_ENOMEM;
-  long long c = 0;
-  if (rc == TD_OK) {
-    const int iters = 200;
-    cudaMemcpy(T, hT.data(), sizeof(cplx) * 512, cudaMemcpyHostToDevice);
-    for (int rep = 0; rep < 2; ++rep) kern<<<1, threads, smem>>>(sink, cyc, iters, T);
-    if (cudaDeviceSynchronize() != cudaSuccess || cudaGetLastError() != cudaSuccess) rc = TD_ECUDA;
-    else { cudaMemcpy(&c, cyc, 8, cudaMemcpyDeviceToHost); *cycles = (double)c / iters; }
-  }
-  cudaFree(sink); cudaFree(cyc); cudaFree(T);
-  return rc;
 }
 
 int td_last_launches(const td_handle* h) { return h ? h->last_launches : 0; }

@@ -11,10 +11,11 @@ from paper_2603_06010_b200 import build as tdbuild
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 HEADER = os.path.join(ROOT, "include", "tdlike.h")
+PROBE_HEADER = os.path.join(ROOT, "include", "tdprobe.h")
 
 
-def _declared():
-    src = open(HEADER).read()
+def _declared(header=HEADER):
+    src = open(header).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
     return sorted(set(re.findall(r"\b(td_[a-z0-9_]+)\s*\(", src)))
 
@@ -35,6 +36,16 @@ def test_every_declared_symbol_is_exported_and_bound():
     exported = set(re.findall(r"\bT (td_[a-z0-9_]+)\b", nm))
     assert set(names) <= exported, set(names) - exported
     assert set(names) == set(tdb.SYMBOLS), set(names) ^ set(tdb.SYMBOLS)
+
+
+def test_probe_library_is_separate_from_the_product_library():
+    """include/tdprobe.h is served by the bench-only libtdprobe.so; the product library exports no probe."""
+    names = _declared(PROBE_HEADER)
+    assert names == ["td_probe_throughput"]
+    nm = subprocess.run(["nm", "-D", "--defined-only", tdb.PROBE_LIB_PATH], capture_output=True, text=True, check=True).stdout
+    assert set(names) <= set(re.findall(r"\bT (td_[a-z0-9_]+)\b", nm))
+    nm = subprocess.run(["nm", "-D", "--defined-only", tdb.LIB_PATH], capture_output=True, text=True, check=True).stdout
+    assert "probe" not in nm
 
 
 def test_library_is_sm100a_with_no_other_arch():

@@ -345,10 +345,12 @@ def test_auto_chooser_mixes_paths():
     assert np.max(np.abs(hh.cpu().numpy() - hh_ref) / np.abs(hh_ref)) <= TOL
 
 
-def test_probe_fp64_reports_plausible_peaks():
-    dfma = tdb.probe_fp64(0)
-    dmma = tdb.probe_fp64(1)
-    assert 10.0 < dfma < 60.0 and 10.0 < dmma < 90.0
+def test_probe_library_reports_plausible_peaks():
+    """bench.py's roofline denominators come from the bench-only probe library (include/tdprobe.h)."""
+    dfma = tdb.probe_throughput(0)
+    dmma = tdb.probe_throughput(1)
+    ffma = tdb.probe_throughput(4)
+    assert 10.0 < dfma < 60.0 and 10.0 < dmma < 90.0 and 30.0 < ffma < 120.0
 
 
 # ------------------------------------------------------------------ full sizes, in the launch configuration bench.py times
@@ -463,7 +465,7 @@ def test_ringdown_params_entry_errors_and_edges():
     w = W.make("c3", B=4)
     with tdb.TDLikelihood(w.acf, w.seg_lengths) as h:
         with pytest.raises(ValueError):
-            h.loglike_ringdown_batch(_dev(w.d), _dev(np.ones((4, 5))), w.fs)   # three segments need [B, 3, 5]
+            h.loglike_family_batch(_dev(w.d), tdb.TD_FAMILY_RINGDOWN, _dev(np.ones((4, 5))), w.fs)   # three segments need [B, 3, 5]
     w = W.make("c1", B=5)
     p = w.params.copy()
     p[1, 4] = 2.0        # t0 beyond the segment: the template is identically zero -> logL = -1/2 <d,d>
@@ -472,9 +474,9 @@ def test_ringdown_params_entry_errors_and_edges():
     assert np.all(H[1] == 0.0) and H[2, 0] != 0.0
     ref = O.loglike_batch(w.acf, w.seg_lengths, w.d, H)
     with tdb.TDLikelihood(w.acf, w.seg_lengths) as h:
-        out = h.loglike_ringdown_batch(_dev(w.d), _dev(p), w.fs).cpu().numpy()
+        out = h.loglike_family_batch(_dev(w.d), tdb.TD_FAMILY_RINGDOWN, _dev(p), w.fs).cpu().numpy()
         with pytest.raises(tdb.TDError):
-            h.loglike_ringdown_batch(_dev(w.d), _dev(p), 0.0)
+            h.loglike_family_batch(_dev(w.d), tdb.TD_FAMILY_RINGDOWN, _dev(p), 0.0)
         with pytest.raises(tdb.TDError) as e:
             h.loglike_family_batch(_dev(w.d), 7, _dev(p), w.fs)
         assert e.value.status == tdb.TD_EINVAL
@@ -562,15 +564,6 @@ def test_long_segment_five_pass_plan():
     assert np.all(out < 0.0)
 
 
-def test_phase_probe_reports_plausible_cycles_and_rejects_unknown_shapes():
-    lockstep = tdb.probe_phase(256, 1)
-    free = tdb.probe_phase(256, 8)
-    assert 1500.0 < free < lockstep < 8000.0       # floors ~2000 cycles; barrier-free groups overlap better
-    with pytest.raises(tdb.TDError) as e:
-        tdb.probe_phase(384, 3)
-    assert e.value.status == tdb.TD_EINVAL
-
-
 def test_staged_two_lane_pipeline_on_a_side_stream():
     """The staged path alternates chunks between the caller's stream and an internal one (fork / join events).
     On a non-default stream, back to back, with the inputs produced on that same stream just before: results must be
@@ -633,3 +626,76 @@ def test_long_non_spd_acf_is_rejected_by_the_cooperative_setup():
     with pytest.raises(tdb.TDError) as e:
         tdb.TDLikelihood(bad, [20000])
     assert e.value.status == tdb.TD_ENOTSPD
+
+
+# ------------------------------------------------------------------ allocation-free, capturable, stream-safe calls
+@pytest.mark.parametrize("name,B,n_scale", [("c1", 64, 1), ("c3", 48, 1), ("c4", 40, 4), ("d2", 256, 1)])
+def test_calls_capture_into_a_cuda_graph_and_replay(name, B, n_scale):
+    """td_loglike_batch + td_inner_batch enqueue kernels only (no allocation, no synchronisation, every attribute set by
+    td_create): both are captured into ONE CUDA graph on a side stream and replayed on new data in the same buffers."""
+    w = W.make(name, B=B, n_scale=n_scale)
+    with tdb.TDLikelihood(w.acf, w.seg_lengths) as h:
+        d, H = _dev(w.d), _dev(w.H)
+        out = torch.empty(B, dtype=torch.float64, device="cuda")
+        dh = torch.empty(B, dtype=torch.float64, device="cuda")
+        eager = h.loglike_batch(d, H).clone()
+        dh_e, hh_e = h.inner_batch(d, H)
+        torch.cuda.synchronize()
+        side = torch.cuda.Stream()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.stream(side):
+            with torch.cuda.graph(g, stream=side):
+                h.loglike_batch(d, H, out=out, stream=side)
+                h.inner_batch(d, H, want_hh=False, stream=side, out_dh=dh)
+        for rep in range(2):
+            if rep == 1:                         # new templates in the captured buffers
+                H.copy_(torch.flip(H, dims=[0]))
+            out.zero_(); dh.zero_()
+            g.replay()
+            torch.cuda.synchronize()
+            ref = eager if rep == 0 else torch.flip(eager, dims=[0])
+            ref_dh = dh_e if rep == 0 else torch.flip(dh_e, dims=[0])
+            assert torch.equal(out, ref), f"{name}: graph replay {rep} differs from the eager call"
+            scale = float((hh_e.abs() + 1.0).max())
+            assert float((dh - ref_dh).abs().max()) <= 1e-9 * scale * 10
+    ref = O.loglike_batch(w.acf, w.seg_lengths, w.d, w.H) if w.n_tot <= 20000 else None
+    if ref is not None:
+        _assert_close(eager.cpu().numpy(), ref, what=f"{name} eager")
+
+
+@pytest.mark.parametrize("name,B,n_scale", [("c4", 48, 4), ("c5", 32, 2)])
+def test_one_handle_alternating_between_two_streams(name, B, n_scale):
+    """the handle owns scratch (staged workspace, z / u of the data vector).  One host thread issuing calls on
+    two different streams must get the results of serial execution: a call on another stream than the previous
+    scratch-using call waits for it (include/tdlike.h, "Threads and streams")."""
+    w = W.make(name, B=B, n_scale=n_scale)
+    with tdb.TDLikelihood(w.acf, w.seg_lengths) as h:
+        d, H = _dev(w.d), _dev(w.H)
+        H2 = torch.flip(H, dims=[0]).contiguous()
+        ref1 = h.loglike_batch(d, H).clone()
+        dh1, _ = h.inner_batch(d, H, want_hh=False)
+        dh1 = dh1.clone()
+        torch.cuda.synchronize()
+        s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+        for _ in range(3):
+            o1 = h.loglike_batch(d, H, stream=s1)
+            o2 = h.loglike_batch(d, H2, stream=s2)
+            a1, _ = h.inner_batch(d, H, want_hh=False, stream=s1)
+            a2, _ = h.inner_batch(d, H2, want_hh=False, stream=s2)
+            torch.cuda.synchronize()
+            assert torch.equal(o1, ref1) and torch.equal(o2, torch.flip(ref1, dims=[0]))
+            assert torch.equal(a1, dh1) and torch.equal(a2, torch.flip(dh1, dims=[0]))
+
+
+def test_family_host_entry_with_odd_batch_keeps_rows_aligned():
+    """5 n_seg B odd used to leave d 8-byte aligned inside the packed device buffer (TMA staging silently off).
+    The sections are now rounded to 16 bytes; results are bit-identical to the device-pointer call."""
+    for name, B in (("c1", 7), ("c5", 5)):
+        w = W.make(name, B=B, n_scale=1 if name == "c1" else 4)
+        with tdb.TDLikelihood(w.acf, w.seg_lengths) as h:
+            h.reserve(B)
+            out_host = h.loglike_family_batch_host(w.d, w.family, w.params, w.fs)
+            out_dev = h.loglike_family_batch(_dev(w.d), w.family, _dev(w.params), w.fs).cpu().numpy()
+        assert np.array_equal(out_host, out_dev)
+        H = OT.family_rows(w.family, w.params, w.seg_lengths, w.fs)
+        _assert_close(out_host, O.loglike_batch(w.acf, w.seg_lengths, w.d, H), what=f"{name} odd B")
