@@ -2,6 +2,7 @@
 """bench.py - the headline metric of BASELINE.json: fp64 likelihood evaluations / second.
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--config c2] [--impl ours|reference]
+                  [--dtype f64|f32] [--scaling weak|strong]
 
 A "step" is one pass of the whole hot path (residual, forward FFT, generator product, inverse
 FFT, fused quadratic reduction, summed over segments) over one batch of B synthetic templates
@@ -34,6 +35,8 @@ UNIT = "evals/s"
 # clocks.max.sm); the register-loop DFMA / DMMA throughputs are measured in every run
 # (libtdprobe.so, include/tdprobe.h) and reported beside it.  DESIGN.md 6.
 FP64_PEAK_TFLOPS = 37.2
+# fp32 evaluation mode (--dtype f32, never the headline): 128 FFMA/clk/SM x 148 SMs x 1.965 GHz x 2 flop
+FP32_PEAK_TFLOPS = 74.4
 # dominant kernel of a step, per config
 DOMINANT = {"c1": "td_fused4_kernel<10>", "c2": "td_fused4_kernel<12>", "c3": "td_cluster_kernel",
             "c4": "staged lg_* kernels", "c5": "td_cluster_kernel"}
@@ -141,10 +144,11 @@ def run_reference(args):
             rates.append(r)
     val = float(np.mean(rates))
     line = {"metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": 1e3 * nb / val, "higher_is_better": True, "scaling": "weak",
+            "warmup": args.warmup, "ms_per_step": 1e3 * nb / val, "higher_is_better": True, "scaling": args.scaling,
             "vs_baseline": None, "dtype": "f64", "data": "synthetic", "impl": "reference",
             "config": {"workload": f"{args.config}: bounded sample, each step = {sample}"},
-            "cpu_baseline": {"value": val, "unit": UNIT, "cores": th, "kind": "oracle", "sample": sample},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": th, "host_cpu_count": os.cpu_count(), "kind": "oracle",
+                             "sample": sample},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line))
@@ -162,6 +166,12 @@ def main():
     ap.add_argument("--fft-variant", type=int, default=0)
     ap.add_argument("--op", default="loglike", choices=["loglike", "dh"],
                     help="loglike: the headline hot path; dh: only the cross term <d|h_b> (td_inner_batch, out_hh = NULL)")
+    ap.add_argument("--dtype", default="f64", choices=["f64", "f32"],
+                    help="f64: the headline; f32: fp32 evaluation with fp64 setup (td_set_precision, PAPER.md:322-324) - "
+                         "a second line with its own fp32-FMA roofline, never the headline")
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
+                    help="--gpus N > 1: weak = every rank its own batch of B (default); strong = ONE batch of B sharded "
+                         "over the ranks with shard.row_slice (no data-path collective either way)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--probe-peaks", action="store_true",
@@ -194,7 +204,16 @@ def main():
         return
 
     w = W.make(args.config, B=args.B)
-    B, n_tot = w.B, w.n_tot
+    B_job, n_tot = w.B, w.n_tot
+    lo, hi = 0, B_job
+    if world > 1 and args.scaling == "strong":
+        from paper_2603_06010_b200 import shard
+        lo, hi = shard.row_slice(B_job, rank, world)     # this rank's rows of the ONE batch
+        w.H = w.H[lo:hi]
+        if w.params is not None:
+            w.params = w.params[lo:hi]
+    B = hi - lo                                          # templates this rank evaluates per step
+    units_per_step = B_job if (world > 1 and args.scaling == "strong") else world * B
     t_setup = time.perf_counter()
     h = tdb.TDLikelihood(w.acf, w.seg_lengths, device=local)   # S0: Levinson-Durbin + generator spectra, once per handle
     t_setup = time.perf_counter() - t_setup
@@ -202,10 +221,12 @@ def main():
         h.set_path(args.path)
     if args.fft_variant:
         h.set_fft_variant(args.fft_variant)
+    if args.dtype == "f32":
+        h.set_precision(tdb.TD_PREC_F32)
     d = torch.as_tensor(w.d).to(dev)
     H_host = torch.as_tensor(w.H).pin_memory()
     # >= 3 distinct device copies of H, rotated, so no step is served from the 126 MB L2
-    nbuf = max(3, int(math.ceil(3 * 126e6 / (8.0 * B * n_tot))))
+    nbuf = max(3, int(math.ceil(3 * 126e6 / (8.0 * max(B, 1) * n_tot))))
     nbuf = min(nbuf, 64)
     Hs = [H_host.to(dev, non_blocking=True) for _ in range(nbuf)]
     out = torch.empty(B, dtype=torch.float64, device=dev)
@@ -254,7 +275,7 @@ def main():
         t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         total_ms = float(t.item())
-    value = world * B * args.steps / (total_ms * 1e-3)
+    value = units_per_step * args.steps / (total_ms * 1e-3)
 
     # ---------------- end to end: host buffers through the C ABI (H2D of H and d, D2H of out, per step)
     e2e = None
@@ -277,7 +298,7 @@ def main():
             t = torch.tensor([ms], dtype=torch.float64, device=dev)
             dist.all_reduce(t, op=dist.ReduceOp.MAX)
             ms = float(t.item())
-        e2e = {"value": world * B * k_e2e / (ms * 1e-3), "unit": UNIT,
+        e2e = {"value": units_per_step * k_e2e / (ms * 1e-3), "unit": UNIT,
                "h2d_bytes_per_step": int(8 * B * n_tot + 8 * n_tot), "d2h_bytes_per_step": int(8 * B),
                "steps": k_e2e, "api": "td_loglike_batch_host (pinned H, chunked copies overlapped with kernels)"}
         max_dev = float(np.max(np.abs(out_host - out.cpu().numpy())))
@@ -305,7 +326,7 @@ def main():
             t = torch.tensor([ms], dtype=torch.float64, device=dev)
             dist.all_reduce(t, op=dist.ReduceOp.MAX)
             ms = float(t.item())
-        e2e_params = {"value": world * B * k_p / (ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(8 * w.params.size + 8 * n_tot),
+        e2e_params = {"value": units_per_step * k_p / (ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(8 * w.params.size + 8 * n_tot),
                       "d2h_bytes_per_step": int(8 * B), "steps": k_p,
                       "api": f"td_loglike_family_batch_host (host parameters, family {W.FAMILIES[w.family]}; templates synthesised on the device)",
                       "max_rel_diff_vs_device_call": float(np.max(np.abs(out_p - out.cpu().numpy()) / np.maximum(np.abs(out_p), 1.0)))}
@@ -320,23 +341,35 @@ def main():
     kern_ms = float(np.mean(step_ms))
     dense = path_used == 2
     falg = float(sum(2.0 * int(n) * int(n) for n in w.seg_lengths)) if dense else alg_flops_per_eval(w.seg_lengths)
+    f32 = args.dtype == "f32"
     probe = {"dfma": tdb.probe_throughput(0, local), "dmma": tdb.probe_throughput(1, local)}
+    if f32:
+        probe["ffma_fp32"] = tdb.probe_throughput(4, local)
+    peak_tf = FP32_PEAK_TFLOPS if f32 else FP64_PEAK_TFLOPS
     ach_tf = falg * B / (kern_ms * 1e-3) / 1e12
     ach_gbs = (8.0 * n_tot * B + 8.0 * B) / (kern_ms * 1e-3) / 1e9
-    traffic = None
+    traffic, traffic_source = None, None
     tp = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(tp):
+    if os.path.exists(tp) and not f32:
         try:
-            traffic = json.load(open(tp)).get(args.config)
+            tj = json.load(open(tp))
+            traffic = tj.get(args.config)
+            traffic_source = ("a constant from a committed ncu capture, NOT a counter of this run: " +
+                              tj.get("_source", "profiles/traffic.json")) if traffic is not None else None
         except Exception:
             traffic = None
-    roofline = {"bound": "tensor" if dense else "alu", "achieved": ach_tf, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
-                "frac": ach_tf / FP64_PEAK_TFLOPS, "traffic": traffic,
-                "kernel": "td_dense_kernel" if dense else DOMINANT.get(args.config, "td_fused_kernel"),
+    roofline = {"bound": "tensor" if dense else "alu", "achieved": ach_tf, "peak": peak_tf, "unit": "TFLOP/s",
+                "frac": ach_tf / peak_tf,
+                # fraction against the DFMA register loop measured in THIS run (state both denominators)
+                "frac_vs_measured_loop": ach_tf / probe["ffma_fp32" if f32 else "dfma"],
+                "traffic": traffic, "traffic_source": traffic_source,
+                "kernel": "td_dense_kernel" if dense else DOMINANT.get(args.config, "td_fused_kernel") + (" (fp32 build)" if f32 else ""),
                 "measured_register_loop_tflops": probe,
                 "kernel_ms": kern_ms, "alg_flops_per_eval": falg,
-                "peak_source": "derived: 64 DFMA/clk/SM x 148 SM x 1.965 GHz x 2 (DESIGN.md 6); the fp64 tensor pipe "
-                               "(DMMA.8x8x4) has the same peak; register-loop measurements of this run beside it"}
+                "peak_source": ("derived: 128 FFMA/clk/SM x 148 SM x 1.965 GHz x 2; the FFMA register loop of this run beside it"
+                                if f32 else
+                                "derived: 64 DFMA/clk/SM x 148 SM x 1.965 GHz x 2 (DESIGN.md 6); the fp64 tensor pipe "
+                                "(DMMA.8x8x4) has the same peak; register-loop measurements of this run beside it")}
     if args.op == "dh":
         # the cross term is one streaming pass over H: HBM is the bounding roofline; 2 flop per 8 bytes
         roofline = {"bound": "hbm", "achieved": ach_gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s",
@@ -354,13 +387,21 @@ def main():
         budget = {"c1": 64, "c2": 2048, "c3": 256, "c4": 2, "c5": 256}.get(args.config, 256)
         r, tf, th, sample, ref = oracle_rate(w, budget)
         got = out.cpu().numpy()[: len(ref)]
-        cpu = {"value": r, "unit": UNIT, "cores": th, "kind": "oracle", "sample": sample,
+        cpu = {"value": r, "unit": UNIT, "cores": th, "host_cpu_count": os.cpu_count(), "kind": "oracle",
+               "note": "the oracle is the O(N^2)-per-template dense Cholesky route (fp64), not the paper's O(N log N) GSCE "
+                       "route: a ratio against it is a ratio against a deliberately plain program",
+               "sample": sample,
                "max_rel_err_gpu_vs_oracle": float(np.max(np.abs(got - ref) / np.maximum(np.abs(ref), 1.0)))}
 
-    line = {"metric": METRIC if args.op == "loglike" else "fp64 cross-term <d|h_b> evals/sec (not the headline)", "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+    metric = METRIC if args.op == "loglike" else "fp64 cross-term <d|h_b> evals/sec (not the headline)"
+    if f32:
+        metric = "fp32-evaluation likelihood evals/sec (fp64 setup; second line, not the headline)"
+    line = {"metric": metric, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": f"{args.config}: {w.description}; N_tot={n_tot}, segments={list(map(int, w.seg_lengths))}, B={B} per GPU",
+            "scaling": args.scaling, "vs_baseline": None, "dtype": args.dtype, "data": "synthetic",
+            "config": {"workload": f"{args.config}: {w.description}; N_tot={n_tot}, segments={list(map(int, w.seg_lengths))}, "
+                                   + (f"B={B_job} sharded over {world} GPUs (rank 0: {B})" if args.scaling == "strong" and world > 1
+                                      else f"B={B} per GPU"),
                        "path": {1: "fft", 2: "dense", 3: "dot"}.get(path_used, "?"),
                        "l2": f"{nbuf} distinct device copies of H rotated between steps (H = {8 * B * n_tot / 2**20:.0f} MiB each)",
                        "parallelism": f"dp{world} over templates",

@@ -154,6 +154,23 @@ td_status td_set_path(td_handle* h, int path);
  * otherwise), 1 = same as 0, 2 = force the staged kernels for every segment (tests, profiling). */
 td_status td_set_fft_variant(td_handle* h, int variant);
 
+/* td_precision: arithmetic of the FFT-path evaluation (td_set_precision). */
+enum { TD_PREC_F64 = 0, TD_PREC_F32 = 1 };
+
+/* td_set_precision - FP32 evaluation with FP64 setup (III.C.3: "it is possible to carry out all the
+ * analysis with FP32 with appropriate normalization.  However, the necessary matrices and whitening operators should be
+ * precomputed in FP64"; :268).  TD_PREC_F32: the Levinson-Durbin recursion, the generator spectra and the twiddles stay
+ * fp64 (td_create) and are rounded once; per template the residual d - h is formed in fp64 from the fp64 inputs, divided
+ * by sqrt(rho_s(0)) (the normalisation; the spectra carry the inverse factor) and rounded once; S2-S4 (both FFTs, the
+ * generator product) run in fp32; the sums of squares are fp32 per thread and fp64 across threads, segments and in out[].
+ * The interface (double d, H, out) is unchanged.  Serves segments of 513..8192 samples (the fused and cluster kernels);
+ * other size classes of the handle, the dense path and the dot-product cross term keep evaluating in fp64.
+ * Accuracy: |out - exact| <= 2e-5 * max(|exact|, 1) per template (DESIGN.md 6.7 derives it; observed ~1e-6); the fp64
+ * default keeps the 1e-9 bar.  The first call builds the fp32 tables (synchronous, allocates); later calls only switch.
+ * Errors: TD_EINVAL (unknown precision), TD_EUNSUPPORTED (no segment of the handle has an fp32 kernel; the setting is
+ * unchanged), TD_ENOMEM, TD_ECUDA. */
+td_status td_set_precision(td_handle* h, int precision);
+
 /* td_get_info - queries.  Any output pointer may be NULL.
  *   n_tot      sum of segment lengths
  *   n_seg      number of segments

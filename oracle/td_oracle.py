@@ -32,6 +32,9 @@ segments of inner_batch against single-segment calls and the brute-force bilinea
 snrs against the white-noise closed form), Eq. 14 as printed (P12), independent library
 Levinson solve (P13), injection sanity (P14); the chunk loop (B > 1024) and the `factors=`
 branch against the AR(1) closed form row by row (test_p1_p9_large_batch_...).
+Very long segments (N = 2^20: neither the dense Cholesky nor a library Levinson solve finishes in test time): the exact
+Gaussian likelihood of an AR(p) process in closed form (`ar_acf`, `ar_quadform_closed`, O(N p); pin P19 holds it to the
+Cholesky route at small N and to the hand-evaluated AR(1) values of P3).
 Every function below is covered by at least one of them; nothing here is "parity unpinned".
 The template families / projection of the step before the hot path live in oracle/templates.py
 (pins P15-P18).
@@ -300,3 +303,46 @@ def loglike_batch_solve_toeplitz(acf, seg_lengths, d, H) -> np.ndarray:
         Z = sla.solve_toeplitz(acf[lo:hi], R, check_finite=False)
         out += np.sum(R * Z, axis=0)
     return -0.5 * out
+
+
+# ----------------------------------------------------------------------------------------
+# Closed form for very long segments: exact likelihood of a stationary AR(p) process
+# ----------------------------------------------------------------------------------------
+# For x_t = sum_{j=1..p} phi_j x_{t-j} + e_t, e_t ~ N(0, s2) iid, stationary, the joint density factorises as
+# p(x_0..x_{p-1}) * prod_{t>=p} p(x_t | x_{t-1}..x_{t-p}), hence (the textbook exact AR likelihood; it is Eq. 10 of the
+# paper, for a covariance whose Cholesky factor is known in closed form: the rows t >= p of L^{-1} are
+# (.., -phi_p, .., -phi_1, 1)/sqrt(s2))
+#     x^T C^{-1} x = x_{0:p}^T C_p^{-1} x_{0:p} + (1/s2) sum_{t>=p} (x_t - sum_j phi_j x_{t-j})^2 ,
+# with C_p the p x p Toeplitz matrix of the first p autocovariances.  O(N p) work: the one oracle route that reaches
+# N = 2^20 ("N >~ 1e7" is the paper's long-N regime).
+
+
+def ar_acf(phi: Sequence[float], s2: float, n: int) -> np.ndarray:
+    """Autocovariances rho_0..rho_{n-1} of the stationary AR(p) process above: rho_0..rho_p from the Yule-Walker
+    equations rho_k = sum_j phi_j rho_|k-j| + s2 [k = 0] (a (p+1) x (p+1) linear solve), the rest by the recursion."""
+    phi = np.asarray(phi, np.float64)
+    p = phi.size
+    A = np.zeros((p + 1, p + 1))
+    for k in range(p + 1):
+        A[k, k] += 1.0
+        for j in range(1, p + 1):
+            A[k, abs(k - j)] -= phi[j - 1]
+    rhs = np.zeros(p + 1)
+    rhs[0] = s2
+    rho = np.zeros(max(n, p + 1))
+    rho[: p + 1] = np.linalg.solve(A, rhs)
+    for k in range(p + 1, n):
+        rho[k] = np.dot(phi, rho[k - 1 : k - p - 1 : -1])
+    return rho[:n].copy()
+
+
+def ar_quadform_closed(phi: Sequence[float], s2: float, x: np.ndarray) -> float:
+    """x^T C^{-1} x for the AR(p) covariance, by the factorisation above (no N x N object, no recursion over lags)."""
+    phi = np.asarray(phi, np.float64)
+    x = np.asarray(x, np.float64)
+    p = phi.size
+    head = quadform(ar_acf(phi, s2, p), x[:p]) if p > 0 else 0.0
+    e = x[p:].copy()
+    for j in range(1, p + 1):
+        e -= phi[j - 1] * x[p - j : x.size - j]
+    return float(head + np.dot(e, e) / s2)

@@ -18,6 +18,7 @@ LIB_PATH = os.path.join(_HERE, "lib", "libtdlike.so")
 TD_OK, TD_EINVAL, TD_ENOTSPD, TD_ENOMEM, TD_ECUDA, TD_EUNSUPPORTED = range(6)
 TD_PATH_AUTO, TD_PATH_FFT, TD_PATH_DENSE, TD_PATH_DOT = 0, 1, 2, 3
 TD_FAMILY_RINGDOWN, TD_FAMILY_SINE_GAUSSIAN, TD_FAMILY_CHIRP = 0, 1, 2
+TD_PREC_F64, TD_PREC_F32 = 0, 1
 
 # every symbol include/tdlike.h declares: name -> (restype, argtypes)
 _VP, _I64, _INT, _DP = C.c_void_p, C.c_int64, C.c_int, C.POINTER(C.c_double)
@@ -32,6 +33,7 @@ SYMBOLS = {
     "td_reserve": (_INT, [_VP, _I64]),
     "td_set_path": (_INT, [_VP, _INT]),
     "td_set_fft_variant": (_INT, [_VP, _INT]),
+    "td_set_precision": (_INT, [_VP, _INT]),
     "td_get_info": (_INT, [_VP, C.POINTER(C.c_int64), C.POINTER(_INT), _DP, _DP, C.POINTER(_INT)]),
     "td_get_generator": (_INT, [_VP, _INT, _DP]),
     "td_last_launches": (_INT, [_VP]),
@@ -216,6 +218,10 @@ class TDLikelihood:
 
     def set_path(self, path: int):
         _check(self._lib.td_set_path(self._h, int(path)), "td_set_path")
+
+    def set_precision(self, precision: int):
+        """TD_PREC_F64 (default) or TD_PREC_F32: fp32 evaluation with fp64 setup (td_set_precision)."""
+        _check(self._lib.td_set_precision(self._h, int(precision)), "td_set_precision")
 
     def set_fft_variant(self, variant: int):
         _check(self._lib.td_set_fft_variant(self._h, int(variant)), "td_set_fft_variant")

@@ -24,7 +24,7 @@
 #pragma once
 #include "td_fused4.cuh"
 
-namespace td {
+namespace TD_NS {
 
 // ---- cos/sin(2 pi k / 64): the odd branch's output twist w_2M^{-256 t} = conj(w_64)^t -------------
 __host__ __device__ constexpr double cos64q(int k) {  // k in [0, 16]
@@ -59,7 +59,7 @@ template <int K> __device__ __forceinline__ cplx mul_w64_inv(cplx a) {
   else if constexpr (k == 32) return mk(-a.x, -a.y);
   else if constexpr (k == 48) return mk(a.y, -a.x);
   else {
-    constexpr double c = cos64(k), s = sin64(k);
+    constexpr real c = (real)cos64(k), s = (real)sin64(k);
     return mk(fma(a.x, c, -(a.y * s)), fma(a.y, c, a.x * s));
   }
 }
@@ -78,23 +78,39 @@ __device__ __forceinline__ uint32_t map_to_cta(uint32_t smem_addr, uint32_t rank
   return r;
 }
 __device__ __forceinline__ void st_cluster(uint32_t addr, cplx v) {
+#ifdef TD_F32
+  asm volatile("st.shared::cluster.v2.f32 [%0], {%1, %2};" ::"r"(addr), "f"(v.x), "f"(v.y) : "memory");
+#else
   asm volatile("st.shared::cluster.v2.f64 [%0], {%1, %2};" ::"r"(addr), "d"(v.x), "d"(v.y) : "memory");
+#endif
 }
 // asynchronous remote store that also counts its 16 bytes on the destination CTA's mbarrier: the receiver waits on a
 // LOCAL mbarrier for the bytes instead of a cluster-wide barrier round trip
 __device__ __forceinline__ void st_async_cluster(uint32_t addr, cplx v, uint32_t mbar) {
+#ifdef TD_F32
+  asm volatile("st.async.shared::cluster.mbarrier::complete_tx::bytes.v2.f32 [%0], {%1, %2}, [%3];" ::"r"(addr), "f"(v.x),
+               "f"(v.y), "r"(mbar)
+               : "memory");
+#else
   asm volatile("st.async.shared::cluster.mbarrier::complete_tx::bytes.v2.f64 [%0], {%1, %2}, [%3];" ::"r"(addr), "d"(v.x),
                "d"(v.y), "r"(mbar)
                : "memory");
+#endif
 }
 
 struct ClusterShape {
   static constexpr int LOG2M = 13, M = 1 << LOG2M, NF = M / 2, TW = 2 * M;
   static constexpr int RF1 = 16, RI1 = 32, NT = 256, NW = 8;
   static constexpr int TWS = 2 * M / RF1;  // 1024 base twiddles w_2M^k
+  using Cols = F4Cols<16>;                 // TMEM window of a thread (256 columns in both precisions)
+  static constexpr int TMEM_COLS = 2 * Cols::WINDOW;
   static constexpr int PADM = SmemArr::padded(M), PADNF = SmemArr::padded(NF);
+  // the staged template row (<= M doubles) lands in the dead U region in fp64; the fp32 U region (8-byte elements) is too
+  // small for a row of doubles, so the fp32 build has a staging region of its own
+  static constexpr size_t STAGE_BYTES = F32 ? sizeof(double) * M : 0;
   static constexpr size_t smem_bytes() {
-    return sizeof(cplx) * ((size_t)PADNF + (size_t)PADM + TWS) + sizeof(double) * (4 * NW + 2) + 48 + 64 + F4_SEGCACHE * sizeof(SegDev);
+    return sizeof(cplx) * ((size_t)PADNF + (size_t)PADM + TWS) + STAGE_BYTES + sizeof(double) * (4 * NW + 2) + 48 + 64 +
+           F4_SEGCACHE * sizeof(SegDev);
   }
   // position of bin k in the inverse transform's input order (plan [32,16,16])
   __host__ __device__ static constexpr int pos(int k) { return ((k & 31) << 8) | (((k >> 5) & 15) << 4) | (k >> 9); }
@@ -109,7 +125,8 @@ __global__ void __launch_bounds__(ClusterShape::NT, 1) td_cluster_kernel(const F
   cplx* sm = reinterpret_cast<cplx*>(smem_raw);
   const SmemArr U{sm}, Z{sm + Sh::PADNF};
   cplx* tw = sm + Sh::PADNF + Sh::PADM;
-  double* red = reinterpret_cast<double*>(tw + Sh::TWS);   // [2][2 NW] per-warp partial sums, double-buffered by item parity
+  double* stage = reinterpret_cast<double*>(tw + Sh::TWS);  // fp32 build only (STAGE_BYTES)
+  double* red = stage + Sh::STAGE_BYTES / sizeof(double);   // [2][2 NW] per-warp partial sums, double-buffered by item parity
   double* xsum = red + 4 * NW;                             // [2] rank 1's partial sums, written remotely (rank 0 only)
   const uint32_t mbar_rows = smem_u32(xsum + 2);
   const uint32_t mbar_x = mbar_rows + 8;                   // the partner's half-results have landed (tx bytes)
@@ -119,7 +136,7 @@ __global__ void __launch_bounds__(ClusterShape::NT, 1) td_cluster_kernel(const F
   Book* bk = reinterpret_cast<Book*>(xsum + 6);
   SegDev* segS = reinterpret_cast<SegDev*>(xsum + 14);
   const SegDev* segs = P.n_seg <= F4_SEGCACHE ? segS : P.segs;
-  double* stH = reinterpret_cast<double*>(sm);             // staged row (<= M doubles) in the U region
+  double* stH = F32 ? stage : reinterpret_cast<double*>(sm);  // staged row (<= M doubles): the U region in fp64
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int br = (int)cluster_ctarank();                   // branch: 0 even bins, 1 odd bins
   const F4Own own = f4_own<Sh::RF1, true>(br, warp);
@@ -134,12 +151,12 @@ __global__ void __launch_bounds__(ClusterShape::NT, 1) td_cluster_kernel(const F
   for (int k = tid; k < Sh::TWS; k += NT) tw[k] = P.T[k];
   if (tid < P.n_seg && tid < F4_SEGCACHE) segS[tid] = P.segs[tid];
   if (tid == 0) { mbar_init(mbar_rows, 1); mbar_init(mbar_x, 1); bk->pend_b = -1; bk->prev_b = -1; }
-  if (warp == 0) tmem_alloc<512>(smem_u32(tmem_slot));
+  if (warp == 0) tmem_alloc<Sh::TMEM_COLS>(smem_u32(tmem_slot));
   tmem_fence_before();
   __syncthreads();
   tmem_fence_after();
-  const uint32_t tcol = *tmem_slot + ((uint32_t)(32 * (warp & 3)) << 16) + (uint32_t)((warp >> 2) * 256);
-  f4_store_twiddles<TW>(lane, tw, tcol + F4_TC_TW);
+  const uint32_t tcol = *tmem_slot + ((uint32_t)(32 * (warp & 3)) << 16) + (uint32_t)((warp >> 2) * Sh::Cols::WINDOW);
+  f4_store_twiddles<TW>(lane, tw, tcol + Sh::Cols::TW);
 
   // rows of item (b, s): hrow is the row that gets staged (the template; d itself for STOREZ)
   auto rows = [&](long long b, int s, const double*& drow, const double*& hrow, int& n) -> bool {
@@ -176,7 +193,7 @@ __global__ void __launch_bounds__(ClusterShape::NT, 1) td_cluster_kernel(const F
   auto s5_deferred = [&]() {
     mbar_wait(mbar_x, par_x);
     par_x ^= 1;
-    double p0[2] = {0.0, 0.0}, p1[2] = {0.0, 0.0};
+    real p0[2] = {real(0), real(0)}, p1[2] = {real(0), real(0)};
     static_for<0, 16>([&](auto t) {
       constexpr int tt = decltype(t)::value;
       const cplx a = Z.p[hslot(tt < 8 ? own.z0 : own.z1, tt)], bq = Z.p[hslot(tt < 8 ? own.z2 : own.z3, tt)];
@@ -195,8 +212,8 @@ __global__ void __launch_bounds__(ClusterShape::NT, 1) td_cluster_kernel(const F
       }
     });
     if (MODE != MODE_STOREZ) {
-      double acc0 = 0.0, acc1 = warp_sum(p1[0] + p1[1]);
-      if (MODE == MODE_INNER) acc0 = warp_sum(p0[0] + p0[1]);
+      double acc0 = 0.0, acc1 = warp_sum((double)(p1[0] + p1[1]));
+      if (MODE == MODE_INNER) acc0 = warp_sum((double)(p0[0] + p0[1]));
       if (lane == 0) { double* r = red + 2 * NW * ((item & 1) ^ 1); r[2 * warp] = acc0; r[2 * warp + 1] = acc1; }
     }
   };
@@ -239,7 +256,8 @@ __global__ void __launch_bounds__(ClusterShape::NT, 1) td_cluster_kernel(const F
 #pragma unroll
       for (int q = 0; q < 16; ++q) {
         const int i0 = 2 * (tid + 256 * q);
-        tmem_st_c(tcol + F4_TC_D + 4 * q, mk(i0 < sg.n ? __ldg(drow + i0) : 0.0, i0 + 1 < sg.n ? __ldg(drow + i0 + 1) : 0.0));
+        double2 dv = make_double2(i0 < sg.n ? __ldg(drow + i0) : 0.0, i0 + 1 < sg.n ? __ldg(drow + i0 + 1) : 0.0);
+        tmem_st_c64(tcol + F4_TC_D + 4 * q, dv);
       }
     }
     tmem_wait_st();
@@ -259,19 +277,27 @@ __global__ void __launch_bounds__(ClusterShape::NT, 1) td_cluster_kernel(const F
           }
           mbar_wait(mbar_rows, par_rows);
           par_rows ^= 1;
+          double2 hs[16];   // the staged samples, fp64 in both precisions
 #pragma unroll
           for (int q = 0; q < 16; ++q) {
             const int i0 = 2 * (j + 256 * q);
-            double2 h = mk(0.0, 0.0);
+            double2 h = make_double2(0.0, 0.0);
             if (i0 < sg.n) h = *reinterpret_cast<const double2*>(stH + i0);  // n even on this path
-            x[q] = h;
+            hs[q] = h;
           }
           if (MODE == MODE_LOGLIKE) {
             tmem_wait_ld();
 #pragma unroll
             for (int g = 0; g < 4; ++g) tmem_use16(dr[g]);
 #pragma unroll
-            for (int q = 0; q < 16; ++q) { const cplx dv = tmem_c(dr[q >> 2], q & 3); x[q] = mk(dv.x - x[q].x, dv.y - x[q].y); }
+            for (int q = 0; q < 16; ++q) {
+              const double2 dv = tmem_c64(dr[q >> 2], q & 3);
+              // S1: r = d - h in fp64 (the fp32 build scales by rscale and rounds once; h = d stays exactly 0)
+              x[q] = to_cplx(dv.x - hs[q].x, dv.y - hs[q].y, sg.rscale);
+            }
+          } else {
+#pragma unroll
+            for (int q = 0; q < 16; ++q) x[q] = to_cplx(hs[q].x, hs[q].y, sg.rscale);
           }
           __syncthreads();  // staging consumed: the U region may now be overwritten
         } else {
@@ -279,7 +305,7 @@ __global__ void __launch_bounds__(ClusterShape::NT, 1) td_cluster_kernel(const F
           rows(b, s, drow, hrow, n);
           const bool vec = ((reinterpret_cast<uintptr_t>(drow) | reinterpret_cast<uintptr_t>(hrow)) & 15) == 0;
 #pragma unroll
-          for (int q = 0; q < 16; ++q) x[q] = load_pair<MODE>(drow, hrow, j + 256 * q, n, vec);
+          for (int q = 0; q < 16; ++q) x[q] = load_pair<MODE>(drow, hrow, j + 256 * q, n, vec, sg.rscale);
         }
         cplx w[16];
         tw_powers<16>(tw[4 * j], w);  // w_NF^j
@@ -298,7 +324,7 @@ __global__ void __launch_bounds__(ClusterShape::NT, 1) td_cluster_kernel(const F
       }
       __syncthreads();
       // ---------------- forward passes 2 and 3, warp-local
-      f4_forward23<TW, true>(U, own, lane, tw, tcol + F4_TC_TW);
+      f4_forward23<TW, true>(U, own, lane, tw, tcol + Sh::Cols::TW);
       __syncwarp();  // mirror-closed ownership (f4_own): mid reads only this warp's U blocks
       // ---------------- S5 of the PREVIOUS item, from the Z blocks this warp is about to overwrite
       if (item > 0) s5_deferred();
@@ -328,7 +354,7 @@ __global__ void __launch_bounds__(ClusterShape::NT, 1) td_cluster_kernel(const F
           // x_q *= conj(w_M^{j q}) (and conj(w_2M^j) on the odd branch); powers as w^{4 hi} * w^{lo}
           cplx lo[4], hi[8];
           tw_powers<4>(tw[2 * j], lo);
-          hi[0] = mk(1.0, 0.0);
+          hi[0] = mk(real(1), real(0));
           hi[1] = csq(lo[2]);
           static_for<2, 8>([&](auto q) {
             constexpr int qq = decltype(q)::value;
@@ -384,7 +410,7 @@ __global__ void __launch_bounds__(ClusterShape::NT, 1) td_cluster_kernel(const F
   cluster_wait();
   if (br == 0 && tid == 0) settle();
   __syncthreads();
-  if (warp == 0) tmem_dealloc<512>(*tmem_slot);
+  if (warp == 0) tmem_dealloc<Sh::TMEM_COLS>(*tmem_slot);
 }
 
-}  // namespace td
+}  // namespace TD_NS

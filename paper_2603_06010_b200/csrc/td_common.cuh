@@ -1,18 +1,36 @@
 // td_common.cuh - complex helpers, in-register radix-R FFT butterflies, twiddle chains and
 // mixed-radix index maps shared by the fused (shared-memory) and staged (global-memory) FFT
 // kernels of the Gohberg-Semencul / circulant-embedding path (Eqs. 14-16).
+// The scalar type is a compile-time choice of the translation unit: fp64 (namespace td, tdlike.cu) or, with TD_F32
+// defined, fp32 (namespace td32, tdlike_f32.cu: the FP32 evaluation mode of PAPER.md:322-324, III.C.3 - operators
+// precomputed in fp64, rounded once, evaluation in fp32).  Both see the same source; `real` / `cplx` are the only types
+// that differ, every literal that enters arithmetic is typed `real`.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
 
-namespace td {
+#ifdef TD_F32
+#define TD_NS td32
+#else
+#define TD_NS td
+#endif
 
+namespace TD_NS {
+
+#ifdef TD_F32
+typedef float real;
+typedef float2 cplx;
+constexpr bool F32 = true;
+#else
+typedef double real;
 typedef double2 cplx;
+constexpr bool F32 = false;
+#endif
 
 // what a batch kernel accumulates: -1/2 <d-h, d-h> | (<d,h>, <h,h>) | nothing (stores z of the data vector)
 enum { MODE_LOGLIKE = 0, MODE_INNER = 1, MODE_STOREZ = 2 };
 
-__host__ __device__ __forceinline__ cplx mk(double x, double y) { return make_double2(x, y); }
+__host__ __device__ __forceinline__ cplx mk(real x, real y) { cplx c; c.x = x; c.y = y; return c; }
 __device__ __forceinline__ cplx cadd(cplx a, cplx b) { return mk(a.x + b.x, a.y + b.y); }
 __device__ __forceinline__ cplx csub(cplx a, cplx b) { return mk(a.x - b.x, a.y - b.y); }
 __device__ __forceinline__ cplx cconj(cplx a) { return mk(a.x, -a.y); }
@@ -24,7 +42,7 @@ __device__ __forceinline__ cplx cmul(cplx a, cplx b) {
 __device__ __forceinline__ cplx cmulc(cplx a, cplx b) {
   return mk(fma(a.x, b.x, a.y * b.y), fma(a.y, b.x, -(a.x * b.y)));
 }
-__device__ __forceinline__ cplx csq(cplx a) { return mk(fma(a.x, a.x, -(a.y * a.y)), 2.0 * a.x * a.y); }
+__device__ __forceinline__ cplx csq(cplx a) { return mk(fma(a.x, a.x, -(a.y * a.y)), real(2) * a.x * a.y); }
 
 // ---- compile-time loops ---------------------------------------------------------------
 template <int I> struct IC { static constexpr int value = I; };
@@ -67,7 +85,7 @@ template <int K, bool INV> __device__ __forceinline__ cplx mul_w32(cplx a) {
   else if constexpr (k == 8) return INV ? mk(-a.y, a.x) : mk(a.y, -a.x);
   else if constexpr (k == 24) return INV ? mk(a.y, -a.x) : mk(-a.y, a.x);
   else {
-    constexpr double c = cos32(k), s = sin32(k);
+    constexpr real c = (real)cos32(k), s = (real)sin32(k);
     if constexpr (!INV) return mk(fma(a.x, c, a.y * s), fma(a.y, c, -(a.x * s)));
     else return mk(fma(a.x, c, -(a.y * s)), fma(a.y, c, a.x * s));
   }
@@ -92,7 +110,7 @@ template <int R> __host__ __device__ constexpr int brevR(int k) { return brev_bi
 
 // w[t] = w1^t, t = 1..R-1 (w[0] unused), by a squaring/multiply tree of depth <= log2(R)+2.
 template <int R> __device__ __forceinline__ void tw_powers(cplx w1, cplx (&w)[R]) {
-  w[0] = mk(1.0, 0.0);
+  w[0] = mk(real(1), real(0));
   if constexpr (R > 1) w[1] = w1;
   static_for<2, R>([&](auto t) {
     constexpr int tt = decltype(t)::value;
@@ -303,14 +321,26 @@ __device__ __forceinline__ void tmem_fence_before() { asm volatile("tcgen05.fenc
 __device__ __forceinline__ void tmem_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
-// one complex double = 4 columns
-__device__ __forceinline__ void tmem_st_c(uint32_t taddr, cplx v) {
+// columns per complex number of the kernel's scalar type: 4 (fp64) or 2 (fp32)
+constexpr int TM_CPC = (int)(sizeof(cplx) / 4);
+// one complex fp64 = 4 columns (the data samples are kept in fp64 in both precisions: r = d - h is formed in fp64)
+__device__ __forceinline__ void tmem_st_c64(uint32_t taddr, double2 v) {
   asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1, %2, %3, %4};" ::"r"(taddr), "r"(__double2loint(v.x)),
                "r"(__double2hiint(v.x)), "r"(__double2loint(v.y)), "r"(__double2hiint(v.y))
                : "memory");
 }
-// 4 complex doubles = 16 columns.  tcgen05.ld is asynchronous: issue all loads, tmem_wait_ld(), then tmem_use16() on each
-// register group (an empty asm that "rewrites" the registers, so that no use can be scheduled above the wait), then read.
+// one complex number of the kernel's scalar type = TM_CPC columns
+__device__ __forceinline__ void tmem_st_c(uint32_t taddr, cplx v) {
+#ifdef TD_F32
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x2.b32 [%0], {%1, %2};" ::"r"(taddr), "r"(__float_as_int(v.x)),
+               "r"(__float_as_int(v.y))
+               : "memory");
+#else
+  tmem_st_c64(taddr, v);
+#endif
+}
+// 16 columns.  tcgen05.ld is asynchronous: issue all loads, tmem_wait_ld(), then tmem_use16() on each register group (an
+// empty asm that "rewrites" the registers, so that no use can be scheduled above the wait), then read.
 __device__ __forceinline__ void tmem_ld16(uint32_t taddr, int (&r)[16]) {
   asm volatile(
       "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
@@ -325,8 +355,28 @@ __device__ __forceinline__ void tmem_use16(int (&r)[16]) {
                :
                : "memory");
 }
-__device__ __forceinline__ cplx tmem_c(const int (&r)[16], int q) {  // q-th complex of a group of 4
-  return mk(__hiloint2double(r[4 * q + 1], r[4 * q]), __hiloint2double(r[4 * q + 3], r[4 * q + 2]));
+__device__ __forceinline__ double2 tmem_c64(const int (&r)[16], int q) {  // q-th complex fp64 of a group of 4
+  return make_double2(__hiloint2double(r[4 * q + 1], r[4 * q]), __hiloint2double(r[4 * q + 3], r[4 * q + 2]));
 }
+// sixteen complex numbers of the kernel's scalar type held in 16 TM_CPC consecutive columns: NG x16 loads
+struct TmemC16 {
+  static constexpr int NG = TM_CPC;  // 16 * TM_CPC columns / 16 per load
+  int r[NG][16];
+  __device__ __forceinline__ void ld(uint32_t taddr) {
+#pragma unroll
+    for (int g = 0; g < NG; ++g) tmem_ld16(taddr + 16 * g, r[g]);
+  }
+  __device__ __forceinline__ void use() {
+#pragma unroll
+    for (int g = 0; g < NG; ++g) tmem_use16(r[g]);
+  }
+  __device__ __forceinline__ cplx get(int q) const {  // q compile-time after unrolling
+#ifdef TD_F32
+    return mk(__int_as_float(r[q >> 3][2 * (q & 7)]), __int_as_float(r[q >> 3][2 * (q & 7) + 1]));
+#else
+    return tmem_c64(r[q >> 2], q & 3);
+#endif
+  }
+};
 
-}  // namespace td
+}  // namespace TD_NS

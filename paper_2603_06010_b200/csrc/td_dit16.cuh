@@ -17,13 +17,13 @@
 #pragma once
 #include "td_common.cuh"
 
-namespace td {
+namespace TD_NS {
 
 // a <- a + w b,  b <- a - w b
-__host__ __device__ __forceinline__ void bf6(cplx& a, cplx& b, double wr, double wi) {
-  const double xr = fma(wr, b.x, fma(-wi, b.y, a.x));
-  const double xi = fma(wr, b.y, fma(wi, b.x, a.y));
-  b = mk(fma(2.0, a.x, -xr), fma(2.0, a.y, -xi));
+__host__ __device__ __forceinline__ void bf6(cplx& a, cplx& b, real wr, real wi) {
+  const real xr = fma(wr, b.x, fma(-wi, b.y, a.x));
+  const real xi = fma(wr, b.y, fma(wi, b.x, a.y));
+  b = mk(fma(real(2), a.x, -xr), fma(real(2), a.y, -xi));
   a = mk(xr, xi);
 }
 // a <- a + b,  b <- a - b
@@ -41,8 +41,8 @@ template <int SGN> __host__ __device__ __forceinline__ void bfi(cplx& a, cplx& b
 }
 // square of a unit-modulus number: (2x^2 - 1, 2xy), 3 ops
 __host__ __device__ __forceinline__ cplx usq(cplx w) {
-  const double x2 = w.x + w.x;
-  return mk(fma(x2, w.x, -1.0), x2 * w.y);
+  const real x2 = w.x + w.x;
+  return mk(fma(x2, w.x, real(-1)), x2 * w.y);
 }
 
 // butterfly with twiddle  w * (sgn i)^Q,  Q = 0 or 1
@@ -54,8 +54,8 @@ template <int Q, int SGN> __host__ __device__ __forceinline__ void bf6q(cplx& a,
 
 template <bool INV, bool TW> __host__ __device__ __forceinline__ void dit16(cplx (&x)[16], cplx w1) {
   constexpr int SG = INV ? 1 : -1;                 // W^4 = SG * i
-  constexpr double C8 = 0.70710678118654752440;    // cos(pi/4)
-  constexpr double C16 = 0.92387953251128675613, S16 = 0.38268343236508977173;  // cos, sin(pi/8)
+  constexpr real C8 = real(0.70710678118654752440);    // cos(pi/4)
+  constexpr real C16 = real(0.92387953251128675613), S16 = real(0.38268343236508977173);  // cos, sin(pi/8)
   if constexpr (TW) {
     const cplx w2 = usq(w1), w4 = usq(w2), w8 = usq(w4);
     // stage A: pairs (s, s+8), twiddle w1^8
@@ -108,4 +108,4 @@ template <bool INV, bool TW> __host__ __device__ __forceinline__ void dit16(cplx
   }
 }
 
-}  // namespace td
+}  // namespace TD_NS

@@ -18,7 +18,7 @@
 #include "td_common.cuh"
 #include "td_dit16.cuh"
 
-namespace td {
+namespace TD_NS {
 
 struct SegDev {
   long long off;    // offset of this segment inside d / a row of H (elements)
@@ -26,6 +26,9 @@ struct SegDev {
   int _pad;
   const cplx* G;    // [2][M]: even-bin then odd-bin generator spectrum, DIT input order, scaled
   cplx* zd;         // [M]: z of the data vector d (td_inner_batch only)
+  double rscale;    // fp32 evaluation only: samples are multiplied by rscale = rho_s(0)^(-1/2) in fp64 before they are
+                    // rounded to fp32, the generator spectrum carries the inverse factor ("appropriate normalization",
+                    // PAPER.md:324); unused (1.0) in fp64
 };
 
 struct FusedParams {
@@ -42,9 +45,14 @@ struct FusedParams {
 };
 
 // x = (sample 2*idx, sample 2*idx+1) of the vector this MODE transforms, zero beyond n.
+// (the combination is formed in fp64 in both precisions; the fp32 build scales by rs and rounds once)
+__device__ __forceinline__ cplx to_cplx(double x, double y, double rs) {
+  if constexpr (F32) return mk((real)(x * rs), (real)(y * rs));
+  else return mk((real)x, (real)y);
+}
 template <int MODE>
 __device__ __forceinline__ cplx load_pair(const double* __restrict__ drow, const double* __restrict__ hrow,
-                                          int idx, int n, bool vec) {
+                                          int idx, int n, bool vec, double rs) {
   const int i0 = 2 * idx;
   double h0 = 0.0, h1 = 0.0, d0 = 0.0, d1 = 0.0;
   if (i0 + 1 < n && vec) {
@@ -66,9 +74,9 @@ __device__ __forceinline__ cplx load_pair(const double* __restrict__ drow, const
       if (MODE != MODE_INNER) d1 = drow[i0 + 1];
     }
   }
-  if (MODE == MODE_LOGLIKE) return mk(d0 - h0, d1 - h1);
-  if (MODE == MODE_INNER) return mk(h0, h1);
-  return mk(d0, d1);
+  if (MODE == MODE_LOGLIKE) return to_cplx(d0 - h0, d1 - h1, rs);
+  if (MODE == MODE_INNER) return to_cplx(h0, h1, rs);
+  return to_cplx(d0, d1, rs);
 }
 
 // First forward pass: reads the packed real input straight from global memory and produces
@@ -79,12 +87,12 @@ template <int R, int MODE, class Arr>
 __device__ __forceinline__ void first_pass_task(const Arr& UE, const Arr& UO, int nf, int g,
                                                 const double* __restrict__ drow,
                                                 const double* __restrict__ hrow, int n, bool vec,
-                                                const cplx* __restrict__ T) {
+                                                const cplx* __restrict__ T, double rs = 1.0) {
   const int S = nf / R;
   const int j = g;  // single block of length nf
   cplx x[R], y[R];
 #pragma unroll
-  for (int s = 0; s < R; ++s) x[s] = load_pair<MODE>(drow, hrow, j + s * S, n, vec);
+  for (int s = 0; s < R; ++s) x[s] = load_pair<MODE>(drow, hrow, j + s * S, n, vec, rs);
   static_for<0, R>([&](auto s) {
     constexpr int ss = decltype(s)::value;
     y[ss] = mul_w32<ss * (16 / R), false>(x[ss]);
@@ -188,9 +196,9 @@ __device__ __forceinline__ void last_pass_task(const Arr& ZE, const Arr& ZO, int
     } else if (i < n) {
       if (MODE == MODE_INNER) {
         const cplx q = zd[i];
-        acc0 = fma(z.x, q.x, fma(-z.y, q.y, acc0));
+        acc0 += (double)fma(z.x, q.x, -z.y * q.y);
       }
-      acc1 = fma(z.x, z.x, fma(-z.y, z.y, acc1));
+      acc1 += (double)fma(z.x, z.x, -z.y * z.y);
     }
   });
 }
@@ -239,11 +247,11 @@ __device__ __forceinline__ void smem_pass16c(const SmemArr& AE, const SmemArr& A
 template <int R, int NF, int MODE>
 __device__ __forceinline__ void first_pass_c(const SmemArr& UE, const SmemArr& UO, int j,
                                              const double* __restrict__ drow, const double* __restrict__ hrow,
-                                             int n, bool vec, const cplx* __restrict__ tw) {
+                                             int n, bool vec, const cplx* __restrict__ tw, double rs = 1.0) {
   constexpr int S = NF / R;
   cplx x[R], y[R];
 #pragma unroll
-  for (int s = 0; s < R; ++s) x[s] = load_pair<MODE>(drow, hrow, j + s * S, n, vec);
+  for (int s = 0; s < R; ++s) x[s] = load_pair<MODE>(drow, hrow, j + s * S, n, vec, rs);
   static_for<0, R>([&](auto s) {
     constexpr int ss = decltype(s)::value;
     y[ss] = mul_w32<ss * (16 / R), false>(x[ss]);
@@ -341,7 +349,7 @@ __device__ __forceinline__ void last_pass_c(const SmemArr& ZE, const SmemArr& ZO
     });
   }
   // four independent partial sums per output (a single chain of 2 R dependent FMAs would be latency-bound)
-  double p0[4] = {0.0, 0.0, 0.0, 0.0}, p1[4] = {0.0, 0.0, 0.0, 0.0};
+  real p0[4] = {real(0), real(0), real(0), real(0)}, p1[4] = {real(0), real(0), real(0), real(0)};
   static_for<0, R>([&](auto t) {
     constexpr int tt = decltype(t)::value;
     const cplx ev = e[brevR<R>(tt)], ov = o[brevR<R>(tt)];
@@ -361,8 +369,8 @@ __device__ __forceinline__ void last_pass_c(const SmemArr& ZE, const SmemArr& ZO
       }
     }
   });
-  if constexpr (MODE == MODE_INNER) acc0 += (p0[0] + p0[1]) + (p0[2] + p0[3]);
-  if constexpr (MODE != MODE_STOREZ) acc1 += (p1[0] + p1[1]) + (p1[2] + p1[3]);
+  if constexpr (MODE == MODE_INNER) acc0 += (double)((p0[0] + p0[1]) + (p0[2] + p0[3]));
+  if constexpr (MODE != MODE_STOREZ) acc1 += (double)((p1[0] + p1[1]) + (p1[2] + p1[3]));
 }
 
 // both branches of one radix-16 butterfly task interleaved (twice the independent work per thread)
@@ -414,17 +422,17 @@ __device__ __forceinline__ void smem_pass16v(const SmemArr& AE, const SmemArr& A
 // first pass fed from the staged (TMA-prefetched) rows in shared memory: values only
 template <int R, int NF, int MODE>
 __device__ __forceinline__ void first_pass_load_staged(cplx (&x)[R], int j, const double* stH, const double* stD,
-                                                       int n) {
+                                                       int n, double rs = 1.0) {
   constexpr int S = NF / R;
 #pragma unroll
   for (int s = 0; s < R; ++s) {
     const int i0 = 2 * (j + s * S);
-    double2 h = mk(0.0, 0.0), d = mk(0.0, 0.0);
+    double2 h = make_double2(0.0, 0.0), d = make_double2(0.0, 0.0);
     if (i0 < n) {  // n even on this path: i0 + 1 < n too
       if (MODE != MODE_STOREZ) h = *reinterpret_cast<const double2*>(stH + i0);
       if (MODE != MODE_INNER) d = *reinterpret_cast<const double2*>(stD + i0);
     }
-    x[s] = (MODE == MODE_LOGLIKE) ? mk(d.x - h.x, d.y - h.y) : (MODE == MODE_INNER ? h : d);
+    x[s] = (MODE == MODE_LOGLIKE) ? to_cplx(d.x - h.x, d.y - h.y, rs) : (MODE == MODE_INNER ? to_cplx(h.x, h.y, rs) : to_cplx(d.x, d.y, rs));
   }
 }
 template <int R, int NF>
@@ -498,6 +506,7 @@ __device__ __forceinline__ void untangle_apply(const SmemArr& U, const SmemArr& 
 
 template <int LOG2M, int NT, int MODE, bool ILV = true>
 __global__ void __launch_bounds__(NT, 1) td_fused_kernel(const FusedParams P) {
+  static_assert(!F32 || LOG2M < 0, "fp64 only: the two staged rows of doubles do not fit the fp32 U region");
   using Sh = FusedShape<LOG2M>;
   constexpr int M = Sh::M, NF = Sh::NF, TW = 2 * M;
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -561,7 +570,7 @@ __global__ void __launch_bounds__(NT, 1) td_fused_kernel(const FusedParams P) {
       cplx xs[IT][Sh::RF1];
 #pragma unroll
       for (int it = 0; it < IT; ++it)
-        if (tid + it * NT < NTASK) first_pass_load_staged<Sh::RF1, NF, MODE>(xs[it], tid + it * NT, stH, stD, sg.n);
+        if (tid + it * NT < NTASK) first_pass_load_staged<Sh::RF1, NF, MODE>(xs[it], tid + it * NT, stH, stD, sg.n, sg.rscale);
       __syncthreads();  // staging consumed: the U region may now be overwritten
 #pragma unroll
       for (int it = 0; it < IT; ++it)
@@ -572,7 +581,7 @@ __global__ void __launch_bounds__(NT, 1) td_fused_kernel(const FusedParams P) {
       const bool vec = ((reinterpret_cast<uintptr_t>(drow) | reinterpret_cast<uintptr_t>(hrow)) & 15) == 0;
 #pragma unroll 1
       for (int g = tid; g < NF / Sh::RF1; g += NT)
-        first_pass_c<Sh::RF1, NF, MODE>(UE, UO, g, drow, hrow, n, vec, tw);
+        first_pass_c<Sh::RF1, NF, MODE>(UE, UO, g, drow, hrow, n, vec, tw, sg.rscale);
     }
     __syncthreads();
     // ---- forward passes 2..NPF (radix 16)
@@ -648,4 +657,4 @@ __global__ void __launch_bounds__(NT, 1) td_fused_kernel(const FusedParams P) {
   }
 }
 
-}  // namespace td
+}  // namespace TD_NS

@@ -22,15 +22,22 @@
 #include "td_fused.cuh"
 #include "td_dit16.cuh"
 
-namespace td {
+namespace TD_NS {
 
 constexpr int F4_SEGCACHE = 8;  // segment records cached in shared memory (more segments: read from global per item)
 
-// TMEM columns of a thread, relative to its warp's column base (a complex double = 4 columns; warps w and w + 4 share
-// a lane quarter and take columns [0, 256) and [256, 512))
-constexpr int F4_TC_G = 0;     // 128 columns: the 2 x 16 generator values of mid
-constexpr int F4_TC_D = 128;   // up to 64 columns: the thread's samples of the data vector (first forward pass)
-constexpr int F4_TC_TW = 192;  // 64 columns: twiddle powers of forward pass 2
+// TMEM columns of a thread, relative to its warp's column base (a complex number = TM_CPC columns: 4 in fp64, 2 in fp32;
+// warps w and w + 4 share a lane quarter and take columns [0, 256) and [256, 512))
+constexpr int F4_TC_G = 0;                  // 32 complex: the 2 x 16 generator values of mid
+constexpr int F4_TC_D = 32 * TM_CPC;        // ND complex fp64 samples of the data vector (first forward pass; fp64 in both
+                                            // precisions: the residual d - h is formed before rounding), 4 columns each
+// ND = 8 (one-CTA kernel) or 16 (cluster kernel) data samples per thread; then 16 complex: twiddle powers of forward pass 2
+template <int ND> struct F4Cols {
+  static constexpr int TW = F4_TC_D + 4 * ND;
+  static constexpr int USED = TW + 16 * TM_CPC;
+  static constexpr int WINDOW = USED <= 128 ? 128 : 256;   // a thread's window: a power of two (allocation granularity)
+  static_assert(USED <= 256, "a thread's TMEM window is at most 256 columns");
+};
 
 template <int LOG2M> struct Fused4Shape {
   static constexpr int M = 1 << LOG2M, NF = M / 2;
@@ -39,7 +46,9 @@ template <int LOG2M> struct Fused4Shape {
   static constexpr int NT = 32 * RF1, NW = RF1, NWB = RF1 / 2;
   static constexpr int TWS = 2 * M / RF1;
   static constexpr int PADM = SmemArr::padded(M), PADNF = SmemArr::padded(NF);
-  static constexpr int TMEM_COLS = NW > 4 ? 512 : 256;  // 256 columns per thread; warps w and w + 4 share a lane quarter
+  using Cols = F4Cols<8>;
+  // Cols::WINDOW columns per thread (256 in fp64, 128 in fp32); warps w and w + 4 share a lane quarter
+  static constexpr int TMEM_COLS = (NW > 4 ? 2 : 1) * Cols::WINDOW;
   static constexpr size_t smem_bytes() {
     return sizeof(cplx) * (2 * (size_t)PADNF + 2 * (size_t)PADM + TWS) + sizeof(double) * 4 * NW + 48 + F4_SEGCACHE * sizeof(SegDev)
 #ifdef TD_PHASE_CLOCKS
@@ -88,10 +97,9 @@ __device__ __forceinline__ void f4_forward23(const SmemArr& U, const F4Own& o, i
     const int s1 = (lane >> 4) ? o.u1 : o.u0, j = lane & 15;
     const int base = s1 * 256 + j;
     cplx w[16];
-    int wr[4][16];
+    TmemC16 wr;
     if constexpr (TWT) {
-#pragma unroll
-      for (int g = 0; g < 4; ++g) tmem_ld16(ttw + 16 * g, wr[g]);
+      wr.ld(ttw);
     } else {
       tw_powers<16>(tw[j * (TW / 256)], w);
     }
@@ -99,10 +107,9 @@ __device__ __forceinline__ void f4_forward23(const SmemArr& U, const F4Own& o, i
     for (int q = 0; q < 16; ++q) x[q] = U.ld(base + 16 * q);
     if constexpr (TWT) {
       tmem_wait_ld();
+      wr.use();
 #pragma unroll
-      for (int g = 0; g < 4; ++g) tmem_use16(wr[g]);
-#pragma unroll
-      for (int q = 0; q < 16; ++q) w[q] = tmem_c(wr[q >> 2], q & 3);
+      for (int q = 0; q < 16; ++q) w[q] = wr.get(q);
     }
     fft_reg<16, false>(x);
     static_for<0, 16>([&](auto t) {
@@ -135,7 +142,7 @@ __device__ __forceinline__ void f4_store_twiddles(int lane, const cplx* __restri
   cplx w[16];
   tw_powers<16>(tw[(lane & 15) * (TW / 256)], w);
 #pragma unroll
-  for (int q = 0; q < 16; ++q) tmem_st_c(ttw + 4 * q, w[q]);
+  for (int q = 0; q < 16; ++q) tmem_st_c(ttw + TM_CPC * q, w[q]);
 }
 
 // this lane's 2 x 16 generator values (g = one branch of the segment's spectrum in the padded Z layout, global memory)
@@ -150,7 +157,7 @@ __device__ __forceinline__ void f4_store_generator(const cplx* __restrict__ g, c
 #pragma unroll
     for (int q = 0; q < 16; ++q) {
       const int i = zb + q;
-      tmem_st_c(tg + 4 * (16 * par + q), __ldg(g + i + (i >> 4)));
+      tmem_st_c(tg + TM_CPC * (16 * par + q), __ldg(g + i + (i >> 4)));
     }
   }
 }
@@ -176,7 +183,7 @@ __device__ __forceinline__ void f4_mid(const SmemArr& U, const SmemArr& Z, int b
   // Two halves (even t -> inverse block tau, odd t -> block tau + M/32), software-pipelined: the U loads of half 1 are in
   // flight while half 0 runs its radix-16 butterfly, and half 0's stores drain while half 1 computes.
   cplx ua[8], ub[8], e[16];
-  int gr[4][16];
+  TmemC16 gr;
   auto load_u = [&](auto par) {
     constexpr int pp = decltype(par)::value;
     static_for<0, 8>([&](auto hh) {
@@ -188,8 +195,7 @@ __device__ __forceinline__ void f4_mid(const SmemArr& U, const SmemArr& Z, int b
   auto load_g = [&](auto par) {
     constexpr int pp = decltype(par)::value;
     if constexpr (GT) {
-#pragma unroll
-      for (int g = 0; g < 4; ++g) tmem_ld16(tg + 64 * pp + 16 * g, gr[g]);
+      gr.ld(tg + 16 * TM_CPC * pp);
     } else {
 #pragma unroll
       for (int q = 0; q < 16; ++q) e[q] = Z.ld(zb0 + pp * 8 * 16 + q);  // generator spectrum sits in Z
@@ -199,10 +205,9 @@ __device__ __forceinline__ void f4_mid(const SmemArr& U, const SmemArr& Z, int b
     constexpr int pp = decltype(par)::value;
     if constexpr (GT) {
       tmem_wait_ld();
+      gr.use();
 #pragma unroll
-      for (int g = 0; g < 4; ++g) tmem_use16(gr[g]);
-#pragma unroll
-      for (int q = 0; q < 16; ++q) e[q] = tmem_c(gr[q >> 2], q & 3);
+      for (int q = 0; q < 16; ++q) e[q] = gr.get(q);
     }
     static_for<0, 8>([&](auto hh) {
       constexpr int h8 = decltype(hh)::value, t = 2 * h8 + pp;
@@ -225,14 +230,14 @@ __device__ __forceinline__ void f4_mid(const SmemArr& U, const SmemArr& Z, int b
     load_g(IC<1>{});
     load_u(IC<1>{});   // in flight during the butterfly below
   }
-  dit16<true, false>(e, mk(1.0, 0.0));
+  dit16<true, false>(e, mk(real(1), real(0)));
   store_e(IC<0>{});
   if constexpr (!GT) {
     load_g(IC<1>{});   // e is the landing area of the generator values on this path: only now free
     load_u(IC<1>{});
   }
   untangle(IC<1>{});
-  dit16<true, false>(e, mk(1.0, 0.0));
+  dit16<true, false>(e, mk(real(1), real(0)));
   store_e(IC<1>{});
 }
 
@@ -295,9 +300,9 @@ __global__ void __launch_bounds__(Fused4Shape<LOG2M>::NT, 1) td_fused4_kernel(co
   tmem_fence_before();
   __syncthreads();
   tmem_fence_after();
-  // this thread's TMEM window: lane 32 (warp % 4) + lane, 256 columns
-  const uint32_t tcol = *tmem_slot + ((uint32_t)(32 * (warp & 3)) << 16) + (uint32_t)((warp >> 2) * 256);
-  f4_store_twiddles<TW>(lane, tw, tcol + F4_TC_TW);
+  // this thread's TMEM window: lane 32 (warp % 4) + lane, Cols::WINDOW columns
+  const uint32_t tcol = *tmem_slot + ((uint32_t)(32 * (warp & 3)) << 16) + (uint32_t)((warp >> 2) * Sh::Cols::WINDOW);
+  f4_store_twiddles<TW>(lane, tw, tcol + Sh::Cols::TW);
 
   // rows of item (b, s); the template row is staged by TMA when it is 16-byte aligned and N_s is even
   auto rows = [&](long long b, int s, const double*& drow, const double*& hrow, int& n) -> bool {
@@ -361,8 +366,8 @@ __global__ void __launch_bounds__(Fused4Shape<LOG2M>::NT, 1) td_fused4_kernel(co
 #pragma unroll
         for (int ss = 0; ss < RF1; ++ss) {
           const int i0 = 2 * (tid + it * NT + ss * S1);
-          const cplx dv = mk(i0 < sg.n ? __ldg(drow + i0) : 0.0, i0 + 1 < sg.n ? __ldg(drow + i0 + 1) : 0.0);
-          tmem_st_c(tcol + F4_TC_D + 4 * (it * RF1 + ss), dv);
+          double2 dv = make_double2(i0 < sg.n ? __ldg(drow + i0) : 0.0, i0 + 1 < sg.n ? __ldg(drow + i0 + 1) : 0.0);
+          tmem_st_c64(tcol + F4_TC_D + 4 * (it * RF1 + ss), dv);
         }
     }
     tmem_wait_st();
@@ -379,14 +384,15 @@ __global__ void __launch_bounds__(Fused4Shape<LOG2M>::NT, 1) td_fused4_kernel(co
         par_rows ^= 1;
         TDCLK(1);
         cplx xs[IT][RF1];
+        double2 hs[IT][RF1];   // the staged samples, fp64 in both precisions
 #pragma unroll
         for (int it = 0; it < IT; ++it)
 #pragma unroll
           for (int ss = 0; ss < RF1; ++ss) {
             const int i0 = 2 * (tid + it * NT + ss * S1);
-            double2 hv = mk(0.0, 0.0);
+            double2 hv = make_double2(0.0, 0.0);
             if (i0 < sg.n) hv = *reinterpret_cast<const double2*>(stH + i0);  // n even on this path: i0 + 1 < n too
-            xs[it][ss] = hv;
+            hs[it][ss] = hv;
           }
         if (MODE == MODE_LOGLIKE) {
           tmem_wait_ld();
@@ -395,9 +401,16 @@ __global__ void __launch_bounds__(Fused4Shape<LOG2M>::NT, 1) td_fused4_kernel(co
           for (int it = 0; it < IT; ++it)
 #pragma unroll
             for (int ss = 0; ss < RF1; ++ss) {
-              const cplx dv = tmem_c(dr[(it * RF1 + ss) >> 2], (it * RF1 + ss) & 3);
-              xs[it][ss] = mk(dv.x - xs[it][ss].x, dv.y - xs[it][ss].y);   // S1: r = d - h
+              const double2 dv = tmem_c64(dr[(it * RF1 + ss) >> 2], (it * RF1 + ss) & 3);
+              const double2 hv = hs[it][ss];
+              // S1: r = d - h, formed in fp64 (the fp32 build scales by rscale and rounds once; h = d stays exactly 0)
+              xs[it][ss] = to_cplx(dv.x - hv.x, dv.y - hv.y, sg.rscale);
             }
+        } else {
+#pragma unroll
+          for (int it = 0; it < IT; ++it)
+#pragma unroll
+            for (int ss = 0; ss < RF1; ++ss) xs[it][ss] = to_cplx(hs[it][ss].x, hs[it][ss].y, sg.rscale);
         }
         TDCLK(2);
         __syncthreads();  // staging consumed: the U region may now be overwritten
@@ -410,7 +423,7 @@ __global__ void __launch_bounds__(Fused4Shape<LOG2M>::NT, 1) td_fused4_kernel(co
         rows(b, s, drow, hrow, n);
         const bool vec = ((reinterpret_cast<uintptr_t>(drow) | reinterpret_cast<uintptr_t>(hrow)) & 15) == 0;
 #pragma unroll 1
-        for (int g = tid; g < NTASK; g += NT) first_pass_c<RF1, NF, MODE>(UE, UO, g, drow, hrow, n, vec, tw);
+        for (int g = tid; g < NTASK; g += NT) first_pass_c<RF1, NF, MODE>(UE, UO, g, drow, hrow, n, vec, tw, sg.rscale);
       }
       __syncthreads();
       if (tid == 0) finalize();  // the previous item's sums: every warp has passed its last pass
@@ -419,7 +432,7 @@ __global__ void __launch_bounds__(Fused4Shape<LOG2M>::NT, 1) td_fused4_kernel(co
 #endif
       TDCLK(5);
       // ---------------- forward passes 2 and 3, warp-local
-      f4_forward23<TW, true>(U, own, lane, tw, tcol + F4_TC_TW);
+      f4_forward23<TW, true>(U, own, lane, tw, tcol + Sh::Cols::TW);
       __syncwarp();  // mirror-closed ownership: mid reads only this warp's U blocks
       TDCLK(6);
       // ---------------- mid: untangle (registers) x generator (TMEM) -> first inverse pass -> Z
@@ -459,4 +472,4 @@ __global__ void __launch_bounds__(Fused4Shape<LOG2M>::NT, 1) td_fused4_kernel(co
 #endif
 }
 
-}  // namespace td
+}  // namespace TD_NS

@@ -11,6 +11,8 @@
 #include <new>
 #include <vector>
 
+#include "td_host.h"
+#include "td_f32.h"
 #include "td_dense.cuh"
 #include "td_dot.cuh"
 #include "td_fused.cuh"
@@ -21,6 +23,7 @@
 #include "td_synth.cuh"
 
 using namespace td;
+using namespace tdhost;
 
 namespace {
 
@@ -36,6 +39,7 @@ struct SegHost {
   int n = 0;
   int log2M = 0;
   double v = 0.0, logdet = 0.0;
+  double rho0 = 0.0;    // rho_s(0): normalisation of the fp32 evaluation mode
   double* a = nullptr;  // device [n]
   cplx* G = nullptr;    // device [2][M]
   cplx* Gp = nullptr;   // device [2][padded(M)], padded Z layout (fused4 classes only)
@@ -49,6 +53,8 @@ struct ClassInfo {
   int max_n = 0;                // longest segment of the class
   SegDev* d_segs = nullptr;     // device [seg_ids.size()]
   const cplx** d_Gp = nullptr;  // device [seg_ids.size()] (fused4 classes only)
+  td32api::ClassTables t32;     // fp32 tables (td_set_precision(TD_PREC_F32); classes the fp32 kernels serve)
+  bool has32 = false;
 };
 
 struct DevGuard {
@@ -70,6 +76,7 @@ struct td_handle {
   std::vector<SegHost> segs;
   std::vector<ClassInfo> classes;
   int path = TD_PATH_AUTO, fft_variant = 0, last_path = 0, last_launches = 0;
+  int precision = TD_PREC_F64;
   int max_n = 0;
   // staged workspace: U / Z sized by td_create (two lanes of an L2-resident chunk), the per-block partial sums by
   // td_create / td_reserve (a batch larger than they hold is processed in sub-batches)
@@ -95,12 +102,6 @@ struct td_handle {
   bool last_valid = false, touched = false;
 };
 
-#define CK(call)                                                                               \
-  do {                                                                                         \
-    cudaError_t e_ = (call);                                                                   \
-    if (e_ != cudaSuccess) return e_ == cudaErrorMemoryAllocation ? TD_ENOMEM : TD_ECUDA;      \
-  } while (0)
-
 #ifdef TD_DEBUG_KNOBS
 // experiment knobs of debug builds (_work probes); the product build compiles the defaults in
 static int g_tune[16] = {-1, -1, -1, -1, -1, -1, -1, -1, -1, -1, -1, -1, -1, -1, -1, -1};
@@ -114,27 +115,10 @@ namespace {
 
 int next_log2(int n) { int l = 0; while ((1 << l) < n) ++l; return l; }
 
-// One-time launch configuration per (kernel instantiation, device): the dynamic shared-memory attribute and the
-// occupancy query run on the first use only; td_create makes that first use (a "dry" pass over every kernel its size
-// classes can reach), so a batch call contains nothing but launches.  `cache` is the caller's function-local static.
-constexpr int TD_MAX_DEV = 64;
-template <class K>
-td_status kernel_config(K kern, int nt, size_t smem_attr, size_t smem, int device, int* cache, int* blocks_per_sm) {
-  if (device < 0 || device >= TD_MAX_DEV) return TD_EUNSUPPORTED;
-  if (cache[device] == 0) {
-    if (smem_attr > 48 * 1024) CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_attr));
-    int nb = 0;
-    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kern, nt, smem));
-    cache[device] = nb + 1;
-  }
-  *blocks_per_sm = cache[device] - 1;
-  return TD_OK;
-}
-
 void free_handle(td_handle* h) {
   if (!h) return;
   for (auto& s : h->segs) { cudaFree(s.a); cudaFree(s.G); cudaFree(s.Gp); cudaFree(s.zd); }
-  for (auto& c : h->classes) { cudaFree(c.T); cudaFree(c.d_segs); cudaFree(c.d_Gp); }
+  for (auto& c : h->classes) { cudaFree(c.T); cudaFree(c.d_segs); cudaFree(c.d_Gp); if (c.has32) td32api::free_class(&c.t32); }
   cudaFree(h->wsU); cudaFree(h->wsZ); cudaFree(h->wsPartial); cudaFree(h->wsDot); cudaFree(h->ud); cudaFree(h->synH); cudaFree(h->synP); cudaFree(h->synSeg);
   cudaFree(h->hsD); cudaFree(h->hsH[0]); cudaFree(h->hsH[1]); cudaFree(h->hsOut);
   if (h->copy_stream) cudaStreamDestroy(h->copy_stream);
@@ -316,7 +300,7 @@ td_status run_staged_sub(td_handle* h, const ClassInfo& cls, const SegHost& sg, 
     cplx* Z = h->wsZ + (two && lane ? zh : 0);
     StagedParams P;
     P.d = d; P.H = H ? H + b0 * ldh : nullptr; P.ldh = ldh; P.CB = cb;
-    P.seg.off = sg.off; P.seg.n = sg.n; P.seg._pad = 0; P.seg.G = sg.G; P.seg.zd = sg.zd;
+    P.seg.off = sg.off; P.seg.n = sg.n; P.seg._pad = 0; P.seg.G = sg.G; P.seg.zd = sg.zd; P.seg.rscale = 1.0;
     P.M = M; P.U = U; P.Z = Z; P.T = cls.T; P.partial = h->wsPartial + (size_t)b0 * nblk * 2; P.nblk = nblk;
     s = launch_first<MODE>(rF, dim3((nf / rF + LG_NT - 1) / LG_NT, cb), P, ls);
     if (s != TD_OK) break;
@@ -543,12 +527,22 @@ td_status launch_dense(td_handle* h, const std::vector<DenseSeg>& segs, const do
 }
 
 // FFT path over all size classes.  MODE_LOGLIKE: out0 = loglike.  MODE_INNER: out0 = <d,h>, out1 = <h,h>.
+// `f32`: classes that have fp32 tables and are not served by the dense kernel run the fp32 build of their kernel
 template <int MODE>
 td_status run_fft_path(td_handle* h, const double* d, const double* H, int64_t ldh, int64_t B, double* out0,
-                       double* out1, cudaStream_t st, bool skip_dense_classes = false, int accumulate = 0) {
+                       double* out1, cudaStream_t st, bool skip_dense_classes = false, int accumulate = 0, bool f32 = false) {
   const double sc0 = (MODE == MODE_LOGLIKE) ? -0.5 : 1.0, sc1 = 1.0;
   for (const ClassInfo& cls : h->classes) {
     if (skip_dense_classes && class_is_dense(h, cls)) continue;
+    if (f32 && cls.has32 && class_is_fused(h, cls) && !class_is_dense(h, cls)) {
+      td32api::Launch L;
+      L.d = d; L.H = H; L.ldh = ldh; L.B = B; L.out0 = out0; L.out1 = out1; L.accumulate = accumulate; L.mode = MODE;
+      td_status s = td32api::launch(cls.t32, L, h->num_sms, h->device, st, false);
+      if (s != TD_OK) return s;
+      ++h->last_launches;
+      accumulate = 1;
+      continue;
+    }
     if (class_is_fused(h, cls)) {
       FusedParams P;
       P.d = d; P.H = H; P.ldh = ldh; P.B = B; P.out0 = out0; P.out1 = out1;
@@ -585,7 +579,7 @@ td_status run_batch(td_handle* h, const double* d, const double* H, int64_t ldh,
   }
   h->last_path = (nd == h->n_seg) ? TD_PATH_DENSE : TD_PATH_FFT;
   if (nd == h->n_seg) return TD_OK;
-  return run_fft_path<MODE>(h, d, H, ldh, B, out0, out1, st, true, accumulate);
+  return run_fft_path<MODE>(h, d, H, ldh, B, out0, out1, st, true, accumulate, h->precision == TD_PREC_F32);
 }
 
 // <d, h_b> = u . h_b with u = C^{-1} d (td_dot.cuh); z of the data vector is already in every segment's zd
@@ -686,7 +680,7 @@ static td_status create_impl(td_handle* h, const double* acf, const int64_t* seg
   int64_t off = 0;
   for (int s = 0; s < n_seg; ++s) {
     SegHost& sg = h->segs[s];
-    sg.off = off; sg.n = (int)seg_lengths[s];
+    sg.off = off; sg.n = (int)seg_lengths[s]; sg.rho0 = acf[off];
     sg.log2M = std::max(FUSED_MIN_LOG2M, next_log2(sg.n));
     off += sg.n;
     h->max_n = std::max(h->max_n, sg.n);
@@ -785,7 +779,7 @@ static td_status create_impl(td_handle* h, const double* acf, const int64_t* seg
     std::vector<SegDev> sd(c.seg_ids.size());
     for (size_t i = 0; i < sd.size(); ++i) {
       const SegHost& sg = h->segs[c.seg_ids[i]];
-      sd[i].off = sg.off; sd[i].n = sg.n; sd[i]._pad = 0; sd[i].G = sg.G; sd[i].zd = sg.zd;
+      sd[i].off = sg.off; sd[i].n = sg.n; sd[i]._pad = 0; sd[i].G = sg.G; sd[i].zd = sg.zd; sd[i].rscale = 1.0;
     }
     CK(cudaMalloc(&c.d_segs, sizeof(SegDev) * sd.size()));
     CK(cudaMemcpy(c.d_segs, sd.data(), sizeof(SegDev) * sd.size(), cudaMemcpyHostToDevice));
@@ -1047,10 +1041,13 @@ td_status td_inner_batch(td_handle* h, const double* d, const double* H, int64_t
   if (s != TD_OK) return s;
   h->touched = true;  // z of the data vector (and u on the dot path) live in the handle
   // z of the data vector, once per call (per segment), then the bilinear sums against it
-  s = run_fft_path<MODE_STOREZ>(h, d, nullptr, h->n_tot, 1, nullptr, nullptr, st);
+  // only the cross term is wanted: one streaming pass over H against the cached weights u = C^{-1} d (fp64 in both
+  // precisions: the pass is HBM-bound, and u needs the fp64 z of the data vector)
+  const bool use_dot = out_dh && !out_hh && h->path == TD_PATH_AUTO && h->max_n <= DOT_MAX_N && h->n_tot <= 0x7fffffff;
+  s = run_fft_path<MODE_STOREZ>(h, d, nullptr, h->n_tot, 1, nullptr, nullptr, st, false, 0,
+                                h->precision == TD_PREC_F32 && !use_dot);
   if (s == TD_OK) {
-    // only the cross term is wanted: one streaming pass over H against the cached weights u = C^{-1} d
-    if (out_dh && !out_hh && h->path == TD_PATH_AUTO && h->max_n <= DOT_MAX_N && h->n_tot <= 0x7fffffff)
+    if (use_dot)
       s = run_dot(h, H, ldh, B, out_dh, st);
     else
       s = run_batch<MODE_INNER>(h, d, H, ldh, B, out_dh, out_hh, st);
@@ -1075,6 +1072,37 @@ td_status td_set_fft_variant(td_handle* h, int variant) {
     if (a != TD_OK) return a;
   }
   h->fft_variant = variant;
+  return TD_OK;
+}
+
+td_status td_set_precision(td_handle* h, int precision) {
+  if (!h || (precision != TD_PREC_F64 && precision != TD_PREC_F32)) return TD_EINVAL;
+  if (precision == TD_PREC_F32) {
+    DevGuard guard(h->device);
+    if (!guard.ok) return TD_ECUDA;
+    bool any = false;
+    for (ClassInfo& c : h->classes) {
+      if (!td32api::supported(c.log2M)) continue;
+      any = true;
+      if (c.has32) continue;
+      std::vector<td32api::SegIn> in(c.seg_ids.size());
+      for (size_t i = 0; i < in.size(); ++i) {
+        const SegHost& sg = h->segs[c.seg_ids[i]];
+        in[i].off = sg.off; in[i].n = sg.n; in[i].Gp64 = sg.Gp; in[i].rho0 = sg.rho0;
+      }
+      td_status s = td32api::build_class(c.log2M, (int)in.size(), in.data(), c.T, &c.t32);
+      if (s != TD_OK) return s;
+      c.has32 = true;
+      for (int mode = 0; mode < 3; ++mode) {  // dry pass: attributes and occupancy of the fp32 kernels
+        td32api::Launch L = {};
+        L.B = 1; L.mode = mode;
+        s = td32api::launch(c.t32, L, h->num_sms, h->device, nullptr, true);
+        if (s != TD_OK) return s;
+      }
+    }
+    if (!any) return TD_EUNSUPPORTED;  // no size class of this handle has an fp32 kernel
+  }
+  h->precision = precision;
   return TD_OK;
 }
 

@@ -1,0 +1,152 @@
+// tdlike_f32.cu - the fused FFT-path kernels compiled with real = float (namespace td32): the FP32 evaluation mode
+// (SURVEY.md 8(f) NEXT-2; PAPER.md:268 "FP32 is sufficient ...", :322-324 III.C.3 "carry out all the analysis with FP32
+// with appropriate normalization ... operators should be precomputed in FP64").  Setup (Levinson-Durbin, generator
+// spectra, twiddles) stays in fp64 in tdlike.cu; this unit rounds those tables once and runs S1-S5 in fp32:
+//   S1  r = (d - h) rho_0^(-1/2) is formed in fp64 from the fp64 inputs and rounded once (normalisation by rho_0);
+//   S2-S4 in fp32 (the same kernels, butterflies, plans and TMEM constant cache as the fp64 build);
+//   S5  per-thread sums of squares in fp32, warp / CTA / segment sums in fp64.
+#define TD_F32 1
+#include "td_f32.h"
+#include "td_host.h"
+
+#include <algorithm>
+#include <vector>
+
+#include "td_cluster.cuh"
+#include "td_fused4.cuh"
+
+using namespace td32;
+using namespace tdhost;
+
+namespace {
+
+__global__ void cvt_cplx_kernel(const double2* __restrict__ src, float2* __restrict__ dst, size_t n, double scale) {
+  const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) dst[i] = make_float2((float)(src[i].x * scale), (float)(src[i].y * scale));
+}
+
+template <int LOG2M, int MODE>
+td_status launch_fused4(const td32api::ClassTables& t, const FusedParams& P, int num_sms, int device, cudaStream_t st, bool dry) {
+  auto kern = td_fused4_kernel<LOG2M, MODE>;
+  constexpr int NT = Fused4Shape<LOG2M>::NT;
+  const size_t smem = Fused4Shape<LOG2M>::smem_bytes();
+  static int cache[TD_MAX_DEV];
+  int nb = 0;
+  td_status cs = kernel_config(kern, NT, smem, smem, device, cache, &nb);
+  if (cs != TD_OK) return cs;
+  if (nb < 1) return TD_EUNSUPPORTED;
+  if (dry) return TD_OK;
+  nb = std::min(nb, 512 / Fused4Shape<LOG2M>::TMEM_COLS);  // co-resident CTAs share the SM's 512 tensor-memory columns
+  const long long maxg = (long long)nb * num_sms;
+  const int grid = (int)std::max<long long>(1, std::min<long long>(MODE == MODE_STOREZ ? 1 : P.B, maxg));
+  Fused4Params P4;
+  P4.base = P; P4.Gp = reinterpret_cast<const cplx* const*>(t.Gp_ptrs);
+  kern<<<grid, NT, smem, st>>>(P4);
+  CK(cudaGetLastError());
+  return TD_OK;
+}
+
+template <int MODE>
+td_status launch_cluster(const td32api::ClassTables& t, const FusedParams& P, int num_sms, int device, cudaStream_t st, bool dry) {
+  auto kern = td_cluster_kernel<MODE>;
+  const size_t smem = ClusterShape::smem_bytes();
+  static int cache[TD_MAX_DEV];  // 0 = not configured on this device yet, else 1 + clusters that can be co-resident
+  if (device < 0 || device >= TD_MAX_DEV) return TD_EUNSUPPORTED;
+  cudaLaunchConfig_t cfg = {};
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeClusterDimension;
+  attr[0].val.clusterDim.x = 2; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+  cfg.blockDim = dim3(ClusterShape::NT); cfg.dynamicSmemBytes = smem; cfg.stream = st;
+  cfg.attrs = attr; cfg.numAttrs = 1;
+  if (cache[device] == 0) {
+    CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    cfg.gridDim = dim3(2 * (num_sms / 2));
+    int n = 0;
+    CK(cudaOccupancyMaxActiveClusters(&n, kern, &cfg));
+    cache[device] = n + 1;
+  }
+  const int ncl = cache[device] - 1;
+  if (ncl < 1) return TD_EUNSUPPORTED;
+  if (dry) return TD_OK;
+  const long long want = MODE == MODE_STOREZ ? 1 : P.B;
+  cfg.gridDim = dim3(2 * (unsigned)std::max<long long>(1, std::min<long long>(want, ncl)));
+  Fused4Params P4;
+  P4.base = P; P4.Gp = reinterpret_cast<const cplx* const*>(t.Gp_ptrs);
+  CK(cudaLaunchKernelEx(&cfg, kern, P4));
+  return TD_OK;
+}
+
+template <int MODE>
+td_status launch_mode(const td32api::ClassTables& t, const FusedParams& P, int num_sms, int device, cudaStream_t st, bool dry) {
+  switch (t.log2M) {
+    case 10: return launch_fused4<10, MODE>(t, P, num_sms, device, st, dry);
+    case 11: return launch_fused4<11, MODE>(t, P, num_sms, device, st, dry);
+    case 12: return launch_fused4<12, MODE>(t, P, num_sms, device, st, dry);
+    case 13: return launch_cluster<MODE>(t, P, num_sms, device, st, dry);
+    default: return TD_EUNSUPPORTED;
+  }
+}
+
+}  // namespace
+
+namespace td32api {
+
+void free_class(ClassTables* t) {
+  if (!t) return;
+  cudaFree(t->T); cudaFree(t->segs); cudaFree(t->Gp_ptrs);
+  for (int s = 0; s < t->n_seg; ++s) {
+    if (t->Gp) cudaFree(t->Gp[s]);
+    if (t->zd) cudaFree(t->zd[s]);
+  }
+  delete[] t->Gp; delete[] t->zd;
+  *t = ClassTables();
+}
+
+td_status build_class(int log2M, int n_seg, const SegIn* segs, const void* T64, ClassTables* out) {
+  if (!supported(log2M) || n_seg < 1 || !segs || !T64 || !out) return TD_EINVAL;
+  ClassTables t;
+  t.log2M = log2M; t.n_seg = n_seg;
+  t.Gp = new (std::nothrow) void*[n_seg]();
+  t.zd = new (std::nothrow) void*[n_seg]();
+  if (!t.Gp || !t.zd) { free_class(&t); return TD_ENOMEM; }
+  const size_t M = (size_t)1 << log2M, TW = 2 * M, gp_elems = 2 * (size_t)SmemArr::padded((int)M);
+  auto fail = [&](td_status s) { free_class(&t); return s; };
+  if (cudaMalloc(&t.T, sizeof(float2) * TW) != cudaSuccess) return fail(TD_ENOMEM);
+  cvt_cplx_kernel<<<(unsigned)((TW + 255) / 256), 256>>>(static_cast<const double2*>(T64), static_cast<float2*>(t.T), TW, 1.0);
+  std::vector<SegDev> sd(n_seg);
+  std::vector<const cplx*> gp(n_seg);
+  for (int s = 0; s < n_seg; ++s) {
+    if (!(segs[s].rho0 > 0.0)) return fail(TD_ENOTSPD);
+    if (cudaMalloc(&t.Gp[s], sizeof(float2) * gp_elems) != cudaSuccess) return fail(TD_ENOMEM);
+    if (cudaMalloc(&t.zd[s], sizeof(float2) * M) != cudaSuccess) return fail(TD_ENOMEM);
+    cvt_cplx_kernel<<<(unsigned)((gp_elems + 255) / 256), 256>>>(static_cast<const double2*>(segs[s].Gp64),
+                                                                 static_cast<float2*>(t.Gp[s]), gp_elems, sqrt(segs[s].rho0));
+    sd[s].off = segs[s].off; sd[s].n = segs[s].n; sd[s]._pad = 0; sd[s].G = nullptr;
+    sd[s].zd = static_cast<cplx*>(t.zd[s]); sd[s].rscale = 1.0 / sqrt(segs[s].rho0);
+    gp[s] = static_cast<const cplx*>(t.Gp[s]);
+  }
+  if (cudaGetLastError() != cudaSuccess) return fail(TD_ECUDA);
+  if (cudaMalloc(&t.segs, sizeof(SegDev) * n_seg) != cudaSuccess || cudaMalloc(&t.Gp_ptrs, sizeof(cplx*) * n_seg) != cudaSuccess)
+    return fail(TD_ENOMEM);
+  if (cudaMemcpy(t.segs, sd.data(), sizeof(SegDev) * n_seg, cudaMemcpyHostToDevice) != cudaSuccess ||
+      cudaMemcpy(t.Gp_ptrs, gp.data(), sizeof(cplx*) * n_seg, cudaMemcpyHostToDevice) != cudaSuccess ||
+      cudaDeviceSynchronize() != cudaSuccess)
+    return fail(TD_ECUDA);
+  *out = t;
+  return TD_OK;
+}
+
+td_status launch(const ClassTables& t, const Launch& L, int num_sms, int device, cudaStream_t st, bool dry) {
+  FusedParams P;
+  P.d = L.d; P.H = L.H; P.ldh = L.ldh; P.B = L.B; P.out0 = L.out0; P.out1 = L.out1;
+  P.segs = static_cast<const SegDev*>(t.segs); P.n_seg = t.n_seg; P.accumulate = L.accumulate;
+  P.T = static_cast<const cplx*>(t.T);
+  switch (L.mode) {
+    case MODE_LOGLIKE: return launch_mode<MODE_LOGLIKE>(t, P, num_sms, device, st, dry);
+    case MODE_INNER: return launch_mode<MODE_INNER>(t, P, num_sms, device, st, dry);
+    case MODE_STOREZ: return launch_mode<MODE_STOREZ>(t, P, num_sms, device, st, dry);
+    default: return TD_EINVAL;
+  }
+}
+
+}  // namespace td32api

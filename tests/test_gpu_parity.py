@@ -699,3 +699,93 @@ def test_family_host_entry_with_odd_batch_keeps_rows_aligned():
         assert np.array_equal(out_host, out_dev)
         H = OT.family_rows(w.family, w.params, w.seg_lengths, w.fs)
         _assert_close(out_host, O.loglike_batch(w.acf, w.seg_lengths, w.d, H), what=f"{name} odd B")
+
+
+# ------------------------------------------------------------------ FP32 evaluation with FP64 setup
+# Tolerance against the SAME fp64 oracle: |dQ|/Q <= 4 (log2(2M) + 1) eps32 kappa, eps32 = 2^-24,
+# kappa = (|y1|^2 + |y2|^2) / (|y1|^2 - |y2|^2) >= 1 the cancellation factor of the Gohberg-Semencul difference
+# (1.003 .. 1.05 on c1-c5, measured with the oracle's time-domain GS route).  At 2M = 16384 and kappa <= 5: 1.8e-5.
+TOL32 = 2e-5
+
+
+@pytest.mark.parametrize("name,B,n_scale", [("c1", 64, 1), ("c2", 96, 1), ("c3", 24, 1), ("c5", 16, 1)])
+def test_f32_evaluation_matches_the_fp64_oracle(name, B, n_scale):
+    w = W.make(name, B=B, n_scale=n_scale)
+    ref = O.loglike_batch(w.acf, w.seg_lengths, w.d, w.H)
+    dh_ref, hh_ref = O.inner_batch(w.acf, w.seg_lengths, w.d, w.H)
+    with tdb.TDLikelihood(w.acf, w.seg_lengths) as h:
+        d, H = _dev(w.d), _dev(w.H)
+        o64 = h.loglike_batch(d, H).clone()
+        h.set_precision(tdb.TD_PREC_F32)
+        o32 = h.loglike_batch(d, H).clone()
+        o32b = h.loglike_batch(d, H).clone()
+        dh, hh = h.inner_batch(d, H)                      # fp32 STOREZ + INNER kernels
+        dh_only, _ = h.inner_batch(d, H, want_hh=False)   # the dot path stays fp64
+        path_dot = h.info()["last_path"]
+        h.set_precision(tdb.TD_PREC_F64)
+        o64b = h.loglike_batch(d, H)
+        torch.cuda.synchronize()
+    e32 = _assert_close(o32.cpu().numpy(), ref, tol=TOL32, what=f"{name} f32")
+    assert e32 > 1e-12, "the fp32 build was not used"            # an fp64 result would sit at 1e-14
+    assert torch.equal(o32, o32b)                                 # deterministic
+    assert torch.equal(o64, o64b)                                 # switching back restores the fp64 kernels bit for bit
+    _assert_close(o64.cpu().numpy(), ref, what=f"{name} f64 beside it")
+    scale = np.abs(hh_ref) + np.abs(dh_ref) + 1.0
+    assert np.max(np.abs(hh.cpu().numpy() - hh_ref) / scale) <= TOL32
+    assert np.max(np.abs(dh.cpu().numpy() - dh_ref) / scale) <= TOL32
+    assert path_dot == tdb.TD_PATH_DOT
+    assert np.max(np.abs(dh_only.cpu().numpy() - dh_ref) / scale) <= TOL
+
+
+def test_f32_edges_exact_zero_nan_unsupported_and_mixed_classes():
+    # h = d gives exactly 0 (the residual is formed in fp64 before rounding); a NaN row stays confined to its output
+    w = W.make("c2", B=6, n_scale=2)
+    H = w.H.copy()
+    H[1] = w.d
+    H[3, 17] = np.nan
+    ref = O.loglike_batch(w.acf, w.seg_lengths, w.d, np.nan_to_num(H))
+    with tdb.TDLikelihood(w.acf, w.seg_lengths) as h:
+        h.set_precision(tdb.TD_PREC_F32)
+        out = h.loglike_batch(_dev(w.d), _dev(H)).cpu().numpy()
+    assert out[1] == 0.0 and np.isnan(out[3])
+    keep = [0, 2, 4, 5]
+    _assert_close(out[keep], ref[keep], tol=TOL32, what="f32 edges")
+    # a handle whose only segment is short (dense / small fused kernels): no fp32 kernel -> EUNSUPPORTED, setting unchanged
+    w = W.make("d3", B=32)
+    with tdb.TDLikelihood(w.acf, w.seg_lengths) as h:
+        with pytest.raises(tdb.TDError) as e:
+            h.set_precision(tdb.TD_PREC_F32)
+        assert e.value.status == tdb.TD_EUNSUPPORTED
+        with pytest.raises(tdb.TDError):
+            h.set_precision(7)
+        out = h.loglike_batch(_dev(w.d), _dev(w.H)).cpu().numpy()
+    _assert_close(out, O.loglike_batch(w.acf, w.seg_lengths, w.d, w.H), what="d3 after a refused precision switch")
+    # mixed size classes: 3000 (fp32 fused kernel), 300 (dense, fp64), 5000 (fp32 cluster kernel), odd offsets
+    rng = np.random.default_rng(5)
+    lens = [3001, 300, 5000]
+    acf = np.concatenate([W.acf_from_psd(4096.0, 2 * n, n) * s for n, s in zip(lens, (1.0, 0.7, 1.9))])
+    d = rng.standard_normal(sum(lens)) * 1e-21
+    Hm = rng.standard_normal((9, sum(lens))) * 1e-21
+    ref = O.loglike_batch(acf, lens, d, Hm)
+    with tdb.TDLikelihood(acf, lens) as h:
+        h.set_precision(tdb.TD_PREC_F32)
+        out = h.loglike_batch(_dev(d), _dev(Hm)).cpu().numpy()
+    _assert_close(out, ref, tol=TOL32, what="f32 mixed classes")
+
+
+@pytest.mark.parametrize("name", ["c2", "c5"])
+def test_f32_full_size_against_the_fp64_path(name):
+    """Full batch in the launch configuration bench.py --dtype f32 times: every row against the fp64 GPU result (itself
+    held to 1e-9 against the oracle by test_full_size_*), a sample of rows against the oracle directly."""
+    w = W.make(name)
+    with tdb.TDLikelihood(w.acf, w.seg_lengths) as h:
+        d, H = _dev(w.d), _dev(w.H)
+        o64 = h.loglike_batch(d, H).cpu().numpy()
+        h.set_precision(tdb.TD_PREC_F32)
+        o32 = h.loglike_batch(d, H).cpu().numpy()
+    err = np.abs(o32 - o64) / np.maximum(np.abs(o64), 1.0)
+    assert err.max() <= TOL32, f"{name}: {err.max():.2e}"
+    idx = np.linspace(0, w.B - 1, 12).astype(int)
+    ref = O.loglike_batch(w.acf, w.seg_lengths, w.d, w.H[idx])
+    _assert_close(o32[idx], ref, tol=TOL32, what=f"{name} f32 full size")
+    print(f"{name}: fp32 vs fp64 over {w.B} rows: max {err.max():.2e}, median {np.median(err):.2e}")

@@ -439,3 +439,29 @@ def test_not_spd_is_rejected():
         O.cholesky_lower(rho)
     with pytest.raises(np.linalg.LinAlgError):
         O.levinson_durbin(rho)
+
+
+# ---------------------------------------------------------------- P19 AR(p) closed form (the long-N oracle route)
+@pytest.mark.parametrize("phi", [[0.9], [1.6, -0.8], [0.5, -0.3, 0.1], [1.9, -0.95]])
+def test_p19_ar_closed_form_against_cholesky_route(phi):
+    """ar_acf / ar_quadform_closed (used at N = 2^20, where nothing else finishes) against the dense Cholesky route,
+    the Levinson recursion (a = (1, -phi_1, .., -phi_p, 0, ..), v = s2) and, for p = 1, the hand-derived tridiagonal
+    form of P3.  A dropped lag, a wrong sign in the Yule-Walker system or a shifted innovation window fails here."""
+    rng = np.random.default_rng(19)
+    n, s2 = 300, 0.37
+    rho = O.ar_acf(phi, s2, n)
+    p = len(phi)
+    # Yule-Walker beyond the solved block, and positive definiteness
+    for k in (p + 1, p + 5, n - 1):
+        assert abs(rho[k] - sum(phi[j] * rho[k - 1 - j] for j in range(p))) < 1e-12 * rho[0]
+    x = rng.standard_normal(n)
+    q = O.ar_quadform_closed(phi, s2, x)
+    assert _rel(O.quadform(rho, x), q) < 1e-9
+    a, v, logdet, kap, E = O.levinson_durbin(rho)
+    expect = np.zeros(n)
+    expect[0] = 1.0
+    expect[1 : p + 1] = -np.asarray(phi)
+    assert np.max(np.abs(a - expect)) < 1e-8 and _rel(v, s2) < 1e-9
+    if p == 1:
+        assert _rel(_ar1_closed(phi[0], s2, x), q) < 1e-12
+        assert np.max(np.abs(rho - s2 * phi[0] ** np.arange(n) / (1 - phi[0] ** 2))) < 1e-12
