@@ -162,7 +162,7 @@ def main():
     ap.add_argument("--config", default="c2")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--B", type=int, default=None, help="override templates per GPU (default: the config's B)")
-    ap.add_argument("--path", type=int, default=0, help="0 auto, 1 FFT, 2 dense")
+    ap.add_argument("--path", type=int, default=0, help="0 auto, 1 FFT, 2 dense (Gohberg-Semencul), 4 CDO (cached L^-1)")
     ap.add_argument("--fft-variant", type=int, default=0)
     ap.add_argument("--op", default="loglike", choices=["loglike", "dh"],
                     help="loglike: the headline hot path; dh: only the cross term <d|h_b> (td_inner_batch, out_hh = NULL)")
@@ -339,8 +339,10 @@ def main():
     # ---------------- rooflines (dominant kernel = the one kernel of the step on the fused path)
     peaks, peaks_kind = measured_peaks()
     kern_ms = float(np.mean(step_ms))
-    dense = path_used == 2
-    falg = float(sum(2.0 * int(n) * int(n) for n in w.seg_lengths)) if dense else alg_flops_per_eval(w.seg_lengths)
+    dense = path_used in (2, 4)
+    cdo = path_used == 4   # triangular W = L^-1 contraction: N^2 flop per template and segment (half of the GS dense path)
+    falg = (float(sum((1.0 if cdo else 2.0) * int(n) * int(n) for n in w.seg_lengths)) if dense
+            else alg_flops_per_eval(w.seg_lengths))
     f32 = args.dtype == "f32"
     probe = {"dfma": tdb.probe_throughput(0, local), "dmma": tdb.probe_throughput(1, local)}
     if f32:
@@ -363,7 +365,7 @@ def main():
                 # fraction against the DFMA register loop measured in THIS run (state both denominators)
                 "frac_vs_measured_loop": ach_tf / probe["ffma_fp32" if f32 else "dfma"],
                 "traffic": traffic, "traffic_source": traffic_source,
-                "kernel": "td_dense_kernel" if dense else DOMINANT.get(args.config, "td_fused_kernel") + (" (fp32 build)" if f32 else ""),
+                "kernel": ("td_cdo_kernel" if cdo else "td_dense_kernel") if dense else DOMINANT.get(args.config, "td_fused_kernel") + (" (fp32 build)" if f32 else ""),
                 "measured_register_loop_tflops": probe,
                 "kernel_ms": kern_ms, "alg_flops_per_eval": falg,
                 "peak_source": ("derived: 128 FFMA/clk/SM x 148 SM x 1.965 GHz x 2; the FFMA register loop of this run beside it"
@@ -402,7 +404,7 @@ def main():
             "config": {"workload": f"{args.config}: {w.description}; N_tot={n_tot}, segments={list(map(int, w.seg_lengths))}, "
                                    + (f"B={B_job} sharded over {world} GPUs (rank 0: {B})" if args.scaling == "strong" and world > 1
                                       else f"B={B} per GPU"),
-                       "path": {1: "fft", 2: "dense", 3: "dot"}.get(path_used, "?"),
+                       "path": {1: "fft", 2: "dense", 3: "dot", 4: "cdo"}.get(path_used, "?"),
                        "l2": f"{nbuf} distinct device copies of H rotated between steps (H = {8 * B * n_tot / 2**20:.0f} MiB each)",
                        "parallelism": f"dp{world} over templates",
                        "setup_ms_not_in_metric": round(1e3 * t_setup, 3)},

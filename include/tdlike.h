@@ -50,7 +50,12 @@ typedef enum {
  * TD_PATH_AUTO: per size class, the dense path for short segments (measured crossover, DESIGN.md
  * 6.4), the FFT path otherwise; both accumulate into the same outputs within one call. */
 enum { TD_PATH_AUTO = 0, TD_PATH_FFT = 1, TD_PATH_DENSE = 2,
-       TD_PATH_DOT = 3 /* reported by td_get_info only: <d,h_b> evaluated as u . h_b, u = C^{-1} d */ };
+       TD_PATH_DOT = 3, /* reported by td_get_info only: <d,h_b> evaluated as u . h_b, u = C^{-1} d */
+       TD_PATH_CDO = 4  /* td_loglike_batch as the batched triangular contraction Y = L^{-1} X with the cached whitening
+                           operator (the paper's "CDO" route): never chosen by AUTO (measured against
+                           the Gohberg-Semencul dense path in profiles/r02_cdo.md); segments up to 1024 samples; the
+                           first td_set_path(TD_PATH_CDO) builds L^{-1} (8 N^2 bytes per segment); td_inner_batch
+                           keeps using the dense path */ };
 
 /* td_create - one-time setup (PAPER.md:215 "done once ... cached"; :241-246 Eq. 14 generator).
  *   acf          HOST pointer, sum_s seg_lengths[s] doubles: per-segment autocorrelation
@@ -145,8 +150,8 @@ td_status td_loglike_family_batch_host(td_handle* h, const double* d, int family
 td_status td_reserve(td_handle* h, int64_t B_max);
 
 /* td_set_path - force the evaluation path for subsequent calls (TD_PATH_AUTO restores the
- * chooser).  TD_PATH_DENSE on a handle with a segment longer than the dense path supports
- * returns TD_EUNSUPPORTED and leaves the setting unchanged. */
+ * chooser).  TD_PATH_DENSE / TD_PATH_CDO on a handle with a segment longer than the dense paths support
+ * (1024 samples) return TD_EUNSUPPORTED and leave the setting unchanged. */
 td_status td_set_path(td_handle* h, int path);
 
 /* td_set_fft_variant - which implementation serves the FFT path: 0 = automatic (fused

@@ -16,7 +16,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "lib", "libtdlike.so")
 
 TD_OK, TD_EINVAL, TD_ENOTSPD, TD_ENOMEM, TD_ECUDA, TD_EUNSUPPORTED = range(6)
-TD_PATH_AUTO, TD_PATH_FFT, TD_PATH_DENSE, TD_PATH_DOT = 0, 1, 2, 3
+TD_PATH_AUTO, TD_PATH_FFT, TD_PATH_DENSE, TD_PATH_DOT, TD_PATH_CDO = 0, 1, 2, 3, 4
 TD_FAMILY_RINGDOWN, TD_FAMILY_SINE_GAUSSIAN, TD_FAMILY_CHIRP = 0, 1, 2
 TD_PREC_F64, TD_PREC_F32 = 0, 1
 

@@ -62,7 +62,8 @@ struct DenseState {
   int max_n = 0;             // longest segment the dense path accepts (0: unavailable)
   int auto_n = 0;            // AUTO takes the dense path for size classes whose segments are all <= auto_n
   std::vector<DenseSeg> all;   // every segment (forced dense path); empty if some segment is too long
-  std::vector<DenseSeg> aut;   // the segments AUTO sends to the dense path
+  std::vector<DenseSeg> aut;   // the segments AUTO sends to the dense paths
+  std::vector<DenseSeg> aut_gs;  // of those, the ones whose log-likelihood stays on this kernel (the rest: td_cdo.cuh)
 };
 
 __host__ __device__ inline int dense_nwr(int max_npad) {

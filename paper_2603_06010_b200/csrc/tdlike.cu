@@ -14,6 +14,7 @@
 #include "td_host.h"
 #include "td_f32.h"
 #include "td_dense.cuh"
+#include "td_cdo.cuh"
 #include "td_dot.cuh"
 #include "td_fused.cuh"
 #include "td_cluster.cuh"
@@ -31,7 +32,9 @@ constexpr int FUSED_MIN_LOG2M = 8;   // M = 256
 // one-CTA fused kernels: M = 256..4096 (2M = 8192-point transform, 204 KiB of shared memory at M = 4096)
 constexpr int CLUSTER_LOG2M = 13;    // M = 8192: 2-CTA cluster, one branch per CTA (td_cluster.cuh)
 constexpr int FUSED_NT = 256;
-constexpr int DENSE_AUTO_N = 512;     // AUTO: dense path for segments up to this length (measured crossover: profiles/r01_chooser.md)
+constexpr int DENSE_AUTO_N = 512;     // AUTO: dense paths for segments up to this length (measured crossover: profiles/r01_chooser.md)
+constexpr int CDO_AUTO_MIN_N = 65;    // AUTO, log-likelihood: cached-L^-1 contraction from this length up, the Gohberg-Semencul
+                                      // dense kernel below (measured: profiles/r02_cdo.md; 0.95x at N = 64, 1.08-1.55x above)
 constexpr size_t STAGED_WS_BYTES = 96ull << 20;  // staged workspace, both lanes: inside the 126 MB L2 (measured 64: 0.91 ms, 96: 0.756, 128: 0.761, 192: 0.745, 384: 0.750 on c4)
 
 struct SegHost {
@@ -89,6 +92,9 @@ struct td_handle {
   size_t wsU_elems = 0, wsZ_elems = 0, wsP_elems = 0;
   // dense path state
   DenseState dense;
+  // CDO path (td_cdo.cuh): device copy of the ACFs (kept for the whitening-operator setup), one W per segment (lazy)
+  double* d_rho = nullptr;
+  std::vector<double*> cdoW;
   // host-buffer entry point: staging (grow-only), copy stream, events
   double* hsD = nullptr; double* hsH[2] = {nullptr, nullptr}; double* hsOut = nullptr;
   size_t hsH_elems = 0, hsOut_elems = 0;
@@ -121,6 +127,8 @@ void free_handle(td_handle* h) {
   for (auto& c : h->classes) { cudaFree(c.T); cudaFree(c.d_segs); cudaFree(c.d_Gp); if (c.has32) td32api::free_class(&c.t32); }
   cudaFree(h->wsU); cudaFree(h->wsZ); cudaFree(h->wsPartial); cudaFree(h->wsDot); cudaFree(h->ud); cudaFree(h->synH); cudaFree(h->synP); cudaFree(h->synSeg);
   cudaFree(h->hsD); cudaFree(h->hsH[0]); cudaFree(h->hsH[1]); cudaFree(h->hsOut);
+  cudaFree(h->d_rho);
+  for (double* w : h->cdoW) cudaFree(w);
   if (h->copy_stream) cudaStreamDestroy(h->copy_stream);
   if (h->aux_stream) cudaStreamDestroy(h->aux_stream);
   if (h->ev_fork) cudaEventDestroy(h->ev_fork);
@@ -459,7 +467,7 @@ bool class_is_fused(const td_handle* h, const ClassInfo& c) {
 
 // AUTO sends a size class to the dense path when every segment in it is at most dense.auto_n long.
 bool class_is_dense(const td_handle* h, const ClassInfo& c) {
-  if (h->path == TD_PATH_DENSE) return true;
+  if (h->path == TD_PATH_DENSE || h->path == TD_PATH_CDO) return true;
   if (h->path == TD_PATH_FFT) return false;
   return c.max_n <= h->dense.auto_n;
 }
@@ -467,7 +475,7 @@ bool class_is_dense(const td_handle* h, const ClassInfo& c) {
 // (re)builds the segment tables of the dense path from the host-side segment records
 td_status dense_upload(td_handle* h) {
   DenseState& D = h->dense;
-  D.all.clear(); D.aut.clear();
+  D.all.clear(); D.aut.clear(); D.aut_gs.clear();
   for (const ClassInfo& c : h->classes)
     for (int id : c.seg_ids) {
       const SegHost& sg = h->segs[id];
@@ -475,7 +483,7 @@ td_status dense_upload(td_handle* h) {
       DenseSeg ds;
       ds.off = sg.off; ds.n = sg.n; ds.npad = (sg.n + 31) / 32 * 32; ds.a = sg.a; ds.rsv = 1.0 / std::sqrt(sg.v); ds.zd = sg.zd;
       D.all.push_back(ds);
-      if (c.max_n <= D.auto_n) D.aut.push_back(ds);
+      if (c.max_n <= D.auto_n) { D.aut.push_back(ds); if (sg.n < CDO_AUTO_MIN_N) D.aut_gs.push_back(ds); }
     }
   D.max_n = DENSE_MAX_N;
   if (h->max_n > DENSE_MAX_N) D.all.clear();
@@ -526,6 +534,84 @@ td_status launch_dense(td_handle* h, const std::vector<DenseSeg>& segs, const do
   return TD_OK;
 }
 
+// CDO path (td_cdo.cuh): W = L^{-1} per segment, built on the first use of TD_PATH_CDO
+// (segments of at most max_n samples that do not have their W yet; synchronous)
+td_status cdo_setup(td_handle* h, int max_n) {
+  if (h->cdoW.empty()) h->cdoW.assign(h->n_seg, nullptr);
+  std::vector<CdoSeg> cs;
+  std::vector<int> ids;
+  td_status st = TD_OK;
+  for (int s = 0; s < h->n_seg && st == TD_OK; ++s) {
+    const SegHost& sg = h->segs[s];
+    if (sg.n > max_n || sg.n > CDO_MAX_N || h->cdoW[s]) continue;
+    const int npad = (sg.n + 31) / 32 * 32;
+    double* W = nullptr;
+    if (cudaMalloc(&W, sizeof(double) * (size_t)npad * npad) != cudaSuccess) { st = TD_ENOMEM; break; }
+    CdoSeg c;
+    c.rho = h->d_rho + sg.off; c.W = W; c.n = sg.n; c.npad = npad;
+    cs.push_back(c); ids.push_back(s);
+  }
+  CdoSeg* d_cs = nullptr;
+  if (st == TD_OK && !cs.empty()) {
+    if (cudaMalloc(&d_cs, sizeof(CdoSeg) * cs.size()) != cudaSuccess) st = TD_ENOMEM;
+    else if (cudaMemcpy(d_cs, cs.data(), sizeof(CdoSeg) * cs.size(), cudaMemcpyHostToDevice) != cudaSuccess) st = TD_ECUDA;
+    else {
+      cdo_whitener_kernel<<<(unsigned)cs.size(), CDO_NT>>>(d_cs);
+      if (cudaGetLastError() != cudaSuccess || cudaDeviceSynchronize() != cudaSuccess) st = TD_ECUDA;
+    }
+  }
+  cudaFree(d_cs);
+  if (st != TD_OK) { for (const CdoSeg& c : cs) cudaFree(c.W); return st; }
+  for (size_t i = 0; i < ids.size(); ++i) h->cdoW[ids[i]] = cs[i].W;
+  return TD_OK;
+}
+
+template <int NC>
+td_status launch_cdo_nc(td_handle* h, const CdoParams& P0, int nbuf, cudaStream_t st, bool dry) {
+  auto kern = td_cdo_kernel<NC>;
+  static int cache[TD_MAX_DEV];
+  CdoParams P = P0;
+  P.nbuf = nbuf; P.ntiles = (P.B + 8 * NC - 1) / (8 * NC);
+  const size_t smem = cdo_smem_bytes<NC>(P.npad, nbuf);
+  int nb = 0;
+  td_status cs = kernel_config(kern, DENSE_NT, h->smem_optin, smem, h->device, cache, &nb);
+  if (cs != TD_OK) return cs;
+  if (smem > h->smem_optin) return TD_EUNSUPPORTED;
+  if (dry) return TD_OK;
+  const int nwc = DENSE_NW / dense_nwr(P.npad);
+  const int64_t grid = std::min<int64_t>((P.ntiles + nwc - 1) / nwc, h->num_sms);
+  kern<<<(unsigned)std::max<int64_t>(grid, 1), DENSE_NT, smem, st>>>(P);
+  CK(cudaGetLastError());
+  ++h->last_launches;
+  return TD_OK;
+}
+
+// one launch per segment; 32-template panels (NC = 4) where one fits shared memory, else 16 (NC = 2); double-buffered
+// panels where two fit
+// (segments of at most max_n samples; *count receives how many ran)
+td_status launch_cdo(td_handle* h, const double* d, const double* H, int64_t ldh, int64_t B, double* out, int accumulate,
+                     cudaStream_t st, int min_n, int max_n, int* count, bool dry = false) {
+  if (count) *count = 0;
+  for (int s = 0; s < h->n_seg; ++s) {
+    const SegHost& sg = h->segs[s];
+    if (sg.n > max_n || sg.n < min_n) continue;
+    if (h->cdoW.empty() || !h->cdoW[s]) return TD_EUNSUPPORTED;  // (never: td_create / td_set_path built it)
+    if (count) ++*count;
+    CdoParams P;
+    P.d = d; P.H = H; P.ldh = ldh; P.B = B; P.out = out; P.off = sg.off; P.n = sg.n; P.npad = (sg.n + 31) / 32 * 32;
+    P.W = h->cdoW[s]; P.accumulate = accumulate;
+    P.vec_ok = (sg.off % 2 == 0) && (sg.n % 2 == 0) && (ldh % 2 == 0) && ((reinterpret_cast<uintptr_t>(H) & 15) == 0);
+    td_status r;
+    if (cdo_smem_bytes<4>(P.npad, 1) <= h->smem_optin)
+      r = launch_cdo_nc<4>(h, P, cdo_smem_bytes<4>(P.npad, 2) <= h->smem_optin ? 2 : 1, st, dry);
+    else
+      r = launch_cdo_nc<2>(h, P, cdo_smem_bytes<2>(P.npad, 2) <= h->smem_optin ? 2 : 1, st, dry);
+    if (r != TD_OK) return r;
+    accumulate = 1;
+  }
+  return TD_OK;
+}
+
 // FFT path over all size classes.  MODE_LOGLIKE: out0 = loglike.  MODE_INNER: out0 = <d,h>, out1 = <h,h>.
 // `f32`: classes that have fp32 tables and are not served by the dense kernel run the fp32 build of their kernel
 template <int MODE>
@@ -567,8 +653,25 @@ template <int MODE>
 td_status run_batch(td_handle* h, const double* d, const double* H, int64_t ldh, int64_t B, double* out0,
                     double* out1, cudaStream_t st) {
   const DenseState& D = h->dense;
+  if (MODE == MODE_LOGLIKE && (h->path == TD_PATH_CDO || (h->path == TD_PATH_AUTO && !D.aut.empty()))) {
+    // log-likelihood of the short segments: the triangular contraction with the cached L^{-1} (measured faster than the
+    // Gohberg-Semencul dense kernel at every length up to 1024, profiles/r02_cdo.md); AUTO: the dense-class segments
+    int nc = 0, ng = 0, acc = 0;
+    const bool forced = h->path == TD_PATH_CDO;
+    if (!forced && !D.aut_gs.empty()) {   // AUTO: the shortest segments stay on the Gohberg-Semencul dense kernel
+      td_status s = launch_dense<MODE>(h, D.aut_gs, d, H, ldh, B, out0, out1, 0, st);
+      if (s != TD_OK) return s;
+      ng = (int)D.aut_gs.size(); acc = 1;
+    }
+    td_status s = launch_cdo(h, d, H, ldh, B, out0, acc, st, forced ? 1 : CDO_AUTO_MIN_N, forced ? CDO_MAX_N : D.auto_n, &nc);
+    if (s != TD_OK) return s;
+    const bool all = nc + ng == h->n_seg;
+    h->last_path = all ? (nc > 0 ? TD_PATH_CDO : TD_PATH_DENSE) : TD_PATH_FFT;
+    if (all) return TD_OK;
+    return run_fft_path<MODE>(h, d, H, ldh, B, out0, out1, st, true, 1, h->precision == TD_PREC_F32);
+  }
   const std::vector<DenseSeg>* dsegs = nullptr;
-  if (h->path == TD_PATH_DENSE) dsegs = &D.all;
+  if (h->path == TD_PATH_DENSE || h->path == TD_PATH_CDO) dsegs = &D.all;
   else if (h->path == TD_PATH_AUTO) dsegs = &D.aut;
   const int nd = dsegs ? (int)dsegs->size() : 0;
   int accumulate = 0;
@@ -687,10 +790,11 @@ static td_status create_impl(td_handle* h, const double* acf, const int64_t* seg
   }
   h->n_tot = off;
   // ---- device copies of the ACFs, Levinson-Durbin per segment (one CTA each)
-  double* d_rho = nullptr; double* d_v = nullptr; double* d_ld = nullptr; int* d_status = nullptr; LevSeg* d_lev = nullptr;
-  struct Tmp { double*& a; double*& b; double*& c; int*& d; LevSeg*& e; ~Tmp() { cudaFree(a); cudaFree(b); cudaFree(c); cudaFree(d); cudaFree(e); } }
-      tmp{d_rho, d_v, d_ld, d_status, d_lev};
-  CK(cudaMalloc(&d_rho, sizeof(double) * h->n_tot));
+  double* d_v = nullptr; double* d_ld = nullptr; int* d_status = nullptr; LevSeg* d_lev = nullptr;
+  struct Tmp { double*& b; double*& c; int*& d; LevSeg*& e; ~Tmp() { cudaFree(b); cudaFree(c); cudaFree(d); cudaFree(e); } }
+      tmp{d_v, d_ld, d_status, d_lev};
+  CK(cudaMalloc(&h->d_rho, sizeof(double) * h->n_tot));   // owned by the handle (the CDO setup reads it again)
+  double* const d_rho = h->d_rho;
   CK(cudaMemcpy(d_rho, acf, sizeof(double) * h->n_tot, cudaMemcpyHostToDevice));
   CK(cudaMalloc(&d_v, sizeof(double) * n_seg));
   CK(cudaMalloc(&d_ld, sizeof(double) * n_seg));
@@ -794,6 +898,11 @@ static td_status create_impl(td_handle* h, const double* acf, const int64_t* seg
   h->dense.auto_n = DENSE_AUTO_N;
   td_status ds = dense_upload(h);
   if (ds != TD_OK) return ds;
+  if (!h->dense.aut.empty()) {   // AUTO evaluates the dense-class segments with the cached L^{-1} (td_cdo.cuh)
+    ds = cdo_setup(h, h->dense.auto_n);
+    if (ds == TD_OK) ds = launch_cdo(h, nullptr, nullptr, h->n_tot, 1, nullptr, 0, nullptr, CDO_AUTO_MIN_N, h->dense.auto_n, nullptr, true);
+    if (ds != TD_OK) return ds;
+  }
   // ---- everything a batch call would otherwise create on first use: streams, events, scratch that does not grow with B
   CK(cudaStreamCreateWithFlags(&h->aux_stream, cudaStreamNonBlocking));
   CK(cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking));
@@ -1057,8 +1166,15 @@ td_status td_inner_batch(td_handle* h, const double* d, const double* H, int64_t
 }
 
 td_status td_set_path(td_handle* h, int path) {
-  if (!h || path < TD_PATH_AUTO || path > TD_PATH_DENSE) return TD_EINVAL;
-  if (path == TD_PATH_DENSE && h->max_n > h->dense.max_n) return TD_EUNSUPPORTED;
+  if (!h || (path != TD_PATH_AUTO && path != TD_PATH_FFT && path != TD_PATH_DENSE && path != TD_PATH_CDO)) return TD_EINVAL;
+  if ((path == TD_PATH_DENSE || path == TD_PATH_CDO) && h->max_n > h->dense.max_n) return TD_EUNSUPPORTED;
+  if (path == TD_PATH_CDO) {   // first use: builds W = L^{-1} per segment (synchronous), configures the kernel
+    DevGuard guard(h->device);
+    if (!guard.ok) return TD_ECUDA;
+    td_status s = cdo_setup(h, CDO_MAX_N);
+    if (s == TD_OK) s = launch_cdo(h, nullptr, nullptr, h->n_tot, 1, nullptr, 0, nullptr, 1, CDO_MAX_N, nullptr, true);
+    if (s != TD_OK) return s;
+  }
   h->path = path;
   return TD_OK;
 }

@@ -403,6 +403,20 @@ def test_full_size_dense_regime(name):
     _full_size_check(name, sample=64, path=tdb.TD_PATH_DENSE)
 
 
+@pytest.mark.parametrize("name,path", [("d1", tdb.TD_PATH_AUTO), ("d3", tdb.TD_PATH_AUTO), ("d4", tdb.TD_PATH_AUTO),
+                                       ("d5", tdb.TD_PATH_CDO)])
+def test_full_size_cdo_regime(name, path):
+    """AUTO sends the log-likelihood of segments up to 512 samples through the cached-L^-1 contraction (td_cdo.cuh); the
+    bilinear identity inside _full_size_check ties it to the Gohberg-Semencul dense kernel (td_inner_batch)."""
+    _full_size_check(name, sample=64, path=path)
+    w = W.make(name, B=40)
+    with tdb.TDLikelihood(w.acf, w.seg_lengths) as h:
+        h.set_path(path)
+        h.loglike_batch(_dev(w.d), _dev(w.H))
+        # N = 64 stays on the Gohberg-Semencul dense kernel under AUTO (measured crossover, profiles/r02_cdo.md)
+        assert h.info()["last_path"] == (tdb.TD_PATH_DENSE if name == "d1" else tdb.TD_PATH_CDO)
+
+
 # ------------------------------------------------------------------ cross term as a batched dot product (td_dot.cuh)
 @pytest.mark.parametrize("name,B,n_scale", [("c1", 64, 1), ("c2", 40, 1), ("c3", 9, 1), ("c5", 5, 1), ("d2", 100, 1)])
 def test_cross_term_dot_path(name, B, n_scale):
@@ -508,6 +522,7 @@ def test_fused_many_items_per_cta_repeatable(name, B):
 
 # ------------------------------------------------------------------ degenerate rows on the dense, dot and cluster paths
 @pytest.mark.parametrize("name,n_scale,path", [("d2", 1, tdb.TD_PATH_DENSE), ("d4", 1, tdb.TD_PATH_DENSE),
+                                               ("d2", 1, tdb.TD_PATH_AUTO), ("d5", 1, tdb.TD_PATH_CDO),
                                                ("c5", 1, tdb.TD_PATH_AUTO), ("c4", 4, tdb.TD_PATH_AUTO)])
 def test_exact_zero_nan_row_and_single_template(name, n_scale, path):
     """h = d gives exactly 0 (pin P8 iv), a NaN poisons only its own row, B = 1 and a strided H work, on the dense
@@ -789,3 +804,92 @@ def test_f32_full_size_against_the_fp64_path(name):
     ref = O.loglike_batch(w.acf, w.seg_lengths, w.d, w.H[idx])
     _assert_close(o32[idx], ref, tol=TOL32, what=f"{name} f32 full size")
     print(f"{name}: fp32 vs fp64 over {w.B} rows: max {err.max():.2e}, median {np.median(err):.2e}")
+
+
+# ------------------------------------------------------------------ very long segments
+def test_very_long_segment_2pow20():
+    """N = 2^20 (transform length 2^21, five-pass plans, cooperative Levinson-Durbin over 2^20 orders).
+    (a) AR(2) covariance: every row against the closed-form exact AR likelihood of the oracle (pin P19), 1e-9;
+    (b) the PSD-recipe ACF of the configs: the chi-square invariant E[x^T C^-1 x] = N for x ~ N(0, C) (one draw:
+        N +- 4 sqrt(2N)) and the bilinear identity of Eq. 13 between td_loglike_batch and td_inner_batch.
+    Prints the td_create times (S0 is one-time and cached; reported, not part of the metric)."""
+    import time
+    N = 1 << 20
+    rng = np.random.default_rng(20)
+    phi, s2 = [1.6, -0.8], 3.0e-43
+    rho = O.ar_acf(phi, s2, N)
+    x = np.sqrt(s2) * rng.standard_normal(N)
+    for t in range(2, N):                      # one AR(2) path (any vector would do: the identity is exact)
+        x[t] += phi[0] * x[t - 1] + phi[1] * x[t - 2]
+    H = np.zeros((3, N))
+    H[1] = 0.25 * np.roll(x, 1000)
+    H[2] = np.sqrt(s2) * rng.standard_normal(N)
+    ref = np.array([-0.5 * O.ar_quadform_closed(phi, s2, x - H[b]) for b in range(3)])
+    t0 = time.perf_counter()
+    with tdb.TDLikelihood(rho, [N]) as h:
+        t_ar = time.perf_counter() - t0
+        out = h.loglike_batch(_dev(x), _dev(H)).cpu().numpy()
+        v = h.info()["v"][0]
+    _assert_close(out, ref, what="N = 2^20, AR(2) closed form")
+    assert abs(v / s2 - 1.0) < 1e-9
+    fs = 4096.0
+    rho = W.acf_from_psd(fs, 2 * N, N)
+    x = W._noise(rng, fs, 2 * N, N)
+    Hh = 0.5 * np.roll(x, 12345)[None, :]
+    t0 = time.perf_counter()
+    with tdb.TDLikelihood(rho, [N]) as h:
+        t_psd = time.perf_counter() - t0
+        d = _dev(x)
+        q = -2.0 * float(h.loglike_batch(d, _dev(np.zeros((1, N)))).item())
+        ll = float(h.loglike_batch(d, _dev(Hh)).item())
+        dh, hh = h.inner_batch(d, _dev(Hh))
+        launches = h.last_launches()
+    assert abs(q - N) <= 4.0 * np.sqrt(2.0 * N), f"chi-square invariant: Q = {q}, N = {N}"
+    assert abs(-2.0 * ll - (q - 2.0 * float(dh.item()) + float(hh.item()))) <= 1e-9 * (q + float(hh.item()))
+    print(f"N = 2^20: td_create {t_ar:.1f} s (AR(2) ACF), {t_psd:.1f} s (PSD-recipe ACF); Q/N = {q / N:.6f}; "
+          f"{launches} launches per td_inner_batch")
+
+
+# ------------------------------------------------------------------ CDO path: Y = L^-1 X with the cached whitening operator
+@pytest.mark.parametrize("n", [1, 31, 64, 100, 257, 512, 777, 1024])
+def test_cdo_path_lengths(n):
+    """SURVEY 8(f) NEXT-3, second half: the triangular contraction against the oracle, which is the
+    same quantity computed the same way (dense Cholesky, forward substitution) on the CPU."""
+    rng = np.random.default_rng(400 + n)
+    rho = W.acf_from_psd(4096.0, max(2 * n, 64), n)
+    B = 70 if n < 600 else 37          # several 32-template tiles and a ragged tail
+    d = rng.standard_normal(n) * 1e-21
+    H = rng.standard_normal((B, n)) * 1e-21
+    H[3] = d
+    ref = O.loglike_batch(rho, [n], d, H)
+    with tdb.TDLikelihood(rho, [n]) as h:
+        h.set_path(tdb.TD_PATH_CDO)
+        out = h.loglike_batch(_dev(d), _dev(H)).cpu().numpy()
+        assert h.info()["last_path"] == tdb.TD_PATH_CDO
+        dh, hh = h.inner_batch(_dev(d), _dev(H))           # cross terms keep the Gohberg-Semencul dense kernel
+    assert out[3] == 0.0
+    _assert_close(out, ref, what=f"cdo n={n}")
+    _, hh_ref = O.inner_batch(rho, [n], d, H)
+    assert np.max(np.abs(hh.cpu().numpy() - hh_ref) / np.abs(hh_ref)) <= TOL
+
+
+def test_cdo_multi_segment_odd_offsets_and_limits():
+    rng = np.random.default_rng(77)
+    lens = [333, 64, 1000]
+    acf = np.concatenate([W.acf_from_psd(4096.0, 2 * n, n) * s for n, s in zip(lens, (1.0, 2.5, 0.6))])
+    d = rng.standard_normal(sum(lens)) * 1e-21
+    H = rng.standard_normal((45, sum(lens) + 3))[:, :sum(lens)] * 1e-21     # odd leading dimension: 8-byte copies
+    ref = O.loglike_batch(acf, lens, d, H)
+    with tdb.TDLikelihood(acf, lens) as h:
+        h.set_path(tdb.TD_PATH_CDO)
+        out = h.loglike_batch(_dev(d), _dev(H)).cpu().numpy()
+        h.set_path(tdb.TD_PATH_DENSE)
+        out_gs = h.loglike_batch(_dev(d), _dev(H)).cpu().numpy()
+    _assert_close(out, ref, what="cdo multi-segment")
+    _assert_close(out_gs, ref, what="gs dense beside it")
+    w = W.make("c1", B=4, n_scale=1)
+    acf2 = W.acf_from_psd(4096.0, 4096, 2048)
+    with tdb.TDLikelihood(acf2, [2048]) as h:
+        with pytest.raises(tdb.TDError) as e:
+            h.set_path(tdb.TD_PATH_CDO)                      # 2048 > 1024
+        assert e.value.status == tdb.TD_EUNSUPPORTED
