@@ -47,8 +47,11 @@ template <int LOG2M> struct Fused4Shape {
   static constexpr int TWS = 2 * M / RF1;
   static constexpr int PADM = SmemArr::padded(M), PADNF = SmemArr::padded(NF);
   using Cols = F4Cols<8>;
-  // Cols::WINDOW columns per thread (256 in fp64, 128 in fp32); warps w and w + 4 share a lane quarter
-  static constexpr int TMEM_COLS = (NW > 4 ? 2 : 1) * Cols::WINDOW;
+  // Cols::WINDOW columns per thread (256 in fp64, 128 in fp32); warps w, w + 4, w + 8, .. of a CTA share a lane quarter
+  static constexpr int tmem_cols(int ngrp) { return ((NW * ngrp + 3) / 4) * Cols::WINDOW; }
+  static constexpr int TMEM_COLS = tmem_cols(1);
+  // bytes of one item pipeline (NGRP > 1: several independent pipelines share a CTA, see the kernel), 16-byte granular
+  static constexpr size_t group_bytes() { return (smem_bytes() + 15) & ~(size_t)15; }
   static constexpr size_t smem_bytes() {
     return sizeof(cplx) * (2 * (size_t)PADNF + 2 * (size_t)PADM + TWS) + sizeof(double) * 4 * NW + 48 + F4_SEGCACHE * sizeof(SegDev)
 #ifdef TD_PHASE_CLOCKS
@@ -264,26 +267,40 @@ __device__ long long g_phase_clk[148 * 16 * 16];
 #define TDCLK(k) do { } while (0)
 #endif
 
-template <int LOG2M, int MODE>
-__global__ void __launch_bounds__(Fused4Shape<LOG2M>::NT, 1) td_fused4_kernel(const Fused4Params P4) {
+// NGRP > 1: the CTA holds NGRP independent item pipelines ("groups" of NT threads, each with its own shared-memory regions,
+// mbarrier, named barrier and TMEM windows) that work on different templates.  A kernel that uses tensor memory is limited
+// to one CTA per SM (profiles/r02_c2_fused4_ncu.md), so this is how the fp32 build - whose working set and register need
+// are half the fp64 ones - puts two items on an SM: their load / butterfly / store phases interleave instead of adding up.
+template <int LOG2M, int MODE, int NGRP = 1>
+__global__ void __launch_bounds__(Fused4Shape<LOG2M>::NT * NGRP, 1) td_fused4_kernel(const Fused4Params P4) {
   using Sh = Fused4Shape<LOG2M>;
   constexpr int M = Sh::M, NF = Sh::NF, TW = 2 * M, NT = Sh::NT, NW = Sh::NW, NWB = Sh::NWB;
+  constexpr int TMEM_COLS = Sh::tmem_cols(NGRP);
+  static_assert(TMEM_COLS <= 512 && (TMEM_COLS & (TMEM_COLS - 1)) == 0, "tensor memory: 512 columns, power-of-two allocations");
   constexpr int RF1 = Sh::RF1, RI1 = Sh::RI1;
   constexpr int NTASK = NF / RF1, IT = NTASK / NT, S1 = NF / RF1;  // first pass: IT tasks of radix RF1 per thread
   static_assert(NTASK % NT == 0 && IT * RF1 == 8, "first pass tiling: 8 complex inputs per thread");
   const FusedParams& P = P4.base;
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  cplx* sm = reinterpret_cast<cplx*>(smem_raw);
+  const int grp = NGRP == 1 ? 0 : (int)threadIdx.x / NT;              // item pipeline of this thread
+  const int vblock = (int)blockIdx.x * NGRP + grp, vgrid = (int)gridDim.x * NGRP;   // pipelines are what items are dealt to
+  auto group_sync = [&]() {
+    if constexpr (NGRP == 1) __syncthreads();
+    else asm volatile("bar.sync %0, %1;" ::"r"(1 + grp), "r"(NT) : "memory");
+  };
+  cplx* sm = reinterpret_cast<cplx*>(smem_raw + (size_t)grp * Sh::group_bytes());
   const SmemArr UE{sm}, UO{sm + Sh::PADNF};
   const SmemArr ZE{sm + 2 * Sh::PADNF}, ZO{sm + 2 * Sh::PADNF + Sh::PADM};
   cplx* tw = sm + 2 * Sh::PADNF + 2 * Sh::PADM;
   double* red = reinterpret_cast<double*>(tw + Sh::TWS);  // [2][2 NW]: per-warp partial sums, double-buffered by item parity
   const uint32_t mbar_rows = smem_u32(red + 4 * NW);
-  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(red + 4 * NW + 1);
+  // (one allocation for the CTA: every group reads group 0's slot)
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(reinterpret_cast<double*>(reinterpret_cast<cplx*>(smem_raw) + 2 * Sh::PADNF + 2 * Sh::PADM + Sh::TWS) + 4 * NW + 1);
   SegDev* segS = reinterpret_cast<SegDev*>(red + 4 * NW + 3);
   const SegDev* segs = P.n_seg <= F4_SEGCACHE ? segS : P.segs;
   double* stH = reinterpret_cast<double*>(sm);  // the staged template row lives in the U region (dead after mid)
-  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int tid = (int)threadIdx.x - grp * NT, warp = tid >> 5, lane = tid & 31;   // within the group
+  const int cwarp = (int)threadIdx.x >> 5;                                        // within the CTA (TMEM lane quarter, window)
   const int br = warp / NWB, wb = warp - br * NWB;  // branch (0 even bins, 1 odd bins), warp within branch
   const SmemArr U = br ? UO : UE, Z = br ? ZO : ZE;
   const F4Own own = f4_own<RF1, true>(br, wb);
@@ -291,7 +308,7 @@ __global__ void __launch_bounds__(Fused4Shape<LOG2M>::NT, 1) td_fused4_kernel(co
   for (int k = tid; k < Sh::TWS; k += NT) tw[k] = P.T[k];
   if (tid < P.n_seg && tid < F4_SEGCACHE) segS[tid] = P.segs[tid];
   if (tid == 0) mbar_init(mbar_rows, 1);
-  if (warp == 0) tmem_alloc<Sh::TMEM_COLS>(smem_u32(tmem_slot));
+  if (cwarp == 0) tmem_alloc<TMEM_COLS>(smem_u32(tmem_slot));
 #ifdef TD_PHASE_CLOCKS
   long long* clk_s = reinterpret_cast<long long*>(segS + F4_SEGCACHE);
   if (tid < 16 * NW) clk_s[tid] = 0;
@@ -301,7 +318,7 @@ __global__ void __launch_bounds__(Fused4Shape<LOG2M>::NT, 1) td_fused4_kernel(co
   __syncthreads();
   tmem_fence_after();
   // this thread's TMEM window: lane 32 (warp % 4) + lane, Cols::WINDOW columns
-  const uint32_t tcol = *tmem_slot + ((uint32_t)(32 * (warp & 3)) << 16) + (uint32_t)((warp >> 2) * Sh::Cols::WINDOW);
+  const uint32_t tcol = *tmem_slot + ((uint32_t)(32 * (cwarp & 3)) << 16) + (uint32_t)((cwarp >> 2) * Sh::Cols::WINDOW);
   f4_store_twiddles<TW>(lane, tw, tcol + Sh::Cols::TW);
 
   // rows of item (b, s); the template row is staged by TMA when it is 16-byte aligned and N_s is even
@@ -323,11 +340,7 @@ __global__ void __launch_bounds__(Fused4Shape<LOG2M>::NT, 1) td_fused4_kernel(co
   };
 
   const long long Bs = (MODE == MODE_STOREZ) ? 1 : P.B;  // STOREZ transforms the data vector itself, once per segment
-  if ((long long)blockIdx.x >= Bs) {                     // (never: the grid is min(B, SMs); keeps the TMEM protocol whole)
-    __syncthreads();
-    if (warp == 0) tmem_dealloc<Sh::TMEM_COLS>(*tmem_slot);
-    return;
-  }
+  const bool active = (long long)vblock < Bs;             // (a pipeline without items still takes part in the CTA barriers)
   // The partial sums of an item are combined (fixed order over the warps) by thread 0 after the first CTA barrier of the
   // NEXT item: no atomics, no fences, no barrier at the end of an item.  Segments accumulate into out[b].
   long long pend_b = -1;
@@ -352,10 +365,10 @@ __global__ void __launch_bounds__(Fused4Shape<LOG2M>::NT, 1) td_fused4_kernel(co
   bool staged;
   {
     const double *dr, *hr; int nn;
-    staged = rows(blockIdx.x, 0, dr, hr, nn);
-    if (tid == 0) prefetch_rows(blockIdx.x, 0);
+    staged = rows(vblock, 0, dr, hr, nn);
+    if (tid == 0 && active) prefetch_rows(vblock, 0);
   }
-  for (int s = 0; s < P.n_seg; ++s) {
+  for (int s = 0; active && s < P.n_seg; ++s) {
     const SegDev sg = segs[s];
     // ---------------- per-segment constants into this thread's TMEM columns: generator values, data samples
     f4_store_generator(P4.Gp[s] + (size_t)br * Sh::PADM, own, lane, tcol + F4_TC_G);
@@ -371,9 +384,9 @@ __global__ void __launch_bounds__(Fused4Shape<LOG2M>::NT, 1) td_fused4_kernel(co
         }
     }
     tmem_wait_st();
-    for (long long b = blockIdx.x; b < Bs; b += gridDim.x) {
-      long long nb = b + gridDim.x; int ns = s;
-      if (nb >= Bs) { nb = blockIdx.x; ns = s + 1; }
+    for (long long b = vblock; b < Bs; b += vgrid) {
+      long long nb = b + vgrid; int ns = s;
+      if (nb >= Bs) { nb = vblock; ns = s + 1; }
       const bool have_next = ns < P.n_seg;
       // ---------------- forward pass 1 (radix RF1, stride 256): both branches from one set of inputs
       if (staged) {
@@ -413,7 +426,7 @@ __global__ void __launch_bounds__(Fused4Shape<LOG2M>::NT, 1) td_fused4_kernel(co
             for (int ss = 0; ss < RF1; ++ss) xs[it][ss] = to_cplx(hs[it][ss].x, hs[it][ss].y, sg.rscale);
         }
         TDCLK(2);
-        __syncthreads();  // staging consumed: the U region may now be overwritten
+        group_sync();  // staging consumed: the U region may now be overwritten
         TDCLK(3);
 #pragma unroll
         for (int it = 0; it < IT; ++it) first_pass_compute<RF1, NF>(UE, UO, tid + it * NT, xs[it], tw);
@@ -425,7 +438,7 @@ __global__ void __launch_bounds__(Fused4Shape<LOG2M>::NT, 1) td_fused4_kernel(co
 #pragma unroll 1
         for (int g = tid; g < NTASK; g += NT) first_pass_c<RF1, NF, MODE>(UE, UO, g, drow, hrow, n, vec, tw, sg.rscale);
       }
-      __syncthreads();
+      group_sync();
       if (tid == 0) finalize();  // the previous item's sums: every warp has passed its last pass
 #ifdef TD_DEBUG_KNOBS
       if (br && P4.skew > 0) { const long long t_ = clock64(); while (clock64() - t_ < P4.skew) { } }
@@ -444,7 +457,7 @@ __global__ void __launch_bounds__(Fused4Shape<LOG2M>::NT, 1) td_fused4_kernel(co
       // ---------------- inverse pass 2 (L = 256), warp-local
       f4_inverse2<TW>(Z, own, lane, tw);
       TDCLK(10);
-      __syncthreads();
+      group_sync();
       // every warp is past mid: the U region is dead and takes the next item's template row
       if (tid == 0 && have_next) prefetch_rows(nb, ns);
       TDCLK(11);
@@ -464,9 +477,10 @@ __global__ void __launch_bounds__(Fused4Shape<LOG2M>::NT, 1) td_fused4_kernel(co
       staged = staged_next;
     }
   }
-  __syncthreads();
-  if (tid == 0) finalize();
-  if (warp == 0) tmem_dealloc<Sh::TMEM_COLS>(*tmem_slot);
+  group_sync();
+  if (tid == 0 && active) finalize();
+  if constexpr (NGRP > 1) __syncthreads();   // every pipeline is done with its TMEM windows
+  if (cwarp == 0) tmem_dealloc<TMEM_COLS>(*tmem_slot);
 #ifdef TD_PHASE_CLOCKS
   if (tid < 16 * NW && blockIdx.x < 148) g_phase_clk[blockIdx.x * 256 + tid] = clk_s[tid];
 #endif

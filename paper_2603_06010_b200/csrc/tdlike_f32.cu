@@ -25,20 +25,22 @@ __global__ void cvt_cplx_kernel(const double2* __restrict__ src, float2* __restr
   if (i < n) dst[i] = make_float2((float)(src[i].x * scale), (float)(src[i].y * scale));
 }
 
+// Two item pipelines per CTA (NGRP = 2, td_fused4.cuh): the fp32 working set of a pipeline is 113 KB at M = 4096, a kernel
+// that uses tensor memory gets one CTA per SM, so the second item on the SM lives in the same CTA.
+constexpr int F32_NGRP = 2;
 template <int LOG2M, int MODE>
 td_status launch_fused4(const td32api::ClassTables& t, const FusedParams& P, int num_sms, int device, cudaStream_t st, bool dry) {
-  auto kern = td_fused4_kernel<LOG2M, MODE>;
-  constexpr int NT = Fused4Shape<LOG2M>::NT;
-  const size_t smem = Fused4Shape<LOG2M>::smem_bytes();
+  auto kern = td_fused4_kernel<LOG2M, MODE, F32_NGRP>;
+  constexpr int NT = Fused4Shape<LOG2M>::NT * F32_NGRP;
+  const size_t smem = Fused4Shape<LOG2M>::group_bytes() * F32_NGRP;
   static int cache[TD_MAX_DEV];
   int nb = 0;
   td_status cs = kernel_config(kern, NT, smem, smem, device, cache, &nb);
   if (cs != TD_OK) return cs;
   if (nb < 1) return TD_EUNSUPPORTED;
   if (dry) return TD_OK;
-  nb = std::min(nb, 512 / Fused4Shape<LOG2M>::TMEM_COLS);  // co-resident CTAs share the SM's 512 tensor-memory columns
-  const long long maxg = (long long)nb * num_sms;
-  const int grid = (int)std::max<long long>(1, std::min<long long>(MODE == MODE_STOREZ ? 1 : P.B, maxg));
+  const long long want = MODE == MODE_STOREZ ? 1 : (P.B + F32_NGRP - 1) / F32_NGRP;   // CTAs: one per F32_NGRP items
+  const int grid = (int)std::max<long long>(1, std::min<long long>(want, num_sms));
   Fused4Params P4;
   P4.base = P; P4.Gp = reinterpret_cast<const cplx* const*>(t.Gp_ptrs);
   kern<<<grid, NT, smem, st>>>(P4);
