@@ -253,12 +253,14 @@ __global__ void __launch_bounds__(ClusterShape::NT, 1) td_cluster_kernel(const F
     f4_store_generator(P4.Gp[s] + (size_t)br * Sh::PADM, own, lane, tcol + F4_TC_G);
     if (MODE == MODE_LOGLIKE) {
       const double* drow = P.d + sg.off;
+      double2 dvs[16];   // loads first, (volatile) TMEM stores after: the latencies overlap
 #pragma unroll
       for (int q = 0; q < 16; ++q) {
         const int i0 = 2 * (tid + 256 * q);
-        double2 dv = make_double2(i0 < sg.n ? __ldg(drow + i0) : 0.0, i0 + 1 < sg.n ? __ldg(drow + i0 + 1) : 0.0);
-        tmem_st_c64(tcol + F4_TC_D + 4 * q, dv);
+        dvs[q] = make_double2(i0 < sg.n ? __ldg(drow + i0) : 0.0, i0 + 1 < sg.n ? __ldg(drow + i0 + 1) : 0.0);
       }
+#pragma unroll
+      for (int q = 0; q < 16; ++q) tmem_st_c64(tcol + F4_TC_D + 4 * q, dvs[q]);
     }
     tmem_wait_st();
     for (long long b = cl; b < Bs; b += ncl) {

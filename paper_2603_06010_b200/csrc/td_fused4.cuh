@@ -153,26 +153,35 @@ __device__ __forceinline__ void f4_store_twiddles(int lane, const cplx* __restri
 // per item.  The element order is the one f4_mid multiplies in.
 __device__ __forceinline__ void f4_store_generator(const cplx* __restrict__ g, const F4Own& o, int lane, uint32_t tg) {
   const int q4 = lane >> 3;
-  const int s1 = q4 == 0 ? o.z0 : q4 == 1 ? o.z1 : q4 == 2 ? o.z2 : o.z3, s2 = lane & 7;
+  const int s1 = q4 == 0 ? o.z0 : q4 == 1 ? o.z2 : q4 == 2 ? o.z1 : o.z3, s2 = lane & 7;  // (half-warps: {z0, z2}, {z1, z3})
+  // all 32 loads are issued before the first (volatile) TMEM store, so their latencies overlap
+  cplx v[2][16];
 #pragma unroll
   for (int par = 0; par < 2; ++par) {
     const int zb = (s1 * 16 + s2) * 16 + par * 8 * 16;
 #pragma unroll
     for (int q = 0; q < 16; ++q) {
       const int i = zb + q;
-      tmem_st_c(tg + TM_CPC * (16 * par + q), __ldg(g + i + (i >> 4)));
+      v[par][q] = __ldg(g + i + (i >> 4));
     }
   }
+#pragma unroll
+  for (int par = 0; par < 2; ++par)
+#pragma unroll
+    for (int q = 0; q < 16; ++q) tmem_st_c(tg + TM_CPC * (16 * par + q), v[par][q]);
 }
 
 // mid: untangle (registers) x generator -> first inverse pass.  GT: the generator values come from TMEM (tg, see
 // f4_store_generator); otherwise they sit in Z (bulk-copied there in the padded layout) and are multiplied in place.
+// Quarter-warp q4 works on Z block z0, z2, z1, z3 (in that order): z0 and z2 = z0 + RF1 read the two halves of the same
+// forward block pair, so with 8-byte elements (fp32 build, half-warp wavefronts) the 16 lanes of a half-warp fall on 16
+// different bank pairs; with 16-byte elements a wavefront is a quarter-warp and either order is conflict-free.
 template <int NF, int RF1, bool GT = false>
 __device__ __forceinline__ void f4_mid(const SmemArr& U, const SmemArr& Z, int br, const F4Own& o, int lane,
                                        const cplx* __restrict__ tw, uint32_t tg = 0) {
   constexpr int RI1 = 2 * RF1;
   const int q4 = lane >> 3;
-  const int s1 = q4 == 0 ? o.z0 : q4 == 1 ? o.z1 : q4 == 2 ? o.z2 : o.z3, s2 = lane & 7;
+  const int s1 = q4 == 0 ? o.z0 : q4 == 1 ? o.z2 : q4 == 2 ? o.z1 : o.z3, s2 = lane & 7;  // (half-warps: {z0, z2}, {z1, z3})
   const int kap = s1 + RI1 * s2;  // forward low-part kappa = inverse block index tau
   int kap2;
   bool selfzero = false;
@@ -374,14 +383,16 @@ __global__ void __launch_bounds__(Fused4Shape<LOG2M>::NT * NGRP, 1) td_fused4_ke
     f4_store_generator(P4.Gp[s] + (size_t)br * Sh::PADM, own, lane, tcol + F4_TC_G);
     if (MODE == MODE_LOGLIKE) {
       const double* drow = P.d + sg.off;
+      double2 dvs[IT * RF1];   // loads first, (volatile) TMEM stores after: the latencies overlap
 #pragma unroll
       for (int it = 0; it < IT; ++it)
 #pragma unroll
         for (int ss = 0; ss < RF1; ++ss) {
           const int i0 = 2 * (tid + it * NT + ss * S1);
-          double2 dv = make_double2(i0 < sg.n ? __ldg(drow + i0) : 0.0, i0 + 1 < sg.n ? __ldg(drow + i0 + 1) : 0.0);
-          tmem_st_c64(tcol + F4_TC_D + 4 * (it * RF1 + ss), dv);
+          dvs[it * RF1 + ss] = make_double2(i0 < sg.n ? __ldg(drow + i0) : 0.0, i0 + 1 < sg.n ? __ldg(drow + i0 + 1) : 0.0);
         }
+#pragma unroll
+      for (int q = 0; q < IT * RF1; ++q) tmem_st_c64(tcol + F4_TC_D + 4 * q, dvs[q]);
     }
     tmem_wait_st();
     for (long long b = vblock; b < Bs; b += vgrid) {
