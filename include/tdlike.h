@@ -156,7 +156,9 @@ td_status td_set_path(td_handle* h, int path);
 
 /* td_set_fft_variant - which implementation serves the FFT path: 0 = automatic (fused
  * shared-memory kernel where a segment's transform fits one SM, staged global-memory kernels
- * otherwise), 1 = same as 0, 2 = force the staged kernels for every segment (tests, profiling). */
+ * otherwise; ringdown parameter rows synthesised inside the fused kernel's first pass), 1 = as 0 but
+ * td_loglike_family_batch always synthesises into the scratch panel first (the r01 route; tests, profiling),
+ * 2 = force the staged kernels for every segment (tests, profiling). */
 td_status td_set_fft_variant(td_handle* h, int variant);
 
 /* td_precision: arithmetic of the FFT-path evaluation (td_set_precision). */

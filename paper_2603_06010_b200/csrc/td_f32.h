@@ -17,6 +17,7 @@ inline bool supported(int log2M) { return log2M >= 10 && log2M <= 13; }
 struct SegIn {
   long long off;      // offset of the segment inside d / a row of H (elements)
   int n;              // N_s
+  int sid;            // index of the segment in the handle
   const void* Gp64;   // device double2 [2][padded(M)]: the fp64 generator spectrum in the padded Z layout
   double rho0;        // rho_s(0): samples are scaled by rho0^(-1/2) before rounding, the spectrum by rho0^(+1/2)
 };
@@ -43,6 +44,8 @@ struct Launch {
   double* out1;
   int accumulate;
   int mode;  // td::MODE_LOGLIKE / MODE_INNER / MODE_STOREZ
+  int syn = 0;      // 1: H holds ringdown parameter rows (ldh = 5 x segments of the handle), fused4 classes, MODE_LOGLIKE only
+  double fs = 0.0;  // sampling rate (syn only)
 };
 // one launch of the class's kernel (dry: configure only - attribute, occupancy cache)
 td_status launch(const ClassTables& t, const Launch& L, int num_sms, int device, cudaStream_t st, bool dry);

@@ -23,7 +23,7 @@ namespace TD_NS {
 struct SegDev {
   long long off;    // offset of this segment inside d / a row of H (elements)
   int n;            // N_s
-  int _pad;
+  int _pad;         // index of the segment in the handle (the SYN kernels find the segment's parameter row with it)
   const cplx* G;    // [2][M]: even-bin then odd-bin generator spectrum, DIT input order, scaled
   cplx* zd;         // [M]: z of the data vector d (td_inner_batch only)
   double rscale;    // fp32 evaluation only: samples are multiplied by rscale = rho_s(0)^(-1/2) in fp64 before they are

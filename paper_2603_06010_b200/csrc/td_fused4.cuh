@@ -21,6 +21,7 @@
 #pragma once
 #include "td_fused.cuh"
 #include "td_dit16.cuh"
+#include "td_ring.cuh"
 
 namespace TD_NS {
 
@@ -53,7 +54,8 @@ template <int LOG2M> struct Fused4Shape {
   // bytes of one item pipeline (NGRP > 1: several independent pipelines share a CTA, see the kernel), 16-byte granular
   static constexpr size_t group_bytes() { return (smem_bytes() + 15) & ~(size_t)15; }
   static constexpr size_t smem_bytes() {
-    return sizeof(cplx) * (2 * (size_t)PADNF + 2 * (size_t)PADM + TWS) + sizeof(double) * 4 * NW + 48 + F4_SEGCACHE * sizeof(SegDev)
+    return sizeof(cplx) * (2 * (size_t)PADNF + 2 * (size_t)PADM + TWS) + sizeof(double) * 4 * NW + 48 + F4_SEGCACHE * sizeof(SegDev) +
+           96   // RingConsts of the item in flight (SYN kernels)
 #ifdef TD_PHASE_CLOCKS
            + 16 * 16 * sizeof(long long)
 #endif
@@ -64,6 +66,8 @@ template <int LOG2M> struct Fused4Shape {
 struct Fused4Params {
   FusedParams base;
   const cplx* const* Gp;  // device array [n_seg]: generator spectrum in the PADDED Z layout [2][padded(M)]
+  double fs;              // SYN kernels: sampling rate; base.H then holds the parameter rows [B][ldh], ldh = 5 x (segments of the
+                          // handle), the row of segment record sg at 5 sg._pad (td_ring.cuh)
 #ifdef TD_DEBUG_KNOBS
   int skew;               // debug builds: cycles the odd-bin warps wait after the barrier that follows pass 1
 #endif
@@ -280,8 +284,11 @@ __device__ long long g_phase_clk[148 * 16 * 16];
 // mbarrier, named barrier and TMEM windows) that work on different templates.  A kernel that uses tensor memory is limited
 // to one CTA per SM (profiles/r02_c2_fused4_ncu.md), so this is how the fp32 build - whose working set and register need
 // are half the fp64 ones - puts two items on an SM: their load / butterfly / store phases interleave instead of adding up.
-template <int LOG2M, int MODE, int NGRP = 1>
+// SYN = 1: the template rows are damped sinusoids synthesised from 5 parameters per (template, segment) inside the first
+// pass (td_ring.cuh) - no row in memory, no TMA copy; MODE_LOGLIKE only.
+template <int LOG2M, int MODE, int NGRP = 1, int SYN = 0>
 __global__ void __launch_bounds__(Fused4Shape<LOG2M>::NT * NGRP, 1) td_fused4_kernel(const Fused4Params P4) {
+  static_assert(SYN == 0 || MODE == MODE_LOGLIKE, "synthesis is wired into the log-likelihood mode only");
   using Sh = Fused4Shape<LOG2M>;
   constexpr int M = Sh::M, NF = Sh::NF, TW = 2 * M, NT = Sh::NT, NW = Sh::NW, NWB = Sh::NWB;
   constexpr int TMEM_COLS = Sh::tmem_cols(NGRP);
@@ -307,6 +314,7 @@ __global__ void __launch_bounds__(Fused4Shape<LOG2M>::NT * NGRP, 1) td_fused4_ke
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(reinterpret_cast<double*>(reinterpret_cast<cplx*>(smem_raw) + 2 * Sh::PADNF + 2 * Sh::PADM + Sh::TWS) + 4 * NW + 1);
   SegDev* segS = reinterpret_cast<SegDev*>(red + 4 * NW + 3);
   const SegDev* segs = P.n_seg <= F4_SEGCACHE ? segS : P.segs;
+  RingConsts* rcs = reinterpret_cast<RingConsts*>(segS + F4_SEGCACHE);
   double* stH = reinterpret_cast<double*>(sm);  // the staged template row lives in the U region (dead after mid)
   const int tid = (int)threadIdx.x - grp * NT, warp = tid >> 5, lane = tid & 31;   // within the group
   const int cwarp = (int)threadIdx.x >> 5;                                        // within the CTA (TMEM lane quarter, window)
@@ -319,7 +327,7 @@ __global__ void __launch_bounds__(Fused4Shape<LOG2M>::NT * NGRP, 1) td_fused4_ke
   if (tid == 0) mbar_init(mbar_rows, 1);
   if (cwarp == 0) tmem_alloc<TMEM_COLS>(smem_u32(tmem_slot));
 #ifdef TD_PHASE_CLOCKS
-  long long* clk_s = reinterpret_cast<long long*>(segS + F4_SEGCACHE);
+  long long* clk_s = reinterpret_cast<long long*>(reinterpret_cast<unsigned char*>(segS + F4_SEGCACHE) + 96);
   if (tid < 16 * NW) clk_s[tid] = 0;
   long long tlast = clock64();
 #endif
@@ -336,7 +344,16 @@ __global__ void __launch_bounds__(Fused4Shape<LOG2M>::NT * NGRP, 1) td_fused4_ke
     drow = P.d + sg.off;
     hrow = (MODE == MODE_STOREZ) ? drow : P.H + b * P.ldh + sg.off;
     n = sg.n;
+    if constexpr (SYN) return true;   // nothing to stage: the "row" is 5 parameters
     return ((reinterpret_cast<uintptr_t>(hrow) & 15) == 0) && ((n & 1) == 0);
+  };
+  // SYN: warp 0 computes the constants of item (b, s) into shared memory and completes the phase of the mbarrier that the
+  // first pass waits on (the hand-over a TMA row copy makes with its byte count)
+  auto prepare_consts = [&](long long b, int s) {  // executed by WARP 0
+    const SegDev sg2 = segs[s];
+    ring_prepare(P.H + b * P.ldh + 5 * sg2._pad, P4.fs, 2 * NT, lane, rcs);
+    __syncwarp();
+    if (lane == 0) mbar_arrive(mbar_rows);
   };
   auto prefetch_rows = [&](long long b, int s) {  // issued by ONE thread
     const double *drow, *hrow; int n;
@@ -375,7 +392,8 @@ __global__ void __launch_bounds__(Fused4Shape<LOG2M>::NT * NGRP, 1) td_fused4_ke
   {
     const double *dr, *hr; int nn;
     staged = rows(vblock, 0, dr, hr, nn);
-    if (tid == 0 && active) prefetch_rows(vblock, 0);
+    if constexpr (SYN) { if (warp == 0 && active) prepare_consts(vblock, 0); }
+    else if (tid == 0 && active) prefetch_rows(vblock, 0);
   }
   for (int s = 0; active && s < P.n_seg; ++s) {
     const SegDev sg = segs[s];
@@ -409,6 +427,17 @@ __global__ void __launch_bounds__(Fused4Shape<LOG2M>::NT * NGRP, 1) td_fused4_ke
         TDCLK(1);
         cplx xs[IT][RF1];
         double2 hs[IT][RF1];   // the staged samples, fp64 in both precisions
+        if constexpr (SYN) {
+          // this thread's pairs are 2 tid + 2 NT k, k = it + IT ss (2 NT IT = 2 S1): synthesised, never read
+          static_assert(2 * NT * IT == 2 * S1, "pair indices of a thread form one arithmetic progression");
+          const RingConsts rc = *rcs;
+          double2 hf[IT * RF1];
+          ring_pairs<IT * RF1>(rc, 2 * tid, ilog2(2 * NT), sg.n, hf);
+#pragma unroll
+          for (int it = 0; it < IT; ++it)
+#pragma unroll
+            for (int ss = 0; ss < RF1; ++ss) hs[it][ss] = hf[it + IT * ss];
+        } else {
 #pragma unroll
         for (int it = 0; it < IT; ++it)
 #pragma unroll
@@ -418,6 +447,7 @@ __global__ void __launch_bounds__(Fused4Shape<LOG2M>::NT * NGRP, 1) td_fused4_ke
             if (i0 < sg.n) hv = *reinterpret_cast<const double2*>(stH + i0);  // n even on this path: i0 + 1 < n too
             hs[it][ss] = hv;
           }
+        }
         if (MODE == MODE_LOGLIKE) {
           tmem_wait_ld();
           tmem_use16(dr[0]); tmem_use16(dr[1]);
@@ -470,7 +500,8 @@ __global__ void __launch_bounds__(Fused4Shape<LOG2M>::NT * NGRP, 1) td_fused4_ke
       TDCLK(10);
       group_sync();
       // every warp is past mid: the U region is dead and takes the next item's template row
-      if (tid == 0 && have_next) prefetch_rows(nb, ns);
+      if constexpr (SYN) { if (warp == 0 && have_next) prepare_consts(nb, ns); }
+      else if (tid == 0 && have_next) prefetch_rows(nb, ns);
       TDCLK(11);
       // ---------------- last inverse pass (radix RI1, joins the branches) + pruned radix-2 stage + S5
       double acc0 = 0.0, acc1 = 0.0;

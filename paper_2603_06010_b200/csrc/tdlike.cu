@@ -375,9 +375,10 @@ td_status launch_fused_nt(td_handle* h, const FusedParams& P, cudaStream_t st, b
   return TD_OK;
 }
 
-template <int LOG2M, int MODE>
-td_status launch_fused4(td_handle* h, const FusedParams& P, const cplx* const* Gp, cudaStream_t st, bool dry) {
-  auto kern = td_fused4_kernel<LOG2M, MODE>;
+// SYN = 1: P.H holds parameter rows (ldh = 5 n_seg), the rows are synthesised in the first pass (td_ring.cuh)
+template <int LOG2M, int MODE, int SYN = 0>
+td_status launch_fused4(td_handle* h, const FusedParams& P, const cplx* const* Gp, cudaStream_t st, bool dry, double fs = 0.0) {
+  auto kern = td_fused4_kernel<LOG2M, MODE, 1, SYN>;
   constexpr int NT = Fused4Shape<LOG2M>::NT;
   const size_t smem = Fused4Shape<LOG2M>::smem_bytes();
   static int cache[TD_MAX_DEV];
@@ -390,7 +391,7 @@ td_status launch_fused4(td_handle* h, const FusedParams& P, const cplx* const* G
   const long long maxg = (long long)nb * h->num_sms;
   const int grid = (int)std::max<long long>(1, std::min<long long>(MODE == MODE_STOREZ ? 1 : P.B, maxg));
   Fused4Params P4;
-  P4.base = P; P4.Gp = Gp;
+  P4.base = P; P4.Gp = Gp; P4.fs = fs;
 #ifdef TD_DEBUG_KNOBS
   P4.skew = tune(1, 0);
 #endif
@@ -425,7 +426,7 @@ td_status launch_cluster(td_handle* h, const FusedParams& P, const cplx* const* 
   const long long want = MODE == MODE_STOREZ ? 1 : P.B;
   cfg.gridDim = dim3(2 * (unsigned)std::max<long long>(1, std::min<long long>(want, ncl)));
   Fused4Params P4;
-  P4.base = P; P4.Gp = Gp;
+  P4.base = P; P4.Gp = Gp; P4.fs = 0.0;
 #ifdef TD_DEBUG_KNOBS
   P4.skew = 0;
 #endif
@@ -613,6 +614,40 @@ td_status launch_cdo(td_handle* h, const double* d, const double* H, int64_t ldh
 }
 
 // FFT path over all size classes.  MODE_LOGLIKE: out0 = loglike.  MODE_INNER: out0 = <d,h>, out1 = <h,h>.
+// Ringdown parameters straight into the fused kernels (td_ring.cuh): possible when every size class of the handle is served
+// by td_fused4_kernel (segments of 513..4096 samples) and none is sent elsewhere (dense chooser, forced staged variant)
+bool ring_fused_ok(const td_handle* h) {
+  if (h->fft_variant != 0 || (h->path != TD_PATH_AUTO && h->path != TD_PATH_FFT)) return false;
+  for (const ClassInfo& c : h->classes)
+    if (c.log2M < 10 || c.log2M > 12 || !c.d_Gp) return false;
+  return true;
+}
+td_status run_ring_fused(td_handle* h, const double* d, const double* params, int64_t B, double fs, double* out,
+                         cudaStream_t st, bool dry = false) {
+  int accumulate = 0;
+  const bool f32 = h->precision == TD_PREC_F32;
+  for (const ClassInfo& cls : h->classes) {
+    if (f32 && cls.has32) {
+      td32api::Launch L;
+      L.d = d; L.H = params; L.ldh = 5ll * h->n_seg; L.B = B; L.out0 = out; L.out1 = nullptr; L.accumulate = accumulate;
+      L.mode = MODE_LOGLIKE; L.syn = 1; L.fs = fs;
+      td_status s = td32api::launch(cls.t32, L, h->num_sms, h->device, st, dry);
+      if (s != TD_OK) return s;
+    } else {
+      FusedParams P;
+      P.d = d; P.H = params; P.ldh = 5ll * h->n_seg; P.B = B; P.out0 = out; P.out1 = nullptr;
+      P.segs = cls.d_segs; P.n_seg = (int)cls.seg_ids.size(); P.accumulate = accumulate; P.T = cls.T;
+      td_status s = cls.log2M == 10 ? launch_fused4<10, MODE_LOGLIKE, 1>(h, P, cls.d_Gp, st, dry, fs)
+                  : cls.log2M == 11 ? launch_fused4<11, MODE_LOGLIKE, 1>(h, P, cls.d_Gp, st, dry, fs)
+                                    : launch_fused4<12, MODE_LOGLIKE, 1>(h, P, cls.d_Gp, st, dry, fs);
+      if (s != TD_OK) return s;
+    }
+    if (!dry) { if (f32 && cls.has32) ++h->last_launches; accumulate = 1; }   // (launch_fused4 counts its own)
+  }
+  if (!dry) h->last_path = TD_PATH_FFT;
+  return TD_OK;
+}
+
 // `f32`: classes that have fp32 tables and are not served by the dense kernel run the fp32 build of their kernel
 template <int MODE>
 td_status run_fft_path(td_handle* h, const double* d, const double* H, int64_t ldh, int64_t B, double* out0,
@@ -746,6 +781,10 @@ template <int MODE> td_status warm_mode(td_handle* h) {
   return TD_OK;
 }
 td_status warm_kernels(td_handle* h) {
+  if (ring_fused_ok(h)) {
+    td_status r = run_ring_fused(h, nullptr, nullptr, 1, 1.0, nullptr, nullptr, true);
+    if (r != TD_OK) return r;
+  }
   td_status s = warm_mode<MODE_LOGLIKE>(h);
   if (s == TD_OK) s = warm_mode<MODE_INNER>(h);
   if (s == TD_OK) s = warm_mode<MODE_STOREZ>(h);
@@ -883,7 +922,7 @@ static td_status create_impl(td_handle* h, const double* acf, const int64_t* seg
     std::vector<SegDev> sd(c.seg_ids.size());
     for (size_t i = 0; i < sd.size(); ++i) {
       const SegHost& sg = h->segs[c.seg_ids[i]];
-      sd[i].off = sg.off; sd[i].n = sg.n; sd[i]._pad = 0; sd[i].G = sg.G; sd[i].zd = sg.zd; sd[i].rscale = 1.0;
+      sd[i].off = sg.off; sd[i].n = sg.n; sd[i]._pad = c.seg_ids[i]; sd[i].G = sg.G; sd[i].zd = sg.zd; sd[i].rscale = 1.0;
     }
     CK(cudaMalloc(&c.d_segs, sizeof(SegDev) * sd.size()));
     CK(cudaMemcpy(c.d_segs, sd.data(), sizeof(SegDev) * sd.size(), cudaMemcpyHostToDevice));
@@ -1071,6 +1110,13 @@ td_status td_loglike_batch_host(td_handle* h, const double* d, const double* H, 
 
 static td_status family_batch_impl(td_handle* h, const double* d, int family, const double* params, int64_t B, double fs,
                                    double* out, cudaStream_t st) {
+  // Small batches (launch-bound): the rows are synthesised inside the first pass of the fused kernel, one launch, no panel.
+  // Large batches: the separate synthesis kernel + panel is measured 3 % (fp64) to 25 % (fp32) faster on c2, because the
+  // in-kernel synthesis puts its exp / sincos anchors on the pipes that already bound the FFT kernel (profiles/r02_ring_fused.md).
+  if (family == SYN_RINGDOWN && ring_fused_ok(h) && B <= 2ll * h->num_sms) {
+    h->last_launches = 0;
+    return run_ring_fused(h, d, params, B, fs, out, st);
+  }
   const int64_t n = h->n_tot, ldh = (n + 1) & ~1ll;  // even leading dimension: 16-byte aligned rows
   const int64_t CH = family_chunk_rows(h, B, ldh);
   {
@@ -1204,7 +1250,7 @@ td_status td_set_precision(td_handle* h, int precision) {
       std::vector<td32api::SegIn> in(c.seg_ids.size());
       for (size_t i = 0; i < in.size(); ++i) {
         const SegHost& sg = h->segs[c.seg_ids[i]];
-        in[i].off = sg.off; in[i].n = sg.n; in[i].Gp64 = sg.Gp; in[i].rho0 = sg.rho0;
+        in[i].off = sg.off; in[i].n = sg.n; in[i].sid = c.seg_ids[i]; in[i].Gp64 = sg.Gp; in[i].rho0 = sg.rho0;
       }
       td_status s = td32api::build_class(c.log2M, (int)in.size(), in.data(), c.T, &c.t32);
       if (s != TD_OK) return s;
@@ -1212,6 +1258,12 @@ td_status td_set_precision(td_handle* h, int precision) {
       for (int mode = 0; mode < 3; ++mode) {  // dry pass: attributes and occupancy of the fp32 kernels
         td32api::Launch L = {};
         L.B = 1; L.mode = mode;
+        s = td32api::launch(c.t32, L, h->num_sms, h->device, nullptr, true);
+        if (s != TD_OK) return s;
+      }
+      if (c.log2M <= 12) {   // and of the fp32 kernel that synthesises ringdown rows in its first pass
+        td32api::Launch L = {};
+        L.B = 1; L.mode = MODE_LOGLIKE; L.syn = 1; L.fs = 1.0;
         s = td32api::launch(c.t32, L, h->num_sms, h->device, nullptr, true);
         if (s != TD_OK) return s;
       }

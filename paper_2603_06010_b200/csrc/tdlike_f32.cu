@@ -28,9 +28,10 @@ __global__ void cvt_cplx_kernel(const double2* __restrict__ src, float2* __restr
 // Two item pipelines per CTA (NGRP = 2, td_fused4.cuh): the fp32 working set of a pipeline is 113 KB at M = 4096, a kernel
 // that uses tensor memory gets one CTA per SM, so the second item on the SM lives in the same CTA.
 constexpr int F32_NGRP = 2;
-template <int LOG2M, int MODE>
-td_status launch_fused4(const td32api::ClassTables& t, const FusedParams& P, int num_sms, int device, cudaStream_t st, bool dry) {
-  auto kern = td_fused4_kernel<LOG2M, MODE, F32_NGRP>;
+template <int LOG2M, int MODE, int SYN = 0>
+td_status launch_fused4(const td32api::ClassTables& t, const FusedParams& P, int num_sms, int device, cudaStream_t st, bool dry,
+                        double fs = 0.0) {
+  auto kern = td_fused4_kernel<LOG2M, MODE, F32_NGRP, SYN>;
   constexpr int NT = Fused4Shape<LOG2M>::NT * F32_NGRP;
   const size_t smem = Fused4Shape<LOG2M>::group_bytes() * F32_NGRP;
   static int cache[TD_MAX_DEV];
@@ -42,7 +43,7 @@ td_status launch_fused4(const td32api::ClassTables& t, const FusedParams& P, int
   const long long want = MODE == MODE_STOREZ ? 1 : (P.B + F32_NGRP - 1) / F32_NGRP;   // CTAs: one per F32_NGRP items
   const int grid = (int)std::max<long long>(1, std::min<long long>(want, num_sms));
   Fused4Params P4;
-  P4.base = P; P4.Gp = reinterpret_cast<const cplx* const*>(t.Gp_ptrs);
+  P4.base = P; P4.Gp = reinterpret_cast<const cplx* const*>(t.Gp_ptrs); P4.fs = fs;
   kern<<<grid, NT, smem, st>>>(P4);
   CK(cudaGetLastError());
   return TD_OK;
@@ -73,7 +74,7 @@ td_status launch_cluster(const td32api::ClassTables& t, const FusedParams& P, in
   const long long want = MODE == MODE_STOREZ ? 1 : P.B;
   cfg.gridDim = dim3(2 * (unsigned)std::max<long long>(1, std::min<long long>(want, ncl)));
   Fused4Params P4;
-  P4.base = P; P4.Gp = reinterpret_cast<const cplx* const*>(t.Gp_ptrs);
+  P4.base = P; P4.Gp = reinterpret_cast<const cplx* const*>(t.Gp_ptrs); P4.fs = 0.0;
   CK(cudaLaunchKernelEx(&cfg, kern, P4));
   return TD_OK;
 }
@@ -123,7 +124,7 @@ td_status build_class(int log2M, int n_seg, const SegIn* segs, const void* T64, 
     if (cudaMalloc(&t.zd[s], sizeof(float2) * M) != cudaSuccess) return fail(TD_ENOMEM);
     cvt_cplx_kernel<<<(unsigned)((gp_elems + 255) / 256), 256>>>(static_cast<const double2*>(segs[s].Gp64),
                                                                  static_cast<float2*>(t.Gp[s]), gp_elems, sqrt(segs[s].rho0));
-    sd[s].off = segs[s].off; sd[s].n = segs[s].n; sd[s]._pad = 0; sd[s].G = nullptr;
+    sd[s].off = segs[s].off; sd[s].n = segs[s].n; sd[s]._pad = segs[s].sid; sd[s].G = nullptr;
     sd[s].zd = static_cast<cplx*>(t.zd[s]); sd[s].rscale = 1.0 / sqrt(segs[s].rho0);
     gp[s] = static_cast<const cplx*>(t.Gp[s]);
   }
@@ -143,6 +144,15 @@ td_status launch(const ClassTables& t, const Launch& L, int num_sms, int device,
   P.d = L.d; P.H = L.H; P.ldh = L.ldh; P.B = L.B; P.out0 = L.out0; P.out1 = L.out1;
   P.segs = static_cast<const SegDev*>(t.segs); P.n_seg = t.n_seg; P.accumulate = L.accumulate;
   P.T = static_cast<const cplx*>(t.T);
+  if (L.syn) {
+    if (L.mode != MODE_LOGLIKE) return TD_EINVAL;
+    switch (t.log2M) {
+      case 10: return launch_fused4<10, MODE_LOGLIKE, 1>(t, P, num_sms, device, st, dry, L.fs);
+      case 11: return launch_fused4<11, MODE_LOGLIKE, 1>(t, P, num_sms, device, st, dry, L.fs);
+      case 12: return launch_fused4<12, MODE_LOGLIKE, 1>(t, P, num_sms, device, st, dry, L.fs);
+      default: return TD_EUNSUPPORTED;
+    }
+  }
   switch (L.mode) {
     case MODE_LOGLIKE: return launch_mode<MODE_LOGLIKE>(t, P, num_sms, device, st, dry);
     case MODE_INNER: return launch_mode<MODE_INNER>(t, P, num_sms, device, st, dry);

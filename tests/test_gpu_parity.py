@@ -469,10 +469,39 @@ def test_family_params_entry_matches_oracle(name, B, n_scale):
     with tdb.TDLikelihood(w.acf, w.seg_lengths) as h:
         out = h.loglike_family_batch(_dev(w.d), w.family, _dev(w.params), w.fs)
         torch.cuda.synchronize()
-        assert h.last_launches() >= 2
+        # c1 / c2 at these batch sizes: ringdown rows synthesised inside the fused kernel's first pass (td_ring.cuh), ONE
+        # launch; everything else: synthesis kernel + panel + likelihood kernels
+        fused_route = name in ("c1", "c2")
+        assert (h.last_launches() == 1) if fused_route else (h.last_launches() >= 2)
         out_host = h.loglike_family_batch_host(w.d, w.family, w.params, w.fs)
-    _assert_close(out.cpu().numpy(), ref, what=f"{name} ringdown params")
+        h.set_fft_variant(1)                                   # the panel route for every family
+        out_panel = h.loglike_family_batch(_dev(w.d), w.family, _dev(w.params), w.fs)
+        torch.cuda.synchronize()
+        assert h.last_launches() >= 2
+    _assert_close(out.cpu().numpy(), ref, what=f"{name} params")
+    _assert_close(out_panel.cpu().numpy(), ref, what=f"{name} params, panel route")
     assert np.array_equal(out.cpu().numpy(), out_host)
+
+
+def test_ringdown_fused_synthesis_chooser_and_fp32():
+    """Above 2 x (SM count) templates the chooser takes the panel route (measured faster, profiles/r02_ring_fused.md); the
+    fused route also exists in the fp32 build (two item pipelines per CTA)."""
+    w = W.make("c2", B=700, n_scale=2)
+    H_ref = OT.family_rows(w.family, w.params, w.seg_lengths, w.fs)
+    ref = O.loglike_batch(w.acf, w.seg_lengths, w.d, H_ref)
+    with tdb.TDLikelihood(w.acf, w.seg_lengths) as h:
+        d, p = _dev(w.d), _dev(w.params)
+        out_big = h.loglike_family_batch(d, w.family, p, w.fs).cpu().numpy()
+        n_big = h.last_launches()
+        out_small = h.loglike_family_batch(d, w.family, p[:100].contiguous(), w.fs).cpu().numpy()
+        n_small = h.last_launches()
+        h.set_precision(tdb.TD_PREC_F32)
+        out32 = h.loglike_family_batch(d, w.family, p[:100].contiguous(), w.fs).cpu().numpy()
+        n32 = h.last_launches()
+    assert n_big >= 2 and n_small == 1 and n32 == 1
+    _assert_close(out_big, ref, what="c2 params, large batch (panel)")
+    _assert_close(out_small, ref[:100], what="c2 params, small batch (fused)")
+    _assert_close(out32, ref[:100], tol=2e-5, what="c2 params, fused, fp32")
 
 
 def test_ringdown_params_entry_errors_and_edges():
