@@ -18,6 +18,7 @@
 #include "td_dot.cuh"
 #include "td_fused.cuh"
 #include "td_cluster.cuh"
+#include "td_cluster16.cuh"
 #include "td_fused4.cuh"
 #include "td_setup.cuh"
 #include "td_staged.cuh"
@@ -46,6 +47,7 @@ struct SegHost {
   double* a = nullptr;  // device [n]
   cplx* G = nullptr;    // device [2][M]
   cplx* Gp = nullptr;   // device [2][padded(M)], padded Z layout (fused4 classes only)
+  cplx* Gc16 = nullptr; // device [16][padded(8192)]: per-CTA generator values of the 16-CTA cluster kernel (M = 65536 only)
   cplx* zd = nullptr;   // device [M] (lazy)
 };
 
@@ -80,6 +82,7 @@ struct td_handle {
   std::vector<ClassInfo> classes;
   int path = TD_PATH_AUTO, fft_variant = 0, last_path = 0, last_launches = 0;
   int precision = TD_PREC_F64;
+  int cluster16_cap = 0;   // co-resident 16-CTA clusters of td_cluster16_kernel (0: M = 65536 stays on the staged kernels)
   int max_n = 0;
   // staged workspace: U / Z sized by td_create (two lanes of an L2-resident chunk), the per-block partial sums by
   // td_create / td_reserve (a batch larger than they hold is processed in sub-batches)
@@ -123,7 +126,7 @@ int next_log2(int n) { int l = 0; while ((1 << l) < n) ++l; return l; }
 
 void free_handle(td_handle* h) {
   if (!h) return;
-  for (auto& s : h->segs) { cudaFree(s.a); cudaFree(s.G); cudaFree(s.Gp); cudaFree(s.zd); }
+  for (auto& s : h->segs) { cudaFree(s.a); cudaFree(s.G); cudaFree(s.Gp); cudaFree(s.Gc16); cudaFree(s.zd); }
   for (auto& c : h->classes) { cudaFree(c.T); cudaFree(c.d_segs); cudaFree(c.d_Gp); if (c.has32) td32api::free_class(&c.t32); }
   cudaFree(h->wsU); cudaFree(h->wsZ); cudaFree(h->wsPartial); cudaFree(h->wsDot); cudaFree(h->ud); cudaFree(h->synH); cudaFree(h->synP); cudaFree(h->synSeg);
   cudaFree(h->hsD); cudaFree(h->hsH[0]); cudaFree(h->hsH[1]); cudaFree(h->hsOut);
@@ -648,6 +651,78 @@ td_status run_ring_fused(td_handle* h, const double* d, const double* params, in
   return TD_OK;
 }
 
+// ---- M = 65536 on a 16-CTA cluster (td_cluster16.cuh): one launch per segment + the rank-ordered sum of the 16 partials
+template <int MODE>
+td_status launch_cluster16(td_handle* h, const Cluster16Params& PC, int* nclusters, cudaStream_t st, bool dry) {
+  auto kern = td_cluster16_kernel<MODE>;
+  const size_t smem = Cluster16Shape::smem_bytes();
+  static int cache[TD_MAX_DEV];  // 0 = not configured on this device yet, else 1 + clusters that can be co-resident
+  if (h->device < 0 || h->device >= TD_MAX_DEV) return TD_EUNSUPPORTED;
+  cudaLaunchConfig_t cfg = {};
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeClusterDimension;
+  attr[0].val.clusterDim.x = Cluster16Shape::CS; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+  cfg.blockDim = dim3(Cluster16Shape::NT); cfg.dynamicSmemBytes = smem; cfg.stream = st;
+  cfg.attrs = attr; cfg.numAttrs = 1;
+  if (cache[h->device] == 0) {
+    int n = 0;
+    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) == cudaSuccess &&
+        cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) == cudaSuccess) {
+      cfg.gridDim = dim3(Cluster16Shape::CS * (h->num_sms / Cluster16Shape::CS));
+      if (cudaOccupancyMaxActiveClusters(&n, kern, &cfg) != cudaSuccess) n = 0;
+    }
+    cudaGetLastError();   // a device that cannot host the cluster is not an error: the staged kernels serve the class
+    cache[h->device] = n + 1;
+  }
+  *nclusters = cache[h->device] - 1;
+  if (dry || *nclusters < 1) return TD_OK;
+  const long long want = MODE == MODE_STOREZ ? 1 : PC.base.B;
+  cfg.gridDim = dim3(Cluster16Shape::CS * (unsigned)std::max<long long>(1, std::min<long long>(want, *nclusters)));
+  CK(cudaLaunchKernelEx(&cfg, kern, PC));
+  ++h->last_launches;
+  return TD_OK;
+}
+
+// how many 16-CTA clusters of the kernel fit the device (0: the class stays on the staged kernels)
+int cluster16_capacity(td_handle* h) {
+  int n = 0;
+  Cluster16Params PC = {};
+  if (launch_cluster16<MODE_LOGLIKE>(h, PC, &n, nullptr, true) != TD_OK) return 0;
+  int m = 0;
+  if (launch_cluster16<MODE_INNER>(h, PC, &m, nullptr, true) != TD_OK) return 0;
+  int z = 0;
+  if (launch_cluster16<MODE_STOREZ>(h, PC, &z, nullptr, true) != TD_OK) return 0;
+  return std::min(n, std::min(m, z));
+}
+
+template <int MODE>
+td_status run_cluster16(td_handle* h, const ClassInfo& cls, int idx_in_class, const double* d, const double* H, int64_t ldh,
+                        int64_t B, double* out0, double* out1, double scale0, double scale1, int accumulate, cudaStream_t st) {
+  const SegHost& sg = h->segs[cls.seg_ids[idx_in_class]];
+  const int64_t SB = std::max<int64_t>(1, (int64_t)(h->wsP_elems / (Cluster16Shape::CS * 2)));   // templates per partial buffer
+  h->touched = true;
+  const int64_t Bn = (MODE == MODE_STOREZ) ? 1 : B;
+  for (int64_t b0 = 0; b0 < Bn; b0 += SB) {
+    const int64_t nb = std::min<int64_t>(SB, Bn - b0);
+    Cluster16Params PC;
+    PC.base.d = d; PC.base.H = H ? H + b0 * ldh : nullptr; PC.base.ldh = ldh; PC.base.B = nb;
+    PC.base.out0 = nullptr; PC.base.out1 = nullptr; PC.base.segs = cls.d_segs + idx_in_class; PC.base.n_seg = 1;
+    PC.base.accumulate = 0; PC.base.T = cls.T;
+    PC.Gp = sg.Gc16; PC.partial = h->wsPartial;
+    int ncl = 0;
+    td_status s = launch_cluster16<MODE>(h, PC, &ncl, st, false);
+    if (s != TD_OK) return s;
+    if (ncl < 1) return TD_EUNSUPPORTED;
+    if (MODE != MODE_STOREZ) {
+      lg_finish_kernel<<<(unsigned)((nb + 127) / 128), 128, 0, st>>>(h->wsPartial, Cluster16Shape::CS, (int)nb, out0 ? out0 + b0 : nullptr,
+                                                                    out1 ? out1 + b0 : nullptr, scale0, scale1, accumulate);
+      CK(cudaGetLastError());
+      ++h->last_launches;
+    }
+  }
+  return TD_OK;
+}
+
 // `f32`: classes that have fp32 tables and are not served by the dense kernel run the fp32 build of their kernel
 template <int MODE>
 td_status run_fft_path(td_handle* h, const double* d, const double* H, int64_t ldh, int64_t B, double* out0,
@@ -672,8 +747,14 @@ td_status run_fft_path(td_handle* h, const double* d, const double* H, int64_t l
       if (s != TD_OK) return s;
       accumulate = 1;
     } else {
-      for (int id : cls.seg_ids) {
-        td_status s = run_staged<MODE>(h, cls, h->segs[id], d, H, ldh, B, out0, out1, sc0, sc1, accumulate, st);
+      // M = 65536 on the 16-CTA cluster kernel only on request (variant 3): measured 0.885 ms against 0.737 ms for the staged
+      // kernels on c4 - its two all-to-all exchanges run at the 16 B/cycle/SM of distributed-shared-memory stores and only 7
+      // clusters (112 of 148 SMs) are co-resident (profiles/r02_c4_cluster16.md)
+      const bool c16 = cls.log2M == Cluster16Shape::LOG2M && h->fft_variant == 3 && h->cluster16_cap > 0;
+      for (size_t i = 0; i < cls.seg_ids.size(); ++i) {
+        const int id = cls.seg_ids[i];
+        td_status s = c16 ? run_cluster16<MODE>(h, cls, (int)i, d, H, ldh, B, out0, out1, sc0, sc1, accumulate, st)
+                          : run_staged<MODE>(h, cls, h->segs[id], d, H, ldh, B, out0, out1, sc0, sc1, accumulate, st);
         if (s != TD_OK) return s;
         accumulate = 1;
       }
@@ -781,6 +862,8 @@ template <int MODE> td_status warm_mode(td_handle* h) {
   return TD_OK;
 }
 td_status warm_kernels(td_handle* h) {
+  for (const ClassInfo& c : h->classes)
+    if (c.log2M == Cluster16Shape::LOG2M) h->cluster16_cap = cluster16_capacity(h);
   if (ring_fused_ok(h)) {
     td_status r = run_ring_fused(h, nullptr, nullptr, 1, 1.0, nullptr, nullptr, true);
     if (r != TD_OK) return r;
@@ -912,6 +995,12 @@ static td_status create_impl(td_handle* h, const double* acf, const int64_t* seg
         if (cudaMalloc(&sg.Gp, pb) != cudaSuccess) { st = TD_ENOMEM; break; }
         cudaMemsetAsync(sg.Gp, 0, pb, 0);
         gen_permute_kernel<<<(n2 + 255) / 256, 256>>>(F, sg.Gp, M, gscale, c.log2M == CLUSTER_LOG2M ? 2 : 1);
+      }
+      if (c.log2M == Cluster16Shape::LOG2M) {
+        const size_t cb = sizeof(cplx) * 16 * Cluster16Shape::PADZ;
+        if (cudaMalloc(&sg.Gc16, cb) != cudaSuccess) { st = TD_ENOMEM; break; }
+        cudaMemsetAsync(sg.Gc16, 0, cb, 0);
+        gen_permute_c16_kernel<<<(n2 + 255) / 256, 256>>>(F, sg.Gc16, gscale);
       }
       if (cudaGetLastError() != cudaSuccess) { st = TD_ECUDA; break; }
     }
@@ -1226,7 +1315,12 @@ td_status td_set_path(td_handle* h, int path) {
 }
 
 td_status td_set_fft_variant(td_handle* h, int variant) {
-  if (!h || variant < 0 || variant > 2) return TD_EINVAL;
+  if (!h || variant < 0 || variant > 3) return TD_EINVAL;
+  if (variant == 3) {   // the 16-CTA cluster kernel needs a 65536-class segment and a device that can host the cluster
+    bool has16 = false;
+    for (const ClassInfo& c : h->classes) has16 = has16 || c.log2M == Cluster16Shape::LOG2M;
+    if (!has16 || h->cluster16_cap < 1) return TD_EUNSUPPORTED;
+  }
   if (variant == 2) {
     DevGuard guard(h->device);
     if (!guard.ok) return TD_ECUDA;

@@ -92,6 +92,44 @@ def test_c4_long_segment_vs_library_levinson():
     ref = O.loglike_batch_solve_toeplitz(w.acf, w.seg_lengths, w.d, w.H)
     out, _, _ = _gpu_loglike(w)
     _assert_close(out, ref, what="c4")
+    # the same segment on the 16-CTA cluster kernel (td_cluster16.cuh, variant 3): all three kernel modes
+    dh_ref = None
+    with tdb.TDLikelihood(w.acf, w.seg_lengths) as h:
+        d, H = _dev(w.d), _dev(w.H)
+        dh_s, hh_s = h.inner_batch(d, H, want_hh=True)
+        dh_s, hh_s = dh_s.clone(), hh_s.clone()
+        h.set_fft_variant(3)
+        out16 = h.loglike_batch(d, H).cpu().numpy()
+        n16 = h.last_launches()
+        dh16, hh16 = h.inner_batch(d, H)
+        torch.cuda.synchronize()
+    _assert_close(out16, ref, what="c4 on the 16-CTA cluster kernel")
+    assert n16 == 2                                  # the cluster kernel + the rank-ordered sum of the 16 partials
+    scale = float(hh_s.abs().max())
+    assert float((hh16 - hh_s).abs().max()) <= 1e-9 * scale and float((dh16 - dh_s).abs().max()) <= 1e-9 * scale
+
+
+def test_cluster16_ragged_length_many_items_and_refusal():
+    """N = 40001 (odd, unaligned rows: scalar loads) and more templates than co-resident clusters, against the staged
+    kernels (themselves held to the oracle above); handles without a 65536-class segment refuse variant 3."""
+    rng = np.random.default_rng(16)
+    n = 40001
+    rho = W.acf_from_psd(4096.0, 2 * 65536, n)
+    d = rng.standard_normal(n) * 1e-21
+    H = rng.standard_normal((23, n)) * 1e-21
+    H[5] = d
+    with tdb.TDLikelihood(rho, [n]) as h:
+        ref = h.loglike_batch(_dev(d), _dev(H)).cpu().numpy()
+        h.set_fft_variant(3)
+        out = h.loglike_batch(_dev(d), _dev(H)).cpu().numpy()
+        out2 = h.loglike_batch(_dev(d), _dev(H)).cpu().numpy()
+    assert out[5] == 0.0 and np.array_equal(out, out2)
+    _assert_close(out, ref, what="cluster16, N = 40001")
+    w = W.make("c2", B=4)
+    with tdb.TDLikelihood(w.acf, w.seg_lengths) as h:
+        with pytest.raises(tdb.TDError) as e:
+            h.set_fft_variant(3)
+        assert e.value.status == tdb.TD_EUNSUPPORTED
 
 
 # ------------------------------------------------------------------ shapes: ragged, tiny, mixed classes
