@@ -321,7 +321,7 @@ td_status run_staged_sub(td_handle* h, const ClassInfo& cls, const SegHost& sg, 
     // (fusing the untangle into the inverse block kernel - one CTA building a block, or a mirror pair of blocks, of Z in
     // shared memory straight from U and G - was measured: 50-68 us per chunk against 18 + 24 us for the two kernels; the
     // gather serialises 16 index-heavy tasks per thread, which the stand-alone kernel hides behind 1.4 M threads)
-    lg_untangle_kernel<<<dim3((nf + LG_NT - 1) / LG_NT, 2, cb), LG_NT, 0, ls>>>(P);
+    lg_untangle_kernel<<<dim3((nf + LG_NT - 1) / LG_NT, 2, (cb + LG_UCPT - 1) / LG_UCPT), LG_NT, 0, ls>>>(P);
     if (cudaGetLastError() != cudaSuccess) { s = TD_ECUDA; break; }
     ++h->last_launches;
     s = staged_inverse_but_last(h->device, Z, 2 * cb, M, cls.T, TW, ls, &h->last_launches);
