@@ -35,6 +35,9 @@ branch against the AR(1) closed form row by row (test_p1_p9_large_batch_...).
 Very long segments (N = 2^20: neither the dense Cholesky nor a library Levinson solve finishes in test time): the exact
 Gaussian likelihood of an AR(p) process in closed form (`ar_acf`, `ar_quadform_closed`, O(N p); pin P19 holds it to the
 Cholesky route at small N and to the hand-evaluated AR(1) values of P3).
+The paper's own fast CPU method (GSCE: Gohberg-Semencul + circulant embedding + FFT) is written out as
+`gsce_factors` / `loglike_batch_gsce` and held to the Cholesky route by pin P20; bench.py times it as a second CPU context
+line (the O(N log N) route the paper advocates) - it is not what grades the GPU.
 Every function below is covered by at least one of them; nothing here is "parity unpinned".
 The template families / projection of the step before the hot path live in oracle/templates.py
 (pins P15-P18).
@@ -346,3 +349,43 @@ def ar_quadform_closed(phi: Sequence[float], s2: float, x: np.ndarray) -> float:
     for j in range(1, p + 1):
         e -= phi[j - 1] * x[p - j : x.size - j]
     return float(head + np.dot(e, e) / s2)
+
+
+# ----------------------------------------------------------------------------------------
+# The paper's fast CPU route: GSCE = Gohberg-Semencul + circulant embedding + FFT
+# ----------------------------------------------------------------------------------------
+# Eq. 14: C^{-1} = (1/x_1)(L_x L_x^T - R_x^T R_x), C x = e_1.  With x = a / v (Levinson), x_1 = 1/v:
+#     r^T C^{-1} r = ( ||L(a)^T r||^2 - ||L(b)^T r||^2 ) / v ,   b = (0, a_{N-1}, .., a_1).
+# Eqs. 15-16: a triangular Toeplitz product is a slice of a circulant product of size m >= 2N - 1, and a
+# circulant product is diagonal in the Fourier basis: (L(c)^T r)_i = sum_{j>=i} c_{j-i} r_j is the correlation of r with c,
+# irfft( conj(rfft(c, m)) * rfft(r, m) )[:N].  numpy's FFT, written exactly in that order; the generator transforms are the
+# once-per-segment "cached" part, the per-template work is one forward and two inverse real FFTs.
+
+
+def gsce_factors(acf: np.ndarray, seg_lengths: Sequence[int]) -> list:
+    """Per segment: (N, m, conj(rfft(a, m)), conj(rfft(b, m)), v) from the Levinson recursion (`levinson_durbin_fast`)."""
+    acf = np.asarray(acf, np.float64)
+    out = []
+    for lo, hi in _segments(seg_lengths):
+        n = hi - lo
+        a, v, _ = levinson_durbin_fast(acf[lo:hi])
+        b = gs_generators(a)
+        m = 2 * n   # any m >= 2n - 1 is exact (PAPER.md:246)
+        out.append((n, m, np.conj(np.fft.rfft(a, m)), np.conj(np.fft.rfft(b, m)), v))
+    return out
+
+
+def loglike_batch_gsce(acf: np.ndarray, seg_lengths: Sequence[int], d: np.ndarray, H: np.ndarray,
+                       factors: Optional[list] = None) -> np.ndarray:
+    """Same quantity as `loglike_batch` by the paper's GSCE route (Eqs. 14-16), batched over the rows of H."""
+    d = np.asarray(d, np.float64)
+    H = np.asarray(H, np.float64)
+    if factors is None:
+        factors = gsce_factors(acf, seg_lengths)
+    out = np.zeros(H.shape[0])
+    for (lo, hi), (n, m, Ac, Bc, v) in zip(_segments(seg_lengths), factors):
+        R = np.fft.rfft(d[None, lo:hi] - H[:, lo:hi], m, axis=1)
+        y1 = np.fft.irfft(Ac[None, :] * R, m, axis=1)[:, :n]
+        y2 = np.fft.irfft(Bc[None, :] * R, m, axis=1)[:, :n]
+        out += (np.einsum("ij,ij->i", y1, y1) - np.einsum("ij,ij->i", y2, y2)) / v
+    return -0.5 * out

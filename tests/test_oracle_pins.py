@@ -465,3 +465,17 @@ def test_p19_ar_closed_form_against_cholesky_route(phi):
     if p == 1:
         assert _rel(_ar1_closed(phi[0], s2, x), q) < 1e-12
         assert np.max(np.abs(rho - s2 * phi[0] ** np.arange(n) / (1 - phi[0] ** 2))) < 1e-12
+
+
+# ---------------------------------------------------------------- P20 the paper's GSCE route (Eqs. 14-16) against Cholesky
+@pytest.mark.parametrize("name,B,scale", [("c1", 12, 4), ("c3", 6, 8), ("c5", 5, 16)])
+def test_p20_gsce_route_equals_cholesky_route(name, B, scale):
+    """`loglike_batch_gsce` (Levinson + circulant embedding + numpy FFT: the CPU method the paper advocates, timed by bench.py
+    as a context line) against the primary oracle, on single-segment, gapped and multi-detector inputs.  A wrong conjugate,
+    a b-generator off by one or an embedding shorter than 2N - 1 fails here."""
+    w = W.make(name, B=B, n_scale=scale)
+    ref = O.loglike_batch(w.acf, w.seg_lengths, w.d, w.H)
+    got = O.loglike_batch_gsce(w.acf, w.seg_lengths, w.d, w.H)
+    assert np.max(np.abs(got - ref) / np.maximum(np.abs(ref), 1.0)) < 1e-9
+    fac = O.gsce_factors(w.acf, w.seg_lengths)
+    assert np.array_equal(O.loglike_batch_gsce(w.acf, w.seg_lengths, w.d, w.H, factors=fac), got)
