@@ -131,8 +131,10 @@ enum { TD_FAMILY_RINGDOWN = 0, TD_FAMILY_SINE_GAUSSIAN = 1, TD_FAMILY_CHIRP = 2 
  *           is such a row: amplitude A hypot(F+, Fx), phase phi - atan2(Fx, F+), onset t0 + dt; a segment that starts at
  *           time ts of a longer record takes t0 - ts (and phi + 2 pi f ts for the sine-Gaussian).
  *   fs      sampling rate in Hz (> 0);  d, out, stream as in td_loglike_batch.
- * The rows are synthesised into a scratch panel owned by the handle, chunk by chunk (about 128 MB),
- * and each chunk goes through the same kernels as td_loglike_batch.  Asynchronous on `stream`.
+ * The rows are synthesised into a scratch panel owned by the handle, chunk by chunk (about 128 MB; td_reserve sizes it),
+ * and each chunk goes through the same kernels as td_loglike_batch; small ringdown batches (up to 2 x the SM count, segments
+ * of 513..4096 samples) are synthesised inside the first pass of the fused kernel instead: one launch, no panel
+ * (profiles/r02_ring_fused.md has both routes measured).  Asynchronous on `stream`.
  * Errors: TD_EINVAL (unknown family, fs <= 0, null pointers), TD_ENOMEM, TD_ECUDA. */
 td_status td_loglike_family_batch(td_handle* h, const double* d, int family, const double* params, int64_t B, double fs,
                                   double* out, void* stream);

@@ -311,7 +311,10 @@ __device__ __forceinline__ void mbar_wait(uint32_t mbar, uint32_t parity) {
 // per-thread storage: 2 KB per lane, shared by the warps w and w + 4 of a CTA.  The fused kernels keep there what a
 // thread needs again for every template and never changes: its 32 values of the generator spectrum, its samples of the
 // data vector and its twiddle powers.  None of this touches shared memory or L2 after the first item.
-// NCOLS = 256 or 512 columns (a power of two >= 32); executed by ONE whole warp, which also frees them.  A CTA that asks for
+// Cost, measured in r02: a kernel that executes tcgen05.alloc gets ONE resident CTA per SM from the driver's occupancy accounting
+// (cudaOccupancyMaxActiveBlocksPerMultiprocessor returns 1 for a 30 KB / 120-register kernel once it contains the instruction),
+// so kernels that want two items per SM put two item pipelines into one CTA (td_fused4.cuh, NGRP).
+// NCOLS = 128, 256 or 512 columns (a power of two >= 32); executed by ONE whole warp, which also frees them.  A CTA that asks for
 // more columns than are free on its SM waits inside the instruction until a co-resident CTA frees its own.
 template <int NCOLS> __device__ __forceinline__ void tmem_alloc(uint32_t smem_slot) {
   asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_slot), "n"(NCOLS) : "memory");

@@ -1,5 +1,5 @@
 // td_fused4.cuh - the fused FFT-path kernel for M = 1024 / 2048 / 4096 (transform lengths
-// 2M = 2048 / 4096 / 8192), built around two measurements (profiles/r02_c2_phase_clocks.md): CTA-wide barriers put every
+// 2M = 2048 / 4096 / 8192), built around two measurements (profiles/r02_c2_fused4_ncu.md, profiles/r01_peaks.md): CTA-wide barriers put every
 // warp in the same load -> compute -> store phase, and whatever a thread needs again for every template costs
 // shared-memory bandwidth each time unless it lives somewhere else.
 //
