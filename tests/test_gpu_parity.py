@@ -960,3 +960,34 @@ def test_cdo_multi_segment_odd_offsets_and_limits():
         with pytest.raises(tdb.TDError) as e:
             h.set_path(tdb.TD_PATH_CDO)                      # 2048 > 1024
         assert e.value.status == tdb.TD_EUNSUPPORTED
+
+
+def test_fp32_and_parameter_calls_capture_into_a_cuda_graph():
+    """After td_set_precision / td_reserve the fp32 kernels and the parameter entry point (fused synthesis for a small
+    batch, panel route for a large one) are launches only as well: captured and replayed."""
+    w = W.make("c2", B=400, n_scale=2)
+    with tdb.TDLikelihood(w.acf, w.seg_lengths) as h:
+        h.set_precision(tdb.TD_PREC_F32)
+        h.reserve(400)
+        d, H, p = _dev(w.d), _dev(w.H), _dev(w.params)
+        p_small = p[:64].contiguous()
+        e_rows = h.loglike_batch(d, H).clone()
+        e_small = h.loglike_family_batch(d, w.family, p_small, w.fs).clone()
+        e_big = h.loglike_family_batch(d, w.family, p, w.fs).clone()
+        torch.cuda.synchronize()
+        o_rows = torch.empty_like(e_rows); o_small = torch.empty_like(e_small); o_big = torch.empty_like(e_big)
+        side = torch.cuda.Stream()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.stream(side):
+            with torch.cuda.graph(g, stream=side):
+                h.loglike_batch(d, H, out=o_rows, stream=side)
+                h.loglike_family_batch(d, w.family, p_small, w.fs, out=o_small, stream=side)
+                h.loglike_family_batch(d, w.family, p, w.fs, out=o_big, stream=side)
+        for _ in range(2):
+            o_rows.zero_(); o_small.zero_(); o_big.zero_()
+            g.replay()
+            torch.cuda.synchronize()
+            assert torch.equal(o_rows, e_rows) and torch.equal(o_small, e_small) and torch.equal(o_big, e_big)
+    ref = O.loglike_batch(w.acf, w.seg_lengths, w.d, w.H[:50])
+    _assert_close(e_rows.cpu().numpy()[:50], ref, tol=TOL32, what="fp32 rows")
+    _assert_close(e_big.cpu().numpy()[:50], ref, tol=TOL32, what="fp32 params")
