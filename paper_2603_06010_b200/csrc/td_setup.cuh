@@ -110,19 +110,12 @@ __global__ void __launch_bounds__(LEVC_NT) levinson_coop_kernel(const LevSeg sg,
   }
   for (int j = gtid; j < n; j += gsz) a[j] = (j == 0) ? 1.0 : 0.0;
   double E = rho0, logdet = log(rho0);
+  // ONE grid barrier per order: the thread that updates the pair (a_j, a_{k-j}) of order k holds both new values in
+  // registers and adds their terms of the NEXT order's dot product sum_j a_j rho_{k+1-j} on the spot, so the dot product needs
+  // no pass (and no barrier) of its own; per-CTA partial sums are double-buffered by the parity of the order.
+  if (tid == 0 && n > 1) partial[(size_t)1 * G + blockIdx.x] = blockIdx.x == 0 ? rho[1] : 0.0;
   grid.sync();
   for (int k = 1; k < n; ++k) {
-    double acc = 0.0;
-    for (int j = gtid; j < k; j += gsz) acc = fma(a[j], rho[k - j], acc);
-    acc = warp_sum(acc);
-    if ((tid & 31) == 0) red[tid >> 5] = acc;
-    __syncthreads();
-    if (tid < 32) {
-      double v = tid < LEVC_NT / 32 ? red[tid] : 0.0;
-      v = warp_sum(v);
-      if (tid == 0) partial[(size_t)(k & 1) * G + blockIdx.x] = v;
-    }
-    grid.sync();
     if (tid < 32) {  // fixed order: lane l adds partials l, l + 32, ...; then the warp tree
       double v = 0.0;
       for (int c = tid; c < G; c += 32) v += partial[(size_t)(k & 1) * G + c];
@@ -135,20 +128,37 @@ __global__ void __launch_bounds__(LEVC_NT) levinson_coop_kernel(const LevSeg sg,
       if (gtid == 0) *status = 2;
       return;
     }
+    const bool more = k + 1 < n;
+    double acc = 0.0;
     for (int j = 1 + gtid; 2 * j < k; j += gsz) {
       const double aj = a[j], ak = a[k - j];
-      a[j] = fma(kk, ak, aj);
-      a[k - j] = fma(kk, aj, ak);
+      const double nj = fma(kk, ak, aj), nk = fma(kk, aj, ak);
+      a[j] = nj;
+      a[k - j] = nk;
+      if (more) acc = fma(nj, rho[k + 1 - j], fma(nk, rho[j + 1], acc));
     }
     if (gtid == 0) {
-      if ((k & 1) == 0) { const double am = a[k / 2]; a[k / 2] = fma(kk, am, am); }
+      if ((k & 1) == 0) {
+        const double am = a[k / 2], nm = fma(kk, am, am);
+        a[k / 2] = nm;
+        if (more) acc = fma(nm, rho[k + 1 - k / 2], acc);
+      }
       a[k] = kk;
+      if (more) acc += fma(kk, rho[1], rho[k + 1]);   // a_k rho_1 + a_0 rho_{k+1}
     }
     E *= (1.0 - kk * kk);
     logdet += log(E);
     if (!(E > 0.0)) {
       if (gtid == 0) *status = 2;
       return;
+    }
+    acc = warp_sum(acc);
+    if ((tid & 31) == 0) red[tid >> 5] = acc;
+    __syncthreads();
+    if (tid < 32) {
+      double v = tid < LEVC_NT / 32 ? red[tid] : 0.0;
+      v = warp_sum(v);
+      if (tid == 0) partial[(size_t)((k + 1) & 1) * G + blockIdx.x] = v;
     }
     grid.sync();
   }

@@ -862,8 +862,6 @@ template <int MODE> td_status warm_mode(td_handle* h) {
   return TD_OK;
 }
 td_status warm_kernels(td_handle* h) {
-  for (const ClassInfo& c : h->classes)
-    if (c.log2M == Cluster16Shape::LOG2M) h->cluster16_cap = cluster16_capacity(h);
   if (ring_fused_ok(h)) {
     td_status r = run_ring_fused(h, nullptr, nullptr, 1, 1.0, nullptr, nullptr, true);
     if (r != TD_OK) return r;
@@ -1319,7 +1317,11 @@ td_status td_set_fft_variant(td_handle* h, int variant) {
   if (variant == 3) {   // the 16-CTA cluster kernel needs a 65536-class segment and a device that can host the cluster
     bool has16 = false;
     for (const ClassInfo& c : h->classes) has16 = has16 || c.log2M == Cluster16Shape::LOG2M;
-    if (!has16 || h->cluster16_cap < 1) return TD_EUNSUPPORTED;
+    if (!has16) return TD_EUNSUPPORTED;
+    DevGuard guard(h->device);
+    if (!guard.ok) return TD_ECUDA;
+    if (h->cluster16_cap < 1) h->cluster16_cap = cluster16_capacity(h);   // configures the kernels, asks how many clusters fit
+    if (h->cluster16_cap < 1) return TD_EUNSUPPORTED;
   }
   if (variant == 2) {
     DevGuard guard(h->device);
