@@ -188,8 +188,9 @@ td_status td_set_precision(td_handle* h, int precision);
  *   n_seg      number of segments
  *   v          HOST array [n_seg]: prediction-error variance v_s = 1/(C_s^{-1})_{00}
  *   logdet     HOST array [n_seg]: log det C_s = sum_k log E_k
- *   last_path  path actually used by the last batch call (0 if none yet): TD_PATH_DENSE if every
- *              segment went through the dense kernel, TD_PATH_DOT for the dot-product cross term, TD_PATH_FFT otherwise
+ *   last_path  path actually used by the last batch call (0 if none yet): TD_PATH_CDO / TD_PATH_DENSE if every segment went
+ *              through the dense kernels (CDO if the cached-L^-1 contraction took part), TD_PATH_DOT for the dot-product
+ *              cross term, TD_PATH_FFT otherwise
  */
 td_status td_get_info(const td_handle* h, int64_t* n_tot, int* n_seg, double* v, double* logdet,
                       int* last_path);
