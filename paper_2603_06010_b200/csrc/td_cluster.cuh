@@ -71,6 +71,7 @@ __device__ __forceinline__ uint32_t cluster_ctarank() {
   return r;
 }
 __device__ __forceinline__ void cluster_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
+__device__ __forceinline__ void cluster_arrive_relaxed() { asm volatile("barrier.cluster.arrive.relaxed.aligned;" ::: "memory"); }
 __device__ __forceinline__ void cluster_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
 __device__ __forceinline__ uint32_t map_to_cta(uint32_t smem_addr, uint32_t rank) {
   uint32_t r;
@@ -226,6 +227,7 @@ __global__ void __launch_bounds__(ClusterShape::NT, 1) td_cluster_kernel(const F
     for (int wq = 0; wq < NW; ++wq) { p0 += r[2 * wq]; p1 += r[2 * wq + 1]; }
     if (br) {
       asm volatile("st.shared::cluster.v2.f64 [%0], {%1, %2};" ::"r"(xsum_remote), "d"(p0), "d"(p1) : "memory");
+      asm volatile("fence.acq_rel.cluster;" ::: "memory");   // releases the sums ahead of this thread's relaxed arrive (A)
     } else {
       bk->pend0 = p0; bk->pend1 = p1; bk->pend_b = bk->prev_b; bk->pend_add = bk->prev_add;
     }
@@ -351,7 +353,6 @@ __global__ void __launch_bounds__(ClusterShape::NT, 1) td_cluster_kernel(const F
         for (int q = 0; q < 32; ++q) x[q] = Z.ld(j + 256 * q);
         // arm the exchange mbarrier for this item's 16 x 256 complex from the partner, then
         if (tid == 0) mbar_expect_tx(mbar_x, (uint32_t)(16 * NT * sizeof(cplx)));
-        cluster_arrive();  // (A) every thread of this CTA has read its Z values: the region may be overwritten
         {
           // x_q *= conj(w_M^{j q}) (and conj(w_2M^j) on the odd branch); powers as w^{4 hi} * w^{lo}
           cplx lo[4], hi[8];
@@ -370,12 +371,18 @@ __global__ void __launch_bounds__(ClusterShape::NT, 1) td_cluster_kernel(const F
           static_for<0, 32>([&](auto q) {
             constexpr int qq = decltype(q)::value;
             if constexpr (qq < 4) {
-              if (qq > 0 || br) x[qq] = cmulc(x[qq], lo[qq]);
+              x[qq] = cmulc(x[qq], lo[qq]);   // (also q = 0 on the even branch, a product with 1: every loaded value is consumed here)
             } else {
               x[qq] = cmulc(x[qq], cmul(hi[qq >> 2], lo[qq & 3]));
             }
           });
         }
+        // (A) "this CTA has read its Z values: the region may be overwritten".  Placed after the twiddle products: every value
+        // read from Z has been consumed by an instruction issued before the arrive (in-order issue), so a RELAXED arrive is enough
+        // for this write-after-read hazard; the one datum that crosses with the barrier, rank 1's partial sums, is released by a
+        // fence of the thread that stored it (cta_sums).  r02: barrier.cluster.arrive.release made every warp execute a
+        // cluster-scope membar per item - 4.3 % of the warp samples, 13 % of the kernel time (c5 1.95 -> 2.20 M evals/s).
+        cluster_arrive_relaxed();
         fft_reg<32, true>(x);
         if (br) static_for<1, 32>([&](auto t) {
           constexpr int tt = decltype(t)::value;

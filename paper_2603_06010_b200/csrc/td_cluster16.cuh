@@ -397,8 +397,15 @@ __global__ void __launch_bounds__(Cluster16Shape::NT, 1) td_cluster16_kernel(con
         mbar_expect_tx(mbar_z, (uint32_t)(2 * ML * sizeof(cplx)));
         if (b + ncl < Bs) mbar_expect_tx(mbar_u, (uint32_t)(2 * NFL * sizeof(cplx)));
       }
-      // (A) every CTA of the cluster has read its Z into registers and is past mid: all Z and U regions are free
-      cluster_arrive();
+      // (A) every CTA of the cluster has read its Z into registers and is past mid: all Z and U regions are free.  A relaxed
+      // arrive suffices for this write-after-read hazard once the loads have returned: a register move per value makes the
+      // warp wait for them (the release form costs a cluster-scope membar in every warp, td_cluster.cuh)
+#pragma unroll
+      for (int c = 0; c < 16; ++c) {
+        asm volatile("mov.b64 %0, %0;" : "+d"(xa[c].x));
+        asm volatile("mov.b64 %0, %0;" : "+d"(xb[c].x));
+      }
+      cluster_arrive_relaxed();
       cluster_wait();
       const int ia = (16 * brG + tsubA) * 256 + tid, ib = (16 * brG + tsubB) * 256 + tid;
       const uint32_t offa = (uint32_t)((ia + (ia >> 4)) * sizeof(cplx)), offb = (uint32_t)((ib + (ib >> 4)) * sizeof(cplx));
