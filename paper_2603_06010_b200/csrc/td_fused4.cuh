@@ -322,9 +322,16 @@ __global__ void __launch_bounds__(Fused4Shape<LOG2M>::NT * NGRP, 1) td_fused4_ke
   const SmemArr U = br ? UO : UE, Z = br ? ZO : ZE;
   const F4Own own = f4_own<RF1, true>(br, wb);
 
-  for (int k = tid; k < Sh::TWS; k += NT) tw[k] = P.T[k];
+  // the base-twiddle table arrives by one bulk copy (it was NT-strided global loads: the longest piece of the prologue, which is
+  // most of a launch when a CTA has a single item, as on c1)
+  const uint32_t mbar_tw = mbar_rows + 16;
   if (tid < P.n_seg && tid < F4_SEGCACHE) segS[tid] = P.segs[tid];
-  if (tid == 0) mbar_init(mbar_rows, 1);
+  if (tid == 0) {
+    mbar_init(mbar_rows, 1);
+    mbar_init(mbar_tw, 1);
+    mbar_expect_tx(mbar_tw, (uint32_t)(Sh::TWS * sizeof(cplx)));
+    bulk_g2s(smem_u32(tw), P.T, (uint32_t)(Sh::TWS * sizeof(cplx)), mbar_tw);
+  }
   if (cwarp == 0) tmem_alloc<TMEM_COLS>(smem_u32(tmem_slot));
 #ifdef TD_PHASE_CLOCKS
   long long* clk_s = reinterpret_cast<long long*>(reinterpret_cast<unsigned char*>(segS + F4_SEGCACHE) + 96);
@@ -336,6 +343,7 @@ __global__ void __launch_bounds__(Fused4Shape<LOG2M>::NT * NGRP, 1) td_fused4_ke
   tmem_fence_after();
   // this thread's TMEM window: lane 32 (warp % 4) + lane, Cols::WINDOW columns
   const uint32_t tcol = *tmem_slot + ((uint32_t)(32 * (cwarp & 3)) << 16) + (uint32_t)((cwarp >> 2) * Sh::Cols::WINDOW);
+  mbar_wait(mbar_tw, 0);
   f4_store_twiddles<TW>(lane, tw, tcol + Sh::Cols::TW);
 
   // rows of item (b, s); the template row is staged by TMA when it is 16-byte aligned and N_s is even
