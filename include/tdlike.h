@@ -175,8 +175,8 @@ enum { TD_PREC_F64 = 0, TD_PREC_F32 = 1 };
  * fp64 (td_create) and are rounded once; per template the residual d - h is formed in fp64 from the fp64 inputs, divided
  * by sqrt(rho_s(0)) (the normalisation; the spectra carry the inverse factor) and rounded once; S2-S4 (both FFTs, the
  * generator product) run in fp32; the sums of squares are fp32 per thread and fp64 across threads, segments and in out[].
- * The interface (double d, H, out) is unchanged.  Serves segments of 513..8192 samples (the fused and cluster kernels);
- * other size classes of the handle, the dense path and the dot-product cross term keep evaluating in fp64.
+ * The interface (double d, H, out) is unchanged.  Serves segments of 513 samples and more (fp32 builds of the fused, cluster
+ * and staged kernels); shorter segments (the dense paths) and the dot-product cross term keep evaluating in fp64.
  * Accuracy: |out - exact| <= 2e-5 * max(|exact|, 1) per template (DESIGN.md 6.7 derives it; observed ~1e-6); the fp64
  * default keeps the 1e-9 bar.  The first call builds the fp32 tables (synchronous, allocates); later calls only switch.
  * Errors: TD_EINVAL (unknown precision), TD_EUNSUPPORTED (no segment of the handle has an fp32 kernel; the setting is

@@ -11,14 +11,17 @@
 
 namespace td32api {
 
-// size classes the fp32 kernels serve: M = 1024 .. 8192 (segments of 513 .. 8192 samples)
-inline bool supported(int log2M) { return log2M >= 10 && log2M <= 13; }
+// size classes the fp32 kernels serve: M = 1024 .. 8192 on the fused / cluster kernels (segments of 513 .. 8192 samples), M >= 16384
+// on the staged kernels (td_staged.cuh compiled with real = float: half the L2 traffic of a path that is bound by it)
+inline bool supported(int log2M) { return log2M >= 10 && log2M <= 26; }
+inline bool staged_class(int log2M) { return log2M >= 14; }
 
 struct SegIn {
   long long off;      // offset of the segment inside d / a row of H (elements)
   int n;              // N_s
   int sid;            // index of the segment in the handle
-  const void* Gp64;   // device double2 [2][padded(M)]: the fp64 generator spectrum in the padded Z layout
+  const void* Gp64;   // device double2 [2][padded(M)]: the fp64 generator spectrum in the padded Z layout (fused / cluster classes)
+  const void* G64;    // device double2 [2][M]: the same spectrum in the plain layout (staged classes)
   double rho0;        // rho_s(0): samples are scaled by rho0^(-1/2) before rounding, the spectrum by rho0^(+1/2)
 };
 
@@ -30,6 +33,17 @@ struct ClassTables {
   void* Gp_ptrs = nullptr;  // const float2* [n_seg]
   void** Gp = nullptr;      // host array [n_seg] of device float2 [2][padded(M)]
   void** zd = nullptr;      // host array [n_seg] of device float2 [M]
+  void* host_segs = nullptr;  // staged classes: host copy of the td32::SegDev records
+};
+
+// what a staged run borrows from the handle (td_staged_host.cuh: StagedCtx)
+struct StagedBorrow {
+  void* wsU = nullptr; size_t wsU_bytes = 0;
+  void* wsZ = nullptr; size_t wsZ_bytes = 0;
+  double* wsPartial = nullptr; size_t wsP_elems = 0;
+  cudaStream_t aux_stream = nullptr;
+  cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+  int* launches = nullptr;
 };
 
 // builds the fp32 tables of a class from the fp64 ones (T64: device double2 [2M]); synchronous
@@ -44,6 +58,7 @@ struct Launch {
   double* out1;
   int accumulate;
   int mode;  // td::MODE_LOGLIKE / MODE_INNER / MODE_STOREZ
+  const StagedBorrow* staged = nullptr;   // staged classes only
   int syn = 0;      // 1: H holds ringdown parameter rows (ldh = 5 x segments of the handle), fused4 classes, MODE_LOGLIKE only
   double fs = 0.0;  // sampling rate (syn only)
 };

@@ -6,7 +6,7 @@
 #pragma once
 #include "td_fused.cuh"
 
-namespace td {
+namespace TD_NS {
 
 constexpr int LG_NT = 128;
 
@@ -35,7 +35,7 @@ __global__ void __launch_bounds__(LG_NT) lg_first_kernel(const StagedParams P) {
   const double* hrow = (MODE == MODE_STOREZ) ? drow : P.H + (long long)c * P.ldh + P.seg.off;
   const bool vec = ((reinterpret_cast<uintptr_t>(drow) | reinterpret_cast<uintptr_t>(hrow)) & 15) == 0;
   const GmemArr UE{P.U + ((size_t)c * 2 + 0) * nf}, UO{P.U + ((size_t)c * 2 + 1) * nf};
-  first_pass_task<R, MODE>(UE, UO, nf, g, drow, hrow, P.seg.n, vec, P.T);
+  first_pass_task<R, MODE>(UE, UO, nf, g, drow, hrow, P.seg.n, vec, P.T, P.seg.rscale);
 }
 
 // generic pass over `narr` independent arrays of length n laid out back to back
@@ -69,7 +69,7 @@ __device__ __forceinline__ void block_inverse3(const SmemArr& A, int tid, const 
 #pragma unroll
     for (int q = 0; q < 16; ++q) x[q] = A.ld(b0 + q * S);
     if constexpr (S > 1) dit16<true, true>(x, cconj(T[(size_t)j * (TW / L)]));
-    else dit16<true, false>(x, mk(1.0, 0.0));
+    else dit16<true, false>(x, mk(real(1), real(0)));
     static_for<0, 16>([&](auto t) { A.st(b0 + decltype(t)::value * S, x[brevR<16>(decltype(t)::value)]); });
     __syncthreads();
   });
@@ -179,4 +179,4 @@ __global__ void lg_finish_kernel(const double* __restrict__ partial, int nblk, i
   if (out1) out1[c] = (accumulate ? out1[c] : 0.0) + scale1 * t1;
 }
 
-}  // namespace td
+}  // namespace TD_NS

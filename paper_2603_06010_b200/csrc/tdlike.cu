@@ -21,7 +21,7 @@
 #include "td_cluster16.cuh"
 #include "td_fused4.cuh"
 #include "td_setup.cuh"
-#include "td_staged.cuh"
+#include "td_staged_host.cuh"
 #include "td_synth.cuh"
 
 using namespace td;
@@ -36,7 +36,6 @@ constexpr int FUSED_NT = 256;
 constexpr int DENSE_AUTO_N = 512;     // AUTO: dense paths for segments up to this length (measured crossover: profiles/r01_chooser.md)
 constexpr int CDO_AUTO_MIN_N = 65;    // AUTO, log-likelihood: cached-L^-1 contraction from this length up, the Gohberg-Semencul
                                       // dense kernel below (measured: profiles/r02_cdo.md; 0.95x at N = 64, 1.08-1.55x above)
-constexpr size_t STAGED_WS_BYTES = 96ull << 20;  // staged workspace, both lanes: inside the 126 MB L2 (measured 64: 0.91 ms, 96: 0.756, 128: 0.761, 192: 0.745, 384: 0.750 on c4)
 
 struct SegHost {
   int64_t off = 0;
@@ -141,102 +140,6 @@ void free_handle(td_handle* h) {
   delete h;
 }
 
-template <bool FWD>
-td_status launch_pass(int R, cplx* base, int narr, int n, int L, const cplx* T, int TW, cudaStream_t st) {
-  dim3 grid((n / R + LG_NT - 1) / LG_NT, narr);
-  switch (R) {
-    case 2: lg_pass_kernel<2, FWD><<<grid, LG_NT, 0, st>>>(base, n, L, T, TW); break;
-    case 4: lg_pass_kernel<4, FWD><<<grid, LG_NT, 0, st>>>(base, n, L, T, TW); break;
-    case 8: lg_pass_kernel<8, FWD><<<grid, LG_NT, 0, st>>>(base, n, L, T, TW); break;
-    case 16: lg_pass_kernel<16, FWD><<<grid, LG_NT, 0, st>>>(base, n, L, T, TW); break;
-    default: return TD_EINVAL;
-  }
-  CK(cudaGetLastError());
-  return TD_OK;
-}
-
-template <bool FWD>
-td_status launch_block(int device, cplx* base, int narr, int n, const cplx* T, int TW, cudaStream_t st, bool dry = false) {
-  auto kern = lg_block_kernel<FWD>;
-  static int cache[TD_MAX_DEV];
-  int nb = 0;
-  td_status cs = kernel_config(kern, LGB_NT, LGB_SMEM, LGB_SMEM, device, cache, &nb);
-  if (cs != TD_OK || dry) return cs;
-  kern<<<dim3(n / LGB_N, narr), LGB_NT, LGB_SMEM, st>>>(base, n, T, TW);
-  CK(cudaGetLastError());
-  return TD_OK;
-}
-
-// forward DIF of `narr` arrays of length n with plan [r1,16,16,...]; the last three passes
-// (L = 4096, 256, 16) run as one shared-memory block kernel when the plan has them
-td_status staged_forward(int device, cplx* base, int narr, int n, int first_pass_done, const cplx* T, int TW,
-                         cudaStream_t st, int* launches) {
-  int L = n;
-  const int r1 = plan_r1(n), np = plan_np(n);
-  for (int q = 0; q < np; ++q) {
-    const int R = q == 0 ? r1 : 16;
-    if (q >= 1 && q == np - 3 && L == LGB_N) {
-      td_status s = launch_block<true>(device, base, narr, n, T, TW, st);
-      if (s != TD_OK) return s;
-      ++*launches;
-      break;
-    }
-    if (!(q == 0 && first_pass_done)) {
-      td_status s = launch_pass<true>(R, base, narr, n, L, T, TW, st);
-      if (s != TD_OK) return s;
-      ++*launches;
-    }
-    L /= R;
-  }
-  return TD_OK;
-}
-
-// inverse DIT passes except the last (radix r1, L = n) one; the first three (L = 16, 256, 4096)
-// as one shared-memory block kernel when the plan has them
-td_status staged_inverse_but_last(int device, cplx* base, int narr, int n, const cplx* T, int TW, cudaStream_t st,
-                                  int* launches) {
-  const int np = plan_np(n);
-  int L = 16, q = 1;
-  if (np - 1 >= 3) {
-    td_status s = launch_block<false>(device, base, narr, n, T, TW, st);
-    if (s != TD_OK) return s;
-    ++*launches;
-    L <<= 12; q = 4;
-  }
-  for (; q < np; ++q) {
-    td_status s = launch_pass<false>(16, base, narr, n, L, T, TW, st);
-    if (s != TD_OK) return s;
-    ++*launches;
-    L <<= 4;
-  }
-  return TD_OK;
-}
-
-template <int MODE>
-td_status launch_first(int R, dim3 grid, const StagedParams& P, cudaStream_t st) {
-  switch (R) {
-    case 2: lg_first_kernel<2, MODE><<<grid, LG_NT, 0, st>>>(P); break;
-    case 4: lg_first_kernel<4, MODE><<<grid, LG_NT, 0, st>>>(P); break;
-    case 8: lg_first_kernel<8, MODE><<<grid, LG_NT, 0, st>>>(P); break;
-    case 16: lg_first_kernel<16, MODE><<<grid, LG_NT, 0, st>>>(P); break;
-    default: return TD_EINVAL;
-  }
-  CK(cudaGetLastError());
-  return TD_OK;
-}
-template <int MODE>
-td_status launch_last(int R, dim3 grid, const StagedParams& P, cudaStream_t st) {
-  switch (R) {
-    case 2: lg_last_kernel<2, MODE><<<grid, LG_NT, 0, st>>>(P); break;
-    case 4: lg_last_kernel<4, MODE><<<grid, LG_NT, 0, st>>>(P); break;
-    case 8: lg_last_kernel<8, MODE><<<grid, LG_NT, 0, st>>>(P); break;
-    case 16: lg_last_kernel<16, MODE><<<grid, LG_NT, 0, st>>>(P); break;
-    default: return TD_EINVAL;
-  }
-  CK(cudaGetLastError());
-  return TD_OK;
-}
-
 // grow-only device buffer (td_create / td_reserve; a batch call reaches the cudaMalloc only when the caller did not reserve)
 template <class T> td_status grow(T*& p, size_t& have, size_t want) {
   if (want <= have) return TD_OK;
@@ -246,19 +149,6 @@ template <class T> td_status grow(T*& p, size_t& have, size_t want) {
   return TD_OK;
 }
 
-// staged path geometry of one size class: templates per lane chunk, workspace shares
-struct StagedGeom { int64_t CB; size_t uh, zh; int nblk, rI, rF; };
-StagedGeom staged_geom(int log2M) {
-  const int M = 1 << log2M, nf = M / 2;
-  const size_t per_tmpl = (size_t)(2 * nf + 2 * M) * sizeof(cplx);
-  StagedGeom g;
-  g.CB = std::max<int64_t>(1, (int64_t)(STAGED_WS_BYTES / 2 / per_tmpl));
-  g.CB = std::min<int64_t>(g.CB, 32767);  // grid.y = 2*CB arrays per pass
-  g.rI = plan_r1(M); g.rF = plan_r1(nf);
-  g.nblk = (M / g.rI + LG_NT - 1) / LG_NT;
-  g.uh = (size_t)g.CB * 2 * nf; g.zh = (size_t)g.CB * 2 * M;
-  return g;
-}
 constexpr size_t STAGED_PARTIAL_DEFAULT = 16ull << 20, STAGED_PARTIAL_MAX = 1ull << 30;  // bytes of per-block partial sums
 
 // cross-stream ordering of the calls that use handle-owned scratch (staged workspace, z / u of the data vector, the
@@ -282,82 +172,26 @@ td_status order_end(td_handle* h, cudaStream_t st) {
   return TD_OK;
 }
 
-// One segment of a size class through the staged pipeline for templates [0, B).
-template <int MODE>
-td_status run_staged_sub(td_handle* h, const ClassInfo& cls, const SegHost& sg, const double* d, const double* H,
-                         int64_t ldh, int64_t B, double* out0, double* out1, double scale0, double scale1,
-                         int accumulate, cudaStream_t st) {
-  const int M = 1 << cls.log2M, nf = M / 2, TW = 2 * M;
-  // Two lanes: chunks alternate between the caller's stream and an internal one, each lane with its own half of the
-  // L2-resident workspace.  No kernel of the pipeline fills the GPU on its own (a few hundred CTAs, each bound by L2
-  // latency at the start and end of its life), so two chunks in flight overlap one another's ramps and tails.
-  const StagedGeom g = staged_geom(cls.log2M);
-  const int64_t CB = std::min<int64_t>(g.CB, std::max<int64_t>(B, 1));
-  const bool two = B > CB;
-  const int rI = g.rI, rF = g.rF, nblk = g.nblk;
-  const size_t uh = g.uh, zh = g.zh;  // one lane's share
-  if (h->wsU_elems < 2 * uh || h->wsZ_elems < 2 * zh) return TD_EUNSUPPORTED;  // (never: td_create sized them)
-  h->touched = true;
-  if (two) {
-    CK(cudaEventRecord(h->ev_fork, st));          // everything enqueued on the caller's stream so far comes first
-    CK(cudaStreamWaitEvent(h->aux_stream, h->ev_fork, 0));
-  }
-  int lane = 0;
-  td_status s = TD_OK;
-  for (int64_t b0 = 0; b0 < B && s == TD_OK; b0 += CB, lane ^= 1) {
-    const int cb = (int)std::min<int64_t>(CB, B - b0);
-    cudaStream_t ls = (two && lane) ? h->aux_stream : st;
-    cplx* U = h->wsU + (two && lane ? uh : 0);
-    cplx* Z = h->wsZ + (two && lane ? zh : 0);
-    StagedParams P;
-    P.d = d; P.H = H ? H + b0 * ldh : nullptr; P.ldh = ldh; P.CB = cb;
-    P.seg.off = sg.off; P.seg.n = sg.n; P.seg._pad = 0; P.seg.G = sg.G; P.seg.zd = sg.zd; P.seg.rscale = 1.0;
-    P.M = M; P.U = U; P.Z = Z; P.T = cls.T; P.partial = h->wsPartial + (size_t)b0 * nblk * 2; P.nblk = nblk;
-    s = launch_first<MODE>(rF, dim3((nf / rF + LG_NT - 1) / LG_NT, cb), P, ls);
-    if (s != TD_OK) break;
-    ++h->last_launches;
-    s = staged_forward(h->device, U, 2 * cb, nf, 1, cls.T, TW, ls, &h->last_launches);
-    if (s != TD_OK) break;
-    // (fusing the untangle into the inverse block kernel - one CTA building a block, or a mirror pair of blocks, of Z in
-    // shared memory straight from U and G - was measured: 50-68 us per chunk against 18 + 24 us for the two kernels; the
-    // gather serialises 16 index-heavy tasks per thread, which the stand-alone kernel hides behind 1.4 M threads)
-    lg_untangle_kernel<<<dim3((nf + LG_NT - 1) / LG_NT, 2, (cb + LG_UCPT - 1) / LG_UCPT), LG_NT, 0, ls>>>(P);
-    if (cudaGetLastError() != cudaSuccess) { s = TD_ECUDA; break; }
-    ++h->last_launches;
-    s = staged_inverse_but_last(h->device, Z, 2 * cb, M, cls.T, TW, ls, &h->last_launches);
-    if (s != TD_OK) break;
-    s = launch_last<MODE>(rI, dim3(nblk, cb), P, ls);
-    if (s != TD_OK) break;
-    ++h->last_launches;
-  }
-  if (two) {  // the aux lane is joined on every path, also after an error
-    const bool j = cudaEventRecord(h->ev_join, h->aux_stream) == cudaSuccess && cudaStreamWaitEvent(st, h->ev_join, 0) == cudaSuccess;
-    if (!j && s == TD_OK) s = TD_ECUDA;
-  }
-  if (s != TD_OK) return s;
-  if (MODE != MODE_STOREZ && B > 0) {  // one reduction of the per-block partial sums for the whole sub-batch (fixed order)
-    lg_finish_kernel<<<(unsigned)((B + 127) / 128), 128, 0, st>>>(h->wsPartial, nblk, (int)B, out0, out1, scale0, scale1, accumulate);
-    CK(cudaGetLastError());
-    ++h->last_launches;
-  }
-  return TD_OK;
+// the staged kernels' driver (td_staged_host.cuh) borrows workspace, second stream and events from the handle
+StagedCtx staged_ctx(td_handle* h) {
+  StagedCtx C;
+  C.device = h->device;
+  C.wsU = h->wsU; C.wsU_bytes = h->wsU_elems * sizeof(cplx);
+  C.wsZ = h->wsZ; C.wsZ_bytes = h->wsZ_elems * sizeof(cplx);
+  C.wsPartial = h->wsPartial; C.wsP_elems = h->wsP_elems;
+  C.aux_stream = h->aux_stream; C.ev_fork = h->ev_fork; C.ev_join = h->ev_join;
+  C.launches = &h->last_launches;
+  return C;
 }
-
-// sub-batches of as many templates as the partial-sum buffer holds (td_reserve sizes it for the caller's largest batch)
 template <int MODE>
 td_status run_staged(td_handle* h, const ClassInfo& cls, const SegHost& sg, const double* d, const double* H,
                      int64_t ldh, int64_t B, double* out0, double* out1, double scale0, double scale1,
                      int accumulate, cudaStream_t st) {
-  const StagedGeom g = staged_geom(cls.log2M);
-  const int64_t SB = std::min<int64_t>(std::max<int64_t>(1, (int64_t)(h->wsP_elems / ((size_t)g.nblk * 2))), 1 << 30);
-  if (h->wsP_elems < (size_t)g.nblk * 2) return TD_EUNSUPPORTED;  // (never: td_create holds at least one template)
-  for (int64_t b0 = 0; b0 < std::max<int64_t>(B, 1); b0 += SB) {
-    const int64_t nb = std::min<int64_t>(SB, B - b0);
-    td_status s = run_staged_sub<MODE>(h, cls, sg, d, H ? H + b0 * ldh : nullptr, ldh, nb, out0 ? out0 + b0 : nullptr,
-                                       out1 ? out1 + b0 : nullptr, scale0, scale1, accumulate, st);
-    if (s != TD_OK) return s;
-  }
-  return TD_OK;
+  StagedCtx C = staged_ctx(h);
+  SegDev sd;
+  sd.off = sg.off; sd.n = sg.n; sd._pad = 0; sd.G = sg.G; sd.zd = sg.zd; sd.rscale = 1.0;
+  h->touched = true;
+  return td::run_staged<MODE>(C, cls.log2M, cls.T, sd, d, H, ldh, B, out0, out1, scale0, scale1, accumulate, st);
 }
 
 template <int LOG2M, int MODE, int FUSED_NT, bool ILV = true>
@@ -730,12 +564,21 @@ td_status run_fft_path(td_handle* h, const double* d, const double* H, int64_t l
   const double sc0 = (MODE == MODE_LOGLIKE) ? -0.5 : 1.0, sc1 = 1.0;
   for (const ClassInfo& cls : h->classes) {
     if (skip_dense_classes && class_is_dense(h, cls)) continue;
-    if (f32 && cls.has32 && class_is_fused(h, cls) && !class_is_dense(h, cls)) {
+    const bool st32 = td32api::staged_class(cls.log2M);   // (a fused-shape class forced onto the staged kernels stays fp64)
+    if (f32 && cls.has32 && !class_is_dense(h, cls) && (st32 || class_is_fused(h, cls)) && h->fft_variant != 3) {
       td32api::Launch L;
       L.d = d; L.H = H; L.ldh = ldh; L.B = B; L.out0 = out0; L.out1 = out1; L.accumulate = accumulate; L.mode = MODE;
+      td32api::StagedBorrow sb;
+      if (st32) {
+        sb.wsU = h->wsU; sb.wsU_bytes = h->wsU_elems * sizeof(cplx); sb.wsZ = h->wsZ; sb.wsZ_bytes = h->wsZ_elems * sizeof(cplx);
+        sb.wsPartial = h->wsPartial; sb.wsP_elems = h->wsP_elems;
+        sb.aux_stream = h->aux_stream; sb.ev_fork = h->ev_fork; sb.ev_join = h->ev_join; sb.launches = &h->last_launches;
+        L.staged = &sb;
+        h->touched = true;
+      }
       td_status s = td32api::launch(cls.t32, L, h->num_sms, h->device, st, false);
       if (s != TD_OK) return s;
-      ++h->last_launches;
+      if (!st32) ++h->last_launches;
       accumulate = 1;
       continue;
     }
@@ -1346,7 +1189,7 @@ td_status td_set_precision(td_handle* h, int precision) {
       std::vector<td32api::SegIn> in(c.seg_ids.size());
       for (size_t i = 0; i < in.size(); ++i) {
         const SegHost& sg = h->segs[c.seg_ids[i]];
-        in[i].off = sg.off; in[i].n = sg.n; in[i].sid = c.seg_ids[i]; in[i].Gp64 = sg.Gp; in[i].rho0 = sg.rho0;
+        in[i].off = sg.off; in[i].n = sg.n; in[i].sid = c.seg_ids[i]; in[i].Gp64 = sg.Gp; in[i].G64 = sg.G; in[i].rho0 = sg.rho0;
       }
       td_status s = td32api::build_class(c.log2M, (int)in.size(), in.data(), c.T, &c.t32);
       if (s != TD_OK) return s;

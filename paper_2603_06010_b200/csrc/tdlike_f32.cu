@@ -10,10 +10,12 @@
 #include "td_host.h"
 
 #include <algorithm>
+#include <new>
 #include <vector>
 
 #include "td_cluster.cuh"
 #include "td_fused4.cuh"
+#include "td_staged_host.cuh"
 
 using namespace td32;
 using namespace tdhost;
@@ -102,6 +104,7 @@ void free_class(ClassTables* t) {
     if (t->zd) cudaFree(t->zd[s]);
   }
   delete[] t->Gp; delete[] t->zd;
+  delete[] static_cast<SegDev*>(t->host_segs);
   *t = ClassTables();
 }
 
@@ -112,7 +115,8 @@ td_status build_class(int log2M, int n_seg, const SegIn* segs, const void* T64, 
   t.Gp = new (std::nothrow) void*[n_seg]();
   t.zd = new (std::nothrow) void*[n_seg]();
   if (!t.Gp || !t.zd) { free_class(&t); return TD_ENOMEM; }
-  const size_t M = (size_t)1 << log2M, TW = 2 * M, gp_elems = 2 * (size_t)SmemArr::padded((int)M);
+  const bool staged = staged_class(log2M);
+  const size_t M = (size_t)1 << log2M, TW = 2 * M, gp_elems = staged ? 2 * M : 2 * (size_t)SmemArr::padded((int)M);
   auto fail = [&](td_status s) { free_class(&t); return s; };
   if (cudaMalloc(&t.T, sizeof(float2) * TW) != cudaSuccess) return fail(TD_ENOMEM);
   cvt_cplx_kernel<<<(unsigned)((TW + 255) / 256), 256>>>(static_cast<const double2*>(T64), static_cast<float2*>(t.T), TW, 1.0);
@@ -122,9 +126,11 @@ td_status build_class(int log2M, int n_seg, const SegIn* segs, const void* T64, 
     if (!(segs[s].rho0 > 0.0)) return fail(TD_ENOTSPD);
     if (cudaMalloc(&t.Gp[s], sizeof(float2) * gp_elems) != cudaSuccess) return fail(TD_ENOMEM);
     if (cudaMalloc(&t.zd[s], sizeof(float2) * M) != cudaSuccess) return fail(TD_ENOMEM);
-    cvt_cplx_kernel<<<(unsigned)((gp_elems + 255) / 256), 256>>>(static_cast<const double2*>(segs[s].Gp64),
-                                                                 static_cast<float2*>(t.Gp[s]), gp_elems, sqrt(segs[s].rho0));
-    sd[s].off = segs[s].off; sd[s].n = segs[s].n; sd[s]._pad = segs[s].sid; sd[s].G = nullptr;
+    const void* src = staged ? segs[s].G64 : segs[s].Gp64;
+    if (!src) return fail(TD_EINVAL);
+    cvt_cplx_kernel<<<(unsigned)((gp_elems + 255) / 256), 256>>>(static_cast<const double2*>(src), static_cast<float2*>(t.Gp[s]),
+                                                                 gp_elems, sqrt(segs[s].rho0));
+    sd[s].off = segs[s].off; sd[s].n = segs[s].n; sd[s]._pad = segs[s].sid; sd[s].G = staged ? static_cast<const cplx*>(t.Gp[s]) : nullptr;
     sd[s].zd = static_cast<cplx*>(t.zd[s]); sd[s].rscale = 1.0 / sqrt(segs[s].rho0);
     gp[s] = static_cast<const cplx*>(t.Gp[s]);
   }
@@ -135,6 +141,17 @@ td_status build_class(int log2M, int n_seg, const SegIn* segs, const void* T64, 
       cudaMemcpy(t.Gp_ptrs, gp.data(), sizeof(cplx*) * n_seg, cudaMemcpyHostToDevice) != cudaSuccess ||
       cudaDeviceSynchronize() != cudaSuccess)
     return fail(TD_ECUDA);
+  if (staged) {
+    SegDev* hs = new (std::nothrow) SegDev[n_seg];
+    if (!hs) return fail(TD_ENOMEM);
+    for (int s = 0; s < n_seg; ++s) hs[s] = sd[s];
+    t.host_segs = hs;
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return fail(TD_ECUDA);
+    td_status a = launch_block<true>(dev, nullptr, 0, 0, nullptr, 0, nullptr, true);   // shared-memory attribute of the block kernels
+    if (a == TD_OK) a = launch_block<false>(dev, nullptr, 0, 0, nullptr, 0, nullptr, true);
+    if (a != TD_OK) return fail(a);
+  }
   *out = t;
   return TD_OK;
 }
@@ -144,6 +161,31 @@ td_status launch(const ClassTables& t, const Launch& L, int num_sms, int device,
   P.d = L.d; P.H = L.H; P.ldh = L.ldh; P.B = L.B; P.out0 = L.out0; P.out1 = L.out1;
   P.segs = static_cast<const SegDev*>(t.segs); P.n_seg = t.n_seg; P.accumulate = L.accumulate;
   P.T = static_cast<const cplx*>(t.T);
+  if (staged_class(t.log2M)) {
+    if (dry) return TD_OK;
+    if (!L.staged || !t.host_segs) return TD_EINVAL;
+    StagedCtx C;
+    C.device = device;
+    C.wsU = L.staged->wsU; C.wsU_bytes = L.staged->wsU_bytes; C.wsZ = L.staged->wsZ; C.wsZ_bytes = L.staged->wsZ_bytes;
+    C.wsPartial = L.staged->wsPartial; C.wsP_elems = L.staged->wsP_elems;
+    C.aux_stream = L.staged->aux_stream; C.ev_fork = L.staged->ev_fork; C.ev_join = L.staged->ev_join;
+    C.launches = L.staged->launches;
+    const SegDev* hs = static_cast<const SegDev*>(t.host_segs);
+    const double sc0 = L.mode == MODE_LOGLIKE ? -0.5 : 1.0;
+    int accumulate = L.accumulate;
+    for (int s = 0; s < t.n_seg; ++s) {   // one segment after the other, accumulating into the outputs
+      td_status r;
+      switch (L.mode) {
+        case MODE_LOGLIKE: r = run_staged<MODE_LOGLIKE>(C, t.log2M, P.T, hs[s], L.d, L.H, L.ldh, L.B, L.out0, L.out1, sc0, 1.0, accumulate, st); break;
+        case MODE_INNER: r = run_staged<MODE_INNER>(C, t.log2M, P.T, hs[s], L.d, L.H, L.ldh, L.B, L.out0, L.out1, sc0, 1.0, accumulate, st); break;
+        case MODE_STOREZ: r = run_staged<MODE_STOREZ>(C, t.log2M, P.T, hs[s], L.d, L.H, L.ldh, L.B, L.out0, L.out1, sc0, 1.0, accumulate, st); break;
+        default: return TD_EINVAL;
+      }
+      if (r != TD_OK) return r;
+      accumulate = 1;
+    }
+    return TD_OK;
+  }
   if (L.syn) {
     if (L.mode != MODE_LOGLIKE) return TD_EINVAL;
     switch (t.log2M) {

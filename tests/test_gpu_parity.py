@@ -991,3 +991,32 @@ def test_fp32_and_parameter_calls_capture_into_a_cuda_graph():
     ref = O.loglike_batch(w.acf, w.seg_lengths, w.d, w.H[:50])
     _assert_close(e_rows.cpu().numpy()[:50], ref, tol=TOL32, what="fp32 rows")
     _assert_close(e_big.cpu().numpy()[:50], ref, tol=TOL32, what="fp32 params")
+
+
+def test_f32_long_segments_on_the_staged_kernels():
+    """Segments of 16384+ samples run the fp32 build of the staged kernels (the paper's own FP32 example is N = 16384,
+    PAPER.md:268): a sample of rows against the fp64 oracle (library Levinson solve), every row against the fp64 GPU result,
+    cross terms, and the full c4 size against the fp64 path."""
+    w = W.make("c4", B=40, n_scale=4)
+    ref = O.loglike_batch_solve_toeplitz(w.acf, w.seg_lengths, w.d, w.H[:4])
+    with tdb.TDLikelihood(w.acf, w.seg_lengths) as h:
+        d, H = _dev(w.d), _dev(w.H)
+        o64 = h.loglike_batch(d, H).cpu().numpy()
+        dh64, hh64 = h.inner_batch(d, H)
+        h.set_precision(tdb.TD_PREC_F32)
+        o32 = h.loglike_batch(d, H).cpu().numpy()
+        dh32, hh32 = h.inner_batch(d, H)
+        torch.cuda.synchronize()
+    _assert_close(o32[:4], ref, tol=TOL32, what="c4/4 fp32 vs oracle")
+    err = np.abs(o32 - o64) / np.maximum(np.abs(o64), 1.0)
+    assert 1e-12 < err.max() <= TOL32
+    scale = hh64.abs() + dh64.abs() + 1.0
+    assert float(((hh32 - hh64).abs() / scale).max()) <= TOL32 and float(((dh32 - dh64).abs() / scale).max()) <= TOL32
+    w = W.make("c4")
+    with tdb.TDLikelihood(w.acf, w.seg_lengths) as h:
+        d, H = _dev(w.d), _dev(w.H)
+        o64 = h.loglike_batch(d, H).cpu().numpy()
+        h.set_precision(tdb.TD_PREC_F32)
+        o32 = h.loglike_batch(d, H).cpu().numpy()
+    err = np.abs(o32 - o64) / np.maximum(np.abs(o64), 1.0)
+    assert 1e-12 < err.max() <= TOL32, f"c4 full size: {err.max():.2e}"
