@@ -1020,3 +1020,27 @@ def test_f32_long_segments_on_the_staged_kernels():
         o32 = h.loglike_batch(d, H).cpu().numpy()
     err = np.abs(o32 - o64) / np.maximum(np.abs(o64), 1.0)
     assert 1e-12 < err.max() <= TOL32, f"c4 full size: {err.max():.2e}"
+
+
+def test_f32_mixed_staged_fused_and_dense_classes():
+    """One handle with a staged-class segment (20000 samples), a cluster-class one (5000), a fused-class one (3000) and a
+    dense-class one (200): fp32 evaluation accumulates over all of them (the dense segment stays fp64) and agrees with the
+    fp64 evaluation of the same handle, itself checked against the oracle on a few rows."""
+    rng = np.random.default_rng(321)
+    lens = [20000, 200, 5000, 3000]
+    acf = np.concatenate([W.acf_from_psd(4096.0, 2 * 32768, n) * s for n, s in zip(lens, (1.0, 0.5, 1.7, 0.9))])
+    nt = sum(lens)
+    d = rng.standard_normal(nt) * 1e-21
+    H = rng.standard_normal((21, nt)) * 1e-21
+    ref = O.loglike_batch_solve_toeplitz(acf, lens, d, H[:3])
+    with tdb.TDLikelihood(acf, lens) as h:
+        o64 = h.loglike_batch(_dev(d), _dev(H)).cpu().numpy()
+        dh64, hh64 = h.inner_batch(_dev(d), _dev(H))
+        h.set_precision(tdb.TD_PREC_F32)
+        o32 = h.loglike_batch(_dev(d), _dev(H)).cpu().numpy()
+        dh32, hh32 = h.inner_batch(_dev(d), _dev(H))
+        torch.cuda.synchronize()
+    _assert_close(o64[:3], ref, what="mixed classes fp64")
+    _assert_close(o32, o64, tol=TOL32, what="mixed classes fp32 vs fp64")
+    scale = hh64.abs() + dh64.abs() + 1.0
+    assert float(((hh32 - hh64).abs() / scale).max()) <= TOL32 and float(((dh32 - dh64).abs() / scale).max()) <= TOL32
