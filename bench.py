@@ -304,16 +304,18 @@ def main():
     # ---------------- end to end: host buffers through the C ABI (H2D of H and d, D2H of out, per step)
     e2e = None
     if not args.no_e2e:
-        out_host = np.empty(B)
+        # every host buffer of the end-to-end legs is page-locked (the contract: inputs come from pinned host memory)
+        d_pin = torch.as_tensor(w.d).pin_memory().numpy()
+        out_host = torch.empty(B, dtype=torch.float64).pin_memory().numpy()
         for _ in range(2):
-            h.loglike_batch_host(w.d, H_host, out_host)
+            h.loglike_batch_host(d_pin, H_host, out_host)
         torch.cuda.synchronize()
         barrier()
         k_e2e = max(3, min(args.steps, 10))
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record(stream)
         for _ in range(k_e2e):
-            h.loglike_batch_host(w.d, H_host, out_host)
+            h.loglike_batch_host(d_pin, H_host, out_host)
         e1.record(stream)
         torch.cuda.synchronize()
         barrier()
@@ -332,16 +334,18 @@ def main():
     # 5 doubles per template cross the bus, the rows are synthesised on the device.  Extra key, not `e2e`.
     e2e_params = None
     if not args.no_e2e and args.op == "loglike" and w.params is not None:
-        out_p = np.empty(B)
+        d_pin = torch.as_tensor(w.d).pin_memory().numpy()
+        p_pin = torch.as_tensor(np.ascontiguousarray(w.params)).pin_memory().numpy()
+        out_p = torch.empty(B, dtype=torch.float64).pin_memory().numpy()
         for _ in range(2):
-            h.loglike_family_batch_host(w.d, w.family, w.params, w.fs, out_p)
+            h.loglike_family_batch_host(d_pin, w.family, p_pin, w.fs, out_p)
         torch.cuda.synchronize()
         barrier()
         k_p = max(3, min(args.steps, 10))
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record(stream)
         for _ in range(k_p):
-            h.loglike_family_batch_host(w.d, w.family, w.params, w.fs, out_p)
+            h.loglike_family_batch_host(d_pin, w.family, p_pin, w.fs, out_p)
         e1.record(stream)
         torch.cuda.synchronize()
         barrier()
