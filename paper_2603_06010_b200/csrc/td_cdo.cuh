@@ -168,6 +168,16 @@ __global__ void __launch_bounds__(DENSE_NT, 1) td_cdo_kernel(const CdoParams P) 
     if (nbuf == 2) asm volatile("cp.async.wait_group 1;" ::: "memory");
     else asm volatile("cp.async.wait_group 0;" ::: "memory");
     group_sync();
+    // single-buffered panels (the large tiles): the rows of this group's NEXT tile start their way from HBM into L2 now, so the
+    // copy that is issued after this tile's contraction - and waited for - finds them there
+    if (nbuf == 1 && vec && wr == 0) {
+      const long long tn = t + gstride;
+      if (tn < ntiles && lane < TB) {
+        const long long bn = tn * TB + lane;
+        if (bn < Btot)
+          asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(P.H + bn * ldh + P.off), "r"((uint32_t)(n * 8)) : "memory");
+      }
+    }
     const double* xb = Xg + (size_t)buf * psz + (size_t)r * ldx + c;
     double q1[NC][2];
 #pragma unroll
