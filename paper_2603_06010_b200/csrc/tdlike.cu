@@ -34,6 +34,8 @@ constexpr int FUSED_MIN_LOG2M = 8;   // M = 256
 constexpr int CLUSTER_LOG2M = 13;    // M = 8192: 2-CTA cluster, one branch per CTA (td_cluster.cuh)
 constexpr int FUSED_NT = 256;
 constexpr int DENSE_AUTO_N = 512;     // AUTO: dense paths for segments up to this length (measured crossover: profiles/r01_chooser.md)
+constexpr int CDO_AUTO_MAX_N = 768;   // AUTO, log-likelihood: size classes whose segments are all at most this long take the CDO kernel
+                                      // (measured against the FFT kernels, profiles/r02_cdo.md: 42 vs 31 M evals/s at 768, 30 vs 31 at 832)
 constexpr int CDO_AUTO_MIN_N = 65;    // AUTO, log-likelihood: cached-L^-1 contraction from this length up, the Gohberg-Semencul
                                       // dense kernel below (measured: profiles/r02_cdo.md; 0.95x at N = 64, 1.08-1.55x above)
 
@@ -43,6 +45,7 @@ struct SegHost {
   int log2M = 0;
   double v = 0.0, logdet = 0.0;
   double rho0 = 0.0;    // rho_s(0): normalisation of the fp32 evaluation mode
+  bool auto_cdo = false;  // AUTO evaluates this segment's log-likelihood with the CDO kernel
   double* a = nullptr;  // device [n]
   cplx* G = nullptr;    // device [2][M]
   cplx* Gp = nullptr;   // device [2][padded(M)], padded Z layout (fused4 classes only)
@@ -81,6 +84,7 @@ struct td_handle {
   std::vector<ClassInfo> classes;
   int path = TD_PATH_AUTO, fft_variant = 0, last_path = 0, last_launches = 0;
   int precision = TD_PREC_F64;
+  bool any_auto_ll = false;   // some size class goes to the dense kernels for the log-likelihood under AUTO
   int cluster16_cap = 0;   // co-resident 16-CTA clusters of td_cluster16_kernel (0: M = 65536 stays on the staged kernels)
   int max_n = 0;
   // staged workspace: U / Z sized by td_create (two lanes of an L2-resident chunk), the per-block partial sums by
@@ -303,11 +307,12 @@ bool class_is_fused(const td_handle* h, const ClassInfo& c) {
 }
 
 
-// AUTO sends a size class to the dense path when every segment in it is at most dense.auto_n long.
-bool class_is_dense(const td_handle* h, const ClassInfo& c) {
+// AUTO sends a size class to the dense paths when every segment in it is short enough: up to CDO_AUTO_MAX_N samples for the
+// log-likelihood (CDO kernel), up to dense.auto_n for the cross terms (Gohberg-Semencul dense kernel)
+bool class_is_dense(const td_handle* h, const ClassInfo& c, int mode) {
   if (h->path == TD_PATH_DENSE || h->path == TD_PATH_CDO) return true;
   if (h->path == TD_PATH_FFT) return false;
-  return c.max_n <= h->dense.auto_n;
+  return c.max_n <= (mode == MODE_LOGLIKE ? CDO_AUTO_MAX_N : h->dense.auto_n);
 }
 
 // (re)builds the segment tables of the dense path from the host-side segment records
@@ -321,7 +326,8 @@ td_status dense_upload(td_handle* h) {
       DenseSeg ds;
       ds.off = sg.off; ds.n = sg.n; ds.npad = (sg.n + 31) / 32 * 32; ds.a = sg.a; ds.rsv = 1.0 / std::sqrt(sg.v); ds.zd = sg.zd;
       D.all.push_back(ds);
-      if (c.max_n <= D.auto_n) { D.aut.push_back(ds); if (sg.n < CDO_AUTO_MIN_N) D.aut_gs.push_back(ds); }
+      if (c.max_n <= D.auto_n) D.aut.push_back(ds);
+      if (c.max_n <= CDO_AUTO_MAX_N && sg.n < CDO_AUTO_MIN_N) D.aut_gs.push_back(ds);
     }
   D.max_n = DENSE_MAX_N;
   if (h->max_n > DENSE_MAX_N) D.all.clear();
@@ -373,15 +379,15 @@ td_status launch_dense(td_handle* h, const std::vector<DenseSeg>& segs, const do
 }
 
 // CDO path (td_cdo.cuh): W = L^{-1} per segment, built on the first use of TD_PATH_CDO
-// (segments of at most max_n samples that do not have their W yet; synchronous)
-td_status cdo_setup(td_handle* h, int max_n) {
+// (every segment, or the ones AUTO gives to the CDO kernel, that do not have their W yet; synchronous)
+td_status cdo_setup(td_handle* h, bool all_segments) {
   if (h->cdoW.empty()) h->cdoW.assign(h->n_seg, nullptr);
   std::vector<CdoSeg> cs;
   std::vector<int> ids;
   td_status st = TD_OK;
   for (int s = 0; s < h->n_seg && st == TD_OK; ++s) {
     const SegHost& sg = h->segs[s];
-    if (sg.n > max_n || sg.n > CDO_MAX_N || h->cdoW[s]) continue;
+    if (!(all_segments || sg.auto_cdo) || sg.n > CDO_MAX_N || h->cdoW[s]) continue;
     const int npad = (sg.n + 31) / 32 * 32;
     double* W = nullptr;
     if (cudaMalloc(&W, sizeof(double) * (size_t)npad * npad) != cudaSuccess) { st = TD_ENOMEM; break; }
@@ -426,13 +432,13 @@ td_status launch_cdo_nc(td_handle* h, const CdoParams& P0, int nbuf, cudaStream_
 
 // one launch per segment; 32-template panels (NC = 4) where one fits shared memory, else 16 (NC = 2); double-buffered
 // panels where two fit
-// (segments of at most max_n samples; *count receives how many ran)
+// (every segment, or the ones AUTO gives to the CDO kernel; *count receives how many ran)
 td_status launch_cdo(td_handle* h, const double* d, const double* H, int64_t ldh, int64_t B, double* out, int accumulate,
-                     cudaStream_t st, int min_n, int max_n, int* count, bool dry = false) {
+                     cudaStream_t st, bool all_segments, int* count, bool dry = false) {
   if (count) *count = 0;
   for (int s = 0; s < h->n_seg; ++s) {
     const SegHost& sg = h->segs[s];
-    if (sg.n > max_n || sg.n < min_n) continue;
+    if (!(all_segments || sg.auto_cdo)) continue;
     if (h->cdoW.empty() || !h->cdoW[s]) return TD_EUNSUPPORTED;  // (never: td_create / td_set_path built it)
     if (count) ++*count;
     CdoParams P;
@@ -563,9 +569,9 @@ td_status run_fft_path(td_handle* h, const double* d, const double* H, int64_t l
                        double* out1, cudaStream_t st, bool skip_dense_classes = false, int accumulate = 0, bool f32 = false) {
   const double sc0 = (MODE == MODE_LOGLIKE) ? -0.5 : 1.0, sc1 = 1.0;
   for (const ClassInfo& cls : h->classes) {
-    if (skip_dense_classes && class_is_dense(h, cls)) continue;
+    if (skip_dense_classes && class_is_dense(h, cls, MODE)) continue;
     const bool st32 = td32api::staged_class(cls.log2M);   // (a fused-shape class forced onto the staged kernels stays fp64)
-    if (f32 && cls.has32 && !class_is_dense(h, cls) && (st32 || class_is_fused(h, cls)) && h->fft_variant != 3) {
+    if (f32 && cls.has32 && !class_is_dense(h, cls, MODE) && (st32 || class_is_fused(h, cls)) && h->fft_variant != 3) {
       td32api::Launch L;
       L.d = d; L.H = H; L.ldh = ldh; L.B = B; L.out0 = out0; L.out1 = out1; L.accumulate = accumulate; L.mode = MODE;
       td32api::StagedBorrow sb;
@@ -612,7 +618,7 @@ template <int MODE>
 td_status run_batch(td_handle* h, const double* d, const double* H, int64_t ldh, int64_t B, double* out0,
                     double* out1, cudaStream_t st) {
   const DenseState& D = h->dense;
-  if (MODE == MODE_LOGLIKE && (h->path == TD_PATH_CDO || (h->path == TD_PATH_AUTO && !D.aut.empty()))) {
+  if (MODE == MODE_LOGLIKE && (h->path == TD_PATH_CDO || (h->path == TD_PATH_AUTO && h->any_auto_ll))) {
     // log-likelihood of the short segments: the triangular contraction with the cached L^{-1} (measured faster than the
     // Gohberg-Semencul dense kernel at every length up to 1024, profiles/r02_cdo.md); AUTO: the dense-class segments
     int nc = 0, ng = 0, acc = 0;
@@ -622,7 +628,7 @@ td_status run_batch(td_handle* h, const double* d, const double* H, int64_t ldh,
       if (s != TD_OK) return s;
       ng = (int)D.aut_gs.size(); acc = 1;
     }
-    td_status s = launch_cdo(h, d, H, ldh, B, out0, acc, st, forced ? 1 : CDO_AUTO_MIN_N, forced ? CDO_MAX_N : D.auto_n, &nc);
+    td_status s = launch_cdo(h, d, H, ldh, B, out0, acc, st, forced, &nc);
     if (s != TD_OK) return s;
     const bool all = nc + ng == h->n_seg;
     h->last_path = all ? (nc > 0 ? TD_PATH_CDO : TD_PATH_DENSE) : TD_PATH_FFT;
@@ -867,9 +873,14 @@ static td_status create_impl(td_handle* h, const double* acf, const int64_t* seg
   h->dense.auto_n = DENSE_AUTO_N;
   td_status ds = dense_upload(h);
   if (ds != TD_OK) return ds;
-  if (!h->dense.aut.empty()) {   // AUTO evaluates the dense-class segments with the cached L^{-1} (td_cdo.cuh)
-    ds = cdo_setup(h, h->dense.auto_n);
-    if (ds == TD_OK) ds = launch_cdo(h, nullptr, nullptr, h->n_tot, 1, nullptr, 0, nullptr, CDO_AUTO_MIN_N, h->dense.auto_n, nullptr, true);
+  for (const ClassInfo& c : h->classes)   // AUTO evaluates the log-likelihood of the short classes with the cached L^{-1} (td_cdo.cuh)
+    if (c.max_n <= CDO_AUTO_MAX_N) {
+      h->any_auto_ll = true;
+      for (int id : c.seg_ids) h->segs[id].auto_cdo = h->segs[id].n >= CDO_AUTO_MIN_N;
+    }
+  if (h->any_auto_ll) {
+    ds = cdo_setup(h, false);
+    if (ds == TD_OK) ds = launch_cdo(h, nullptr, nullptr, h->n_tot, 1, nullptr, 0, nullptr, false, nullptr, true);
     if (ds != TD_OK) return ds;
   }
   // ---- everything a batch call would otherwise create on first use: streams, events, scratch that does not grow with B
@@ -1147,8 +1158,8 @@ td_status td_set_path(td_handle* h, int path) {
   if (path == TD_PATH_CDO) {   // first use: builds W = L^{-1} per segment (synchronous), configures the kernel
     DevGuard guard(h->device);
     if (!guard.ok) return TD_ECUDA;
-    td_status s = cdo_setup(h, CDO_MAX_N);
-    if (s == TD_OK) s = launch_cdo(h, nullptr, nullptr, h->n_tot, 1, nullptr, 0, nullptr, 1, CDO_MAX_N, nullptr, true);
+    td_status s = cdo_setup(h, true);
+    if (s == TD_OK) s = launch_cdo(h, nullptr, nullptr, h->n_tot, 1, nullptr, 0, nullptr, true, nullptr, true);
     if (s != TD_OK) return s;
   }
   h->path = path;
