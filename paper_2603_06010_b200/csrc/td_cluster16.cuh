@@ -173,12 +173,10 @@ __device__ __forceinline__ cplx c16_basew(const C16Own& own, int lane, const cpl
 // in Z: E_s at s * 256 + jl, O_s at 4096 + s * 256 + jl), the pruned radix-2 join and the fused sums (last_pass_c of
 // td_fused.cuh with the strides of the distributed layout and the twiddles of the global table)
 template <int MODE>
-__device__ __forceinline__ void c16_last(const SmemArr& Z, int jl, int j, int n, cplx beta /* w_2M^j */, cplx w1 /* w_M^(-j) */,
-                                         cplx* __restrict__ zd, double& acc0, double& acc1) {
+__device__ __forceinline__ void c16_last_regs(cplx (&e)[16], cplx (&o)[16], int j, int n, cplx beta /* w_2M^j */,
+                                              cplx w1 /* w_M^(-j) */, cplx* __restrict__ zd, double& acc0, double& acc1) {
   constexpr int ML = Cluster16Shape::ML;
-  cplx e[16], o[16], gm[16];
-#pragma unroll
-  for (int ss = 0; ss < 16; ++ss) { e[ss] = Z.ld(ss * 256 + jl); o[ss] = Z.ld(ML + ss * 256 + jl); }
+  cplx gm[16];
   dit16<true, true>(e, w1);
   dit16<true, true>(o, w1);
   const cplx cb = cconj(beta);
@@ -205,6 +203,15 @@ __device__ __forceinline__ void c16_last(const SmemArr& Z, int jl, int j, int n,
   });
   if constexpr (MODE == MODE_INNER) acc0 += (double)((p0[0] + p0[1]) + (p0[2] + p0[3]));
   if constexpr (MODE != MODE_STOREZ) acc1 += (double)((p1[0] + p1[1]) + (p1[2] + p1[3]));
+}
+template <int MODE>
+__device__ __forceinline__ void c16_last(const SmemArr& Z, int jl, int j, int n, cplx beta, cplx w1, cplx* __restrict__ zd,
+                                         double& acc0, double& acc1) {
+  constexpr int ML = Cluster16Shape::ML;
+  cplx e[16], o[16];
+#pragma unroll
+  for (int ss = 0; ss < 16; ++ss) { e[ss] = Z.ld(ss * 256 + jl); o[ss] = Z.ld(ML + ss * 256 + jl); }
+  c16_last_regs<MODE>(e, o, j, n, beta, w1, zd, acc0, acc1);
 }
 
 

@@ -19,6 +19,7 @@
 #include "td_fused.cuh"
 #include "td_cluster.cuh"
 #include "td_cluster16.cuh"
+#include "td_group16.cuh"
 #include "td_fused4.cuh"
 #include "td_setup.cuh"
 #include "td_staged_host.cuh"
@@ -85,6 +86,8 @@ struct td_handle {
   int path = TD_PATH_AUTO, fft_variant = 0, last_path = 0, last_launches = 0;
   int precision = TD_PREC_F64;
   bool any_auto_ll = false;   // some size class goes to the dense kernels for the log-likelihood under AUTO
+  int group16_cap = 0;     // co-resident 16-CTA groups of td_group16_kernel (td_group16.cuh)
+  unsigned* g16_bar = nullptr;  // device [G16_MAX_GROUPS][2] arrival counters of that kernel
   int cluster16_cap = 0;   // co-resident 16-CTA clusters of td_cluster16_kernel (0: M = 65536 stays on the staged kernels)
   int max_n = 0;
   // staged workspace: U / Z sized by td_create (two lanes of an L2-resident chunk), the per-block partial sums by
@@ -131,7 +134,7 @@ void free_handle(td_handle* h) {
   if (!h) return;
   for (auto& s : h->segs) { cudaFree(s.a); cudaFree(s.G); cudaFree(s.Gp); cudaFree(s.Gc16); cudaFree(s.zd); }
   for (auto& c : h->classes) { cudaFree(c.T); cudaFree(c.d_segs); cudaFree(c.d_Gp); if (c.has32) td32api::free_class(&c.t32); }
-  cudaFree(h->wsU); cudaFree(h->wsZ); cudaFree(h->wsPartial); cudaFree(h->wsDot); cudaFree(h->ud); cudaFree(h->synH); cudaFree(h->synP); cudaFree(h->synSeg);
+  cudaFree(h->wsU); cudaFree(h->wsZ); cudaFree(h->wsPartial); cudaFree(h->g16_bar); cudaFree(h->wsDot); cudaFree(h->ud); cudaFree(h->synH); cudaFree(h->synP); cudaFree(h->synSeg);
   cudaFree(h->hsD); cudaFree(h->hsH[0]); cudaFree(h->hsH[1]); cudaFree(h->hsOut);
   cudaFree(h->d_rho);
   for (double* w : h->cdoW) cudaFree(w);
@@ -523,6 +526,74 @@ td_status launch_cluster16(td_handle* h, const Cluster16Params& PC, int* ncluste
   return TD_OK;
 }
 
+// ---- M = 65536 as one persistent kernel of 16-CTA groups exchanging through L2 (td_group16.cuh)
+constexpr int G16_MAX_GROUPS = 16;
+template <int MODE>
+td_status launch_group16(td_handle* h, const Group16Params& PG, int* ngroups, cudaStream_t st, bool dry) {
+  auto kern = td_group16_kernel<MODE>;
+  const size_t smem = Cluster16Shape::smem_bytes();
+  static int cache[TD_MAX_DEV];
+  int per_sm = 0;
+  td_status cs = kernel_config(kern, Cluster16Shape::NT, smem, smem, h->device, cache, &per_sm);
+  if (cs != TD_OK) return cs;
+  *ngroups = std::min(G16_MAX_GROUPS, per_sm * h->num_sms / Cluster16Shape::CS);
+  if (dry || *ngroups < 1) return TD_OK;
+  const long long want = MODE == MODE_STOREZ ? 1 : PG.base.B;
+  const unsigned groups = (unsigned)std::max<long long>(1, std::min<long long>(want, *ngroups));
+  CK(cudaMemsetAsync(PG.bar, 0, sizeof(unsigned) * 2 * G16_MAX_GROUPS, st));
+  cudaLaunchConfig_t cfg = {};
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeCooperative;   // every CTA co-resident: the groups synchronise through global counters
+  attr[0].val.cooperative = 1;
+  cfg.gridDim = dim3(Cluster16Shape::CS * groups); cfg.blockDim = dim3(Cluster16Shape::NT);
+  cfg.dynamicSmemBytes = smem; cfg.stream = st; cfg.attrs = attr; cfg.numAttrs = 1;
+  CK(cudaLaunchKernelEx(&cfg, kern, PG));
+  ++h->last_launches;
+  return TD_OK;
+}
+int group16_capacity(td_handle* h) {
+  Group16Params PG = {};
+  int n = 0, m = 0, z = 0;
+  if (launch_group16<MODE_LOGLIKE>(h, PG, &n, nullptr, true) != TD_OK) return 0;
+  if (launch_group16<MODE_INNER>(h, PG, &m, nullptr, true) != TD_OK) return 0;
+  if (launch_group16<MODE_STOREZ>(h, PG, &z, nullptr, true) != TD_OK) return 0;
+  return std::min(n, std::min(m, z));
+}
+// the exchange buffers are the staged workspace (L2-resident by size): groups x 2 parities x (2 NF | 2 M) elements
+bool group16_fits(const td_handle* h, int groups) {
+  return h->g16_bar && h->wsU_elems >= (size_t)groups * 4 * Cluster16Shape::NF && h->wsZ_elems >= (size_t)groups * 4 * Cluster16Shape::M &&
+         h->wsP_elems >= (size_t)Cluster16Shape::CS * 2;
+}
+
+template <int MODE>
+td_status run_group16(td_handle* h, const ClassInfo& cls, int idx_in_class, const double* d, const double* H, int64_t ldh,
+                      int64_t B, double* out0, double* out1, double scale0, double scale1, int accumulate, cudaStream_t st) {
+  const SegHost& sg = h->segs[cls.seg_ids[idx_in_class]];
+  const int64_t SB = std::max<int64_t>(1, (int64_t)(h->wsP_elems / (Cluster16Shape::CS * 2)));   // templates per partial buffer
+  h->touched = true;
+  const int64_t Bn = (MODE == MODE_STOREZ) ? 1 : B;
+  for (int64_t b0 = 0; b0 < Bn; b0 += SB) {
+    const int64_t nb = std::min<int64_t>(SB, Bn - b0);
+    Group16Params PG;
+    PG.base.d = d; PG.base.H = H ? H + b0 * ldh : nullptr; PG.base.ldh = ldh; PG.base.B = nb;
+    PG.base.out0 = nullptr; PG.base.out1 = nullptr; PG.base.segs = cls.d_segs + idx_in_class; PG.base.n_seg = 1;
+    PG.base.accumulate = 0; PG.base.T = cls.T;
+    PG.Gp = sg.Gc16; PG.partial = h->wsPartial;
+    PG.wsU = static_cast<cplx*>(h->wsU); PG.wsZ = static_cast<cplx*>(h->wsZ); PG.bar = h->g16_bar;
+    int ng = 0;
+    td_status s = launch_group16<MODE>(h, PG, &ng, st, false);
+    if (s != TD_OK) return s;
+    if (ng < 1) return TD_EUNSUPPORTED;
+    if (MODE != MODE_STOREZ) {
+      lg_finish_kernel<<<(unsigned)((nb + 127) / 128), 128, 0, st>>>(h->wsPartial, Cluster16Shape::CS, (int)nb, out0 ? out0 + b0 : nullptr,
+                                                                    out1 ? out1 + b0 : nullptr, scale0, scale1, accumulate);
+      CK(cudaGetLastError());
+      ++h->last_launches;
+    }
+  }
+  return TD_OK;
+}
+
 // how many 16-CTA clusters of the kernel fit the device (0: the class stays on the staged kernels)
 int cluster16_capacity(td_handle* h) {
   int n = 0;
@@ -600,10 +671,12 @@ td_status run_fft_path(td_handle* h, const double* d, const double* H, int64_t l
       // kernels on c4 - its two all-to-all exchanges run at the 16 B/cycle/SM of distributed-shared-memory stores and only 7
       // clusters (112 of 148 SMs) are co-resident (profiles/r02_c4_cluster16.md)
       const bool c16 = cls.log2M == Cluster16Shape::LOG2M && h->fft_variant == 3 && h->cluster16_cap > 0;
+      const bool g16 = cls.log2M == Cluster16Shape::LOG2M && h->fft_variant == 4 && h->group16_cap > 0;
       for (size_t i = 0; i < cls.seg_ids.size(); ++i) {
         const int id = cls.seg_ids[i];
         td_status s = c16 ? run_cluster16<MODE>(h, cls, (int)i, d, H, ldh, B, out0, out1, sc0, sc1, accumulate, st)
-                          : run_staged<MODE>(h, cls, h->segs[id], d, H, ldh, B, out0, out1, sc0, sc1, accumulate, st);
+                      : g16 ? run_group16<MODE>(h, cls, (int)i, d, H, ldh, B, out0, out1, sc0, sc1, accumulate, st)
+                            : run_staged<MODE>(h, cls, h->segs[id], d, H, ldh, B, out0, out1, sc0, sc1, accumulate, st);
         if (s != TD_OK) return s;
         accumulate = 1;
       }
@@ -1167,7 +1240,18 @@ td_status td_set_path(td_handle* h, int path) {
 }
 
 td_status td_set_fft_variant(td_handle* h, int variant) {
-  if (!h || variant < 0 || variant > 3) return TD_EINVAL;
+  if (!h || variant < 0 || variant > 4) return TD_EINVAL;
+  if (variant == 4) {   // 16-CTA groups exchanging through L2
+    bool has16 = false;
+    for (const ClassInfo& c : h->classes) has16 = has16 || c.log2M == Cluster16Shape::LOG2M;
+    if (!has16) return TD_EUNSUPPORTED;
+    DevGuard guard(h->device);
+    if (!guard.ok) return TD_ECUDA;
+    if (!h->g16_bar && cudaMalloc(&h->g16_bar, sizeof(unsigned) * 2 * G16_MAX_GROUPS) != cudaSuccess) { cudaGetLastError(); return TD_ENOMEM; }
+    if (h->group16_cap < 1) h->group16_cap = group16_capacity(h);
+    while (h->group16_cap > 0 && !group16_fits(h, h->group16_cap)) --h->group16_cap;
+    if (h->group16_cap < 1) return TD_EUNSUPPORTED;
+  }
   if (variant == 3) {   // the 16-CTA cluster kernel needs a 65536-class segment and a device that can host the cluster
     bool has16 = false;
     for (const ClassInfo& c : h->classes) has16 = has16 || c.log2M == Cluster16Shape::LOG2M;
