@@ -39,7 +39,15 @@ FP64_PEAK_TFLOPS = 37.2
 FP32_PEAK_TFLOPS = 74.4
 # dominant kernel of a step, per config
 DOMINANT = {"c1": "td_fused4_kernel<10>", "c2": "td_fused4_kernel<12>", "c3": "td_cluster_kernel",
-            "c4": "staged lg_* kernels", "c5": "td_cluster_kernel"}
+            "c4": "td_group16_kernel", "c5": "td_cluster_kernel"}
+
+
+def _dominant(config, variant, f32):
+    if config == "c4":   # 65536 class: group kernel by default; the staged kernels in fp32 and on request; the cluster kernel on request
+        if f32 or variant == 2:
+            return "staged lg_* kernels" + (" (fp32 build)" if f32 else "")
+        return "td_cluster16_kernel" if variant == 3 else "td_group16_kernel"
+    return DOMINANT.get(config, "td_fused_kernel") + (" (fp32 build)" if f32 else "")
 
 
 def alg_flops_per_eval(seg_lengths) -> float:
@@ -393,7 +401,7 @@ def main():
                 # fraction against the DFMA register loop measured in THIS run (state both denominators)
                 "frac_vs_measured_loop": ach_tf / probe["ffma_fp32" if f32 else "dfma"],
                 "traffic": traffic, "traffic_source": traffic_source,
-                "kernel": ("td_cdo_kernel" if cdo else "td_dense_kernel") if dense else DOMINANT.get(args.config, "td_fused_kernel") + (" (fp32 build)" if f32 else ""),
+                "kernel": ("td_cdo_kernel" if cdo else "td_dense_kernel") if dense else _dominant(args.config, args.fft_variant, f32),
                 "measured_register_loop_tflops": probe,
                 "kernel_ms": kern_ms, "alg_flops_per_eval": falg,
                 "peak_source": ("derived: 128 FFMA/clk/SM x 148 SM x 1.965 GHz x 2; the FFMA register loop of this run beside it"

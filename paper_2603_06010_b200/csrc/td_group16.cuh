@@ -31,8 +31,7 @@ struct Group16Params {
 
 // one thread, after the CTA's barrier: the CTA's stores are visible device-wide before the count moves
 __device__ __forceinline__ void g16_arrive(unsigned* ctr) {
-  __threadfence();
-  atomicAdd(ctr, 1u);
+  asm volatile("red.release.gpu.global.add.u32 [%0], %1;" ::"l"(ctr), "r"(1u) : "memory");
 }
 __device__ __forceinline__ void g16_wait(const unsigned* ctr, unsigned target) {
   const long long t0 = clock64();
@@ -58,7 +57,7 @@ __global__ void __launch_bounds__(Cluster16Shape::NT, 1) td_group16_kernel(const
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(red + 2 * Sh::NW + 2);
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int rank = blockIdx.x & 15;
-  const long long grp = blockIdx.x >> 4, ngrp = gridDim.x >> 4;
+  const int grp = blockIdx.x >> 4, ngrp = gridDim.x >> 4;
   const int brG = c16_branch(rank), tsubA = c16_sub(rank, 0), tsubB = c16_sub(rank, 1);
   const C16Own own = c16_own(rank, warp);
   const cplx* __restrict__ T = P.T;
@@ -79,10 +78,6 @@ __global__ void __launch_bounds__(Cluster16Shape::NT, 1) td_group16_kernel(const
   tmem_wait_st();
   const cplx basew = c16_basew(own, lane, T, tsubA, tsubB, brG);
   const int g0 = tid >> 7, j0 = 128 * rank + (tid & 127), jr = 256 * rank + tid;
-  const cplx f0_w1 = __ldg(T + 4 * j0);            // w_NF^j0
-  const cplx f0_beta = __ldg(T + 2 * j0);          // w_M^j0
-  const cplx l0_beta = __ldg(T + jr);              // w_2M^jr
-  const cplx l0_w1 = cconj(__ldg(T + 2 * jr));     // w_M^(-jr)
   if (MODE == MODE_LOGLIKE) {                      // this thread's 16 sample pairs of the data vector, once per launch
     const double* drow = P.d + sg.off;
     double2 dvs[16];
@@ -107,7 +102,7 @@ __global__ void __launch_bounds__(Cluster16Shape::NT, 1) td_group16_kernel(const
 #pragma unroll
     for (int ss = 0; ss < 16; ++ss) { e[ss] = __ldcg(Zb + ss * ML + jr); o[ss] = __ldcg(Zb + M + ss * ML + jr); }
     double acc0 = 0.0, acc1 = 0.0;
-    c16_last_regs<MODE>(e, o, jr, sg.n, l0_beta, l0_w1, sg.zd, acc0, acc1);
+    c16_last_regs<MODE>(e, o, jr, sg.n, __ldg(T + jr) /* w_2M^jr */, cconj(__ldg(T + 2 * jr)) /* w_M^(-jr) */, sg.zd, acc0, acc1);
     if (MODE != MODE_STOREZ) {
       if (MODE == MODE_INNER) acc0 = warp_sum(acc0);
       acc1 = warp_sum(acc1);
@@ -177,7 +172,9 @@ __global__ void __launch_bounds__(Cluster16Shape::NT, 1) td_group16_kernel(const
           }
         }
       }
-      tw_powers<16>(f0_w1, w);
+      // (the per-thread constants of the two cross passes are re-read per item, L1 hits: registers are what this kernel lacks)
+      const cplx f0_beta = __ldg(T + 2 * j0);          // w_M^j0
+      tw_powers<16>(__ldg(T + 4 * j0), w);             // powers of w_NF^j0
       if (g0) {
         static_for<0, 16>([&](auto q) { x[decltype(q)::value] = mul_w32<decltype(q)::value, false>(x[decltype(q)::value]); });
         static_for<0, 16>([&](auto t) { w[decltype(t)::value] = cmul(w[decltype(t)::value], f0_beta); });

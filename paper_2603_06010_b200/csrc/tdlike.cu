@@ -565,6 +565,17 @@ bool group16_fits(const td_handle* h, int groups) {
          h->wsP_elems >= (size_t)Cluster16Shape::CS * 2;
 }
 
+// counters + occupancy; leaves group16_cap = -1 (class stays on the staged kernels) when the device cannot host a group
+td_status group16_setup(td_handle* h) {
+  if (!h->g16_bar && cudaMalloc(&h->g16_bar, sizeof(unsigned) * 2 * G16_MAX_GROUPS) != cudaSuccess) { cudaGetLastError(); return TD_ENOMEM; }
+  int coop = 0;
+  if (cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, h->device) != cudaSuccess || !coop) { cudaGetLastError(); h->group16_cap = -1; return TD_OK; }
+  h->group16_cap = group16_capacity(h);
+  while (h->group16_cap > 0 && !group16_fits(h, h->group16_cap)) --h->group16_cap;
+  if (h->group16_cap < 1) h->group16_cap = -1;   // asked and answered
+  return TD_OK;
+}
+
 template <int MODE>
 td_status run_group16(td_handle* h, const ClassInfo& cls, int idx_in_class, const double* d, const double* H, int64_t ldh,
                       int64_t B, double* out0, double* out1, double scale0, double scale1, int accumulate, cudaStream_t st) {
@@ -667,11 +678,12 @@ td_status run_fft_path(td_handle* h, const double* d, const double* H, int64_t l
       if (s != TD_OK) return s;
       accumulate = 1;
     } else {
-      // M = 65536 on the 16-CTA cluster kernel only on request (variant 3): measured 0.885 ms against 0.737 ms for the staged
+      // M = 65536: the group kernel (16 CTAs per template exchanging through L2, td_group16.cuh) when the device co-hosts a
+      // group, else the staged kernels.  The 16-CTA cluster kernel only on request (variant 3): measured 0.885 ms against 0.737 ms for the staged
       // kernels on c4 - its two all-to-all exchanges run at the 16 B/cycle/SM of distributed-shared-memory stores and only 7
       // clusters (112 of 148 SMs) are co-resident (profiles/r02_c4_cluster16.md)
       const bool c16 = cls.log2M == Cluster16Shape::LOG2M && h->fft_variant == 3 && h->cluster16_cap > 0;
-      const bool g16 = cls.log2M == Cluster16Shape::LOG2M && h->fft_variant == 4 && h->group16_cap > 0;
+      const bool g16 = cls.log2M == Cluster16Shape::LOG2M && h->fft_variant != 2 && h->fft_variant != 3 && h->group16_cap > 0;
       for (size_t i = 0; i < cls.seg_ids.size(); ++i) {
         const int id = cls.seg_ids[i];
         td_status s = c16 ? run_cluster16<MODE>(h, cls, (int)i, d, H, ldh, B, out0, out1, sc0, sc1, accumulate, st)
@@ -983,6 +995,13 @@ static td_status create_impl(td_handle* h, const double* acf, const int64_t* seg
     td_status a = staged_alloc(h, false);
     if (a != TD_OK) return a;
   }
+  // the 65536 class runs on the group kernel (td_group16.cuh) when the device can co-host at least one 16-CTA group; its
+  // exchange buffers are the staged workspace
+  for (const ClassInfo& c : h->classes)
+    if (c.log2M == Cluster16Shape::LOG2M && h->group16_cap == 0) {
+      td_status g = group16_setup(h);
+      if (g != TD_OK) return g;
+    }
   // ---- one dry pass over every kernel this handle can launch: shared-memory attributes and occupancy are cached now,
   // so that a batch call is launches only (and can be captured into a CUDA graph)
   return warm_kernels(h);
@@ -1241,16 +1260,10 @@ td_status td_set_path(td_handle* h, int path) {
 
 td_status td_set_fft_variant(td_handle* h, int variant) {
   if (!h || variant < 0 || variant > 4) return TD_EINVAL;
-  if (variant == 4) {   // 16-CTA groups exchanging through L2
+  if (variant == 4) {   // 16-CTA groups exchanging through L2: what variant 0 uses for the 65536 class when the device can
     bool has16 = false;
     for (const ClassInfo& c : h->classes) has16 = has16 || c.log2M == Cluster16Shape::LOG2M;
-    if (!has16) return TD_EUNSUPPORTED;
-    DevGuard guard(h->device);
-    if (!guard.ok) return TD_ECUDA;
-    if (!h->g16_bar && cudaMalloc(&h->g16_bar, sizeof(unsigned) * 2 * G16_MAX_GROUPS) != cudaSuccess) { cudaGetLastError(); return TD_ENOMEM; }
-    if (h->group16_cap < 1) h->group16_cap = group16_capacity(h);
-    while (h->group16_cap > 0 && !group16_fits(h, h->group16_cap)) --h->group16_cap;
-    if (h->group16_cap < 1) return TD_EUNSUPPORTED;
+    if (!has16 || h->group16_cap < 1) return TD_EUNSUPPORTED;
   }
   if (variant == 3) {   // the 16-CTA cluster kernel needs a 65536-class segment and a device that can host the cluster
     bool has16 = false;

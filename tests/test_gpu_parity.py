@@ -90,8 +90,12 @@ def test_c4_long_segment_vs_library_levinson():
     """N = 65536: dense C would be 32 GiB, so the oracle route is solve_toeplitz (pin P13)."""
     w = W.make("c4", B=3)
     ref = O.loglike_batch_solve_toeplitz(w.acf, w.seg_lengths, w.d, w.H)
-    out, _, _ = _gpu_loglike(w)
+    out, _, nl = _gpu_loglike(w)
     _assert_close(out, ref, what="c4")
+    assert nl == 2                                   # the group kernel (td_group16.cuh) + the rank-ordered sum of its partials
+    out_st, _, nl_st = _gpu_loglike(w, variant=2)    # the staged kernels (what a device that cannot co-host a group runs)
+    _assert_close(out_st, ref, what="c4 on the staged kernels")
+    assert nl_st > 2
     # the same segment on the 16-CTA cluster kernel (td_cluster16.cuh, variant 3): all three kernel modes
     dh_ref = None
     with tdb.TDLikelihood(w.acf, w.seg_lengths) as h:
@@ -130,6 +134,64 @@ def test_cluster16_ragged_length_many_items_and_refusal():
         with pytest.raises(tdb.TDError) as e:
             h.set_fft_variant(3)
         assert e.value.status == tdb.TD_EUNSUPPORTED
+
+
+def test_group16_ragged_length_many_items_modes_graph_and_two_handles():
+    """The default kernel of the 65536 class (16-CTA groups exchanging through L2, td_group16.cuh) against the staged
+    kernels (variant 2, themselves held to the oracle above): N = 40001 (odd, unaligned rows: scalar loads), more templates
+    than groups with an uneven remainder, all three kernel modes, bit-identical repeats, capture into a CUDA graph, and two
+    handles working at the same time on two streams (cooperative launches queue behind one another; nothing may hang)."""
+    rng = np.random.default_rng(161)
+    n = 40001
+    rho = W.acf_from_psd(4096.0, 2 * 65536, n)
+    d = rng.standard_normal(n) * 1e-21
+    H = rng.standard_normal((23, n)) * 1e-21
+    H[5] = d
+    H[7, 100] = np.nan
+    dd, HH = _dev(d), _dev(H)
+    with tdb.TDLikelihood(rho, [n]) as h, tdb.TDLikelihood(rho * 1.5, [n]) as h2:
+        h.set_fft_variant(2)
+        ref = h.loglike_batch(dd, HH).cpu().numpy()
+        dh_s, hh_s = h.inner_batch(dd, HH, want_hh=True)
+        dh_s, hh_s = dh_s.cpu().numpy(), hh_s.cpu().numpy()
+        assert h.last_launches() > 4
+        h.set_fft_variant(0)
+        out = h.loglike_batch(dd, HH).cpu().numpy()
+        assert h.last_launches() == 2
+        out2 = h.loglike_batch(dd, HH).cpu().numpy()
+        dh, hh = h.inner_batch(dd, HH, want_hh=True)
+        dh, hh = dh.cpu().numpy(), hh.cpu().numpy()
+        h.set_fft_variant(4)                                        # the explicit name of the same kernel
+        out4 = h.loglike_batch(dd, HH).cpu().numpy()
+        # graph capture: memset of the arrival counters + cooperative launch + reduction
+        s = torch.cuda.Stream()
+        og = torch.empty(23, dtype=torch.float64, device="cuda")
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.stream(s):
+            h.loglike_batch(dd, HH, out=og, stream=s)               # warm
+            s.synchronize()
+            with torch.cuda.graph(g, stream=s):
+                h.loglike_batch(dd, HH, out=og, stream=s)
+            og.zero_()
+            g.replay(); g.replay()
+            s.synchronize()
+        # two handles, two streams, interleaved calls
+        s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+        o1 = torch.empty(23, dtype=torch.float64, device="cuda")
+        o2 = torch.empty(23, dtype=torch.float64, device="cuda")
+        torch.cuda.synchronize()
+        for _ in range(4):
+            h.loglike_batch(dd, HH, out=o1, stream=s1)
+            h2.loglike_batch(dd, HH, out=o2, stream=s2)
+        torch.cuda.synchronize()
+    ok = np.isfinite(ref)
+    assert not ok[7] and ok.sum() == 22 and np.isnan(out[7])
+    assert out[5] == 0.0 and np.array_equal(out, out2, equal_nan=True) and np.array_equal(out, out4, equal_nan=True)
+    _assert_close(out[ok], ref[ok], what="group16, N = 40001")
+    assert np.array_equal(og.cpu().numpy(), out, equal_nan=True) and np.array_equal(o1.cpu().numpy(), out, equal_nan=True)
+    _assert_close(o2.cpu().numpy()[ok] * 1.5, ref[ok], what="group16, second handle (C scaled by 1.5)")
+    scale = np.max(np.abs(hh_s[ok]))
+    assert np.max(np.abs(hh[ok] - hh_s[ok])) <= 1e-9 * scale and np.max(np.abs(dh[ok] - dh_s[ok])) <= 1e-9 * scale
 
 
 # ------------------------------------------------------------------ shapes: ragged, tiny, mixed classes
