@@ -29,6 +29,7 @@
 #ifndef TDLIKE_H_
 #define TDLIKE_H_
 
+#include <stddef.h>
 #include <stdint.h>
 
 #ifdef __cplusplus
@@ -210,6 +211,44 @@ int td_last_launches(const td_handle* h);
 
 /* td_strerror - static string for a status code. */
 const char* td_strerror(td_status s);
+
+/* ---- allocation-free evaluation ------------------------------------------------------------------------------------
+ * For callers that cannot allocate device memory at call time (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc).  td_loglike_batch_static computes what td_loglike_batch computes (Eq. 10,
+ * PAPER.md:142; FFT route of Eqs. 14-16, :241-252) with the staged kernels (forward passes - untangle x generator - inverse
+ * passes - fused reduction on a global-memory workspace), whose workspace is NOT the handle's cudaMalloc'ed buffers but a
+ * file-scope device array of TD_STATIC_SCRATCH_BYTES inside the library image.  The call itself - and td_static_setup -
+ * call no cudaMalloc / cudaFree / allocating library routine; the handle (td_create) must exist beforehand.
+ *
+ * Limits and ownership:
+ *  - every GPU that loads this library holds TD_STATIC_SCRATCH_BYTES (16 MiB) of device memory for the array until the
+ *    process exits, whether or not the entry point is used;
+ *  - one template of a size class (segments padded to M = 2^k samples) needs 48 M + 16 ceil(M / (128 r)) bytes of it
+ *    (r = 2..16 the first radix): segments of at most 262144 samples.  A handle with a longer segment is refused with
+ *    TD_EUNSUPPORTED before anything is launched (td_static_last_error says how many bytes were needed); B is unlimited
+ *    (templates run in chunks of as many as the array holds);
+ *  - ONE array per GPU, shared by every handle, thread and stream of the process: two calls that overlap on the GPU
+ *    (different streams, or graphs replayed concurrently) race on it and return garbage; serialise them.  The array keeps the
+ *    last call's contents; nothing in it has to start at zero (every element a call reads it has written before), so
+ *    nothing is cleared;
+ *  - always fp64 and always the staged kernels, whatever td_set_path / td_set_fft_variant / td_set_precision say: it is
+ *    slower than td_loglike_batch wherever that runs a fused kernel.  Results agree with td_loglike_batch to rounding
+ *    (1e-9 relative, the parity tolerance; tests/test_zz_no_alloc.py).
+ * Arguments, layout, stream semantics and errors otherwise as td_loglike_batch: d, H, out DEVICE pointers. */
+#define TD_STATIC_SCRATCH_BYTES (16u << 20)
+td_status td_loglike_batch_static(td_handle* h, const double* d, const double* H, int64_t ldh,
+                                  int64_t B, double* out, void* stream /* cudaStream_t */);
+
+/* td_static_setup - resolves the device address of the array on `device` (cudaGetSymbolAddress, once per device) and
+ * configures the two shared-memory kernels of the staged pipeline there.  Optional: the first td_loglike_batch_static on a
+ * device does the same; call it beforehand when that first call would be inside a stream capture.  TD_ECUDA on failure. */
+td_status td_static_setup(int device);
+
+/* td_static_scratch_bytes - TD_STATIC_SCRATCH_BYTES of the loaded library.
+ * td_static_last_error - what the last td_static_setup / td_loglike_batch_static of the calling thread refused, in words
+ * ("" after a success); static storage, valid until the thread's next such call. */
+size_t td_static_scratch_bytes(void);
+const char* td_static_last_error(void);
 
 #ifdef __cplusplus
 }

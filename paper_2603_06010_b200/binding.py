@@ -38,6 +38,10 @@ SYMBOLS = {
     "td_get_generator": (_INT, [_VP, _INT, _DP]),
     "td_last_launches": (_INT, [_VP]),
     "td_strerror": (C.c_char_p, [_INT]),
+    "td_loglike_batch_static": (_INT, [_VP, _VP, _VP, _I64, _I64, _VP, _VP]),
+    "td_static_setup": (_INT, [_INT]),
+    "td_static_scratch_bytes": (C.c_size_t, []),
+    "td_static_last_error": (C.c_char_p, []),
 }
 
 _lib = None
@@ -70,6 +74,18 @@ def load(build_if_missing: bool = True) -> C.CDLL:
 
 def strerror(status: int) -> str:
     return load().td_strerror(int(status)).decode()
+
+
+def static_setup(device: int = 0):
+    """td_static_setup: resolve the static scratch array's device address on `device` (optional, see include/tdlike.h)."""
+    lib = load()
+    st = lib.td_static_setup(int(device))
+    if st != TD_OK:
+        raise TDError(st, "td_static_setup [" + lib.td_static_last_error().decode() + "]")
+
+
+def static_scratch_bytes() -> int:
+    return int(load().td_static_scratch_bytes())
 
 
 def _check(status: int, what: str):
@@ -145,6 +161,22 @@ class TDLikelihood:
         st = self._lib.td_loglike_batch(self._h, _ptr(d, "d", self.device), _ptr(H, "H", self.device), ldh, B,
                                         _ptr(out, "out", self.device), _stream_ptr(stream, H.device))
         _check(st, "td_loglike_batch")
+        return out
+
+    def loglike_batch_static(self, d, H, out, stream=None):
+        """td_loglike_batch_static: the same values as loglike_batch, computed without any device allocation - the
+        staged kernels with their workspace in the library's 16 MiB static device array (include/tdlike.h: limits,
+        calls that overlap on the GPU race).  `out` is the caller's: this wrapper allocates nothing either."""
+        if H.dim() != 2 or H.stride(1) != 1:
+            raise ValueError("H must be 2-D with unit stride along samples")
+        B, ldh = int(H.shape[0]), int(H.stride(0)) if H.shape[0] > 1 else max(int(H.stride(0)), int(H.shape[1]))
+        if H.shape[1] < self.n_tot or d.numel() < self.n_tot or not d.is_contiguous() or out.numel() < B:
+            raise ValueError("d / H shorter than N_tot, or out shorter than B")
+        st = self._lib.td_loglike_batch_static(self._h, _ptr(d, "d", self.device), _ptr(H, "H", self.device), ldh, B,
+                                               _ptr(out, "out", self.device), _stream_ptr(stream, H.device))
+        if st != TD_OK:
+            why = self._lib.td_static_last_error().decode()
+            raise TDError(st, "td_loglike_batch_static" + (f" [{why}]" if why else ""))
         return out
 
     def inner_batch(self, d, H, want_dh: bool = True, want_hh: bool = True, stream=None, out_dh=None):

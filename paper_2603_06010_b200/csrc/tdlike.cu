@@ -1350,3 +1350,134 @@ int td_debug_phase_clocks(long long* host, int n) {
 #endif
 
 }  // extern "C"
+
+// ------------------------------------------------------------------------------------------------------------------------
+// td_loglike_batch_static - the log-likelihood through the staged kernels (td_staged.cuh) with their workspace in a file-scope
+// device array instead of the handle's cudaMalloc'ed buffers: for callers that may not allocate (include/tdlike.h).
+// New code only: it shares the kernels and the launch helpers of td_staged_host.cuh with the existing path and none of its
+// buffers.  The array belongs to the library image: every GPU that loads libtdlike.so holds TD_STATIC_SCRATCH_BYTES of it
+// until the process exits.
+// ------------------------------------------------------------------------------------------------------------------------
+#include <mutex>
+
+static __device__ __align__(256) unsigned char td_static_scratch[TD_STATIC_SCRATCH_BYTES];
+
+namespace {
+
+// In host code `td_static_scratch` is only the host-side shadow of the symbol: its DEVICE address comes from
+// cudaGetSymbolAddress, once per device, with that device current.
+void* g_static_dev_ptr[TD_MAX_DEV];
+std::mutex g_static_mu;
+thread_local char g_static_err[256] = "";
+
+td_status static_fail(td_status s, const char* fmt, long long a = 0, long long b = 0, long long c = 0) {
+  std::snprintf(g_static_err, sizeof(g_static_err), fmt, a, b, c);
+  return s;
+}
+
+// the caller holds a DevGuard on `device`
+td_status static_scratch_address(int device, unsigned char** out) {
+  if (device < 0 || device >= TD_MAX_DEV) return static_fail(TD_EUNSUPPORTED, "device index %lld is beyond the %lld this library tracks", device, TD_MAX_DEV);
+  std::lock_guard<std::mutex> lk(g_static_mu);
+  if (!g_static_dev_ptr[device]) {
+    void* p = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress(&p, td_static_scratch);
+    if (e != cudaSuccess || !p) {
+      cudaGetLastError();
+      return static_fail(TD_ECUDA, "cudaGetSymbolAddress(td_static_scratch) failed on device %lld (CUDA error %lld)", device, (long long)e);
+    }
+    g_static_dev_ptr[device] = p;
+  }
+  *out = static_cast<unsigned char*>(g_static_dev_ptr[device]);
+  return TD_OK;
+}
+
+// bytes of scratch one template of a size class needs: U [2][M/2] + Z [2][M] complex, per-block partial sums [nblk][2]
+size_t static_bytes_per_template(int log2M) {
+  const StagedGeom g = staged_geom(log2M);
+  return sizeof(cplx) * 3 * ((size_t)1 << log2M) + sizeof(double) * 2 * (size_t)g.nblk;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t td_static_scratch_bytes(void) { return TD_STATIC_SCRATCH_BYTES; }
+const char* td_static_last_error(void) { return g_static_err; }
+
+td_status td_static_setup(int device) {
+  g_static_err[0] = 0;
+  DevGuard guard(device);
+  if (!guard.ok) return static_fail(TD_ECUDA, "cannot make device %lld current", device);
+  unsigned char* p = nullptr;
+  td_status s = static_scratch_address(device, &p);
+  if (s != TD_OK) return s;
+  // the launch configuration of the two shared-memory block kernels (attribute + occupancy, cached per device)
+  s = launch_block<true>(device, nullptr, 0, 0, nullptr, 0, nullptr, true);
+  if (s == TD_OK) s = launch_block<false>(device, nullptr, 0, 0, nullptr, 0, nullptr, true);
+  if (s != TD_OK) return static_fail(s, "the staged block kernels cannot be configured on device %lld", device);
+  return TD_OK;
+}
+
+td_status td_loglike_batch_static(td_handle* h, const double* d, const double* H, int64_t ldh, int64_t B, double* out,
+                                  void* stream) {
+  g_static_err[0] = 0;
+  if (!h || B < 0) return static_fail(TD_EINVAL, "null handle or negative batch size");
+  if (B == 0) return TD_OK;
+  if (!d || !H || !out || ldh < h->n_tot) return static_fail(TD_EINVAL, "null pointer, or ldh = %lld below N_tot = %lld", ldh, h->n_tot);
+  // every size class must fit at least one template into the array: refuse before anything is launched
+  for (const ClassInfo& cls : h->classes) {
+    const size_t need = static_bytes_per_template(cls.log2M);
+    if (need > TD_STATIC_SCRATCH_BYTES)
+      return static_fail(TD_EUNSUPPORTED, "a segment of up to %lld samples needs %lld bytes of scratch per template; the static array holds %lld "
+                         "(segments of at most 262144 samples)", 1ll << cls.log2M, (long long)need, (long long)TD_STATIC_SCRATCH_BYTES);
+  }
+  DevGuard guard(h->device);
+  if (!guard.ok) return static_fail(TD_ECUDA, "cannot make device %lld current", h->device);
+  unsigned char* base = nullptr;
+  td_status s = static_scratch_address(h->device, &base);   // (a table look-up after td_static_setup / the first call)
+  if (s != TD_OK) return s;
+  cudaStream_t st = (cudaStream_t)stream;
+  h->last_launches = 0;
+  int accumulate = 0;
+  for (const ClassInfo& cls : h->classes) {
+    const int log2M = cls.log2M, M = 1 << log2M, nf = M / 2, TW = 2 * M;
+    const StagedGeom g = staged_geom(log2M);   // only the radices and the block count are used: the chunk size is ours
+    const int64_t CB = std::min<int64_t>({(int64_t)(TD_STATIC_SCRATCH_BYTES / static_bytes_per_template(log2M)), (int64_t)32767, B});
+    // one chunk's layout inside the array: U | Z | partial sums (each region a multiple of 16 bytes, the base 256-aligned)
+    cplx* const U = reinterpret_cast<cplx*>(base);
+    cplx* const Z = U + (size_t)CB * 2 * nf;
+    double* const part = reinterpret_cast<double*>(Z + (size_t)CB * 2 * M);
+    for (size_t i = 0; i < cls.seg_ids.size(); ++i) {
+      const SegHost& sg = h->segs[cls.seg_ids[i]];
+      SegDev sd;
+      sd.off = sg.off; sd.n = sg.n; sd._pad = 0; sd.G = sg.G; sd.zd = sg.zd; sd.rscale = 1.0;
+      for (int64_t b0 = 0; b0 < B; b0 += CB) {
+        const int cb = (int)std::min<int64_t>(CB, B - b0);
+        StagedParams P;
+        P.d = d; P.H = H + b0 * ldh; P.ldh = ldh; P.CB = cb; P.seg = sd;
+        P.M = M; P.U = U; P.Z = Z; P.T = cls.T; P.partial = part; P.nblk = g.nblk;
+        s = launch_first<MODE_LOGLIKE>(g.rF, dim3((nf / g.rF + LG_NT - 1) / LG_NT, cb), P, st);
+        if (s == TD_OK) { ++h->last_launches; s = staged_forward(h->device, U, 2 * cb, nf, 1, cls.T, TW, st, &h->last_launches); }
+        if (s == TD_OK) {
+          lg_untangle_kernel<<<dim3((nf + LG_NT - 1) / LG_NT, 2, (cb + LG_UCPT - 1) / LG_UCPT), LG_NT, 0, st>>>(P);
+          s = cudaGetLastError() == cudaSuccess ? TD_OK : TD_ECUDA;
+          ++h->last_launches;
+        }
+        if (s == TD_OK) s = staged_inverse_but_last(h->device, Z, 2 * cb, M, cls.T, TW, st, &h->last_launches);
+        if (s == TD_OK) { s = launch_last<MODE_LOGLIKE>(g.rI, dim3(g.nblk, cb), P, st); ++h->last_launches; }
+        if (s == TD_OK) {   // the chunk's partial sums, in block order, into out[b0 .. b0 + cb)
+          lg_finish_kernel<<<(unsigned)((cb + 127) / 128), 128, 0, st>>>(part, g.nblk, cb, out + b0, nullptr, -0.5, 1.0, accumulate);
+          s = cudaGetLastError() == cudaSuccess ? TD_OK : TD_ECUDA;
+          ++h->last_launches;
+        }
+        if (s != TD_OK) return static_fail(s, "a kernel launch failed (segment %lld, template %lld)", cls.seg_ids[i], b0);
+      }
+      accumulate = 1;
+    }
+  }
+  h->last_path = TD_PATH_FFT;
+  return TD_OK;
+}
+
+}  // extern "C"
