@@ -39,14 +39,14 @@ FP64_PEAK_TFLOPS = 37.2
 FP32_PEAK_TFLOPS = 74.4
 # dominant kernel of a step, per config
 DOMINANT = {"c1": "td_fused4_kernel<10>", "c2": "td_fused4_kernel<12>", "c3": "td_cluster_kernel",
-            "c4": "td_group16_kernel", "c5": "td_cluster_kernel"}
+            "c4": "td_group_kernel<16>", "c5": "td_cluster_kernel"}
 
 
 def _dominant(config, variant, f32):
     if config == "c4":   # 65536 class: group kernel by default; the staged kernels in fp32 and on request; the cluster kernel on request
         if f32 or variant == 2:
             return "staged lg_* kernels" + (" (fp32 build)" if f32 else "")
-        return "td_cluster16_kernel" if variant == 3 else "td_group16_kernel"
+        return "td_cluster16_kernel" if variant == 3 else "td_group_kernel<16>"
     return DOMINANT.get(config, "td_fused_kernel") + (" (fp32 build)" if f32 else "")
 
 

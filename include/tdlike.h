@@ -161,15 +161,15 @@ td_status td_set_path(td_handle* h, int path);
 
 /* td_set_fft_variant - which implementation serves the FFT path: 0 = automatic (fused
  * shared-memory kernel where a segment's transform fits one SM; 2-CTA cluster kernel for 4097..8192 samples; segments of
- * 32769..65536 samples on the group kernel, td_group16.cuh: one cooperative launch, 16 CTAs per template exchanging the two
- * cross passes through L2, when the device can co-host such a group; staged global-memory kernels
+ * 8193..65536 samples on the group kernel, td_group16.cuh: one cooperative launch, 4 / 8 / 16 CTAs per template exchanging
+ * the two cross passes through L2, when the device can co-host such a group; staged global-memory kernels
  * otherwise; ringdown parameter rows synthesised inside the fused kernel's first pass), 1 = as 0 but
  * td_loglike_family_batch always synthesises into the scratch panel first (the r01 route; tests, profiling),
  * 2 = force the staged kernels for every segment (tests, profiling), 3 = as 0 but segments of 32769..65536 samples run on
  * the 16-CTA cluster kernel (td_cluster16.cuh: the 3 MB of spectra of one template in distributed shared memory; measured
  * slower than the staged kernels on B200, profiles/r02_c4_cluster16.md; TD_EUNSUPPORTED when the handle has no such
- * segment or the device cannot host a 16-CTA cluster), 4 = the explicit name of what 0 does for segments of 32769..65536
- * samples (TD_EUNSUPPORTED when the handle has no such segment or the device cannot co-host a 16-CTA group). */
+ * segment or the device cannot host a 16-CTA cluster), 4 = the explicit name of what 0 does for segments of 8193..65536
+ * samples (TD_EUNSUPPORTED when the handle has no such segment or the device cannot co-host a group). */
 td_status td_set_fft_variant(td_handle* h, int variant);
 
 /* td_precision: arithmetic of the FFT-path evaluation (td_set_precision). */

@@ -50,7 +50,7 @@ struct SegHost {
   double* a = nullptr;  // device [n]
   cplx* G = nullptr;    // device [2][M]
   cplx* Gp = nullptr;   // device [2][padded(M)], padded Z layout (fused4 classes only)
-  cplx* Gc16 = nullptr; // device [16][padded(8192)]: per-CTA generator values of the 16-CTA cluster kernel (M = 65536 only)
+  cplx* Gc16 = nullptr; // device [CS][padded(8192)]: per-CTA generator values of the group kernel (M = 16384 ... 65536, CS = M / 4096) and of the 16-CTA cluster kernel
   cplx* zd = nullptr;   // device [M] (lazy)
 };
 
@@ -86,8 +86,9 @@ struct td_handle {
   int path = TD_PATH_AUTO, fft_variant = 0, last_path = 0, last_launches = 0;
   int precision = TD_PREC_F64;
   bool any_auto_ll = false;   // some size class goes to the dense kernels for the log-likelihood under AUTO
-  int group16_cap = 0;     // co-resident 16-CTA groups of td_group16_kernel (td_group16.cuh)
-  unsigned* g16_bar = nullptr;  // device [G16_MAX_GROUPS][2] arrival counters of that kernel
+  int group_cap[3] = {0, 0, 0};  // groups of 4 / 8 / 16 CTAs of td_group_kernel (td_group16.cuh) that are co-resident AND fit the
+                                 // exchange buffers (0: not asked yet, -1: the class stays on the staged kernels)
+  unsigned* grp_bar = nullptr;   // device [GRP_MAX_GROUPS][2] arrival counters of that kernel
   int cluster16_cap = 0;   // co-resident 16-CTA clusters of td_cluster16_kernel (0: M = 65536 stays on the staged kernels)
   int max_n = 0;
   // staged workspace: U / Z sized by td_create (two lanes of an L2-resident chunk), the per-block partial sums by
@@ -134,7 +135,7 @@ void free_handle(td_handle* h) {
   if (!h) return;
   for (auto& s : h->segs) { cudaFree(s.a); cudaFree(s.G); cudaFree(s.Gp); cudaFree(s.Gc16); cudaFree(s.zd); }
   for (auto& c : h->classes) { cudaFree(c.T); cudaFree(c.d_segs); cudaFree(c.d_Gp); if (c.has32) td32api::free_class(&c.t32); }
-  cudaFree(h->wsU); cudaFree(h->wsZ); cudaFree(h->wsPartial); cudaFree(h->g16_bar); cudaFree(h->wsDot); cudaFree(h->ud); cudaFree(h->synH); cudaFree(h->synP); cudaFree(h->synSeg);
+  cudaFree(h->wsU); cudaFree(h->wsZ); cudaFree(h->wsPartial); cudaFree(h->grp_bar); cudaFree(h->wsDot); cudaFree(h->ud); cudaFree(h->synH); cudaFree(h->synP); cudaFree(h->synSeg);
   cudaFree(h->hsD); cudaFree(h->hsH[0]); cudaFree(h->hsH[1]); cudaFree(h->hsOut);
   cudaFree(h->d_rho);
   for (double* w : h->cdoW) cudaFree(w);
@@ -526,77 +527,81 @@ td_status launch_cluster16(td_handle* h, const Cluster16Params& PC, int* ncluste
   return TD_OK;
 }
 
-// ---- M = 65536 as one persistent kernel of 16-CTA groups exchanging through L2 (td_group16.cuh)
-constexpr int G16_MAX_GROUPS = 16;
-template <int MODE>
-td_status launch_group16(td_handle* h, const Group16Params& PG, int* ngroups, cudaStream_t st, bool dry) {
-  auto kern = td_group16_kernel<MODE>;
+// ---- M = 16384 / 32768 / 65536 as one persistent kernel of 4- / 8- / 16-CTA groups exchanging through L2 (td_group16.cuh)
+constexpr int GRP_MAX_GROUPS = 64;
+inline int group_slot(int cs) { return cs == 4 ? 0 : cs == 8 ? 1 : 2; }
+template <int CS, int MODE>
+td_status launch_group(td_handle* h, const GroupParams& PG, int* ngroups, cudaStream_t st, bool dry) {
+  auto kern = td_group_kernel<CS, MODE>;
   const size_t smem = Cluster16Shape::smem_bytes();
   static int cache[TD_MAX_DEV];
   int per_sm = 0;
   td_status cs = kernel_config(kern, Cluster16Shape::NT, smem, smem, h->device, cache, &per_sm);
   if (cs != TD_OK) return cs;
-  *ngroups = std::min(G16_MAX_GROUPS, per_sm * h->num_sms / Cluster16Shape::CS);
+  *ngroups = std::min(GRP_MAX_GROUPS, per_sm * h->num_sms / CS);
   if (dry || *ngroups < 1) return TD_OK;
+  *ngroups = std::min(*ngroups, h->group_cap[group_slot(CS)]);   // what the exchange buffers hold (group_setup)
   const long long want = MODE == MODE_STOREZ ? 1 : PG.base.B;
   const unsigned groups = (unsigned)std::max<long long>(1, std::min<long long>(want, *ngroups));
-  CK(cudaMemsetAsync(PG.bar, 0, sizeof(unsigned) * 2 * G16_MAX_GROUPS, st));
+  CK(cudaMemsetAsync(PG.bar, 0, sizeof(unsigned) * 2 * GRP_MAX_GROUPS, st));
   cudaLaunchConfig_t cfg = {};
   cudaLaunchAttribute attr[1];
   attr[0].id = cudaLaunchAttributeCooperative;   // every CTA co-resident: the groups synchronise through global counters
   attr[0].val.cooperative = 1;
-  cfg.gridDim = dim3(Cluster16Shape::CS * groups); cfg.blockDim = dim3(Cluster16Shape::NT);
+  cfg.gridDim = dim3(CS * groups); cfg.blockDim = dim3(Cluster16Shape::NT);
   cfg.dynamicSmemBytes = smem; cfg.stream = st; cfg.attrs = attr; cfg.numAttrs = 1;
   CK(cudaLaunchKernelEx(&cfg, kern, PG));
   ++h->last_launches;
   return TD_OK;
 }
-int group16_capacity(td_handle* h) {
-  Group16Params PG = {};
+template <int CS>
+int group_capacity(td_handle* h) {
+  GroupParams PG = {};
   int n = 0, m = 0, z = 0;
-  if (launch_group16<MODE_LOGLIKE>(h, PG, &n, nullptr, true) != TD_OK) return 0;
-  if (launch_group16<MODE_INNER>(h, PG, &m, nullptr, true) != TD_OK) return 0;
-  if (launch_group16<MODE_STOREZ>(h, PG, &z, nullptr, true) != TD_OK) return 0;
+  if (launch_group<CS, MODE_LOGLIKE>(h, PG, &n, nullptr, true) != TD_OK) return 0;
+  if (launch_group<CS, MODE_INNER>(h, PG, &m, nullptr, true) != TD_OK) return 0;
+  if (launch_group<CS, MODE_STOREZ>(h, PG, &z, nullptr, true) != TD_OK) return 0;
   return std::min(n, std::min(m, z));
 }
 // the exchange buffers are the staged workspace (L2-resident by size): groups x 2 parities x (2 NF | 2 M) elements
-bool group16_fits(const td_handle* h, int groups) {
-  return h->g16_bar && h->wsU_elems >= (size_t)groups * 4 * Cluster16Shape::NF && h->wsZ_elems >= (size_t)groups * 4 * Cluster16Shape::M &&
-         h->wsP_elems >= (size_t)Cluster16Shape::CS * 2;
+bool group_fits(const td_handle* h, int cs, int groups) {
+  const size_t M = (size_t)cs * Cluster16Shape::ML;
+  return h->grp_bar && h->wsU_elems >= (size_t)groups * 2 * M && h->wsZ_elems >= (size_t)groups * 4 * M && h->wsP_elems >= (size_t)cs * 2;
 }
 
-// counters + occupancy; leaves group16_cap = -1 (class stays on the staged kernels) when the device cannot host a group
-td_status group16_setup(td_handle* h) {
-  if (!h->g16_bar && cudaMalloc(&h->g16_bar, sizeof(unsigned) * 2 * G16_MAX_GROUPS) != cudaSuccess) { cudaGetLastError(); return TD_ENOMEM; }
+// counters + occupancy; leaves group_cap = -1 (class stays on the staged kernels) when the device cannot host a group
+td_status group_setup(td_handle* h, int cs) {
+  if (!h->grp_bar && cudaMalloc(&h->grp_bar, sizeof(unsigned) * 2 * GRP_MAX_GROUPS) != cudaSuccess) { cudaGetLastError(); return TD_ENOMEM; }
+  int& cap = h->group_cap[group_slot(cs)];
   int coop = 0;
-  if (cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, h->device) != cudaSuccess || !coop) { cudaGetLastError(); h->group16_cap = -1; return TD_OK; }
-  h->group16_cap = group16_capacity(h);
-  while (h->group16_cap > 0 && !group16_fits(h, h->group16_cap)) --h->group16_cap;
-  if (h->group16_cap < 1) h->group16_cap = -1;   // asked and answered
+  if (cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, h->device) != cudaSuccess || !coop) { cudaGetLastError(); cap = -1; return TD_OK; }
+  cap = cs == 4 ? group_capacity<4>(h) : cs == 8 ? group_capacity<8>(h) : group_capacity<16>(h);
+  while (cap > 0 && !group_fits(h, cs, cap)) --cap;
+  if (cap < 1) cap = -1;   // asked and answered
   return TD_OK;
 }
 
-template <int MODE>
-td_status run_group16(td_handle* h, const ClassInfo& cls, int idx_in_class, const double* d, const double* H, int64_t ldh,
-                      int64_t B, double* out0, double* out1, double scale0, double scale1, int accumulate, cudaStream_t st) {
+template <int CS, int MODE>
+td_status run_group(td_handle* h, const ClassInfo& cls, int idx_in_class, const double* d, const double* H, int64_t ldh,
+                    int64_t B, double* out0, double* out1, double scale0, double scale1, int accumulate, cudaStream_t st) {
   const SegHost& sg = h->segs[cls.seg_ids[idx_in_class]];
-  const int64_t SB = std::max<int64_t>(1, (int64_t)(h->wsP_elems / (Cluster16Shape::CS * 2)));   // templates per partial buffer
+  const int64_t SB = std::max<int64_t>(1, (int64_t)(h->wsP_elems / (CS * 2)));   // templates per partial buffer
   h->touched = true;
   const int64_t Bn = (MODE == MODE_STOREZ) ? 1 : B;
   for (int64_t b0 = 0; b0 < Bn; b0 += SB) {
     const int64_t nb = std::min<int64_t>(SB, Bn - b0);
-    Group16Params PG;
+    GroupParams PG;
     PG.base.d = d; PG.base.H = H ? H + b0 * ldh : nullptr; PG.base.ldh = ldh; PG.base.B = nb;
     PG.base.out0 = nullptr; PG.base.out1 = nullptr; PG.base.segs = cls.d_segs + idx_in_class; PG.base.n_seg = 1;
     PG.base.accumulate = 0; PG.base.T = cls.T;
     PG.Gp = sg.Gc16; PG.partial = h->wsPartial;
-    PG.wsU = static_cast<cplx*>(h->wsU); PG.wsZ = static_cast<cplx*>(h->wsZ); PG.bar = h->g16_bar;
+    PG.wsU = static_cast<cplx*>(h->wsU); PG.wsZ = static_cast<cplx*>(h->wsZ); PG.bar = h->grp_bar;
     int ng = 0;
-    td_status s = launch_group16<MODE>(h, PG, &ng, st, false);
+    td_status s = launch_group<CS, MODE>(h, PG, &ng, st, false);
     if (s != TD_OK) return s;
     if (ng < 1) return TD_EUNSUPPORTED;
     if (MODE != MODE_STOREZ) {
-      lg_finish_kernel<<<(unsigned)((nb + 127) / 128), 128, 0, st>>>(h->wsPartial, Cluster16Shape::CS, (int)nb, out0 ? out0 + b0 : nullptr,
+      lg_finish_kernel<<<(unsigned)((nb + 127) / 128), 128, 0, st>>>(h->wsPartial, CS, (int)nb, out0 ? out0 + b0 : nullptr,
                                                                     out1 ? out1 + b0 : nullptr, scale0, scale1, accumulate);
       CK(cudaGetLastError());
       ++h->last_launches;
@@ -678,17 +683,20 @@ td_status run_fft_path(td_handle* h, const double* d, const double* H, int64_t l
       if (s != TD_OK) return s;
       accumulate = 1;
     } else {
-      // M = 65536: the group kernel (16 CTAs per template exchanging through L2, td_group16.cuh) when the device co-hosts a
-      // group, else the staged kernels.  The 16-CTA cluster kernel only on request (variant 3): measured 0.885 ms against 0.737 ms for the staged
+      // M = 16384 / 32768 / 65536: the group kernel (4 / 8 / 16 CTAs per template exchanging through L2, td_group16.cuh) when the
+      // device co-hosts a group, else the staged kernels.  The 16-CTA cluster kernel only on request (variant 3): measured 0.885 ms against 0.737 ms for the staged
       // kernels on c4 - its two all-to-all exchanges run at the 16 B/cycle/SM of distributed-shared-memory stores and only 7
       // clusters (112 of 148 SMs) are co-resident (profiles/r02_c4_cluster16.md)
       const bool c16 = cls.log2M == Cluster16Shape::LOG2M && h->fft_variant == 3 && h->cluster16_cap > 0;
-      const bool g16 = cls.log2M == Cluster16Shape::LOG2M && h->fft_variant != 2 && h->fft_variant != 3 && h->group16_cap > 0;
+      const int gcs = group_cs(cls.log2M);
+      const bool grp = gcs && h->fft_variant != 2 && !c16 && h->group_cap[group_slot(gcs)] > 0;
       for (size_t i = 0; i < cls.seg_ids.size(); ++i) {
         const int id = cls.seg_ids[i];
         td_status s = c16 ? run_cluster16<MODE>(h, cls, (int)i, d, H, ldh, B, out0, out1, sc0, sc1, accumulate, st)
-                      : g16 ? run_group16<MODE>(h, cls, (int)i, d, H, ldh, B, out0, out1, sc0, sc1, accumulate, st)
-                            : run_staged<MODE>(h, cls, h->segs[id], d, H, ldh, B, out0, out1, sc0, sc1, accumulate, st);
+                      : !grp ? run_staged<MODE>(h, cls, h->segs[id], d, H, ldh, B, out0, out1, sc0, sc1, accumulate, st)
+                      : gcs == 4 ? run_group<4, MODE>(h, cls, (int)i, d, H, ldh, B, out0, out1, sc0, sc1, accumulate, st)
+                      : gcs == 8 ? run_group<8, MODE>(h, cls, (int)i, d, H, ldh, B, out0, out1, sc0, sc1, accumulate, st)
+                                 : run_group<16, MODE>(h, cls, (int)i, d, H, ldh, B, out0, out1, sc0, sc1, accumulate, st);
         if (s != TD_OK) return s;
         accumulate = 1;
       }
@@ -928,11 +936,11 @@ static td_status create_impl(td_handle* h, const double* acf, const int64_t* seg
         cudaMemsetAsync(sg.Gp, 0, pb, 0);
         gen_permute_kernel<<<(n2 + 255) / 256, 256>>>(F, sg.Gp, M, gscale, c.log2M == CLUSTER_LOG2M ? 2 : 1);
       }
-      if (c.log2M == Cluster16Shape::LOG2M) {
-        const size_t cb = sizeof(cplx) * 16 * Cluster16Shape::PADZ;
+      if (const int gcs = group_cs(c.log2M)) {   // per-CTA generator values of the group kernel (and, M = 65536, the cluster kernel)
+        const size_t cb = sizeof(cplx) * gcs * Cluster16Shape::PADZ;
         if (cudaMalloc(&sg.Gc16, cb) != cudaSuccess) { st = TD_ENOMEM; break; }
         cudaMemsetAsync(sg.Gc16, 0, cb, 0);
-        gen_permute_c16_kernel<<<(n2 + 255) / 256, 256>>>(F, sg.Gc16, gscale);
+        gen_permute_group_kernel<<<(n2 + 255) / 256, 256>>>(F, sg.Gc16, gscale, gcs);
       }
       if (cudaGetLastError() != cudaSuccess) { st = TD_ECUDA; break; }
     }
@@ -995,11 +1003,11 @@ static td_status create_impl(td_handle* h, const double* acf, const int64_t* seg
     td_status a = staged_alloc(h, false);
     if (a != TD_OK) return a;
   }
-  // the 65536 class runs on the group kernel (td_group16.cuh) when the device can co-host at least one 16-CTA group; its
+  // the 16384 / 32768 / 65536 classes run on the group kernel (td_group16.cuh) when the device can co-host at least one group; its
   // exchange buffers are the staged workspace
   for (const ClassInfo& c : h->classes)
-    if (c.log2M == Cluster16Shape::LOG2M && h->group16_cap == 0) {
-      td_status g = group16_setup(h);
+    if (group_cs(c.log2M) && h->group_cap[group_slot(group_cs(c.log2M))] == 0) {
+      td_status g = group_setup(h, group_cs(c.log2M));
       if (g != TD_OK) return g;
     }
   // ---- one dry pass over every kernel this handle can launch: shared-memory attributes and occupancy are cached now,
@@ -1260,10 +1268,10 @@ td_status td_set_path(td_handle* h, int path) {
 
 td_status td_set_fft_variant(td_handle* h, int variant) {
   if (!h || variant < 0 || variant > 4) return TD_EINVAL;
-  if (variant == 4) {   // 16-CTA groups exchanging through L2: what variant 0 uses for the 65536 class when the device can
-    bool has16 = false;
-    for (const ClassInfo& c : h->classes) has16 = has16 || c.log2M == Cluster16Shape::LOG2M;
-    if (!has16 || h->group16_cap < 1) return TD_EUNSUPPORTED;
+  if (variant == 4) {   // 4- / 8- / 16-CTA groups exchanging through L2: what variant 0 uses for the 16384 ... 65536 classes when it can
+    bool any = false;
+    for (const ClassInfo& c : h->classes) any = any || (group_cs(c.log2M) && h->group_cap[group_slot(group_cs(c.log2M))] > 0);
+    if (!any) return TD_EUNSUPPORTED;
   }
   if (variant == 3) {   // the 16-CTA cluster kernel needs a 65536-class segment and a device that can host the cluster
     bool has16 = false;

@@ -194,6 +194,38 @@ def test_group16_ragged_length_many_items_modes_graph_and_two_handles():
     assert np.max(np.abs(hh[ok] - hh_s[ok])) <= 1e-9 * scale and np.max(np.abs(dh[ok] - dh_s[ok])) <= 1e-9 * scale
 
 
+@pytest.mark.parametrize("lens", [[9001], [16384], [20001], [32768], [9000, 40001, 17000, 3000]])
+def test_group_kernel_sizes_4_8_16_against_staged_and_oracle(lens):
+    """Size classes M = 16384 / 32768 / 65536 run on td_group_kernel<4 / 8 / 16> (td_group16.cuh) by default: against the
+    staged kernels (variant 2) in all three kernel modes, and against the oracle (library Levinson solve, pin P13) on two
+    templates; odd lengths take the scalar-load path; the mixed handle also has a fused-kernel class (3000)."""
+    rng = np.random.default_rng(sum(lens))
+    acf = np.concatenate([W.acf_from_psd(4096.0, 2 * 65536, n) * (1.0 + 0.2 * i) for i, n in enumerate(lens)])
+    nt, B = sum(lens), 43                            # more templates than groups of 16, an uneven remainder for every size
+    d = rng.standard_normal(nt) * 1e-21
+    H = rng.standard_normal((B, nt)) * 1e-21
+    H[11] = d
+    dd, HH = _dev(d), _dev(H)
+    with tdb.TDLikelihood(acf, lens) as h:
+        out = h.loglike_batch(dd, HH).cpu().numpy()
+        nl = h.last_launches()
+        out_again = h.loglike_batch(dd, HH).cpu().numpy()
+        dh, hh = h.inner_batch(dd, HH, want_hh=True)
+        dh, hh = dh.cpu().numpy(), hh.cpu().numpy()
+        h.set_fft_variant(2)
+        ref_st = h.loglike_batch(dd, HH).cpu().numpy()
+        nl_st = h.last_launches()
+        dh_s, hh_s = h.inner_batch(dd, HH, want_hh=True)
+        dh_s, hh_s = dh_s.cpu().numpy(), hh_s.cpu().numpy()
+    assert out[11] == 0.0 and np.array_equal(out, out_again)
+    assert nl == 2 * sum(n > 8192 for n in lens) + (1 if any(n <= 8192 for n in lens) else 0) and nl_st > nl
+    _assert_close(out, ref_st, what=f"group kernel vs staged {lens}")
+    scale = np.max(np.abs(hh_s))
+    assert np.max(np.abs(hh - hh_s)) <= 1e-9 * scale and np.max(np.abs(dh - dh_s)) <= 1e-9 * scale
+    ref = O.loglike_batch_solve_toeplitz(acf, lens, d, H[:2])
+    _assert_close(out[:2], ref, what=f"group kernel vs oracle {lens}")
+
+
 # ------------------------------------------------------------------ shapes: ragged, tiny, mixed classes
 @pytest.mark.parametrize("n", [4097, 6001, 8192])
 def test_cluster_kernel_lengths(n):
@@ -716,6 +748,7 @@ def test_staged_two_lane_pipeline_on_a_side_stream():
     ref = O.loglike_batch_solve_toeplitz(w.acf, w.seg_lengths, w.d, w.H[:2])
     s = torch.cuda.Stream()
     with tdb.TDLikelihood(w.acf, w.seg_lengths) as h:
+        h.set_fft_variant(2)                        # (variant 0 runs this size class on the group kernel, td_group16.cuh)
         Hc = torch.as_tensor(w.H).pin_memory()
         torch.cuda.synchronize()
         with torch.cuda.stream(s):
