@@ -43,10 +43,10 @@ DOMINANT = {"c1": "td_fused4_kernel<10>", "c2": "td_fused4_kernel<12>", "c3": "t
 
 
 def _dominant(config, variant, f32):
-    if config == "c4":   # 65536 class: group kernel by default; the staged kernels in fp32 and on request; the cluster kernel on request
-        if f32 or variant == 2:
+    if config == "c4":   # 65536 class: group kernel by default (both precisions); the staged kernels and the fp64 cluster kernel on request
+        if variant == 2 or (f32 and variant == 3):
             return "staged lg_* kernels" + (" (fp32 build)" if f32 else "")
-        return "td_cluster16_kernel" if variant == 3 else "td_group_kernel<16>"
+        return "td_cluster16_kernel" if variant == 3 else "td_group_kernel<16>" + (" (fp32 build)" if f32 else "")
     return DOMINANT.get(config, "td_fused_kernel") + (" (fp32 build)" if f32 else "")
 
 

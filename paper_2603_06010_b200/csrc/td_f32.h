@@ -23,6 +23,8 @@ struct SegIn {
   const void* Gp64;   // device double2 [2][padded(M)]: the fp64 generator spectrum in the padded Z layout (fused / cluster classes)
   const void* G64;    // device double2 [2][M]: the same spectrum in the plain layout (staged classes)
   double rho0;        // rho_s(0): samples are scaled by rho0^(-1/2) before rounding, the spectrum by rho0^(+1/2)
+  const void* Gc64 = nullptr;   // device double2 [CS][padded(8192)]: per-CTA generator values of the group kernel (td_group16.cuh;
+                                // classes 14..16, CS = M / 4096), or null
 };
 
 // device tables of one size class in fp32 (owned by the handle through this opaque record)
@@ -34,6 +36,7 @@ struct ClassTables {
   void** Gp = nullptr;      // host array [n_seg] of device float2 [2][padded(M)]
   void** zd = nullptr;      // host array [n_seg] of device float2 [M]
   void* host_segs = nullptr;  // staged classes: host copy of the td32::SegDev records
+  void** Gc = nullptr;        // classes 14..16: host array [n_seg] of device float2 [CS][padded(8192)] (group kernel), entries may be null
 };
 
 // what a staged run borrows from the handle (td_staged_host.cuh: StagedCtx)
@@ -44,6 +47,8 @@ struct StagedBorrow {
   cudaStream_t aux_stream = nullptr;
   cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
   int* launches = nullptr;
+  unsigned* grp_bar = nullptr;   // arrival counters of the group kernel (td_group16.cuh)
+  int group_cap = 0;             // groups the exchange buffers (wsU / wsZ) hold; 0: run the staged kernels
 };
 
 // builds the fp32 tables of a class from the fp64 ones (T64: device double2 [2M]); synchronous

@@ -666,6 +666,9 @@ td_status run_fft_path(td_handle* h, const double* d, const double* H, int64_t l
         sb.wsU = h->wsU; sb.wsU_bytes = h->wsU_elems * sizeof(cplx); sb.wsZ = h->wsZ; sb.wsZ_bytes = h->wsZ_elems * sizeof(cplx);
         sb.wsPartial = h->wsPartial; sb.wsP_elems = h->wsP_elems;
         sb.aux_stream = h->aux_stream; sb.ev_fork = h->ev_fork; sb.ev_join = h->ev_join; sb.launches = &h->last_launches;
+        const int gcs = group_cs(cls.log2M);   // the group kernel where the fp64 path would use it (its buffers hold twice the groups in fp32)
+        sb.grp_bar = h->grp_bar;
+        sb.group_cap = (gcs && h->fft_variant != 2) ? std::max(0, h->group_cap[group_slot(gcs)]) : 0;
         L.staged = &sb;
         h->touched = true;
       }
@@ -1305,7 +1308,7 @@ td_status td_set_precision(td_handle* h, int precision) {
       std::vector<td32api::SegIn> in(c.seg_ids.size());
       for (size_t i = 0; i < in.size(); ++i) {
         const SegHost& sg = h->segs[c.seg_ids[i]];
-        in[i].off = sg.off; in[i].n = sg.n; in[i].sid = c.seg_ids[i]; in[i].Gp64 = sg.Gp; in[i].G64 = sg.G; in[i].rho0 = sg.rho0;
+        in[i].off = sg.off; in[i].n = sg.n; in[i].sid = c.seg_ids[i]; in[i].Gp64 = sg.Gp; in[i].G64 = sg.G; in[i].rho0 = sg.rho0; in[i].Gc64 = sg.Gc16;
       }
       td_status s = td32api::build_class(c.log2M, (int)in.size(), in.data(), c.T, &c.t32);
       if (s != TD_OK) return s;

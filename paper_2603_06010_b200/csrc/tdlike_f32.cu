@@ -16,6 +16,7 @@
 #include "td_cluster.cuh"
 #include "td_fused4.cuh"
 #include "td_staged_host.cuh"
+#include "td_group16.cuh"
 
 using namespace td32;
 using namespace tdhost;
@@ -81,6 +82,45 @@ td_status launch_cluster(const td32api::ClassTables& t, const FusedParams& P, in
   return TD_OK;
 }
 
+// ---- the group kernel (td_group16.cuh) in fp32: classes 14..16, one cooperative launch per segment
+constexpr int GRP_MAX_GROUPS = 64;   // as in tdlike.cu: the counters' array holds this many groups
+template <int CS, int MODE>
+td_status launch_group(const GroupParams& PG, int cap, int num_sms, int device, cudaStream_t st, bool dry) {
+  auto kern = td_group_kernel<CS, MODE>;
+  const size_t smem = Cluster16Shape::smem_bytes();
+  static int cache[TD_MAX_DEV];
+  int per_sm = 0;
+  td_status cs = kernel_config(kern, Cluster16Shape::NT, smem, smem, device, cache, &per_sm);
+  if (cs != TD_OK || dry) return cs;
+  const int ng = std::min(std::min(cap, GRP_MAX_GROUPS), per_sm * num_sms / CS);
+  if (ng < 1) return TD_EUNSUPPORTED;
+  const long long want = MODE == MODE_STOREZ ? 1 : PG.base.B;
+  const unsigned groups = (unsigned)std::max<long long>(1, std::min<long long>(want, ng));
+  CK(cudaMemsetAsync(PG.bar, 0, sizeof(unsigned) * 2 * GRP_MAX_GROUPS, st));
+  cudaLaunchConfig_t cfg = {};
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeCooperative;
+  attr[0].val.cooperative = 1;
+  cfg.gridDim = dim3(CS * groups); cfg.blockDim = dim3(Cluster16Shape::NT);
+  cfg.dynamicSmemBytes = smem; cfg.stream = st; cfg.attrs = attr; cfg.numAttrs = 1;
+  CK(cudaLaunchKernelEx(&cfg, kern, PG));
+  return TD_OK;
+}
+template <int CS>
+td_status launch_group_mode(int mode, const GroupParams& PG, int cap, int num_sms, int device, cudaStream_t st, bool dry) {
+  switch (mode) {
+    case MODE_LOGLIKE: return launch_group<CS, MODE_LOGLIKE>(PG, cap, num_sms, device, st, dry);
+    case MODE_INNER: return launch_group<CS, MODE_INNER>(PG, cap, num_sms, device, st, dry);
+    case MODE_STOREZ: return launch_group<CS, MODE_STOREZ>(PG, cap, num_sms, device, st, dry);
+    default: return TD_EINVAL;
+  }
+}
+td_status launch_group_any(int cs, int mode, const GroupParams& PG, int cap, int num_sms, int device, cudaStream_t st, bool dry) {
+  return cs == 4 ? launch_group_mode<4>(mode, PG, cap, num_sms, device, st, dry)
+       : cs == 8 ? launch_group_mode<8>(mode, PG, cap, num_sms, device, st, dry)
+                 : launch_group_mode<16>(mode, PG, cap, num_sms, device, st, dry);
+}
+
 template <int MODE>
 td_status launch_mode(const td32api::ClassTables& t, const FusedParams& P, int num_sms, int device, cudaStream_t st, bool dry) {
   switch (t.log2M) {
@@ -102,8 +142,9 @@ void free_class(ClassTables* t) {
   for (int s = 0; s < t->n_seg; ++s) {
     if (t->Gp) cudaFree(t->Gp[s]);
     if (t->zd) cudaFree(t->zd[s]);
+    if (t->Gc) cudaFree(t->Gc[s]);
   }
-  delete[] t->Gp; delete[] t->zd;
+  delete[] t->Gp; delete[] t->zd; delete[] t->Gc;
   delete[] static_cast<SegDev*>(t->host_segs);
   *t = ClassTables();
 }
@@ -114,7 +155,9 @@ td_status build_class(int log2M, int n_seg, const SegIn* segs, const void* T64, 
   t.log2M = log2M; t.n_seg = n_seg;
   t.Gp = new (std::nothrow) void*[n_seg]();
   t.zd = new (std::nothrow) void*[n_seg]();
-  if (!t.Gp || !t.zd) { free_class(&t); return TD_ENOMEM; }
+  const int gcs = group_cs(log2M);
+  if (gcs) t.Gc = new (std::nothrow) void*[n_seg]();
+  if (!t.Gp || !t.zd || (gcs && !t.Gc)) { free_class(&t); return TD_ENOMEM; }
   const bool staged = staged_class(log2M);
   const size_t M = (size_t)1 << log2M, TW = 2 * M, gp_elems = staged ? 2 * M : 2 * (size_t)SmemArr::padded((int)M);
   auto fail = [&](td_status s) { free_class(&t); return s; };
@@ -130,6 +173,12 @@ td_status build_class(int log2M, int n_seg, const SegIn* segs, const void* T64, 
     if (!src) return fail(TD_EINVAL);
     cvt_cplx_kernel<<<(unsigned)((gp_elems + 255) / 256), 256>>>(static_cast<const double2*>(src), static_cast<float2*>(t.Gp[s]),
                                                                  gp_elems, sqrt(segs[s].rho0));
+    if (gcs && segs[s].Gc64) {
+      const size_t ge = (size_t)gcs * Cluster16Shape::PADZ;
+      if (cudaMalloc(&t.Gc[s], sizeof(float2) * ge) != cudaSuccess) return fail(TD_ENOMEM);
+      cvt_cplx_kernel<<<(unsigned)((ge + 255) / 256), 256>>>(static_cast<const double2*>(segs[s].Gc64), static_cast<float2*>(t.Gc[s]), ge,
+                                                            sqrt(segs[s].rho0));
+    }
     sd[s].off = segs[s].off; sd[s].n = segs[s].n; sd[s]._pad = segs[s].sid; sd[s].G = staged ? static_cast<const cplx*>(t.Gp[s]) : nullptr;
     sd[s].zd = static_cast<cplx*>(t.zd[s]); sd[s].rscale = 1.0 / sqrt(segs[s].rho0);
     gp[s] = static_cast<const cplx*>(t.Gp[s]);
@@ -162,8 +211,45 @@ td_status launch(const ClassTables& t, const Launch& L, int num_sms, int device,
   P.segs = static_cast<const SegDev*>(t.segs); P.n_seg = t.n_seg; P.accumulate = L.accumulate;
   P.T = static_cast<const cplx*>(t.T);
   if (staged_class(t.log2M)) {
-    if (dry) return TD_OK;
+    const int gcs = t.Gc ? group_cs(t.log2M) : 0;
+    if (dry) {   // configure the group kernels of the class (attribute, occupancy cache)
+      GroupParams PG = {};
+      for (int m = 0; gcs && m < 3; ++m) {
+        td_status r = launch_group_any(gcs, m, PG, 0, num_sms, device, st, true);
+        if (r != TD_OK) return r;
+      }
+      return TD_OK;
+    }
     if (!L.staged || !t.host_segs) return TD_EINVAL;
+    if (gcs && L.staged->group_cap > 0 && L.staged->grp_bar) {   // one cooperative launch + the sum of the per-CTA partials per segment
+      bool all = true;
+      for (int s = 0; s < t.n_seg; ++s) all = all && t.Gc[s];
+      const long long SB = std::max<long long>(1, (long long)(L.staged->wsP_elems / ((size_t)gcs * 2)));
+      const double sc0 = L.mode == MODE_LOGLIKE ? -0.5 : 1.0;
+      int accumulate = L.accumulate;
+      for (int s = 0; all && s < t.n_seg; ++s) {
+        const long long Bn = L.mode == MODE_STOREZ ? 1 : L.B;
+        for (long long b0 = 0; b0 < Bn; b0 += SB) {
+          const long long nb = std::min<long long>(SB, Bn - b0);
+          GroupParams PG;
+          PG.base = P; PG.base.H = L.H ? L.H + b0 * L.ldh : nullptr; PG.base.B = nb; PG.base.out0 = nullptr; PG.base.out1 = nullptr;
+          PG.base.segs = static_cast<const SegDev*>(t.segs) + s; PG.base.n_seg = 1; PG.base.accumulate = 0;
+          PG.Gp = static_cast<const cplx*>(t.Gc[s]); PG.partial = L.staged->wsPartial;
+          PG.wsU = static_cast<cplx*>(L.staged->wsU); PG.wsZ = static_cast<cplx*>(L.staged->wsZ); PG.bar = L.staged->grp_bar;
+          td_status r = launch_group_any(gcs, L.mode, PG, L.staged->group_cap, num_sms, device, st, false);
+          if (r != TD_OK) return r;
+          ++*L.staged->launches;
+          if (L.mode != MODE_STOREZ) {
+            lg_finish_kernel<<<(unsigned)((nb + 127) / 128), 128, 0, st>>>(L.staged->wsPartial, gcs, (int)nb, L.out0 ? L.out0 + b0 : nullptr,
+                                                                          L.out1 ? L.out1 + b0 : nullptr, sc0, 1.0, accumulate);
+            CK(cudaGetLastError());
+            ++*L.staged->launches;
+          }
+        }
+        accumulate = 1;
+      }
+      if (all) return TD_OK;
+    }
     StagedCtx C;
     C.device = device;
     C.wsU = L.staged->wsU; C.wsU_bytes = L.staged->wsU_bytes; C.wsZ = L.staged->wsZ; C.wsZ_bytes = L.staged->wsZ_bytes;

@@ -1118,10 +1118,12 @@ def test_fp32_and_parameter_calls_capture_into_a_cuda_graph():
     _assert_close(e_big.cpu().numpy()[:50], ref, tol=TOL32, what="fp32 params")
 
 
-def test_f32_long_segments_on_the_staged_kernels():
-    """Segments of 16384+ samples run the fp32 build of the staged kernels (the paper's own FP32 example is N = 16384,
-    PAPER.md:268): a sample of rows against the fp64 oracle (library Levinson solve), every row against the fp64 GPU result,
-    cross terms, and the full c4 size against the fp64 path."""
+@pytest.mark.parametrize("variant", [0, 2])
+def test_f32_long_segments_on_the_group_and_staged_kernels(variant):
+    """Segments of 8193+ samples run the fp32 build of the group kernel (variant 0; classes up to 65536) or of the staged
+    kernels (variant 2, and every longer class) - the paper's own FP32 example is N = 16384: a sample of rows
+    against the fp64 oracle (library Levinson solve), every row against the fp64 GPU result, cross terms, and the full c4
+    size against the fp64 path."""
     w = W.make("c4", B=40, n_scale=4)
     ref = O.loglike_batch_solve_toeplitz(w.acf, w.seg_lengths, w.d, w.H[:4])
     with tdb.TDLikelihood(w.acf, w.seg_lengths) as h:
@@ -1129,7 +1131,9 @@ def test_f32_long_segments_on_the_staged_kernels():
         o64 = h.loglike_batch(d, H).cpu().numpy()
         dh64, hh64 = h.inner_batch(d, H)
         h.set_precision(tdb.TD_PREC_F32)
+        h.set_fft_variant(variant)
         o32 = h.loglike_batch(d, H).cpu().numpy()
+        assert (h.last_launches() == 2) == (variant == 0)
         dh32, hh32 = h.inner_batch(d, H)
         torch.cuda.synchronize()
     _assert_close(o32[:4], ref, tol=TOL32, what="c4/4 fp32 vs oracle")
@@ -1142,9 +1146,32 @@ def test_f32_long_segments_on_the_staged_kernels():
         d, H = _dev(w.d), _dev(w.H)
         o64 = h.loglike_batch(d, H).cpu().numpy()
         h.set_precision(tdb.TD_PREC_F32)
+        h.set_fft_variant(variant)
         o32 = h.loglike_batch(d, H).cpu().numpy()
     err = np.abs(o32 - o64) / np.maximum(np.abs(o64), 1.0)
     assert 1e-12 < err.max() <= TOL32, f"c4 full size: {err.max():.2e}"
+
+
+def test_f32_group_kernel_ragged_mixed_sizes_and_exact_zero():
+    """fp32 group kernel: odd lengths (scalar loads), group sizes 4 / 8 / 16 and a fused-kernel class in one handle, more
+    templates than groups; h = d gives exactly 0; against the fp64 oracle on two rows and the fp64 GPU path on all."""
+    lens = [9001, 40001, 20000, 3000]
+    rng = np.random.default_rng(3232)
+    acf = np.concatenate([W.acf_from_psd(4096.0, 2 * 65536, n) * (1.0 + 0.2 * i) for i, n in enumerate(lens)])
+    nt, B = sum(lens), 43
+    d = rng.standard_normal(nt) * 1e-21
+    H = rng.standard_normal((B, nt)) * 1e-21
+    H[11] = d
+    dd, HH = _dev(d), _dev(H)
+    with tdb.TDLikelihood(acf, lens) as h:
+        o64 = h.loglike_batch(dd, HH).cpu().numpy()
+        h.set_precision(tdb.TD_PREC_F32)
+        o32 = h.loglike_batch(dd, HH).cpu().numpy()
+        assert h.last_launches() == 7                       # 3 x (group kernel + partial sums) + one fused kernel
+        o32b = h.loglike_batch(dd, HH).cpu().numpy()
+    assert o32[11] == 0.0 and np.array_equal(o32, o32b)
+    _assert_close(o32, o64, tol=TOL32, what="fp32 group kernel vs fp64 path")
+    _assert_close(o32[:2], O.loglike_batch_solve_toeplitz(acf, lens, d, H[:2]), tol=TOL32, what="fp32 group kernel vs oracle")
 
 
 def test_f32_mixed_staged_fused_and_dense_classes():
