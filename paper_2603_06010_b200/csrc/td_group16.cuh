@@ -20,7 +20,7 @@
 //
 // The staged kernels (td_staged.cuh) move ~12 MB per template through L2 at M = 65536 in 5 kernels per chunk; this kernel moves
 // 6.5 MB in one launch per segment, with generator values, data samples and twiddles in tensor memory.
-// The launch is cooperative (all CTAs co-resident, or the launch fails); a wait that does not end within ~2 s traps.
+// The launch is cooperative (all CTAs co-resident, or the launch fails); a wait that does not end within ~10 s traps.
 #pragma once
 #include "td_cluster16.cuh"
 
@@ -116,7 +116,7 @@ __device__ __forceinline__ void grp_wait(const unsigned* ctr, unsigned target) {
     asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(ctr) : "memory");
     if (v >= target) return;
     __nanosleep(32);
-    if (clock64() - t0 > 4000000000ll) __trap();   // a partner that never arrives must not hang the device
+    if (clock64() - t0 > 20000000000ll) __trap();   // (~10 s) a partner that never arrives must not hang the device
   }
 }
 
