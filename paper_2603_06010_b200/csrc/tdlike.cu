@@ -550,7 +550,13 @@ td_status launch_group(td_handle* h, const GroupParams& PG, int* ngroups, cudaSt
   attr[0].val.cooperative = 1;
   cfg.gridDim = dim3(CS * groups); cfg.blockDim = dim3(Cluster16Shape::NT);
   cfg.dynamicSmemBytes = smem; cfg.stream = st; cfg.attrs = attr; cfg.numAttrs = 1;
-  CK(cudaLaunchKernelEx(&cfg, kern, PG));
+  const cudaError_t le = cudaLaunchKernelEx(&cfg, kern, PG);
+  if (le == cudaErrorCooperativeLaunchTooLarge) {   // the device is shared (MPS, a partition): fewer CTAs fit than the occupancy
+    cudaGetLastError();                             // query promised - the class goes back to the staged kernels for good
+    h->group_cap[group_slot(CS)] = -1;
+    return TD_EUNSUPPORTED;
+  }
+  CK(le);
   ++h->last_launches;
   return TD_OK;
 }
@@ -700,6 +706,8 @@ td_status run_fft_path(td_handle* h, const double* d, const double* H, int64_t l
                       : gcs == 4 ? run_group<4, MODE>(h, cls, (int)i, d, H, ldh, B, out0, out1, sc0, sc1, accumulate, st)
                       : gcs == 8 ? run_group<8, MODE>(h, cls, (int)i, d, H, ldh, B, out0, out1, sc0, sc1, accumulate, st)
                                  : run_group<16, MODE>(h, cls, (int)i, d, H, ldh, B, out0, out1, sc0, sc1, accumulate, st);
+        if (s == TD_EUNSUPPORTED && grp && h->group_cap[group_slot(gcs)] < 0)   // the cooperative launch was refused: nothing ran
+          s = run_staged<MODE>(h, cls, h->segs[id], d, H, ldh, B, out0, out1, sc0, sc1, accumulate, st);
         if (s != TD_OK) return s;
         accumulate = 1;
       }

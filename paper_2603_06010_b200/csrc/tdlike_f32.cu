@@ -103,7 +103,9 @@ td_status launch_group(const GroupParams& PG, int cap, int num_sms, int device, 
   attr[0].val.cooperative = 1;
   cfg.gridDim = dim3(CS * groups); cfg.blockDim = dim3(Cluster16Shape::NT);
   cfg.dynamicSmemBytes = smem; cfg.stream = st; cfg.attrs = attr; cfg.numAttrs = 1;
-  CK(cudaLaunchKernelEx(&cfg, kern, PG));
+  const cudaError_t le = cudaLaunchKernelEx(&cfg, kern, PG);
+  if (le == cudaErrorCooperativeLaunchTooLarge) { cudaGetLastError(); return TD_EUNSUPPORTED; }   // the caller falls back to the staged kernels
+  CK(le);
   return TD_OK;
 }
 template <int CS>
@@ -237,6 +239,7 @@ td_status launch(const ClassTables& t, const Launch& L, int num_sms, int device,
           PG.Gp = static_cast<const cplx*>(t.Gc[s]); PG.partial = L.staged->wsPartial;
           PG.wsU = static_cast<cplx*>(L.staged->wsU); PG.wsZ = static_cast<cplx*>(L.staged->wsZ); PG.bar = L.staged->grp_bar;
           td_status r = launch_group_any(gcs, L.mode, PG, L.staged->group_cap, num_sms, device, st, false);
+          if (r == TD_EUNSUPPORTED && s == 0 && b0 == 0) { all = false; break; }   // refused before anything ran: staged kernels below
           if (r != TD_OK) return r;
           ++*L.staged->launches;
           if (L.mode != MODE_STOREZ) {
