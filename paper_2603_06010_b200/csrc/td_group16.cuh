@@ -183,8 +183,8 @@ __global__ void __launch_bounds__(Cluster16Shape::NT, 1) td_group_kernel(const G
   unsigned it = 0;   // items this group has started
   // S5 of the previous item: this CTA's 4096 / CS output columns from the 2 CS sub-transforms in Z[parity of that item]
   auto reduce_prev = [&](const cplx* __restrict__ Zb, unsigned target) {
-    if (tid == 0) grp_wait(bar_z, target);
-    __syncthreads();
+    if (lane == 0) grp_wait(bar_z, target);   // every warp polls for itself: no CTA barrier behind the wait
+    __syncwarp();
     double acc0 = 0.0, acc1 = 0.0;
     if constexpr (CS == 16) {
       const int jr = jL(0);
@@ -298,11 +298,11 @@ __global__ void __launch_bounds__(Cluster16Shape::NT, 1) td_group_kernel(const G
       });
     }
     __syncthreads();
-    if (tid == 0) grp_arrive(bar_u);
+    if (tid == 32) grp_arrive(bar_u);   // (not the thread that polls next: its fence would delay the poll)
     // S5 of the previous item while the partners finish their first pass
     if (prev_b >= 0) reduce_prev(Zg + (size_t)((it & 1) ^ 1) * (2 * M), (unsigned)CS * it);
-    if (tid == 0) grp_wait(bar_u, (unsigned)CS * (it + 1));
-    __syncthreads();
+    if (lane == 0) grp_wait(bar_u, (unsigned)CS * (it + 1));
+    __syncwarp();
     // ---------------- first local forward pass (radix 8, L = 2048) of A and B: inputs from the exchange buffer
     {
       const cplx* __restrict__ sa = Ub + (size_t)brG * NF + (size_t)tsubA * NFL + tid;
@@ -340,7 +340,7 @@ __global__ void __launch_bounds__(Cluster16Shape::NT, 1) td_group_kernel(const G
       static_for<0, 16>([&](auto t) { __stcg(dst + 256 * decltype(t)::value, x[brevR<16>(decltype(t)::value)]); });
     }
     __syncthreads();   // also: every warp is past mid and the last pass, U and Z (shared) are free for the next item
-    if (tid == 0) grp_arrive(bar_z);
+    if (tid == 32) grp_arrive(bar_z);
     prev_b = b;
   }
   if (prev_b >= 0) reduce_prev(Zg + (size_t)((it & 1) ^ 1) * (2 * M), (unsigned)CS * it);
