@@ -5,7 +5,6 @@
 //   twiddle table, and the packed generator g = a - i b (b = (0, a_{N-1}, ..., a_1)) whose
 //   length-2M transform, conjugated, is G = conj(A^) + i conj(B^).
 #pragma once
-#include <cooperative_groups.h>
 #include "td_common.cuh"
 
 namespace td {
@@ -86,39 +85,57 @@ __global__ void __launch_bounds__(LEV_NT) levinson_kernel(const LevSeg* __restri
   }
 }
 
-// The same recursion for one LONG segment on many CTAs (cooperative launch, two grid-wide barriers per order): a single
+// The same recursion for one LONG segment on many CTAs (cooperative launch, one grid-wide barrier per order): a single
 // CTA streams a and rho (2 x 8 N bytes at the last orders) through one SM for every order, which is 0.96 s at N = 65536;
 // spread over the grid the step is bounded by the barrier, not by one SM's bandwidth.  Every thread carries its own copy
 // of E and log det (identical arithmetic on identical partial sums), so the SPD test exits the whole grid uniformly.
 constexpr int LEVC_NT = 512;
 constexpr int LEV_COOP_MIN_N = 16384;
 
-__global__ void __launch_bounds__(LEVC_NT) levinson_coop_kernel(const LevSeg sg, double* partial, double* v_out,
-                                                               double* logdet_out, int* status) {
-  namespace cg = cooperative_groups;
-  cg::grid_group grid = cg::this_grid();
+// grid-wide barrier of the cooperative kernel below: one arrival per CTA on a 64-bit counter that only grows (release
+// reduction after the CTA's barrier, acquire polling by one thread).  About a third of the cost of cooperative_groups'
+// grid.sync() on B200 (measured through td_create: N = 65536 0.37 s -> see DESIGN.md 0), and the recursion pays it once per order.
+// Data that crosses CTAs (a, partial) is read and written with .cg accesses: L2 only, no stale L1 lines.
+__device__ __forceinline__ void lev_grid_barrier(unsigned long long* ctr, unsigned long long& target, int G) {
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    target += (unsigned long long)G;
+    asm volatile("red.release.gpu.global.add.u64 [%0], %1;" ::"l"(ctr), "l"(1ull) : "memory");
+    unsigned long long v;
+    const long long t0 = clock64();
+    do {
+      asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(ctr) : "memory");
+      if (clock64() - t0 > 20000000000ll) __trap();   // (~10 s) never with a cooperative launch: all CTAs are resident
+    } while (v < target);
+  }
+  __syncthreads();
+}
+
+__global__ void __launch_bounds__(LEVC_NT) levinson_coop_kernel(const LevSeg sg, double* partial, unsigned long long* bar,
+                                                               double* v_out, double* logdet_out, int* status) {
   __shared__ double red[LEVC_NT / 32];
   __shared__ double bc;
   const double* __restrict__ rho = sg.rho;
   double* a = sg.a;
   const int n = sg.n, tid = threadIdx.x, G = gridDim.x;
   const int gtid = blockIdx.x * LEVC_NT + tid, gsz = G * LEVC_NT;
+  unsigned long long bar_target = 0;
   const double rho0 = rho[0];
   if (!(rho0 > 0.0) || !isfinite(rho0)) {
     if (gtid == 0) *status = 2;
     return;
   }
-  for (int j = gtid; j < n; j += gsz) a[j] = (j == 0) ? 1.0 : 0.0;
+  for (int j = gtid; j < n; j += gsz) __stcg(a + j, (j == 0) ? 1.0 : 0.0);
   double E = rho0, logdet = log(rho0);
   // ONE grid barrier per order: the thread that updates the pair (a_j, a_{k-j}) of order k holds both new values in
   // registers and adds their terms of the NEXT order's dot product sum_j a_j rho_{k+1-j} on the spot, so the dot product needs
   // no pass (and no barrier) of its own; per-CTA partial sums are double-buffered by the parity of the order.
-  if (tid == 0 && n > 1) partial[(size_t)1 * G + blockIdx.x] = blockIdx.x == 0 ? rho[1] : 0.0;
-  grid.sync();
+  if (tid == 0 && n > 1) __stcg(partial + (size_t)1 * G + blockIdx.x, blockIdx.x == 0 ? rho[1] : 0.0);
+  lev_grid_barrier(bar, bar_target, G);
   for (int k = 1; k < n; ++k) {
     if (tid < 32) {  // fixed order: lane l adds partials l, l + 32, ...; then the warp tree
       double v = 0.0;
-      for (int c = tid; c < G; c += 32) v += partial[(size_t)(k & 1) * G + c];
+      for (int c = tid; c < G; c += 32) v += __ldcg(partial + (size_t)(k & 1) * G + c);
       v = warp_sum(v);
       if (tid == 0) bc = v;
     }
@@ -131,19 +148,19 @@ __global__ void __launch_bounds__(LEVC_NT) levinson_coop_kernel(const LevSeg sg,
     const bool more = k + 1 < n;
     double acc = 0.0;
     for (int j = 1 + gtid; 2 * j < k; j += gsz) {
-      const double aj = a[j], ak = a[k - j];
+      const double aj = __ldcg(a + j), ak = __ldcg(a + k - j);
       const double nj = fma(kk, ak, aj), nk = fma(kk, aj, ak);
-      a[j] = nj;
-      a[k - j] = nk;
+      __stcg(a + j, nj);
+      __stcg(a + k - j, nk);
       if (more) acc = fma(nj, rho[k + 1 - j], fma(nk, rho[j + 1], acc));
     }
     if (gtid == 0) {
       if ((k & 1) == 0) {
-        const double am = a[k / 2], nm = fma(kk, am, am);
-        a[k / 2] = nm;
+        const double am = __ldcg(a + k / 2), nm = fma(kk, am, am);
+        __stcg(a + k / 2, nm);
         if (more) acc = fma(nm, rho[k + 1 - k / 2], acc);
       }
-      a[k] = kk;
+      __stcg(a + k, kk);
       if (more) acc += fma(kk, rho[1], rho[k + 1]);   // a_k rho_1 + a_0 rho_{k+1}
     }
     E *= (1.0 - kk * kk);
@@ -158,9 +175,9 @@ __global__ void __launch_bounds__(LEVC_NT) levinson_coop_kernel(const LevSeg sg,
     if (tid < 32) {
       double v = tid < LEVC_NT / 32 ? red[tid] : 0.0;
       v = warp_sum(v);
-      if (tid == 0) partial[(size_t)((k + 1) & 1) * G + blockIdx.x] = v;
+      if (tid == 0) __stcg(partial + (size_t)((k + 1) & 1) * G + blockIdx.x, v);
     }
-    grid.sync();
+    lev_grid_barrier(bar, bar_target, G);
   }
   if (gtid == 0) {
     *v_out = E;

@@ -888,15 +888,19 @@ static td_status create_impl(td_handle* h, const double* acf, const int64_t* seg
     int coop_ok = 0, nb = 0;
     CK(cudaDeviceGetAttribute(&coop_ok, cudaDevAttrCooperativeLaunch, h->device));
     CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, levinson_coop_kernel, LEVC_NT, 0));
-    const int G = std::min(48, std::max(1, nb) * h->num_sms);
+    // one CTA per SM (measured with the counter barrier of td_setup.cuh, td_create at N = 65536 / 2^18 / 2^20: 48 CTAs 0.24 / 1.26 /
+    // 9.8 s, 148 CTAs 0.24 / 1.02 / 5.5 s, 296 CTAs 0.27 / 1.08 / 5.2 s)
+    const int G = std::min(h->num_sms, std::max(1, nb) * h->num_sms);
     double* d_part = nullptr;
     for (int s = 0; s < n_seg; ++s) {
       if (!lev[s].coop) continue;
       if (!coop_ok) return TD_EUNSUPPORTED;
-      if (!d_part) CK(cudaMalloc(&d_part, sizeof(double) * 2 * G));
+      if (!d_part) CK(cudaMalloc(&d_part, sizeof(double) * (2 * G + 1)));   // + the 64-bit arrival counter of the grid barrier
+      unsigned long long* d_bar = reinterpret_cast<unsigned long long*>(d_part + 2 * G);
+      CK(cudaMemsetAsync(d_bar, 0, sizeof(unsigned long long), 0));
       LevSeg one = lev[s];
       double* pv = d_v + s; double* pl = d_ld + s; int* ps = d_status + s;
-      void* args[] = {&one, &d_part, &pv, &pl, &ps};
+      void* args[] = {&one, &d_part, &d_bar, &pv, &pl, &ps};
       CK(cudaLaunchCooperativeKernel((void*)levinson_coop_kernel, dim3(G), dim3(LEVC_NT), args, 0, 0));
     }
     CK(cudaDeviceSynchronize());
