@@ -147,7 +147,27 @@ __global__ void __launch_bounds__(LEVC_NT) levinson_coop_kernel(const LevSeg sg,
     }
     const bool more = k + 1 < n;
     double acc = 0.0;
-    for (int j = 1 + gtid; 2 * j < k; j += gsz) {
+    // four pairs per trip with all their loads issued first: the pairs of different j are disjoint, which the compiler cannot
+    // know (it would keep every load behind the previous trip's stores), and a thread has only a handful of trips per order
+    int j = 1 + gtid;
+    for (; 2 * (j + 3 * gsz) < k; j += 4 * gsz) {
+      double aj[4], ak[4], r0[4], r1[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const int ju = j + u * gsz;
+        aj[u] = __ldcg(a + ju); ak[u] = __ldcg(a + k - ju);
+        r0[u] = more ? rho[k + 1 - ju] : 0.0; r1[u] = more ? rho[ju + 1] : 0.0;
+      }
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const int ju = j + u * gsz;
+        const double nj = fma(kk, ak[u], aj[u]), nk = fma(kk, aj[u], ak[u]);
+        __stcg(a + ju, nj);
+        __stcg(a + k - ju, nk);
+        acc = fma(nj, r0[u], fma(nk, r1[u], acc));
+      }
+    }
+    for (; 2 * j < k; j += gsz) {
       const double aj = __ldcg(a + j), ak = __ldcg(a + k - j);
       const double nj = fma(kk, ak, aj), nk = fma(kk, aj, ak);
       __stcg(a + j, nj);
