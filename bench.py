@@ -278,14 +278,16 @@ def main():
             h.loglike_batch(d, Hd, out=out)
 
     # ---------------- device-resident throughput
-    for i in range(args.warmup):
-        step(Hs[i % nbuf])
-    torch.cuda.synchronize()
-    barrier()
+    # (the clock sampler starts BEFORE the warm-up steps: its start-up pause used to sit between warm-up and timed region,
+    # and a GPU that has idled for 0.1 s runs its next few steps 1-30 % slower - the warm-up must be what directly precedes
+    # the timed steps)
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
         time.sleep(0.12)
+    barrier()
+    for i in range(args.warmup):
+        step(Hs[i % nbuf])
     evs = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
     launches = 0
     torch.cuda.synchronize()
