@@ -42,11 +42,14 @@ DOMINANT = {"c1": "td_fused4_kernel<10>", "c2": "td_fused4_kernel<12>", "c3": "t
             "c4": "td_group_kernel<16>", "c5": "td_cluster_kernel"}
 
 
-def _dominant(config, variant, f32):
-    if config == "c4":   # 65536 class: group kernel by default (both precisions); the staged kernels and the fp64 cluster kernel on request
-        if variant == 2 or (f32 and variant == 3):
+def _dominant(config, variant, f32, n_scale=1):
+    if config == "c4":   # 16384 ... 65536 classes: group kernel by default (both precisions); staged kernels and the fp64 cluster kernel on request
+        cs = {1: 16, 2: 8, 4: 4}.get(n_scale)
+        if cs is None:
+            return "td_fused4_kernel / td_cluster_kernel (reduced c4)" + (" (fp32 build)" if f32 else "")
+        if variant == 2 or (variant == 3 and (f32 or cs != 16)):
             return "staged lg_* kernels" + (" (fp32 build)" if f32 else "")
-        return "td_cluster16_kernel" if variant == 3 else "td_group_kernel<16>" + (" (fp32 build)" if f32 else "")
+        return "td_cluster16_kernel" if variant == 3 else f"td_group_kernel<{cs}>" + (" (fp32 build)" if f32 else "")
     return DOMINANT.get(config, "td_fused_kernel") + (" (fp32 build)" if f32 else "")
 
 
@@ -186,6 +189,9 @@ def main():
     ap.add_argument("--config", default="c2")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--B", type=int, default=None, help="override templates per GPU (default: the config's B)")
+    ap.add_argument("--n-scale", type=int, default=1,
+                    help="divide every segment length of the config by this (workloads.make: the reduced-size versions the "
+                         "parity tests use; profiling of the size classes between the configs, never the headline)")
     ap.add_argument("--path", type=int, default=0, help="0 auto, 1 FFT, 2 dense (Gohberg-Semencul), 4 CDO (cached L^-1)")
     ap.add_argument("--fft-variant", type=int, default=0)
     ap.add_argument("--op", default="loglike", choices=["loglike", "dh"],
@@ -227,7 +233,7 @@ def main():
                               "derived_fp64_peak": FP64_PEAK_TFLOPS}))
         return
 
-    w = W.make(args.config, B=args.B)
+    w = W.make(args.config, B=args.B, n_scale=args.n_scale)
     B_job, n_tot = w.B, w.n_tot
     lo, hi = 0, B_job
     if world > 1 and args.scaling == "strong":
@@ -403,7 +409,7 @@ def main():
                 # fraction against the DFMA register loop measured in THIS run (state both denominators)
                 "frac_vs_measured_loop": ach_tf / probe["ffma_fp32" if f32 else "dfma"],
                 "traffic": traffic, "traffic_source": traffic_source,
-                "kernel": ("td_cdo_kernel" if cdo else "td_dense_kernel") if dense else _dominant(args.config, args.fft_variant, f32),
+                "kernel": ("td_cdo_kernel" if cdo else "td_dense_kernel") if dense else _dominant(args.config, args.fft_variant, f32, args.n_scale),
                 "measured_register_loop_tflops": probe,
                 "kernel_ms": kern_ms, "alg_flops_per_eval": falg,
                 "peak_source": ("derived: 128 FFMA/clk/SM x 148 SM x 1.965 GHz x 2; the FFMA register loop of this run beside it"
