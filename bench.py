@@ -37,20 +37,25 @@ UNIT = "evals/s"
 FP64_PEAK_TFLOPS = 37.2
 # fp32 evaluation mode (--dtype f32, never the headline): 128 FFMA/clk/SM x 148 SMs x 1.965 GHz x 2 flop
 FP32_PEAK_TFLOPS = 74.4
-# dominant kernel of a step, per config
-DOMINANT = {"c1": "td_fused4_kernel<10>", "c2": "td_fused4_kernel<12>", "c3": "td_cluster_kernel",
-            "c4": "td_group_kernel<16>", "c5": "td_cluster_kernel"}
 
-
-def _dominant(config, variant, f32, n_scale=1):
-    if config == "c4":   # 16384 ... 65536 classes: group kernel by default (both precisions); staged kernels and the fp64 cluster kernel on request
-        cs = {1: 16, 2: 8, 4: 4}.get(n_scale)
-        if cs is None:
-            return "td_fused4_kernel / td_cluster_kernel (reduced c4)" + (" (fp32 build)" if f32 else "")
-        if variant == 2 or (variant == 3 and (f32 or cs != 16)):
-            return "staged lg_* kernels" + (" (fp32 build)" if f32 else "")
-        return "td_cluster16_kernel" if variant == 3 else f"td_group_kernel<{cs}>" + (" (fp32 build)" if f32 else "")
-    return DOMINANT.get(config, "td_fused_kernel") + (" (fp32 build)" if f32 else "")
+def _dominant(seg_lengths, variant, f32):
+    """Name of the FFT-path kernel that serves the longest segment (the dominant kernel of a step)."""
+    n = int(max(seg_lengths))
+    log2m = max(8, int(math.ceil(math.log2(max(n, 1)))))
+    tail = " (fp32 build)" if f32 else ""
+    if variant == 2:
+        return "staged lg_* kernels" + tail
+    if log2m <= 9:
+        return f"td_fused_kernel<{log2m}>"
+    if log2m <= 12:
+        return f"td_fused4_kernel<{log2m}>" + tail
+    if log2m == 13:
+        return "td_cluster_kernel" + tail
+    if log2m <= 16:
+        if variant == 3 and log2m == 16 and not f32:
+            return "td_cluster16_kernel"
+        return f"td_group_kernel<{1 << (log2m - 12)}>" + tail
+    return "staged lg_* kernels" + tail
 
 
 def alg_flops_per_eval(seg_lengths) -> float:
@@ -409,7 +414,7 @@ def main():
                 # fraction against the DFMA register loop measured in THIS run (state both denominators)
                 "frac_vs_measured_loop": ach_tf / probe["ffma_fp32" if f32 else "dfma"],
                 "traffic": traffic, "traffic_source": traffic_source,
-                "kernel": ("td_cdo_kernel" if cdo else "td_dense_kernel") if dense else _dominant(args.config, args.fft_variant, f32, args.n_scale),
+                "kernel": ("td_cdo_kernel" if cdo else "td_dense_kernel") if dense else _dominant(w.seg_lengths, args.fft_variant, f32),
                 "measured_register_loop_tflops": probe,
                 "kernel_ms": kern_ms, "alg_flops_per_eval": falg,
                 "peak_source": ("derived: 128 FFMA/clk/SM x 148 SM x 1.965 GHz x 2; the FFMA register loop of this run beside it"

@@ -177,7 +177,14 @@ def make(name: str, B: Optional[int] = None, n_scale: int = 1) -> Workload:
     same structure for tests the oracle must finish in seconds.
     """
     name = name.lower()
-    seed, B0 = _SPECS[name]
+    dn = 0
+    if name.startswith("d:"):   # "d:<N>": the d-type workload (one ringdown-only segment) at any length N, B = 2^24 / N
+        dn = int(name[2:])
+        if not 1 <= dn <= 4096:
+            raise KeyError(name)
+        seed, B0 = 260306100 + dn, max(1, (1 << 24) // dn)
+    else:
+        seed, B0 = _SPECS[name]
     B = int(B0 if B is None else B)
     rng = np.random.default_rng(seed)
     U = rng.uniform
@@ -285,10 +292,10 @@ def make(name: str, B: Optional[int] = None, n_scale: int = 1) -> Workload:
         return Workload(name, seed, fs, np.array([N] * 3, np.int64), acf, noise + H[0], H, scales,
                         "3 detectors x N, projected damped sinusoids, network SNR", params)
 
-    if name in ("d1", "d2", "d3", "d4", "d5"):
+    if name in ("d1", "d2", "d3", "d4", "d5") or dn:
         fs = 4096.0
-        N = {"d1": 64, "d2": 128, "d3": 256, "d4": 512, "d5": 1024}[name]
-        M = 2 * 4096                      # ACF taken from the 1 s grid, truncated (Eq. 11)
+        N = dn if dn else {"d1": 64, "d2": 128, "d3": 256, "d4": 512, "d5": 1024}[name]
+        M = 2 * max(4096, 1 << int(np.ceil(np.log2(N))))   # ACF taken from the 1 s grid (longer for N > 4096), truncated (Eq. 11)
         rho = acf_from_psd(fs, M, N)
         n = _noise(rng, fs, M, N)
         f, tau, phi, snr = U(150, 400, B), U(2e-3, 10e-3, B), U(0, 2 * np.pi, B), U(8, 30, B)
