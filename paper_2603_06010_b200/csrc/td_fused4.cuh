@@ -53,6 +53,12 @@ template <int LOG2M> struct Fused4Shape {
   static constexpr int TMEM_COLS = tmem_cols(1);
   // bytes of one item pipeline (NGRP > 1: several independent pipelines share a CTA, see the kernel), 16-byte granular
   static constexpr size_t group_bytes() { return (smem_bytes() + 15) & ~(size_t)15; }
+  // layout of a CTA with NGRP pipelines: [U, Z of every pipeline] [ONE base-twiddle table] [sums, mbarriers, segment cache of
+  // every pipeline]; with one pipeline this is the layout smem_bytes() describes
+  static constexpr size_t uz_bytes() { return sizeof(cplx) * (2 * (size_t)PADNF + 2 * (size_t)PADM); }
+  static constexpr size_t tw_bytes() { return sizeof(cplx) * (size_t)TWS; }
+  static constexpr size_t tail_bytes() { return group_bytes() - uz_bytes() - tw_bytes(); }
+  static constexpr size_t total_bytes(int ngrp) { return ngrp * (uz_bytes() + tail_bytes()) + tw_bytes(); }
   static constexpr size_t smem_bytes() {
     return sizeof(cplx) * (2 * (size_t)PADNF + 2 * (size_t)PADM + TWS) + sizeof(double) * 4 * NW + 48 + F4_SEGCACHE * sizeof(SegDev) +
            96   // RingConsts of the item in flight (SYN kernels)
@@ -304,14 +310,15 @@ __global__ void __launch_bounds__(Fused4Shape<LOG2M>::NT * NGRP, 1) td_fused4_ke
     if constexpr (NGRP == 1) __syncthreads();
     else asm volatile("bar.sync %0, %1;" ::"r"(1 + grp), "r"(NT) : "memory");
   };
-  cplx* sm = reinterpret_cast<cplx*>(smem_raw + (size_t)grp * Sh::group_bytes());
+  cplx* sm = reinterpret_cast<cplx*>(smem_raw + (size_t)grp * Sh::uz_bytes());
   const SmemArr UE{sm}, UO{sm + Sh::PADNF};
   const SmemArr ZE{sm + 2 * Sh::PADNF}, ZO{sm + 2 * Sh::PADNF + Sh::PADM};
-  cplx* tw = sm + 2 * Sh::PADNF + 2 * Sh::PADM;
-  double* red = reinterpret_cast<double*>(tw + Sh::TWS);  // [2][2 NW]: per-warp partial sums, double-buffered by item parity
+  cplx* tw = reinterpret_cast<cplx*>(smem_raw + (size_t)NGRP * Sh::uz_bytes());   // ONE base-twiddle table for all pipelines
+  unsigned char* tail0 = smem_raw + (size_t)NGRP * Sh::uz_bytes() + Sh::tw_bytes();
+  double* red = reinterpret_cast<double*>(tail0 + (size_t)grp * Sh::tail_bytes());  // [2][2 NW]: per-warp partial sums, double-buffered by item parity
   const uint32_t mbar_rows = smem_u32(red + 4 * NW);
   // (one allocation for the CTA: every group reads group 0's slot)
-  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(reinterpret_cast<double*>(reinterpret_cast<cplx*>(smem_raw) + 2 * Sh::PADNF + 2 * Sh::PADM + Sh::TWS) + 4 * NW + 1);
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(reinterpret_cast<double*>(tail0) + 4 * NW + 1);
   SegDev* segS = reinterpret_cast<SegDev*>(red + 4 * NW + 3);
   const SegDev* segs = P.n_seg <= F4_SEGCACHE ? segS : P.segs;
   RingConsts* rcs = reinterpret_cast<RingConsts*>(segS + F4_SEGCACHE);
@@ -324,13 +331,15 @@ __global__ void __launch_bounds__(Fused4Shape<LOG2M>::NT * NGRP, 1) td_fused4_ke
 
   // the base-twiddle table arrives by one bulk copy (it was NT-strided global loads: the longest piece of the prologue, which is
   // most of a launch when a CTA has a single item, as on c1)
-  const uint32_t mbar_tw = mbar_rows + 16;
+  const uint32_t mbar_tw = smem_u32(reinterpret_cast<double*>(tail0) + 4 * NW) + 16;   // pipeline 0's: it fetches the table for all
   if (tid < P.n_seg && tid < F4_SEGCACHE) segS[tid] = P.segs[tid];
   if (tid == 0) {
     mbar_init(mbar_rows, 1);
-    mbar_init(mbar_tw, 1);
-    mbar_expect_tx(mbar_tw, (uint32_t)(Sh::TWS * sizeof(cplx)));
-    bulk_g2s(smem_u32(tw), P.T, (uint32_t)(Sh::TWS * sizeof(cplx)), mbar_tw);
+    if (grp == 0) {
+      mbar_init(mbar_tw, 1);
+      mbar_expect_tx(mbar_tw, (uint32_t)(Sh::TWS * sizeof(cplx)));
+      bulk_g2s(smem_u32(tw), P.T, (uint32_t)(Sh::TWS * sizeof(cplx)), mbar_tw);
+    }
   }
   if (cwarp == 0) tmem_alloc<TMEM_COLS>(smem_u32(tmem_slot));
 #ifdef TD_PHASE_CLOCKS

@@ -35,8 +35,9 @@ constexpr int FUSED_MIN_LOG2M = 8;   // M = 256
 constexpr int CLUSTER_LOG2M = 13;    // M = 8192: 2-CTA cluster, one branch per CTA (td_cluster.cuh)
 constexpr int FUSED_NT = 256;
 constexpr int DENSE_AUTO_N = 512;     // AUTO: dense paths for segments up to this length (measured crossover: profiles/r01_chooser.md)
-constexpr int CDO_AUTO_MAX_N = 768;   // AUTO, log-likelihood: size classes whose segments are all at most this long take the CDO kernel
-                                      // (measured against the FFT kernels, profiles/r02_cdo.md: 42 vs 31 M evals/s at 768, 30 vs 31 at 832)
+constexpr int CDO_AUTO_MAX_N = 512;   // AUTO, log-likelihood: size classes whose segments are all at most this long take the CDO kernel
+                                      // (profiles/r02_cdo.md: 768 while the M = 1024 FFT kernel ran one 64-thread pipeline per SM - 31 M evals/s
+                                      // against 41 for CDO at N = 768; with four pipelines it does 80 M and wins from 513 samples up)
 constexpr int CDO_AUTO_MIN_N = 65;    // AUTO, log-likelihood: cached-L^-1 contraction from this length up, the Gohberg-Semencul
                                       // dense kernel below (measured: profiles/r02_cdo.md; 0.95x at N = 64, 1.08-1.55x above)
 
@@ -221,20 +222,26 @@ td_status launch_fused_nt(td_handle* h, const FusedParams& P, cudaStream_t st, b
 }
 
 // SYN = 1: P.H holds parameter rows (ldh = 5 n_seg), the rows are synthesised in the first pass (td_ring.cuh)
+// Item pipelines per CTA (NGRP of td_fused4.cuh).  A kernel that allocates tensor memory gets ONE resident CTA per SM, and the CTA
+// of the M = 1024 shape has 64 threads, that of M = 2048 has 128: four / two pipelines (independent items, one shared base-twiddle
+// table; 222 KB / 221 KB of shared memory) put eight warps on the SM in every shape.  M = 4096 (256 threads, 204 KB) holds one.
+constexpr int f64_ngrp(int log2M) { return log2M == 10 ? 4 : log2M == 11 ? 2 : 1; }
 template <int LOG2M, int MODE, int SYN = 0>
 td_status launch_fused4(td_handle* h, const FusedParams& P, const cplx* const* Gp, cudaStream_t st, bool dry, double fs = 0.0) {
-  auto kern = td_fused4_kernel<LOG2M, MODE, 1, SYN>;
-  constexpr int NT = Fused4Shape<LOG2M>::NT;
-  const size_t smem = Fused4Shape<LOG2M>::smem_bytes();
+  constexpr int NGRP = f64_ngrp(LOG2M);
+  auto kern = td_fused4_kernel<LOG2M, MODE, NGRP, SYN>;
+  constexpr int NT = Fused4Shape<LOG2M>::NT * NGRP;
+  const size_t smem = Fused4Shape<LOG2M>::total_bytes(NGRP);
   static int cache[TD_MAX_DEV];
   int nb = 0;
   td_status cs = kernel_config(kern, NT, smem, smem, h->device, cache, &nb);
   if (cs != TD_OK) return cs;
   if (nb < 1) return TD_EUNSUPPORTED;
   if (dry) return TD_OK;
-  nb = std::min(nb, 512 / Fused4Shape<LOG2M>::TMEM_COLS);  // co-resident CTAs share the SM's 512 tensor-memory columns
+  nb = std::min(nb, 512 / Fused4Shape<LOG2M>::tmem_cols(NGRP));  // co-resident CTAs share the SM's 512 tensor-memory columns
   const long long maxg = (long long)nb * h->num_sms;
-  const int grid = (int)std::max<long long>(1, std::min<long long>(MODE == MODE_STOREZ ? 1 : P.B, maxg));
+  const long long want = MODE == MODE_STOREZ ? 1 : (P.B + NGRP - 1) / NGRP;   // CTAs: one per NGRP items
+  const int grid = (int)std::max<long long>(1, std::min<long long>(want, maxg));
   Fused4Params P4;
   P4.base = P; P4.Gp = Gp; P4.fs = fs;
 #ifdef TD_DEBUG_KNOBS

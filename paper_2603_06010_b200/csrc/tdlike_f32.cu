@@ -28,15 +28,17 @@ __global__ void cvt_cplx_kernel(const double2* __restrict__ src, float2* __restr
   if (i < n) dst[i] = make_float2((float)(src[i].x * scale), (float)(src[i].y * scale));
 }
 
-// Two item pipelines per CTA (NGRP = 2, td_fused4.cuh): the fp32 working set of a pipeline is 113 KB at M = 4096, a kernel
-// that uses tensor memory gets one CTA per SM, so the second item on the SM lives in the same CTA.
-constexpr int F32_NGRP = 2;
+// Several item pipelines per CTA (NGRP of td_fused4.cuh): a kernel that uses tensor memory gets one CTA per SM, so the other items
+// on the SM live in the same CTA.  M = 4096: two (113 KB each); M = 2048 / 1024, whose pipelines have 128 / 64 threads: four /
+// eight, i.e. sixteen warps of 128 registers in every shape.
+constexpr int f32_ngrp(int log2M) { return log2M == 10 ? 8 : log2M == 11 ? 4 : 2; }
 template <int LOG2M, int MODE, int SYN = 0>
 td_status launch_fused4(const td32api::ClassTables& t, const FusedParams& P, int num_sms, int device, cudaStream_t st, bool dry,
                         double fs = 0.0) {
+  constexpr int F32_NGRP = f32_ngrp(LOG2M);
   auto kern = td_fused4_kernel<LOG2M, MODE, F32_NGRP, SYN>;
   constexpr int NT = Fused4Shape<LOG2M>::NT * F32_NGRP;
-  const size_t smem = Fused4Shape<LOG2M>::group_bytes() * F32_NGRP;
+  const size_t smem = Fused4Shape<LOG2M>::total_bytes(F32_NGRP);
   static int cache[TD_MAX_DEV];
   int nb = 0;
   td_status cs = kernel_config(kern, NT, smem, smem, device, cache, &nb);

@@ -538,7 +538,7 @@ def test_full_size_dense_regime(name):
 @pytest.mark.parametrize("name,path", [("d1", tdb.TD_PATH_AUTO), ("d3", tdb.TD_PATH_AUTO), ("d4", tdb.TD_PATH_AUTO),
                                        ("d5", tdb.TD_PATH_CDO)])
 def test_full_size_cdo_regime(name, path):
-    """AUTO sends the log-likelihood of size classes up to 768 samples through the cached-L^-1 contraction (td_cdo.cuh); the
+    """AUTO sends the log-likelihood of size classes up to 512 samples through the cached-L^-1 contraction (td_cdo.cuh); the
     bilinear identity inside _full_size_check ties it to the Gohberg-Semencul dense kernel (td_inner_batch)."""
     _full_size_check(name, sample=64, path=path)
     w = W.make(name, B=40)
@@ -1035,11 +1035,12 @@ def test_cdo_path_lengths(n):
     assert np.max(np.abs(hh.cpu().numpy() - hh_ref) / np.abs(hh_ref)) <= TOL
 
 
-@pytest.mark.parametrize("lens,paths", [([700], "cdo"), ([768], "cdo"), ([769], "fft"), ([700, 900], "fft"),
-                                        ([40, 600, 3000], "cdo+fft"), ([600], "inner")])
-def test_auto_chooser_up_to_768(lens, paths):
-    """AUTO, log-likelihood: a size class whose segments are all at most 768 samples long takes the CDO kernel (measured
-    crossover with the FFT kernels, profiles/r02_cdo.md); the cross terms keep the Gohberg-Semencul limit of 512."""
+@pytest.mark.parametrize("lens,paths", [([500], "cdo"), ([512], "cdo"), ([513], "fft"), ([700], "fft"), ([1024], "fft"),
+                                        ([300, 900], "cdo+fft2"), ([40, 500, 3000], "cdo+fft")])
+def test_auto_chooser_crossover_at_512(lens, paths):
+    """AUTO, log-likelihood: a size class whose segments are all at most 512 samples long takes the dense kernels (CDO from 65
+    samples), everything longer the FFT kernels - the M = 1024 kernel with four item pipelines per CTA beats the CDO kernel
+    from 513 samples up (crossover scan in profiles/r02_cdo.md; the limit was 768 while that kernel ran one pipeline)."""
     rng = np.random.default_rng(sum(lens))
     acf = np.concatenate([W.acf_from_psd(4096.0, 2 * max(n, 32), n) * (1.0 + 0.3 * i) for i, n in enumerate(lens)])
     nt, B = sum(lens), 41
@@ -1047,22 +1048,18 @@ def test_auto_chooser_up_to_768(lens, paths):
     H = rng.standard_normal((B, nt)) * 1e-21
     H[5] = d
     with tdb.TDLikelihood(acf, lens) as h:
-        if paths == "inner":
-            dh, hh = h.inner_batch(_dev(d), _dev(H))
-            assert h.info()["last_path"] == tdb.TD_PATH_FFT        # 600 > 512: the FFT kernels (two of them, dh and hh)
-            dh_ref, hh_ref = O.inner_batch(acf, lens, d, H)
-            assert np.max(np.abs(hh.cpu().numpy() - hh_ref) / np.abs(hh_ref)) <= TOL
-            assert np.max(np.abs(dh.cpu().numpy() - dh_ref)) <= TOL * np.max(np.abs(hh_ref))
         out = h.loglike_batch(_dev(d), _dev(H)).cpu().numpy()
         lp, nl = h.info()["last_path"], h.last_launches()
     _assert_close(out, O.loglike_batch(acf, lens, d, H), what=f"auto {lens}")
-    assert out[5] == 0.0 or paths == "cdo+fft" and abs(out[5]) <= 1e-9
-    if paths in ("cdo", "inner"):
+    assert out[5] == 0.0 or "+" in paths and abs(out[5]) <= 1e-9
+    if paths == "cdo":
         assert lp == tdb.TD_PATH_CDO and nl == 1
     elif paths == "fft":
-        assert lp == tdb.TD_PATH_FFT
+        assert lp == tdb.TD_PATH_FFT and nl == 1
+    elif paths == "cdo+fft2":
+        assert nl == 2                                         # CDO (300), fused FFT (900)
     else:
-        assert nl == 3                                         # GS dense (40), CDO (600), fused FFT (3000)
+        assert nl == 3                                         # GS dense (40), CDO (500), fused FFT (3000)
 
 
 def test_cdo_multi_segment_odd_offsets_and_limits():
