@@ -50,13 +50,13 @@ typedef enum {
 /* td_path: evaluation path selector for td_set_path / reported by td_get_info.
  * TD_PATH_AUTO: per size class (power-of-two padded length), the dense kernels for short segments, the FFT kernels
  * otherwise; all accumulate into the same outputs within one call.  Measured crossovers:
- * td_loglike_batch - classes whose segments are all <= 768 samples: CDO contraction (segments under 65 samples: the
+ * td_loglike_batch - classes whose segments are all <= 512 samples: CDO contraction (segments under 65 samples: the
  * Gohberg-Semencul dense kernel); td_inner_batch - classes whose segments are all <= 512 samples: Gohberg-Semencul. */
 enum { TD_PATH_AUTO = 0, TD_PATH_FFT = 1, TD_PATH_DENSE = 2,
        TD_PATH_DOT = 3, /* reported by td_get_info only: <d,h_b> evaluated as u . h_b, u = C^{-1} d */
        TD_PATH_CDO = 4  /* td_loglike_batch as the batched triangular contraction Y = L^{-1} X with the cached whitening
                            operator (the paper's "CDO" route) for EVERY segment (AUTO uses it for
-                           classes up to 768 samples, profiles/r02_cdo.md); segments up to 1024 samples; the first
+                           classes up to 512 samples, profiles/r02_cdo.md, r02_short_segments.md); segments up to 1024 samples; the first
                            td_set_path(TD_PATH_CDO) builds the L^{-1} that td_create has not (8 N^2 bytes per
                            segment); td_inner_batch keeps using the dense path */ };
 
