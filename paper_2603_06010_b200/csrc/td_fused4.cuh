@@ -305,7 +305,8 @@ __global__ void __launch_bounds__(Fused4Shape<LOG2M>::NT * NGRP, 1) td_fused4_ke
   const FusedParams& P = P4.base;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int grp = NGRP == 1 ? 0 : (int)threadIdx.x / NT;              // item pipeline of this thread
-  const int vblock = (int)blockIdx.x * NGRP + grp, vgrid = (int)gridDim.x * NGRP;   // pipelines are what items are dealt to
+  // pipelines are what items are dealt to, pipeline 0 of every CTA first: a small batch spreads over the SMs before it stacks up on them
+  const int vblock = grp * (int)gridDim.x + (int)blockIdx.x, vgrid = (int)gridDim.x * NGRP;
   auto group_sync = [&]() {
     if constexpr (NGRP == 1) __syncthreads();
     else asm volatile("bar.sync %0, %1;" ::"r"(1 + grp), "r"(NT) : "memory");

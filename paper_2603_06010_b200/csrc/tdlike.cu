@@ -240,7 +240,7 @@ td_status launch_fused4(td_handle* h, const FusedParams& P, const cplx* const* G
   if (dry) return TD_OK;
   nb = std::min(nb, 512 / Fused4Shape<LOG2M>::tmem_cols(NGRP));  // co-resident CTAs share the SM's 512 tensor-memory columns
   const long long maxg = (long long)nb * h->num_sms;
-  const long long want = MODE == MODE_STOREZ ? 1 : (P.B + NGRP - 1) / NGRP;   // CTAs: one per NGRP items
+  const long long want = MODE == MODE_STOREZ ? 1 : P.B;   // one CTA per item while SMs are free, then NGRP items per CTA
   const int grid = (int)std::max<long long>(1, std::min<long long>(want, maxg));
   Fused4Params P4;
   P4.base = P; P4.Gp = Gp; P4.fs = fs;

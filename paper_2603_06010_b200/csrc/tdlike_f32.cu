@@ -45,7 +45,7 @@ td_status launch_fused4(const td32api::ClassTables& t, const FusedParams& P, int
   if (cs != TD_OK) return cs;
   if (nb < 1) return TD_EUNSUPPORTED;
   if (dry) return TD_OK;
-  const long long want = MODE == MODE_STOREZ ? 1 : (P.B + F32_NGRP - 1) / F32_NGRP;   // CTAs: one per F32_NGRP items
+  const long long want = MODE == MODE_STOREZ ? 1 : P.B;   // one CTA per item while SMs are free, then F32_NGRP items per CTA
   const int grid = (int)std::max<long long>(1, std::min<long long>(want, num_sms));
   Fused4Params P4;
   P4.base = P; P4.Gp = reinterpret_cast<const cplx* const*>(t.Gp_ptrs); P4.fs = fs;
