@@ -1062,6 +1062,26 @@ def test_auto_chooser_crossover_at_512(lens, paths):
         assert nl == 3                                         # GS dense (40), CDO (500), fused FFT (3000)
 
 
+@pytest.mark.parametrize("n,Bs", [(1000, (1, 3, 149, 300, 593)), (2000, (1, 2, 149, 297))])
+def test_item_pipelines_every_batch_shape(n, Bs):
+    """The one-CTA kernel runs 4 (M = 1024) / 2 (M = 2048) item pipelines per CTA, items dealt pipeline-major over min(B, SMs)
+    CTAs: batches smaller than a pipeline set, one more than the SM count, between one and NGRP items per SM, and one more
+    than a full wave - every row against the oracle, in fp64 and in the fp32 build (8 / 4 pipelines), rows independent of B."""
+    rng = np.random.default_rng(n)
+    rho = W.acf_from_psd(4096.0, 4096, n)
+    d = rng.standard_normal(n) * 1e-21
+    Hall = rng.standard_normal((max(Bs), n)) * 1e-21
+    Hall[0] = d
+    ref = O.loglike_batch(rho, [n], d, Hall)
+    with tdb.TDLikelihood(rho, [n]) as h:
+        for prec, tol in ((tdb.TD_PREC_F64, TOL), (tdb.TD_PREC_F32, TOL32)):
+            h.set_precision(prec)
+            for B in Bs:
+                out = h.loglike_batch(_dev(d), _dev(Hall[:B])).cpu().numpy()
+                assert h.last_launches() == 1 and out[0] == 0.0
+                _assert_close(out, ref[:B], tol=tol, what=f"pipelines n={n} B={B} prec={prec}")
+
+
 def test_cdo_multi_segment_odd_offsets_and_limits():
     rng = np.random.default_rng(77)
     lens = [333, 64, 1000]
