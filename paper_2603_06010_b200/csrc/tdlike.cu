@@ -1176,7 +1176,12 @@ static td_status family_batch_impl(td_handle* h, const double* d, int family, co
   // Small batches (launch-bound): the rows are synthesised inside the first pass of the fused kernel, one launch, no panel.
   // Large batches: the separate synthesis kernel + panel is measured 3 % (fp64) to 25 % (fp32) faster on c2, because the
   // in-kernel synthesis puts its exp / sincos anchors on the pipes that already bound the FFT kernel (profiles/r02_ring_fused.md).
-  if (family == SYN_RINGDOWN && ring_fused_ok(h) && B <= 2ll * h->num_sms) {
+  // Segments of 513..1024 samples (M = 1024: four item pipelines per CTA, eight with fp32): the fused route is the faster one at
+  // every batch size (B = 16384: fp64 0.271 against 0.275 ms, fp32 0.171 against 0.207 ms; at M = 2048 / 4096 the panel wins
+  // by 3-14 %, profiles/r02_ring_fused.md).
+  bool short_only = true;
+  for (const ClassInfo& c : h->classes) short_only = short_only && c.log2M == 10;
+  if (family == SYN_RINGDOWN && ring_fused_ok(h) && (short_only || B <= 2ll * h->num_sms)) {
     h->last_launches = 0;
     return run_ring_fused(h, d, params, B, fs, out, st);
   }
